@@ -1,0 +1,150 @@
+/* libtm - C ABI of the B200-native coupled T-matrix multiple-scattering solver.
+ *
+ * Hot path of arXiv 2107.09879 (Appendix I.3-I.4): solve
+ *        (I - T A) s = T p                                   (Eqs. I22 + I25)
+ * for N scatterers with VSWF truncation lmax, L = 2 lmax (lmax+2) coefficients each, where
+ *        A_ji = xi^T(x_j, x_i)  (j != i, same window),  A_jj = 0   (Eq. I21)
+ * is the outgoing->regular translation (addition-theorem) operator, built on the fly and never stored
+ * (PAPER.md:382-384), T = blockdiag(T_j) are the per-scatterer transition matrices (Eq. I9)
+ * and p = a^(0) are the incident-field coefficients (Eq. I12).
+ *
+ * Conventions (part of the ABI):
+ *   - time convention e^{-i w t}, outgoing waves h_l^(1)
+ *   - mode (l, m, p), l = 1..lmax, m = -l..l, p in {0 (M-type), 1 (N-type)}
+ *     flat index  idx = p*(L/2) + l*(l+1) - 1 + m                                (reading R1)
+ *   - normalised associated Legendre functions WITHOUT Condon-Shortley phase     (reading R2)
+ *   - every complex array in this API is interleaved double precision (tm_c64), row-major [n_scat][L]
+ *   - every data pointer may be a HOST or a DEVICE pointer (resolved with cudaPointerGetAttributes)
+ *     unless stated otherwise; the caller owns every buffer it passes; tm_set_* copy what they need.
+ *   - all device work is enqueued on the stream given to tm_create; calls that return results to the
+ *     caller synchronise that stream before returning.
+ *   - return value: TM_OK (0); > 0 soft status (outputs valid); < 0 hard error (context unchanged,
+ *     message from tm_last_error).  No exceptions cross the boundary.
+ * There is no CPU fallback: every call that computes needs a CUDA device.
+ */
+#ifndef TM_H_
+#define TM_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tm_ctx tm_ctx;
+typedef struct { double re, im; } tm_c64;
+
+enum { TM_FP64 = 0, TM_FP32 = 1 };                       /* internal compute precision of the solver */
+enum { TM_OK = 0, TM_NOT_CONVERGED = 1,
+       TM_E_INVALID = -1, TM_E_OVERLAP = -2, TM_E_STATE = -3, TM_E_CUDA = -4, TM_E_NOMEM = -5 };
+enum { TM_INC_PLANE = 0, TM_INC_GAUSS = 1, TM_INC_COEFFS = 2 };
+enum { TM_FIELD_E_SCA = 0, TM_FIELD_H_SCA = 1 };           /* H is returned as Z_b * H (reading R10) */
+enum { TM_KERNEL_AUTO = 0, TM_KERNEL_GENERAL = 1, TM_KERNEL_COPLANAR = 2 };
+
+/* Plane wave travelling along (beta = polar angle from +z, alpha = azimuth) with amplitude
+ * A = A_beta * beta_hat + A_alpha * alpha_hat  (Eqs. II6-II7).
+ * Normal incidence, x-polarised, unit amplitude: beta = 0, alpha = 0, A_beta = 1, A_alpha = 0. */
+typedef struct { double beta, alpha; tm_c64 A_beta, A_alpha; } tm_plane_desc;
+
+/* Gaussian beam along +z, one focus per window (reading R9 of DESIGN.md: the angular-spectrum machinery of
+ * Eqs. II9-II17, with a Gaussian spectral weight).  Transverse field on the focal plane
+ * (Ax, Ay) exp(-|x_T - focus_T|^2 / w0^2).  focus: HOST pointer [n_win][3].  n_beta: Gauss-Legendre nodes in
+ * the polar angle (0 -> default 400). */
+typedef struct { const double *focus; double w0; tm_c64 Ax, Ay; int n_beta; } tm_gauss_desc;
+
+/* Caller-supplied incident coefficients p[n_scat][L] (host or device). */
+typedef struct { const tm_c64 *p; } tm_coeffs_desc;
+
+/* GMRES options (reading R13): x0 = 0, restarted GMRES(restart) with CGS2 orthogonalisation on
+ * (I - T A) s = T p; stop when ||b - M x|| / ||b|| <= tol per window (true residual, recomputed at every
+ * restart and at exit); at most max_iter Arnoldi steps per window. */
+typedef struct { double tol; int restart; int max_iter; } tm_solve_opts;
+
+/* Per-window report. */
+typedef struct {
+  int    iterations;      /* Arnoldi steps taken by this window's solve                         */
+  int    restarts;        /* restart cycles started                                             */
+  int    converged;       /* 1 if rel_residual <= tol                                           */
+  int    matvecs;         /* all-pairs operator applications (shared by all windows)            */
+  double rel_residual;    /* true ||b - M x||_2 / ||b||_2 at exit                               */
+  double seconds;         /* device time of the whole solve (CUDA events), same for all windows */
+} tm_solve_info;
+
+/* Create a context (scatterers at x_i with non-intersecting enclosing spheres).
+ *   pos_xyz   [n_scat][3] doubles (host or device), units such that k_b * |x| is the phase
+ *   win_ptr   HOST pointer [n_win+1], monotone, win_ptr[0] = 0, win_ptr[n_win] = n_scat; NULL (with
+ *             n_win = 1) => one window.  Scatterers interact only inside their window (reading R16;
+ *             independent Nyquist windows batched on one GPU).
+ *   lmax      1..6 (coplanar fast kernel for lmax <= 3 when all z are equal; general 3-D kernel otherwise)
+ *   k_b       background wavenumber (wavelength 1 => 2 pi)
+ *   precision TM_FP64 or TM_FP32 (API data stays fp64)
+ *   cuda_stream  a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) or NULL for the default stream
+ * Errors: TM_E_INVALID (bad sizes, non-finite or coincident positions), TM_E_CUDA, TM_E_NOMEM. */
+int tm_create(tm_ctx **out, int n_scat, const double *pos_xyz, int n_win, const int *win_ptr,
+              int lmax, double k_b, int precision, void *cuda_stream);
+
+/* Per-scatterer transition matrices s = T a (Eq. I9), given per type.
+ *   diag_only != 0: T [n_types][L] (diagonal, e.g. Mie spheres); else T [n_types][L][L] row-major.
+ *   type_of   [n_scat] ints (host or device), values in [0, n_types)
+ *   r_enclosing  HOST [n_types] radii or NULL; when given, overlapping enclosing spheres inside a window
+ *             => TM_E_OVERLAP (the paper's assumption).  O(N^2) check on the device. */
+int tm_set_tmatrices(tm_ctx *ctx, int n_types, int diag_only, const tm_c64 *T, const int *type_of,
+                     const double *r_enclosing);
+
+/* Incident field -> coefficients p_j = a^(0)_j of every scatterer, computed on the device
+ * (Eq. I12; kind selects tm_plane_desc / tm_gauss_desc / tm_coeffs_desc). */
+int tm_set_incident(tm_ctx *ctx, int kind, const void *desc);
+
+/* Copy the current incident coefficients p [n_scat][L] out (host or device). */
+int tm_get_incident(tm_ctx *ctx, tm_c64 *p_out);
+
+/* Forward solve (I - T A) s = T p by device-resident restarted GMRES.
+ *   s_out [n_scat][L] (host or device); info: HOST [n_win] or NULL.
+ * Returns TM_OK, TM_NOT_CONVERGED (best iterate returned), or an error.  TM_E_STATE before
+ * tm_set_tmatrices / tm_set_incident. */
+int tm_solve(tm_ctx *ctx, const tm_solve_opts *opts, tm_c64 *s_out, tm_solve_info *info);
+
+/* Adjoint (plain transpose, Eq. IV9): (I - T A)^T lambda = w, with the same all-pairs kernel
+ * through the identity A^T = P A P, P = (m -> -m) permutation (structural identity S3). */
+int tm_solve_adjoint(tm_ctx *ctx, const tm_c64 *w, const tm_solve_opts *opts, tm_c64 *lambda_out,
+                     tm_solve_info *info);
+
+/* One operator application: y = (I - T A) x (transpose = 0) or y = (I - T A)^T x (transpose = 1).
+ * transpose = 2: y = A x (bare all-pairs translation matvec, Eq. I21; no T needed).  Parity and throughput. */
+int tm_matvec(tm_ctx *ctx, int transpose, const tm_c64 *x, tm_c64 *y);
+
+/* Scattered fields at detector points (Eqs. I13/I24):
+ *   E_sca(x) = sum_i sum_{lmp} s_{lmp;i} Phi_{lmp}(k_b (x - x_i)),  Z_b H_sca = -i sum s Phi_{l,m,1-p} (reading R10).
+ *   pts [n_pts][3] doubles, s [n_scat][L], out [n_pts][3] Cartesian complex; all windows are summed
+ *   (the paper sums the sub-region fields).  Points must not coincide with a scatterer centre. */
+int tm_fields(tm_ctx *ctx, int n_pts, const double *pts, const tm_c64 *s, int which, tm_c64 *out);
+
+/* Device scratch.  tm_workspace_bytes: bytes tm_solve / tm_solve_adjoint need for these options (Krylov
+ * basis etc.).  tm_set_workspace: hand in caller-allocated DEVICE memory (e.g. a torch tensor), 256-byte
+ * aligned, which must outlive its use; without it the library allocates (and caches) its own. */
+size_t tm_workspace_bytes(const tm_ctx *ctx, const tm_solve_opts *opts);
+int tm_set_workspace(tm_ctx *ctx, void *dev_ptr, size_t bytes);
+
+/* Force the all-pairs kernel variant (TM_KERNEL_*).  COPLANAR is refused (TM_E_INVALID) unless all z are
+ * equal and lmax <= 3.  Default AUTO. */
+int tm_set_kernel(tm_ctx *ctx, int kernel);
+/* Which variant AUTO resolved to (TM_KERNEL_GENERAL or TM_KERNEL_COPLANAR). */
+int tm_get_kernel(const tm_ctx *ctx);
+
+/* Device time (ms, CUDA events on the context's stream) of the all-pairs kernel launches since the last
+ * call with reset != 0, and their count: lets a caller attribute time without a profiler. */
+int tm_kernel_time(tm_ctx *ctx, int reset, double *allpairs_ms, long long *allpairs_launches,
+                   long long *total_launches);
+
+/* Host helper: diagonal of the Lorenz-Mie T-matrix of a homogeneous sphere (reading R11; closed form,
+ * T_{l,p=0} = -b_l, T_{l,p=1} = -a_l), out[L] in flat mode order.  eps_r complex relative permittivity. */
+int tm_mie_tmatrix(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64 *out);
+
+int tm_num_modes(int lmax);                    /* L = 2 lmax (lmax + 2) */
+const char *tm_last_error(const tm_ctx *ctx);  /* ctx may be NULL: last error of tm_create */
+void tm_destroy(tm_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TM_H_ */

@@ -1,0 +1,256 @@
+#!/usr/bin/env python3
+"""Build-time generator for the constant part of the translation (addition-theorem) operator.
+
+Product-side code: shares nothing with oracle/ (own Wigner-3j, own Legendre values).  It restates
+PAPER.md:299-327 (Eqs. I16-I19) with the readings R3-R8 of DESIGN.md:
+
+  [A_ji]_{b,a} = e^{i(m_a-m_b)phi} sum_q c(q;a->b) h_q^(1)(k r) Pbar_q^{|m_a-m_b|}(cos theta),
+  (r, theta, phi) = x_j - x_i,   a = source mode (l,m,p), b = destination mode (l',m',p'),
+  c = a5(l,m|l',m'|q) for p = p', b5(l,m|l',m'|q) for p != p'.
+
+Outputs (written next to this file, under generated/):
+  tm_tables_gen.h        sparse (row, col, q, value, is_imag) term lists for lmax = 1..6
+                         (general 3-D kernel; value already includes nothing angle-dependent)
+  tm_coplanar_gen.cuh    straight-line device code for the coplanar (theta = pi/2) specialisation,
+                         lmax = 1..3, in the "tilde" basis x~ = i^p x where every coefficient is real,
+                         split into the two mirror-parity halves (-1)^{l+m+p} = +-1 that coplanar
+                         translations do not mix (structural identity S2).
+
+Run:  python gen_tables.py            (build.py runs it when generated/ is missing or stale)
+"""
+import os
+import sys
+from fractions import Fraction
+from math import comb, factorial
+
+import mpmath as mp
+
+mp.mp.dps = 40
+HERE = os.path.dirname(os.path.abspath(__file__))
+OUT = os.path.join(HERE, "generated")
+
+
+# ----------------------------------------------------------------------------- mode bookkeeping
+def n_modes(lmax):
+    return 2 * lmax * (lmax + 2)
+
+
+def modes(lmax):
+    """flat order idx = p*(L/2) + l(l+1) - 1 + m  (reading R1, part of the ABI)."""
+    return [(l, m, p) for p in (0, 1) for l in range(1, lmax + 1) for m in range(-l, l + 1)]
+
+
+# ----------------------------------------------------------------------------- Wigner 3j
+_w3j_cache = {}
+
+
+def w3j(j1, j2, j3, m1, m2, m3):
+    """Exact-rational Racah sum in binomial form; returns an mpf.
+    (j1 j2 j3; m1 m2 m3) = (-1)^{j1-j2-m3} sqrt(D) sum_t (-1)^t / (t! (j3-j2+t+m1)! ...)"""
+    key = (j1, j2, j3, m1, m2, m3)
+    if key in _w3j_cache:
+        return _w3j_cache[key]
+    val = mp.mpf(0)
+    if m1 + m2 + m3 == 0 and abs(j1 - j2) <= j3 <= j1 + j2 and abs(m1) <= j1 and abs(m2) <= j2 and abs(m3) <= j3:
+        J = j1 + j2 + j3
+        # squared prefactor as an exact fraction
+        d2 = Fraction(factorial(J - 2 * j1) * factorial(J - 2 * j2) * factorial(J - 2 * j3), factorial(J + 1))
+        d2 *= (factorial(j1 + m1) * factorial(j1 - m1) * factorial(j2 + m2) * factorial(j2 - m2)
+               * factorial(j3 + m3) * factorial(j3 - m3))
+        lo = max(0, j2 - j3 - m1, j1 - j3 + m2)
+        hi = min(j1 + j2 - j3, j1 - m1, j2 + m2)
+        s = Fraction(0)
+        for t in range(lo, hi + 1):
+            s += Fraction((-1) ** t, factorial(t) * factorial(j3 - j2 + t + m1) * factorial(j3 - j1 + t - m2)
+                          * factorial(j1 + j2 - j3 - t) * factorial(j1 - t - m1) * factorial(j2 - t + m2))
+        val = (-1) ** ((j1 - j2 - m3) % 2) * mp.sqrt(mp.mpf(d2.numerator) / mp.mpf(d2.denominator)) \
+            * (mp.mpf(s.numerator) / mp.mpf(s.denominator))
+    _w3j_cache[key] = val
+    return val
+
+
+# ----------------------------------------------------------------------------- Eq. I18 (repairs R5, R6)
+def _iphase(l, m, lp, mp_, q):
+    """(exponent of i) mod 4 of i^{|m-m'|-|m|-|m'|+l'-l+q} (-1)^{m-m'}."""
+    e = abs(m - mp_) - abs(m) - abs(mp_) + lp - l + q + 2 * ((m - mp_) % 2)
+    return e % 4
+
+
+def _nrm(l, lp):
+    return mp.sqrt(mp.mpf((2 * l + 1) * (2 * lp + 1)) / (2 * l * (l + 1) * lp * (lp + 1)))
+
+
+def coupling(l, m, p, lp, mp_, pp, q):
+    """-> (ipow, real magnitude incl. sign) with c = i^ipow * value; value = 0 when the term is absent."""
+    if q < abs(m - mp_) or q > l + lp:
+        return 0, mp.mpf(0)
+    if p == pp:
+        if q < abs(l - lp):
+            return 0, mp.mpf(0)
+        v = ((l * (l + 1) + lp * (lp + 1) - q * (q + 1)) * mp.sqrt(2 * q + 1) * _nrm(l, lp)
+             * w3j(l, lp, q, m, -mp_, mp_ - m) * w3j(l, lp, q, 0, 0, 0))
+    else:
+        if q < abs(l - lp) + 1:
+            return 0, mp.mpf(0)
+        rad = (l + lp + 1 + q) * (l + lp + 1 - q) * (q + l - lp) * (q - l + lp) * (2 * q + 1)
+        if rad <= 0:
+            return 0, mp.mpf(0)
+        v = mp.sqrt(rad) * _nrm(l, lp) * w3j(l, lp, q, m, -mp_, mp_ - m) * w3j(l, lp, q - 1, 0, 0, 0)
+    return _iphase(l, m, lp, mp_, q), v
+
+
+# ----------------------------------------------------------------------------- Pbar_q^mu(0), no Condon-Shortley phase (R2)
+def pbar_at_zero(q, mu):
+    if (q - mu) % 2:
+        return mp.mpf(0)
+    k = (q - mu) // 2
+    # mu-th derivative at 0 of P_q(x) = 2^-q sum_k (-1)^k C(q,k) C(2q-2k,q) x^{q-2k}
+    d = Fraction((-1) ** k * comb(q, k) * comb(2 * q - 2 * k, q) * factorial(mu), 2 ** q)
+    n2 = Fraction((2 * q + 1) * factorial(q - mu), 2 * factorial(q + mu))
+    return mp.mpf(d.numerator) / mp.mpf(d.denominator) * mp.sqrt(mp.mpf(n2.numerator) / mp.mpf(n2.denominator))
+
+
+def lit(v):
+    return repr(float(v))
+
+
+# ----------------------------------------------------------------------------- general 3-D term lists
+def general_terms(lmax):
+    """[(b, a, q, ipow, value)] sorted by destination row b, then source column a, then q."""
+    md = modes(lmax)
+    out = []
+    for b, (lp, mp_, pp) in enumerate(md):
+        for a, (l, m, p) in enumerate(md):
+            for q in range(0, 2 * lmax + 1):
+                ip, v = coupling(l, m, p, lp, mp_, pp, q)
+                if v != 0:
+                    out.append((b, a, q, ip, v))
+    return out
+
+
+def emit_tables(lmaxes, path):
+    with open(path, "w") as f:
+        f.write("// GENERATED by gen_tables.py - do not edit.  Sparse constant part of Eqs. I16-I18 (PAPER.md:299-323).\n")
+        f.write("// term t of row b (row_ptr[b] <= t < row_ptr[b+1]): A[b][col[t]] += i^ipow[t] * val[t] * h_q[t] * Pbar_q[t]^{|m_col - m_b|}\n")
+        f.write("#pragma once\n#include <cstdint>\n\n")
+        f.write("struct TmTermTable { int lmax; int n_terms; const int* row_ptr; const uint8_t* col; const uint8_t* q; const uint8_t* ipow; const double* val; };\n\n")
+        for lmax in lmaxes:
+            terms = general_terms(lmax)
+            L = n_modes(lmax)
+            rp = [0] * (L + 1)
+            for t in terms:
+                rp[t[0] + 1] += 1
+            for b in range(L):
+                rp[b + 1] += rp[b]
+            tag = f"L{lmax}"
+            f.write(f"static const int tm_rowptr_{tag}[{L + 1}] = {{{', '.join(map(str, rp))}}};\n")
+            f.write(f"static const uint8_t tm_col_{tag}[{len(terms)}] = {{{', '.join(str(t[1]) for t in terms)}}};\n")
+            f.write(f"static const uint8_t tm_q_{tag}[{len(terms)}] = {{{', '.join(str(t[2]) for t in terms)}}};\n")
+            f.write(f"static const uint8_t tm_ipow_{tag}[{len(terms)}] = {{{', '.join(str(t[3]) for t in terms)}}};\n")
+            f.write(f"static const double tm_val_{tag}[{len(terms)}] = {{\n")
+            for s in range(0, len(terms), 6):
+                f.write("  " + ", ".join(lit(t[4]) for t in terms[s:s + 6]) + ",\n")
+            f.write("};\n\n")
+            print(f"lmax={lmax}: L={L} general terms={len(terms)}", file=sys.stderr)
+        f.write(f"static const int tm_max_table_lmax = {max(lmaxes)};\n")
+        f.write("static const TmTermTable tm_term_tables[] = {\n")
+        for lmax in lmaxes:
+            tag = f"L{lmax}"
+            f.write(f"  {{{lmax}, (int)(sizeof(tm_col_{tag})), tm_rowptr_{tag}, tm_col_{tag}, tm_q_{tag}, tm_ipow_{tag}, tm_val_{tag}}},\n")
+        f.write("};\n")
+
+
+# ----------------------------------------------------------------------------- coplanar specialisation
+def coplanar_rows(lmax):
+    """Real coefficients of the tilde-basis coplanar operator.
+    K[b][q] = [(a, value)] with  u~'_b = sum_q h_q sum_a value * x~'_a,
+    x~'_a = e^{i m_a phi} i^{p_a} x_a,   u_b = (-i)^{p_b} e^{-i m_b phi} u~'_b."""
+    md = modes(lmax)
+    L = len(md)
+    K = [[[] for _ in range(2 * lmax + 1)] for _ in range(L)]
+    for b, (lp, mp_, pp) in enumerate(md):
+        for a, (l, m, p) in enumerate(md):
+            for q in range(0, 2 * lmax + 1):
+                ip, v = coupling(l, m, p, lp, mp_, pp, q)
+                if v == 0:
+                    continue
+                v = v * pbar_at_zero(q, abs(m - mp_))
+                if v == 0:
+                    continue
+                tot = (ip + (pp - p)) % 4              # i^{p_b - p_a} * i^ipow must be real
+                assert tot % 2 == 0, (b, a, q, ip)
+                assert (l + m + p) % 2 == (lp + mp_ + pp) % 2, "mirror parity must be conserved (S2)"
+                K[b][q].append((a, v if tot == 0 else -v))
+    return K
+
+
+def emit_coplanar(lmaxes, path):
+    with open(path, "w") as f:
+        f.write("// GENERATED by gen_tables.py - do not edit.\n")
+        f.write("// Coplanar (theta = pi/2) translation apply, one mirror-parity half per call (DESIGN.md, kernel K2c).\n")
+        f.write("// xs: interleaved (re,im) tilde-basis source coefficients of this half; cm/sm: cos/sin(m phi);\n")
+        f.write("// hr/hi: Re/Im h_q^(1)(kr), q = 0..2 lmax; ar/ai: accumulators of this half.\n#pragma once\n\n")
+        for lmax in lmaxes:
+            md = modes(lmax)
+            K = coplanar_rows(lmax)
+            for h in (0, 1):
+                half = [i for i, (l, m, p) in enumerate(md) if (l + m + p) % 2 == h]
+                pos = {idx: k for k, idx in enumerate(half)}
+                nterm = 0
+                nrowq = 0
+                f.write(f"// lmax={lmax} half={h}: modes (flat idx) {half}\n")
+                f.write("template <typename R>\n__device__ __forceinline__ void "
+                        f"tm_cop_pair_L{lmax}_H{h}(const R* __restrict__ xs, const R* cm, const R* sm, const R* hr, const R* hi, R* ar, R* ai) {{\n")
+                for idx in half:
+                    l, m, p = md[idx]
+                    k = pos[idx]
+                    if m == 0:
+                        f.write(f"  const R xr{k} = xs[{2 * k}], xi{k} = xs[{2 * k + 1}];\n")
+                    else:
+                        sg = "" if m > 0 else "-"
+                        am = abs(m)
+                        f.write(f"  const R xr{k} = xs[{2 * k}] * cm[{am}] - xs[{2 * k + 1}] * ({sg}sm[{am}]), "
+                                f"xi{k} = xs[{2 * k}] * ({sg}sm[{am}]) + xs[{2 * k + 1}] * cm[{am}];\n")
+                for idx in half:
+                    lp, mp_, pp = md[idx]
+                    kb = pos[idx]
+                    f.write("  {\n    R ur = R(0), ui = R(0), yr, yi;\n")
+                    for q in range(2 * lmax + 1):
+                        terms = K[idx][q]
+                        if not terms:
+                            continue
+                        nrowq += 1
+                        for t, (a, v) in enumerate(terms):
+                            ka = pos[a]
+                            nterm += 1
+                            if t == 0:
+                                f.write(f"    yr = R({lit(v)}) * xr{ka}; yi = R({lit(v)}) * xi{ka};\n")
+                            else:
+                                f.write(f"    yr = fma(R({lit(v)}), xr{ka}, yr); yi = fma(R({lit(v)}), xi{ka}, yi);\n")
+                        f.write(f"    ur = fma(hr[{q}], yr, ur); ur = fma(-hi[{q}], yi, ur); ui = fma(hr[{q}], yi, ui); ui = fma(hi[{q}], yr, ui);\n")
+                    if mp_ == 0:
+                        f.write(f"    ar[{kb}] += ur; ai[{kb}] += ui;\n")
+                    else:
+                        am = abs(mp_)
+                        sg = "-" if mp_ > 0 else ""      # e^{-i m_b phi}
+                        f.write(f"    ar[{kb}] = fma(ur, cm[{am}], ar[{kb}]); ar[{kb}] = fma(-ui, {sg}sm[{am}], ar[{kb}]);\n")
+                        f.write(f"    ai[{kb}] = fma(ur, {sg}sm[{am}], ai[{kb}]); ai[{kb}] = fma(ui, cm[{am}], ai[{kb}]);\n")
+                    f.write("  }\n")
+                f.write("}\n")
+                print(f"lmax={lmax} half={h}: n={len(half)} coplanar terms={nterm} (row,q) combos={nrowq} "
+                      f"-> ~{2 * nterm + 4 * nrowq + 8 * len(half)} FP ops/pair/half", file=sys.stderr)
+            # half membership tables for the hand-written kernel
+            for h in (0, 1):
+                half = [i for i, (l, m, p) in enumerate(md) if (l + m + p) % 2 == h]
+                f.write(f"__device__ __constant__ int tm_cop_half_L{lmax}_H{h}[{len(half)}] = {{{', '.join(map(str, half))}}};\n")
+            f.write(f"#define TM_COP_NH_L{lmax} {len(md) // 2}\n\n")
+
+
+def main():
+    os.makedirs(OUT, exist_ok=True)
+    emit_tables([1, 2, 3, 4, 5, 6], os.path.join(OUT, "tm_tables_gen.h"))
+    emit_coplanar([1, 2, 3], os.path.join(OUT, "tm_coplanar_gen.cuh"))
+
+
+if __name__ == "__main__":
+    main()
