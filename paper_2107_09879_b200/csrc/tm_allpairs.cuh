@@ -1,0 +1,261 @@
+// All-pairs translation + block matvec  u_j = sum_{i != j, same window} A_ji x_i
+// (PAPER.md:336 Eq. I21: blocks are built on the fly and never stored).
+//
+// Two variants:
+//   k_allpairs_coplanar  lmax <= 3, all scatterers in one plane z = const (every experiment of the paper):
+//                        straight-line generated code, thread = (target, mirror-parity half), register
+//                        accumulators, FP64/FP32 FMA-pipe bound.
+//   k_allpairs_general   any lmax <= 6, arbitrary 3-D positions: table-driven, warp per target.
+// Both write per-source-chunk partial sums u_part[chunk][n_scat][L]; the finishing kernel (tm_vecops.cuh)
+// adds the chunks in a fixed order (deterministic) and applies T.
+#pragma once
+#include "tm_common.cuh"
+#include "generated/tm_coplanar_gen.cuh"
+
+// ---------------------------------------------------------------------------------------------------
+// h_q^(1)(x), q = 0..NQ-1, by upward recurrence from h_{-1} = e^{ix}/x, h_0 = -i e^{ix}/x  (stable upward for
+// the outgoing function); t = 1/x, (c, s) = (cos x, sin x).  t = 0 (self pair) gives h_q = 0 for all q.
+template <typename R, int NQ>
+__device__ __forceinline__ void hankel_up(R t, R c, R s, R* hr, R* hi) {
+  R pr = c * t, pi = s * t;            // h_{-1}
+  hr[0] = s * t; hi[0] = -c * t;       // h_0
+#pragma unroll
+  for (int q = 0; q + 1 < NQ; ++q) {
+    const R f = R(2 * q + 1) * t;
+    const R nr = fma(f, hr[q], -pr), ni = fma(f, hi[q], -pi);
+    pr = hr[q]; pi = hi[q];
+    hr[q + 1] = nr; hi[q + 1] = ni;
+  }
+}
+
+// cos/sin of k*r with the range reduction done in double (fp32 hazard: k r reaches ~900).
+template <typename R> __device__ __forceinline__ void phase_kr(double k_over_pi, double r, R& c, R& s);
+template <> __device__ __forceinline__ void phase_kr<double>(double k_over_pi, double r, double& c, double& s) {
+  sincospi(k_over_pi * r, &s, &c);
+}
+template <> __device__ __forceinline__ void phase_kr<float>(double k_over_pi, double r, float& c, float& s) {
+  double t = k_over_pi * r;
+  t -= 2.0 * rint(0.5 * t);            // exact: t in [-1, 1]
+  sincospif((float)t, &s, &c);
+}
+
+template <typename R, int LMAX, int H> struct CopPair;
+#define TM_COP_SPEC(LM, HH)                                                                              \
+  template <typename R> struct CopPair<R, LM, HH> {                                                      \
+    static __device__ __forceinline__ void run(const R* xs, const R* cm, const R* sm, const R* hr,       \
+                                               const R* hi, R* ar, R* ai) {                              \
+      tm_cop_pair_L##LM##_H##HH<R>(xs, cm, sm, hr, hi, ar, ai);                                          \
+    }                                                                                                    \
+  };
+TM_COP_SPEC(1, 0) TM_COP_SPEC(1, 1) TM_COP_SPEC(2, 0) TM_COP_SPEC(2, 1) TM_COP_SPEC(3, 0) TM_COP_SPEC(3, 1)
+#undef TM_COP_SPEC
+
+// ---------------------------------------------------------------------------------------------------
+// Coplanar kernel.  grid = (n_tiles, n_chunk); block = 2*TJ threads: thread t handles target
+// tile.tgt_start + (t % TJ) and mirror-parity half t / TJ (warp-uniform, so the generated code's
+// coefficients are immediate / constant-bank operands).  Sources of the tile's window are split into
+// n_chunk contiguous chunks (blockIdx.y) so that small problems still fill 148 SMs; each chunk is streamed
+// through shared memory SS sources at a time (positions + coefficient vectors in the tilde basis
+// x~ = i^p x, permuted so that each half is contiguous).
+template <typename R, int LMAX, int TJ, int SS>
+__global__ void __launch_bounds__(2 * TJ)
+k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
+                    const TmTile* __restrict__ tiles, const TmConst* __restrict__ cst, int n_scat,
+                    double k_over_pi, double inv_k, const int* __restrict__ n_active) {
+  constexpr int L = 2 * LMAX * (LMAX + 2);
+  constexpr int NH = L / 2;
+  constexpr int NQ = 2 * LMAX + 1;
+  if (n_active != nullptr && *n_active == 0) return;
+
+  __shared__ double s_px[SS], s_py[SS];
+  __shared__ __align__(16) R s_x[SS * L * 2];          // [source][half][NH] complex, tilde basis
+  __shared__ int s_slot[L];
+
+  const TmTile tile = tiles[blockIdx.x];
+  const int tid = threadIdx.x;
+  const int half = tid / TJ;
+  const int tj = tid % TJ;
+  const int j = tile.tgt_start + (tj < tile.tgt_count ? tj : tile.tgt_count - 1);
+  const double xj = pos[3 * j], yj = pos[3 * j + 1];
+
+  // this block's chunk of the window's sources
+  const int per = (tile.src_count + gridDim.y - 1) / gridDim.y;
+  const int c0 = tile.src_start + blockIdx.y * per;
+  const int c1 = min(tile.src_start + tile.src_count, c0 + per);
+
+  for (int e = tid; e < L; e += 2 * TJ) s_slot[e] = cst->cop_slot[e];
+
+  R ar[NH], ai[NH];
+#pragma unroll
+  for (int b = 0; b < NH; ++b) { ar[b] = R(0); ai[b] = R(0); }
+
+  for (int s0 = c0; s0 < c1; s0 += SS) {
+    const int ns = min(SS, c1 - s0);
+    __syncthreads();                                   // previous stage fully consumed (also orders s_slot)
+    for (int e = tid; e < ns; e += 2 * TJ) { s_px[e] = pos[3 * (s0 + e)]; s_py[e] = pos[3 * (s0 + e) + 1]; }
+    for (int e = tid; e < ns * L; e += 2 * TJ) {
+      const int src = e / L, idx = e - src * L;
+      Cx<R> v = x[(size_t)(s0 + src) * L + idx];
+      if (idx >= NH) v = cx<R>(-v.im, v.re);           // tilde basis: multiply p = 1 modes by i
+      const int slot = s_slot[idx];
+      s_x[(src * L + slot) * 2] = v.re;
+      s_x[(src * L + slot) * 2 + 1] = v.im;
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int s = 0; s < ns; ++s) {
+      const double dx = xj - s_px[s], dy = yj - s_py[s];        // d = x_dest - x_source (reading R3)
+      const double r2 = dx * dx + dy * dy;
+      const double rinv = r2 > 0.0 ? rsqrt(r2) : 0.0;           // self pair -> h_q = 0 -> contributes nothing
+      const double r = r2 * rinv;
+      R cm[LMAX + 1], sm[LMAX + 1];
+      cm[0] = R(1); sm[0] = R(0);
+      cm[1] = (R)(dx * rinv); sm[1] = (R)(dy * rinv);
+      if (r2 == 0.0) cm[1] = R(1);
+#pragma unroll
+      for (int m = 2; m <= LMAX; ++m) {
+        cm[m] = cm[m - 1] * cm[1] - sm[m - 1] * sm[1];
+        sm[m] = sm[m - 1] * cm[1] + cm[m - 1] * sm[1];
+      }
+      R ck, sk;
+      phase_kr<R>(k_over_pi, r, ck, sk);
+      R hr[NQ], hi[NQ];
+      hankel_up<R, NQ>((R)(rinv * inv_k), ck, sk, hr, hi);
+      const R* xs = &s_x[(s * L + half * NH) * 2];
+      if (half == 0) CopPair<R, LMAX, 0>::run(xs, cm, sm, hr, hi, ar, ai);
+      else           CopPair<R, LMAX, 1>::run(xs, cm, sm, hr, hi, ar, ai);
+    }
+  }
+
+  // write this chunk's partial sums, back in the standard basis: u_b = (-i)^{p_b} u~_b.
+  // Stage through shared memory so the global writes are coalesced rows of L complex numbers.
+  __syncthreads();
+  static_assert(SS >= TJ, "output staging reuses the source buffer");
+#pragma unroll
+  for (int b = 0; b < NH; ++b) {
+    s_x[(tj * L + half * NH + b) * 2] = ar[b];
+    s_x[(tj * L + half * NH + b) * 2 + 1] = ai[b];
+  }
+  __syncthreads();
+  Cx<R>* out = u_part + ((size_t)blockIdx.y * n_scat + tile.tgt_start) * L;
+  for (int e = tid; e < tile.tgt_count * L; e += 2 * TJ) {
+    const int t = e / L, idx = e - t * L;
+    const int slot = s_slot[idx];
+    R vr = s_x[(t * L + slot) * 2], vi = s_x[(t * L + slot) * 2 + 1];
+    out[e] = (idx >= NH) ? cx<R>(vi, -vr) : cx<R>(vr, vi);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// General 3-D kernel (any lmax <= 6).  Term table on the device: for destination row b, terms
+// row_ptr[b] <= t < row_ptr[b+1] with source column col[t], scalar-wave index widx[t] = q^2 + q + mu
+// (mu = m_col - m_b) and coefficient coef[t] (real part if !imag[t], imaginary part otherwise):
+//      A[b][col] += coef * h_q(kr) Pbar_q^{|mu|}(cos theta) e^{i mu phi}                 (Eq. I17)
+struct TmTermsDev { const int* row_ptr; const uint8_t* col; const uint8_t* widx; const uint8_t* imag; const double* coef; };
+
+template <int LMAX> struct GenCfg {
+  static constexpr int L = 2 * LMAX * (LMAX + 2);
+  static constexpr int NQ = 2 * LMAX + 1;
+  static constexpr int NW2 = NQ * NQ;
+  static constexpr int SG = 16;                         // sources per stage
+  static constexpr int WJ = (LMAX <= 3) ? 4 : 2;        // targets (warps) per block
+  static constexpr int RB = (L + 31) / 32;              // rows per lane
+  template <typename R> static constexpr size_t smem() { return sizeof(Cx<R>) * (size_t)(SG * L + WJ * SG * NW2); }
+};
+
+template <typename R, int LMAX>
+__global__ void __launch_bounds__(32 * GenCfg<LMAX>::WJ)
+k_allpairs_general(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
+                   const TmTile* __restrict__ tiles, const TmConst* __restrict__ cst, TmTermsDev tb, int n_scat,
+                   double k_over_pi, double inv_k, const int* __restrict__ n_active) {
+  using G = GenCfg<LMAX>;
+  constexpr int L = G::L, NQ = G::NQ, NW2 = G::NW2, SG = G::SG, WJ = G::WJ, RB = G::RB;
+  if (n_active != nullptr && *n_active == 0) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Cx<R>* s_x = reinterpret_cast<Cx<R>*>(smem_raw);                 // [SG][L]
+  Cx<R>* s_w = s_x + SG * L;                                       // [WJ][SG][NW2]
+
+  const TmTile tile = tiles[blockIdx.x];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const bool live = warp < tile.tgt_count;
+  const int j = tile.tgt_start + (live ? warp : 0);
+  const double xj = pos[3 * j], yj = pos[3 * j + 1], zj = pos[3 * j + 2];
+  const int per = (tile.src_count + gridDim.y - 1) / gridDim.y;
+  const int c0 = tile.src_start + blockIdx.y * per;
+  const int c1 = min(tile.src_start + tile.src_count, c0 + per);
+
+  Cx<R> acc[RB];
+  int m_b[RB];
+#pragma unroll
+  for (int rb = 0; rb < RB; ++rb) { acc[rb] = cx<R>(R(0), R(0)); const int b = lane + 32 * rb; m_b[rb] = b < L ? cst->mode_m[b] : 0; }
+
+  for (int s0 = c0; s0 < c1; s0 += SG) {
+    const int ns = min(SG, c1 - s0);
+    __syncthreads();
+    for (int e = threadIdx.x; e < ns * L; e += 32 * WJ) s_x[e] = x[(size_t)s0 * L + e];
+    // phase 1: lane s builds the (2 lmax + 1)^2 scalar outgoing waves of pair (j, s0 + s)
+    if (lane < ns) {
+      const int i = s0 + lane;
+      const double dx = xj - pos[3 * i], dy = yj - pos[3 * i + 1], dz = zj - pos[3 * i + 2];
+      const double rho2 = dx * dx + dy * dy, r2 = rho2 + dz * dz;
+      const double rinv = r2 > 0.0 ? rsqrt(r2) : 0.0;
+      const double r = r2 * rinv;
+      const double rhoinv = rho2 > 0.0 ? rsqrt(rho2) : 0.0;
+      const R ct = (R)(dz * rinv), st = (R)(rho2 * rhoinv * rinv);
+      const R cph = rho2 > 0.0 ? (R)(dx * rhoinv) : R(1), sph = (R)(dy * rhoinv);
+      R ck, sk;
+      phase_kr<R>(k_over_pi, r, ck, sk);
+      R hr[NQ], hi[NQ];
+      hankel_up<R, NQ>((R)(rinv * inv_k), ck, sk, hr, hi);
+      Cx<R>* w = s_w + (size_t)(warp * SG + lane) * NW2;
+      R pmm = R(0.70710678118654752440);                 // Pbar_0^0
+      R em_r = R(1), em_i = R(0);                        // e^{i mu phi}
+#pragma unroll
+      for (int mu = 0; mu < NQ; ++mu) {
+        if (mu > 0) {
+          pmm *= (R)cst->leg_d[mu] * st;
+          const R t = em_r * cph - em_i * sph; em_i = em_i * cph + em_r * sph; em_r = t;
+        }
+        R p2 = R(0), p1 = pmm;                           // Pbar_{q-2}^mu, Pbar_{q-1}^mu
+#pragma unroll
+        for (int q = mu; q < NQ; ++q) {
+          R pq;
+          if (q == mu) pq = pmm;
+          else { pq = (R)cst->leg_a[q][mu] * (ct * p1 - (R)cst->leg_b[q][mu] * p2); p2 = p1; p1 = pq; }
+          const R gr = hr[q] * pq, gi = hi[q] * pq;      // h_q Pbar_q^mu
+          w[q * q + q + mu] = cx<R>(gr * em_r - gi * em_i, gr * em_i + gi * em_r);
+          if (mu > 0) w[q * q + q - mu] = cx<R>(gr * em_r + gi * em_i, -gr * em_i + gi * em_r);
+        }
+      }
+    }
+    __syncthreads();
+    // phase 2: lane = destination row(s) b; loop terms of the row, then the staged sources
+    if (live) {
+      const Cx<R>* wj = s_w + (size_t)warp * SG * NW2;
+#pragma unroll
+      for (int rb = 0; rb < RB; ++rb) {
+        const int b = lane + 32 * rb;
+        if (b >= L) continue;
+        const int t0 = tb.row_ptr[b], t1 = tb.row_ptr[b + 1];
+        Cx<R> a = acc[rb];
+        for (int t = t0; t < t1; ++t) {
+          const int col = tb.col[t], wi = tb.widx[t];
+          const R cf = (R)tb.coef[t];
+          const bool im = tb.imag[t] != 0;
+          for (int s = 0; s < ns; ++s) {
+            const Cx<R> wv = wj[s * NW2 + wi];
+            const Cx<R> e = im ? cx<R>(-cf * wv.im, cf * wv.re) : cx<R>(cf * wv.re, cf * wv.im);
+            a = cfma(e, s_x[s * L + col], a);
+          }
+        }
+        acc[rb] = a;
+      }
+    }
+  }
+  if (live) {
+    Cx<R>* out = u_part + ((size_t)blockIdx.y * n_scat + j) * L;
+#pragma unroll
+    for (int rb = 0; rb < RB; ++rb) { const int b = lane + 32 * rb; if (b < L) out[b] = acc[rb]; }
+  }
+  (void)m_b;
+}

@@ -1,0 +1,480 @@
+// libtm: C-ABI entry points (include/tm.h) and host orchestration.  sm_100a only, no CPU fallback.
+#include "../../include/tm.h"
+
+#include <algorithm>
+#include <cmath>
+#include <complex>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "tm_allpairs.cuh"
+#include "tm_common.cuh"
+#include "tm_fields.cuh"
+#include "tm_gmres.cuh"
+#include "tm_incident.cuh"
+#include "tm_special.cuh"
+#include "tm_vecops.cuh"
+#include "generated/tm_tables_gen.h"
+
+namespace {
+
+std::string g_create_error;
+
+constexpr int COP_TJ = 64;       // coplanar kernel: targets per block (block = 2*TJ threads)
+constexpr int COP_SS = 64;       // coplanar kernel: sources per shared-memory stage
+constexpr int MAX_RESTART = 300;
+
+struct Gmres {                   // device scalars of the Krylov solver, sized for `restart`
+  int restart = 0;
+  TmGmresDev dev{};
+  double2* part = nullptr;       // [(restart+1)][n_chunks]
+  double* normpart = nullptr;    // [n_chunks]
+  void* blob = nullptr;
+};
+
+}  // namespace
+
+struct tm_ctx {
+  int n_scat = 0, n_win = 0, lmax = 0, L = 0, precision = TM_FP64;
+  double k = 0.0;
+  size_t n = 0;                  // n_scat * L
+  cudaStream_t stream = nullptr;
+  std::vector<int> win_ptr;
+  bool coplanar = false;
+  int kernel_req = TM_KERNEL_AUTO, kernel = TM_KERNEL_GENERAL;
+
+  double* d_pos = nullptr;
+  int* d_win_of = nullptr;
+  int* d_type_of = nullptr;
+  void* d_T = nullptr;           // Cx<R> [n_types][L] or [n_types][L][L]
+  int n_types = 0, diag = 1;
+  bool has_T = false, has_inc = false;
+  double2* d_p = nullptr;        // incident coefficients, fp64 [n]
+  TmConst* d_const = nullptr;
+  TmConst h_const{};
+  int* d_rowptr = nullptr; uint8_t* d_col = nullptr; uint8_t* d_widx = nullptr; uint8_t* d_imag = nullptr; double* d_coef = nullptr;
+
+  TmTile* d_tiles = nullptr; int n_tiles = 0, n_chunk = 1;
+  void* d_upart = nullptr; size_t upart_bytes = 0;
+  TmChunk* d_chunks = nullptr; int n_chunks = 0; int* d_win_chunk_ptr = nullptr;
+
+  void* d_v[3] = {nullptr, nullptr, nullptr};   // Cx<R> work vectors [n]: X, B, Z
+  double2* d_io = nullptr;                      // fp64 staging [n]
+
+  void* ws = nullptr; size_t ws_bytes = 0; bool ws_owned = false;
+  Gmres gm;
+
+  // timing of the all-pairs kernel
+  bool time_kernels = false;
+  std::vector<cudaEvent_t> ev;   // pairs
+  size_t ev_used = 0;
+  long long allpairs_launches = 0, total_launches = 0;
+
+  std::string err;
+};
+
+namespace {
+
+int fail(tm_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg; else g_create_error = msg;
+  return code;
+}
+
+#define TM_CUDA(call)                                                                       \
+  do {                                                                                      \
+    cudaError_t e_ = (call);                                                                \
+    if (e_ != cudaSuccess)                                                                  \
+      return fail(ctx, e_ == cudaErrorMemoryAllocation ? TM_E_NOMEM : TM_E_CUDA,            \
+                  std::string(#call) + ": " + cudaGetErrorString(e_));                      \
+  } while (0)
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+cudaError_t copy_in(void* dst_dev, const void* src, size_t bytes, cudaStream_t s) {
+  return cudaMemcpyAsync(dst_dev, src, bytes, is_device_ptr(src) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s);
+}
+cudaError_t copy_out(void* dst, const void* src_dev, size_t bytes, cudaStream_t s) {
+  return cudaMemcpyAsync(dst, src_dev, bytes, is_device_ptr(dst) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s);
+}
+
+size_t elem_bytes(const tm_ctx* c) { return c->precision == TM_FP64 ? sizeof(Cx<double>) : sizeof(Cx<float>); }
+
+// ---------------------------------------------------------------------------------------- host math
+// Gauss-Legendre nodes/weights on [-1, 1] by Newton iteration on P_n.
+void gauss_legendre(int n, std::vector<double>& x, std::vector<double>& w) {
+  x.resize(n); w.resize(n);
+  for (int i = 0; i < (n + 1) / 2; ++i) {
+    double z = std::cos(M_PI * (i + 0.75) / (n + 0.5)), pp = 0.0;
+    for (int it = 0; it < 100; ++it) {
+      double p1 = 1.0, p2 = 0.0;
+      for (int j = 1; j <= n; ++j) { const double p3 = p2; p2 = p1; p1 = ((2.0 * j - 1.0) * z * p2 - (j - 1.0) * p3) / j; }
+      pp = n * (z * p1 - p2) / (z * z - 1.0);
+      const double dz = p1 / pp;
+      z -= dz;
+      if (std::fabs(dz) < 1e-16) break;
+    }
+    // one more evaluation of P_n' at the converged root for the weight
+    double p1 = 1.0, p2 = 0.0;
+    for (int j = 1; j <= n; ++j) { const double p3 = p2; p2 = p1; p1 = ((2.0 * j - 1.0) * z * p2 - (j - 1.0) * p3) / j; }
+    pp = n * (z * p1 - p2) / (z * z - 1.0);
+    x[i] = -z; x[n - 1 - i] = z;
+    w[i] = w[n - 1 - i] = 2.0 / ((1.0 - z * z) * pp * pp);
+  }
+}
+
+typedef std::complex<double> cd;
+
+// spherical Bessel j_0..j_lmax at complex z (Miller backward recurrence, normalised with j_0 or j_1)
+void sph_jn_complex(int lmax, cd z, std::vector<cd>& j) {
+  j.assign(lmax + 1, cd(0));
+  if (std::abs(z) < 1e-12) { j[0] = 1.0; return; }
+  const int N = lmax + 40 + (int)std::abs(z) * 2;
+  std::vector<cd> f(N + 2, cd(0));
+  f[N + 1] = 0.0; f[N] = 1e-280;
+  for (int n = N; n >= 1; --n) {
+    f[n - 1] = (2.0 * n + 1.0) / z * f[n] - f[n + 1];
+    if (std::abs(f[n - 1]) > 1e200) for (int q = n - 1; q <= N; ++q) f[q] *= 1e-200;
+  }
+  const cd j0 = std::sin(z) / z, j1 = std::sin(z) / (z * z) - std::cos(z) / z;
+  const cd sc = (std::abs(j0) >= std::abs(j1)) ? j0 / f[0] : j1 / f[1];
+  for (int l = 0; l <= lmax; ++l) j[l] = f[l] * sc;
+}
+
+// spherical Neumann y_0..y_lmax at real x > 0 (upward recurrence, stable)
+void sph_yn_real(int lmax, double x, std::vector<double>& y) {
+  y.assign(lmax + 2, 0.0);
+  y[0] = -std::cos(x) / x;
+  y[1] = -std::cos(x) / (x * x) - std::sin(x) / x;
+  for (int l = 1; l < lmax + 1; ++l) y[l + 1] = (2.0 * l + 1.0) / x * y[l] - y[l - 1];
+}
+
+}  // namespace
+
+// ============================================================================================ typed launches
+namespace {
+
+template <typename R> Cx<R>* vec(tm_ctx* c, int i) { return reinterpret_cast<Cx<R>*>(c->d_v[i]); }
+
+int grid_for(size_t n, int block) { return (int)std::min<size_t>((n + block - 1) / block, 148 * 32); }
+
+void tick(tm_ctx* c, bool allpairs_begin) {
+  if (!c->time_kernels) return;
+  if (c->ev_used + 2 > c->ev.size()) return;
+  if (allpairs_begin) cudaEventRecord(c->ev[c->ev_used], c->stream);
+  else { cudaEventRecord(c->ev[c->ev_used + 1], c->stream); c->ev_used += 2; }
+}
+
+// u_part <- A x   (all chunks)
+template <typename R>
+cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
+  const double k_over_pi = c->k / M_PI, inv_k = 1.0 / c->k;
+  Cx<R>* up = reinterpret_cast<Cx<R>*>(c->d_upart);
+  dim3 grid(c->n_tiles, c->n_chunk);
+  tick(c, true);
+  if (c->kernel == TM_KERNEL_COPLANAR) {
+    dim3 block(2 * COP_TJ);
+#define TM_LAUNCH_COP(LM)                                                                                          \
+  k_allpairs_coplanar<R, LM, COP_TJ, COP_SS><<<grid, block, 0, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->d_const, \
+                                                                             c->n_scat, k_over_pi, inv_k, n_active)
+    switch (c->lmax) {
+      case 1: TM_LAUNCH_COP(1); break;
+      case 2: TM_LAUNCH_COP(2); break;
+      default: TM_LAUNCH_COP(3); break;
+    }
+#undef TM_LAUNCH_COP
+  } else {
+    TmTermsDev tb{c->d_rowptr, c->d_col, c->d_widx, c->d_imag, c->d_coef};
+#define TM_LAUNCH_GEN(LM)                                                                                         \
+  {                                                                                                               \
+    const size_t sm = GenCfg<LM>::smem<R>();                                                                      \
+    cudaFuncSetAttribute(k_allpairs_general<R, LM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);        \
+    k_allpairs_general<R, LM><<<grid, 32 * GenCfg<LM>::WJ, sm, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->d_const, \
+                                                                            tb, c->n_scat, k_over_pi, inv_k, n_active); \
+  }
+    switch (c->lmax) {
+      case 1: TM_LAUNCH_GEN(1) break;
+      case 2: TM_LAUNCH_GEN(2) break;
+      case 3: TM_LAUNCH_GEN(3) break;
+      case 4: TM_LAUNCH_GEN(4) break;
+      case 5: TM_LAUNCH_GEN(5) break;
+      default: TM_LAUNCH_GEN(6) break;
+    }
+#undef TM_LAUNCH_GEN
+  }
+  tick(c, false);
+  c->allpairs_launches++; c->total_launches++;
+  return cudaGetLastError();
+}
+
+template <typename R>
+cudaError_t launch_tapply(tm_ctx* c, int mode, const Cx<R>* x, Cx<R>* y, const int* n_active) {
+  constexpr int JB = 8;
+  const int grid = (c->n_scat + JB - 1) / JB;
+  k_tapply<R, JB><<<grid, 256, 0, c->stream>>>(mode, c->L, c->n_scat, c->n_chunk, x, reinterpret_cast<Cx<R>*>(c->d_upart), y,
+                                               reinterpret_cast<Cx<R>*>(c->d_T), c->diag, c->d_type_of, c->d_const, n_active);
+  c->total_launches++;
+  return cudaGetLastError();
+}
+
+// y = op(x): transpose 0: (I - T A) x; 1: (I - T A)^T x; 2: A x.   z = scratch vector for the transposed pre-step.
+template <typename R>
+cudaError_t apply_operator(tm_ctx* c, int transpose, const Cx<R>* x, Cx<R>* y, Cx<R>* z, const int* n_active) {
+  cudaError_t e;
+  if (transpose == 1) {
+    if ((e = launch_tapply<R>(c, 4, x, z, n_active)) != cudaSuccess) return e;       // z = P T^T x
+    if ((e = launch_allpairs<R>(c, z, n_active)) != cudaSuccess) return e;           // u = A z
+    return launch_tapply<R>(c, 1, x, y, n_active);                                    // y = x - P u
+  }
+  if ((e = launch_allpairs<R>(c, x, n_active)) != cudaSuccess) return e;
+  return launch_tapply<R>(c, transpose == 2 ? 2 : 0, x, y, n_active);
+}
+
+template <typename R>
+cudaError_t load_c64(tm_ctx* c, const tm_c64* src, Cx<R>* dst) {     // host/device fp64 -> device Cx<R>
+  cudaError_t e = copy_in(c->d_io, src, c->n * sizeof(double2), c->stream);
+  if (e != cudaSuccess) return e;
+  k_from_c64<R><<<grid_for(c->n, 256), 256, 0, c->stream>>>(reinterpret_cast<const double*>(c->d_io), dst, c->n);
+  c->total_launches++;
+  return cudaGetLastError();
+}
+template <typename R>
+cudaError_t store_c64(tm_ctx* c, const Cx<R>* src, tm_c64* dst) {
+  k_to_c64<R><<<grid_for(c->n, 256), 256, 0, c->stream>>>(src, reinterpret_cast<double*>(c->d_io), c->n);
+  c->total_launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  return copy_out(dst, c->d_io, c->n * sizeof(double2), c->stream);
+}
+
+// ---------------------------------------------------------------------------------------- GMRES driver
+template <typename R>
+int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_info* info) {
+  // on entry: d_v[1] = right-hand side b; on exit d_v[0] = x.
+  Cx<R>* X = vec<R>(ctx, 0); Cx<R>* B = vec<R>(ctx, 1); Cx<R>* Z = vec<R>(ctx, 2);
+  const size_t n = ctx->n;
+  const int m = o.restart, nw = ctx->n_win, nc = ctx->n_chunks;
+  Cx<R>* V = reinterpret_cast<Cx<R>*>(ctx->ws);
+  Cx<R>* W = V + (size_t)(m + 1) * n;
+  TmGmresDev& S = ctx->gm.dev;
+  cudaStream_t st = ctx->stream;
+  const int wb = (nw + 63) / 64;
+  cudaEvent_t e0, e1;
+  TM_CUDA(cudaEventCreate(&e0)); TM_CUDA(cudaEventCreate(&e1));
+  TM_CUDA(cudaEventRecord(e0, st));
+  TM_CUDA(cudaMemsetAsync(X, 0, n * sizeof(Cx<R>), st));
+
+  std::vector<int> h_k(nw), h_done(nw), iters(nw, 0), restarts(nw, 0);
+  std::vector<double> h_res(nw, 0.0);
+  int matvecs = 0, total = 0, cycle = 0;
+  bool all_ok = false;
+  const Cx<R>* resid_vec = B;                         // first cycle: x0 = 0 so r = b
+  while (true) {
+    // beta = ||r|| per window
+    k_norm2<R><<<nc, TM_VT, 0, st>>>(resid_vec, ctx->d_chunks, ctx->gm.normpart);
+    k_reduce_norm<<<nw, 64, 0, st>>>(ctx->gm.normpart, ctx->d_win_chunk_ptr, S.normw);
+    if (cycle > 0) {
+      k_gmres_true_resid<<<wb, 64, 0, st>>>(S, nw);
+      TM_CUDA(cudaMemcpyAsync(h_res.data(), S.resid, nw * sizeof(double), cudaMemcpyDeviceToHost, st));
+      TM_CUDA(cudaMemcpyAsync(h_k.data(), S.kcols, nw * sizeof(int), cudaMemcpyDeviceToHost, st));
+      TM_CUDA(cudaStreamSynchronize(st));
+      int kmax = 0;
+      all_ok = true;
+      for (int w = 0; w < nw; ++w) {
+        iters[w] += h_k[w]; kmax = std::max(kmax, h_k[w]);
+        if (h_k[w] > 0) restarts[w]++;
+        if (!(h_res[w] <= o.tol)) all_ok = false;
+      }
+      total += kmax;
+      if (all_ok || total >= o.max_iter || kmax == 0) break;
+    }
+    TM_CUDA(cudaMemsetAsync(S.n_active, 0, sizeof(int), st));
+    k_gmres_init_cycle<<<wb, 64, 0, st>>>(S, nw, cycle == 0 ? 1 : 0, o.tol);
+    k_scale_or_sub<R><<<nc, TM_VT, 0, st>>>(resid_vec, nullptr, S.inv_norm, V, ctx->d_chunks, nullptr);   // V_0 = r / beta
+    ctx->total_launches += 4;
+    const int mc = std::min(m, o.max_iter - total);
+    for (int j = 0; j < mc; ++j) {
+      Cx<R>* Vj = V + (size_t)j * n;
+      TM_CUDA(apply_operator<R>(ctx, transpose, Vj, W, Z, S.n_active));
+      matvecs++;
+      const size_t sm_d = (size_t)(j + 1) * (TM_VT / 32) * sizeof(double2);
+      const size_t sm_a = (size_t)(j + 1) * sizeof(double2);
+      k_dots<R><<<nc, TM_VT, sm_d, st>>>(V, n, j + 1, W, ctx->d_chunks, nc, ctx->gm.part, S.n_active);
+      k_reduce_h<<<dim3(j + 1, nw), 64, 0, st>>>(ctx->gm.part, nc, ctx->d_win_chunk_ptr, S.h1, S.ldh, 0, S.n_active);
+      k_axpy<R><<<nc, TM_VT, sm_a, st>>>(V, n, j + 1, S.h1, S.ldh, -1.0, W, ctx->d_chunks, nullptr, S.n_active);
+      k_dots<R><<<nc, TM_VT, sm_d, st>>>(V, n, j + 1, W, ctx->d_chunks, nc, ctx->gm.part, S.n_active);
+      k_reduce_h<<<dim3(j + 1, nw), 64, 0, st>>>(ctx->gm.part, nc, ctx->d_win_chunk_ptr, S.h2, S.ldh, 0, S.n_active);
+      k_axpy<R><<<nc, TM_VT, sm_a, st>>>(V, n, j + 1, S.h2, S.ldh, -1.0, W, ctx->d_chunks, ctx->gm.normpart, S.n_active);
+      k_reduce_norm<<<nw, 64, 0, st>>>(ctx->gm.normpart, ctx->d_win_chunk_ptr, S.normw);
+      k_gmres_givens<<<wb, 64, 0, st>>>(S, nw, j, o.tol);
+      k_scale_or_sub<R><<<nc, TM_VT, 0, st>>>(W, nullptr, S.inv_norm, V + (size_t)(j + 1) * n, ctx->d_chunks, S.n_active);
+      ctx->total_launches += 9;
+    }
+    // x += V y ; r = b - M x
+    k_gmres_solve_y<<<wb, 64, 0, st>>>(S, nw);
+    k_axpy<R><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr);
+    TM_CUDA(apply_operator<R>(ctx, transpose, X, W, Z, nullptr));
+    matvecs++;
+    k_scale_or_sub<R><<<nc, TM_VT, 0, st>>>(B, W, nullptr, W, ctx->d_chunks, nullptr);      // W = b - M x
+    ctx->total_launches += 3;
+    TM_CUDA(cudaGetLastError());
+    resid_vec = W;
+    cycle++;
+  }
+  TM_CUDA(cudaEventRecord(e1, st));
+  TM_CUDA(cudaEventSynchronize(e1));
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if (info)
+    for (int w = 0; w < nw; ++w) {
+      info[w].iterations = iters[w]; info[w].restarts = restarts[w]; info[w].converged = h_res[w] <= o.tol ? 1 : 0;
+      info[w].matvecs = matvecs; info[w].rel_residual = h_res[w]; info[w].seconds = ms * 1e-3;
+    }
+  return all_ok ? TM_OK : TM_NOT_CONVERGED;
+}
+
+}  // namespace
+
+// ============================================================================================ setup helpers
+namespace {
+
+// min over same-window pairs of |x_i - x_j| - r_i - r_j  <= 0  -> flag (coincident centres when radii are null)
+__global__ void k_check_overlap(const double* __restrict__ pos, const int* __restrict__ win_of, const int* __restrict__ win_ptr,
+                                const int* __restrict__ type_of, const double* __restrict__ radii, int n_scat, int* flag) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n_scat) return;
+  const int w = win_of[j];
+  const double xj = pos[3 * j], yj = pos[3 * j + 1], zj = pos[3 * j + 2];
+  const double rj = radii ? radii[type_of[j]] : 0.0;
+  bool bad = false;
+  for (int i = win_ptr[w]; i < win_ptr[w + 1]; ++i) {
+    if (i == j) continue;
+    const double dx = xj - pos[3 * i], dy = yj - pos[3 * i + 1], dz = zj - pos[3 * i + 2];
+    const double ri = radii ? radii[type_of[i]] : 0.0;
+    const double lim = ri + rj;
+    const double d2 = dx * dx + dy * dy + dz * dz;
+    if (radii ? (d2 < lim * lim) : (d2 == 0.0)) bad = true;
+  }
+  if (bad) atomicExch(flag, 1);
+}
+
+void fill_const(tm_ctx* c) {
+  TmConst& t = c->h_const;
+  std::memset(&t, 0, sizeof(t));
+  const int lmax = c->lmax, L = c->L, LH = L / 2;
+  int cnt[2] = {0, 0};
+  for (int p = 0; p < 2; ++p)
+    for (int l = 1; l <= lmax; ++l)
+      for (int m = -l; m <= l; ++m) {
+        const int idx = p * LH + l * (l + 1) - 1 + m;
+        t.mode_l[idx] = l; t.mode_m[idx] = m; t.mode_p[idx] = p;
+        t.perm_neg_m[idx] = p * LH + l * (l + 1) - 1 - m;
+      }
+  for (int idx = 0; idx < L; ++idx) {                    // flat order within each mirror-parity half
+    const int h = (t.mode_l[idx] + t.mode_m[idx] + t.mode_p[idx]) & 1;
+    t.cop_slot[idx] = h * LH + cnt[h]++;
+  }
+  for (int q = 0; q <= TM_MAX_NQ; ++q)
+    for (int mu = 0; mu <= q && mu <= TM_MAX_NQ; ++mu) {
+      if (q > mu) {
+        t.leg_a[q][mu] = std::sqrt((4.0 * q * q - 1.0) / ((double)q * q - (double)mu * mu));
+        const double qq = (q - 1.0);
+        t.leg_b[q][mu] = (q - 1 > mu) ? std::sqrt((qq * qq - (double)mu * mu) / (4.0 * qq * qq - 1.0)) : 0.0;
+      }
+    }
+  for (int mu = 1; mu <= TM_MAX_NQ; ++mu) t.leg_d[mu] = std::sqrt((2.0 * mu + 1.0) / (2.0 * mu));
+}
+
+int configure_kernel(tm_ctx* ctx) {
+  int want = ctx->kernel_req;
+  if (want == TM_KERNEL_AUTO) want = (ctx->coplanar && ctx->lmax <= 3) ? TM_KERNEL_COPLANAR : TM_KERNEL_GENERAL;
+  if (want == TM_KERNEL_COPLANAR && !(ctx->coplanar && ctx->lmax <= 3))
+    return fail(ctx, TM_E_INVALID, "coplanar kernel needs all z equal and lmax <= 3");
+  ctx->kernel = want;
+  int tgt_per_tile;
+  switch (want == TM_KERNEL_COPLANAR ? 0 : ctx->lmax) {
+    case 0: tgt_per_tile = COP_TJ; break;
+    case 1: case 2: case 3: tgt_per_tile = 4; break;
+    default: tgt_per_tile = 2; break;
+  }
+  std::vector<TmTile> tiles;
+  int min_win = ctx->n_scat;
+  for (int w = 0; w < ctx->n_win; ++w) {
+    const int lo = ctx->win_ptr[w], hi = ctx->win_ptr[w + 1];
+    if (hi > lo) min_win = std::min(min_win, hi - lo);
+    for (int s = lo; s < hi; s += tgt_per_tile) tiles.push_back(TmTile{s, std::min(tgt_per_tile, hi - s), lo, hi - lo});
+  }
+  ctx->n_tiles = (int)tiles.size();
+  // source chunks: enough blocks for ~16 waves of 148 SMs x 3 resident blocks, at least one stage of sources each
+  const int stage = (want == TM_KERNEL_COPLANAR) ? COP_SS : 16;
+  const long long target_blocks = 148LL * 3 * 16;
+  long long nchunk = (target_blocks + ctx->n_tiles - 1) / std::max(1, ctx->n_tiles);
+  nchunk = std::min<long long>(nchunk, std::max(1, min_win / stage));
+  nchunk = std::min<long long>(nchunk, 64);
+  const size_t vec_bytes = ctx->n * elem_bytes(ctx);
+  while (nchunk > 1 && (size_t)nchunk * vec_bytes > ((size_t)2 << 30)) --nchunk;
+  ctx->n_chunk = (int)std::max<long long>(1, nchunk);
+  if (ctx->d_tiles) cudaFree(ctx->d_tiles);
+  TM_CUDA(cudaMalloc(&ctx->d_tiles, tiles.size() * sizeof(TmTile)));
+  TM_CUDA(cudaMemcpy(ctx->d_tiles, tiles.data(), tiles.size() * sizeof(TmTile), cudaMemcpyHostToDevice));
+  const size_t need = (size_t)ctx->n_chunk * vec_bytes;
+  if (need > ctx->upart_bytes) {
+    if (ctx->d_upart) cudaFree(ctx->d_upart);
+    ctx->d_upart = nullptr; ctx->upart_bytes = 0;
+    TM_CUDA(cudaMalloc(&ctx->d_upart, need));
+    ctx->upart_bytes = need;
+  }
+  return TM_OK;
+}
+
+int ensure_gmres(tm_ctx* ctx, int restart) {
+  if (ctx->gm.restart >= restart && ctx->gm.blob) { ctx->gm.dev.ldh = restart + 1; ctx->gm.dev.m = restart; return TM_OK; }
+  if (ctx->gm.blob) cudaFree(ctx->gm.blob);
+  ctx->gm = Gmres{};
+  const size_t nw = ctx->n_win, ldh = restart + 1, m = restart, nc = ctx->n_chunks;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) / 256 * 256; return o; };
+  const size_t o_h1 = take(nw * ldh * 16), o_h2 = take(nw * ldh * 16), o_R = take(nw * m * ldh * 16), o_cs = take(nw * m * 8),
+               o_sn = take(nw * m * 16), o_g = take(nw * ldh * 16), o_y = take(nw * ldh * 16), o_nw = take(nw * 8),
+               o_bn = take(nw * 8), o_in = take(nw * 8), o_rs = take(nw * 8), o_k = take(nw * 4), o_d = take(nw * 4),
+               o_na = take(4), o_part = take(ldh * nc * 16), o_np = take(nc * 8);
+  TM_CUDA(cudaMalloc(&ctx->gm.blob, off));
+  TM_CUDA(cudaMemset(ctx->gm.blob, 0, off));
+  char* b = reinterpret_cast<char*>(ctx->gm.blob);
+  TmGmresDev& S = ctx->gm.dev;
+  S.h1 = (double2*)(b + o_h1); S.h2 = (double2*)(b + o_h2); S.Rm = (double2*)(b + o_R); S.cs = (double*)(b + o_cs);
+  S.sn = (double2*)(b + o_sn); S.g = (double2*)(b + o_g); S.y = (double2*)(b + o_y); S.normw = (double*)(b + o_nw);
+  S.bnorm = (double*)(b + o_bn); S.inv_norm = (double*)(b + o_in); S.resid = (double*)(b + o_rs); S.kcols = (int*)(b + o_k);
+  S.done = (int*)(b + o_d); S.n_active = (int*)(b + o_na);
+  S.ldh = (int)ldh; S.m = (int)m;
+  ctx->gm.part = (double2*)(b + o_part); ctx->gm.normpart = (double*)(b + o_np);
+  ctx->gm.restart = restart;
+  return TM_OK;
+}
+
+size_t ws_bytes_for(const tm_ctx* c, int restart) { return (size_t)(restart + 2) * c->n * elem_bytes(c) + 256; }
+
+int ensure_workspace(tm_ctx* ctx, int restart) {
+  const size_t need = ws_bytes_for(ctx, restart);
+  if (ctx->ws && ctx->ws_bytes >= need) return TM_OK;
+  if (ctx->ws && !ctx->ws_owned) return fail(ctx, TM_E_NOMEM, "caller workspace too small: see tm_workspace_bytes");
+  if (ctx->ws) cudaFree(ctx->ws);
+  ctx->ws = nullptr; ctx->ws_bytes = 0;
+  TM_CUDA(cudaMalloc(&ctx->ws, need));
+  ctx->ws_bytes = need; ctx->ws_owned = true;
+  return TM_OK;
+}
+
+int check_opts(tm_ctx* ctx, const tm_solve_opts* o) {
+  if (!o) return fail(ctx, TM_E_INVALID, "opts is NULL");
+  if (!(o->tol > 0.0) || o->restart < 1 || o->restart > MAX_RESTART || o->max_iter < 1)
+    return fail(ctx, TM_E_INVALID, "need tol > 0, 1 <= restart <= 300, max_iter >= 1");
+  return TM_OK;
+}
+
+}  // namespace

@@ -1,0 +1,119 @@
+// Per-window scalar part of the device-resident restarted GMRES ("operations in GMRES other
+// than the matrix-vector product"; reading R13): Givens-rotated Hessenberg, residual estimate, convergence
+// mask, back-substitution.  All in double precision regardless of the vector precision.  One thread per
+// window: these are O(m) / O(m^2) scalar recurrences, their cost is the launch.
+#pragma once
+#include "tm_common.cuh"
+
+struct TmGmresDev {
+  double2* h1;        // [n_win][ldh]   first CGS pass  V^H w
+  double2* h2;        // [n_win][ldh]   second CGS pass
+  double2* Rm;        // [n_win][m][ldh] rotated Hessenberg columns (upper triangular after rotation)
+  double*  cs;        // [n_win][m]
+  double2* sn;        // [n_win][m]
+  double2* g;         // [n_win][ldh]
+  double2* y;         // [n_win][ldh]   solution of the small least-squares problem (zero-padded)
+  double*  normw;     // [n_win]        sqrt(sum |w|^2) of the current vector
+  double*  bnorm;     // [n_win]
+  double*  inv_norm;  // [n_win]
+  double*  resid;     // [n_win]        current estimate / true relative residual
+  int*     kcols;     // [n_win]        Krylov columns accepted in this cycle
+  int*     done;      // [n_win]
+  int*     n_active;  // [1]            windows still iterating in this cycle
+  int ldh;            // restart + 1
+  int m;              // restart
+};
+
+__device__ __forceinline__ double2 d2mul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ double2 d2conj(double2 a) { return make_double2(a.x, -a.y); }
+
+// Start of a restart cycle: beta = ||r||; first cycle also fixes ||b||.
+__global__ void k_gmres_init_cycle(TmGmresDev S, int n_win, int first, double tol) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= n_win) return;
+  const double beta = S.normw[w];
+  if (first) S.bnorm[w] = beta;
+  const double bn = S.bnorm[w];
+  S.kcols[w] = 0;
+  for (int i = 0; i < S.ldh; ++i) { S.g[(size_t)w * S.ldh + i] = make_double2(0.0, 0.0); S.y[(size_t)w * S.ldh + i] = make_double2(0.0, 0.0); }
+  S.g[(size_t)w * S.ldh] = make_double2(beta, 0.0);
+  const bool fin = !(beta > tol * bn) || beta == 0.0;       // also catches NaN-free zero RHS
+  S.done[w] = fin ? 1 : 0;
+  S.inv_norm[w] = fin ? 0.0 : 1.0 / beta;
+  S.resid[w] = bn > 0.0 ? beta / bn : 0.0;
+  if (!fin) atomicAdd(S.n_active, 1);
+}
+
+// After Arnoldi step j (0-based): column j of the Hessenberg is h1 + h2 (rows 0..j) and normw (row j+1).
+__global__ void k_gmres_givens(TmGmresDev S, int n_win, int j, double tol) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= n_win) return;
+  if (*S.n_active == 0 || S.done[w]) return;
+  const int ldh = S.ldh;
+  double2* col = S.Rm + ((size_t)w * S.m + j) * ldh;
+  const double2* a1 = S.h1 + (size_t)w * ldh;
+  const double2* a2 = S.h2 + (size_t)w * ldh;
+  double* cs = S.cs + (size_t)w * S.m;
+  double2* sn = S.sn + (size_t)w * S.m;
+  double2* g = S.g + (size_t)w * ldh;
+  for (int i = 0; i <= j; ++i) col[i] = make_double2(a1[i].x + a2[i].x, a1[i].y + a2[i].y);
+  const double hn = S.normw[w];
+  for (int i = 0; i < j; ++i) {            // previous rotations
+    const double2 a = col[i], b = col[i + 1];
+    const double2 sb = d2mul(sn[i], b);
+    const double2 sa = d2mul(d2conj(sn[i]), a);
+    col[i] = make_double2(cs[i] * a.x + sb.x, cs[i] * a.y + sb.y);
+    col[i + 1] = make_double2(cs[i] * b.x - sa.x, cs[i] * b.y - sa.y);
+  }
+  const double2 a = col[j];
+  const double aa = sqrt(a.x * a.x + a.y * a.y);
+  const double den = sqrt(aa * aa + hn * hn);
+  double c; double2 s, r;
+  if (den == 0.0) { c = 1.0; s = make_double2(0.0, 0.0); r = make_double2(0.0, 0.0); }
+  else if (aa == 0.0) { c = 0.0; s = make_double2(1.0, 0.0); r = make_double2(hn, 0.0); }
+  else {
+    c = aa / den;
+    const double f = hn / (aa * den);                        // s = (a/|a|) * conj(b)/den, b = hn real
+    s = make_double2(a.x * f, a.y * f);
+    r = make_double2(a.x / aa * den, a.y / aa * den);
+  }
+  cs[j] = c; sn[j] = s; col[j] = r;
+  const double2 gj = g[j];
+  const double2 gn = d2mul(d2conj(s), gj);
+  g[j + 1] = make_double2(-gn.x, -gn.y);
+  g[j] = make_double2(c * gj.x, c * gj.y);
+  const double est = sqrt(gn.x * gn.x + gn.y * gn.y);
+  S.kcols[w] = j + 1;
+  const double bn = S.bnorm[w];
+  S.resid[w] = est / bn;
+  const bool fin = !(est > tol * bn) || !(hn > 0.0);
+  if (fin) { S.done[w] = 1; S.inv_norm[w] = 0.0; atomicSub(S.n_active, 1); }
+  else S.inv_norm[w] = 1.0 / hn;
+}
+
+// y = R^{-1} g over the accepted columns.
+__global__ void k_gmres_solve_y(TmGmresDev S, int n_win) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= n_win) return;
+  const int ldh = S.ldh, k = S.kcols[w];
+  double2* y = S.y + (size_t)w * ldh;
+  const double2* g = S.g + (size_t)w * ldh;
+  for (int i = 0; i < ldh; ++i) y[i] = make_double2(0.0, 0.0);
+  for (int i = k - 1; i >= 0; --i) {
+    double2 acc = g[i];
+    for (int c = i + 1; c < k; ++c) {
+      const double2 t = d2mul(S.Rm[((size_t)w * S.m + c) * ldh + i], y[c]);
+      acc.x -= t.x; acc.y -= t.y;
+    }
+    const double2 d = S.Rm[((size_t)w * S.m + i) * ldh + i];
+    const double dd = d.x * d.x + d.y * d.y;
+    if (dd > 0.0) y[i] = make_double2((acc.x * d.x + acc.y * d.y) / dd, (acc.y * d.x - acc.x * d.y) / dd);
+  }
+}
+
+// resid[w] = normw[w] / bnorm[w]  (true residual after the cycle's update)
+__global__ void k_gmres_true_resid(TmGmresDev S, int n_win) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= n_win) return;
+  S.resid[w] = S.bnorm[w] > 0.0 ? S.normw[w] / S.bnorm[w] : 0.0;
+}

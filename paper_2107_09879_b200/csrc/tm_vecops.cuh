@@ -1,0 +1,245 @@
+// Vector-phase kernels: conversions, per-scatterer T application (Eq. I25), and the
+// device-resident GMRES building blocks (reading R13).  All are HBM/L2-streaming kernels.
+// Windows (independent problems batched on one GPU) are handled through a chunk table: every
+// chunk of <= TM_CHUNK consecutive vector elements lies inside exactly one window.
+#pragma once
+#include "tm_common.cuh"
+
+#define TM_CHUNK 1024            // complex elements per chunk (one block of 256 threads, 4 per thread)
+#define TM_VT 256
+
+struct TmChunk { int win; int start; int count; };   // element range [start, start+count) of window win
+
+// ------------------------------------------------------------------------------------------------ conversions
+template <typename R>
+__global__ void k_from_c64(const double* __restrict__ in, Cx<R>* __restrict__ out, size_t n) {
+  for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x)
+    out[e] = cx<R>((R)in[2 * e], (R)in[2 * e + 1]);
+}
+template <typename R>
+__global__ void k_to_c64(const Cx<R>* __restrict__ in, double* __restrict__ out, size_t n) {
+  for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+    out[2 * e] = (double)in[e].re; out[2 * e + 1] = (double)in[e].im;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ T application
+// One block per JB scatterers.  mode:
+//   0  y = x - T (sum_c u_c)          forward operator  (I - T A) x
+//   1  y = x - P (sum_c u_c)          transposed operator, u = A (P T^T x)   (identity S3: A^T = P A P)
+//   2  y = sum_c u_c                  bare A x
+//   3  y = T x                        right-hand side b = T p  (u unused)
+//   4  y = P T^T x                    pre-step of the transposed operator (u unused)
+template <typename R, int JB>
+__global__ void __launch_bounds__(256)
+k_tapply(int mode, int L, int n_scat, int n_chunk, const Cx<R>* __restrict__ x, const Cx<R>* __restrict__ u_part,
+         Cx<R>* __restrict__ y, const Cx<R>* __restrict__ T, int diag, const int* __restrict__ type_of,
+         const TmConst* __restrict__ cst, const int* __restrict__ n_active) {
+  if (n_active != nullptr && *n_active == 0) return;
+  __shared__ Cx<R> s_v[JB * 96];
+  const int j0 = blockIdx.x * JB;
+  const int nj = min(JB, n_scat - j0);
+  const int ne = nj * L;
+  // stage the vector T (or P) acts on
+  for (int e = threadIdx.x; e < ne; e += blockDim.x) {
+    const size_t g = (size_t)j0 * L + e;
+    Cx<R> v;
+    if (mode <= 2) {
+      v = u_part[g];
+      for (int c = 1; c < n_chunk; ++c) v = cadd(v, u_part[(size_t)c * n_scat * L + g]);   // fixed order
+    } else {
+      v = x[g];
+    }
+    s_v[e] = v;
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e < ne; e += blockDim.x) {
+    const int jj = e / L, a = e - jj * L;
+    const size_t g = (size_t)j0 * L + e;
+    const Cx<R>* v = s_v + jj * L;
+    Cx<R> out;
+    if (mode == 2) out = v[a];
+    else if (mode == 1) out = csub(x[g], v[cst->perm_neg_m[a]]);
+    else {
+      const int ty = type_of[j0 + jj];
+      Cx<R> tv;
+      if (mode == 4) {                      // (P T^T x)[a] = (T^T x)[perm a] = sum_b T[b][perm a] x[b]
+        const int ap = cst->perm_neg_m[a];
+        if (diag) tv = cmul(T[(size_t)ty * L + ap], v[ap]);
+        else {
+          tv = cx<R>(R(0), R(0));
+          const Cx<R>* Tt = T + (size_t)ty * L * L;
+          for (int b = 0; b < L; ++b) tv = cfma(Tt[(size_t)b * L + ap], v[b], tv);
+        }
+        out = tv;
+      } else {
+        if (diag) tv = cmul(T[(size_t)ty * L + a], v[a]);
+        else {
+          tv = cx<R>(R(0), R(0));
+          const Cx<R>* Tr = T + ((size_t)ty * L + a) * L;
+          for (int b = 0; b < L; ++b) tv = cfma(Tr[b], v[b], tv);
+        }
+        out = (mode == 0) ? csub(x[g], tv) : tv;
+      }
+    }
+    y[g] = out;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ GMRES pieces
+// part[i * n_chunks + c] = sum_{e in chunk c} conj(V_i[e]) w[e],  i < nvec  (double accumulation)
+template <typename R>
+__global__ void __launch_bounds__(TM_VT)
+k_dots(const Cx<R>* __restrict__ V, size_t stride, int nvec, const Cx<R>* __restrict__ w,
+       const TmChunk* __restrict__ chunks, int n_chunks, double2* __restrict__ part, const int* __restrict__ n_active) {
+  if (n_active != nullptr && *n_active == 0) return;
+  extern __shared__ double2 s_red[];                 // [nvec][TM_VT/32]
+  const TmChunk ch = chunks[blockIdx.x];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  Cx<R> wv[TM_CHUNK / TM_VT];
+#pragma unroll
+  for (int k = 0; k < TM_CHUNK / TM_VT; ++k) {
+    const int e = threadIdx.x + k * TM_VT;
+    wv[k] = e < ch.count ? w[(size_t)ch.start + e] : cx<R>(R(0), R(0));
+  }
+  for (int i = 0; i < nvec; ++i) {
+    const Cx<R>* v = V + (size_t)i * stride + ch.start;
+    double sr = 0.0, si = 0.0;
+#pragma unroll
+    for (int k = 0; k < TM_CHUNK / TM_VT; ++k) {
+      const int e = threadIdx.x + k * TM_VT;
+      if (e < ch.count) {
+        const Cx<R> a = v[e];
+        sr += (double)a.re * (double)wv[k].re + (double)a.im * (double)wv[k].im;
+        si += (double)a.re * (double)wv[k].im - (double)a.im * (double)wv[k].re;
+      }
+    }
+    sr = warp_sum(sr); si = warp_sum(si);
+    if (lane == 0) s_red[i * (TM_VT / 32) + warp] = make_double2(sr, si);
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < nvec; i += TM_VT) {
+    double sr = 0.0, si = 0.0;
+#pragma unroll
+    for (int k = 0; k < TM_VT / 32; ++k) { sr += s_red[i * (TM_VT / 32) + k].x; si += s_red[i * (TM_VT / 32) + k].y; }
+    part[(size_t)i * n_chunks + blockIdx.x] = make_double2(sr, si);
+  }
+}
+
+// h[win * ldh + i] (+)= sum over the window's chunks of part[i][c].  grid = (nvec, n_win), block = 64.
+__global__ void k_reduce_h(const double2* __restrict__ part, int n_chunks, const int* __restrict__ win_chunk_ptr,
+                           double2* __restrict__ h, int ldh, int accumulate, const int* __restrict__ n_active) {
+  if (n_active != nullptr && *n_active == 0) return;
+  const int i = blockIdx.x, w = blockIdx.y;
+  double sr = 0.0, si = 0.0;
+  for (int c = win_chunk_ptr[w] + threadIdx.x; c < win_chunk_ptr[w + 1]; c += blockDim.x) {
+    const double2 p = part[(size_t)i * n_chunks + c];
+    sr += p.x; si += p.y;
+  }
+  __shared__ double2 s[2];
+  sr = warp_sum(sr); si = warp_sum(si);
+  if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = make_double2(sr, si);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double2 r = make_double2(s[0].x + s[1].x, s[0].y + s[1].y);
+    if (accumulate) { r.x += h[(size_t)w * ldh + i].x; r.y += h[(size_t)w * ldh + i].y; }
+    h[(size_t)w * ldh + i] = r;
+  }
+}
+
+// w += sign * sum_i coef[win][i] V_i ;  optionally normpart[c] = sum |w|^2 over the chunk (after the update).
+// `coef_off`: coefficient i of window win is coef[win * ldc + coef_off + i].
+template <typename R>
+__global__ void __launch_bounds__(TM_VT)
+k_axpy(const Cx<R>* __restrict__ V, size_t stride, int nvec, const double2* __restrict__ coef, int ldc, double sign,
+       Cx<R>* __restrict__ w, const TmChunk* __restrict__ chunks, double* __restrict__ normpart,
+       const int* __restrict__ n_active) {
+  if (n_active != nullptr && *n_active == 0) return;
+  extern __shared__ double2 s_c[];                   // [nvec] then reduction scratch
+  const TmChunk ch = chunks[blockIdx.x];
+  for (int i = threadIdx.x; i < nvec; i += TM_VT) {
+    const double2 c = coef[(size_t)ch.win * ldc + i];
+    s_c[i] = make_double2(sign * c.x, sign * c.y);
+  }
+  __syncthreads();
+  double nrm = 0.0;
+#pragma unroll
+  for (int k = 0; k < TM_CHUNK / TM_VT; ++k) {
+    const int e = threadIdx.x + k * TM_VT;
+    if (e < ch.count) {
+      const size_t g = (size_t)ch.start + e;
+      double ar = (double)w[g].re, ai = (double)w[g].im;
+      for (int i = 0; i < nvec; ++i) {
+        const double2 c = s_c[i];
+        if (c.x == 0.0 && c.y == 0.0) continue;      // block-uniform; also keeps never-written basis vectors out
+        const Cx<R> v = V[(size_t)i * stride + g];
+        ar += c.x * (double)v.re - c.y * (double)v.im;
+        ai += c.x * (double)v.im + c.y * (double)v.re;
+      }
+      w[g] = cx<R>((R)ar, (R)ai);
+      nrm += ar * ar + ai * ai;
+    }
+  }
+  if (normpart != nullptr) {
+    __shared__ double s_n[TM_VT / 32];
+    nrm = warp_sum(nrm);
+    if ((threadIdx.x & 31) == 0) s_n[threadIdx.x >> 5] = nrm;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      double t = 0.0;
+#pragma unroll
+      for (int k = 0; k < TM_VT / 32; ++k) t += s_n[k];
+      normpart[blockIdx.x] = t;
+    }
+  }
+}
+
+// normpart[c] = sum |v|^2 over chunk c
+template <typename R>
+__global__ void __launch_bounds__(TM_VT)
+k_norm2(const Cx<R>* __restrict__ v, const TmChunk* __restrict__ chunks, double* __restrict__ normpart) {
+  const TmChunk ch = chunks[blockIdx.x];
+  double nrm = 0.0;
+  for (int e = threadIdx.x; e < ch.count; e += TM_VT) {
+    const Cx<R> a = v[(size_t)ch.start + e];
+    nrm += (double)a.re * (double)a.re + (double)a.im * (double)a.im;
+  }
+  __shared__ double s_n[TM_VT / 32];
+  nrm = warp_sum(nrm);
+  if ((threadIdx.x & 31) == 0) s_n[threadIdx.x >> 5] = nrm;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+#pragma unroll
+    for (int k = 0; k < TM_VT / 32; ++k) t += s_n[k];
+    normpart[blockIdx.x] = t;
+  }
+}
+
+// out[win] = sqrt(sum of the window's normpart).  One block (64 threads) per window.
+__global__ void k_reduce_norm(const double* __restrict__ normpart, const int* __restrict__ win_chunk_ptr,
+                              double* __restrict__ out) {
+  const int w = blockIdx.x;
+  double s = 0.0;
+  for (int c = win_chunk_ptr[w] + threadIdx.x; c < win_chunk_ptr[w + 1]; c += blockDim.x) s += normpart[c];
+  __shared__ double sh[2];
+  s = warp_sum(s);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) out[w] = sqrt(sh[0] + sh[1]);
+}
+
+// dst = a * scale[win]  (V_{j+1} = w / h_{j+1,j});  dst = a - b when b != nullptr (scale ignored)
+template <typename R>
+__global__ void __launch_bounds__(TM_VT)
+k_scale_or_sub(const Cx<R>* __restrict__ a, const Cx<R>* __restrict__ b, const double* __restrict__ scale,
+               Cx<R>* __restrict__ dst, const TmChunk* __restrict__ chunks, const int* __restrict__ n_active) {
+  if (n_active != nullptr && *n_active == 0) return;
+  const TmChunk ch = chunks[blockIdx.x];
+  const double sc = (b == nullptr) ? scale[ch.win] : 1.0;
+  for (int e = threadIdx.x; e < ch.count; e += TM_VT) {
+    const size_t g = (size_t)ch.start + e;
+    if (b == nullptr) dst[g] = cx<R>((R)(sc * (double)a[g].re), (R)(sc * (double)a[g].im));
+    else dst[g] = csub(a[g], b[g]);
+  }
+}
