@@ -1,0 +1,50 @@
+"""Builds paper_2107_09879_b200/libtm.so (the C-ABI CUDA library, include/tm.h) in-tree (lib/libtm.so) with nvcc for sm_100a.
+
+    python -m paper_2107_09879_b200.build [--force]
+
+nvcc cross-compiles without a GPU.  The generated headers under csrc/generated/ are (re)written by
+csrc/gen_tables.py when missing or older than the generator.
+"""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+GEN = os.path.join(CSRC, "generated")
+SO = os.path.join(HERE, "lib", "libtm.so")
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+         "-shared", "-Xcompiler", "-fPIC", "-cudart", "static"]
+
+
+def _mtime(p):
+    return os.path.getmtime(p) if os.path.exists(p) else 0.0
+
+
+def generate(force=False):
+    gen_py = os.path.join(CSRC, "gen_tables.py")
+    outs = [os.path.join(GEN, "tm_tables_gen.h"), os.path.join(GEN, "tm_coplanar_gen.cuh")]
+    if force or any(_mtime(o) < _mtime(gen_py) for o in outs):
+        subprocess.check_call([sys.executable, gen_py])
+
+
+def sources():
+    out = [os.path.join(HERE, "..", "include", "tm.h")]
+    for root, _, files in os.walk(CSRC):
+        out += [os.path.join(root, f) for f in files if f.endswith((".cu", ".cuh", ".h"))]
+    return out
+
+
+def build(force=False, verbose=False):
+    generate()
+    if not force and _mtime(SO) >= max(_mtime(s) for s in sources()):
+        return SO
+    os.makedirs(os.path.dirname(SO), exist_ok=True)
+    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", SO, os.path.join(CSRC, "tm_api.cu")]
+    subprocess.check_call(cmd, cwd=CSRC)
+    return SO
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -478,3 +478,482 @@ int check_opts(tm_ctx* ctx, const tm_solve_opts* o) {
 }
 
 }  // namespace
+
+// ============================================================================================ C ABI
+extern "C" {
+
+int tm_num_modes(int lmax) { return 2 * lmax * (lmax + 2); }
+
+const char* tm_last_error(const tm_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+void tm_destroy(tm_ctx* c) {
+  if (!c) return;
+  cudaStreamSynchronize(c->stream);
+  cudaFree(c->d_pos); cudaFree(c->d_win_of); cudaFree(c->d_type_of); cudaFree(c->d_T); cudaFree(c->d_p);
+  cudaFree(c->d_const); cudaFree(c->d_rowptr); cudaFree(c->d_col); cudaFree(c->d_widx); cudaFree(c->d_imag);
+  cudaFree(c->d_coef); cudaFree(c->d_tiles); cudaFree(c->d_upart); cudaFree(c->d_chunks); cudaFree(c->d_win_chunk_ptr);
+  for (int i = 0; i < 3; ++i) cudaFree(c->d_v[i]);
+  cudaFree(c->d_io);
+  if (c->ws_owned) cudaFree(c->ws);
+  cudaFree(c->gm.blob);
+  for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  delete c;
+}
+
+int tm_create(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const int* win_ptr, int lmax, double k_b,
+              int precision, void* cuda_stream) {
+  tm_ctx* ctx = nullptr;                                  // errors before allocation go to g_create_error
+  if (!out) return fail(ctx, TM_E_INVALID, "out is NULL");
+  *out = nullptr;
+  if (n_scat < 1 || !pos_xyz) return fail(ctx, TM_E_INVALID, "need n_scat >= 1 and positions");
+  if (lmax < 1 || lmax > tm_max_table_lmax) return fail(ctx, TM_E_INVALID, "lmax must be in 1..6");
+  if (!(k_b > 0.0) || !std::isfinite(k_b)) return fail(ctx, TM_E_INVALID, "k_b must be positive and finite");
+  if (precision != TM_FP64 && precision != TM_FP32) return fail(ctx, TM_E_INVALID, "precision must be TM_FP64 or TM_FP32");
+  if (n_win < 1) return fail(ctx, TM_E_INVALID, "n_win must be >= 1");
+  std::vector<int> wp;
+  if (win_ptr) {
+    wp.assign(win_ptr, win_ptr + n_win + 1);
+    if (wp[0] != 0 || wp[n_win] != n_scat) return fail(ctx, TM_E_INVALID, "win_ptr must start at 0 and end at n_scat");
+    for (int w = 0; w < n_win; ++w)
+      if (wp[w + 1] < wp[w]) return fail(ctx, TM_E_INVALID, "win_ptr must be monotone");
+  } else {
+    if (n_win != 1) return fail(ctx, TM_E_INVALID, "win_ptr is NULL but n_win != 1");
+    wp = {0, n_scat};
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return fail(ctx, TM_E_CUDA, "no CUDA device: libtm has no CPU fallback");
+  }
+  std::vector<double> hpos((size_t)n_scat * 3);
+  {
+    cudaError_t e = cudaMemcpy(hpos.data(), pos_xyz, hpos.size() * sizeof(double),
+                               is_device_ptr(pos_xyz) ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost);
+    if (e != cudaSuccess) return fail(ctx, TM_E_CUDA, std::string("copy positions: ") + cudaGetErrorString(e));
+  }
+  bool coplanar = true;
+  for (size_t i = 0; i < hpos.size(); ++i)
+    if (!std::isfinite(hpos[i])) return fail(ctx, TM_E_INVALID, "non-finite position");
+  for (int i = 1; i < n_scat; ++i)
+    if (hpos[3 * (size_t)i + 2] != hpos[2]) { coplanar = false; break; }
+
+  tm_ctx* c = new tm_ctx();
+  c->n_scat = n_scat; c->n_win = n_win; c->lmax = lmax; c->L = tm_num_modes(lmax); c->precision = precision;
+  c->k = k_b; c->n = (size_t)n_scat * c->L; c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+  c->win_ptr = wp; c->coplanar = coplanar;
+  ctx = c;
+#define TM_CREATE_CUDA(call)                                                                  \
+  do {                                                                                        \
+    cudaError_t e_ = (call);                                                                  \
+    if (e_ != cudaSuccess) {                                                                  \
+      g_create_error = std::string(#call) + ": " + cudaGetErrorString(e_);                    \
+      const int code_ = e_ == cudaErrorMemoryAllocation ? TM_E_NOMEM : TM_E_CUDA;             \
+      tm_destroy(c);                                                                          \
+      return code_;                                                                           \
+    }                                                                                         \
+  } while (0)
+  TM_CREATE_CUDA(cudaMalloc(&c->d_pos, hpos.size() * sizeof(double)));
+  TM_CREATE_CUDA(cudaMemcpy(c->d_pos, hpos.data(), hpos.size() * sizeof(double), cudaMemcpyHostToDevice));
+  std::vector<int> win_of(n_scat);
+  for (int w = 0; w < n_win; ++w) for (int i = wp[w]; i < wp[w + 1]; ++i) win_of[i] = w;
+  TM_CREATE_CUDA(cudaMalloc(&c->d_win_of, n_scat * sizeof(int)));
+  TM_CREATE_CUDA(cudaMemcpy(c->d_win_of, win_of.data(), n_scat * sizeof(int), cudaMemcpyHostToDevice));
+  TM_CREATE_CUDA(cudaMalloc(&c->d_type_of, n_scat * sizeof(int)));
+  fill_const(c);
+  TM_CREATE_CUDA(cudaMalloc(&c->d_const, sizeof(TmConst)));
+  TM_CREATE_CUDA(cudaMemcpy(c->d_const, &c->h_const, sizeof(TmConst), cudaMemcpyHostToDevice));
+  {   // general-kernel term table of this lmax
+    const TmTermTable& t = tm_term_tables[lmax - 1];
+    const int nt = t.n_terms, L = c->L;
+    std::vector<uint8_t> widx(nt), imag(nt);
+    std::vector<double> coef(nt);
+    for (int b = 0; b < L; ++b)
+      for (int q = t.row_ptr[b]; q < t.row_ptr[b + 1]; ++q) {
+        const int mu = c->h_const.mode_m[t.col[q]] - c->h_const.mode_m[b];
+        const int qq = t.q[q];
+        widx[q] = (uint8_t)(qq * qq + qq + mu);
+        imag[q] = t.ipow[q] & 1;
+        coef[q] = (t.ipow[q] & 2) ? -t.val[q] : t.val[q];
+      }
+    TM_CREATE_CUDA(cudaMalloc(&c->d_rowptr, (L + 1) * sizeof(int)));
+    TM_CREATE_CUDA(cudaMemcpy(c->d_rowptr, t.row_ptr, (L + 1) * sizeof(int), cudaMemcpyHostToDevice));
+    TM_CREATE_CUDA(cudaMalloc(&c->d_col, nt)); TM_CREATE_CUDA(cudaMemcpy(c->d_col, t.col, nt, cudaMemcpyHostToDevice));
+    TM_CREATE_CUDA(cudaMalloc(&c->d_widx, nt)); TM_CREATE_CUDA(cudaMemcpy(c->d_widx, widx.data(), nt, cudaMemcpyHostToDevice));
+    TM_CREATE_CUDA(cudaMalloc(&c->d_imag, nt)); TM_CREATE_CUDA(cudaMemcpy(c->d_imag, imag.data(), nt, cudaMemcpyHostToDevice));
+    TM_CREATE_CUDA(cudaMalloc(&c->d_coef, nt * sizeof(double)));
+    TM_CREATE_CUDA(cudaMemcpy(c->d_coef, coef.data(), nt * sizeof(double), cudaMemcpyHostToDevice));
+  }
+  {   // vector chunks: every chunk inside one window
+    std::vector<TmChunk> ch;
+    std::vector<int> wcp(n_win + 1, 0);
+    for (int w = 0; w < n_win; ++w) {
+      const long long e0 = (long long)wp[w] * c->L, e1 = (long long)wp[w + 1] * c->L;
+      for (long long s = e0; s < e1; s += TM_CHUNK) ch.push_back(TmChunk{w, (int)s, (int)std::min<long long>(TM_CHUNK, e1 - s)});
+      wcp[w + 1] = (int)ch.size();
+    }
+    if (c->n > (size_t)0x7fffffff) { g_create_error = "problem too large (n_scat * L must fit in int32)"; tm_destroy(c); return TM_E_INVALID; }
+    c->n_chunks = (int)ch.size();
+    TM_CREATE_CUDA(cudaMalloc(&c->d_chunks, ch.size() * sizeof(TmChunk)));
+    TM_CREATE_CUDA(cudaMemcpy(c->d_chunks, ch.data(), ch.size() * sizeof(TmChunk), cudaMemcpyHostToDevice));
+    TM_CREATE_CUDA(cudaMalloc(&c->d_win_chunk_ptr, (n_win + 1) * sizeof(int)));
+    TM_CREATE_CUDA(cudaMemcpy(c->d_win_chunk_ptr, wcp.data(), (n_win + 1) * sizeof(int), cudaMemcpyHostToDevice));
+  }
+  for (int i = 0; i < 3; ++i) TM_CREATE_CUDA(cudaMalloc(&c->d_v[i], c->n * elem_bytes(c)));
+  TM_CREATE_CUDA(cudaMalloc(&c->d_io, c->n * sizeof(double2)));
+  TM_CREATE_CUDA(cudaMalloc(&c->d_p, c->n * sizeof(double2)));
+  {   // coincident centres are always an error (h_q diverges)
+    int* d_flag = nullptr; int* d_wp = nullptr; int h_flag = 0;
+    TM_CREATE_CUDA(cudaMalloc(&d_flag, sizeof(int)));
+    TM_CREATE_CUDA(cudaMemset(d_flag, 0, sizeof(int)));
+    TM_CREATE_CUDA(cudaMalloc(&d_wp, (n_win + 1) * sizeof(int)));
+    TM_CREATE_CUDA(cudaMemcpy(d_wp, wp.data(), (n_win + 1) * sizeof(int), cudaMemcpyHostToDevice));
+    k_check_overlap<<<(n_scat + 127) / 128, 128>>>(c->d_pos, c->d_win_of, d_wp, nullptr, nullptr, n_scat, d_flag);
+    cudaError_t e = cudaMemcpy(&h_flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost);
+    cudaFree(d_flag); cudaFree(d_wp);
+    TM_CREATE_CUDA(e);
+    if (h_flag) { g_create_error = "two scatterers of one window share a centre"; tm_destroy(c); return TM_E_INVALID; }
+  }
+  {
+    const int rc = configure_kernel(c);
+    if (rc != TM_OK) { g_create_error = c->err; tm_destroy(c); return rc; }
+  }
+#undef TM_CREATE_CUDA
+  *out = c;
+  return TM_OK;
+}
+
+int tm_set_kernel(tm_ctx* ctx, int kernel) {
+  if (!ctx) return TM_E_INVALID;
+  if (kernel < TM_KERNEL_AUTO || kernel > TM_KERNEL_COPLANAR) return fail(ctx, TM_E_INVALID, "unknown kernel id");
+  const int old = ctx->kernel_req;
+  ctx->kernel_req = kernel;
+  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  const int rc = configure_kernel(ctx);
+  if (rc != TM_OK) { ctx->kernel_req = old; configure_kernel(ctx); }
+  return rc;
+}
+
+int tm_get_kernel(const tm_ctx* ctx) { return ctx ? ctx->kernel : TM_E_INVALID; }
+
+size_t tm_workspace_bytes(const tm_ctx* ctx, const tm_solve_opts* opts) {
+  if (!ctx || !opts || opts->restart < 1) return 0;
+  return ws_bytes_for(ctx, opts->restart);
+}
+
+int tm_set_workspace(tm_ctx* ctx, void* dev_ptr, size_t bytes) {
+  if (!ctx) return TM_E_INVALID;
+  if (dev_ptr && (!is_device_ptr(dev_ptr) || (reinterpret_cast<uintptr_t>(dev_ptr) & 255)))
+    return fail(ctx, TM_E_INVALID, "workspace must be 256-byte aligned device memory");
+  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  if (ctx->ws && ctx->ws_owned) cudaFree(ctx->ws);
+  ctx->ws = dev_ptr; ctx->ws_bytes = dev_ptr ? bytes : 0; ctx->ws_owned = false;
+  return TM_OK;
+}
+
+int tm_kernel_time(tm_ctx* ctx, int reset, double* allpairs_ms, long long* allpairs_launches, long long* total_launches) {
+  if (!ctx) return TM_E_INVALID;
+  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  double ms = 0.0;
+  for (size_t i = 0; i + 1 < ctx->ev_used; i += 2) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, ctx->ev[i], ctx->ev[i + 1]) == cudaSuccess) ms += t;
+  }
+  // scale to all launches if the event pool ran out (stated in DESIGN.md: average over the recorded ones)
+  const long long recorded = (long long)(ctx->ev_used / 2);
+  if (recorded > 0 && ctx->allpairs_launches > recorded) ms *= (double)ctx->allpairs_launches / (double)recorded;
+  if (allpairs_ms) *allpairs_ms = ms;
+  if (allpairs_launches) *allpairs_launches = ctx->allpairs_launches;
+  if (total_launches) *total_launches = ctx->total_launches;
+  if (reset) {
+    if (ctx->ev.empty()) {
+      ctx->ev.resize(2 * 4096);
+      for (cudaEvent_t& e : ctx->ev) TM_CUDA(cudaEventCreate(&e));
+    }
+    ctx->ev_used = 0; ctx->allpairs_launches = 0; ctx->total_launches = 0; ctx->time_kernels = true;
+  }
+  return TM_OK;
+}
+
+}  // extern "C"
+
+// ============================================================================================ C ABI, part 2
+namespace {
+
+template <typename R>
+int set_T_typed(tm_ctx* ctx, size_t count, const tm_c64* T) {
+  // stage fp64 -> Cx<R>
+  double2* tmp = nullptr;
+  TM_CUDA(cudaMalloc(&tmp, count * sizeof(double2)));
+  cudaError_t e = copy_in(tmp, T, count * sizeof(double2), ctx->stream);
+  if (e == cudaSuccess) {
+    k_from_c64<R><<<grid_for(count, 256), 256, 0, ctx->stream>>>(reinterpret_cast<const double*>(tmp),
+                                                                 reinterpret_cast<Cx<R>*>(ctx->d_T), count);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  cudaFree(tmp);
+  TM_CUDA(e);
+  return TM_OK;
+}
+
+template <typename R>
+int matvec_typed(tm_ctx* ctx, int transpose, const tm_c64* x, tm_c64* y) {
+  TM_CUDA(load_c64<R>(ctx, x, vec<R>(ctx, 0)));
+  TM_CUDA(apply_operator<R>(ctx, transpose, vec<R>(ctx, 0), vec<R>(ctx, 1), vec<R>(ctx, 2), nullptr));
+  TM_CUDA(store_c64<R>(ctx, vec<R>(ctx, 1), y));
+  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  return TM_OK;
+}
+
+template <typename R>
+int solve_typed(tm_ctx* ctx, int adjoint, const tm_c64* w, const tm_solve_opts& o, tm_c64* out, tm_solve_info* info) {
+  if (adjoint) {
+    TM_CUDA(load_c64<R>(ctx, w, vec<R>(ctx, 1)));                           // b = w
+  } else {
+    k_from_c64<R><<<grid_for(ctx->n, 256), 256, 0, ctx->stream>>>(reinterpret_cast<const double*>(ctx->d_p), vec<R>(ctx, 2), ctx->n);
+    TM_CUDA(cudaGetLastError());
+    TM_CUDA(launch_tapply<R>(ctx, 3, vec<R>(ctx, 2), vec<R>(ctx, 1), nullptr));   // b = T p   (Eq. I25)
+    ctx->total_launches++;
+  }
+  const int rc = gmres_solve<R>(ctx, adjoint ? 1 : 0, o, info);
+  if (rc < 0) return rc;
+  TM_CUDA(store_c64<R>(ctx, vec<R>(ctx, 0), out));
+  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tm_set_tmatrices(tm_ctx* ctx, int n_types, int diag_only, const tm_c64* T, const int* type_of, const double* r_enclosing) {
+  if (!ctx) return TM_E_INVALID;
+  if (n_types < 1 || !T || !type_of) return fail(ctx, TM_E_INVALID, "need n_types >= 1, T and type_of");
+  std::vector<int> ht(ctx->n_scat);
+  TM_CUDA(cudaMemcpy(ht.data(), type_of, ht.size() * sizeof(int), is_device_ptr(type_of) ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost));
+  for (int v : ht) if (v < 0 || v >= n_types) return fail(ctx, TM_E_INVALID, "type_of out of range");
+  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  if (r_enclosing) {
+    for (int t = 0; t < n_types; ++t)
+      if (!(r_enclosing[t] >= 0.0)) return fail(ctx, TM_E_INVALID, "negative enclosing radius");
+    int *d_flag = nullptr, *d_wp = nullptr, *d_ty = nullptr; double* d_r = nullptr; int h_flag = 0;
+    cudaError_t e = cudaMalloc(&d_flag, sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(d_flag, 0, sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&d_wp, (ctx->n_win + 1) * sizeof(int));
+    if (e == cudaSuccess) e = cudaMemcpy(d_wp, ctx->win_ptr.data(), (ctx->n_win + 1) * sizeof(int), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&d_ty, ht.size() * sizeof(int));
+    if (e == cudaSuccess) e = cudaMemcpy(d_ty, ht.data(), ht.size() * sizeof(int), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&d_r, n_types * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemcpy(d_r, r_enclosing, n_types * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+      k_check_overlap<<<(ctx->n_scat + 127) / 128, 128>>>(ctx->d_pos, ctx->d_win_of, d_wp, d_ty, d_r, ctx->n_scat, d_flag);
+      e = cudaMemcpy(&h_flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost);
+    }
+    cudaFree(d_flag); cudaFree(d_wp); cudaFree(d_ty); cudaFree(d_r);
+    TM_CUDA(e);
+    if (h_flag) return fail(ctx, TM_E_OVERLAP, "enclosing spheres of two scatterers intersect (PAPER.md:275)");
+  }
+  const size_t count = (size_t)n_types * ctx->L * (diag_only ? 1 : ctx->L);
+  void* newT = nullptr;
+  TM_CUDA(cudaMalloc(&newT, count * elem_bytes(ctx)));
+  void* oldT = ctx->d_T;
+  ctx->d_T = newT;
+  const int rc = ctx->precision == TM_FP64 ? set_T_typed<double>(ctx, count, T) : set_T_typed<float>(ctx, count, T);
+  if (rc != TM_OK) { cudaFree(newT); ctx->d_T = oldT; return rc; }
+  cudaFree(oldT);
+  TM_CUDA(cudaMemcpy(ctx->d_type_of, ht.data(), ht.size() * sizeof(int), cudaMemcpyHostToDevice));
+  ctx->n_types = n_types; ctx->diag = diag_only ? 1 : 0; ctx->has_T = true;
+  return TM_OK;
+}
+
+int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
+  if (!ctx) return TM_E_INVALID;
+  if (!desc) return fail(ctx, TM_E_INVALID, "desc is NULL");
+  const int L = ctx->L, lmax = ctx->lmax, LH = L / 2;
+  if (kind == TM_INC_COEFFS) {
+    const tm_coeffs_desc* d = static_cast<const tm_coeffs_desc*>(desc);
+    if (!d->p) return fail(ctx, TM_E_INVALID, "p is NULL");
+    TM_CUDA(copy_in(ctx->d_p, d->p, ctx->n * sizeof(double2), ctx->stream));
+    TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  } else if (kind == TM_INC_PLANE) {
+    // Eq. II7 (explicit right-hand forms, reading R9b):
+    //   a_{l,m,0} = -4 i^l     e^{-i m alpha} c_l [ i m pibar A_beta + taubar A_alpha ]
+    //   a_{l,m,1} = -4 i^{l+1} e^{-i m alpha} c_l [ taubar A_beta - i m pibar A_alpha ]
+    const tm_plane_desc* d = static_cast<const tm_plane_desc*>(desc);
+    if (!std::isfinite(d->beta) || !std::isfinite(d->alpha)) return fail(ctx, TM_E_INVALID, "non-finite angles");
+    double P[TM_MAX_LMAX + 1][TM_MAX_LMAX + 1], PI[TM_MAX_LMAX + 1][TM_MAX_LMAX + 1], TAU[TM_MAX_LMAX + 1][TM_MAX_LMAX + 1];
+    ang_functions<TM_MAX_LMAX>(std::cos(d->beta), std::fabs(std::sin(d->beta)), P, PI, TAU);
+    // beta in [0, pi] assumed; sin(beta) >= 0
+    const cd Ab(d->A_beta.re, d->A_beta.im), Aa(d->A_alpha.re, d->A_alpha.im), I(0.0, 1.0);
+    std::vector<cd> a(L);
+    for (int l = 1; l <= lmax; ++l) {
+      const double cl = 1.0 / std::sqrt(2.0 * l * (l + 1));
+      const cd il = std::pow(I, l), il1 = std::pow(I, l + 1);
+      for (int m = -l; m <= l; ++m) {
+        const int am = std::abs(m);
+        const cd e = std::exp(-I * (double)m * d->alpha);
+        const double mpi = m * PI[l][am], tau = TAU[l][am];
+        const int a0 = l * (l + 1) - 1 + m;
+        a[a0] = -4.0 * il * e * cl * (I * mpi * Ab + tau * Aa);
+        a[LH + a0] = -4.0 * il1 * e * cl * (tau * Ab - I * mpi * Aa);
+      }
+    }
+    double2* d_a = nullptr;
+    TM_CUDA(cudaMalloc(&d_a, L * sizeof(double2)));
+    cudaError_t e = cudaMemcpyAsync(d_a, a.data(), L * sizeof(double2), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) {
+      const double sb = std::sin(d->beta);
+      const size_t tot = ctx->n;
+      k_incident_plane<<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(ctx->d_pos, ctx->n_scat, L, d_a,
+          ctx->k * sb * std::cos(d->alpha), ctx->k * sb * std::sin(d->alpha), ctx->k * std::cos(d->beta), ctx->d_p);
+      ctx->total_launches++;
+      e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(d_a);
+    TM_CUDA(e);
+  } else if (kind == TM_INC_GAUSS) {
+    const tm_gauss_desc* d = static_cast<const tm_gauss_desc*>(desc);
+    if (!d->focus || !(d->w0 > 0.0)) return fail(ctx, TM_E_INVALID, "need focus[n_win][3] and w0 > 0");
+    if (lmax > 3) return fail(ctx, TM_E_INVALID, "Gaussian-beam expansion is built for lmax <= 3");
+    const int nb = d->n_beta > 0 ? d->n_beta : 400;
+    // beta in [0, beta_max]: G(beta) < 1e-40 beyond (or pi/2: evanescent part dropped, reading R9)
+    const double kw = ctx->k * d->w0;
+    const double smax = std::min(1.0, 2.0 * std::sqrt(40.0 * std::log(10.0)) / kw);
+    const double bmax = std::asin(smax);
+    std::vector<double> xg, wg, beta(nb), wq(nb);
+    gauss_legendre(nb, xg, wg);
+    for (int q = 0; q < nb; ++q) { beta[q] = 0.5 * bmax * (xg[q] + 1.0); wq[q] = 0.5 * bmax * wg[q]; }
+    double *d_beta = nullptr, *d_wq = nullptr, *d_focus = nullptr; void* d_nodes = nullptr;
+    const size_t node_bytes = lmax == 1 ? sizeof(GaussNode<1>) : lmax == 2 ? sizeof(GaussNode<2>) : sizeof(GaussNode<3>);
+    cudaError_t e = cudaMalloc(&d_beta, nb * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&d_wq, nb * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&d_focus, (size_t)ctx->n_win * 3 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&d_nodes, nb * node_bytes);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_beta, beta.data(), nb * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_wq, wq.data(), nb * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_focus, d->focus, (size_t)ctx->n_win * 3 * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) {
+      const double2 Ax = make_double2(d->Ax.re, d->Ax.im), Ay = make_double2(d->Ay.re, d->Ay.im);
+#define TM_GAUSS(LM)                                                                                                   \
+  k_gauss_nodes<LM><<<(nb + 127) / 128, 128, 0, ctx->stream>>>(d_beta, d_wq, nb, kw, static_cast<GaussNode<LM>*>(d_nodes)); \
+  k_incident_gauss<LM><<<ctx->n_scat, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->d_win_of, d_focus,                        \
+                                                            static_cast<GaussNode<LM>*>(d_nodes), nb, ctx->k, Ax, Ay, ctx->d_p)
+      if (lmax == 1) { TM_GAUSS(1); } else if (lmax == 2) { TM_GAUSS(2); } else { TM_GAUSS(3); }
+#undef TM_GAUSS
+      ctx->total_launches += 2;
+      e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(d_beta); cudaFree(d_wq); cudaFree(d_focus); cudaFree(d_nodes);
+    TM_CUDA(e);
+  } else {
+    return fail(ctx, TM_E_INVALID, "unknown incident kind");
+  }
+  ctx->has_inc = true;
+  return TM_OK;
+}
+
+int tm_get_incident(tm_ctx* ctx, tm_c64* p_out) {
+  if (!ctx) return TM_E_INVALID;
+  if (!ctx->has_inc) return fail(ctx, TM_E_STATE, "tm_set_incident has not been called");
+  if (!p_out) return fail(ctx, TM_E_INVALID, "p_out is NULL");
+  TM_CUDA(copy_out(p_out, ctx->d_p, ctx->n * sizeof(double2), ctx->stream));
+  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  return TM_OK;
+}
+
+int tm_matvec(tm_ctx* ctx, int transpose, const tm_c64* x, tm_c64* y) {
+  if (!ctx) return TM_E_INVALID;
+  if (!x || !y || transpose < 0 || transpose > 2) return fail(ctx, TM_E_INVALID, "bad arguments");
+  if (transpose != 2 && !ctx->has_T) return fail(ctx, TM_E_STATE, "tm_set_tmatrices has not been called");
+  return ctx->precision == TM_FP64 ? matvec_typed<double>(ctx, transpose, x, y) : matvec_typed<float>(ctx, transpose, x, y);
+}
+
+int tm_solve(tm_ctx* ctx, const tm_solve_opts* opts, tm_c64* s_out, tm_solve_info* info) {
+  if (!ctx) return TM_E_INVALID;
+  int rc = check_opts(ctx, opts);
+  if (rc != TM_OK) return rc;
+  if (!s_out) return fail(ctx, TM_E_INVALID, "s_out is NULL");
+  if (!ctx->has_T || !ctx->has_inc) return fail(ctx, TM_E_STATE, "tm_set_tmatrices and tm_set_incident must be called first");
+  if ((rc = ensure_workspace(ctx, opts->restart)) != TM_OK) return rc;
+  if ((rc = ensure_gmres(ctx, opts->restart)) != TM_OK) return rc;
+  return ctx->precision == TM_FP64 ? solve_typed<double>(ctx, 0, nullptr, *opts, s_out, info)
+                                   : solve_typed<float>(ctx, 0, nullptr, *opts, s_out, info);
+}
+
+int tm_solve_adjoint(tm_ctx* ctx, const tm_c64* w, const tm_solve_opts* opts, tm_c64* lambda_out, tm_solve_info* info) {
+  if (!ctx) return TM_E_INVALID;
+  int rc = check_opts(ctx, opts);
+  if (rc != TM_OK) return rc;
+  if (!w || !lambda_out) return fail(ctx, TM_E_INVALID, "w or lambda_out is NULL");
+  if (!ctx->has_T) return fail(ctx, TM_E_STATE, "tm_set_tmatrices must be called first");
+  if ((rc = ensure_workspace(ctx, opts->restart)) != TM_OK) return rc;
+  if ((rc = ensure_gmres(ctx, opts->restart)) != TM_OK) return rc;
+  return ctx->precision == TM_FP64 ? solve_typed<double>(ctx, 1, w, *opts, lambda_out, info)
+                                   : solve_typed<float>(ctx, 1, w, *opts, lambda_out, info);
+}
+
+int tm_fields(tm_ctx* ctx, int n_pts, const double* pts, const tm_c64* s, int which, tm_c64* out) {
+  if (!ctx) return TM_E_INVALID;
+  if (n_pts < 1 || !pts || !s || !out) return fail(ctx, TM_E_INVALID, "bad arguments");
+  if (which != TM_FIELD_E_SCA && which != TM_FIELD_H_SCA) return fail(ctx, TM_E_INVALID, "unknown field id");
+  if (ctx->lmax > 3) return fail(ctx, TM_E_INVALID, "field evaluation is built for lmax <= 3");
+  const int nchunk = std::max(1, std::min(64, (int)(148LL * 8 * 128 / std::max(1, n_pts))));
+  const int nch = std::min(nchunk, std::max(1, ctx->n_scat / 32));
+  double* d_pts = nullptr; double2 *d_part = nullptr, *d_out = nullptr;
+  const size_t nout = (size_t)n_pts * 3;
+  cudaError_t e = cudaMalloc(&d_pts, nout * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&d_part, nout * nch * sizeof(double2));
+  if (e == cudaSuccess) e = cudaMalloc(&d_out, nout * sizeof(double2));
+  if (e == cudaSuccess) e = copy_in(d_pts, pts, nout * sizeof(double), ctx->stream);
+  if (e == cudaSuccess) e = copy_in(ctx->d_io, s, ctx->n * sizeof(double2), ctx->stream);
+  if (e == cudaSuccess) {
+    dim3 grid((n_pts + 127) / 128, nch);
+    const int swap = which == TM_FIELD_H_SCA ? 1 : 0;
+    if (ctx->lmax == 1) k_fields<1><<<grid, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->n_scat, ctx->d_io, d_pts, n_pts, ctx->k, swap, d_part);
+    else if (ctx->lmax == 2) k_fields<2><<<grid, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->n_scat, ctx->d_io, d_pts, n_pts, ctx->k, swap, d_part);
+    else k_fields<3><<<grid, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->n_scat, ctx->d_io, d_pts, n_pts, ctx->k, swap, d_part);
+    k_fields_reduce<<<(unsigned)((nout + 255) / 256), 256, 0, ctx->stream>>>(d_part, nch, nout, d_out);
+    ctx->total_launches += 2;
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = copy_out(out, d_out, nout * sizeof(double2), ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  cudaFree(d_pts); cudaFree(d_part); cudaFree(d_out);
+  TM_CUDA(e);
+  return TM_OK;
+}
+
+// Lorenz-Mie coefficients (reading R11), x = k_b R, m_r = sqrt(eps_r), psi_l(z) = z j_l(z), xi_l(z) = z h_l^(1)(z):
+//   a_l = [m psi_l(mx) psi_l'(x) - psi_l(x) psi_l'(mx)] / [m psi_l(mx) xi_l'(x) - xi_l(x) psi_l'(mx)]
+//   b_l = [psi_l(mx) psi_l'(x) - m psi_l(x) psi_l'(mx)] / [psi_l(mx) xi_l'(x) - m xi_l(x) psi_l'(mx)]
+//   psi_l'(z) = z j_{l-1}(z) - l j_l(z)   (same for xi_l with h_l)
+int tm_mie_tmatrix(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64* out) {
+  if (lmax < 1 || lmax > TM_MAX_LMAX || !(k_b > 0.0) || !(radius > 0.0) || !out) return TM_E_INVALID;
+  const double x = k_b * radius;
+  const cd mr = std::sqrt(cd(eps_r.re, eps_r.im));
+  std::vector<cd> jx, jm;
+  std::vector<double> yx;
+  sph_jn_complex(lmax, cd(x, 0.0), jx);
+  sph_jn_complex(lmax, mr * x, jm);
+  sph_yn_real(lmax, x, yx);
+  const int LH = lmax * (lmax + 2);
+  for (int l = 1; l <= lmax; ++l) {
+    const cd z = mr * x;
+    const cd psx = x * jx[l], dpsx = x * jx[l - 1] - (double)l * jx[l];
+    const cd psm = z * jm[l], dpsm = z * jm[l - 1] - (double)l * jm[l];
+    const cd hx = jx[l] + cd(0, 1) * yx[l], hx1 = jx[l - 1] + cd(0, 1) * yx[l - 1];
+    const cd xix = x * hx, dxix = x * hx1 - (double)l * hx;
+    const cd a = (mr * psm * dpsx - psx * dpsm) / (mr * psm * dxix - xix * dpsm);
+    const cd b = (psm * dpsx - mr * psx * dpsm) / (psm * dxix - mr * xix * dpsm);
+    for (int m = -l; m <= l; ++m) {
+      const int a0 = l * (l + 1) - 1 + m;
+      out[a0].re = -b.real(); out[a0].im = -b.imag();              // p = 0 (M-type, magnetic multipoles)
+      out[LH + a0].re = -a.real(); out[LH + a0].im = -a.imag();    // p = 1 (N-type, electric multipoles)
+    }
+  }
+  return TM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,263 @@
+"""Thin ctypes binding over libtm.so (include/tm.h): argument marshalling only.
+
+Every step of the path runs in the CUDA library; this module never computes.  It fails loudly when the
+library is missing (there is no CPU fallback).  PyTorch is used only to allocate device memory / hand over
+the current CUDA stream (``Solver(..., use_torch=True)``); numpy arrays are passed as host pointers.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "lib", "libtm.so")
+
+TM_FP64, TM_FP32 = 0, 1
+TM_OK, TM_NOT_CONVERGED = 0, 1
+TM_E_INVALID, TM_E_OVERLAP, TM_E_STATE, TM_E_CUDA, TM_E_NOMEM = -1, -2, -3, -4, -5
+TM_INC_PLANE, TM_INC_GAUSS, TM_INC_COEFFS = 0, 1, 2
+TM_FIELD_E_SCA, TM_FIELD_H_SCA = 0, 1
+TM_KERNEL_AUTO, TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR = 0, 1, 2
+
+EXPORTS = ["tm_create", "tm_set_tmatrices", "tm_set_incident", "tm_get_incident", "tm_solve", "tm_solve_adjoint",
+           "tm_matvec", "tm_fields", "tm_workspace_bytes", "tm_set_workspace", "tm_set_kernel", "tm_get_kernel",
+           "tm_kernel_time", "tm_mie_tmatrix", "tm_num_modes", "tm_last_error", "tm_destroy"]
+
+
+class c64(ctypes.Structure):
+    _fields_ = [("re", ctypes.c_double), ("im", ctypes.c_double)]
+
+
+class PlaneDesc(ctypes.Structure):
+    _fields_ = [("beta", ctypes.c_double), ("alpha", ctypes.c_double), ("A_beta", c64), ("A_alpha", c64)]
+
+
+class GaussDesc(ctypes.Structure):
+    _fields_ = [("focus", ctypes.c_void_p), ("w0", ctypes.c_double), ("Ax", c64), ("Ay", c64), ("n_beta", ctypes.c_int)]
+
+
+class CoeffsDesc(ctypes.Structure):
+    _fields_ = [("p", ctypes.c_void_p)]
+
+
+class SolveOpts(ctypes.Structure):
+    _fields_ = [("tol", ctypes.c_double), ("restart", ctypes.c_int), ("max_iter", ctypes.c_int)]
+
+
+class SolveInfo(ctypes.Structure):
+    _fields_ = [("iterations", ctypes.c_int), ("restarts", ctypes.c_int), ("converged", ctypes.c_int),
+                ("matvecs", ctypes.c_int), ("rel_residual", ctypes.c_double), ("seconds", ctypes.c_double)]
+
+
+class TmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libtm error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libtm.so (hard error when it has not been built: run __graft_entry__.build())."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise ImportError(f"{_SO} not found: build it with `python -m paper_2107_09879_b200.build` "
+                              "(the CUDA library is required; there is no CPU fallback)")
+        L = ctypes.CDLL(_SO)
+        vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+        L.tm_create.argtypes = [ctypes.POINTER(vp), ci, vp, ci, vp, ci, cd, ci, vp]
+        L.tm_set_tmatrices.argtypes = [vp, ci, ci, vp, vp, vp]
+        L.tm_set_incident.argtypes = [vp, ci, vp]
+        L.tm_get_incident.argtypes = [vp, vp]
+        L.tm_solve.argtypes = [vp, ctypes.POINTER(SolveOpts), vp, vp]
+        L.tm_solve_adjoint.argtypes = [vp, vp, ctypes.POINTER(SolveOpts), vp, vp]
+        L.tm_matvec.argtypes = [vp, ci, vp, vp]
+        L.tm_fields.argtypes = [vp, ci, vp, vp, ci, vp]
+        L.tm_workspace_bytes.argtypes = [vp, ctypes.POINTER(SolveOpts)]
+        L.tm_workspace_bytes.restype = ctypes.c_size_t
+        L.tm_set_workspace.argtypes = [vp, vp, ctypes.c_size_t]
+        L.tm_set_kernel.argtypes = [vp, ci]
+        L.tm_get_kernel.argtypes = [vp]
+        L.tm_kernel_time.argtypes = [vp, ci, ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(ctypes.c_longlong)]
+        L.tm_mie_tmatrix.argtypes = [ci, cd, cd, c64, vp]
+        L.tm_num_modes.argtypes = [ci]
+        L.tm_last_error.argtypes = [vp]
+        L.tm_last_error.restype = ctypes.c_char_p
+        L.tm_destroy.argtypes = [vp]
+        L.tm_destroy.restype = None
+        _lib = L
+    return _lib
+
+
+def _ptr(a):
+    """Host numpy array or torch tensor (host or CUDA) -> raw pointer; None -> NULL."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        assert a.flags["C_CONTIGUOUS"]
+        return a.ctypes.data
+    return a.data_ptr()      # torch tensor
+
+
+def _c64(z):
+    z = complex(z)
+    return c64(z.real, z.imag)
+
+
+def mie_tmatrix(lmax, k_b, radius, eps_r):
+    """Diagonal Mie T-matrix (tm_mie_tmatrix), shape (L,) complex128."""
+    out = np.zeros(lib().tm_num_modes(lmax), dtype=np.complex128)
+    rc = lib().tm_mie_tmatrix(lmax, float(k_b), float(radius), _c64(eps_r), out.ctypes.data)
+    if rc != TM_OK:
+        raise TmError(rc, "tm_mie_tmatrix: invalid arguments")
+    return out
+
+
+class Solver:
+    """One tm_ctx.  Arrays may be numpy (host) or torch CUDA tensors (device); complex data is complex128
+    [n_scat, L] (torch.complex128 on the device)."""
+
+    def __init__(self, pos, lmax, k_b, win_ptr=None, precision=TM_FP64, stream=None):
+        self._h = ctypes.c_void_p()
+        L = lib()
+        self.pos = np.ascontiguousarray(pos, dtype=np.float64) if isinstance(pos, np.ndarray) else pos
+        self.n_scat = int(self.pos.shape[0])
+        self.lmax = int(lmax)
+        self.L = L.tm_num_modes(self.lmax)
+        wp = None
+        self.n_win = 1
+        if win_ptr is not None:
+            wp = np.ascontiguousarray(win_ptr, dtype=np.int32)
+            self.n_win = wp.size - 1
+        rc = L.tm_create(ctypes.byref(self._h), self.n_scat, _ptr(self.pos), self.n_win, _ptr(wp), self.lmax, float(k_b),
+                         int(precision), ctypes.c_void_p(stream) if stream else None)
+        if rc != TM_OK:
+            msg = L.tm_last_error(None).decode()
+            self._h = ctypes.c_void_p()
+            raise TmError(rc, msg)
+        self._keep = []          # buffers the library keeps using (workspace)
+
+    def _check(self, rc):
+        if rc < 0:
+            raise TmError(rc, lib().tm_last_error(self._h).decode())
+        return rc
+
+    def close(self):
+        if self._h:
+            lib().tm_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- setup
+    def set_tmatrices(self, T, type_of, diag_only, r_enclosing=None):
+        T = np.ascontiguousarray(T, dtype=np.complex128) if isinstance(T, np.ndarray) else T
+        ty = np.ascontiguousarray(type_of, dtype=np.int32) if isinstance(type_of, np.ndarray) else type_of
+        re = None if r_enclosing is None else np.ascontiguousarray(r_enclosing, dtype=np.float64)
+        return self._check(lib().tm_set_tmatrices(self._h, int(T.shape[0]), 1 if diag_only else 0, _ptr(T), _ptr(ty), _ptr(re)))
+
+    def set_incident_plane(self, beta, alpha, A_beta, A_alpha):
+        d = PlaneDesc(float(beta), float(alpha), _c64(A_beta), _c64(A_alpha))
+        return self._check(lib().tm_set_incident(self._h, TM_INC_PLANE, ctypes.addressof(d)))
+
+    def set_incident_gauss(self, focus, w0, Ax, Ay, n_beta=0):
+        f = np.ascontiguousarray(focus, dtype=np.float64).reshape(self.n_win, 3)
+        d = GaussDesc(f.ctypes.data, float(w0), _c64(Ax), _c64(Ay), int(n_beta))
+        return self._check(lib().tm_set_incident(self._h, TM_INC_GAUSS, ctypes.addressof(d)))
+
+    def set_incident_coeffs(self, p):
+        p = np.ascontiguousarray(p, dtype=np.complex128) if isinstance(p, np.ndarray) else p
+        d = CoeffsDesc(_ptr(p))
+        return self._check(lib().tm_set_incident(self._h, TM_INC_COEFFS, ctypes.addressof(d)))
+
+    def get_incident(self, out=None):
+        out = np.empty((self.n_scat, self.L), dtype=np.complex128) if out is None else out
+        self._check(lib().tm_get_incident(self._h, _ptr(out)))
+        return out
+
+    def set_kernel(self, kernel):
+        return self._check(lib().tm_set_kernel(self._h, int(kernel)))
+
+    def get_kernel(self):
+        return lib().tm_get_kernel(self._h)
+
+    def workspace_bytes(self, restart):
+        o = SolveOpts(1e-6, int(restart), 1)
+        return int(lib().tm_workspace_bytes(self._h, ctypes.byref(o)))
+
+    def set_workspace(self, tensor):
+        """tensor: torch CUDA uint8 tensor (kept alive by this object) or None."""
+        self._keep = [tensor]
+        if tensor is None:
+            return self._check(lib().tm_set_workspace(self._h, None, 0))
+        return self._check(lib().tm_set_workspace(self._h, tensor.data_ptr(), tensor.numel() * tensor.element_size()))
+
+    # ---- compute
+    def matvec(self, x, transpose=0, out=None):
+        x = np.ascontiguousarray(x, dtype=np.complex128) if isinstance(x, np.ndarray) else x
+        out = self._like(x) if out is None else out
+        self._check(lib().tm_matvec(self._h, int(transpose), _ptr(x), _ptr(out)))
+        return out
+
+    def _like(self, x):
+        if isinstance(x, np.ndarray):
+            return np.empty((self.n_scat, self.L), dtype=np.complex128)
+        import torch
+        return torch.empty((self.n_scat, self.L), dtype=torch.complex128, device=x.device)
+
+    def solve(self, tol, restart, max_iter, out=None):
+        out = np.empty((self.n_scat, self.L), dtype=np.complex128) if out is None else out
+        o = SolveOpts(float(tol), int(restart), int(max_iter))
+        info = (SolveInfo * self.n_win)()
+        rc = self._check(lib().tm_solve(self._h, ctypes.byref(o), _ptr(out), ctypes.addressof(info)))
+        return out, list(info), rc
+
+    def solve_adjoint(self, w, tol, restart, max_iter, out=None):
+        w = np.ascontiguousarray(w, dtype=np.complex128) if isinstance(w, np.ndarray) else w
+        out = self._like(w) if out is None else out
+        o = SolveOpts(float(tol), int(restart), int(max_iter))
+        info = (SolveInfo * self.n_win)()
+        rc = self._check(lib().tm_solve_adjoint(self._h, _ptr(w), ctypes.byref(o), _ptr(out), ctypes.addressof(info)))
+        return out, list(info), rc
+
+    def fields(self, pts, s, which=TM_FIELD_E_SCA, out=None):
+        pts = np.ascontiguousarray(pts, dtype=np.float64) if isinstance(pts, np.ndarray) else pts
+        s = np.ascontiguousarray(s, dtype=np.complex128) if isinstance(s, np.ndarray) else s
+        n_pts = int(pts.shape[0])
+        if out is None:
+            if isinstance(pts, np.ndarray):
+                out = np.empty((n_pts, 3), dtype=np.complex128)
+            else:
+                import torch
+                out = torch.empty((n_pts, 3), dtype=torch.complex128, device=pts.device)
+        self._check(lib().tm_fields(self._h, n_pts, _ptr(pts), _ptr(s), int(which), _ptr(out)))
+        return out
+
+    def kernel_time(self, reset=False):
+        ms, n_ap, n_tot = ctypes.c_double(), ctypes.c_longlong(), ctypes.c_longlong()
+        self._check(lib().tm_kernel_time(self._h, 1 if reset else 0, ctypes.byref(ms), ctypes.byref(n_ap), ctypes.byref(n_tot)))
+        return ms.value, n_ap.value, n_tot.value
+
+
+def solver_for_workload(w, precision=TM_FP64, stream=None, kernel=TM_KERNEL_AUTO):
+    """Build a Solver for a workloads.py dict: positions, windows, T (Mie via tm_mie_tmatrix or given full T) and
+    the incident field.  Input marshalling only."""
+    s = Solver(w["pos"], w["lmax"], w["k"], win_ptr=w["win_ptr"], precision=precision, stream=stream)
+    if kernel != TM_KERNEL_AUTO:
+        s.set_kernel(kernel)
+    if w["t_kind"] in ("mie_types", "mie_sites"):
+        T = np.stack([mie_tmatrix(w["lmax"], w["k"], r, w["eps_r"]) for r in w["radii"]])
+        s.set_tmatrices(T, w["type_of"], True, r_enclosing=np.asarray(w["radii"], dtype=np.float64))
+    else:
+        s.set_tmatrices(w["t_full"], w["type_of"], False)
+    if w["inc_kind"] == "plane":
+        s.set_incident_plane(w["beta"], w["alpha"], w["A_beta"], w["A_alpha"])
+    else:
+        s.set_incident_gauss(w["focus"], w["w0"], w["Ax"], w["Ay"])
+    return s

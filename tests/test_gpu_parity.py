@@ -1,0 +1,280 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle,
+element by element on the same seeded inputs.  Tolerances:
+  matvec: rel. L2 <= 1e-12 (fp64) / 2e-5 (fp32);  solve: <= 1e-9 (fp64, GMRES 1e-10..1e-11) / 1e-4 (fp32, 1e-6).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from oracle import driver, fields, incident, matvec as omv, system, tmatrix  # noqa: E402
+from paper_2107_09879_b200 import workloads as W  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def tm():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2107_09879_b200 import libtm
+    libtm.lib()          # hard error if the extension is missing
+    return libtm
+
+
+def rel(a, b):
+    return np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(b)
+
+
+def rand_x(shape, seed):
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+
+
+# ------------------------------------------------------------------------------------------ T-matrix helper
+def test_mie_tmatrix_matches_oracle(tm):
+    for lmax in (1, 2, 3, 5):
+        for R in (0.05, 0.10, 0.2, 0.24, 0.7):
+            t = tm.mie_tmatrix(lmax, W.K_B, R, 4.0)
+            ref = tmatrix.mie_tmatrix_diag(lmax, W.K_B, R, 4.0)
+            assert np.abs(t - ref).max() <= 1e-13 * max(1.0, np.abs(ref).max())
+    t = tm.mie_tmatrix(3, W.K_B, 0.2, 2.5 + 0.3j)
+    assert np.abs(t - tmatrix.mie_tmatrix_diag(3, W.K_B, 0.2, 2.5 + 0.3j)).max() < 1e-13
+
+
+# ------------------------------------------------------------------------------------------ bare A x
+@pytest.mark.parametrize("kernel", ["coplanar", "general"])
+@pytest.mark.parametrize("lmax,n_side", [(1, 9), (2, 11), (3, 13)])
+def test_allpairs_matvec_lattice(tm, kernel, lmax, n_side):
+    """u = A x on a planar lattice spanning several target tiles (64) and a ragged tail, both kernels."""
+    pos = W.lattice(n_side, n_side + 2)
+    x = rand_x((pos.shape[0], W.n_modes(lmax)), 10 + lmax)
+    s = tm.Solver(pos, lmax, W.K_B)
+    s.set_kernel(tm.TM_KERNEL_COPLANAR if kernel == "coplanar" else tm.TM_KERNEL_GENERAL)
+    assert s.get_kernel() == (tm.TM_KERNEL_COPLANAR if kernel == "coplanar" else tm.TM_KERNEL_GENERAL)
+    u = s.matvec(x, transpose=2)
+    ref = omv.matvec_rows(lmax, W.K_B, pos, x)
+    assert rel(u, ref) <= 1e-12
+    s.close()
+
+
+@pytest.mark.parametrize("lmax", [1, 2, 3, 4])
+def test_allpairs_matvec_random_3d_cloud(tm, lmax):
+    """Random non-lattice 3-D positions (PAPER.md:375 uses random positions): general kernel is selected."""
+    n = 150 if lmax <= 3 else 40
+    pos = W.random_cloud(n, seed=20 + lmax)
+    x = rand_x((n, W.n_modes(lmax)), 30 + lmax)
+    s = tm.Solver(pos, lmax, W.K_B)
+    assert s.get_kernel() == tm.TM_KERNEL_GENERAL
+    u = s.matvec(x, transpose=2)
+    ref = omv.matvec_rows(lmax, W.K_B, pos, x)
+    assert rel(u, ref) <= 1e-12
+    s.close()
+
+
+def test_allpairs_matvec_planar_cloud_auto_selects_coplanar(tm):
+    pos = W.random_cloud(300, seed=5, planar=True)
+    pos[:, 2] = 0.37                                   # any common z
+    x = rand_x((300, 30), 6)
+    s = tm.Solver(pos, 3, W.K_B)
+    assert s.get_kernel() == tm.TM_KERNEL_COPLANAR
+    assert rel(s.matvec(x, transpose=2), omv.matvec_rows(3, W.K_B, pos, x)) <= 1e-12
+    s.close()
+
+
+def test_allpairs_matvec_windows(tm):
+    """Windows are independent problems (reading R16): ragged window sizes incl. a single-scatterer window."""
+    pos = W.random_cloud(200, seed=8, planar=True)
+    wp = np.array([0, 1, 70, 71, 200], dtype=np.int32)
+    x = rand_x((200, 30), 9)
+    for kern in (tm.TM_KERNEL_COPLANAR, tm.TM_KERNEL_GENERAL):
+        s = tm.Solver(pos, 3, W.K_B, win_ptr=wp)
+        s.set_kernel(kern)
+        u = s.matvec(x, transpose=2)
+        ref = omv.matvec_rows(3, W.K_B, pos, x, win_ptr=wp)
+        assert rel(u, ref) <= 1e-12
+        assert np.all(u[0] == 0) and np.all(u[70] == 0)      # lone scatterers see nobody
+        s.close()
+
+
+def test_fp32_matvec(tm):
+    w = W.config(2, scale=12)
+    pos = w["pos"] * 8.0                                 # stretch so that k r reaches ~600 (phase-reduction hazard)
+    x = rand_x((pos.shape[0], 30), 11)
+    s = tm.Solver(pos, 3, W.K_B, precision=tm.TM_FP32)
+    u = s.matvec(x, transpose=2)
+    assert rel(u, omv.matvec_rows(3, W.K_B, pos, x)) <= 2e-5
+    s.close()
+
+
+# ------------------------------------------------------------------------------------------ full operator and transpose
+@pytest.mark.parametrize("full_t", [False, True])
+def test_operator_and_transpose_vs_dense(tm, full_t):
+    w = W.cloud_workload(60, seed=3, lmax=3, planar=False, full_t=full_t, n_win=2)
+    t, type_of, diag = driver.tmatrices(w)
+    M = system.assemble_M(3, w["k"], w["pos"], t, type_of, diag, list(w["win_ptr"]))
+    x = rand_x((60, 30), 4)
+    s = tm.Solver(w["pos"], 3, w["k"], win_ptr=w["win_ptr"])
+    s.set_tmatrices(t, type_of, diag)
+    assert rel(s.matvec(x, 0).reshape(-1), M @ x.reshape(-1)) <= 1e-12
+    assert rel(s.matvec(x, 1).reshape(-1), M.T @ x.reshape(-1)) <= 1e-12
+    s.close()
+
+
+# ------------------------------------------------------------------------------------------ incident, fields
+def test_incident_plane_and_gauss(tm):
+    w = W.cloud_workload(40, seed=12, lmax=3, planar=False)
+    s = tm.solver_for_workload(w)
+    assert rel(s.get_incident(), driver.incident_coeffs(w)) <= 1e-13
+    # Gaussian beams, one focus per window, oblique polarisation
+    wp = np.array([0, 15, 40], dtype=np.int32)
+    focus = np.array([[0.1, -0.2, 0.3], [-0.5, 0.4, -0.1]])
+    for w0 in (2.0, 10.0):
+        g = tm.Solver(w["pos"], 3, w["k"], win_ptr=wp)
+        g.set_incident_gauss(focus, w0, 0.8, 0.3 - 0.4j)
+        ref = np.concatenate([incident.gaussian_beam_incident(3, w["k"], w["pos"][wp[i]:wp[i + 1]], focus[i], w0, 0.8, 0.3 - 0.4j)
+                              for i in range(2)])
+        assert rel(g.get_incident(), ref) <= 1e-11
+        g.close()
+    s.close()
+
+
+def test_fields_E_and_H(tm):
+    w = W.cloud_workload(30, seed=13, lmax=3, planar=False)
+    s = tm.Solver(w["pos"], 3, w["k"])
+    coef = rand_x((30, 30), 14)
+    rng = np.random.default_rng(15)
+    pts = rng.uniform(-6, 6, (257, 3))
+    pts[0] = w["pos"][3] + [0, 0, 0.8]                   # straight above a scatterer (theta = 0)
+    pts[1] = w["pos"][5] - [0, 0, 1.1]                   # straight below (theta = pi)
+    d = np.linalg.norm(pts[:, None, :] - w["pos"][None], axis=2).min(axis=1)
+    pts = pts[d > 0.3]
+    E = s.fields(pts, coef, tm.TM_FIELD_E_SCA)
+    H = s.fields(pts, coef, tm.TM_FIELD_H_SCA)
+    assert rel(E, fields.e_sca(3, w["k"], w["pos"], coef, pts)) <= 1e-12
+    assert rel(H, fields.zh_sca(3, w["k"], w["pos"], coef, pts)) <= 1e-12
+    s.close()
+
+
+# ------------------------------------------------------------------------------------------ solves
+def test_solve_cfg1(tm):
+    w = W.config(1)
+    ref = driver.solve(w)
+    s = tm.solver_for_workload(w)
+    sol, info, rc = s.solve(w["tol"], w["restart"], w["max_iter"])
+    assert rc == 0 and info[0].converged and info[0].rel_residual <= w["tol"]
+    assert rel(sol, ref["s"]) <= 1e-9
+    cext, csca = fields.cross_sections(w["lmax"], w["k"], w["pos"], sol, s.get_incident())
+    assert abs(cext - csca) <= 1e-8 * abs(cext)          # lossless spheres: extinction = scattering
+    s.close()
+
+
+@pytest.mark.parametrize("cfg,scale", [(2, 12), (5, 12), ("3b", 8)])
+def test_solve_reduced_configs(tm, cfg, scale):
+    """Same generators as BASELINE.json configs 2 / 5 / 3b at a size where the dense LU oracle fits."""
+    w = W.config(cfg, scale=scale)
+    ref = driver.solve(w)
+    s = tm.solver_for_workload(w)
+    sol, info, rc = s.solve(1e-11, w["restart"], w["max_iter"])
+    assert rc == 0, info[0].rel_residual
+    assert rel(sol, ref["s"]) <= 1e-9
+    s.close()
+
+
+def test_solve_windows_and_adjoint(tm):
+    """Config-4 shape at reduced size: 4 independent windows, Gaussian beams, forward + adjoint."""
+    w = W.config(4, scale=6)
+    rng = np.random.default_rng(44)
+    ref = driver.solve(w, adjoint_w=w["w_adj"])
+    s = tm.solver_for_workload(w)
+    sol, info, rc = s.solve(1e-11, 50, 2000)
+    assert rc == 0 and len(info) == 4
+    assert rel(sol, ref["s"]) <= 1e-9
+    lam, info2, rc2 = s.solve_adjoint(w["w_adj"], 1e-11, 50, 2000)
+    assert rc2 == 0
+    assert rel(lam, ref["lam"]) <= 1e-9
+    # bilinear identity lam^T (T p) = w^T s  (exact link between forward and adjoint solves)
+    t, type_of, diag = driver.tmatrices(w)
+    b = system.apply_T(t, type_of, ref["p"], diag)
+    lhs, rhs = np.sum(lam * b), np.sum(w["w_adj"] * sol)
+    assert abs(lhs - rhs) <= 1e-8 * abs(rhs)
+    # a window solved alone gives the same answer as inside the batch
+    lo, hi = w["win_ptr"][1], w["win_ptr"][2]
+    w1 = dict(w, pos=w["pos"][lo:hi], win_ptr=np.array([0, hi - lo], dtype=np.int32), radii=w["radii"][lo:hi],
+              type_of=np.arange(hi - lo, dtype=np.int32), focus=w["focus"][1:2])
+    s1 = tm.solver_for_workload(w1)
+    sol1, _, _ = s1.solve(1e-11, 50, 2000)
+    assert rel(sol1, sol[lo:hi]) <= 1e-9
+    s.close(); s1.close()
+    del rng
+
+
+def test_solve_3d_cloud_full_T_general_kernel(tm):
+    w = W.cloud_workload(50, seed=21, lmax=2, planar=False, full_t=True)
+    ref = driver.solve(w)
+    s = tm.solver_for_workload(w)
+    sol, info, rc = s.solve(w["tol"], w["restart"], w["max_iter"])
+    assert rc == 0 and rel(sol, ref["s"]) <= 1e-9
+    s.close()
+
+
+def test_solve_fp32(tm):
+    w = W.config(2, scale=10)
+    ref = driver.solve(w)
+    s = tm.solver_for_workload(w, precision=tm.TM_FP32)
+    sol, info, rc = s.solve(1e-6, 50, 2000)
+    assert rel(sol, ref["s"]) <= 1e-4
+    assert info[0].rel_residual <= 5e-6
+    s.close()
+
+
+def test_not_converged_is_soft(tm):
+    w = W.config(2, scale=10)
+    s = tm.solver_for_workload(w)
+    sol, info, rc = s.solve(1e-12, 5, 10)
+    assert rc == tm.TM_NOT_CONVERGED and not info[0].converged and info[0].iterations == 10
+    assert np.all(np.isfinite(sol))
+    s.close()
+
+
+# ------------------------------------------------------------------------------------------ boundary behaviour
+def test_error_codes(tm):
+    pos = W.lattice(3, 3)
+    with pytest.raises(tm.TmError) as e:
+        tm.Solver(pos, 9, W.K_B)
+    assert e.value.code == tm.TM_E_INVALID
+    bad = pos.copy(); bad[4] = bad[0]
+    with pytest.raises(tm.TmError) as e:
+        tm.Solver(bad, 2, W.K_B)
+    assert e.value.code == tm.TM_E_INVALID
+    s = tm.Solver(pos, 2, W.K_B)
+    with pytest.raises(tm.TmError) as e:
+        s.solve(1e-8, 10, 10)
+    assert e.value.code == tm.TM_E_STATE
+    T = np.stack([tm.mie_tmatrix(2, W.K_B, 0.3, 4.0)])
+    with pytest.raises(tm.TmError) as e:
+        s.set_tmatrices(T, np.zeros(9, dtype=np.int32), True, r_enclosing=np.array([0.3]))   # 0.6 > pitch 0.5
+    assert e.value.code == tm.TM_E_OVERLAP
+    pos3 = pos.copy(); pos3[2, 2] = 0.1
+    s3 = tm.Solver(pos3, 2, W.K_B)
+    with pytest.raises(tm.TmError) as e:
+        s3.set_kernel(tm.TM_KERNEL_COPLANAR)
+    assert e.value.code == tm.TM_E_INVALID
+    s.close(); s3.close()
+
+
+def test_device_pointers_and_torch_workspace(tm):
+    """PyTorch supplies device memory and the stream; data stays on the device."""
+    import torch
+    w = W.config(2, scale=10)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        s = tm.solver_for_workload(w, stream=st.cuda_stream)
+        ws = torch.empty(s.workspace_bytes(50), dtype=torch.uint8, device="cuda")
+        s.set_workspace(ws)
+        out = torch.empty((s.n_scat, s.L), dtype=torch.complex128, device="cuda")
+        sol, info, rc = s.solve(1e-11, 50, 2000, out=out)
+        host, _, _ = tm.solver_for_workload(w).solve(1e-11, 50, 2000)
+        assert rc == 0 and rel(out.cpu().numpy(), host) <= 1e-12
+        x = torch.randn((s.n_scat, s.L), dtype=torch.complex128, device="cuda")
+        y = s.matvec(x, 0)
+        assert rel(y.cpu().numpy(), s.matvec(x.cpu().numpy(), 0)) == 0.0
+        s.close()
