@@ -1,0 +1,358 @@
+#!/usr/bin/env python3
+"""bench.py - one JSON line per run (driver contract).
+
+A "step" is one pass of the WHOLE hot path over one batch of synthetic input:
+  a1 incident expansion -> a2 RHS -> a3-a6 forward GMRES solve (on-the-fly translation + all-pairs matvec +
+  T application + Arnoldi/Givens) -> a7 adjoint solve with a seeded random weight vector -> a8 scattered
+  E field on a detector plane.
+Metric (BASELINE.json): pair-block complex MAC/s = (all-pairs matvecs in the step) x (ordered pairs) x L^2 / time.
+Default workload: BASELINE.json configs[1] (32x32 lattice, lmax 3, fp64), whose full solve fits a step of well
+under a second; `--workload cfg5` etc. run the larger configs (their full solves take minutes).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg2]
+
+N > 1 (torchrun): replicas only - every rank runs the same independent problem (the paper's windows are
+independent units); no data-path collective; value = sum over ranks / max time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2107_09879_b200 import workloads as W  # noqa: E402
+
+METRIC = "pair_block_complex_MAC_per_s"
+UNIT = "cMAC/s"
+
+
+def n_pairs(w):
+    wp = np.asarray(w["win_ptr"], dtype=np.int64)
+    c = np.diff(wp)
+    return int(np.sum(c * (c - 1)))
+
+
+def detector_points(w, n_side=64, height=5.0):
+    pos = w["pos"]
+    lo, hi = pos.min(axis=0), pos.max(axis=0)
+    gx = np.linspace(lo[0], hi[0], n_side)
+    gy = np.linspace(lo[1], hi[1], n_side)
+    X, Y = np.meshgrid(gx, gy, indexing="xy")
+    return np.ascontiguousarray(np.stack([X.ravel(), Y.ravel(), np.full(X.size, pos[0, 2] + height)], axis=1))
+
+
+def adjoint_weight(w):
+    if "w_adj" in w:
+        return np.ascontiguousarray(w["w_adj"])
+    rng = np.random.default_rng(1234)
+    return W.complex_normal((w["pos"].shape[0], W.n_modes(w["lmax"])), rng)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(len(r) >= 7 and r[3 + k].lower().startswith("active") for r in self.rows)]
+        pw = [float(r[2]) for r in self.rows if len(r) >= 7 and r[2].replace(".", "").isdigit()]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
+
+
+# --------------------------------------------------------------------------------------------- reference arm
+def run_reference(args, w, rank, world):
+    """The oracle (CPU, as it stands) on a bounded sample of the same workload: its matrix-free all-pairs
+    matvec (oracle/matvec_c.c, OpenMP) on a row sample per step."""
+    if rank != 0:
+        return
+    from oracle import matvec as omv
+    omv.build()
+    N, L = w["pos"].shape[0], W.n_modes(w["lmax"])
+    x = adjoint_weight(w)
+    rng = np.random.default_rng(7)
+    omv.matvec_rows(w["lmax"], w["k"], w["pos"], x, rows=np.arange(2, dtype=np.int32), win_ptr=w["win_ptr"])   # tables, load
+    t0 = time.perf_counter()
+    omv.matvec_rows(w["lmax"], w["k"], w["pos"], x, rows=np.arange(min(64, N), dtype=np.int32), win_ptr=w["win_ptr"])
+    per_row = (time.perf_counter() - t0) / min(64, N)
+    rows_per_step = int(max(4, min(N, 4.0 / per_row)))          # ~4 s of CPU work per step
+    wp = np.asarray(w["win_ptr"])
+    win_of = np.searchsorted(wp, np.arange(N), side="right") - 1
+    times, pairs = [], []
+    for it in range(args.warmup + args.steps):
+        rows = np.sort(rng.choice(N, rows_per_step, replace=False)).astype(np.int32)
+        t0 = time.perf_counter()
+        omv.matvec_rows(w["lmax"], w["k"], w["pos"], x, rows=rows, win_ptr=w["win_ptr"])
+        dt = time.perf_counter() - t0
+        if it >= args.warmup:
+            times.append(dt)
+            pairs.append(int(np.sum(wp[win_of[rows] + 1] - wp[win_of[rows]] - 1)))
+    val = sum(pairs) * L * L / sum(times)
+    sample = f"{rows_per_step} random target rows of one all-pairs matvec per step (oracle/matvec_c.c, OpenMP)"
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times), "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": w["name"], "n_scat": N, "lmax": w["lmax"], "L": L, "sample": sample},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": omv.num_threads(), "kind": "oracle", "sample": sample},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+# --------------------------------------------------------------------------------------------- our arm
+def cpu_baseline(w):
+    from oracle import matvec as omv
+    omv.build()
+    N, L = w["pos"].shape[0], W.n_modes(w["lmax"])
+    x = adjoint_weight(w)
+    omv.matvec_rows(w["lmax"], w["k"], w["pos"], x, rows=np.arange(2, dtype=np.int32), win_ptr=w["win_ptr"])   # tables, load
+    t0 = time.perf_counter()
+    omv.matvec_rows(w["lmax"], w["k"], w["pos"], x, rows=np.arange(min(64, N), dtype=np.int32), win_ptr=w["win_ptr"])
+    per_row = (time.perf_counter() - t0) / min(64, N)
+    n_rows = int(max(4, min(N, 12.0 / per_row)))
+    rows = np.sort(np.random.default_rng(7).choice(N, n_rows, replace=False)).astype(np.int32)
+    wp = np.asarray(w["win_ptr"])
+    win_of = np.searchsorted(wp, np.arange(N), side="right") - 1
+    t0 = time.perf_counter()
+    omv.matvec_rows(w["lmax"], w["k"], w["pos"], x, rows=rows, win_ptr=w["win_ptr"])
+    dt = time.perf_counter() - t0
+    prs = int(np.sum(wp[win_of[rows] + 1] - wp[win_of[rows]] - 1))
+    return {"value": prs * L * L / dt, "unit": UNIT, "cores": omv.num_threads(), "kind": "oracle",
+            "sample": f"{n_rows} of {N} target rows of one all-pairs matvec ({prs} ordered pairs, {dt:.1f} s, oracle/matvec_c.c)"}
+
+
+def run_ours(args, w, rank, world, local_rank):
+    import torch
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    from paper_2107_09879_b200 import libtm
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    prec = libtm.TM_FP32 if args.precision == "fp32" else libtm.TM_FP64
+    st = torch.cuda.Stream()
+    N, L = w["pos"].shape[0], W.n_modes(w["lmax"])
+    pairs = n_pairs(w)
+    pts = detector_points(w)
+    wadj = adjoint_weight(w)
+    max_iter = args.max_iter or w["max_iter"]
+    tol = args.tol or w["tol"]
+
+    with torch.cuda.stream(st):
+        peak = libtm.measure_fma_peak(prec, st.cuda_stream)
+        s = libtm.solver_for_workload(w, precision=prec, stream=st.cuda_stream)
+        ws = torch.empty(s.workspace_bytes(w["restart"]), dtype=torch.uint8, device="cuda")
+        s.set_workspace(ws)
+        d_w = torch.from_numpy(wadj).cuda()
+        d_pts = torch.from_numpy(pts).cuda()
+        d_s = torch.empty((N, L), dtype=torch.complex128, device="cuda")
+        d_lam = torch.empty_like(d_s)
+        d_E = torch.empty((pts.shape[0], 3), dtype=torch.complex128, device="cuda")
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2
+
+        def set_inc(sol):
+            if w["inc_kind"] == "plane":
+                sol.set_incident_plane(w["beta"], w["alpha"], w["A_beta"], w["A_alpha"])
+            else:
+                sol.set_incident_gauss(w["focus"], w["w0"], w["Ax"], w["Ay"])
+
+        d_x = torch.from_numpy(wadj).cuda()
+        d_y = torch.empty_like(d_x)
+
+        def step_matvec():
+            s.matvec(d_x, 0, out=d_y)
+            one = libtm.SolveInfo(0, 0, 1, 1, 0.0, 0.0)
+            zero = libtm.SolveInfo(0, 0, 1, 0, 0.0, 0.0)
+            return [one], [zero], 0, 0
+
+        def step_resident():
+            set_inc(s)
+            _, info, rc = s.solve(tol, w["restart"], max_iter, out=d_s)
+            _, info2, rc2 = s.solve_adjoint(d_w, tol, w["restart"], max_iter, out=d_lam)
+            s.fields(d_pts, d_s, libtm.TM_FIELD_E_SCA, out=d_E)
+            return info, info2, rc, rc2
+
+        def timed(fn, n_warm, n_steps):
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_steps)]
+            res = None
+            for it in range(n_warm + n_steps):
+                flush.fill_(it & 0xff)                      # L2 flush between iterations (outside the timed bracket)
+                if it == n_warm:
+                    s.kernel_time(reset=True)
+                    if dist is not None:
+                        dist.barrier()
+                    torch.cuda.synchronize()
+                if it >= n_warm:
+                    ev[it - n_warm][0].record(st)
+                res = fn()
+                if it >= n_warm:
+                    ev[it - n_warm][1].record(st)
+            torch.cuda.synchronize()
+            if dist is not None:
+                dist.barrier()
+            return [a.elapsed_time(b) for a, b in ev], res
+
+        clocks = ClockSampler(local_rank)
+        clocks.start()
+        ms_list, (info, info2, rc, rc2) = timed(step_matvec if args.mode == "matvec" else step_resident, args.warmup, args.steps)
+        ap_ms, ap_launches, tot_launches = s.kernel_time(reset=False)
+        clk = clocks.stop()
+        matvecs = info[0].matvecs + info2[0].matvecs
+        total_ms = float(sum(ms_list))
+
+        # end to end through the C ABI with HOST buffers: context creation (uploads positions, T, types), incident,
+        # both solves and the field evaluation, every result copied back to host memory
+        T_host = None
+        if w["t_kind"] in ("mie_types", "mie_sites"):
+            T_host = np.stack([libtm.mie_tmatrix(w["lmax"], w["k"], r, w["eps_r"]) for r in w["radii"]])
+        else:
+            T_host = np.ascontiguousarray(w["t_full"])
+        h_s = np.empty((N, L), dtype=np.complex128)
+        h_lam = np.empty_like(h_s)
+        h_E = np.empty((pts.shape[0], 3), dtype=np.complex128)
+
+        h_y = np.empty_like(wadj)
+
+        def step_e2e_matvec():
+            s.matvec(wadj, 0, out=h_y)
+            return [libtm.SolveInfo(0, 0, 1, 1, 0.0, 0.0)], [libtm.SolveInfo(0, 0, 1, 0, 0.0, 0.0)], 0, 0
+
+        def step_e2e():
+            s2 = libtm.Solver(w["pos"], w["lmax"], w["k"], win_ptr=w["win_ptr"], precision=prec, stream=st.cuda_stream)
+            s2.set_workspace(ws)
+            s2.set_tmatrices(T_host, w["type_of"], w["t_kind"] != "full_types")
+            set_inc(s2)
+            _, i1, _ = s2.solve(tol, w["restart"], max_iter, out=h_s)
+            _, i2, _ = s2.solve_adjoint(wadj, tol, w["restart"], max_iter, out=h_lam)
+            s2.fields(pts, h_s, libtm.TM_FIELD_E_SCA, out=h_E)
+            s2.close()
+            return i1, i2, 0, 0
+
+        e2e_steps = max(1, min(args.steps, 3))
+        e2e_ms, (i1, i2, _, _) = timed(step_e2e_matvec if args.mode == "matvec" else step_e2e, 1, e2e_steps)
+        e2e_matvecs = i1[0].matvecs + i2[0].matvecs
+        if args.mode == "matvec":
+            h2d, d2h = wadj.nbytes, h_y.nbytes
+        else:
+            h2d = 0
+        h2d = h2d or w["pos"].nbytes + T_host.nbytes + np.asarray(w["type_of"]).nbytes + wadj.nbytes + pts.nbytes + h_s.nbytes
+        d2h = d2h if args.mode == "matvec" else h_s.nbytes + h_lam.nbytes + h_E.nbytes
+        fpinst, flop = s.pair_cost()
+        kern = s.get_kernel()
+
+    # max over ranks
+    t_step = total_ms / len(ms_list)
+    t_e2e = float(sum(e2e_ms)) / len(e2e_ms)
+    if dist is not None:
+        tt = torch.tensor([t_step, t_e2e], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_step, t_e2e = float(tt[0]), float(tt[1])
+    cmac_step = matvecs * pairs * L * L
+    value = world * cmac_step / (t_step * 1e-3)
+    e2e_value = world * e2e_matvecs * pairs * L * L / (t_e2e * 1e-3)
+
+    if rank == 0:
+        ap_avg_ms = ap_ms / max(1, ap_launches)
+        achieved = pairs * flop / (ap_avg_ms * 1e-3) * 1e-12 if ap_launches else None
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+        if os.path.exists(tpath):
+            try:
+                traffic = json.load(open(tpath)).get(w["name"])
+            except Exception:
+                traffic = None
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": t_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64" if prec == libtm.TM_FP64 else "f32", "data": "synthetic",
+            "config": {"workload": w["name"], "n_scat": N, "lmax": w["lmax"], "L": L, "n_windows": len(w["win_ptr"]) - 1,
+                       "ordered_pairs": pairs, "tol": tol, "restart": w["restart"],
+                       "step": ("one operator application y = (I - T A) x (matvec-only mode)" if args.mode == "matvec" else
+                                "incident + forward GMRES solve + adjoint GMRES solve + E field on 64x64 detector points"),
+                       "l2": "flushed between steps (256 MB write)",
+                       "kernel": "coplanar" if kern == libtm.TM_KERNEL_COPLANAR else "general",
+                       "parallelism": "replicas" if world > 1 else "single"},
+            "solve": {"forward_iterations": max(i.iterations for i in info), "adjoint_iterations": max(i.iterations for i in info2),
+                      "forward_rel_residual": max(i.rel_residual for i in info), "adjoint_rel_residual": max(i.rel_residual for i in info2),
+                      "forward_seconds": info[0].seconds, "adjoint_seconds": info2[0].seconds, "converged": bool(rc == 0 and rc2 == 0),
+                      "matvecs_per_step": matvecs, "matvecs_per_s": matvecs / (t_step * 1e-3)},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "ms_per_step": t_e2e, "steps": e2e_steps},
+            "gpu_launches": int(tot_launches),
+            "roofline": {"bound": "alu", "kernel": "k_allpairs_coplanar" if kern == libtm.TM_KERNEL_COPLANAR else "k_allpairs_general",
+                         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": (achieved / peak) if achieved else None,
+                         "peak_source": "measured live: tm_measure_fma_peak (register-resident FMA chains, this GPU, this run)",
+                         "flop_per_pair": flop, "fp_instr_per_pair": fpinst, "pairs_per_launch": pairs,
+                         "avg_launch_ms": ap_avg_ms, "launches": int(ap_launches), "share_of_step": ap_ms / total_ms if total_ms else None,
+                         "pipe_frac": (pairs * fpinst / (ap_avg_ms * 1e-3)) / (peak * 1e12 / 2) if ap_launches else None,
+                         "pairs_per_s": pairs / (ap_avg_ms * 1e-3) if ap_launches else None, "traffic": traffic},
+            "clocks": clk,
+        }
+        if not args.no_cpu_baseline and world == 1:
+            out["cpu_baseline"] = cpu_baseline(w)
+        print(json.dumps(out), flush=True)
+    s.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--mode", default="full", choices=["full", "matvec"], help="matvec: time operator applications only")
+    ap.add_argument("--scale", type=int, default=None, help="lattice side override (parity-size runs)")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
+    ap.add_argument("--max-iter", type=int, default=None)
+    ap.add_argument("--tol", type=float, default=None)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    name = args.workload[3:] if args.workload.startswith("cfg") else args.workload
+    w = W.config(name if name == "3b" else int(name), scale=args.scale)
+    if args.impl == "reference":
+        run_reference(args, w, rank, world)
+    else:
+        run_ours(args, w, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

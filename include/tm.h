@@ -136,6 +136,17 @@ int tm_get_kernel(const tm_ctx *ctx);
 int tm_kernel_time(tm_ctx *ctx, int reset, double *allpairs_ms, long long *allpairs_launches,
                    long long *total_launches);
 
+/* Executed floating-point work of the active all-pairs kernel per ORDERED pair:
+ * fp_instructions = FMA/MUL/ADD issue slots on the FP64 (or FP32) pipe, flop with FMA = 2.  Counted from the
+ * generated straight-line code (coplanar kernel; per-pair geometry excluded, so rooflines are conservative) or
+ * from the term table (general kernel). */
+int tm_pair_cost(const tm_ctx *ctx, double *fp_instructions, double *flop);
+
+/* Register-resident FMA microbenchmark on the current device (no memory traffic, 8 independent chains per
+ * thread): the measured peak of the plain FP64 / FP32 pipe that the all-pairs kernel is bounded by.
+ * precision TM_FP64 / TM_FP32; result in TFLOP/s (FMA = 2 flop).  Needs a CUDA device. */
+int tm_measure_fma_peak(int precision, double *tflops, void *cuda_stream);
+
 /* Host helper: diagonal of the Lorenz-Mie T-matrix of a homogeneous sphere (reading R11; closed form,
  * T_{l,p=0} = -b_l, T_{l,p=1} = -a_l), out[L] in flat mode order.  eps_r complex relative permittivity. */
 int tm_mie_tmatrix(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64 *out);

@@ -190,6 +190,7 @@ def emit_coplanar(lmaxes, path):
         f.write("// Coplanar (theta = pi/2) translation apply, one mirror-parity half per call (DESIGN.md, kernel K2c).\n")
         f.write("// xs: interleaved (re,im) tilde-basis source coefficients of this half; cm/sm: cos/sin(m phi);\n")
         f.write("// hr/hi: Re/Im h_q^(1)(kr), q = 0..2 lmax; ar/ai: accumulators of this half.\n#pragma once\n\n")
+        cost = {lmax: [0, 0] for lmax in lmaxes}
         for lmax in lmaxes:
             md = modes(lmax)
             K = coplanar_rows(lmax)
@@ -237,13 +238,25 @@ def emit_coplanar(lmaxes, path):
                         f.write(f"    ai[{kb}] = fma(ur, {sg}sm[{am}], ai[{kb}]); ai[{kb}] = fma(ui, cm[{am}], ai[{kb}]);\n")
                     f.write("  }\n")
                 f.write("}\n")
+                # executed floating-point work of this half per pair (generated code only; the ~70 geometry /
+                # Hankel instructions per thread are NOT counted, so rooflines built on this are conservative):
+                #   first term of a (row,q): 2 MUL; other terms: 2 FMA; per (row,q): 4 FMA;
+                #   output phase: 4 FMA (m != 0) or 2 ADD; input phase: 2 MUL + 2 FMA (m != 0)
+                n_m0 = sum(1 for idx in half if md[idx][1] == 0)
+                n_mx = len(half) - n_m0
+                inst = 2 * nrowq + 2 * (nterm - nrowq) + 4 * nrowq + 4 * n_mx + 2 * n_m0 + 4 * n_mx
+                flop = 2 * nrowq + 4 * (nterm - nrowq) + 8 * nrowq + 8 * n_mx + 2 * n_m0 + 6 * n_mx
+                cost[lmax][0] += inst
+                cost[lmax][1] += flop
                 print(f"lmax={lmax} half={h}: n={len(half)} coplanar terms={nterm} (row,q) combos={nrowq} "
-                      f"-> ~{2 * nterm + 4 * nrowq + 8 * len(half)} FP ops/pair/half", file=sys.stderr)
+                      f"-> {inst} FP instructions, {flop} flop per pair-half", file=sys.stderr)
             # half membership tables for the hand-written kernel
             for h in (0, 1):
                 half = [i for i, (l, m, p) in enumerate(md) if (l + m + p) % 2 == h]
                 f.write(f"__device__ __constant__ int tm_cop_half_L{lmax}_H{h}[{len(half)}] = {{{', '.join(map(str, half))}}};\n")
-            f.write(f"#define TM_COP_NH_L{lmax} {len(md) // 2}\n\n")
+            f.write(f"#define TM_COP_NH_L{lmax} {len(md) // 2}\n")
+            f.write(f"#define TM_COP_FPINST_L{lmax} {cost[lmax][0]}   // FP instructions per ordered pair (both halves)\n")
+            f.write(f"#define TM_COP_FLOP_L{lmax} {cost[lmax][1]}     // flop per ordered pair (FMA = 2)\n\n")
 
 
 def main():

@@ -957,3 +957,74 @@ int tm_mie_tmatrix(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64* ou
 }
 
 }  // extern "C"
+
+// ============================================================================================ measurement helpers
+namespace {
+
+template <typename R>
+__global__ void __launch_bounds__(256) k_fma_peak(R* out, int iters, R a, R b) {
+  R x0 = R(threadIdx.x) * R(1e-3), x1 = x0 + R(1), x2 = x0 + R(2), x3 = x0 + R(3), x4 = x0 + R(4), x5 = x0 + R(5),
+    x6 = x0 + R(6), x7 = x0 + R(7);
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+      x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+      x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+  }
+  const R s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+  if (s == R(123.456)) out[0] = s;                      // never true; keeps the chains alive
+}
+
+template <typename R>
+int fma_peak_typed(double* tflops, cudaStream_t st) {
+  R* d = nullptr;
+  if (cudaMalloc(&d, sizeof(R)) != cudaSuccess) return TM_E_CUDA;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int blocks = 148 * 8, iters = 4096;
+  double best = 0.0;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0, st);
+    k_fma_peak<R><<<blocks, 256, 0, st>>>(d, iters, R(0.999999), R(1e-7));
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return TM_E_CUDA; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double fl = 2.0 * 8 * 16 * (double)iters * 256.0 * blocks;
+    if (rep > 0) best = std::max(best, fl / (ms * 1e-3) * 1e-12);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+  *tflops = best;
+  return TM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tm_pair_cost(const tm_ctx* ctx, double* fp_instructions, double* flop) {
+  if (!ctx) return TM_E_INVALID;
+  double inst = 0.0, fl = 0.0;
+  if (ctx->kernel == TM_KERNEL_COPLANAR) {
+    const int I[4] = {0, TM_COP_FPINST_L1, TM_COP_FPINST_L2, TM_COP_FPINST_L3};
+    const int F[4] = {0, TM_COP_FLOP_L1, TM_COP_FLOP_L2, TM_COP_FLOP_L3};
+    inst = I[ctx->lmax]; fl = F[ctx->lmax];
+  } else {   // general kernel: per (term, source): 2 MUL + 4 FMA
+    const double nt = tm_term_tables[ctx->lmax - 1].n_terms;
+    inst = 6.0 * nt; fl = 10.0 * nt;
+  }
+  if (fp_instructions) *fp_instructions = inst;
+  if (flop) *flop = fl;
+  return TM_OK;
+}
+
+int tm_measure_fma_peak(int precision, double* tflops, void* cuda_stream) {
+  if (!tflops) return TM_E_INVALID;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return TM_E_CUDA; }
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  return precision == TM_FP32 ? fma_peak_typed<float>(tflops, st) : fma_peak_typed<double>(tflops, st);
+}
+
+}  // extern "C"

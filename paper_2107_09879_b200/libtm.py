@@ -21,7 +21,7 @@ TM_KERNEL_AUTO, TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR = 0, 1, 2
 
 EXPORTS = ["tm_create", "tm_set_tmatrices", "tm_set_incident", "tm_get_incident", "tm_solve", "tm_solve_adjoint",
            "tm_matvec", "tm_fields", "tm_workspace_bytes", "tm_set_workspace", "tm_set_kernel", "tm_get_kernel",
-           "tm_kernel_time", "tm_mie_tmatrix", "tm_num_modes", "tm_last_error", "tm_destroy"]
+           "tm_kernel_time", "tm_pair_cost", "tm_measure_fma_peak", "tm_mie_tmatrix", "tm_num_modes", "tm_last_error", "tm_destroy"]
 
 
 class c64(ctypes.Structure):
@@ -82,6 +82,8 @@ def lib():
         L.tm_get_kernel.argtypes = [vp]
         L.tm_kernel_time.argtypes = [vp, ci, ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(ctypes.c_longlong)]
         L.tm_mie_tmatrix.argtypes = [ci, cd, cd, c64, vp]
+        L.tm_pair_cost.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(cd)]
+        L.tm_measure_fma_peak.argtypes = [ci, ctypes.POINTER(cd), vp]
         L.tm_num_modes.argtypes = [ci]
         L.tm_last_error.argtypes = [vp]
         L.tm_last_error.restype = ctypes.c_char_p
@@ -113,6 +115,15 @@ def mie_tmatrix(lmax, k_b, radius, eps_r):
     if rc != TM_OK:
         raise TmError(rc, "tm_mie_tmatrix: invalid arguments")
     return out
+
+
+def measure_fma_peak(precision=TM_FP64, stream=None):
+    """Measured register-resident FMA peak of the device in TFLOP/s (tm_measure_fma_peak)."""
+    v = ctypes.c_double()
+    rc = lib().tm_measure_fma_peak(int(precision), ctypes.byref(v), ctypes.c_void_p(stream) if stream else None)
+    if rc != TM_OK:
+        raise TmError(rc, "tm_measure_fma_peak failed (no CUDA device?)")
+    return v.value
 
 
 class Solver:
@@ -238,6 +249,12 @@ class Solver:
                 out = torch.empty((n_pts, 3), dtype=torch.complex128, device=pts.device)
         self._check(lib().tm_fields(self._h, n_pts, _ptr(pts), _ptr(s), int(which), _ptr(out)))
         return out
+
+    def pair_cost(self):
+        """(fp_instructions, flop) per ordered pair of the active all-pairs kernel."""
+        a, b = ctypes.c_double(), ctypes.c_double()
+        self._check(lib().tm_pair_cost(self._h, ctypes.byref(a), ctypes.byref(b)))
+        return a.value, b.value
 
     def kernel_time(self, reset=False):
         ms, n_ap, n_tot = ctypes.c_double(), ctypes.c_longlong(), ctypes.c_longlong()
