@@ -261,7 +261,10 @@ def run_ours(args, w, rank, world, local_rank):
             return i1, i2, 0, 0
 
         e2e_steps = max(1, min(args.steps, 3))
-        e2e_ms, (i1, i2, _, _) = timed(step_e2e_matvec if args.mode == "matvec" else step_e2e, 1, e2e_steps)
+        if args.profile:
+            e2e_ms, (i1, i2) = [float("nan")], (info, info2)
+        else:
+            e2e_ms, (i1, i2, _, _) = timed(step_e2e_matvec if args.mode == "matvec" else step_e2e, 1, e2e_steps)
         e2e_matvecs = i1[0].matvecs + i2[0].matvecs
         if args.mode == "matvec":
             h2d, d2h = wadj.nbytes, h_y.nbytes
@@ -341,8 +344,13 @@ def main():
     ap.add_argument("--max-iter", type=int, default=None)
     ap.add_argument("--tol", type=float, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--profile", action="store_true", help="for ncu: 1 warm-up, no e2e leg, no CPU baseline (not a bench value)")
     args = ap.parse_args()
-    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.profile:
+        args.no_cpu_baseline = True
+        args.warmup = min(args.warmup, 1)
+    elif args.impl == "ours":
+        args.warmup = max(args.warmup, 3)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

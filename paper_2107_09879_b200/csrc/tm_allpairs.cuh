@@ -3,8 +3,8 @@
 //
 // Two variants:
 //   k_allpairs_coplanar  lmax <= 3, all scatterers in one plane z = const (every experiment of the paper):
-//                        straight-line generated code, thread = (target, mirror-parity half), register
-//                        accumulators, FP64/FP32 FMA-pipe bound.
+//                        straight-line generated code, thread = target, block = one mirror-parity half,
+//                        register accumulators, FP64/FP32 FMA-pipe bound.
 //   k_allpairs_general   any lmax <= 6, arbitrary 3-D positions: table-driven, warp per target.
 // Both write per-source-chunk partial sums u_part[chunk][n_scat][L]; the finishing kernel (tm_vecops.cuh)
 // adds the chunks in a fixed order (deterministic) and applies T.
@@ -51,31 +51,39 @@ TM_COP_SPEC(1, 0) TM_COP_SPEC(1, 1) TM_COP_SPEC(2, 0) TM_COP_SPEC(2, 1) TM_COP_S
 #undef TM_COP_SPEC
 
 // ---------------------------------------------------------------------------------------------------
-// Coplanar kernel.  grid = (n_tiles, n_chunk); block = 2*TJ threads: thread t handles target
-// tile.tgt_start + (t % TJ) and mirror-parity half t / TJ (warp-uniform, so the generated code's
-// coefficients are immediate / constant-bank operands).  Sources of the tile's window are split into
-// n_chunk contiguous chunks (blockIdx.y) so that small problems still fill 148 SMs; each chunk is streamed
-// through shared memory SS sources at a time (positions + coefficient vectors in the tilde basis
-// x~ = i^p x, permuted so that each half is contiguous).
-template <typename R, int LMAX, int TJ, int SS>
-__global__ void __launch_bounds__(2 * TJ)
+// Coplanar kernel.  grid = (n_tiles, n_chunk, 2); block = TJ threads.  blockIdx.z selects the mirror-parity
+// half: it is the SLOWEST grid dimension, so at any time (almost) all resident blocks of an SM run the same
+// half and its ~30 KB of straight-line code stays within the 32 KB L1.5 instruction cache (ncu showed the
+// two-halves-per-block version stalled on instruction fetch: profiles/r01_allpairs_cfg3_v1.md).
+// Thread t handles target tile.tgt_start + t.  Sources of the tile's window are split into n_chunk contiguous
+// chunks (blockIdx.y) so that small problems still fill 148 SMs; each chunk is streamed through shared memory
+// SS sources at a time (positions + this half's coefficients in the tilde basis x~ = i^p x).
+// LOCKSTEP: a __syncthreads() per source keeps the block's warps on the same instructions (the two warps
+// that share an SM sub-partition then hit in its L0 instruction cache).
+template <int LMAX> __device__ __forceinline__ const int* cop_half_table(int half);
+template <> __device__ __forceinline__ const int* cop_half_table<1>(int half) { return half ? tm_cop_half_L1_H1 : tm_cop_half_L1_H0; }
+template <> __device__ __forceinline__ const int* cop_half_table<2>(int half) { return half ? tm_cop_half_L2_H1 : tm_cop_half_L2_H0; }
+template <> __device__ __forceinline__ const int* cop_half_table<3>(int half) { return half ? tm_cop_half_L3_H1 : tm_cop_half_L3_H0; }
+
+template <typename R, int LMAX, int TJ, int SS, bool LOCKSTEP>
+__global__ void __launch_bounds__(TJ)
 k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
-                    const TmTile* __restrict__ tiles, const TmConst* __restrict__ cst, int n_scat,
-                    double k_over_pi, double inv_k, const int* __restrict__ n_active) {
+                    const TmTile* __restrict__ tiles, int n_scat, double k_over_pi, double inv_k,
+                    const int* __restrict__ n_active) {
   constexpr int L = 2 * LMAX * (LMAX + 2);
   constexpr int NH = L / 2;
   constexpr int NQ = 2 * LMAX + 1;
   if (n_active != nullptr && *n_active == 0) return;
 
   __shared__ double s_px[SS], s_py[SS];
-  __shared__ __align__(16) R s_x[SS * L * 2];          // [source][half][NH] complex, tilde basis
-  __shared__ int s_slot[L];
+  __shared__ __align__(16) R s_x[SS * NH * 2];         // [source][NH] complex, tilde basis, this half only
+  __shared__ int s_half[NH];
 
   const TmTile tile = tiles[blockIdx.x];
   const int tid = threadIdx.x;
-  const int half = tid / TJ;
-  const int tj = tid % TJ;
-  const int j = tile.tgt_start + (tj < tile.tgt_count ? tj : tile.tgt_count - 1);
+  const int half = blockIdx.z;
+  const bool live = tid < tile.tgt_count;
+  const int j = tile.tgt_start + (live ? tid : tile.tgt_count - 1);
   const double xj = pos[3 * j], yj = pos[3 * j + 1];
 
   // this block's chunk of the window's sources
@@ -83,7 +91,7 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
   const int c0 = tile.src_start + blockIdx.y * per;
   const int c1 = min(tile.src_start + tile.src_count, c0 + per);
 
-  for (int e = tid; e < L; e += 2 * TJ) s_slot[e] = cst->cop_slot[e];
+  if (tid < NH) s_half[tid] = cop_half_table<LMAX>(half)[tid];
 
   R ar[NH], ai[NH];
 #pragma unroll
@@ -91,19 +99,20 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
 
   for (int s0 = c0; s0 < c1; s0 += SS) {
     const int ns = min(SS, c1 - s0);
-    __syncthreads();                                   // previous stage fully consumed (also orders s_slot)
-    for (int e = tid; e < ns; e += 2 * TJ) { s_px[e] = pos[3 * (s0 + e)]; s_py[e] = pos[3 * (s0 + e) + 1]; }
-    for (int e = tid; e < ns * L; e += 2 * TJ) {
-      const int src = e / L, idx = e - src * L;
+    __syncthreads();                                   // previous stage fully consumed (also orders s_half)
+    for (int e = tid; e < ns; e += TJ) { s_px[e] = pos[3 * (s0 + e)]; s_py[e] = pos[3 * (s0 + e) + 1]; }
+    for (int e = tid; e < ns * NH; e += TJ) {
+      const int src = e / NH, kk = e - src * NH;
+      const int idx = s_half[kk];
       Cx<R> v = x[(size_t)(s0 + src) * L + idx];
       if (idx >= NH) v = cx<R>(-v.im, v.re);           // tilde basis: multiply p = 1 modes by i
-      const int slot = s_slot[idx];
-      s_x[(src * L + slot) * 2] = v.re;
-      s_x[(src * L + slot) * 2 + 1] = v.im;
+      s_x[2 * e] = v.re;
+      s_x[2 * e + 1] = v.im;
     }
     __syncthreads();
 #pragma unroll 1
     for (int s = 0; s < ns; ++s) {
+      if (LOCKSTEP) __syncthreads();
       const double dx = xj - s_px[s], dy = yj - s_py[s];        // d = x_dest - x_source (reading R3)
       const double r2 = dx * dx + dy * dy;
       const double rinv = r2 > 0.0 ? rsqrt(r2) : 0.0;           // self pair -> h_q = 0 -> contributes nothing
@@ -121,28 +130,20 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
       phase_kr<R>(k_over_pi, r, ck, sk);
       R hr[NQ], hi[NQ];
       hankel_up<R, NQ>((R)(rinv * inv_k), ck, sk, hr, hi);
-      const R* xs = &s_x[(s * L + half * NH) * 2];
+      const R* xs = &s_x[s * NH * 2];
       if (half == 0) CopPair<R, LMAX, 0>::run(xs, cm, sm, hr, hi, ar, ai);
       else           CopPair<R, LMAX, 1>::run(xs, cm, sm, hr, hi, ar, ai);
     }
   }
 
-  // write this chunk's partial sums, back in the standard basis: u_b = (-i)^{p_b} u~_b.
-  // Stage through shared memory so the global writes are coalesced rows of L complex numbers.
-  __syncthreads();
-  static_assert(SS >= TJ, "output staging reuses the source buffer");
+  // this chunk's partial sums of this half, back in the standard basis: u_b = (-i)^{p_b} u~_b
+  if (live) {
+    Cx<R>* out = u_part + ((size_t)blockIdx.y * n_scat + j) * L;
 #pragma unroll
-  for (int b = 0; b < NH; ++b) {
-    s_x[(tj * L + half * NH + b) * 2] = ar[b];
-    s_x[(tj * L + half * NH + b) * 2 + 1] = ai[b];
-  }
-  __syncthreads();
-  Cx<R>* out = u_part + ((size_t)blockIdx.y * n_scat + tile.tgt_start) * L;
-  for (int e = tid; e < tile.tgt_count * L; e += 2 * TJ) {
-    const int t = e / L, idx = e - t * L;
-    const int slot = s_slot[idx];
-    R vr = s_x[(t * L + slot) * 2], vi = s_x[(t * L + slot) * 2 + 1];
-    out[e] = (idx >= NH) ? cx<R>(vi, -vr) : cx<R>(vr, vi);
+    for (int b = 0; b < NH; ++b) {
+      const int idx = s_half[b];
+      out[idx] = (idx >= NH) ? cx<R>(ai[b], -ar[b]) : cx<R>(ar[b], ai[b]);
+    }
   }
 }
 

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <complex>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -21,7 +22,6 @@ namespace {
 
 std::string g_create_error;
 
-constexpr int COP_TJ = 64;       // coplanar kernel: targets per block (block = 2*TJ threads)
 constexpr int COP_SS = 64;       // coplanar kernel: sources per shared-memory stage
 constexpr int MAX_RESTART = 300;
 
@@ -43,6 +43,7 @@ struct tm_ctx {
   std::vector<int> win_ptr;
   bool coplanar = false;
   int kernel_req = TM_KERNEL_AUTO, kernel = TM_KERNEL_GENERAL;
+  int cop_tj = 128, cop_lockstep = 0;   // coplanar kernel launch shape (env TM_COP_TJ / TM_COP_LOCKSTEP override)
 
   double* d_pos = nullptr;
   int* d_win_of = nullptr;
@@ -177,16 +178,22 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
   dim3 grid(c->n_tiles, c->n_chunk);
   tick(c, true);
   if (c->kernel == TM_KERNEL_COPLANAR) {
-    dim3 block(2 * COP_TJ);
-#define TM_LAUNCH_COP(LM)                                                                                          \
-  k_allpairs_coplanar<R, LM, COP_TJ, COP_SS><<<grid, block, 0, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->d_const, \
-                                                                             c->n_scat, k_over_pi, inv_k, n_active)
+    grid.z = 2;                                         // mirror-parity half: slowest grid dimension
+#define TM_LAUNCH_COP2(LM, TJ, LS)                                                                          \
+  k_allpairs_coplanar<R, LM, TJ, COP_SS, LS><<<grid, TJ, 0, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat, \
+                                                                         k_over_pi, inv_k, n_active)
+#define TM_LAUNCH_COP(LM)                                                                                   \
+  do {                                                                                                      \
+    if (c->cop_tj == 256) { if (c->cop_lockstep) TM_LAUNCH_COP2(LM, 256, true); else TM_LAUNCH_COP2(LM, 256, false); } \
+    else { if (c->cop_lockstep) TM_LAUNCH_COP2(LM, 128, true); else TM_LAUNCH_COP2(LM, 128, false); }       \
+  } while (0)
     switch (c->lmax) {
       case 1: TM_LAUNCH_COP(1); break;
       case 2: TM_LAUNCH_COP(2); break;
       default: TM_LAUNCH_COP(3); break;
     }
 #undef TM_LAUNCH_COP
+#undef TM_LAUNCH_COP2
   } else {
     TmTermsDev tb{c->d_rowptr, c->d_col, c->d_widx, c->d_imag, c->d_coef};
 #define TM_LAUNCH_GEN(LM)                                                                                         \
@@ -396,9 +403,11 @@ int configure_kernel(tm_ctx* ctx) {
   if (want == TM_KERNEL_COPLANAR && !(ctx->coplanar && ctx->lmax <= 3))
     return fail(ctx, TM_E_INVALID, "coplanar kernel needs all z equal and lmax <= 3");
   ctx->kernel = want;
+  if (const char* e = std::getenv("TM_COP_TJ")) ctx->cop_tj = std::atoi(e) == 256 ? 256 : 128;
+  if (const char* e = std::getenv("TM_COP_LOCKSTEP")) ctx->cop_lockstep = std::atoi(e) != 0;
   int tgt_per_tile;
   switch (want == TM_KERNEL_COPLANAR ? 0 : ctx->lmax) {
-    case 0: tgt_per_tile = COP_TJ; break;
+    case 0: tgt_per_tile = ctx->cop_tj; break;
     case 1: case 2: case 3: tgt_per_tile = 4; break;
     default: tgt_per_tile = 2; break;
   }
@@ -412,8 +421,9 @@ int configure_kernel(tm_ctx* ctx) {
   ctx->n_tiles = (int)tiles.size();
   // source chunks: enough blocks for ~16 waves of 148 SMs x 3 resident blocks, at least one stage of sources each
   const int stage = (want == TM_KERNEL_COPLANAR) ? COP_SS : 16;
-  const long long target_blocks = 148LL * 3 * 16;
-  long long nchunk = (target_blocks + ctx->n_tiles - 1) / std::max(1, ctx->n_tiles);
+  const long long target_blocks = 148LL * 2 * 16;
+  const long long per_chunk_blocks = (long long)ctx->n_tiles * (want == TM_KERNEL_COPLANAR ? 2 : 1);
+  long long nchunk = (target_blocks + per_chunk_blocks - 1) / std::max(1LL, per_chunk_blocks);
   nchunk = std::min<long long>(nchunk, std::max(1, min_win / stage));
   nchunk = std::min<long long>(nchunk, 64);
   const size_t vec_bytes = ctx->n * elem_bytes(ctx);
