@@ -59,6 +59,7 @@ struct tm_ctx {
   TmTile* d_tiles = nullptr; int n_tiles = 0, n_chunk = 1;
   void* d_upart = nullptr; size_t upart_bytes = 0;
   TmChunk* d_chunks = nullptr; int n_chunks = 0; int* d_win_chunk_ptr = nullptr;
+  int ept = 4;                   // vector kernels: elements per thread (chunk = ept * TM_VT)
 
   void* d_v[3] = {nullptr, nullptr, nullptr};   // Cx<R> work vectors [n]: X, B, Z
   double2* d_io = nullptr;                      // fp64 staging [n]
@@ -308,14 +309,27 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
       Cx<R>* Vj = V + (size_t)j * n;
       TM_CUDA(apply_operator<R>(ctx, transpose, Vj, W, Z, S.n_active));
       matvecs++;
-      const size_t sm_d = (size_t)(j + 1) * (TM_VT / 32) * sizeof(double2);
+      // split the basis vectors of a dot-product pass over gridDim.y when there are few chunks
+      const int G = std::max(1, std::min(j + 1, (148 * 4 + nc - 1) / nc));
+      const size_t sm_d = (size_t)((j + 1 + G - 1) / G) * (TM_VT / 32) * sizeof(double2);
       const size_t sm_a = (size_t)(j + 1) * sizeof(double2);
-      k_dots<R><<<nc, TM_VT, sm_d, st>>>(V, n, j + 1, W, ctx->d_chunks, nc, ctx->gm.part, S.n_active);
-      k_reduce_h<<<dim3(j + 1, nw), 64, 0, st>>>(ctx->gm.part, nc, ctx->d_win_chunk_ptr, S.h1, S.ldh, 0, S.n_active);
-      k_axpy<R><<<nc, TM_VT, sm_a, st>>>(V, n, j + 1, S.h1, S.ldh, -1.0, W, ctx->d_chunks, nullptr, S.n_active);
-      k_dots<R><<<nc, TM_VT, sm_d, st>>>(V, n, j + 1, W, ctx->d_chunks, nc, ctx->gm.part, S.n_active);
-      k_reduce_h<<<dim3(j + 1, nw), 64, 0, st>>>(ctx->gm.part, nc, ctx->d_win_chunk_ptr, S.h2, S.ldh, 0, S.n_active);
-      k_axpy<R><<<nc, TM_VT, sm_a, st>>>(V, n, j + 1, S.h2, S.ldh, -1.0, W, ctx->d_chunks, ctx->gm.normpart, S.n_active);
+#define TM_DOTS(H)                                                                                              \
+  do {                                                                                                          \
+    if (ctx->ept == 1) k_dots<R, 1><<<dim3(nc, G), TM_VT, sm_d, st>>>(V, n, j + 1, W, ctx->d_chunks, nc, ctx->gm.part, S.n_active); \
+    else k_dots<R, 4><<<dim3(nc, G), TM_VT, sm_d, st>>>(V, n, j + 1, W, ctx->d_chunks, nc, ctx->gm.part, S.n_active); \
+    k_reduce_h<<<dim3(j + 1, nw), 64, 0, st>>>(ctx->gm.part, nc, ctx->d_win_chunk_ptr, H, S.ldh, 0, S.n_active); \
+  } while (0)
+#define TM_AXPY(H, NP)                                                                                          \
+  do {                                                                                                          \
+    if (ctx->ept == 1) k_axpy<R, 1><<<nc, TM_VT, sm_a, st>>>(V, n, j + 1, H, S.ldh, -1.0, W, ctx->d_chunks, NP, S.n_active); \
+    else k_axpy<R, 4><<<nc, TM_VT, sm_a, st>>>(V, n, j + 1, H, S.ldh, -1.0, W, ctx->d_chunks, NP, S.n_active);   \
+  } while (0)
+      TM_DOTS(S.h1);
+      TM_AXPY(S.h1, nullptr);
+      TM_DOTS(S.h2);
+      TM_AXPY(S.h2, ctx->gm.normpart);
+#undef TM_DOTS
+#undef TM_AXPY
       k_reduce_norm<<<nw, 64, 0, st>>>(ctx->gm.normpart, ctx->d_win_chunk_ptr, S.normw);
       k_gmres_givens<<<wb, 64, 0, st>>>(S, nw, j, o.tol);
       k_scale_or_sub<R><<<nc, TM_VT, 0, st>>>(W, nullptr, S.inv_norm, V + (size_t)(j + 1) * n, ctx->d_chunks, S.n_active);
@@ -323,7 +337,8 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
     }
     // x += V y ; r = b - M x
     k_gmres_solve_y<<<wb, 64, 0, st>>>(S, nw);
-    k_axpy<R><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr);
+    if (ctx->ept == 1) k_axpy<R, 1><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr);
+    else k_axpy<R, 4><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr);
     TM_CUDA(apply_operator<R>(ctx, transpose, X, W, Z, nullptr));
     matvecs++;
     k_scale_or_sub<R><<<nc, TM_VT, 0, st>>>(B, W, nullptr, W, ctx->d_chunks, nullptr);      // W = b - M x
@@ -419,15 +434,22 @@ int configure_kernel(tm_ctx* ctx) {
     for (int s = lo; s < hi; s += tgt_per_tile) tiles.push_back(TmTile{s, std::min(tgt_per_tile, hi - s), lo, hi - lo});
   }
   ctx->n_tiles = (int)tiles.size();
-  // source chunks: enough blocks for ~16 waves of 148 SMs x 3 resident blocks, at least one stage of sources each
-  const int stage = (want == TM_KERNEL_COPLANAR) ? COP_SS : 16;
-  const long long target_blocks = 148LL * 2 * 16;
-  const long long per_chunk_blocks = (long long)ctx->n_tiles * (want == TM_KERNEL_COPLANAR ? 2 : 1);
-  long long nchunk = (target_blocks + per_chunk_blocks - 1) / std::max(1LL, per_chunk_blocks);
-  nchunk = std::min<long long>(nchunk, std::max(1, min_win / stage));
-  nchunk = std::min<long long>(nchunk, 64);
+  // Source chunks: pick the chunk count that minimises (waves of resident blocks) x (sources per block), so that
+  // small problems fill the 148 SMs (2 resident 128-thread blocks each at 255 registers) and large ones end
+  // without a long tail; bounded by 64 chunks, >= 32 sources per chunk and 2 GB of partial sums.
+  const long long slots = 148LL * (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj : 4);
+  const long long blocks1 = (long long)ctx->n_tiles * (want == TM_KERNEL_COPLANAR ? 2 : 1);
+  int max_win = 1;
+  for (int w = 0; w < ctx->n_win; ++w) max_win = std::max(max_win, ctx->win_ptr[w + 1] - ctx->win_ptr[w]);
   const size_t vec_bytes = ctx->n * elem_bytes(ctx);
-  while (nchunk > 1 && (size_t)nchunk * vec_bytes > ((size_t)2 << 30)) --nchunk;
+  long long nchunk = 1;
+  double best = 1e300;
+  for (long long cnd = 1; cnd <= 64; ++cnd) {
+    if (cnd > 1 && (min_win / cnd < 32 || (size_t)cnd * vec_bytes > ((size_t)2 << 30))) break;
+    const long long waves = (blocks1 * cnd + slots - 1) / slots;
+    const double cost = (double)waves * (double)((max_win + cnd - 1) / cnd + 8);     // +8: per-block fixed cost
+    if (cost < best * 0.995) { best = cost; nchunk = cnd; }
+  }
   ctx->n_chunk = (int)std::max<long long>(1, nchunk);
   if (ctx->d_tiles) cudaFree(ctx->d_tiles);
   TM_CUDA(cudaMalloc(&ctx->d_tiles, tiles.size() * sizeof(TmTile)));
@@ -596,9 +618,11 @@ int tm_create(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const 
   {   // vector chunks: every chunk inside one window
     std::vector<TmChunk> ch;
     std::vector<int> wcp(n_win + 1, 0);
+    c->ept = (c->n < (size_t)148 * 2 * 4 * TM_VT) ? 1 : 4;       // small vectors: more, smaller blocks
+    const long long chunk = (long long)c->ept * TM_VT;
     for (int w = 0; w < n_win; ++w) {
       const long long e0 = (long long)wp[w] * c->L, e1 = (long long)wp[w + 1] * c->L;
-      for (long long s = e0; s < e1; s += TM_CHUNK) ch.push_back(TmChunk{w, (int)s, (int)std::min<long long>(TM_CHUNK, e1 - s)});
+      for (long long s = e0; s < e1; s += chunk) ch.push_back(TmChunk{w, (int)s, (int)std::min<long long>(chunk, e1 - s)});
       wcp[w + 1] = (int)ch.size();
     }
     if (c->n > (size_t)0x7fffffff) { g_create_error = "problem too large (n_scat * L must fit in int32)"; tm_destroy(c); return TM_E_INVALID; }

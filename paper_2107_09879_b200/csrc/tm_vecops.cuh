@@ -1,12 +1,13 @@
 // Vector-phase kernels: conversions, per-scatterer T application (Eq. I25), and the
 // device-resident GMRES building blocks (reading R13).  All are HBM/L2-streaming kernels.
 // Windows (independent problems batched on one GPU) are handled through a chunk table: every
-// chunk of <= TM_CHUNK consecutive vector elements lies inside exactly one window.
+// chunk of <= EPT * TM_VT consecutive vector elements lies inside exactly one window.
 #pragma once
 #include "tm_common.cuh"
 
-#define TM_CHUNK 1024            // complex elements per chunk (one block of 256 threads, 4 per thread)
-#define TM_VT 256
+#define TM_VT 256                // threads per block of the vector kernels
+// A chunk holds EPT * TM_VT complex elements (EPT = elements per thread: 4 for large problems, 1 for small ones so
+// that a 30 720-element vector still spreads over 120 blocks; chosen once per context).
 
 struct TmChunk { int win; int start; int count; };   // element range [start, start+count) of window win
 
@@ -87,26 +88,28 @@ k_tapply(int mode, int L, int n_scat, int n_chunk, const Cx<R>* __restrict__ x, 
 }
 
 // ------------------------------------------------------------------------------------------------ GMRES pieces
-// part[i * n_chunks + c] = sum_{e in chunk c} conj(V_i[e]) w[e],  i < nvec  (double accumulation)
-template <typename R>
+// part[i * n_chunks + c] = sum_{e in chunk c} conj(V_i[e]) w[e],  i < nvec  (double accumulation).
+// grid = (n_chunks, G): block (c, g) handles the basis vectors i = g, g + G, ...
+template <typename R, int EPT>
 __global__ void __launch_bounds__(TM_VT)
 k_dots(const Cx<R>* __restrict__ V, size_t stride, int nvec, const Cx<R>* __restrict__ w,
        const TmChunk* __restrict__ chunks, int n_chunks, double2* __restrict__ part, const int* __restrict__ n_active) {
   if (n_active != nullptr && *n_active == 0) return;
-  extern __shared__ double2 s_red[];                 // [nvec][TM_VT/32]
+  extern __shared__ double2 s_red[];                 // [ceil(nvec/G)][TM_VT/32]
   const TmChunk ch = chunks[blockIdx.x];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  Cx<R> wv[TM_CHUNK / TM_VT];
+  Cx<R> wv[EPT];
 #pragma unroll
-  for (int k = 0; k < TM_CHUNK / TM_VT; ++k) {
+  for (int k = 0; k < EPT; ++k) {
     const int e = threadIdx.x + k * TM_VT;
     wv[k] = e < ch.count ? w[(size_t)ch.start + e] : cx<R>(R(0), R(0));
   }
-  for (int i = 0; i < nvec; ++i) {
+  int slot = 0;
+  for (int i = blockIdx.y; i < nvec; i += gridDim.y, ++slot) {
     const Cx<R>* v = V + (size_t)i * stride + ch.start;
     double sr = 0.0, si = 0.0;
 #pragma unroll
-    for (int k = 0; k < TM_CHUNK / TM_VT; ++k) {
+    for (int k = 0; k < EPT; ++k) {
       const int e = threadIdx.x + k * TM_VT;
       if (e < ch.count) {
         const Cx<R> a = v[e];
@@ -115,14 +118,14 @@ k_dots(const Cx<R>* __restrict__ V, size_t stride, int nvec, const Cx<R>* __rest
       }
     }
     sr = warp_sum(sr); si = warp_sum(si);
-    if (lane == 0) s_red[i * (TM_VT / 32) + warp] = make_double2(sr, si);
+    if (lane == 0) s_red[slot * (TM_VT / 32) + warp] = make_double2(sr, si);
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < nvec; i += TM_VT) {
+  for (int t = threadIdx.x; t < slot; t += TM_VT) {
     double sr = 0.0, si = 0.0;
 #pragma unroll
-    for (int k = 0; k < TM_VT / 32; ++k) { sr += s_red[i * (TM_VT / 32) + k].x; si += s_red[i * (TM_VT / 32) + k].y; }
-    part[(size_t)i * n_chunks + blockIdx.x] = make_double2(sr, si);
+    for (int k = 0; k < TM_VT / 32; ++k) { sr += s_red[t * (TM_VT / 32) + k].x; si += s_red[t * (TM_VT / 32) + k].y; }
+    part[(size_t)(blockIdx.y + t * gridDim.y) * n_chunks + blockIdx.x] = make_double2(sr, si);
   }
 }
 
@@ -149,7 +152,7 @@ __global__ void k_reduce_h(const double2* __restrict__ part, int n_chunks, const
 
 // w += sign * sum_i coef[win][i] V_i ;  optionally normpart[c] = sum |w|^2 over the chunk (after the update).
 // `coef_off`: coefficient i of window win is coef[win * ldc + coef_off + i].
-template <typename R>
+template <typename R, int EPT>
 __global__ void __launch_bounds__(TM_VT)
 k_axpy(const Cx<R>* __restrict__ V, size_t stride, int nvec, const double2* __restrict__ coef, int ldc, double sign,
        Cx<R>* __restrict__ w, const TmChunk* __restrict__ chunks, double* __restrict__ normpart,
@@ -164,7 +167,7 @@ k_axpy(const Cx<R>* __restrict__ V, size_t stride, int nvec, const double2* __re
   __syncthreads();
   double nrm = 0.0;
 #pragma unroll
-  for (int k = 0; k < TM_CHUNK / TM_VT; ++k) {
+  for (int k = 0; k < EPT; ++k) {
     const int e = threadIdx.x + k * TM_VT;
     if (e < ch.count) {
       const size_t g = (size_t)ch.start + e;
