@@ -1,0 +1,93 @@
+"""Full-size parity (BASELINE.json sizes, in the launch configuration bench.py times): sampled outputs the oracle can
+compute one by one, and properties that hold at any size.  DESIGN.md section 6 / SURVEY.md 8(c) "full-size parity"."""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from oracle import driver, matvec as omv  # noqa: E402
+from paper_2107_09879_b200 import workloads as W  # noqa: E402
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+@pytest.fixture(scope="module")
+def tm():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2107_09879_b200 import libtm
+    libtm.lib()
+    return libtm
+
+
+def rel(a, b):
+    return np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(b)
+
+
+def rand_x(shape, seed):
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+
+
+def sampled_operator_rows(w, x, rows):
+    """Oracle rows of y = (I - T A) x for the sampled targets (diag or full T)."""
+    t, type_of, diag = driver.tmatrices(w)
+    u = omv.matvec_rows(w["lmax"], w["k"], w["pos"], x, rows=rows, win_ptr=w["win_ptr"])
+    if diag:
+        tu = t[type_of[rows]] * u
+    else:
+        tu = np.einsum("nab,nb->na", t[type_of[rows]], u)
+    return x[rows] - tu
+
+
+@pytest.mark.parametrize("cfg,prec,tol,n_rows", [(2, "fp64", 1e-12, 64), (3, "fp64", 1e-12, 16), (3, "fp32", 2e-5, 16),
+                                                 (4, "fp64", 1e-12, 24), (5, "fp64", 1e-12, 8)])
+def test_operator_rows_at_full_size(tm, cfg, prec, tol, n_rows):
+    w = W.config(cfg)
+    N, L = w["pos"].shape[0], W.n_modes(w["lmax"])
+    x = rand_x((N, L), 100 + cfg)
+    s = tm.solver_for_workload(w, precision=tm.TM_FP32 if prec == "fp32" else tm.TM_FP64)
+    assert s.get_kernel() == tm.TM_KERNEL_COPLANAR
+    y = s.matvec(x, 0)
+    rng = np.random.default_rng(200 + cfg)
+    rows = np.sort(rng.choice(N, n_rows, replace=False)).astype(np.int32)
+    rows[0], rows[-1] = 0, N - 1                          # first and last scatterer (tile / chunk edges)
+    ref = sampled_operator_rows(w, x, rows)
+    assert rel(y[rows], ref) <= tol
+    # transpose consistency at full size: z^T (M x) = (M^T z)^T x  (bilinear, no conjugation)
+    z = rand_x((N, L), 300 + cfg)
+    yt = s.matvec(z, 1)
+    lhs, rhs = np.sum(z * y), np.sum(yt * x)
+    assert abs(lhs - rhs) <= (1e-10 if prec == "fp64" else 1e-3) * abs(lhs)
+    s.close()
+
+
+def test_cfg2_full_solve_vs_dense_lu_golden(tm):
+    """Config 2 at full size: GPU GMRES(50) to 1e-10 against the oracle's dense LU (tests/golden/make_golden.py cfg2)."""
+    path = os.path.join(GOLD, "cfg2_solution.npy")
+    if not os.path.exists(path):
+        pytest.skip("golden file not generated (python tests/golden/make_golden.py cfg2)")
+    ref = np.load(path)
+    w = W.config(2)
+    s = tm.solver_for_workload(w)
+    sol, info, rc = s.solve(w["tol"], w["restart"], w["max_iter"])
+    assert rc == 0 and info[0].rel_residual <= w["tol"]
+    assert rel(sol, ref) <= 1e-9
+    s.close()
+
+
+def test_cfg4_windows_are_independent_at_full_size(tm):
+    """One 64x64 window solved alone vs. inside the 64-window batch: a few GMRES cycles give identical iterates."""
+    w = W.config(4)
+    lo, hi = int(w["win_ptr"][5]), int(w["win_ptr"][6])
+    s = tm.solver_for_workload(w)
+    sol, info, rc = s.solve(1e-3, 20, 20)
+    w1 = dict(w, pos=w["pos"][lo:hi], win_ptr=np.array([0, hi - lo], dtype=np.int32), radii=w["radii"][lo:hi],
+              type_of=np.arange(hi - lo, dtype=np.int32), focus=w["focus"][5:6])
+    s1 = tm.solver_for_workload(w1)
+    sol1, info1, rc1 = s1.solve(1e-3, 20, 20)
+    assert rel(sol1, sol[lo:hi]) <= 1e-10
+    assert info1[0].iterations == info[5].iterations
+    s.close(); s1.close()
