@@ -7,7 +7,7 @@ import pytest
 
 pytestmark = pytest.mark.gpu
 
-from oracle import driver, matvec as omv  # noqa: E402
+from oracle import matvec as omv  # noqa: E402
 from paper_2107_09879_b200 import workloads as W  # noqa: E402
 
 GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
@@ -32,13 +32,16 @@ def rand_x(shape, seed):
 
 
 def sampled_operator_rows(w, x, rows):
-    """Oracle rows of y = (I - T A) x for the sampled targets (diag or full T)."""
-    t, type_of, diag = driver.tmatrices(w)
+    """Oracle rows of y = (I - T A) x for the sampled targets (diag or full T); the oracle's T is evaluated for the
+    sampled scatterers only (per-site Mie for 2.6e5 sites through scipy would take hours)."""
+    from oracle import tmatrix
     u = omv.matvec_rows(w["lmax"], w["k"], w["pos"], x, rows=rows, win_ptr=w["win_ptr"])
-    if diag:
-        tu = t[type_of[rows]] * u
+    type_of = np.asarray(w["type_of"])
+    if w["t_kind"] in ("mie_types", "mie_sites"):
+        t_rows = np.stack([tmatrix.mie_tmatrix_diag(w["lmax"], w["k"], w["radii"][type_of[r]], w["eps_r"]) for r in rows])
+        tu = t_rows * u
     else:
-        tu = np.einsum("nab,nb->na", t[type_of[rows]], u)
+        tu = np.einsum("nab,nb->na", np.asarray(w["t_full"])[type_of[rows]], u)
     return x[rows] - tu
 
 
