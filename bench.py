@@ -200,7 +200,10 @@ def run_ours(args, w, rank, world, local_rank):
         def step_resident():
             set_inc(s)
             _, info, rc = s.solve(tol, w["restart"], max_iter, out=d_s)
-            _, info2, rc2 = s.solve_adjoint(d_w, tol, w["restart"], max_iter, out=d_lam)
+            if args.forward_only:
+                info2, rc2 = [libtm.SolveInfo(0, 0, 1, 0, 0.0, 0.0)], 0
+            else:
+                _, info2, rc2 = s.solve_adjoint(d_w, tol, w["restart"], max_iter, out=d_lam)
             s.fields(d_pts, d_s, libtm.TM_FIELD_E_SCA, out=d_E)
             return info, info2, rc, rc2
 
@@ -303,6 +306,7 @@ def run_ours(args, w, rank, world, local_rank):
             "config": {"workload": w["name"], "n_scat": N, "lmax": w["lmax"], "L": L, "n_windows": len(w["win_ptr"]) - 1,
                        "ordered_pairs": pairs, "tol": tol, "restart": w["restart"],
                        "step": ("one operator application y = (I - T A) x (matvec-only mode)" if args.mode == "matvec" else
+                                "incident + forward GMRES solve + E field (adjoint skipped: --forward-only)" if args.forward_only else
                                 "incident + forward GMRES solve + adjoint GMRES solve + E field on 64x64 detector points"),
                        "l2": "flushed between steps (256 MB write)",
                        "kernel": "coplanar" if kern == libtm.TM_KERNEL_COPLANAR else "general",
@@ -344,6 +348,7 @@ def main():
     ap.add_argument("--max-iter", type=int, default=None)
     ap.add_argument("--tol", type=float, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--forward-only", action="store_true", help="recorded big-config runs: skip the adjoint solve (not the contract step)")
     ap.add_argument("--profile", action="store_true", help="for ncu: 1 warm-up, no e2e leg, no CPU baseline (not a bench value)")
     args = ap.parse_args()
     if args.profile:
