@@ -184,79 +184,193 @@ def coplanar_rows(lmax):
     return K
 
 
+def coplanar_sym(lmax):
+    """The coplanar operator in the pair frame, reduced by BOTH mirror symmetries of a pair:
+      * z -> -z  (structural identity S2): modes split into the halves (-1)^{l+m+p} = +-1;
+      * y' -> -y' in the frame whose x' axis is the pair axis: K_q[(l',-m',p'),(l,-m,p)] = +-K_q[(l',m',p'),(l,m,p)]
+        (+ for p = p', - for p != p'), so in the basis x^+- = x'_{l,m,p} +- x'_{l,-m,p} (m > 0) each half splits
+        again into two sectors that do not couple.
+    Returns per half: slots [(l, am, p, kind)], kind in '0+-', and Knew[q][row_slot] = [(col_slot, value)]."""
+    md = modes(lmax)
+    L = len(md)
+    idx = {t: i for i, t in enumerate(md)}
+    rows = coplanar_rows(lmax)
+    nq = 2 * lmax + 1
+    Kd = [[[mp.mpf(0)] * L for _ in range(L)] for _ in range(nq)]
+    for b in range(L):
+        for q in range(nq):
+            for (a, v) in rows[b][q]:
+                Kd[q][b][a] += v
+    out = []
+    for h in (0, 1):
+        slots = []
+        for p in (0, 1):
+            for l in range(1, lmax + 1):
+                for am in range(0, l + 1):
+                    if (l + am + p) % 2 != h:
+                        continue
+                    if am == 0:
+                        slots.append((l, 0, p, "0"))
+                    else:
+                        slots.append((l, am, p, "+"))
+                        slots.append((l, am, p, "-"))
+        n = len(slots)
+        # S: new = S x' ; Sinv: x' = Sinv new
+        S = [[mp.mpf(0)] * L for _ in range(n)]
+        Sinv = [[mp.mpf(0)] * n for _ in range(L)]
+        for k, (l, am, p, kind) in enumerate(slots):
+            if kind == "0":
+                S[k][idx[(l, 0, p)]] = mp.mpf(1)
+                Sinv[idx[(l, 0, p)]][k] = mp.mpf(1)
+            else:
+                sg = 1 if kind == "+" else -1
+                S[k][idx[(l, am, p)]] = mp.mpf(1)
+                S[k][idx[(l, -am, p)]] = mp.mpf(sg)
+                Sinv[idx[(l, am, p)]][k] = mp.mpf(1) / 2
+                Sinv[idx[(l, -am, p)]][k] = mp.mpf(sg) / 2
+        Knew = []
+        for q in range(nq):
+            per_row = []
+            for r in range(n):
+                terms = []
+                for c in range(n):
+                    v = mp.mpf(0)
+                    for b in range(L):
+                        if S[r][b] == 0:
+                            continue
+                        for a in range(L):
+                            if Sinv[a][c] != 0 and Kd[q][b][a] != 0:
+                                v += S[r][b] * Kd[q][b][a] * Sinv[a][c]
+                    if abs(v) > mp.mpf(10) ** -30:
+                        terms.append((c, v))
+                per_row.append(terms)
+            Knew.append(per_row)
+        out.append((slots, Knew))
+    return out
+
+
 def emit_coplanar(lmaxes, path):
     with open(path, "w") as f:
         f.write("// GENERATED by gen_tables.py - do not edit.\n")
-        f.write("// Coplanar (theta = pi/2) translation apply, one mirror-parity half per call (DESIGN.md, kernel K2c).\n")
-        f.write("// xs: interleaved (re,im) tilde-basis source coefficients of this half; cm/sm: cos/sin(m phi);\n")
-        f.write("// hr/hi: Re/Im h_q^(1)(kr), q = 0..2 lmax; ar/ai: accumulators of this half.\n#pragma once\n\n")
-        cost = {lmax: [0, 0] for lmax in lmaxes}
+        f.write("// Coplanar (theta = pi/2) translation apply in the pair frame, one z-mirror-parity half per call, reduced by\n")
+        f.write("// the pair's y'-mirror symmetry (DESIGN.md, kernel K2c).  Basis of a half (\"slots\"): for every (l, |m|, p):\n")
+        f.write("// d^0 = x~_{l,0,p};  d^+- = x~_{l,m,p} +- x~_{l,-m,p}  (x~ = i^p x), staged by the kernel with the tables below.\n")
+        f.write("// xs: interleaved (re,im) d-values of this half; cm/sm: cos/sin(m phi); hr/hi: Re/Im h_q^(1)(kr);\n")
+        f.write("// ar/ai: accumulators A^0, A^+- = u~_{l,m,p} +- u~_{l,-m,p} of this half (unmixed once at the end).\n#pragma once\n\n")
         for lmax in lmaxes:
             md = modes(lmax)
-            K = coplanar_rows(lmax)
+            idx = {t: i for i, t in enumerate(md)}
+            sym = coplanar_sym(lmax)
+            cost = [0, 0]
             for h in (0, 1):
-                half = [i for i, (l, m, p) in enumerate(md) if (l + m + p) % 2 == h]
-                pos = {idx: k for k, idx in enumerate(half)}
-                nterm = 0
-                nrowq = 0
-                f.write(f"// lmax={lmax} half={h}: modes (flat idx) {half}\n")
+                slots, Knew = sym[h]
+                n = len(slots)
+                nq = 2 * lmax + 1
+                nterm = nrowq = 0
+                f.write(f"// lmax={lmax} half={h}: slots (l,|m|,p,kind) {[(l, am, p, k) for (l, am, p, k) in slots]}\n")
                 f.write("template <typename R>\n__device__ __forceinline__ void "
                         f"tm_cop_pair_L{lmax}_H{h}(const R* __restrict__ xs, const R* cm, const R* sm, const R* hr, const R* hi, R* ar, R* ai) {{\n")
-                for idx in half:
-                    l, m, p = md[idx]
-                    k = pos[idx]
-                    if m == 0:
+                # input phase rotation in the +- basis
+                k = 0
+                n_pairs = n_zero = 0
+                while k < n:
+                    l, am, p, kind = slots[k]
+                    if kind == "0":
                         f.write(f"  const R xr{k} = xs[{2 * k}], xi{k} = xs[{2 * k + 1}];\n")
-                    else:
-                        sg = "" if m > 0 else "-"
-                        am = abs(m)
-                        f.write(f"  const R xr{k} = xs[{2 * k}] * cm[{am}] - xs[{2 * k + 1}] * ({sg}sm[{am}]), "
-                                f"xi{k} = xs[{2 * k}] * ({sg}sm[{am}]) + xs[{2 * k + 1}] * cm[{am}];\n")
-                for idx in half:
-                    lp, mp_, pp = md[idx]
-                    kb = pos[idx]
-                    f.write("  {\n    R ur = R(0), ui = R(0), yr, yi;\n")
-                    for q in range(2 * lmax + 1):
-                        terms = K[idx][q]
+                        n_zero += 1
+                        k += 1
+                    else:       # slots k (+) and k+1 (-):  x^+ = c d^+ + i s d^- ,  x^- = c d^- + i s d^+
+                        kp, km = k, k + 1
+                        f.write(f"  const R xr{kp} = xs[{2 * kp}] * cm[{am}] - xs[{2 * km + 1}] * sm[{am}], "
+                                f"xi{kp} = xs[{2 * kp + 1}] * cm[{am}] + xs[{2 * km}] * sm[{am}];\n")
+                        f.write(f"  const R xr{km} = xs[{2 * km}] * cm[{am}] - xs[{2 * kp + 1}] * sm[{am}], "
+                                f"xi{km} = xs[{2 * km + 1}] * cm[{am}] + xs[{2 * kp}] * sm[{am}];\n")
+                        n_pairs += 1
+                        k += 2
+
+                def row_code(r):
+                    nonlocal nterm, nrowq
+                    f.write(f"    R ur{r} = R(0), ui{r} = R(0);\n")
+                    first_q = True
+                    for q in range(nq):
+                        terms = Knew[q][r]
                         if not terms:
                             continue
                         nrowq += 1
-                        for t, (a, v) in enumerate(terms):
-                            ka = pos[a]
+                        for t, (c, v) in enumerate(terms):
                             nterm += 1
                             if t == 0:
-                                f.write(f"    yr = R({lit(v)}) * xr{ka}; yi = R({lit(v)}) * xi{ka};\n")
+                                f.write(f"    yr = R({lit(v)}) * xr{c}; yi = R({lit(v)}) * xi{c};\n")
                             else:
-                                f.write(f"    yr = fma(R({lit(v)}), xr{ka}, yr); yi = fma(R({lit(v)}), xi{ka}, yi);\n")
-                        f.write(f"    ur = fma(hr[{q}], yr, ur); ur = fma(-hi[{q}], yi, ur); ui = fma(hr[{q}], yi, ui); ui = fma(hi[{q}], yr, ui);\n")
-                    if mp_ == 0:
-                        f.write(f"    ar[{kb}] += ur; ai[{kb}] += ui;\n")
-                    else:
-                        am = abs(mp_)
-                        sg = "-" if mp_ > 0 else ""      # e^{-i m_b phi}
-                        f.write(f"    ar[{kb}] = fma(ur, cm[{am}], ar[{kb}]); ar[{kb}] = fma(-ui, {sg}sm[{am}], ar[{kb}]);\n")
-                        f.write(f"    ai[{kb}] = fma(ur, {sg}sm[{am}], ai[{kb}]); ai[{kb}] = fma(ui, cm[{am}], ai[{kb}]);\n")
+                                f.write(f"    yr = fma(R({lit(v)}), xr{c}, yr); yi = fma(R({lit(v)}), xi{c}, yi);\n")
+                        if first_q:
+                            f.write(f"    ur{r} = hr[{q}] * yr; ur{r} = fma(-hi[{q}], yi, ur{r}); ui{r} = hr[{q}] * yi; ui{r} = fma(hi[{q}], yr, ui{r});\n")
+                            first_q = False
+                        else:
+                            f.write(f"    ur{r} = fma(hr[{q}], yr, ur{r}); ur{r} = fma(-hi[{q}], yi, ur{r}); ui{r} = fma(hr[{q}], yi, ui{r}); ui{r} = fma(hi[{q}], yr, ui{r});\n")
+
+                k = 0
+                while k < n:
+                    l, am, p, kind = slots[k]
+                    f.write("  {\n    R yr, yi;\n")
+                    if kind == "0":
+                        row_code(k)
+                        f.write(f"    ar[{k}] += ur{k}; ai[{k}] += ui{k};\n")
+                        k += 1
+                    else:       # A^+ += c u^+ - i s u^- ;  A^- += c u^- - i s u^+
+                        kp, km = k, k + 1
+                        row_code(kp)
+                        row_code(km)
+                        f.write(f"    ar[{kp}] = fma(ur{kp}, cm[{am}], ar[{kp}]); ar[{kp}] = fma(ui{km}, sm[{am}], ar[{kp}]);\n")
+                        f.write(f"    ai[{kp}] = fma(ui{kp}, cm[{am}], ai[{kp}]); ai[{kp}] = fma(-ur{km}, sm[{am}], ai[{kp}]);\n")
+                        f.write(f"    ar[{km}] = fma(ur{km}, cm[{am}], ar[{km}]); ar[{km}] = fma(ui{kp}, sm[{am}], ar[{km}]);\n")
+                        f.write(f"    ai[{km}] = fma(ui{km}, cm[{am}], ai[{km}]); ai[{km}] = fma(-ur{kp}, sm[{am}], ai[{km}]);\n")
+                        k += 2
                     f.write("  }\n")
                 f.write("}\n")
-                # executed floating-point work of this half per pair (generated code only; the ~70 geometry /
-                # Hankel instructions per thread are NOT counted, so rooflines built on this are conservative):
-                #   first term of a (row,q): 2 MUL; other terms: 2 FMA; per (row,q): 4 FMA;
-                #   output phase: 4 FMA (m != 0) or 2 ADD; input phase: 2 MUL + 2 FMA (m != 0)
-                n_m0 = sum(1 for idx in half if md[idx][1] == 0)
-                n_mx = len(half) - n_m0
-                inst = 2 * nrowq + 2 * (nterm - nrowq) + 4 * nrowq + 4 * n_mx + 2 * n_m0 + 4 * n_mx
-                flop = 2 * nrowq + 4 * (nterm - nrowq) + 8 * nrowq + 8 * n_mx + 2 * n_m0 + 6 * n_mx
-                cost[lmax][0] += inst
-                cost[lmax][1] += flop
-                print(f"lmax={lmax} half={h}: n={len(half)} coplanar terms={nterm} (row,q) combos={nrowq} "
+                # executed FP work per pair-half (generated code only; geometry/Hankel not counted):
+                #   first term of a (row,q): 2 MUL, other terms 2 FMA; per (row,q): 4 FMA (first q of a row: 2 MUL + 2 FMA);
+                #   input rotation per +- pair: 4 MUL + 4 FMA; output per pair: 8 FMA; m = 0 rows: 2 ADD
+                inst = 2 * nterm + 4 * nrowq + 8 * n_pairs + 8 * n_pairs + 2 * n_zero
+                flop = (2 * nrowq + 4 * (nterm - nrowq)) + (8 * nrowq - 2 * n) + (4 + 8) * n_pairs + 16 * n_pairs + 2 * n_zero
+                cost[0] += inst
+                cost[1] += flop
+                print(f"lmax={lmax} half={h}: n={n} sym terms={nterm} (row,q) combos={nrowq} "
                       f"-> {inst} FP instructions, {flop} flop per pair-half", file=sys.stderr)
-            # half membership tables for the hand-written kernel
-            for h in (0, 1):
-                half = [i for i, (l, m, p) in enumerate(md) if (l + m + p) % 2 == h]
-                f.write(f"__device__ __constant__ int tm_cop_half_L{lmax}_H{h}[{len(half)}] = {{{', '.join(map(str, half))}}};\n")
+                # staging tables: d_k = x~[sa] + ss * x~[sb]
+                sa, sb, ss = [], [], []
+                for (l, am, p, kind) in slots:
+                    sa.append(idx[(l, am, p)])
+                    sb.append(idx[(l, -am, p)])
+                    ss.append({"0": 0, "+": 1, "-": -1}[kind])
+                f.write(f"__device__ __constant__ int tm_cop_sa_L{lmax}_H{h}[{n}] = {{{', '.join(map(str, sa))}}};\n")
+                f.write(f"__device__ __constant__ int tm_cop_sb_L{lmax}_H{h}[{n}] = {{{', '.join(map(str, sb))}}};\n")
+                f.write(f"__device__ __constant__ int tm_cop_ss_L{lmax}_H{h}[{n}] = {{{', '.join(map(str, ss))}}};\n")
+                # unmix: u~_{l,+-m,p} = (A^+ +- A^-)/2, then u = (-i)^p u~
+                f.write("template <typename R, typename C>\n__device__ __forceinline__ void "
+                        f"tm_cop_unmix_L{lmax}_H{h}(const R* ar, const R* ai, C* out) {{\n")
+                half_l = len(md) // 2
+                k = 0
+                while k < n:
+                    l, am, p, kind = slots[k]
+
+                    def store(i_flat, re, im):
+                        if i_flat >= half_l:      # p = 1: multiply by -i
+                            f.write(f"  out[{i_flat}].re = {im}; out[{i_flat}].im = -({re});\n")
+                        else:
+                            f.write(f"  out[{i_flat}].re = {re}; out[{i_flat}].im = {im};\n")
+                    if kind == "0":
+                        store(idx[(l, 0, p)], f"ar[{k}]", f"ai[{k}]")
+                        k += 1
+                    else:
+                        kp, km = k, k + 1
+                        store(idx[(l, am, p)], f"R(0.5) * (ar[{kp}] + ar[{km}])", f"R(0.5) * (ai[{kp}] + ai[{km}])")
+                        store(idx[(l, -am, p)], f"R(0.5) * (ar[{kp}] - ar[{km}])", f"R(0.5) * (ai[{kp}] - ai[{km}])")
+                        k += 2
+                f.write("}\n")
             f.write(f"#define TM_COP_NH_L{lmax} {len(md) // 2}\n")
-            f.write(f"#define TM_COP_FPINST_L{lmax} {cost[lmax][0]}   // FP instructions per ordered pair (both halves)\n")
-            f.write(f"#define TM_COP_FLOP_L{lmax} {cost[lmax][1]}     // flop per ordered pair (FMA = 2)\n\n")
+            f.write(f"#define TM_COP_FPINST_L{lmax} {cost[0]}   // FP instructions per ordered pair (both halves)\n")
+            f.write(f"#define TM_COP_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")
 
 
 def main():

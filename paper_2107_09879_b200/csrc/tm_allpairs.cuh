@@ -46,6 +46,12 @@ template <typename R, int LMAX, int H> struct CopPair;
                                                const R* hi, R* ar, R* ai) {                              \
       tm_cop_pair_L##LM##_H##HH<R>(xs, cm, sm, hr, hi, ar, ai);                                          \
     }                                                                                                    \
+    static __device__ __forceinline__ void unmix(const R* ar, const R* ai, Cx<R>* out) {                 \
+      tm_cop_unmix_L##LM##_H##HH<R, Cx<R>>(ar, ai, out);                                                 \
+    }                                                                                                    \
+    static __device__ __forceinline__ void stage_entry(int k, int& a, int& b, int& sg) {                 \
+      a = tm_cop_sa_L##LM##_H##HH[k]; b = tm_cop_sb_L##LM##_H##HH[k]; sg = tm_cop_ss_L##LM##_H##HH[k];   \
+    }                                                                                                    \
   };
 TM_COP_SPEC(1, 0) TM_COP_SPEC(1, 1) TM_COP_SPEC(2, 0) TM_COP_SPEC(2, 1) TM_COP_SPEC(3, 0) TM_COP_SPEC(3, 1)
 #undef TM_COP_SPEC
@@ -60,11 +66,6 @@ TM_COP_SPEC(1, 0) TM_COP_SPEC(1, 1) TM_COP_SPEC(2, 0) TM_COP_SPEC(2, 1) TM_COP_S
 // SS sources at a time (positions + this half's coefficients in the tilde basis x~ = i^p x).
 // LOCKSTEP: a __syncthreads() per source keeps the block's warps on the same instructions (the two warps
 // that share an SM sub-partition then hit in its L0 instruction cache).
-template <int LMAX> __device__ __forceinline__ const int* cop_half_table(int half);
-template <> __device__ __forceinline__ const int* cop_half_table<1>(int half) { return half ? tm_cop_half_L1_H1 : tm_cop_half_L1_H0; }
-template <> __device__ __forceinline__ const int* cop_half_table<2>(int half) { return half ? tm_cop_half_L2_H1 : tm_cop_half_L2_H0; }
-template <> __device__ __forceinline__ const int* cop_half_table<3>(int half) { return half ? tm_cop_half_L3_H1 : tm_cop_half_L3_H0; }
-
 template <typename R, int LMAX, int TJ, int SS, bool LOCKSTEP>
 __global__ void __launch_bounds__(TJ)
 k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
@@ -77,7 +78,7 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
 
   __shared__ double s_px[SS], s_py[SS];
   __shared__ __align__(16) R s_x[SS * NH * 2];         // [source][NH] complex, tilde basis, this half only
-  __shared__ int s_half[NH];
+  __shared__ int s_sa[NH], s_sb[NH], s_ss[NH];       // staging: d_k = x~[sa] + ss * x~[sb]
 
   const TmTile tile = tiles[blockIdx.x];
   const int tid = threadIdx.x;
@@ -91,7 +92,11 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
   const int c0 = tile.src_start + blockIdx.y * per;
   const int c1 = min(tile.src_start + tile.src_count, c0 + per);
 
-  if (tid < NH) s_half[tid] = cop_half_table<LMAX>(half)[tid];
+  if (tid < NH) {
+    int a, b, sg;
+    if (half == 0) CopPair<R, LMAX, 0>::stage_entry(tid, a, b, sg); else CopPair<R, LMAX, 1>::stage_entry(tid, a, b, sg);
+    s_sa[tid] = a; s_sb[tid] = b; s_ss[tid] = sg;
+  }
 
   R ar[NH], ai[NH];
 #pragma unroll
@@ -99,13 +104,18 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
 
   for (int s0 = c0; s0 < c1; s0 += SS) {
     const int ns = min(SS, c1 - s0);
-    __syncthreads();                                   // previous stage fully consumed (also orders s_half)
+    __syncthreads();                                   // previous stage fully consumed (also orders the staging tables)
     for (int e = tid; e < ns; e += TJ) { s_px[e] = pos[3 * (s0 + e)]; s_py[e] = pos[3 * (s0 + e) + 1]; }
     for (int e = tid; e < ns * NH; e += TJ) {
       const int src = e / NH, kk = e - src * NH;
-      const int idx = s_half[kk];
-      Cx<R> v = x[(size_t)(s0 + src) * L + idx];
-      if (idx >= NH) v = cx<R>(-v.im, v.re);           // tilde basis: multiply p = 1 modes by i
+      const Cx<R>* xrow = x + (size_t)(s0 + src) * L;
+      const int ia = s_sa[kk], sg = s_ss[kk];
+      Cx<R> v = xrow[ia];
+      if (sg != 0) {                                   // d^+- = x_{l,m,p} +- x_{l,-m,p}  (pair's y'-mirror symmetry)
+        const Cx<R> o = xrow[s_sb[kk]];
+        v = sg > 0 ? cadd(v, o) : csub(v, o);
+      }
+      if (ia >= NH) v = cx<R>(-v.im, v.re);            // tilde basis: multiply p = 1 modes by i
       s_x[2 * e] = v.re;
       s_x[2 * e + 1] = v.im;
     }
@@ -136,14 +146,12 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
     }
   }
 
-  // this chunk's partial sums of this half, back in the standard basis: u_b = (-i)^{p_b} u~_b
+  // this chunk's partial sums of this half, back in the standard basis:
+  // u~_{l,+-m,p} = (A^+ +- A^-)/2,  u_b = (-i)^{p_b} u~_b
   if (live) {
     Cx<R>* out = u_part + ((size_t)blockIdx.y * n_scat + j) * L;
-#pragma unroll
-    for (int b = 0; b < NH; ++b) {
-      const int idx = s_half[b];
-      out[idx] = (idx >= NH) ? cx<R>(ai[b], -ar[b]) : cx<R>(ar[b], ai[b]);
-    }
+    if (half == 0) CopPair<R, LMAX, 0>::unmix(ar, ai, out);
+    else           CopPair<R, LMAX, 1>::unmix(ar, ai, out);
   }
 }
 

@@ -1,0 +1,61 @@
+"""CPU pins of the PRODUCT's build-time generated code against the oracle (no GPU needed):
+the straight-line coplanar pair code is compiled as host C++ (tests/hostcheck_coplanar.cpp) and the general-kernel
+term tables are evaluated with numpy; both must reproduce the oracle's translation block (PAPER.md Eqs. I16-I21)."""
+import os
+import re
+import subprocess
+
+import numpy as np
+import pytest
+
+from oracle import special as sp, translation as tr
+from oracle.modes import mode_list, n_modes
+from oracle.vswf import cart_to_sph
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+GEN = os.path.join(ROOT, "paper_2107_09879_b200", "csrc", "generated")
+K = 2 * np.pi
+
+
+@pytest.mark.parametrize("lmax", [1, 2, 3])
+def test_generated_coplanar_pair_code_matches_oracle_block(lmax, tmp_path):
+    exe = str(tmp_path / f"hostcheck{lmax}")
+    subprocess.check_call(["g++", "-O1", f"-DLMAX={lmax}", "-o", exe, os.path.join(ROOT, "tests", "hostcheck_coplanar.cpp")])
+    rng = np.random.default_rng(40 + lmax)
+    L = n_modes(lmax)
+    for d in ([0.5, 0.0], [0.0, -0.5], [-1.7, 2.9], rng.uniform(-40, 40, 2), rng.uniform(-3, 3, 2)):
+        x = rng.standard_normal(L) + 1j * rng.standard_normal(L)
+        inp = f"{float(d[0])!r} {float(d[1])!r}\n" + "\n".join(f"{float(z.real)!r} {float(z.imag)!r}" for z in x) + "\n"
+        out = subprocess.run([exe], input=inp, capture_output=True, text=True, check=True).stdout
+        u = np.array([complex(*map(float, ln.split())) for ln in out.strip().splitlines()])
+        ref = tr.block(lmax, K, np.array([d[0], d[1], 0.0]), np.zeros(3)) @ x
+        assert np.abs(u - ref).max() <= 2e-13 * np.abs(ref).max()
+
+
+def _parse_table(text, name, conv):
+    m = re.search(name + r"\[\d+\] = \{(.*?)\};", text, flags=re.S)
+    return [conv(t) for t in m.group(1).replace("\n", " ").split(",") if t.strip()]
+
+
+@pytest.mark.parametrize("lmax", [1, 2, 3, 4])
+def test_generated_general_term_table_matches_oracle_block(lmax):
+    text = open(os.path.join(GEN, "tm_tables_gen.h")).read()
+    tag = f"L{lmax}"
+    rp = _parse_table(text, f"tm_rowptr_{tag}", int)
+    col = _parse_table(text, f"tm_col_{tag}", int)
+    qq = _parse_table(text, f"tm_q_{tag}", int)
+    ip = _parse_table(text, f"tm_ipow_{tag}", int)
+    val = _parse_table(text, f"tm_val_{tag}", float)
+    modes = mode_list(lmax)
+    L = n_modes(lmax)
+    d = np.array([0.7, -1.3, 0.45])
+    r, th, ph = cart_to_sph(d)
+    h = [sp.sph_h1(q, K * r) for q in range(2 * lmax + 1)]
+    B = np.zeros((L, L), dtype=complex)
+    for b in range(L):
+        for t in range(rp[b], rp[b + 1]):
+            a = col[t]
+            mu = modes[a][1] - modes[b][1]
+            B[b, a] += (1j) ** ip[t] * val[t] * h[qq[t]] * sp.pbar(qq[t], abs(mu), np.cos(th)) * np.exp(1j * mu * ph)
+    ref = tr.block(lmax, K, d, np.zeros(3))
+    assert np.abs(B - ref).max() <= 1e-13 * np.abs(ref).max()
