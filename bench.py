@@ -305,13 +305,13 @@ def run_ours(args, w, rank, world, local_rank):
     if rank == 0:
         ap_avg_ms = ap_ms / max(1, ap_launches)
         achieved = pairs * flop / (ap_avg_ms * 1e-3) * 1e-12 if ap_launches else None
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+        traffic = None          # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
+        tpath = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
         if os.path.exists(tpath):
-            try:
-                traffic = json.load(open(tpath)).get(w["name"])
-            except Exception:
-                traffic = None
+            for ln in open(tpath).read().splitlines()[1:]:
+                f = ln.split(",")
+                if len(f) >= 3 and f[0] == w["name"]:
+                    traffic = float(f[2])
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": t_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
