@@ -188,7 +188,8 @@ def run_ours(args, w, rank, world, local_rank):
 
     with torch.cuda.stream(st):
         peak = libtm.measure_fma_peak(prec, st.cuda_stream)
-        s = libtm.solver_for_workload(w, precision=prec, stream=st.cuda_stream)
+        kern_req = {"auto": libtm.TM_KERNEL_AUTO, "general": libtm.TM_KERNEL_GENERAL, "coplanar": libtm.TM_KERNEL_COPLANAR}[args.kernel]
+        s = libtm.solver_for_workload(w, precision=prec, stream=st.cuda_stream, kernel=kern_req)
         ws = torch.empty(s.workspace_bytes(w["restart"]), dtype=torch.uint8, device="cuda")
         s.set_workspace(ws)
         d_w = torch.from_numpy(wadj).cuda()
@@ -338,7 +339,7 @@ def run_ours(args, w, rank, world, local_rank):
                          "avg_launch_ms": ap_avg_ms, "launches": int(ap_launches), "share_of_step": ap_ms / total_ms if total_ms else None,
                          "pipe_frac": (pairs * fpinst / (ap_avg_ms * 1e-3)) / (peak * 1e12 / 2) if ap_launches else None,
                          "pairs_per_s": pairs / (ap_avg_ms * 1e-3) if ap_launches else None, "traffic": traffic},
-            "clocks": clk,
+            "clocks": clk, "ms_steps": [round(v, 3) for v in ms_list],
         }
         if not args.no_cpu_baseline and world == 1:
             out["cpu_baseline"] = cpu_baseline(w)
@@ -356,6 +357,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--mode", default="full", choices=["full", "matvec"], help="matvec: time operator applications only")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "general", "coplanar"], help="force the all-pairs kernel variant")
     ap.add_argument("--scale", type=int, default=None, help="lattice side override (parity-size runs)")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
     ap.add_argument("--max-iter", type=int, default=None)

@@ -60,6 +60,7 @@ struct tm_ctx {
   void* d_upart = nullptr; size_t upart_bytes = 0;
   TmChunk* d_chunks = nullptr; int n_chunks = 0; int* d_win_chunk_ptr = nullptr;
   int ept = 4;                   // vector kernels: elements per thread (chunk = ept * TM_VT)
+  int max_chunks_per_win = 0;
 
   void* d_v[3] = {nullptr, nullptr, nullptr};   // Cx<R> work vectors [n]: X, B, Z
   double2* d_io = nullptr;                      // fp64 staging [n]
@@ -275,6 +276,7 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
   TM_CUDA(cudaEventCreate(&e0)); TM_CUDA(cudaEventCreate(&e1));
   TM_CUDA(cudaEventRecord(e0, st));
   TM_CUDA(cudaMemsetAsync(X, 0, n * sizeof(Cx<R>), st));
+  TM_CUDA(cudaMemsetAsync(V, 0, (size_t)(m + 2) * n * sizeof(Cx<R>), st));   // basis vectors must be finite (k_axpy)
 
   std::vector<int> h_k(nw), h_done(nw), iters(nw, 0), restarts(nw, 0);
   std::vector<double> h_res(nw, 0.0);
@@ -310,19 +312,21 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
       TM_CUDA(apply_operator<R>(ctx, transpose, Vj, W, Z, S.n_active));
       matvecs++;
       // split the basis vectors of a dot-product pass over gridDim.y when there are few chunks
-      const int G = std::max(1, std::min(j + 1, (148 * 4 + nc - 1) / nc));
-      const size_t sm_d = (size_t)((j + 1 + G - 1) / G) * (TM_VT / 32) * sizeof(double2);
+      const int G = std::max(1, std::min((j + 1 + 7) / 8, (148 * 4 + nc - 1) / nc));
       const size_t sm_a = (size_t)(j + 1) * sizeof(double2);
+      // small windows: the axpy blocks reduce the partial dots themselves (saves a launch per pass)
+      const bool fuse = ctx->max_chunks_per_win <= 512;
 #define TM_DOTS(H)                                                                                              \
   do {                                                                                                          \
-    if (ctx->ept == 1) k_dots<R, 1><<<dim3(nc, G), TM_VT, sm_d, st>>>(V, n, j + 1, W, ctx->d_chunks, nc, ctx->gm.part, S.n_active); \
-    else k_dots<R, 4><<<dim3(nc, G), TM_VT, sm_d, st>>>(V, n, j + 1, W, ctx->d_chunks, nc, ctx->gm.part, S.n_active); \
-    k_reduce_h<<<dim3(j + 1, nw), 64, 0, st>>>(ctx->gm.part, nc, ctx->d_win_chunk_ptr, H, S.ldh, 0, S.n_active); \
+    if (ctx->ept == 1) k_dots<R, 1><<<dim3(nc, G), TM_VT, 0, st>>>(V, n, j + 1, W, ctx->d_chunks, nc, ctx->gm.part, S.n_active); \
+    else k_dots<R, 4><<<dim3(nc, G), TM_VT, 0, st>>>(V, n, j + 1, W, ctx->d_chunks, nc, ctx->gm.part, S.n_active); \
+    if (!fuse) k_reduce_h<<<dim3(j + 1, nw), 64, 0, st>>>(ctx->gm.part, nc, ctx->d_win_chunk_ptr, H, S.ldh, 0, S.n_active); \
   } while (0)
 #define TM_AXPY(H, NP)                                                                                          \
   do {                                                                                                          \
-    if (ctx->ept == 1) k_axpy<R, 1><<<nc, TM_VT, sm_a, st>>>(V, n, j + 1, H, S.ldh, -1.0, W, ctx->d_chunks, NP, S.n_active); \
-    else k_axpy<R, 4><<<nc, TM_VT, sm_a, st>>>(V, n, j + 1, H, S.ldh, -1.0, W, ctx->d_chunks, NP, S.n_active);   \
+    const double2* pp = fuse ? ctx->gm.part : nullptr;                                                          \
+    if (ctx->ept == 1) k_axpy<R, 1><<<nc, TM_VT, sm_a, st>>>(V, n, j + 1, H, S.ldh, -1.0, W, ctx->d_chunks, NP, pp, nc, ctx->d_win_chunk_ptr, S.n_active); \
+    else k_axpy<R, 4><<<nc, TM_VT, sm_a, st>>>(V, n, j + 1, H, S.ldh, -1.0, W, ctx->d_chunks, NP, pp, nc, ctx->d_win_chunk_ptr, S.n_active); \
   } while (0)
       TM_DOTS(S.h1);
       TM_AXPY(S.h1, nullptr);
@@ -330,15 +334,15 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
       TM_AXPY(S.h2, ctx->gm.normpart);
 #undef TM_DOTS
 #undef TM_AXPY
-      k_reduce_norm<<<nw, 64, 0, st>>>(ctx->gm.normpart, ctx->d_win_chunk_ptr, S.normw);
-      k_gmres_givens<<<wb, 64, 0, st>>>(S, nw, j, o.tol);
+      k_gmres_givens<<<nw, 32, (size_t)(2 * j + 2) * sizeof(double2) + (size_t)(j + 1) * sizeof(double), st>>>(
+          S, nw, j, o.tol, ctx->gm.normpart, ctx->d_win_chunk_ptr);
       k_scale_or_sub<R><<<nc, TM_VT, 0, st>>>(W, nullptr, S.inv_norm, V + (size_t)(j + 1) * n, ctx->d_chunks, S.n_active);
-      ctx->total_launches += 9;
+      ctx->total_launches += fuse ? 6 : 8;
     }
     // x += V y ; r = b - M x
     k_gmres_solve_y<<<wb, 64, 0, st>>>(S, nw);
-    if (ctx->ept == 1) k_axpy<R, 1><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr);
-    else k_axpy<R, 4><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr);
+    if (ctx->ept == 1) k_axpy<R, 1><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr, nc, ctx->d_win_chunk_ptr, nullptr);
+    else k_axpy<R, 4><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr, nc, ctx->d_win_chunk_ptr, nullptr);
     TM_CUDA(apply_operator<R>(ctx, transpose, X, W, Z, nullptr));
     matvecs++;
     k_scale_or_sub<R><<<nc, TM_VT, 0, st>>>(B, W, nullptr, W, ctx->d_chunks, nullptr);      // W = b - M x
@@ -624,6 +628,7 @@ int tm_create(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const 
       const long long e0 = (long long)wp[w] * c->L, e1 = (long long)wp[w + 1] * c->L;
       for (long long s = e0; s < e1; s += chunk) ch.push_back(TmChunk{w, (int)s, (int)std::min<long long>(chunk, e1 - s)});
       wcp[w + 1] = (int)ch.size();
+      c->max_chunks_per_win = std::max(c->max_chunks_per_win, wcp[w + 1] - wcp[w]);
     }
     if (c->n > (size_t)0x7fffffff) { g_create_error = "problem too large (n_scat * L must fit in int32)"; tm_destroy(c); return TM_E_INVALID; }
     c->n_chunks = (int)ch.size();

@@ -44,28 +44,43 @@ __global__ void k_gmres_init_cycle(TmGmresDev S, int n_win, int first, double to
   if (!fin) atomicAdd(S.n_active, 1);
 }
 
-// After Arnoldi step j (0-based): column j of the Hessenberg is h1 + h2 (rows 0..j) and normw (row j+1).
-__global__ void k_gmres_givens(TmGmresDev S, int n_win, int j, double tol) {
-  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+// After Arnoldi step j (0-based): column j of the Hessenberg is h1 + h2 (rows 0..j) and ||w|| (row j+1).
+// One WARP per window (blockDim = 32, grid = n_win): the lanes first reduce the window's chunk norms (fixed order) and
+// stage the column and the previous rotations in shared memory with parallel loads; lane 0 then runs the sequential
+// rotation recurrence out of shared memory.
+__global__ void __launch_bounds__(32)
+k_gmres_givens(TmGmresDev S, int n_win, int j, double tol, const double* __restrict__ normpart,
+               const int* __restrict__ win_chunk_ptr) {
+  const int w = blockIdx.x, lane = threadIdx.x;
   if (w >= n_win) return;
   if (*S.n_active == 0 || S.done[w]) return;
+  extern __shared__ double2 s_col[];                  // [j+1] column, then [j] sn, then cs as doubles
+  double2* s_sn = s_col + (j + 1);
+  double* s_cs = reinterpret_cast<double*>(s_sn + j);
   const int ldh = S.ldh;
-  double2* col = S.Rm + ((size_t)w * S.m + j) * ldh;
+  double nn = 0.0;
+  for (int c = win_chunk_ptr[w] + lane; c < win_chunk_ptr[w + 1]; c += 32) nn += normpart[c];
+  nn = warp_sum(nn);
+  const double hn = sqrt(nn);
   const double2* a1 = S.h1 + (size_t)w * ldh;
   const double2* a2 = S.h2 + (size_t)w * ldh;
   double* cs = S.cs + (size_t)w * S.m;
   double2* sn = S.sn + (size_t)w * S.m;
+  for (int i = lane; i <= j; i += 32) s_col[i] = make_double2(a1[i].x + a2[i].x, a1[i].y + a2[i].y);
+  for (int i = lane; i < j; i += 32) { s_sn[i] = sn[i]; s_cs[i] = cs[i]; }
+  __syncwarp();
+  if (lane != 0) return;
+  double2* col = S.Rm + ((size_t)w * S.m + j) * ldh;
   double2* g = S.g + (size_t)w * ldh;
-  for (int i = 0; i <= j; ++i) col[i] = make_double2(a1[i].x + a2[i].x, a1[i].y + a2[i].y);
-  const double hn = S.normw[w];
+  S.normw[w] = hn;
   for (int i = 0; i < j; ++i) {            // previous rotations
-    const double2 a = col[i], b = col[i + 1];
-    const double2 sb = d2mul(sn[i], b);
-    const double2 sa = d2mul(d2conj(sn[i]), a);
-    col[i] = make_double2(cs[i] * a.x + sb.x, cs[i] * a.y + sb.y);
-    col[i + 1] = make_double2(cs[i] * b.x - sa.x, cs[i] * b.y - sa.y);
+    const double2 a = s_col[i], b = s_col[i + 1];
+    const double2 sb = d2mul(s_sn[i], b);
+    const double2 sa = d2mul(d2conj(s_sn[i]), a);
+    s_col[i] = make_double2(s_cs[i] * a.x + sb.x, s_cs[i] * a.y + sb.y);
+    s_col[i + 1] = make_double2(s_cs[i] * b.x - sa.x, s_cs[i] * b.y - sa.y);
   }
-  const double2 a = col[j];
+  const double2 a = s_col[j];
   const double aa = sqrt(a.x * a.x + a.y * a.y);
   const double den = sqrt(aa * aa + hn * hn);
   double c; double2 s, r;
@@ -77,7 +92,8 @@ __global__ void k_gmres_givens(TmGmresDev S, int n_win, int j, double tol) {
     s = make_double2(a.x * f, a.y * f);
     r = make_double2(a.x / aa * den, a.y / aa * den);
   }
-  cs[j] = c; sn[j] = s; col[j] = r;
+  cs[j] = c; sn[j] = s; s_col[j] = r;
+  for (int i = 0; i <= j; ++i) col[i] = s_col[i];
   const double2 gj = g[j];
   const double2 gn = d2mul(d2conj(s), gj);
   g[j + 1] = make_double2(-gn.x, -gn.y);

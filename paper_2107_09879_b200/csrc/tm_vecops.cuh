@@ -89,43 +89,37 @@ k_tapply(int mode, int L, int n_scat, int n_chunk, const Cx<R>* __restrict__ x, 
 
 // ------------------------------------------------------------------------------------------------ GMRES pieces
 // part[i * n_chunks + c] = sum_{e in chunk c} conj(V_i[e]) w[e],  i < nvec  (double accumulation).
-// grid = (n_chunks, G): block (c, g) handles the basis vectors i = g, g + G, ...
+// grid = (n_chunks, G): block (c, g) handles the basis vectors i = g, g + G, ...; inside the block the chunk of w is
+// staged in shared memory and every WARP takes whole vectors (lanes stride over the chunk, one shuffle reduction per
+// vector instead of one per vector and warp).
 template <typename R, int EPT>
 __global__ void __launch_bounds__(TM_VT)
 k_dots(const Cx<R>* __restrict__ V, size_t stride, int nvec, const Cx<R>* __restrict__ w,
        const TmChunk* __restrict__ chunks, int n_chunks, double2* __restrict__ part, const int* __restrict__ n_active) {
   if (n_active != nullptr && *n_active == 0) return;
-  extern __shared__ double2 s_red[];                 // [ceil(nvec/G)][TM_VT/32]
+  __shared__ Cx<R> s_w[EPT * TM_VT];
   const TmChunk ch = chunks[blockIdx.x];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  Cx<R> wv[EPT];
 #pragma unroll
   for (int k = 0; k < EPT; ++k) {
     const int e = threadIdx.x + k * TM_VT;
-    wv[k] = e < ch.count ? w[(size_t)ch.start + e] : cx<R>(R(0), R(0));
+    s_w[e] = e < ch.count ? w[(size_t)ch.start + e] : cx<R>(R(0), R(0));
   }
-  int slot = 0;
-  for (int i = blockIdx.y; i < nvec; i += gridDim.y, ++slot) {
+  __syncthreads();
+  for (int i = blockIdx.y + warp * gridDim.y; i < nvec; i += gridDim.y * (TM_VT / 32)) {
     const Cx<R>* v = V + (size_t)i * stride + ch.start;
     double sr = 0.0, si = 0.0;
 #pragma unroll
-    for (int k = 0; k < EPT; ++k) {
-      const int e = threadIdx.x + k * TM_VT;
+    for (int k = 0; k < EPT * TM_VT / 32; ++k) {
+      const int e = lane + 32 * k;
       if (e < ch.count) {
-        const Cx<R> a = v[e];
-        sr += (double)a.re * (double)wv[k].re + (double)a.im * (double)wv[k].im;
-        si += (double)a.re * (double)wv[k].im - (double)a.im * (double)wv[k].re;
+        const Cx<R> a = v[e], b = s_w[e];
+        sr += (double)a.re * (double)b.re + (double)a.im * (double)b.im;
+        si += (double)a.re * (double)b.im - (double)a.im * (double)b.re;
       }
     }
     sr = warp_sum(sr); si = warp_sum(si);
-    if (lane == 0) s_red[slot * (TM_VT / 32) + warp] = make_double2(sr, si);
-  }
-  __syncthreads();
-  for (int t = threadIdx.x; t < slot; t += TM_VT) {
-    double sr = 0.0, si = 0.0;
-#pragma unroll
-    for (int k = 0; k < TM_VT / 32; ++k) { sr += s_red[t * (TM_VT / 32) + k].x; si += s_red[t * (TM_VT / 32) + k].y; }
-    part[(size_t)(blockIdx.y + t * gridDim.y) * n_chunks + blockIdx.x] = make_double2(sr, si);
+    if (lane == 0) part[(size_t)i * n_chunks + blockIdx.x] = make_double2(sr, si);
   }
 }
 
@@ -150,19 +144,46 @@ __global__ void k_reduce_h(const double2* __restrict__ part, int n_chunks, const
   }
 }
 
-// w += sign * sum_i coef[win][i] V_i ;  optionally normpart[c] = sum |w|^2 over the chunk (after the update).
-// `coef_off`: coefficient i of window win is coef[win * ldc + coef_off + i].
+// w += sign * sum_i coef_i V_i ;  optionally normpart[c] = sum |w|^2 over the chunk (after the update).
+// The coefficients of window `win` are either given (coef[win * ldc + i]) or, when `part` != nullptr, reduced here from
+// the per-chunk partial dot products of k_dots (coef_i = sum over the window's chunks of part[i][c], fixed order ->
+// deterministic); the block owning the window's first chunk then also stores them to coef for the Givens kernel.
+// Basis vectors must hold finite numbers (the workspace is zeroed at the start of a solve): a zero coefficient
+// multiplies whatever is there.
 template <typename R, int EPT>
 __global__ void __launch_bounds__(TM_VT)
-k_axpy(const Cx<R>* __restrict__ V, size_t stride, int nvec, const double2* __restrict__ coef, int ldc, double sign,
+k_axpy(const Cx<R>* __restrict__ V, size_t stride, int nvec, double2* __restrict__ coef, int ldc, double sign,
        Cx<R>* __restrict__ w, const TmChunk* __restrict__ chunks, double* __restrict__ normpart,
+       const double2* __restrict__ part, int n_chunks, const int* __restrict__ win_chunk_ptr,
        const int* __restrict__ n_active) {
   if (n_active != nullptr && *n_active == 0) return;
-  extern __shared__ double2 s_c[];                   // [nvec] then reduction scratch
+  extern __shared__ double2 s_c[];                   // [nvec]
   const TmChunk ch = chunks[blockIdx.x];
-  for (int i = threadIdx.x; i < nvec; i += TM_VT) {
-    const double2 c = coef[(size_t)ch.win * ldc + i];
-    s_c[i] = make_double2(sign * c.x, sign * c.y);
+  if (part != nullptr) {
+    const int c0 = win_chunk_ptr[ch.win], c1 = win_chunk_ptr[ch.win + 1];
+    // 4 lanes per vector, each sums a contiguous quarter of the chunk list; lanes combined in fixed order
+    for (int base = 0; base < nvec; base += TM_VT / 4) {
+      const int i = base + (threadIdx.x >> 2), q = threadIdx.x & 3;
+      double sr = 0.0, si = 0.0;
+      if (i < nvec) {
+        const int len = (c1 - c0 + 3) / 4;
+        const int lo = c0 + q * len, hi = min(c1, lo + len);
+        const double2* p = part + (size_t)i * n_chunks;
+#pragma unroll 4
+        for (int c = lo; c < hi; ++c) { sr += p[c].x; si += p[c].y; }
+      }
+      sr += __shfl_xor_sync(0xffffffffu, sr, 1); si += __shfl_xor_sync(0xffffffffu, si, 1);
+      sr += __shfl_xor_sync(0xffffffffu, sr, 2); si += __shfl_xor_sync(0xffffffffu, si, 2);
+      if (i < nvec && q == 0) {
+        s_c[i] = make_double2(sign * sr, sign * si);
+        if (blockIdx.x == c0) coef[(size_t)ch.win * ldc + i] = make_double2(sr, si);
+      }
+    }
+  } else {
+    for (int i = threadIdx.x; i < nvec; i += TM_VT) {
+      const double2 c = coef[(size_t)ch.win * ldc + i];
+      s_c[i] = make_double2(sign * c.x, sign * c.y);
+    }
   }
   __syncthreads();
   double nrm = 0.0;
@@ -172,9 +193,9 @@ k_axpy(const Cx<R>* __restrict__ V, size_t stride, int nvec, const double2* __re
     if (e < ch.count) {
       const size_t g = (size_t)ch.start + e;
       double ar = (double)w[g].re, ai = (double)w[g].im;
+#pragma unroll 8
       for (int i = 0; i < nvec; ++i) {
         const double2 c = s_c[i];
-        if (c.x == 0.0 && c.y == 0.0) continue;      // block-uniform; also keeps never-written basis vectors out
         const Cx<R> v = V[(size_t)i * stride + g];
         ar += c.x * (double)v.re - c.y * (double)v.im;
         ai += c.x * (double)v.im + c.y * (double)v.re;
