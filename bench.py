@@ -188,7 +188,8 @@ def run_ours(args, w, rank, world, local_rank):
 
     with torch.cuda.stream(st):
         peak = libtm.measure_fma_peak(prec, st.cuda_stream)
-        kern_req = {"auto": libtm.TM_KERNEL_AUTO, "general": libtm.TM_KERNEL_GENERAL, "coplanar": libtm.TM_KERNEL_COPLANAR}[args.kernel]
+        kern_req = {"auto": libtm.TM_KERNEL_AUTO, "general": libtm.TM_KERNEL_GENERAL, "coplanar": libtm.TM_KERNEL_COPLANAR,
+                    "sym3d": libtm.TM_KERNEL_SYM3D}[args.kernel]
         s = libtm.solver_for_workload(w, precision=prec, stream=st.cuda_stream, kernel=kern_req)
         ws = torch.empty(s.workspace_bytes(w["restart"]), dtype=torch.uint8, device="cuda")
         s.set_workspace(ws)
@@ -323,7 +324,7 @@ def run_ours(args, w, rank, world, local_rank):
                                 "incident + forward GMRES solve + E field (adjoint skipped: --forward-only)" if args.forward_only else
                                 "incident + forward GMRES solve + adjoint GMRES solve + E field on 64x64 detector points"),
                        "l2": "flushed between steps (256 MB write)",
-                       "kernel": "coplanar" if kern == libtm.TM_KERNEL_COPLANAR else "general",
+                       "kernel": {libtm.TM_KERNEL_COPLANAR: "coplanar", libtm.TM_KERNEL_SYM3D: "sym3d"}.get(kern, "general"),
                        "parallelism": "replicas" if world > 1 else "single"},
             "solve": {"forward_iterations": max(i.iterations for i in info), "adjoint_iterations": max(i.iterations for i in info2),
                       "forward_rel_residual": max(i.rel_residual for i in info), "adjoint_rel_residual": max(i.rel_residual for i in info2),
@@ -332,7 +333,7 @@ def run_ours(args, w, rank, world, local_rank):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": t_e2e, "steps": e2e_steps},
             "gpu_launches": int(tot_launches),
-            "roofline": {"bound": "alu", "kernel": "k_allpairs_coplanar" if kern == libtm.TM_KERNEL_COPLANAR else "k_allpairs_general",
+            "roofline": {"bound": "alu", "kernel": {libtm.TM_KERNEL_COPLANAR: "k_allpairs_coplanar", libtm.TM_KERNEL_SYM3D: "k_allpairs_sym3d"}.get(kern, "k_allpairs_general"),
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": (achieved / peak) if achieved else None,
                          "peak_source": "measured live: tm_measure_fma_peak (register-resident FMA chains, this GPU, this run)",
                          "flop_per_pair": flop, "fp_instr_per_pair": fpinst, "pairs_per_launch": pairs,
@@ -357,7 +358,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--mode", default="full", choices=["full", "matvec"], help="matvec: time operator applications only")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "general", "coplanar"], help="force the all-pairs kernel variant")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "general", "coplanar", "sym3d"], help="force the all-pairs kernel variant")
     ap.add_argument("--scale", type=int, default=None, help="lattice side override (parity-size runs)")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
     ap.add_argument("--max-iter", type=int, default=None)

@@ -39,7 +39,7 @@ enum { TM_OK = 0, TM_NOT_CONVERGED = 1,
        TM_E_INVALID = -1, TM_E_OVERLAP = -2, TM_E_STATE = -3, TM_E_CUDA = -4, TM_E_NOMEM = -5 };
 enum { TM_INC_PLANE = 0, TM_INC_GAUSS = 1, TM_INC_COEFFS = 2 };
 enum { TM_FIELD_E_SCA = 0, TM_FIELD_H_SCA = 1 };           /* H is returned as Z_b * H (reading R10) */
-enum { TM_KERNEL_AUTO = 0, TM_KERNEL_GENERAL = 1, TM_KERNEL_COPLANAR = 2 };
+enum { TM_KERNEL_AUTO = 0, TM_KERNEL_GENERAL = 1, TM_KERNEL_COPLANAR = 2, TM_KERNEL_SYM3D = 3 };
 
 /* Plane wave travelling along (beta = polar angle from +z, alpha = azimuth) with amplitude
  * A = A_beta * beta_hat + A_alpha * alpha_hat  (Eqs. II6-II7).
@@ -75,7 +75,7 @@ typedef struct {
  *   win_ptr   HOST pointer [n_win+1], monotone, win_ptr[0] = 0, win_ptr[n_win] = n_scat; NULL (with
  *             n_win = 1) => one window.  Scatterers interact only inside their window (reading R16;
  *             independent Nyquist windows batched on one GPU).
- *   lmax      1..6 (coplanar fast kernel for lmax <= 3 when all z are equal; general 3-D kernel otherwise)
+ *   lmax      1..6 (generated kernels for lmax <= 3: coplanar when all z are equal, else 3-D; table-driven kernel above)
  *   k_b       background wavenumber (wavelength 1 => 2 pi)
  *   precision TM_FP64 or TM_FP32 (API data stays fp64)
  *   cuda_stream  a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) or NULL for the default stream
@@ -125,10 +125,13 @@ int tm_fields(tm_ctx *ctx, int n_pts, const double *pts, const tm_c64 *s, int wh
 size_t tm_workspace_bytes(const tm_ctx *ctx, const tm_solve_opts *opts);
 int tm_set_workspace(tm_ctx *ctx, void *dev_ptr, size_t bytes);
 
-/* Force the all-pairs kernel variant (TM_KERNEL_*).  COPLANAR is refused (TM_E_INVALID) unless all z are
- * equal and lmax <= 3.  Default AUTO. */
+/* Force the all-pairs kernel variant (TM_KERNEL_*):
+ *   COPLANAR  generated code, all z equal and lmax <= 3 (refused with TM_E_INVALID otherwise)
+ *   SYM3D     generated code, arbitrary 3-D positions, lmax <= 3 (refused otherwise)
+ *   GENERAL   table-driven, arbitrary positions, lmax <= 6
+ * Default AUTO = COPLANAR if applicable, else SYM3D if lmax <= 3, else GENERAL. */
 int tm_set_kernel(tm_ctx *ctx, int kernel);
-/* Which variant AUTO resolved to (TM_KERNEL_GENERAL or TM_KERNEL_COPLANAR). */
+/* Which variant is active (TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR or TM_KERNEL_SYM3D). */
 int tm_get_kernel(const tm_ctx *ctx);
 
 /* Device time (ms, CUDA events on the context's stream) of the all-pairs kernel launches since the last

@@ -373,10 +373,190 @@ def emit_coplanar(lmaxes, path):
             f.write(f"#define TM_COP_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")
 
 
+# ----------------------------------------------------------------------------- general 3-D, symmetric-basis code
+def general_sym(lmax):
+    """3-D operator in the frame rotated about z so that the pair lies in the x'z plane (phi = 0):
+         u'_b = sum_a sum_q c~_q(b,a) h_q(kr) Pbar_q^{|m_a-m_b|}(cos theta) x'_a      (c~ real in the tilde basis)
+    The pair lies in the mirror plane y' = 0, so c~_q((l',-m',p'),(l,-m,p)) = +-c~_q((l',m',p'),(l,m,p)) and the +- basis
+    of coplanar_sym splits the L modes into two uncoupled SECTORS of L/2:
+         sector 0 = {p=0: '0','+'; p=1: '-'},   sector 1 = {p=0: '-'; p=1: '0','+'}.
+    Returns per sector: slots [(l, am, p, kind)] and rows[r][q] = [(c, [(mu, kappa)])]:
+         u^new_r = sum_q h_q sum_c ( sum_mu kappa Pbar_q^mu ) x^new_c ."""
+    md = modes(lmax)
+    idx = {t: i for i, t in enumerate(md)}
+    nq = 2 * lmax + 1
+    C = {}
+    for (b, a, q, ip, v) in general_terms(lmax):
+        (lp, mp_, pp), (l, m, p) = md[b], md[a]
+        tot = (ip + (pp - p)) % 4
+        assert tot % 2 == 0
+        C[(b, a, q)] = v if tot == 0 else -v
+    sectors = [[], []]
+    for p in (0, 1):
+        for l in range(1, lmax + 1):
+            for am in range(0, l + 1):
+                for kind in (["0"] if am == 0 else ["+", "-"]):
+                    in0 = (p == 0 and kind in "0+") or (p == 1 and kind == "-")
+                    sectors[0 if in0 else 1].append((l, am, p, kind))
+    out = []
+    for sec in sectors:
+        n = len(sec)
+        rows = [[[] for _ in range(nq)] for _ in range(n)]
+        for r, (lr, mr, pr, kr) in enumerate(sec):
+            rws = [(idx[(lr, mr, pr)], 1)] if kr == "0" else [(idx[(lr, mr, pr)], 1), (idx[(lr, -mr, pr)], 1 if kr == "+" else -1)]
+            for c, (lc, mc, pc, kc) in enumerate(sec):
+                cls = ([(idx[(lc, mc, pc)], mp.mpf(1))] if kc == "0" else
+                       [(idx[(lc, mc, pc)], mp.mpf(1) / 2), (idx[(lc, -mc, pc)], (mp.mpf(1) if kc == "+" else -mp.mpf(1)) / 2)])
+                acc = {}
+                for (b, sb) in rws:
+                    for (a, sa) in cls:
+                        mu = abs(md[a][1] - md[b][1])
+                        for q in range(nq):
+                            if (b, a, q) in C:
+                                acc[(q, mu)] = acc.get((q, mu), mp.mpf(0)) + sb * sa * C[(b, a, q)]
+                for q in range(nq):
+                    lst = [(mu, v) for (qq, mu), v in sorted(acc.items()) if qq == q and abs(v) > mp.mpf(10) ** -30]
+                    if lst:
+                        rows[r][q].append((c, lst))
+        # the other sector must not couple (checked through the full matrix): every (b,a,q) term is consumed above
+        out.append((sec, rows))
+    return out
+
+
+def emit_general_sym(lmaxes, path):
+    with open(path, "w") as f:
+        f.write("// GENERATED by gen_tables.py - do not edit.\n")
+        f.write("// General 3-D translation apply in the frame rotated about z onto the pair's azimuth, one y'-mirror SECTOR per call\n")
+        f.write("// (DESIGN.md, kernel K2s).  Slots as in tm_coplanar_gen.cuh; P[q(q+1)/2+mu] = Pbar_q^mu(cos theta).\n#pragma once\n\n")
+        for lmax in lmaxes:
+            md = modes(lmax)
+            idx = {t: i for i, t in enumerate(md)}
+            nq = 2 * lmax + 1
+            # normalised Legendre functions Pbar_q^mu(ct), st = sin(theta) >= 0, no Condon-Shortley phase (R2)
+            f.write(f"template <typename R>\n__device__ __forceinline__ void tm_pbar_all_L{lmax}(R ct, R st, R* P) {{\n")
+            pi = lambda q, mu: q * (q + 1) // 2 + mu
+            f.write(f"  P[0] = R({lit(mp.sqrt(mp.mpf(1) / 2))});\n")
+            for mu in range(0, nq):
+                if mu > 0:
+                    f.write(f"  P[{pi(mu, mu)}] = R({lit(mp.sqrt(mp.mpf(2 * mu + 1) / (2 * mu)))}) * st * P[{pi(mu - 1, mu - 1)}];\n")
+                if mu + 1 < nq:
+                    f.write(f"  P[{pi(mu + 1, mu)}] = R({lit(mp.sqrt(mp.mpf(2 * mu + 3)))}) * ct * P[{pi(mu, mu)}];\n")
+                for q in range(mu + 2, nq):
+                    a_ = mp.sqrt(mp.mpf(4 * q * q - 1) / (q * q - mu * mu))
+                    b_ = mp.sqrt(mp.mpf((q - 1) ** 2 - mu * mu) / (4 * (q - 1) ** 2 - 1))
+                    f.write(f"  P[{pi(q, mu)}] = R({lit(a_)}) * (ct * P[{pi(q - 1, mu)}] - R({lit(b_)}) * P[{pi(q - 2, mu)}]);\n")
+            f.write("}\n")
+            cost = [0, 0]
+            for sct, (slots, rows) in enumerate(general_sym(lmax)):
+                n = len(slots)
+                f.write(f"// lmax={lmax} sector={sct}: slots (l,|m|,p,kind) {slots}\n")
+                f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
+                        f"tm_g3d_pair_L{lmax}_S{sct}(const R* __restrict__ xs, const R* cm, const R* sm, const R* hr, const R* hi, const R* P, R* ar, R* ai) {{\n")
+                k = 0
+                n_pairs = n_zero = 0
+                while k < n:
+                    l, am, p, kind = slots[k]
+                    if kind == "0":
+                        f.write(f"  const R xr{k} = xs[{2 * k}], xi{k} = xs[{2 * k + 1}];\n")
+                        n_zero += 1
+                        k += 1
+                    else:
+                        # '+' and '-' partners of a (l,am,p) pair live in DIFFERENT sectors here: the rotation needs d^+ and d^-
+                        # of the same (l,am,p), so the kernel stages both (slot k: this sector's, slot n + k: the partner's)
+                        f.write(f"  const R xr{k} = xs[{2 * k}] * cm[{am}] - xs[{2 * (n + k) + 1}] * sm[{am}], "
+                                f"xi{k} = xs[{2 * k + 1}] * cm[{am}] + xs[{2 * (n + k)}] * sm[{am}];\n")
+                        n_pairs += 1
+                        k += 1
+                nterm = nrc = nrowq = 0
+                for r in range(n):
+                    l, am, p, kind = slots[r]
+                    f.write("  {\n    R ur = R(0), ui = R(0), zr, zi, rho;\n")
+                    first_q = True
+                    for q in range(nq):
+                        ent = rows[r][q]
+                        if not ent:
+                            continue
+                        nrowq += 1
+                        for t, (c, lst) in enumerate(ent):
+                            nrc += 1
+                            expr = None
+                            for (mu, v) in lst:
+                                nterm += 1
+                                if expr is None:
+                                    expr = f"R({lit(v)}) * P[{q * (q + 1) // 2 + mu}]"
+                                else:
+                                    expr = f"fma(R({lit(v)}), P[{q * (q + 1) // 2 + mu}], {expr})"
+                            f.write(f"    rho = {expr};\n")
+                            if t == 0:
+                                f.write(f"    zr = rho * xr{c}; zi = rho * xi{c};\n")
+                            else:
+                                f.write(f"    zr = fma(rho, xr{c}, zr); zi = fma(rho, xi{c}, zi);\n")
+                        if first_q:
+                            f.write(f"    ur = hr[{q}] * zr; ur = fma(-hi[{q}], zi, ur); ui = hr[{q}] * zi; ui = fma(hi[{q}], zr, ui);\n")
+                            first_q = False
+                        else:
+                            f.write(f"    ur = fma(hr[{q}], zr, ur); ur = fma(-hi[{q}], zi, ur); ui = fma(hr[{q}], zi, ui); ui = fma(hi[{q}], zr, ui);\n")
+                    # output: this sector's u^new_r feeds A^same (cos) and the PARTNER sector's accumulator (sin):
+                    #   A^+ += c u^+ - i s u^- ;  A^- += c u^- - i s u^+   -> ar/ai hold [own n slots | partner n slots]
+                    if kind == "0":
+                        f.write(f"    ar[{r} * AS] += ur; ai[{r} * AS] += ui;\n")
+                    else:
+                        f.write(f"    ar[{r} * AS] = fma(ur, cm[{am}], ar[{r} * AS]); ai[{r} * AS] = fma(ui, cm[{am}], ai[{r} * AS]);\n")
+                        f.write(f"    ar[{n + r} * AS] = fma(ui, sm[{am}], ar[{n + r} * AS]); ai[{n + r} * AS] = fma(-ur, sm[{am}], ai[{n + r} * AS]);\n")
+                    f.write("  }\n")
+                f.write("}\n")
+                inst = nterm + 2 * nrc + 4 * nrowq + 4 * n_pairs + 4 * n_pairs + 2 * n_zero
+                flop = (2 * nterm - nrc) + (4 * nrc - 2 * nrowq) + (8 * nrowq - 2 * n) + 6 * n_pairs + 8 * n_pairs + 2 * n_zero
+                cost[0] += inst
+                cost[1] += flop
+                print(f"lmax={lmax} sector={sct}: n={n} terms={nterm} (row,col,q)={nrc} (row,q)={nrowq} -> {inst} FP instructions, {flop} flop",
+                      file=sys.stderr)
+                # staging tables for this sector: own slots then partner slots (kind flipped; '0' has no partner -> itself, unused)
+                sa, sb, ss = [], [], []
+                for (l, am, p, kind) in slots:
+                    sa.append(idx[(l, am, p)]); sb.append(idx[(l, -am, p)]); ss.append({"0": 0, "+": 1, "-": -1}[kind])
+                for (l, am, p, kind) in slots:
+                    sa.append(idx[(l, am, p)]); sb.append(idx[(l, -am, p)]); ss.append({"0": 0, "+": -1, "-": 1}[kind])
+                f.write(f"__device__ __constant__ int tm_g3d_sa_L{lmax}_S{sct}[{2 * n}] = {{{', '.join(map(str, sa))}}};\n")
+                f.write(f"__device__ __constant__ int tm_g3d_sb_L{lmax}_S{sct}[{2 * n}] = {{{', '.join(map(str, sb))}}};\n")
+                f.write(f"__device__ __constant__ int tm_g3d_ss_L{lmax}_S{sct}[{2 * n}] = {{{', '.join(map(str, ss))}}};\n")
+                # Each block (one sector) produces, for every (l,am,p) of its slots, a contribution to A^own (slot r) and to
+                # A^partner (slot n + r).  u~_{l,+-m,p} = (A^+ +- A^-)/2 needs both sectors' contributions, so each sector
+                # writes its share of u~ into its own partial buffer (the finishing kernel adds the two):
+                #   own kind '+': A^+ part = ar[r], A^- part = ar[n+r]  ->  u~_{+m} += (ar[r] + ar[n+r])/2, u~_{-m} += (ar[r] - ar[n+r])/2
+                #   own kind '-': A^- part = ar[r], A^+ part = ar[n+r]  ->  u~_{+m} += (ar[n+r] + ar[r])/2, u~_{-m} += (ar[n+r] - ar[r])/2
+                f.write("template <typename R, typename C, int AS>\n__device__ __forceinline__ void "
+                        f"tm_g3d_unmix_L{lmax}_S{sct}(const R* ar, const R* ai, C* out) {{\n")
+                half_l = len(md) // 2
+                for r, (l, am, p, kind) in enumerate(slots):
+                    def store(i_flat, re, im):
+                        if i_flat >= half_l:
+                            f.write(f"  out[{i_flat}].re = {im}; out[{i_flat}].im = -({re});\n")
+                        else:
+                            f.write(f"  out[{i_flat}].re = {re}; out[{i_flat}].im = {im};\n")
+                    if kind == "0":
+                        store(idx[(l, 0, p)], f"ar[{r} * AS]", f"ai[{r} * AS]")
+                    else:
+                        plus_r, plus_i = (f"ar[{r} * AS]", f"ai[{r} * AS]") if kind == "+" else (f"ar[{n + r} * AS]", f"ai[{n + r} * AS]")
+                        minus_r, minus_i = (f"ar[{n + r} * AS]", f"ai[{n + r} * AS]") if kind == "+" else (f"ar[{r} * AS]", f"ai[{r} * AS]")
+                        store(idx[(l, am, p)], f"R(0.5) * ({plus_r} + {minus_r})", f"R(0.5) * ({plus_i} + {minus_i})")
+                        store(idx[(l, -am, p)], f"R(0.5) * ({plus_r} - {minus_r})", f"R(0.5) * ({plus_i} - {minus_i})")
+                covered = set()
+                for (l, am, p, kind) in slots:
+                    covered.add(idx[(l, am, p)]); covered.add(idx[(l, -am, p)])
+                for i_flat in range(len(md)):
+                    if i_flat not in covered:      # m = 0 modes owned by the other sector: this sector contributes nothing
+                        f.write(f"  out[{i_flat}].re = R(0); out[{i_flat}].im = R(0);\n")
+                f.write("}\n")
+            f.write(f"#define TM_G3D_FPINST_L{lmax} {cost[0]}   // FP instructions per ordered pair (both sectors, generated apply code only)\n")
+            f.write(f"#define TM_G3D_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")
+
+
 def main():
     os.makedirs(OUT, exist_ok=True)
     emit_tables([1, 2, 3, 4, 5, 6], os.path.join(OUT, "tm_tables_gen.h"))
     emit_coplanar([1, 2, 3], os.path.join(OUT, "tm_coplanar_gen.cuh"))
+    emit_general_sym([1, 2, 3], os.path.join(OUT, "tm_general3d_gen.cuh"))
 
 
 if __name__ == "__main__":

@@ -268,3 +268,137 @@ k_allpairs_general(const double* __restrict__ pos, const Cx<R>* __restrict__ x, 
   }
   (void)m_b;
 }
+
+// ---------------------------------------------------------------------------------------------------
+// Generated 3-D kernel (arbitrary positions, lmax <= 3).  Same scheme as the coplanar kernel - rotate about z onto
+// the pair's azimuth, exploit the mirror y' -> -y' of the rotated pair (+- basis), never form the block:
+//     u^new_r = sum_q h_q(kr) sum_c ( sum_mu kappa Pbar_q^mu(cos theta) ) x^new_c      (kappa real constants)
+// but without the z-mirror: the L modes split into two SECTORS of L/2 (blockIdx.z, slowest grid dimension).
+// Thread = target; x^new (L/2 complex), Pbar (NQ(NQ+1)/2 reals) and h_q in registers; the accumulators
+// (own sector's A and the partner sector's share produced by the output rotation: L complex) live in shared memory
+// [slot][thread] (conflict-free).  Each sector writes its share of u to its own partial buffer
+// u_part[(chunk * 2 + sector)][n_scat][L]; the finishing kernel adds them in fixed order.
+#include "generated/tm_general3d_gen.cuh"
+
+template <typename R, int LMAX, int S> struct G3dPair;
+#define TM_G3D_SPEC(LM, SS_)                                                                             \
+  template <typename R> struct G3dPair<R, LM, SS_> {                                                     \
+    template <int AS>                                                                                    \
+    static __device__ __forceinline__ void run(const R* xs, const R* cm, const R* sm, const R* hr,       \
+                                               const R* hi, const R* P, R* ar, R* ai) {                  \
+      tm_g3d_pair_L##LM##_S##SS_<R, AS>(xs, cm, sm, hr, hi, P, ar, ai);                                  \
+    }                                                                                                    \
+    template <int AS>                                                                                    \
+    static __device__ __forceinline__ void unmix(const R* ar, const R* ai, Cx<R>* out) {                 \
+      tm_g3d_unmix_L##LM##_S##SS_<R, Cx<R>, AS>(ar, ai, out);                                            \
+    }                                                                                                    \
+    static __device__ __forceinline__ void stage_entry(int k, int& a, int& b, int& sg) {                 \
+      a = tm_g3d_sa_L##LM##_S##SS_[k]; b = tm_g3d_sb_L##LM##_S##SS_[k]; sg = tm_g3d_ss_L##LM##_S##SS_[k]; \
+    }                                                                                                    \
+  };
+TM_G3D_SPEC(1, 0) TM_G3D_SPEC(1, 1) TM_G3D_SPEC(2, 0) TM_G3D_SPEC(2, 1) TM_G3D_SPEC(3, 0) TM_G3D_SPEC(3, 1)
+#undef TM_G3D_SPEC
+
+template <int LMAX> struct PbarAll;
+template <> struct PbarAll<1> { template <typename R> static __device__ __forceinline__ void run(R ct, R st, R* P) { tm_pbar_all_L1<R>(ct, st, P); } };
+template <> struct PbarAll<2> { template <typename R> static __device__ __forceinline__ void run(R ct, R st, R* P) { tm_pbar_all_L2<R>(ct, st, P); } };
+template <> struct PbarAll<3> { template <typename R> static __device__ __forceinline__ void run(R ct, R st, R* P) { tm_pbar_all_L3<R>(ct, st, P); } };
+
+template <typename R, int LMAX, int TJ, int SS> struct Sym3dSmem {
+  static constexpr int L = 2 * LMAX * (LMAX + 2);
+  static constexpr size_t bytes = sizeof(double) * 3 * SS + sizeof(R) * (size_t)(SS * L * 2 + 2 * L * TJ) + sizeof(int) * 3 * L;
+};
+
+template <typename R, int LMAX, int TJ, int SS>
+__global__ void __launch_bounds__(TJ)
+k_allpairs_sym3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
+                 const TmTile* __restrict__ tiles, int n_scat, double k_over_pi, double inv_k,
+                 const int* __restrict__ n_active) {
+  constexpr int L = 2 * LMAX * (LMAX + 2);
+  constexpr int NS = L / 2;                 // slots per sector
+  constexpr int NQ = 2 * LMAX + 1;
+  constexpr int NP = NQ * (NQ + 1) / 2;
+  if (n_active != nullptr && *n_active == 0) return;
+
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* s_px = reinterpret_cast<double*>(smem_raw);
+  double* s_py = s_px + SS;
+  double* s_pz = s_py + SS;
+  R* s_x = reinterpret_cast<R*>(s_pz + SS);          // [source][2 NS] complex: own slots then partner slots
+  R* s_acc = s_x + SS * L * 2;                       // [re/im][2 NS][TJ]
+  int* s_sa = reinterpret_cast<int*>(s_acc + 2 * L * TJ);
+  int* s_sb = s_sa + L;
+  int* s_ss = s_sb + L;
+
+  const TmTile tile = tiles[blockIdx.x];
+  const int tid = threadIdx.x;
+  const int sct = blockIdx.z;
+  const bool live = tid < tile.tgt_count;
+  const int j = tile.tgt_start + (live ? tid : tile.tgt_count - 1);
+  const double xj = pos[3 * j], yj = pos[3 * j + 1], zj = pos[3 * j + 2];
+  const int per = (tile.src_count + gridDim.y - 1) / gridDim.y;
+  const int c0 = tile.src_start + blockIdx.y * per;
+  const int c1 = min(tile.src_start + tile.src_count, c0 + per);
+
+  if (tid < L) {
+    int a, b, sg;
+    if (sct == 0) G3dPair<R, LMAX, 0>::stage_entry(tid, a, b, sg); else G3dPair<R, LMAX, 1>::stage_entry(tid, a, b, sg);
+    s_sa[tid] = a; s_sb[tid] = b; s_ss[tid] = sg;
+  }
+  R* ar = s_acc + tid;
+  R* ai = s_acc + L * TJ + tid;
+#pragma unroll
+  for (int b = 0; b < L; ++b) { ar[b * TJ] = R(0); ai[b * TJ] = R(0); }
+
+  for (int s0 = c0; s0 < c1; s0 += SS) {
+    const int ns = min(SS, c1 - s0);
+    __syncthreads();
+    for (int e = tid; e < ns; e += TJ) {
+      s_px[e] = pos[3 * (s0 + e)]; s_py[e] = pos[3 * (s0 + e) + 1]; s_pz[e] = pos[3 * (s0 + e) + 2];
+    }
+    for (int e = tid; e < ns * L; e += TJ) {
+      const int src = e / L, kk = e - src * L;
+      const Cx<R>* xrow = x + (size_t)(s0 + src) * L;
+      const int ia = s_sa[kk], sg = s_ss[kk];
+      Cx<R> v = xrow[ia];
+      if (sg != 0) {
+        const Cx<R> o = xrow[s_sb[kk]];
+        v = sg > 0 ? cadd(v, o) : csub(v, o);
+      }
+      if (ia >= NS) v = cx<R>(-v.im, v.re);            // tilde basis: multiply p = 1 modes by i
+      s_x[2 * e] = v.re;
+      s_x[2 * e + 1] = v.im;
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int s = 0; s < ns; ++s) {
+      const double dx = xj - s_px[s], dy = yj - s_py[s], dz = zj - s_pz[s];   // d = x_dest - x_source (reading R3)
+      const double rho2 = dx * dx + dy * dy, r2 = rho2 + dz * dz;
+      const double rinv = r2 > 0.0 ? rsqrt(r2) : 0.0;          // self pair -> h_q = 0 -> contributes nothing
+      const double rhoinv = rho2 > 0.0 ? rsqrt(rho2) : 0.0;
+      const double r = r2 * rinv;
+      R cm[LMAX + 1], sm[LMAX + 1];
+      cm[0] = R(1); sm[0] = R(0);
+      cm[1] = rho2 > 0.0 ? (R)(dx * rhoinv) : R(1); sm[1] = (R)(dy * rhoinv);
+#pragma unroll
+      for (int m = 2; m <= LMAX; ++m) {
+        cm[m] = cm[m - 1] * cm[1] - sm[m - 1] * sm[1];
+        sm[m] = sm[m - 1] * cm[1] + cm[m - 1] * sm[1];
+      }
+      R ck, sk;
+      phase_kr<R>(k_over_pi, r, ck, sk);
+      R hr[NQ], hi[NQ];
+      hankel_up<R, NQ>((R)(rinv * inv_k), ck, sk, hr, hi);
+      R P[NP];
+      PbarAll<LMAX>::template run<R>((R)(dz * rinv), (R)(rho2 * rhoinv * rinv), P);
+      const R* xs = &s_x[s * L * 2];
+      if (sct == 0) G3dPair<R, LMAX, 0>::template run<TJ>(xs, cm, sm, hr, hi, P, ar, ai);
+      else          G3dPair<R, LMAX, 1>::template run<TJ>(xs, cm, sm, hr, hi, P, ar, ai);
+    }
+  }
+  if (live) {
+    Cx<R>* out = u_part + ((size_t)(blockIdx.y * 2 + sct) * n_scat + j) * L;
+    if (sct == 0) G3dPair<R, LMAX, 0>::template unmix<TJ>(ar, ai, out);
+    else          G3dPair<R, LMAX, 1>::template unmix<TJ>(ar, ai, out);
+  }
+}

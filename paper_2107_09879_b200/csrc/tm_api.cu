@@ -23,6 +23,8 @@ namespace {
 std::string g_create_error;
 
 constexpr int COP_SS = 64;       // coplanar kernel: sources per shared-memory stage
+constexpr int SYM3D_TJ = 128;    // generated 3-D kernel: targets per block
+constexpr int SYM3D_SS = 32;     // generated 3-D kernel: sources per stage
 constexpr int MAX_RESTART = 300;
 
 struct Gmres {                   // device scalars of the Krylov solver, sized for `restart`
@@ -56,7 +58,7 @@ struct tm_ctx {
   TmConst h_const{};
   int* d_rowptr = nullptr; uint8_t* d_col = nullptr; uint8_t* d_widx = nullptr; uint8_t* d_imag = nullptr; double* d_coef = nullptr;
 
-  TmTile* d_tiles = nullptr; int n_tiles = 0, n_chunk = 1;
+  TmTile* d_tiles = nullptr; int n_tiles = 0, n_chunk = 1, n_part = 1;   // n_part: partial-sum buffers the finishing kernel adds
   void* d_upart = nullptr; size_t upart_bytes = 0;
   TmChunk* d_chunks = nullptr; int n_chunks = 0; int* d_win_chunk_ptr = nullptr;
   int ept = 4;                   // vector kernels: elements per thread (chunk = ept * TM_VT)
@@ -196,6 +198,21 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
     }
 #undef TM_LAUNCH_COP
 #undef TM_LAUNCH_COP2
+  } else if (c->kernel == TM_KERNEL_SYM3D) {
+    grid.z = 2;                                         // y'-mirror sector: slowest grid dimension
+#define TM_LAUNCH_S3(LM)                                                                                        \
+  {                                                                                                             \
+    const size_t sm = Sym3dSmem<R, LM, SYM3D_TJ, SYM3D_SS>::bytes;                                              \
+    cudaFuncSetAttribute(k_allpairs_sym3d<R, LM, SYM3D_TJ, SYM3D_SS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
+    k_allpairs_sym3d<R, LM, SYM3D_TJ, SYM3D_SS><<<grid, SYM3D_TJ, sm, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat, \
+                                                                                   k_over_pi, inv_k, n_active); \
+  }
+    switch (c->lmax) {
+      case 1: TM_LAUNCH_S3(1) break;
+      case 2: TM_LAUNCH_S3(2) break;
+      default: TM_LAUNCH_S3(3) break;
+    }
+#undef TM_LAUNCH_S3
   } else {
     TmTermsDev tb{c->d_rowptr, c->d_col, c->d_widx, c->d_imag, c->d_coef};
 #define TM_LAUNCH_GEN(LM)                                                                                         \
@@ -224,7 +241,7 @@ template <typename R>
 cudaError_t launch_tapply(tm_ctx* c, int mode, const Cx<R>* x, Cx<R>* y, const int* n_active) {
   constexpr int JB = 8;
   const int grid = (c->n_scat + JB - 1) / JB;
-  k_tapply<R, JB><<<grid, 256, 0, c->stream>>>(mode, c->L, c->n_scat, c->n_chunk, x, reinterpret_cast<Cx<R>*>(c->d_upart), y,
+  k_tapply<R, JB><<<grid, 256, 0, c->stream>>>(mode, c->L, c->n_scat, c->n_part, x, reinterpret_cast<Cx<R>*>(c->d_upart), y,
                                                reinterpret_cast<Cx<R>*>(c->d_T), c->diag, c->d_type_of, c->d_const, n_active);
   c->total_launches++;
   return cudaGetLastError();
@@ -418,15 +435,18 @@ void fill_const(tm_ctx* c) {
 
 int configure_kernel(tm_ctx* ctx) {
   int want = ctx->kernel_req;
-  if (want == TM_KERNEL_AUTO) want = (ctx->coplanar && ctx->lmax <= 3) ? TM_KERNEL_COPLANAR : TM_KERNEL_GENERAL;
+  if (want == TM_KERNEL_AUTO)
+    want = (ctx->coplanar && ctx->lmax <= 3) ? TM_KERNEL_COPLANAR : (ctx->lmax <= 3 ? TM_KERNEL_SYM3D : TM_KERNEL_GENERAL);
   if (want == TM_KERNEL_COPLANAR && !(ctx->coplanar && ctx->lmax <= 3))
     return fail(ctx, TM_E_INVALID, "coplanar kernel needs all z equal and lmax <= 3");
+  if (want == TM_KERNEL_SYM3D && ctx->lmax > 3) return fail(ctx, TM_E_INVALID, "generated 3-D kernel needs lmax <= 3");
   ctx->kernel = want;
   if (const char* e = std::getenv("TM_COP_TJ")) ctx->cop_tj = std::atoi(e) == 256 ? 256 : 128;
   if (const char* e = std::getenv("TM_COP_LOCKSTEP")) ctx->cop_lockstep = std::atoi(e) != 0;
   int tgt_per_tile;
-  switch (want == TM_KERNEL_COPLANAR ? 0 : ctx->lmax) {
-    case 0: tgt_per_tile = ctx->cop_tj; break;
+  const bool gen = want == TM_KERNEL_COPLANAR || want == TM_KERNEL_SYM3D;      // generated kernels: thread = target
+  switch (gen ? 0 : ctx->lmax) {
+    case 0: tgt_per_tile = want == TM_KERNEL_SYM3D ? SYM3D_TJ : ctx->cop_tj; break;
     case 1: case 2: case 3: tgt_per_tile = 4; break;
     default: tgt_per_tile = 2; break;
   }
@@ -441,15 +461,16 @@ int configure_kernel(tm_ctx* ctx) {
   // Source chunks: pick the chunk count that minimises (waves of resident blocks) x (sources per block), so that
   // small problems fill the 148 SMs (2 resident 128-thread blocks each at 255 registers) and large ones end
   // without a long tail; bounded by 64 chunks, >= 32 sources per chunk and 2 GB of partial sums.
-  const long long slots = 148LL * (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj : 4);
-  const long long blocks1 = (long long)ctx->n_tiles * (want == TM_KERNEL_COPLANAR ? 2 : 1);
+  const long long slots = 148LL * (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj : (want == TM_KERNEL_SYM3D ? 2 : 4));
+  const long long blocks1 = (long long)ctx->n_tiles * (gen ? 2 : 1);
+  const int part_mult = want == TM_KERNEL_SYM3D ? 2 : 1;        // SYM3D: one partial buffer per (chunk, sector)
   int max_win = 1;
   for (int w = 0; w < ctx->n_win; ++w) max_win = std::max(max_win, ctx->win_ptr[w + 1] - ctx->win_ptr[w]);
   const size_t vec_bytes = ctx->n * elem_bytes(ctx);
   long long nchunk = 1;
   double best = 1e300;
   for (long long cnd = 1; cnd <= 64; ++cnd) {
-    if (cnd > 1 && (min_win / cnd < 32 || (size_t)cnd * vec_bytes > ((size_t)2 << 30))) break;
+    if (cnd > 1 && (min_win / cnd < 32 || (size_t)cnd * part_mult * vec_bytes > ((size_t)2 << 30))) break;
     const long long waves = (blocks1 * cnd + slots - 1) / slots;
     const double cost = (double)waves * (double)((max_win + cnd - 1) / cnd + 8);     // +8: per-block fixed cost
     if (cost < best * 0.995) { best = cost; nchunk = cnd; }
@@ -458,7 +479,8 @@ int configure_kernel(tm_ctx* ctx) {
   if (ctx->d_tiles) cudaFree(ctx->d_tiles);
   TM_CUDA(cudaMalloc(&ctx->d_tiles, tiles.size() * sizeof(TmTile)));
   TM_CUDA(cudaMemcpy(ctx->d_tiles, tiles.data(), tiles.size() * sizeof(TmTile), cudaMemcpyHostToDevice));
-  const size_t need = (size_t)ctx->n_chunk * vec_bytes;
+  ctx->n_part = ctx->n_chunk * part_mult;
+  const size_t need = (size_t)ctx->n_part * vec_bytes;
   if (need > ctx->upart_bytes) {
     if (ctx->d_upart) cudaFree(ctx->d_upart);
     ctx->d_upart = nullptr; ctx->upart_bytes = 0;
@@ -663,7 +685,7 @@ int tm_create(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const 
 
 int tm_set_kernel(tm_ctx* ctx, int kernel) {
   if (!ctx) return TM_E_INVALID;
-  if (kernel < TM_KERNEL_AUTO || kernel > TM_KERNEL_COPLANAR) return fail(ctx, TM_E_INVALID, "unknown kernel id");
+  if (kernel < TM_KERNEL_AUTO || kernel > TM_KERNEL_SYM3D) return fail(ctx, TM_E_INVALID, "unknown kernel id");
   const int old = ctx->kernel_req;
   ctx->kernel_req = kernel;
   TM_CUDA(cudaStreamSynchronize(ctx->stream));
@@ -1048,6 +1070,10 @@ int tm_pair_cost(const tm_ctx* ctx, double* fp_instructions, double* flop) {
   if (ctx->kernel == TM_KERNEL_COPLANAR) {
     const int I[4] = {0, TM_COP_FPINST_L1, TM_COP_FPINST_L2, TM_COP_FPINST_L3};
     const int F[4] = {0, TM_COP_FLOP_L1, TM_COP_FLOP_L2, TM_COP_FLOP_L3};
+    inst = I[ctx->lmax]; fl = F[ctx->lmax];
+  } else if (ctx->kernel == TM_KERNEL_SYM3D) {
+    const int I[4] = {0, TM_G3D_FPINST_L1, TM_G3D_FPINST_L2, TM_G3D_FPINST_L3};
+    const int F[4] = {0, TM_G3D_FLOP_L1, TM_G3D_FLOP_L2, TM_G3D_FLOP_L3};
     inst = I[ctx->lmax]; fl = F[ctx->lmax];
   } else {   // general kernel: per (term, source): 2 MUL + 4 FMA
     const double nt = tm_term_tables[ctx->lmax - 1].n_terms;

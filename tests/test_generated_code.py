@@ -32,6 +32,21 @@ def test_generated_coplanar_pair_code_matches_oracle_block(lmax, tmp_path):
         assert np.abs(u - ref).max() <= 2e-13 * np.abs(ref).max()
 
 
+@pytest.mark.parametrize("lmax", [1, 2, 3])
+def test_generated_3d_pair_code_matches_oracle_block(lmax, tmp_path):
+    exe = str(tmp_path / f"hostcheck3d{lmax}")
+    subprocess.check_call(["g++", "-O1", f"-DLMAX={lmax}", "-o", exe, os.path.join(ROOT, "tests", "hostcheck_general3d.cpp")])
+    rng = np.random.default_rng(50 + lmax)
+    L = n_modes(lmax)
+    for d in ([0.3, -0.4, 0.8], [0.0, 0.0, 1.2], [0.0, 0.0, -0.7], [1.0, 0.5, 0.0], rng.uniform(-30, 30, 3), rng.uniform(-3, 3, 3)):
+        x = rng.standard_normal(L) + 1j * rng.standard_normal(L)
+        inp = " ".join(repr(float(v)) for v in d) + "\n" + "\n".join(f"{float(z.real)!r} {float(z.imag)!r}" for z in x) + "\n"
+        out = subprocess.run([exe], input=inp, capture_output=True, text=True, check=True).stdout
+        u = np.array([complex(*map(float, ln.split())) for ln in out.strip().splitlines()])
+        ref = tr.block(lmax, K, np.array(d, dtype=float), np.zeros(3)) @ x
+        assert np.abs(u - ref).max() <= 2e-13 * np.abs(ref).max()
+
+
 def _parse_table(text, name, conv):
     m = re.search(name + r"\[\d+\] = \{(.*?)\};", text, flags=re.S)
     return [conv(t) for t in m.group(1).replace("\n", " ").split(",") if t.strip()]

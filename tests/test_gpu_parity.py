@@ -58,15 +58,44 @@ def test_allpairs_matvec_lattice(tm, kernel, lmax, n_side):
 
 @pytest.mark.parametrize("lmax", [1, 2, 3, 4])
 def test_allpairs_matvec_random_3d_cloud(tm, lmax):
-    """Random non-lattice 3-D positions (PAPER.md:375 uses random positions): general kernel is selected."""
+    """Random non-lattice 3-D positions (PAPER.md:375 uses random positions): AUTO picks the generated 3-D kernel for
+    lmax <= 3 and the table-driven kernel above; the table-driven kernel is also checked for lmax <= 3."""
     n = 150 if lmax <= 3 else 40
     pos = W.random_cloud(n, seed=20 + lmax)
+    pos[7] = pos[3] + [0.0, 0.0, 0.9]                    # a pair on a common vertical axis (theta = 0, rho = 0)
     x = rand_x((n, W.n_modes(lmax)), 30 + lmax)
-    s = tm.Solver(pos, lmax, W.K_B)
-    assert s.get_kernel() == tm.TM_KERNEL_GENERAL
-    u = s.matvec(x, transpose=2)
     ref = omv.matvec_rows(lmax, W.K_B, pos, x)
-    assert rel(u, ref) <= 1e-12
+    s = tm.Solver(pos, lmax, W.K_B)
+    assert s.get_kernel() == (tm.TM_KERNEL_SYM3D if lmax <= 3 else tm.TM_KERNEL_GENERAL)
+    assert rel(s.matvec(x, transpose=2), ref) <= 1e-12
+    if lmax <= 3:
+        s.set_kernel(tm.TM_KERNEL_GENERAL)
+        assert s.get_kernel() == tm.TM_KERNEL_GENERAL
+        assert rel(s.matvec(x, transpose=2), ref) <= 1e-12
+    s.close()
+
+
+def test_sym3d_kernel_tiles_chunks_windows_fp32(tm):
+    """Generated 3-D kernel over several 128-target tiles, a ragged tail, several source chunks, ragged windows; fp32."""
+    pos = W.random_cloud(700, seed=77)
+    wp = np.array([0, 300, 301, 700], dtype=np.int32)
+    x = rand_x((700, 30), 78)
+    ref = omv.matvec_rows(3, W.K_B, pos, x, win_ptr=wp)
+    s = tm.Solver(pos, 3, W.K_B, win_ptr=wp)
+    assert s.get_kernel() == tm.TM_KERNEL_SYM3D
+    u = s.matvec(x, transpose=2)
+    assert rel(u, ref) <= 1e-12 and np.all(u[300] == 0)
+    s.close()
+    s = tm.Solver(pos, 3, W.K_B, win_ptr=wp, precision=tm.TM_FP32)
+    assert rel(s.matvec(x, transpose=2), ref) <= 2e-5
+    s.close()
+    # a planar layout forced through the 3-D kernel must agree with the coplanar one
+    posp = W.lattice(9, 11)
+    xp = rand_x((99, 30), 79)
+    s = tm.Solver(posp, 3, W.K_B)
+    a = s.matvec(xp, transpose=2)
+    s.set_kernel(tm.TM_KERNEL_SYM3D)
+    assert rel(s.matvec(xp, transpose=2), a) <= 1e-13
     s.close()
 
 
@@ -85,7 +114,7 @@ def test_allpairs_matvec_windows(tm):
     pos = W.random_cloud(200, seed=8, planar=True)
     wp = np.array([0, 1, 70, 71, 200], dtype=np.int32)
     x = rand_x((200, 30), 9)
-    for kern in (tm.TM_KERNEL_COPLANAR, tm.TM_KERNEL_GENERAL):
+    for kern in (tm.TM_KERNEL_COPLANAR, tm.TM_KERNEL_GENERAL, tm.TM_KERNEL_SYM3D):
         s = tm.Solver(pos, 3, W.K_B, win_ptr=wp)
         s.set_kernel(kern)
         u = s.matvec(x, transpose=2)
