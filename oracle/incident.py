@@ -107,3 +107,68 @@ def gaussian_beam_field_direct(k, x, focus, w0, Ax, Ay, n_beta=200, n_alpha=256)
     Az = -np.tan(B) * (Ax * np.cos(Al) + Ay * np.sin(Al))
     w = wb[:, None] * (2 * np.pi / n_alpha) * np.sin(B) * np.cos(B) * G * ph / (2 * np.pi)
     return np.array([np.sum(w * Ax), np.sum(w * Ay), np.sum(w * Az)])
+
+
+# ------------------------------------------------------------------------------------------------ jinc sources (NEXT-1)
+def jinc_source_incident(lmax, k, pos, src, Ax, Ay, n_beta=400):
+    """a^(0)_j of ONE jinc source: flat angular spectrum inside the light cone, Eq. II3, centred at
+    `src` = (x_0, y_0, z_0), transverse amplitude (Ax, Ay).  Eq. II9 with the alpha integral done in closed form
+    (Eqs. II15 / II17) and Gauss-Legendre in beta on [0, pi/2] (n_beta nodes: part of the definition, as for reading R9).
+    With Eq. II3 (and the k_0^2 of d^2k dropped in Eq. II9) the transverse field on the source plane is
+        E^T(x^T, z_0) = A^T J_1(k_0 rho) / (k_0 rho),  rho = |x^T - x_0^T|     (cylindrical J_1; reading R17)."""
+    pos = np.atleast_2d(np.asarray(pos, dtype=float))
+    src = np.asarray(src, dtype=float)
+    xg, wg = np.polynomial.legendre.leggauss(n_beta)
+    beta = 0.25 * np.pi * (xg + 1.0)
+    wq = 0.25 * np.pi * wg
+    out = np.zeros((pos.shape[0], n_modes(lmax)), dtype=complex)
+    for j in range(pos.shape[0]):
+        rel = pos[j] - src
+        for idx, (l, m, p) in enumerate(mode_list(lmax)):
+            out[j, idx] = np.sum(wq * _alpha_integrated(l, m, p, k, rel, beta, Ax, Ay))
+    return out
+
+
+def jinc_field_direct(k, x, src, Ax, Ay, n_beta=300, n_alpha=512):
+    """Direct 2-D quadrature of Eq. II4 with the flat spectrum (pin for jinc_source_incident), k_0^2 dropped as in II9."""
+    x = np.asarray(x, dtype=float) - np.asarray(src, dtype=float)
+    xg, wg = np.polynomial.legendre.leggauss(n_beta)
+    beta = 0.25 * np.pi * (xg + 1.0)
+    wb = 0.25 * np.pi * wg
+    alpha = 2 * np.pi * np.arange(n_alpha) / n_alpha
+    B, Al = np.meshgrid(beta, alpha, indexing="ij")
+    kx, ky, kz = k * np.sin(B) * np.cos(Al), k * np.sin(B) * np.sin(Al), k * np.cos(B)
+    ph = np.exp(1j * (kx * x[0] + ky * x[1] + kz * x[2]))
+    Az = -np.tan(B) * (Ax * np.cos(Al) + Ay * np.sin(Al))
+    w = wb[:, None] * (2 * np.pi / n_alpha) * np.sin(B) * np.cos(B) * ph / (2 * np.pi)
+    return np.array([np.sum(w * Ax), np.sum(w * Ay), np.sum(w * Az)])
+
+
+def nyquist_source_amplitude(E_sample):
+    """Amplitude of the jinc source that carries the Nyquist sample E^T(x_i, y_j) (Eq. II1; reading R17).
+    For a field band-limited to the light cone and sampled on the square grid of pitch lambda/2 = pi/k_0 the
+    reconstruction kernel is the ideal disc low-pass
+        f(rho) = (pi/k_0)^2 / (2 pi)^2 * int_{|k|<k_0} e^{i k.rho} d^2k = (pi/2) J_1(k_0 rho)/(k_0 rho),
+    i.e. (pi/2) times the unit jinc source of jinc_source_incident (Eq. II1 prints the kernel without the constant)."""
+    return 0.5 * np.pi * np.asarray(E_sample)
+
+
+def nyquist_sources(k, x_range, y_range, z0, field_fn):
+    """Sample a transverse field field_fn(x, y) -> (Ex, Ey) on the lambda/2 grid covering the ranges:
+    returns (src (S,3), amp (S,2)) with amp the jinc-source amplitudes."""
+    h = np.pi / k
+    ix = np.arange(int(np.ceil(x_range[0] / h)), int(np.floor(x_range[1] / h)) + 1)
+    iy = np.arange(int(np.ceil(y_range[0] / h)), int(np.floor(y_range[1] / h)) + 1)
+    X, Y = np.meshgrid(ix * h, iy * h, indexing="xy")
+    src = np.stack([X.ravel(), Y.ravel(), np.full(X.size, float(z0))], axis=1)
+    Ex, Ey = field_fn(src[:, 0], src[:, 1])
+    amp = np.stack([nyquist_source_amplitude(Ex), nyquist_source_amplitude(Ey)], axis=1).astype(complex)
+    return src, amp
+
+
+def jinc_sources_incident(lmax, k, pos, src, amp, n_beta=400):
+    """Superposition of jinc sources: sum_s jinc_source_incident(..., src[s], amp[s,0], amp[s,1])."""
+    out = np.zeros((np.atleast_2d(pos).shape[0], n_modes(lmax)), dtype=complex)
+    for s in range(len(src)):
+        out += jinc_source_incident(lmax, k, pos, src[s], amp[s, 0], amp[s, 1], n_beta)
+    return out
