@@ -37,7 +37,7 @@ typedef struct { double re, im; } tm_c64;
 enum { TM_FP64 = 0, TM_FP32 = 1 };                       /* internal compute precision of the solver */
 enum { TM_OK = 0, TM_NOT_CONVERGED = 1,
        TM_E_INVALID = -1, TM_E_OVERLAP = -2, TM_E_STATE = -3, TM_E_CUDA = -4, TM_E_NOMEM = -5 };
-enum { TM_INC_PLANE = 0, TM_INC_GAUSS = 1, TM_INC_COEFFS = 2 };
+enum { TM_INC_PLANE = 0, TM_INC_GAUSS = 1, TM_INC_COEFFS = 2, TM_INC_JINC = 3 };
 enum { TM_FIELD_E_SCA = 0, TM_FIELD_H_SCA = 1 };           /* H is returned as Z_b * H (reading R10) */
 enum { TM_KERNEL_AUTO = 0, TM_KERNEL_GENERAL = 1, TM_KERNEL_COPLANAR = 2, TM_KERNEL_SYM3D = 3 };
 
@@ -51,6 +51,15 @@ typedef struct { double beta, alpha; tm_c64 A_beta, A_alpha; } tm_plane_desc;
  * (Ax, Ay) exp(-|x_T - focus_T|^2 / w0^2).  focus: HOST pointer [n_win][3].  n_beta: Gauss-Legendre nodes in
  * the polar angle (0 -> default 400). */
 typedef struct { const double *focus; double w0; tm_c64 Ax, Ay; int n_beta; } tm_gauss_desc;
+
+/* Superposition of jinc sources per window - the paper's Nyquist decomposition of a band-limited incident field
+ * (Eqs. II1-II17; reading R17).  Source s: flat angular spectrum inside the light cone,
+ * centred at src_xyz[s] = (x_0, y_0, z_0), propagating along +z, transverse field on its plane
+ * (Ax_s, Ay_s) J_1(k rho)/(k rho); window w owns the sources src_ptr[w] <= s < src_ptr[w+1].
+ * A field sampled on the lambda/2 grid is carried by sources of amplitude (pi/2) x sample (reading R17).
+ * All pointers are HOST pointers.  n_beta: Gauss-Legendre nodes on [0, pi/2] (0 -> 400). */
+typedef struct { int n_src; const double *src_xyz; const tm_c64 *amp /* [n_src][2] */; const int *src_ptr /* [n_win+1] */;
+                 int n_beta; } tm_jinc_desc;
 
 /* Caller-supplied incident coefficients p[n_scat][L] (host or device). */
 typedef struct { const tm_c64 *p; } tm_coeffs_desc;
@@ -92,7 +101,7 @@ int tm_set_tmatrices(tm_ctx *ctx, int n_types, int diag_only, const tm_c64 *T, c
                      const double *r_enclosing);
 
 /* Incident field -> coefficients p_j = a^(0)_j of every scatterer, computed on the device
- * (Eq. I12; kind selects tm_plane_desc / tm_gauss_desc / tm_coeffs_desc). */
+ * (Eq. I12; kind selects tm_plane_desc / tm_gauss_desc / tm_coeffs_desc / tm_jinc_desc). */
 int tm_set_incident(tm_ctx *ctx, int kind, const void *desc);
 
 /* Copy the current incident coefficients p [n_scat][L] out (host or device). */

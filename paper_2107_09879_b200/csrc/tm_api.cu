@@ -873,40 +873,68 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     cudaFree(d_a);
     TM_CUDA(e);
-  } else if (kind == TM_INC_GAUSS) {
-    const tm_gauss_desc* d = static_cast<const tm_gauss_desc*>(desc);
-    if (!d->focus || !(d->w0 > 0.0)) return fail(ctx, TM_E_INVALID, "need focus[n_win][3] and w0 > 0");
-    if (lmax > 3) return fail(ctx, TM_E_INVALID, "Gaussian-beam expansion is built for lmax <= 3");
-    const int nb = d->n_beta > 0 ? d->n_beta : 400;
-    // beta in [0, beta_max]: G(beta) < 1e-40 beyond (or pi/2: evanescent part dropped, reading R9)
-    const double kw = ctx->k * d->w0;
-    const double smax = std::min(1.0, 2.0 * std::sqrt(40.0 * std::log(10.0)) / kw);
-    const double bmax = std::asin(smax);
+  } else if (kind == TM_INC_GAUSS || kind == TM_INC_JINC) {
+    // both are angular-spectrum sources (Eqs. II9-II17): per window a list of source centres with transverse amplitudes
+    if (lmax > 3) return fail(ctx, TM_E_INVALID, "beam / jinc-source expansion is built for lmax <= 3");
+    std::vector<double> hsrc;
+    std::vector<double2> hamp;
+    std::vector<int> hptr(ctx->n_win + 1);
+    int nb_req = 0;
+    double kw = -1.0, bmax = 0.5 * M_PI;                 // jinc: flat spectrum on [0, pi/2]
+    if (kind == TM_INC_GAUSS) {
+      const tm_gauss_desc* d = static_cast<const tm_gauss_desc*>(desc);
+      if (!d->focus || !(d->w0 > 0.0)) return fail(ctx, TM_E_INVALID, "need focus[n_win][3] and w0 > 0");
+      hsrc.assign(d->focus, d->focus + (size_t)ctx->n_win * 3);
+      for (int w = 0; w < ctx->n_win; ++w) {
+        hamp.push_back(make_double2(d->Ax.re, d->Ax.im)); hamp.push_back(make_double2(d->Ay.re, d->Ay.im));
+        hptr[w] = w;
+      }
+      hptr[ctx->n_win] = ctx->n_win;
+      nb_req = d->n_beta;
+      // beta in [0, beta_max]: G(beta) < 1e-40 beyond (or pi/2: evanescent part dropped, reading R9)
+      kw = ctx->k * d->w0;
+      bmax = std::asin(std::min(1.0, 2.0 * std::sqrt(40.0 * std::log(10.0)) / kw));
+    } else {
+      const tm_jinc_desc* d = static_cast<const tm_jinc_desc*>(desc);
+      if (d->n_src < 0 || !d->src_ptr || (d->n_src > 0 && (!d->src_xyz || !d->amp)))
+        return fail(ctx, TM_E_INVALID, "need src_xyz, amp and src_ptr");
+      hptr.assign(d->src_ptr, d->src_ptr + ctx->n_win + 1);
+      if (hptr[0] != 0 || hptr[ctx->n_win] != d->n_src) return fail(ctx, TM_E_INVALID, "src_ptr must start at 0 and end at n_src");
+      for (int w = 0; w < ctx->n_win; ++w) if (hptr[w + 1] < hptr[w]) return fail(ctx, TM_E_INVALID, "src_ptr must be monotone");
+      hsrc.assign(d->src_xyz, d->src_xyz + (size_t)d->n_src * 3);
+      for (int sidx = 0; sidx < 2 * d->n_src; ++sidx) hamp.push_back(make_double2(d->amp[sidx].re, d->amp[sidx].im));
+      nb_req = d->n_beta;
+    }
+    const int nb = nb_req > 0 ? nb_req : 400;
+    const size_t nsrc = hsrc.size() / 3;
     std::vector<double> xg, wg, beta(nb), wq(nb);
     gauss_legendre(nb, xg, wg);
     for (int q = 0; q < nb; ++q) { beta[q] = 0.5 * bmax * (xg[q] + 1.0); wq[q] = 0.5 * bmax * wg[q]; }
-    double *d_beta = nullptr, *d_wq = nullptr, *d_focus = nullptr; void* d_nodes = nullptr;
+    double *d_beta = nullptr, *d_wq = nullptr, *d_src = nullptr; double2* d_amp = nullptr; int* d_ptr = nullptr; void* d_nodes = nullptr;
     const size_t node_bytes = lmax == 1 ? sizeof(GaussNode<1>) : lmax == 2 ? sizeof(GaussNode<2>) : sizeof(GaussNode<3>);
     cudaError_t e = cudaMalloc(&d_beta, nb * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&d_wq, nb * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc(&d_focus, (size_t)ctx->n_win * 3 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&d_src, std::max<size_t>(1, nsrc) * 3 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&d_amp, std::max<size_t>(1, nsrc) * 2 * sizeof(double2));
+    if (e == cudaSuccess) e = cudaMalloc(&d_ptr, (ctx->n_win + 1) * sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&d_nodes, nb * node_bytes);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_beta, beta.data(), nb * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_wq, wq.data(), nb * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_focus, d->focus, (size_t)ctx->n_win * 3 * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess && nsrc) e = cudaMemcpyAsync(d_src, hsrc.data(), nsrc * 3 * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess && nsrc) e = cudaMemcpyAsync(d_amp, hamp.data(), nsrc * 2 * sizeof(double2), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_ptr, hptr.data(), (ctx->n_win + 1) * sizeof(int), cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) {
-      const double2 Ax = make_double2(d->Ax.re, d->Ax.im), Ay = make_double2(d->Ay.re, d->Ay.im);
 #define TM_GAUSS(LM)                                                                                                   \
   k_gauss_nodes<LM><<<(nb + 127) / 128, 128, 0, ctx->stream>>>(d_beta, d_wq, nb, kw, static_cast<GaussNode<LM>*>(d_nodes)); \
-  k_incident_gauss<LM><<<ctx->n_scat, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->d_win_of, d_focus,                        \
-                                                            static_cast<GaussNode<LM>*>(d_nodes), nb, ctx->k, Ax, Ay, ctx->d_p)
+  k_incident_gauss<LM><<<ctx->n_scat, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->d_win_of, d_src, d_amp, d_ptr,            \
+                                                            static_cast<GaussNode<LM>*>(d_nodes), nb, ctx->k, ctx->d_p)
       if (lmax == 1) { TM_GAUSS(1); } else if (lmax == 2) { TM_GAUSS(2); } else { TM_GAUSS(3); }
 #undef TM_GAUSS
       ctx->total_launches += 2;
       e = cudaGetLastError();
     }
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
-    cudaFree(d_beta); cudaFree(d_wq); cudaFree(d_focus); cudaFree(d_nodes);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);   // the host vectors above must outlive the copies
+    cudaFree(d_beta); cudaFree(d_wq); cudaFree(d_src); cudaFree(d_amp); cudaFree(d_ptr); cudaFree(d_nodes);
     TM_CUDA(e);
   } else {
     return fail(ctx, TM_E_INVALID, "unknown incident kind");

@@ -2,6 +2,8 @@
 //   plane wave:    Eqs. II6-II7: one L-vector (host, closed form) times exp(i k . x_j)
 //   Gaussian beam: reading R9 - Eqs. II9-II17 with the alpha integral in closed form
 //                  (Gamma_m, Eq. II11) and a Gauss-Legendre sum in beta, Gaussian spectral weight.
+//   jinc sources:  the paper's own case (flat spectrum inside the light cone, Eqs. II3-II17), superposed per window
+//                  with the Nyquist amplitudes of reading R17 (Eq. II1).
 #pragma once
 #include "tm_common.cuh"
 #include "tm_special.cuh"
@@ -26,6 +28,8 @@ template <int LMAX> struct GaussNode {
   double tau[LMAX + 1][LMAX + 1];
 };
 
+// kw0 > 0: Gaussian spectral weight G(beta) = (k w0)^2/2 exp(-(k w0 sin beta)^2/4) (reading R9);
+// kw0 <= 0: flat spectrum inside the light cone = jinc source (Eq. II3 with the k_0^2 of d^2k dropped as in Eq. II9).
 template <int LMAX>
 __global__ void k_gauss_nodes(const double* __restrict__ beta, const double* __restrict__ wq, int n_beta, double kw0,
                               GaussNode<LMAX>* __restrict__ nodes) {
@@ -36,34 +40,40 @@ __global__ void k_gauss_nodes(const double* __restrict__ beta, const double* __r
   double P[LMAX + 1][LMAX + 1], PI[LMAX + 1][LMAX + 1], TAU[LMAX + 1][LMAX + 1];
   ang_functions<LMAX>(cb, sb, P, PI, TAU);
   GaussNode<LMAX>& nd = nodes[q];
-  nd.wgt = wq[q] * 0.5 * kw0 * kw0 * exp(-0.25 * kw0 * kw0 * sb * sb) * sb;
+  nd.wgt = wq[q] * (kw0 > 0.0 ? 0.5 * kw0 * kw0 * exp(-0.25 * kw0 * kw0 * sb * sb) : 1.0) * sb;
   nd.cb = cb; nd.sb = sb;
   for (int l = 1; l <= LMAX; ++l)
     for (int m = 0; m <= l; ++m) { nd.pi_[l][m] = PI[l][m]; nd.tau[l][m] = TAU[l][m]; }
 }
 
-// One block (128 threads) per scatterer; threads stride over the beta nodes, each accumulating all L modes.
-//   rel = x_j - focus = (rho_T, phi0, z);  rho = k rho_T sin(beta);  ez = exp(i k z cos(beta))
+// One block (128 threads) per scatterer; threads stride over (source, beta node), each accumulating all L modes.
+//   rel = x_j - source centre = (rho_T, phi0, z);  rho = k rho_T sin(beta);  ez = exp(i k z cos(beta))
 //   Gamma_m(xi, eta, rho) = i^{m-1} e^{-i m xi}/2 [ e^{i(xi-eta)} J_{m-1}(rho) - e^{-i(xi-eta)} J_{m+1}(rho) ]   (II11)
 //   p = 0: -4 i^l     c_l ez [ (i m pi Ax + tau cb Ay) G(0) + (i m pi Ay - tau cb Ax) G(pi/2) ]                    (II15)
 //   p = 1: -4 i^{l+1} c_l ez [ (tau Ax - i m pi cb Ay) G(0) + (tau Ay + i m pi cb Ax) G(pi/2) ]                    (II17)
 template <int LMAX>
 __global__ void __launch_bounds__(128)
-k_incident_gauss(const double* __restrict__ pos, const int* __restrict__ win_of, const double* __restrict__ focus,
-                 const GaussNode<LMAX>* __restrict__ nodes, int n_beta, double k, double2 Ax, double2 Ay,
-                 double2* __restrict__ p) {
+k_incident_gauss(const double* __restrict__ pos, const int* __restrict__ win_of, const double* __restrict__ src,
+                 const double2* __restrict__ amp, const int* __restrict__ src_ptr,
+                 const GaussNode<LMAX>* __restrict__ nodes, int n_beta, double k, double2* __restrict__ p) {
+  // Sources (beam foci or jinc-source centres) of the scatterer's window: src_ptr[w] <= s < src_ptr[w+1], centre src[s],
+  // transverse amplitude (amp[2s], amp[2s+1]).  The block's threads stride over the flattened (source, node) pairs.
   constexpr int L = 2 * LMAX * (LMAX + 2);
   constexpr int LH = L / 2;
   const int j = blockIdx.x;
   const int w = win_of[j];
-  const double rx = pos[3 * j] - focus[3 * w], ry = pos[3 * j + 1] - focus[3 * w + 1], rz = pos[3 * j + 2] - focus[3 * w + 2];
-  const double rhoT = sqrt(rx * rx + ry * ry);
-  const double cph = rhoT > 0.0 ? rx / rhoT : 1.0, sph = rhoT > 0.0 ? ry / rhoT : 0.0;    // e^{i phi0}
+  const int s_lo = src_ptr[w], n_src = src_ptr[w + 1] - s_lo;
   double ar[L], ai[L];
 #pragma unroll
   for (int a = 0; a < L; ++a) { ar[a] = 0.0; ai[a] = 0.0; }
 
-  for (int q = threadIdx.x; q < n_beta; q += blockDim.x) {
+  for (long long it = threadIdx.x; it < (long long)n_src * n_beta; it += blockDim.x) {
+    const int sidx = s_lo + (int)(it / n_beta), q = (int)(it % n_beta);
+    const double rx = pos[3 * j] - src[3 * sidx], ry = pos[3 * j + 1] - src[3 * sidx + 1], rz = pos[3 * j + 2] - src[3 * sidx + 2];
+    const double2 Ax = amp[2 * sidx], Ay = amp[2 * sidx + 1];
+    const double rhoT = sqrt(rx * rx + ry * ry);
+    const double cph = rhoT > 0.0 ? rx / rhoT : 1.0, sph = rhoT > 0.0 ? ry / rhoT : 0.0;    // e^{i phi0}
+    {
     const GaussNode<LMAX>& nd = nodes[q];
     double J[LMAX + 2];
     bessel_j_all<LMAX + 1>(k * rhoT * nd.sb, J);
@@ -129,6 +139,7 @@ k_incident_gauss(const double* __restrict__ pos, const int* __restrict__ win_of,
         ar[a1] += sc * (v1r * fr - v1i * fi); ai[a1] += sc * (v1r * fi + v1i * fr);
       }
     }
+  }
   }
   // block reduction
   __shared__ double s_r[4][2 * L];

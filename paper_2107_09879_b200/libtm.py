@@ -15,7 +15,7 @@ _SO = os.path.join(_HERE, "lib", "libtm.so")
 TM_FP64, TM_FP32 = 0, 1
 TM_OK, TM_NOT_CONVERGED = 0, 1
 TM_E_INVALID, TM_E_OVERLAP, TM_E_STATE, TM_E_CUDA, TM_E_NOMEM = -1, -2, -3, -4, -5
-TM_INC_PLANE, TM_INC_GAUSS, TM_INC_COEFFS = 0, 1, 2
+TM_INC_PLANE, TM_INC_GAUSS, TM_INC_COEFFS, TM_INC_JINC = 0, 1, 2, 3
 TM_FIELD_E_SCA, TM_FIELD_H_SCA = 0, 1
 TM_KERNEL_AUTO, TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR, TM_KERNEL_SYM3D = 0, 1, 2, 3
 
@@ -34,6 +34,11 @@ class PlaneDesc(ctypes.Structure):
 
 class GaussDesc(ctypes.Structure):
     _fields_ = [("focus", ctypes.c_void_p), ("w0", ctypes.c_double), ("Ax", c64), ("Ay", c64), ("n_beta", ctypes.c_int)]
+
+
+class JincDesc(ctypes.Structure):
+    _fields_ = [("n_src", ctypes.c_int), ("src_xyz", ctypes.c_void_p), ("amp", ctypes.c_void_p), ("src_ptr", ctypes.c_void_p),
+                ("n_beta", ctypes.c_int)]
 
 
 class CoeffsDesc(ctypes.Structure):
@@ -181,6 +186,14 @@ class Solver:
         f = np.ascontiguousarray(focus, dtype=np.float64).reshape(self.n_win, 3)
         d = GaussDesc(f.ctypes.data, float(w0), _c64(Ax), _c64(Ay), int(n_beta))
         return self._check(lib().tm_set_incident(self._h, TM_INC_GAUSS, ctypes.addressof(d)))
+
+    def set_incident_jinc(self, src, amp, src_ptr=None, n_beta=0):
+        """Jinc sources (PAPER.md Eqs. II1-II17): src (S,3), amp (S,2) complex transverse amplitudes, src_ptr (n_win+1,)."""
+        src = np.ascontiguousarray(src, dtype=np.float64).reshape(-1, 3)
+        amp = np.ascontiguousarray(amp, dtype=np.complex128).reshape(-1, 2)
+        ptr = np.array([0, src.shape[0]], dtype=np.int32) if src_ptr is None else np.ascontiguousarray(src_ptr, dtype=np.int32)
+        d = JincDesc(int(src.shape[0]), src.ctypes.data, amp.ctypes.data, ptr.ctypes.data, int(n_beta))
+        return self._check(lib().tm_set_incident(self._h, TM_INC_JINC, ctypes.addressof(d)))
 
     def set_incident_coeffs(self, p):
         p = np.ascontiguousarray(p, dtype=np.complex128) if isinstance(p, np.ndarray) else p

@@ -1,0 +1,93 @@
+"""Nyquist-sampled jinc sources and the low-overhead window decomposition (the paper's distribution strategy,
+PAPER.md:27-39, 386-397), on top of the batched-window solver.
+
+The incident field, band-limited to the light cone, is represented by its samples on the lambda/2 grid, each sample
+carried by one jinc source (Eq. II1).  The sources are divided into groups; each group is simulated with only the
+scatterers inside the group's footprint plus a padding (an independent "window"), all windows are batched on one GPU
+(or spread over GPUs as replicas: nothing is exchanged during a solve), and the scattered fields of all windows are
+summed at the end.  Host-side planning only: every field / coefficient / solve runs in libtm.
+"""
+import numpy as np
+
+from . import libtm
+
+
+def sample_grid(k, x_range, y_range):
+    """Nyquist sample coordinates x_i = i lambda/2 covering the ranges: returns (xs, ys)."""
+    h = np.pi / k
+    ix = np.arange(int(np.ceil(x_range[0] / h - 1e-12)), int(np.floor(x_range[1] / h + 1e-12)) + 1)
+    iy = np.arange(int(np.ceil(y_range[0] / h - 1e-12)), int(np.floor(y_range[1] / h + 1e-12)) + 1)
+    return ix * h, iy * h
+
+
+def jinc_sources(k, x_range, y_range, z0, field_fn, drop_below=0.0):
+    """Sources for a transverse field field_fn(x, y) -> (Ex, Ey) sampled on the Nyquist grid at z = z0.
+    A sample E is carried by a unit jinc source (transverse profile J_1(k rho)/(k rho)) of amplitude (pi/2) E: the ideal
+    disc low-pass of the lambda/2 lattice (reading R17).  Returns src (S,3), amp (S,2) complex, grid index (S,2)."""
+    xs, ys = sample_grid(k, x_range, y_range)
+    X, Y = np.meshgrid(xs, ys, indexing="xy")
+    IX, IY = np.meshgrid(np.arange(xs.size), np.arange(ys.size), indexing="xy")
+    Ex, Ey = field_fn(X.ravel(), Y.ravel())
+    amp = 0.5 * np.pi * np.stack([np.asarray(Ex, dtype=complex), np.asarray(Ey, dtype=complex)], axis=1)
+    src = np.stack([X.ravel(), Y.ravel(), np.full(X.size, float(z0))], axis=1)
+    gi = np.stack([IX.ravel(), IY.ravel()], axis=1)
+    keep = np.abs(amp).max(axis=1) > drop_below
+    return src[keep], amp[keep], gi[keep]
+
+
+def plan_windows(pos, src, grid_index, group, padding):
+    """Divide the sources into square groups of `group` x `group` Nyquist samples; the window of a group holds the
+    scatterers inside the group's bounding box grown by `padding` on every side (Fig. 2a).
+    Returns a list of (source indices, scatterer indices); every source belongs to exactly one window."""
+    gx, gy = grid_index[:, 0] // group, grid_index[:, 1] // group
+    plans = []
+    for key in sorted(set(zip(gx.tolist(), gy.tolist()))):
+        sidx = np.nonzero((gx == key[0]) & (gy == key[1]))[0]
+        lo = src[sidx, :2].min(axis=0) - padding
+        hi = src[sidx, :2].max(axis=0) + padding
+        inside = np.all((pos[:, :2] >= lo - 1e-12) & (pos[:, :2] <= hi + 1e-12), axis=1)
+        plans.append((sidx, np.nonzero(inside)[0]))
+    return plans
+
+
+def build_batch(pos, src, amp, plans):
+    """Concatenate the windows into one batched problem: positions (scatterers are duplicated where windows overlap),
+    win_ptr, the global index of every batched scatterer, and the per-window source lists (src_ptr)."""
+    plans = [p for p in plans if p[1].size > 0]
+    scat = np.concatenate([p[1] for p in plans]) if plans else np.zeros(0, dtype=int)
+    win_ptr = np.concatenate([[0], np.cumsum([p[1].size for p in plans])]).astype(np.int32)
+    sord = np.concatenate([p[0] for p in plans]) if plans else np.zeros(0, dtype=int)
+    src_ptr = np.concatenate([[0], np.cumsum([p[0].size for p in plans])]).astype(np.int32)
+    return dict(pos=np.ascontiguousarray(pos[scat]), win_ptr=win_ptr, scat_index=scat,
+                src=np.ascontiguousarray(src[sord]), amp=np.ascontiguousarray(amp[sord]), src_ptr=src_ptr)
+
+
+def simulate(w, src, amp, grid_index, group, padding, pts, tol=1e-8, restart=50, max_iter=5000, precision=libtm.TM_FP64,
+             stream=None):
+    """Distributed simulation of workload `w` (global layout: pos, lmax, k, Mie radii per site or per type) driven by the
+    jinc sources (src, amp): plan windows, batch them, solve once, sum the scattered E fields of all windows at `pts`.
+    group = None: one window with every scatterer and every source (the undistributed reference).
+    Returns (E (M,3), info dict)."""
+    pos = w["pos"]
+    if group is None:
+        plans = [(np.arange(src.shape[0]), np.arange(pos.shape[0]))]
+    else:
+        plans = plan_windows(pos, src, grid_index, group, padding)
+    b = build_batch(pos, src, amp, plans)
+    s = libtm.Solver(b["pos"], w["lmax"], w["k"], win_ptr=b["win_ptr"], precision=precision, stream=stream)
+    type_of = np.asarray(w["type_of"])[b["scat_index"]]
+    if w["t_kind"] in ("mie_types", "mie_sites"):
+        radii = np.asarray(w["radii"])
+        used, inv = np.unique(type_of, return_inverse=True)
+        T = np.stack([libtm.mie_tmatrix(w["lmax"], w["k"], radii[t], w["eps_r"]) for t in used])
+        s.set_tmatrices(T, inv.astype(np.int32), True, r_enclosing=radii[used])
+    else:
+        s.set_tmatrices(w["t_full"], type_of.astype(np.int32), False)
+    s.set_incident_jinc(b["src"], b["amp"], b["src_ptr"])
+    sol, info, rc = s.solve(tol, restart, max_iter)
+    E = s.fields(np.ascontiguousarray(pts, dtype=np.float64), sol, libtm.TM_FIELD_E_SCA)
+    out = dict(n_windows=len(b["win_ptr"]) - 1, n_batched_scatterers=int(b["pos"].shape[0]), rc=rc,
+               iterations=max(i.iterations for i in info), seconds=info[0].seconds,
+               max_rel_residual=max(i.rel_residual for i in info), batch=b, solution=sol)
+    s.close()
+    return E, out
