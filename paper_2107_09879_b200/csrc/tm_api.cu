@@ -297,7 +297,8 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
 
   std::vector<int> h_k(nw), h_done(nw), iters(nw, 0), restarts(nw, 0);
   std::vector<double> h_res(nw, 0.0);
-  int matvecs = 0, total = 0, cycle = 0;
+  int matvecs = 0, total = 0, cycle = 0, stagnant = 0, last_mc = 0;
+  std::vector<double> prev_res(nw, 1e300);
   bool all_ok = false;
   const Cx<R>* resid_vec = B;                         // first cycle: x0 = 0 so r = b
   while (true) {
@@ -318,12 +319,21 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
       }
       total += kmax;
       if (all_ok || total >= o.max_iter || kmax == 0) break;
+      // Precision floor (fp32 mode): every window met the ESTIMATED residual before the cycle ended, yet the true
+      // residual of the unconverged ones no longer improves - further cycles only repeat that.  Stop (soft status).
+      bool floor_hit = kmax < last_mc;
+      for (int w = 0; w < nw && floor_hit; ++w)
+        if (!(h_res[w] <= o.tol) && h_res[w] < 0.9 * prev_res[w]) floor_hit = false;
+      stagnant = floor_hit ? stagnant + 1 : 0;
+      prev_res = h_res;
+      if (stagnant >= 2) break;
     }
     TM_CUDA(cudaMemsetAsync(S.n_active, 0, sizeof(int), st));
     k_gmres_init_cycle<<<wb, 64, 0, st>>>(S, nw, cycle == 0 ? 1 : 0, o.tol);
     k_scale_or_sub<R><<<nc, TM_VT, 0, st>>>(resid_vec, nullptr, S.inv_norm, V, ctx->d_chunks, nullptr);   // V_0 = r / beta
     ctx->total_launches += 4;
     const int mc = std::min(m, o.max_iter - total);
+    last_mc = mc;
     for (int j = 0; j < mc; ++j) {
       Cx<R>* Vj = V + (size_t)j * n;
       TM_CUDA(apply_operator<R>(ctx, transpose, Vj, W, Z, S.n_active));

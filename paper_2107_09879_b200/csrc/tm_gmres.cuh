@@ -48,13 +48,10 @@ __global__ void k_gmres_init_cycle(TmGmresDev S, int n_win, int first, double to
 // One WARP per window (blockDim = 32, grid = n_win): the lanes first reduce the window's chunk norms (fixed order) and
 // stage the column and the previous rotations in shared memory with parallel loads; lane 0 then runs the sequential
 // rotation recurrence out of shared memory.
-__global__ void __launch_bounds__(32)
-k_gmres_givens(TmGmresDev S, int n_win, int j, double tol, const double* __restrict__ normpart,
-               const int* __restrict__ win_chunk_ptr) {
-  const int w = blockIdx.x, lane = threadIdx.x;
-  if (w >= n_win) return;
-  if (*S.n_active == 0 || S.done[w]) return;
-  extern __shared__ double2 s_col[];                  // [j+1] column, then [j] sn, then cs as doubles
+// (called by one full warp; s_col: shared scratch of (2j+2) double2 + (j+1) doubles)
+__device__ __forceinline__ void givens_body(const TmGmresDev& S, int w, int j, double tol, const double* __restrict__ normpart,
+                                            const int* __restrict__ win_chunk_ptr, int lane, double2* s_col) {
+  if (S.done[w]) return;
   double2* s_sn = s_col + (j + 1);
   double* s_cs = reinterpret_cast<double*>(s_sn + j);
   const int ldh = S.ldh;
@@ -105,6 +102,15 @@ k_gmres_givens(TmGmresDev S, int n_win, int j, double tol, const double* __restr
   const bool fin = !(est > tol * bn) || !(hn > 0.0);
   if (fin) { S.done[w] = 1; S.inv_norm[w] = 0.0; atomicSub(S.n_active, 1); }
   else S.inv_norm[w] = 1.0 / hn;
+}
+
+__global__ void __launch_bounds__(32)
+k_gmres_givens(TmGmresDev S, int n_win, int j, double tol, const double* __restrict__ normpart,
+               const int* __restrict__ win_chunk_ptr) {
+  const int w = blockIdx.x;
+  if (w >= n_win || *S.n_active == 0) return;
+  extern __shared__ double2 s_givens[];               // [j+1] column, then [j] sn, then cs as doubles
+  givens_body(S, w, j, tol, normpart, win_chunk_ptr, threadIdx.x, s_givens);
 }
 
 // y = R^{-1} g over the accepted columns.

@@ -93,12 +93,9 @@ k_tapply(int mode, int L, int n_scat, int n_chunk, const Cx<R>* __restrict__ x, 
 // staged in shared memory and every WARP takes whole vectors (lanes stride over the chunk, one shuffle reduction per
 // vector instead of one per vector and warp).
 template <typename R, int EPT>
-__global__ void __launch_bounds__(TM_VT)
-k_dots(const Cx<R>* __restrict__ V, size_t stride, int nvec, const Cx<R>* __restrict__ w,
-       const TmChunk* __restrict__ chunks, int n_chunks, double2* __restrict__ part, const int* __restrict__ n_active) {
-  if (n_active != nullptr && *n_active == 0) return;
-  __shared__ Cx<R> s_w[EPT * TM_VT];
-  const TmChunk ch = chunks[blockIdx.x];
+__device__ __forceinline__ void dots_body(const Cx<R>* __restrict__ V, size_t stride, int nvec, const Cx<R>* __restrict__ w,
+                                          const TmChunk ch, int cidx, int n_chunks, double2* __restrict__ part, int gy, int ngy,
+                                          Cx<R>* s_w) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 #pragma unroll
   for (int k = 0; k < EPT; ++k) {
@@ -106,7 +103,7 @@ k_dots(const Cx<R>* __restrict__ V, size_t stride, int nvec, const Cx<R>* __rest
     s_w[e] = e < ch.count ? w[(size_t)ch.start + e] : cx<R>(R(0), R(0));
   }
   __syncthreads();
-  for (int i = blockIdx.y + warp * gridDim.y; i < nvec; i += gridDim.y * (TM_VT / 32)) {
+  for (int i = gy + warp * ngy; i < nvec; i += ngy * (TM_VT / 32)) {
     const Cx<R>* v = V + (size_t)i * stride + ch.start;
     double sr = 0.0, si = 0.0;
 #pragma unroll
@@ -119,8 +116,17 @@ k_dots(const Cx<R>* __restrict__ V, size_t stride, int nvec, const Cx<R>* __rest
       }
     }
     sr = warp_sum(sr); si = warp_sum(si);
-    if (lane == 0) part[(size_t)i * n_chunks + blockIdx.x] = make_double2(sr, si);
+    if (lane == 0) part[(size_t)i * n_chunks + cidx] = make_double2(sr, si);
   }
+}
+
+template <typename R, int EPT>
+__global__ void __launch_bounds__(TM_VT)
+k_dots(const Cx<R>* __restrict__ V, size_t stride, int nvec, const Cx<R>* __restrict__ w,
+       const TmChunk* __restrict__ chunks, int n_chunks, double2* __restrict__ part, const int* __restrict__ n_active) {
+  if (n_active != nullptr && *n_active == 0) return;
+  __shared__ Cx<R> s_w[EPT * TM_VT];
+  dots_body<R, EPT>(V, stride, nvec, w, chunks[blockIdx.x], blockIdx.x, n_chunks, part, blockIdx.y, gridDim.y, s_w);
 }
 
 // h[win * ldh + i] (+)= sum over the window's chunks of part[i][c].  grid = (nvec, n_win), block = 64.
@@ -151,14 +157,10 @@ __global__ void k_reduce_h(const double2* __restrict__ part, int n_chunks, const
 // Basis vectors must hold finite numbers (the workspace is zeroed at the start of a solve): a zero coefficient
 // multiplies whatever is there.
 template <typename R, int EPT>
-__global__ void __launch_bounds__(TM_VT)
-k_axpy(const Cx<R>* __restrict__ V, size_t stride, int nvec, double2* __restrict__ coef, int ldc, double sign,
-       Cx<R>* __restrict__ w, const TmChunk* __restrict__ chunks, double* __restrict__ normpart,
-       const double2* __restrict__ part, int n_chunks, const int* __restrict__ win_chunk_ptr,
-       const int* __restrict__ n_active) {
-  if (n_active != nullptr && *n_active == 0) return;
-  extern __shared__ double2 s_c[];                   // [nvec]
-  const TmChunk ch = chunks[blockIdx.x];
+__device__ __forceinline__ void axpy_body(const Cx<R>* __restrict__ V, size_t stride, int nvec, double2* __restrict__ coef, int ldc,
+                                          double sign, Cx<R>* __restrict__ w, const TmChunk ch, int cidx,
+                                          double* __restrict__ normpart, const double2* __restrict__ part, int n_chunks,
+                                          const int* __restrict__ win_chunk_ptr, double2* s_c, double* s_n) {
   if (part != nullptr) {
     const int c0 = win_chunk_ptr[ch.win], c1 = win_chunk_ptr[ch.win + 1];
     // 4 lanes per vector, each sums a contiguous quarter of the chunk list; lanes combined in fixed order
@@ -176,7 +178,7 @@ k_axpy(const Cx<R>* __restrict__ V, size_t stride, int nvec, double2* __restrict
       sr += __shfl_xor_sync(0xffffffffu, sr, 2); si += __shfl_xor_sync(0xffffffffu, si, 2);
       if (i < nvec && q == 0) {
         s_c[i] = make_double2(sign * sr, sign * si);
-        if (blockIdx.x == c0) coef[(size_t)ch.win * ldc + i] = make_double2(sr, si);
+        if (cidx == c0) coef[(size_t)ch.win * ldc + i] = make_double2(sr, si);
       }
     }
   } else {
@@ -205,7 +207,6 @@ k_axpy(const Cx<R>* __restrict__ V, size_t stride, int nvec, double2* __restrict
     }
   }
   if (normpart != nullptr) {
-    __shared__ double s_n[TM_VT / 32];
     nrm = warp_sum(nrm);
     if ((threadIdx.x & 31) == 0) s_n[threadIdx.x >> 5] = nrm;
     __syncthreads();
@@ -213,9 +214,22 @@ k_axpy(const Cx<R>* __restrict__ V, size_t stride, int nvec, double2* __restrict
       double t = 0.0;
 #pragma unroll
       for (int k = 0; k < TM_VT / 32; ++k) t += s_n[k];
-      normpart[blockIdx.x] = t;
+      normpart[cidx] = t;
     }
   }
+}
+
+template <typename R, int EPT>
+__global__ void __launch_bounds__(TM_VT)
+k_axpy(const Cx<R>* __restrict__ V, size_t stride, int nvec, double2* __restrict__ coef, int ldc, double sign,
+       Cx<R>* __restrict__ w, const TmChunk* __restrict__ chunks, double* __restrict__ normpart,
+       const double2* __restrict__ part, int n_chunks, const int* __restrict__ win_chunk_ptr,
+       const int* __restrict__ n_active) {
+  if (n_active != nullptr && *n_active == 0) return;
+  extern __shared__ double2 s_c[];                   // [nvec]
+  __shared__ double s_n[TM_VT / 32];
+  axpy_body<R, EPT>(V, stride, nvec, coef, ldc, sign, w, chunks[blockIdx.x], blockIdx.x, normpart, part, n_chunks,
+                    win_chunk_ptr, s_c, s_n);
 }
 
 // normpart[c] = sum |v|^2 over chunk c

@@ -1,0 +1,119 @@
+"""GPU edge cases: degenerate sizes, empty / single-scatterer windows, zero right-hand side, extreme solver options,
+maximum lmax of each kernel.  Every result is compared with the oracle."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from oracle import driver, matvec as omv, tmatrix  # noqa: E402
+from paper_2107_09879_b200 import workloads as W  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def tm():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2107_09879_b200 import libtm
+    libtm.lib()
+    return libtm
+
+
+def rel(a, b):
+    return np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(b)
+
+
+def rand_x(shape, seed):
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+
+
+def test_single_scatterer_is_mie(tm):
+    """N = 1: A = 0, so s = T p exactly (closed-form Mie response) and GMRES stops after one step."""
+    pos = np.array([[0.3, -0.2, 0.1]])
+    for lmax in (1, 2, 3):
+        s = tm.Solver(pos, lmax, W.K_B)
+        t = tm.mie_tmatrix(lmax, W.K_B, 0.2, 4.0)
+        s.set_tmatrices(t[None, :], np.zeros(1, dtype=np.int32), True)
+        s.set_incident_plane(0.3, 0.7, 1.0, 0.5j)
+        sol, info, rc = s.solve(1e-12, 10, 10)
+        ref = tmatrix.mie_tmatrix_diag(lmax, W.K_B, 0.2, 4.0) * s.get_incident()[0]
+        assert rc == 0 and info[0].iterations <= 1 and rel(sol[0], ref) <= 1e-13
+        assert np.all(s.matvec(rand_x((1, s.L), 1), transpose=2) == 0)
+        s.close()
+
+
+def test_empty_and_singleton_windows(tm):
+    """win_ptr with an empty window and a one-scatterer window between two real ones."""
+    w = W.cloud_workload(41, seed=9, lmax=2, planar=True)
+    wp = np.array([0, 20, 20, 21, 41], dtype=np.int32)
+    w["win_ptr"] = wp
+    ref = driver.solve(w)
+    s = tm.solver_for_workload(w)
+    sol, info, rc = s.solve(1e-11, 30, 500)
+    assert rc == 0 and len(info) == 4 and info[1].iterations == 0 and info[1].converged
+    assert rel(sol, ref["s"]) <= 1e-9
+    x = rand_x(sol.shape, 3)
+    assert rel(s.matvec(x, 2), omv.matvec_rows(2, w["k"], w["pos"], x, win_ptr=wp)) <= 1e-12
+    s.close()
+
+
+def test_zero_incident_gives_zero_solution(tm):
+    w = W.config(1)
+    s = tm.solver_for_workload(w)
+    s.set_incident_coeffs(np.zeros((16, 16), dtype=np.complex128))
+    sol, info, rc = s.solve(1e-10, 20, 100)
+    assert rc == 0 and info[0].converged and info[0].iterations == 0 and np.all(sol == 0)
+    lam, info2, rc2 = s.solve_adjoint(np.zeros((16, 16), dtype=np.complex128), 1e-10, 20, 100)
+    assert rc2 == 0 and np.all(lam == 0)
+    s.close()
+
+
+def test_short_and_long_restart_agree(tm):
+    """GMRES(8) with many restarts and unrestarted GMRES reach the same solution."""
+    w = W.config(1)
+    ref = driver.solve(w)
+    s = tm.solver_for_workload(w)
+    a, ia, rca = s.solve(1e-10, 300, 300)
+    b, ib, rcb = s.solve(1e-10, 8, 20000)
+    assert rca == 0 and ia[0].restarts == 1 and rel(a, ref["s"]) <= 1e-9
+    assert rcb == 0 and ib[0].iterations > ia[0].iterations and rel(b, ref["s"]) <= 1e-9
+    with pytest.raises(tm.TmError):
+        s.solve(1e-10, 301, 10)                       # restart above the supported maximum
+    with pytest.raises(tm.TmError):
+        s.solve(0.0, 10, 10)
+    s.close()
+
+
+@pytest.mark.parametrize("lmax", [5, 6])
+def test_table_kernel_at_maximum_lmax(tm, lmax):
+    """lmax = 6 is the paper's own truncation: L = 96, table-driven kernel, 3 rows per lane."""
+    pos = W.random_cloud(12, seed=60 + lmax)
+    x = rand_x((12, W.n_modes(lmax)), lmax)
+    s = tm.Solver(pos, lmax, W.K_B)
+    assert s.get_kernel() == tm.TM_KERNEL_GENERAL
+    assert rel(s.matvec(x, 2), omv.matvec_rows(lmax, W.K_B, pos, x)) <= 1e-12
+    with pytest.raises(tm.TmError):
+        s.set_kernel(tm.TM_KERNEL_SYM3D)
+    s.close()
+
+
+def test_lmax6_solve_small(tm):
+    w = W.cloud_workload(8, seed=66, lmax=6, planar=True)
+    ref = driver.solve(w)
+    s = tm.solver_for_workload(w)
+    assert s.get_kernel() == tm.TM_KERNEL_GENERAL        # planar but lmax > 3
+    p = s.get_incident()
+    assert rel(p, ref["p"]) <= 1e-13
+    sol, info, rc = s.solve(1e-11, 60, 600)
+    assert rc == 0 and rel(sol, ref["s"]) <= 1e-9
+    s.close()
+
+
+def test_far_apart_and_close_pairs(tm):
+    """k r from 1.9 (nearly touching small spheres) to 6e4 (phase accuracy at long range)."""
+    pos = np.array([[0.0, 0.0, 0.0], [0.3, 0.0, 0.0], [9000.0, 4000.0, 0.0], [0.0, 0.31, 0.0]])
+    x = rand_x((4, 30), 8)
+    ref = omv.matvec_rows(3, W.K_B, pos, x)
+    s = tm.Solver(pos, 3, W.K_B)
+    assert rel(s.matvec(x, 2), ref) <= 1e-11             # k r = 6e4: 6e4 * 1.1e-16 phase rounding on both sides
+    s.close()
