@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "tm_allpairs.cuh"
+#include "tm_arnoldi.cuh"
 #include "tm_common.cuh"
 #include "tm_fields.cuh"
 #include "tm_gmres.cuh"
@@ -300,6 +301,20 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
   int matvecs = 0, total = 0, cycle = 0, stagnant = 0, last_mc = 0;
   std::vector<double> prev_res(nw, 1e300);
   bool all_ok = false;
+  // cooperative single-launch Arnoldi step: only when every chunk's block can be resident at once
+  bool coop = false;
+  if (ctx->max_chunks_per_win <= 512 && !std::getenv("TM_NO_COOP")) {
+    int per_sm = 0, dev = 0, n_sm = 0, can = 0;
+    const void* fn = ctx->ept == 1 ? (const void*)k_arnoldi_fused<R, 1> : (const void*)k_arnoldi_fused<R, 4>;
+    const size_t sm_max = (size_t)(2 * m + 2) * sizeof(double2) + (size_t)(m + 1) * sizeof(double);
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&can, cudaDevAttrCooperativeLaunch, dev);
+    if (ctx->ept == 1) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_arnoldi_fused<R, 1>, TM_VT, sm_max);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_arnoldi_fused<R, 4>, TM_VT, sm_max);
+    coop = can && (long long)per_sm * n_sm >= nc;
+    (void)fn;
+  }
   const Cx<R>* resid_vec = B;                         // first cycle: x0 = 0 so r = b
   while (true) {
     // beta = ||r|| per window
@@ -355,16 +370,26 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
     if (ctx->ept == 1) k_axpy<R, 1><<<nc, TM_VT, sm_a, st>>>(V, n, j + 1, H, S.ldh, -1.0, W, ctx->d_chunks, NP, pp, nc, ctx->d_win_chunk_ptr, S.n_active); \
     else k_axpy<R, 4><<<nc, TM_VT, sm_a, st>>>(V, n, j + 1, H, S.ldh, -1.0, W, ctx->d_chunks, NP, pp, nc, ctx->d_win_chunk_ptr, S.n_active); \
   } while (0)
-      TM_DOTS(S.h1);
-      TM_AXPY(S.h1, nullptr);
-      TM_DOTS(S.h2);
-      TM_AXPY(S.h2, ctx->gm.normpart);
+      const size_t sm_g = (size_t)(2 * j + 2) * sizeof(double2) + (size_t)(j + 1) * sizeof(double);
+      if (coop) {            // whole step in one cooperative launch (all chunks co-resident)
+        const Cx<R>* Vc = V; size_t nn = n; int jj = j, ncc = nc, nww = nw; double tl = o.tol;
+        Cx<R>* Wc = W; const TmChunk* chk = ctx->d_chunks; double2* prt = ctx->gm.part; double* npt = ctx->gm.normpart;
+        const int* wcp = ctx->d_win_chunk_ptr; TmGmresDev Sc = S;
+        void* args[] = {&Vc, &nn, &jj, &Wc, &chk, &ncc, &prt, &npt, &wcp, &Sc, &nww, &tl};
+        const void* fn = ctx->ept == 1 ? (const void*)k_arnoldi_fused<R, 1> : (const void*)k_arnoldi_fused<R, 4>;
+        TM_CUDA(cudaLaunchCooperativeKernel(fn, dim3(nc), dim3(TM_VT), args, std::max(sm_a, sm_g), st));
+        ctx->total_launches += 1;
+      } else {
+        TM_DOTS(S.h1);
+        TM_AXPY(S.h1, nullptr);
+        TM_DOTS(S.h2);
+        TM_AXPY(S.h2, ctx->gm.normpart);
+        k_gmres_givens<<<nw, 32, sm_g, st>>>(S, nw, j, o.tol, ctx->gm.normpart, ctx->d_win_chunk_ptr);
+        k_scale_or_sub<R><<<nc, TM_VT, 0, st>>>(W, nullptr, S.inv_norm, V + (size_t)(j + 1) * n, ctx->d_chunks, S.n_active);
+        ctx->total_launches += fuse ? 6 : 8;
+      }
 #undef TM_DOTS
 #undef TM_AXPY
-      k_gmres_givens<<<nw, 32, (size_t)(2 * j + 2) * sizeof(double2) + (size_t)(j + 1) * sizeof(double), st>>>(
-          S, nw, j, o.tol, ctx->gm.normpart, ctx->d_win_chunk_ptr);
-      k_scale_or_sub<R><<<nc, TM_VT, 0, st>>>(W, nullptr, S.inv_norm, V + (size_t)(j + 1) * n, ctx->d_chunks, S.n_active);
-      ctx->total_launches += fuse ? 6 : 8;
     }
     // x += V y ; r = b - M x
     k_gmres_solve_y<<<wb, 64, 0, st>>>(S, nw);
