@@ -450,8 +450,10 @@ def emit_general_sym(lmaxes, path):
             for sct, (slots, rows) in enumerate(general_sym(lmax)):
                 n = len(slots)
                 f.write(f"// lmax={lmax} sector={sct}: slots (l,|m|,p,kind) {slots}\n")
+                f.write("// q-outer order: Pbar_q^mu is produced level by level (recurrence in q) and dies after its level, so the\n")
+                f.write("// live state is x^new, the row sums u and two Legendre levels (no spills at 255 registers).\n")
                 f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
-                        f"tm_g3d_pair_L{lmax}_S{sct}(const R* __restrict__ xs, const R* cm, const R* sm, const R* hr, const R* hi, const R* P, R* ar, R* ai) {{\n")
+                        f"tm_g3d_pair_L{lmax}_S{sct}(const R* __restrict__ xs, const R* cm, const R* sm, const R* hr, const R* hi, R ct, R st, R* ar, R* ai) {{\n")
                 k = 0
                 n_pairs = n_zero = 0
                 while k < n:
@@ -459,20 +461,30 @@ def emit_general_sym(lmaxes, path):
                     if kind == "0":
                         f.write(f"  const R xr{k} = xs[{2 * k}], xi{k} = xs[{2 * k + 1}];\n")
                         n_zero += 1
-                        k += 1
                     else:
-                        # '+' and '-' partners of a (l,am,p) pair live in DIFFERENT sectors here: the rotation needs d^+ and d^-
-                        # of the same (l,am,p), so the kernel stages both (slot k: this sector's, slot n + k: the partner's)
                         f.write(f"  const R xr{k} = xs[{2 * k}] * cm[{am}] - xs[{2 * (n + k) + 1}] * sm[{am}], "
                                 f"xi{k} = xs[{2 * k + 1}] * cm[{am}] + xs[{2 * (n + k)}] * sm[{am}];\n")
                         n_pairs += 1
-                        k += 1
-                nterm = nrc = nrowq = 0
+                    k += 1
                 for r in range(n):
-                    l, am, p, kind = slots[r]
-                    f.write("  {\n    R ur = R(0), ui = R(0), zr, zi, rho;\n")
-                    first_q = True
-                    for q in range(nq):
+                    f.write(f"  R ur{r} = R(0), ui{r} = R(0);\n")
+                nterm = nrc = nrowq = 0
+                for q in range(nq):
+                    f.write("  {\n")
+                    # Legendre level q: P{q}_{mu}, mu = 0..q
+                    for mu in range(0, q + 1):
+                        if q == 0:
+                            f.write(f"    const R P0_0 = R({lit(mp.sqrt(mp.mpf(1) / 2))});\n")
+                        elif mu == q:
+                            f.write(f"    const R P{q}_{mu} = R({lit(mp.sqrt(mp.mpf(2 * mu + 1) / (2 * mu)))}) * st * P{q - 1}_{mu - 1};\n")
+                        elif mu == q - 1:
+                            f.write(f"    const R P{q}_{mu} = R({lit(mp.sqrt(mp.mpf(2 * mu + 3)))}) * ct * P{q - 1}_{mu};\n")
+                        else:
+                            a_ = mp.sqrt(mp.mpf(4 * q * q - 1) / (q * q - mu * mu))
+                            b_ = mp.sqrt(mp.mpf((q - 1) ** 2 - mu * mu) / (4 * (q - 1) ** 2 - 1))
+                            f.write(f"    const R P{q}_{mu} = R({lit(a_)}) * (ct * P{q - 1}_{mu} - R({lit(b_)}) * P{q - 2}_{mu});\n")
+                    f.write("    R zr, zi, rho;\n")
+                    for r in range(n):
                         ent = rows[r][q]
                         if not ent:
                             continue
@@ -482,31 +494,26 @@ def emit_general_sym(lmaxes, path):
                             expr = None
                             for (mu, v) in lst:
                                 nterm += 1
-                                if expr is None:
-                                    expr = f"R({lit(v)}) * P[{q * (q + 1) // 2 + mu}]"
-                                else:
-                                    expr = f"fma(R({lit(v)}), P[{q * (q + 1) // 2 + mu}], {expr})"
+                                expr = f"R({lit(v)}) * P{q}_{mu}" if expr is None else f"fma(R({lit(v)}), P{q}_{mu}, {expr})"
                             f.write(f"    rho = {expr};\n")
                             if t == 0:
                                 f.write(f"    zr = rho * xr{c}; zi = rho * xi{c};\n")
                             else:
                                 f.write(f"    zr = fma(rho, xr{c}, zr); zi = fma(rho, xi{c}, zi);\n")
-                        if first_q:
-                            f.write(f"    ur = hr[{q}] * zr; ur = fma(-hi[{q}], zi, ur); ui = hr[{q}] * zi; ui = fma(hi[{q}], zr, ui);\n")
-                            first_q = False
-                        else:
-                            f.write(f"    ur = fma(hr[{q}], zr, ur); ur = fma(-hi[{q}], zi, ur); ui = fma(hr[{q}], zi, ui); ui = fma(hi[{q}], zr, ui);\n")
-                    # output: this sector's u^new_r feeds A^same (cos) and the PARTNER sector's accumulator (sin):
-                    #   A^+ += c u^+ - i s u^- ;  A^- += c u^- - i s u^+   -> ar/ai hold [own n slots | partner n slots]
+                        f.write(f"    ur{r} = fma(hr[{q}], zr, ur{r}); ur{r} = fma(-hi[{q}], zi, ur{r}); ui{r} = fma(hr[{q}], zi, ui{r}); ui{r} = fma(hi[{q}], zr, ui{r});\n")
+                    # nested scopes keep level q-1 and q-2 visible: close nothing here (levels are declared in nested blocks)
+                # output rotation: this sector's u^new_r feeds A^own (cos) and the PARTNER sector's accumulator (sin):
+                #   A^+ += c u^+ - i s u^- ;  A^- += c u^- - i s u^+   -> ar/ai hold [own n slots | partner n slots]
+                for r in range(n):
+                    l, am, p, kind = slots[r]
                     if kind == "0":
-                        f.write(f"    ar[{r} * AS] += ur; ai[{r} * AS] += ui;\n")
+                        f.write(f"    ar[{r} * AS] += ur{r}; ai[{r} * AS] += ui{r};\n")
                     else:
-                        f.write(f"    ar[{r} * AS] = fma(ur, cm[{am}], ar[{r} * AS]); ai[{r} * AS] = fma(ui, cm[{am}], ai[{r} * AS]);\n")
-                        f.write(f"    ar[{n + r} * AS] = fma(ui, sm[{am}], ar[{n + r} * AS]); ai[{n + r} * AS] = fma(-ur, sm[{am}], ai[{n + r} * AS]);\n")
-                    f.write("  }\n")
-                f.write("}\n")
+                        f.write(f"    ar[{r} * AS] = fma(ur{r}, cm[{am}], ar[{r} * AS]); ai[{r} * AS] = fma(ui{r}, cm[{am}], ai[{r} * AS]);\n")
+                        f.write(f"    ar[{n + r} * AS] = fma(ui{r}, sm[{am}], ar[{n + r} * AS]); ai[{n + r} * AS] = fma(-ur{r}, sm[{am}], ai[{n + r} * AS]);\n")
+                f.write("  " + "}" * nq + "\n}\n")
                 inst = nterm + 2 * nrc + 4 * nrowq + 4 * n_pairs + 4 * n_pairs + 2 * n_zero
-                flop = (2 * nterm - nrc) + (4 * nrc - 2 * nrowq) + (8 * nrowq - 2 * n) + 6 * n_pairs + 8 * n_pairs + 2 * n_zero
+                flop = (2 * nterm - nrc) + (4 * nrc - 2 * nrowq) + 8 * nrowq + 6 * n_pairs + 8 * n_pairs + 2 * n_zero
                 cost[0] += inst
                 cost[1] += flop
                 print(f"lmax={lmax} sector={sct}: n={n} terms={nterm} (row,col,q)={nrc} (row,q)={nrowq} -> {inst} FP instructions, {flop} flop",

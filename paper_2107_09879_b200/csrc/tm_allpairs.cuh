@@ -274,7 +274,7 @@ k_allpairs_general(const double* __restrict__ pos, const Cx<R>* __restrict__ x, 
 // the pair's azimuth, exploit the mirror y' -> -y' of the rotated pair (+- basis), never form the block:
 //     u^new_r = sum_q h_q(kr) sum_c ( sum_mu kappa Pbar_q^mu(cos theta) ) x^new_c      (kappa real constants)
 // but without the z-mirror: the L modes split into two SECTORS of L/2 (blockIdx.z, slowest grid dimension).
-// Thread = target; x^new (L/2 complex), Pbar (NQ(NQ+1)/2 reals) and h_q in registers; the accumulators
+// Thread = target; x^new (L/2 complex), the row sums, h_q and two levels of the Legendre recurrence in registers; the accumulators
 // (own sector's A and the partner sector's share produced by the output rotation: L complex) live in shared memory
 // [slot][thread] (conflict-free).  Each sector writes its share of u to its own partial buffer
 // u_part[(chunk * 2 + sector)][n_scat][L]; the finishing kernel adds them in fixed order.
@@ -285,8 +285,8 @@ template <typename R, int LMAX, int S> struct G3dPair;
   template <typename R> struct G3dPair<R, LM, SS_> {                                                     \
     template <int AS>                                                                                    \
     static __device__ __forceinline__ void run(const R* xs, const R* cm, const R* sm, const R* hr,       \
-                                               const R* hi, const R* P, R* ar, R* ai) {                  \
-      tm_g3d_pair_L##LM##_S##SS_<R, AS>(xs, cm, sm, hr, hi, P, ar, ai);                                  \
+                                               const R* hi, R ct, R st, R* ar, R* ai) {                  \
+      tm_g3d_pair_L##LM##_S##SS_<R, AS>(xs, cm, sm, hr, hi, ct, st, ar, ai);                             \
     }                                                                                                    \
     template <int AS>                                                                                    \
     static __device__ __forceinline__ void unmix(const R* ar, const R* ai, Cx<R>* out) {                 \
@@ -298,11 +298,6 @@ template <typename R, int LMAX, int S> struct G3dPair;
   };
 TM_G3D_SPEC(1, 0) TM_G3D_SPEC(1, 1) TM_G3D_SPEC(2, 0) TM_G3D_SPEC(2, 1) TM_G3D_SPEC(3, 0) TM_G3D_SPEC(3, 1)
 #undef TM_G3D_SPEC
-
-template <int LMAX> struct PbarAll;
-template <> struct PbarAll<1> { template <typename R> static __device__ __forceinline__ void run(R ct, R st, R* P) { tm_pbar_all_L1<R>(ct, st, P); } };
-template <> struct PbarAll<2> { template <typename R> static __device__ __forceinline__ void run(R ct, R st, R* P) { tm_pbar_all_L2<R>(ct, st, P); } };
-template <> struct PbarAll<3> { template <typename R> static __device__ __forceinline__ void run(R ct, R st, R* P) { tm_pbar_all_L3<R>(ct, st, P); } };
 
 template <typename R, int LMAX, int TJ, int SS> struct Sym3dSmem {
   static constexpr int L = 2 * LMAX * (LMAX + 2);
@@ -317,7 +312,6 @@ k_allpairs_sym3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
   constexpr int L = 2 * LMAX * (LMAX + 2);
   constexpr int NS = L / 2;                 // slots per sector
   constexpr int NQ = 2 * LMAX + 1;
-  constexpr int NP = NQ * (NQ + 1) / 2;
   if (n_active != nullptr && *n_active == 0) return;
 
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -389,11 +383,10 @@ k_allpairs_sym3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
       phase_kr<R>(k_over_pi, r, ck, sk);
       R hr[NQ], hi[NQ];
       hankel_up<R, NQ>((R)(rinv * inv_k), ck, sk, hr, hi);
-      R P[NP];
-      PbarAll<LMAX>::template run<R>((R)(dz * rinv), (R)(rho2 * rhoinv * rinv), P);
+      const R ct = (R)(dz * rinv), st = (R)(rho2 * rhoinv * rinv);      // cos / sin of the polar angle of d
       const R* xs = &s_x[s * L * 2];
-      if (sct == 0) G3dPair<R, LMAX, 0>::template run<TJ>(xs, cm, sm, hr, hi, P, ar, ai);
-      else          G3dPair<R, LMAX, 1>::template run<TJ>(xs, cm, sm, hr, hi, P, ar, ai);
+      if (sct == 0) G3dPair<R, LMAX, 0>::template run<TJ>(xs, cm, sm, hr, hi, ct, st, ar, ai);
+      else          G3dPair<R, LMAX, 1>::template run<TJ>(xs, cm, sm, hr, hi, ct, st, ar, ai);
     }
   }
   if (live) {

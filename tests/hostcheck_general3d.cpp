@@ -31,8 +31,7 @@ int main() {
     const double f = (2 * q + 1) * t, nr = f * hr[q] - pr, ni = f * hi[q] - pi;
     pr = hr[q]; pi = hi[q]; hr[q + 1] = nr; hi[q + 1] = ni;
   }
-  double P[NQ * (NQ + 1) / 2];
-  CAT1(tm_pbar_all_L, LMAX)<double>(dz / r, rho / r, P);
+  const double ct = dz / r, st = rho / r;
   for (int sct = 0; sct < 2; ++sct) {
     const int* sa = sct ? CAT(tm_g3d_sa_L, LMAX, _S, 1) : CAT(tm_g3d_sa_L, LMAX, _S, 0);
     const int* sb = sct ? CAT(tm_g3d_sb_L, LMAX, _S, 1) : CAT(tm_g3d_sb_L, LMAX, _S, 0);
@@ -47,8 +46,8 @@ int main() {
     }
     C part[L];
     for (int i = 0; i < L; ++i) part[i].re = part[i].im = 0.0;
-    if (sct == 0) { CAT(tm_g3d_pair_L, LMAX, _S, 0)<double, 1>(xs, cm, sm, hr, hi, P, ar, ai); CAT(tm_g3d_unmix_L, LMAX, _S, 0)<double, C, 1>(ar, ai, part); }
-    else { CAT(tm_g3d_pair_L, LMAX, _S, 1)<double, 1>(xs, cm, sm, hr, hi, P, ar, ai); CAT(tm_g3d_unmix_L, LMAX, _S, 1)<double, C, 1>(ar, ai, part); }
+    if (sct == 0) { CAT(tm_g3d_pair_L, LMAX, _S, 0)<double, 1>(xs, cm, sm, hr, hi, ct, st, ar, ai); CAT(tm_g3d_unmix_L, LMAX, _S, 0)<double, C, 1>(ar, ai, part); }
+    else { CAT(tm_g3d_pair_L, LMAX, _S, 1)<double, 1>(xs, cm, sm, hr, hi, ct, st, ar, ai); CAT(tm_g3d_unmix_L, LMAX, _S, 1)<double, C, 1>(ar, ai, part); }
     for (int i = 0; i < L; ++i) { u[i].re += part[i].re; u[i].im += part[i].im; }
   }
   for (int i = 0; i < L; ++i) printf("%.17g %.17g\n", u[i].re, u[i].im);
