@@ -350,6 +350,36 @@ def run_ours(args, w, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_nyquist(args, w):
+    """Recorded run of the paper's distribution strategy (NEXT-1; not the contract line): a Gaussian beam sampled on the
+    lambda/2 grid -> jinc sources -> groups + padded windows batched on one GPU -> summed fields, against the undistributed
+    solve of the same sources."""
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2107_09879_b200 import nyquist
+    half = float(np.abs(w["pos"][:, 0]).max()) + 0.25
+    w0 = half / 2.0
+    field = lambda x, y: (np.exp(-(x * x + y * y) / w0 ** 2), np.zeros_like(x))
+    src, amp, gi = nyquist.jinc_sources(w["k"], (-half, half), (-half, half), 0.0, field, drop_below=1e-6)
+    g = np.linspace(-half, half, 33)
+    pts = np.array([[a, b, 5.0] for a in g for b in g])
+    out = {"mode": "nyquist", "workload": w["name"], "n_scat": int(w["pos"].shape[0]), "n_sources": int(src.shape[0]),
+           "group_samples": args.group, "padding": args.padding, "tol": args.tol or 1e-8}
+    t0 = time.perf_counter()
+    E, inf = nyquist.simulate(w, src, amp, gi, args.group, args.padding, pts, tol=args.tol or 1e-8)
+    torch.cuda.synchronize()
+    out.update(distributed={"n_windows": inf["n_windows"], "batched_scatterers": inf["n_batched_scatterers"], "iterations": inf["iterations"],
+                            "solve_seconds": inf["seconds"], "wall_seconds": time.perf_counter() - t0, "max_rel_residual": inf["max_rel_residual"],
+                            "converged": inf["rc"] == 0})
+    t0 = time.perf_counter()
+    E0, inf0 = nyquist.simulate(w, src, amp, gi, None, 0.0, pts, tol=args.tol or 1e-8)
+    torch.cuda.synchronize()
+    out.update(undistributed={"iterations": inf0["iterations"], "solve_seconds": inf0["seconds"], "wall_seconds": time.perf_counter() - t0,
+                              "converged": inf0["rc"] == 0},
+               field_rel_l2_error=float(np.linalg.norm(E - E0) / np.linalg.norm(E0)))
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -357,7 +387,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2")
-    ap.add_argument("--mode", default="full", choices=["full", "matvec"], help="matvec: time operator applications only")
+    ap.add_argument("--mode", default="full", choices=["full", "matvec", "nyquist"],
+                    help="matvec: time operator applications only; nyquist: recorded run of the window decomposition")
+    ap.add_argument("--group", type=int, default=16, help="nyquist mode: samples per group side")
+    ap.add_argument("--padding", type=float, default=4.0, help="nyquist mode: padding in wavelengths")
     ap.add_argument("--kernel", default="auto", choices=["auto", "general", "coplanar", "sym3d"], help="force the all-pairs kernel variant")
     ap.add_argument("--scale", type=int, default=None, help="lattice side override (parity-size runs)")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
@@ -377,7 +410,10 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     name = args.workload[3:] if args.workload.startswith("cfg") else args.workload
     w = W.config(name if name == "3b" else int(name), scale=args.scale)
-    if args.impl == "reference":
+    if args.mode == "nyquist":
+        if rank == 0:
+            run_nyquist(args, w)
+    elif args.impl == "reference":
         run_reference(args, w, rank, world)
     else:
         run_ours(args, w, rank, world, local_rank)
