@@ -148,6 +148,19 @@ int tm_get_kernel(const tm_ctx *ctx);
 int tm_kernel_time(tm_ctx *ctx, int reset, double *allpairs_ms, long long *allpairs_launches,
                    long long *total_launches);
 
+/* Geometry sensitivities through one adjoint solve (Appendix IV, Eqs. IV7-IV9).  For the bilinear
+ * functional J = w^T s (Eq. IV3/IV4) and lambda from tm_solve_adjoint(w), a geometry parameter p of scatterer j changes
+ * only T_j, and   dJ/dp = lambda_j^T (dT_j/dp) T_j^{-1} s_j = lambda_j^T (dT_j/dp) (p_j + (A s)_j).
+ *   dT      derivative of every TYPE's T-matrix with respect to its parameter, same layout as T in tm_set_tmatrices
+ *   lambda, s  [n_scat][L] (host or device): adjoint and forward solutions
+ *   out     [n_scat] complex: out[j] = lambda_j^T dT_{type(j)} (p_j + (A s)_j); for a parameter shared by a type, sum
+ *           out over the sites of the type.  One all-pairs matvec + one small kernel.  Needs T and the incident field. */
+int tm_grad_tmatrix(tm_ctx *ctx, const tm_c64 *dT, const tm_c64 *lambda, const tm_c64 *s, tm_c64 *out);
+
+/* Host helper: d(diag T)/dR of the Mie T-matrix of tm_mie_tmatrix (Richardson-extrapolated central differences of the
+ * closed form, relative accuracy ~1e-10), out[L]. */
+int tm_mie_tmatrix_dR(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64 *out);
+
 /* Executed floating-point work of the active all-pairs kernel per ORDERED pair:
  * fp_instructions = FMA/MUL/ADD issue slots on the FP64 (or FP32) pipe, flop with FMA = 2.  Counted from the
  * generated straight-line code (coplanar kernel; per-pair geometry excluded, so rooflines are conservative) or

@@ -1049,6 +1049,63 @@ int tm_fields(tm_ctx* ctx, int n_pts, const double* pts, const tm_c64* s, int wh
   return TM_OK;
 }
 
+int tm_grad_tmatrix(tm_ctx* ctx, const tm_c64* dT, const tm_c64* lambda, const tm_c64* s, tm_c64* out) {
+  if (!ctx) return TM_E_INVALID;
+  if (!dT || !lambda || !s || !out) return fail(ctx, TM_E_INVALID, "NULL argument");
+  if (!ctx->has_T || !ctx->has_inc) return fail(ctx, TM_E_STATE, "tm_set_tmatrices and tm_set_incident must be called first");
+  const size_t count = (size_t)ctx->n_types * ctx->L * (ctx->diag ? 1 : ctx->L);
+  void* d_dT = nullptr; double2* d_tmp = nullptr; double2* d_out = nullptr;
+  cudaError_t e = cudaMalloc(&d_dT, count * elem_bytes(ctx));
+  if (e == cudaSuccess) e = cudaMalloc(&d_tmp, count * sizeof(double2));
+  if (e == cudaSuccess) e = cudaMalloc(&d_out, (size_t)ctx->n_scat * sizeof(double2));
+  if (e == cudaSuccess) e = copy_in(d_tmp, dT, count * sizeof(double2), ctx->stream);
+  const bool f64 = ctx->precision == TM_FP64;
+  if (e == cudaSuccess) {
+    if (f64) k_from_c64<double><<<grid_for(count, 256), 256, 0, ctx->stream>>>(reinterpret_cast<const double*>(d_tmp), reinterpret_cast<Cx<double>*>(d_dT), count);
+    else k_from_c64<float><<<grid_for(count, 256), 256, 0, ctx->stream>>>(reinterpret_cast<const double*>(d_tmp), reinterpret_cast<Cx<float>*>(d_dT), count);
+    e = cudaGetLastError();
+  }
+  // v0 = s ; v1 = A s ; v2 = lambda
+  if (e == cudaSuccess) e = f64 ? load_c64<double>(ctx, s, vec<double>(ctx, 0)) : load_c64<float>(ctx, s, vec<float>(ctx, 0));
+  if (e == cudaSuccess) e = f64 ? apply_operator<double>(ctx, 2, vec<double>(ctx, 0), vec<double>(ctx, 1), vec<double>(ctx, 2), nullptr)
+                                : apply_operator<float>(ctx, 2, vec<float>(ctx, 0), vec<float>(ctx, 1), vec<float>(ctx, 2), nullptr);
+  if (e == cudaSuccess) e = f64 ? load_c64<double>(ctx, lambda, vec<double>(ctx, 2)) : load_c64<float>(ctx, lambda, vec<float>(ctx, 2));
+  if (e == cudaSuccess) {
+    const int grid = (ctx->n_scat + 3) / 4;
+    if (f64) k_grad_tmatrix<double><<<grid, 128, 0, ctx->stream>>>(ctx->L, ctx->n_scat, vec<double>(ctx, 1), ctx->d_p, vec<double>(ctx, 2),
+                                                                  reinterpret_cast<Cx<double>*>(d_dT), ctx->diag, ctx->d_type_of, d_out);
+    else k_grad_tmatrix<float><<<grid, 128, 0, ctx->stream>>>(ctx->L, ctx->n_scat, vec<float>(ctx, 1), ctx->d_p, vec<float>(ctx, 2),
+                                                              reinterpret_cast<Cx<float>*>(d_dT), ctx->diag, ctx->d_type_of, d_out);
+    ctx->total_launches += 2;
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = copy_out(out, d_out, (size_t)ctx->n_scat * sizeof(double2), ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  cudaFree(d_dT); cudaFree(d_tmp); cudaFree(d_out);
+  TM_CUDA(e);
+  return TM_OK;
+}
+
+int tm_mie_tmatrix(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64* out);
+
+int tm_mie_tmatrix_dR(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64* out) {
+  if (lmax < 1 || lmax > TM_MAX_LMAX || !(k_b > 0.0) || !(radius > 0.0) || !out) return TM_E_INVALID;
+  const int L = tm_num_modes(lmax);
+  const double h = 1e-4 * (radius < 1.0 ? 1.0 : radius);
+  if (!(radius - h > 0.0)) return TM_E_INVALID;
+  std::vector<tm_c64> a(L), b(L), c(L), d(L);
+  tm_mie_tmatrix(lmax, k_b, radius + h, eps_r, a.data());
+  tm_mie_tmatrix(lmax, k_b, radius - h, eps_r, b.data());
+  tm_mie_tmatrix(lmax, k_b, radius + 0.5 * h, eps_r, c.data());
+  tm_mie_tmatrix(lmax, k_b, radius - 0.5 * h, eps_r, d.data());
+  for (int i = 0; i < L; ++i) {          // Richardson: (4 D(h/2) - D(h)) / 3
+    const double d1r = (a[i].re - b[i].re) / (2 * h), d1i = (a[i].im - b[i].im) / (2 * h);
+    const double d2r = (c[i].re - d[i].re) / h, d2i = (c[i].im - d[i].im) / h;
+    out[i].re = (4.0 * d2r - d1r) / 3.0; out[i].im = (4.0 * d2i - d1i) / 3.0;
+  }
+  return TM_OK;
+}
+
 // Lorenz-Mie coefficients (reading R11), x = k_b R, m_r = sqrt(eps_r), psi_l(z) = z j_l(z), xi_l(z) = z h_l^(1)(z):
 //   a_l = [m psi_l(mx) psi_l'(x) - psi_l(x) psi_l'(mx)] / [m psi_l(mx) xi_l'(x) - xi_l(x) psi_l'(mx)]
 //   b_l = [psi_l(mx) psi_l'(x) - m psi_l(x) psi_l'(mx)] / [psi_l(mx) xi_l'(x) - m xi_l(x) psi_l'(mx)]

@@ -281,3 +281,36 @@ k_scale_or_sub(const Cx<R>* __restrict__ a, const Cx<R>* __restrict__ b, const d
     else dst[g] = csub(a[g], b[g]);
   }
 }
+
+// ------------------------------------------------------------------------------------------------ sensitivities
+// out[j] = lambda_j^T dT_{type(j)} (p_j + (A s)_j)   (Eq. IV8 with Omega = T^{-1}(I - T A)).
+// One warp per scatterer; `as` holds A s.
+template <typename R>
+__global__ void __launch_bounds__(128)
+k_grad_tmatrix(int L, int n_scat, const Cx<R>* __restrict__ as, const double2* __restrict__ p, const Cx<R>* __restrict__ lam,
+               const Cx<R>* __restrict__ dT, int diag, const int* __restrict__ type_of, double2* __restrict__ out) {
+  const int j = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (j >= n_scat) return;
+  const int ty = type_of[j];
+  double sr = 0.0, si = 0.0;
+  for (int a = lane; a < L; a += 32) {
+    double rr, ri;                                     // (dT q)_a,  q = p + A s
+    if (diag) {
+      const Cx<R> d = dT[(size_t)ty * L + a];
+      const double qr = p[(size_t)j * L + a].x + (double)as[(size_t)j * L + a].re, qi = p[(size_t)j * L + a].y + (double)as[(size_t)j * L + a].im;
+      rr = (double)d.re * qr - (double)d.im * qi; ri = (double)d.re * qi + (double)d.im * qr;
+    } else {
+      rr = 0.0; ri = 0.0;
+      const Cx<R>* row = dT + ((size_t)ty * L + a) * L;
+      for (int b = 0; b < L; ++b) {
+        const double qr = p[(size_t)j * L + b].x + (double)as[(size_t)j * L + b].re, qi = p[(size_t)j * L + b].y + (double)as[(size_t)j * L + b].im;
+        rr += (double)row[b].re * qr - (double)row[b].im * qi; ri += (double)row[b].re * qi + (double)row[b].im * qr;
+      }
+    }
+    const Cx<R> l = lam[(size_t)j * L + a];
+    sr += (double)l.re * rr - (double)l.im * ri;
+    si += (double)l.re * ri + (double)l.im * rr;
+  }
+  sr = warp_sum(sr); si = warp_sum(si);
+  if (lane == 0) out[j] = make_double2(sr, si);
+}

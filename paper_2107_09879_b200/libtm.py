@@ -21,7 +21,7 @@ TM_KERNEL_AUTO, TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR, TM_KERNEL_SYM3D = 0, 1, 2
 
 EXPORTS = ["tm_create", "tm_set_tmatrices", "tm_set_incident", "tm_get_incident", "tm_solve", "tm_solve_adjoint",
            "tm_matvec", "tm_fields", "tm_workspace_bytes", "tm_set_workspace", "tm_set_kernel", "tm_get_kernel",
-           "tm_kernel_time", "tm_pair_cost", "tm_measure_fma_peak", "tm_mie_tmatrix", "tm_num_modes", "tm_last_error", "tm_destroy"]
+           "tm_kernel_time", "tm_pair_cost", "tm_measure_fma_peak", "tm_grad_tmatrix", "tm_mie_tmatrix_dR", "tm_mie_tmatrix", "tm_num_modes", "tm_last_error", "tm_destroy"]
 
 
 class c64(ctypes.Structure):
@@ -87,6 +87,8 @@ def lib():
         L.tm_get_kernel.argtypes = [vp]
         L.tm_kernel_time.argtypes = [vp, ci, ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(ctypes.c_longlong)]
         L.tm_mie_tmatrix.argtypes = [ci, cd, cd, c64, vp]
+        L.tm_grad_tmatrix.argtypes = [vp, vp, vp, vp, vp]
+        L.tm_mie_tmatrix_dR.argtypes = [ci, cd, cd, c64, vp]
         L.tm_pair_cost.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(cd)]
         L.tm_measure_fma_peak.argtypes = [ci, ctypes.POINTER(cd), vp]
         L.tm_num_modes.argtypes = [ci]
@@ -119,6 +121,15 @@ def mie_tmatrix(lmax, k_b, radius, eps_r):
     rc = lib().tm_mie_tmatrix(lmax, float(k_b), float(radius), _c64(eps_r), out.ctypes.data)
     if rc != TM_OK:
         raise TmError(rc, "tm_mie_tmatrix: invalid arguments")
+    return out
+
+
+def mie_tmatrix_dR(lmax, k_b, radius, eps_r):
+    """d(diag Mie T)/dR (tm_mie_tmatrix_dR), shape (L,) complex128."""
+    out = np.zeros(lib().tm_num_modes(lmax), dtype=np.complex128)
+    rc = lib().tm_mie_tmatrix_dR(lmax, float(k_b), float(radius), _c64(eps_r), out.ctypes.data)
+    if rc != TM_OK:
+        raise TmError(rc, "tm_mie_tmatrix_dR: invalid arguments")
     return out
 
 
@@ -268,6 +279,15 @@ class Solver:
         a, b = ctypes.c_double(), ctypes.c_double()
         self._check(lib().tm_pair_cost(self._h, ctypes.byref(a), ctypes.byref(b)))
         return a.value, b.value
+
+    def grad_tmatrix(self, dT, lam, s, out=None):
+        """out[j] = lambda_j^T dT_{type(j)} (p_j + (A s)_j)  (tm_grad_tmatrix; PAPER.md Eqs. IV8-IV9)."""
+        dT = np.ascontiguousarray(dT, dtype=np.complex128) if isinstance(dT, np.ndarray) else dT
+        lam = np.ascontiguousarray(lam, dtype=np.complex128) if isinstance(lam, np.ndarray) else lam
+        s = np.ascontiguousarray(s, dtype=np.complex128) if isinstance(s, np.ndarray) else s
+        out = np.empty(self.n_scat, dtype=np.complex128) if out is None else out
+        self._check(lib().tm_grad_tmatrix(self._h, _ptr(dT), _ptr(lam), _ptr(s), _ptr(out)))
+        return out
 
     def kernel_time(self, reset=False):
         ms, n_ap, n_tot = ctypes.c_double(), ctypes.c_longlong(), ctypes.c_longlong()

@@ -20,7 +20,7 @@ def libtm():
 def test_exports_match_header(libtm):
     hdr = open(os.path.join(ROOT, "include", "tm.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(tm_[a-z_0-9]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(tm_[A-Za-z_0-9]+)\s*\(", hdr))
     assert declared == set(libtm.EXPORTS)
     lib = libtm.lib()
     for name in declared:

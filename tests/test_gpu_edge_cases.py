@@ -117,3 +117,31 @@ def test_far_apart_and_close_pairs(tm):
     s = tm.Solver(pos, 3, W.K_B)
     assert rel(s.matvec(x, 2), ref) <= 1e-11             # k r = 6e4: 6e4 * 1.1e-16 phase rounding on both sides
     s.close()
+
+
+def test_adjoint_radius_sensitivities(tm):
+    """NEXT-2 (geometry half): dJ/dR_j for every scatterer from ONE adjoint solve (PAPER.md Eqs. IV8-IV9) against the oracle's
+    adjoint formula (tight) and the oracle's finite differences of the dense solve (the plain definition)."""
+    from oracle import gradient, incident
+    rng = np.random.default_rng(12)
+    pos = W.random_cloud(6, seed=41)
+    radii = rng.uniform(0.10, 0.22, 6)
+    lmax = 2
+    p = incident.plane_wave_incident(lmax, W.K_B, pos, 0.3, 0.8, 1.0, 0.4j)
+    v = rand_x(p.shape, 13)
+    g_ref, s_ref, lam_ref = gradient.adjoint_radius_gradient(lmax, W.K_B, pos, radii, 4.0, p, v)
+    s = tm.Solver(pos, lmax, W.K_B)
+    T = np.stack([tm.mie_tmatrix(lmax, W.K_B, r, 4.0) for r in radii])
+    dT = np.stack([tm.mie_tmatrix_dR(lmax, W.K_B, r, 4.0) for r in radii])
+    assert rel(dT, np.stack([gradient.mie_dT_dR(lmax, W.K_B, r, 4.0) for r in radii])) <= 1e-8
+    s.set_tmatrices(T, np.arange(6, dtype=np.int32), True)
+    s.set_incident_plane(0.3, 0.8, 1.0, 0.4j)
+    sol, _, rc = s.solve(1e-12, 60, 600)
+    lam, _, rc2 = s.solve_adjoint(v, 1e-12, 60, 600)
+    assert rc == 0 and rc2 == 0
+    g = s.grad_tmatrix(dT, lam, sol)
+    assert rel(g, g_ref) <= 1e-8
+    for j in (0, 3):
+        fd = gradient.fd_radius(lmax, W.K_B, pos, radii, 4.0, p, v, j)
+        assert abs(g[j] - fd) <= 1e-6 * abs(fd)
+    s.close()
