@@ -157,6 +157,19 @@ int tm_kernel_time(tm_ctx *ctx, int reset, double *allpairs_ms, long long *allpa
  *           out over the sites of the type.  One all-pairs matvec + one small kernel.  Needs T and the incident field. */
 int tm_grad_tmatrix(tm_ctx *ctx, const tm_c64 *dT, const tm_c64 *lambda, const tm_c64 *s, tm_c64 *out);
 
+/* Position sensitivities through the same adjoint solve (Eqs. IV3-IV6, IV9):
+ *   out[j][alpha] = lambda^T T (dA/dx_{j,alpha}) s  (+ lambda_j^T T_j dp_j/dx_{j,alpha} when dp is given)
+ * = dJ/dx_{j,alpha} for J = w^T s at fixed w (the explicit term of Eq. IV6 - the detector overlap of the moved
+ * scatterer's own waves - is the caller's, it does not involve the solver).  Identity S3 folds the row-block and
+ * column-block parts of dA/dx_j into two all-pairs products with the DERIVATIVE of the translation operator,
+ *   G_j = mu_j^T (d_alpha A s)_j + (P s_j)^T (d_alpha A P mu)_j ,  mu = T^T lambda,
+ * and d_alpha A is taken by Richardson-extrapolated central differences of the on-the-fly operator in its displacement
+ * argument (targets displaced rigidly by +-h, +-h/2; error O((k h)^4); h in the units of the positions, 0 -> 2e-4
+ * wavelengths) - a stated deviation from the paper's analytic dOmega/dq.  24 all-pairs launches.
+ *   lambda, s [n_scat][L]; dp [n_scat][3][L] or NULL (plane wave: dp = i k_alpha p); out [n_scat][3] complex.
+ * lmax <= 3 (uses the generated 3-D kernel for all three directions). */
+int tm_grad_positions(tm_ctx *ctx, const tm_c64 *lambda, const tm_c64 *s, const tm_c64 *dp, double h, tm_c64 *out);
+
 /* Host helper: d(diag T)/dR of the Mie T-matrix of tm_mie_tmatrix (Richardson-extrapolated central differences of the
  * closed form, relative accuracy ~1e-10), out[L]. */
 int tm_mie_tmatrix_dR(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64 *out);

@@ -46,3 +46,33 @@ def adjoint_radius_gradient(lmax, k, pos, radii, eps_r, p_inc, v):
     q = p_inc + (A @ s.reshape(-1)).reshape(N, L)                 # a^(0) + A s  (= T^{-1} s)
     dT = np.stack([mie_dT_dR(lmax, k, r, eps_r) for r in radii])
     return np.sum(lam * dT * q, axis=1), s, lam
+
+
+# ------------------------------------------------------------------------------------------------ positions (Eqs. IV3-IV6)
+def fd_position(lmax, k, pos, radii, eps_r, inc_fn, v, j, alpha, h=1e-5):
+    """dJ/dx_{j,alpha} at fixed v by central differences of the full dense solve; inc_fn(pos) -> a^(0) (N, L)."""
+    pp, pm = np.array(pos, dtype=float), np.array(pos, dtype=float)
+    pp[j, alpha] += h
+    pm[j, alpha] -= h
+    return (_solve_J(lmax, k, pp, radii, eps_r, inc_fn(pp), v)[0] - _solve_J(lmax, k, pm, radii, eps_r, inc_fn(pm), v)[0]) / (2 * h)
+
+
+def adjoint_position_gradient(lmax, k, pos, radii, eps_r, inc_fn, v, h=1e-5):
+    """All dJ/dx_{j,alpha} through ONE adjoint solve: lambda^T T (dA/dx_{j,alpha}) s + lambda^T T da^(0)/dx_{j,alpha}
+    (Eq. IV6 with Omega = T^{-1} M; dOmega/dq = -dA/dq).  dA/dq and da^(0)/dq by central differences of the oracle's own
+    dense assembly (the paper differentiates Eq. I23 analytically; numerically the same matrix).  Returns (N, 3)."""
+    p_inc = inc_fn(pos)
+    J, s, M, t = _solve_J(lmax, k, pos, radii, eps_r, p_inc, v)
+    lam = system.solve_adjoint(M, v)
+    N, L = s.shape
+    mu = (t * lam).reshape(-1)                                     # T^T lambda (T diagonal)
+    out = np.zeros((N, 3), dtype=complex)
+    for j in range(N):
+        for alpha in range(3):
+            pp, pm = np.array(pos, dtype=float), np.array(pos, dtype=float)
+            pp[j, alpha] += h
+            pm[j, alpha] -= h
+            dA = (system.assemble_A(lmax, k, pp) - system.assemble_A(lmax, k, pm)) / (2 * h)
+            dp = (inc_fn(pp) - inc_fn(pm)) / (2 * h)
+            out[j, alpha] = mu @ (dA @ s.reshape(-1)) + mu @ dp.reshape(-1)
+    return out, s, lam

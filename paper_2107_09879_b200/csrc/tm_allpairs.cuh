@@ -39,6 +39,11 @@ template <> __device__ __forceinline__ void phase_kr<float>(double k_over_pi, do
   sincospif((float)t, &s, &c);
 }
 
+// Optional rigid displacement of all TARGETS against the sources (tm_grad_positions: numerical differentiation of the
+// translation operator in its displacement argument).  With a non-zero shift the self pair no longer has r = 0 and is
+// excluded by index instead.
+struct TmShift { double x, y, z; int on; };
+
 template <typename R, int LMAX, int H> struct CopPair;
 #define TM_COP_SPEC(LM, HH)                                                                              \
   template <typename R> struct CopPair<R, LM, HH> {                                                      \
@@ -70,7 +75,7 @@ template <typename R, int LMAX, int TJ, int SS, bool LOCKSTEP>
 __global__ void __launch_bounds__(TJ)
 k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
                     const TmTile* __restrict__ tiles, int n_scat, double k_over_pi, double inv_k,
-                    const int* __restrict__ n_active) {
+                    const int* __restrict__ n_active, TmShift shift) {
   constexpr int L = 2 * LMAX * (LMAX + 2);
   constexpr int NH = L / 2;
   constexpr int NQ = 2 * LMAX + 1;
@@ -85,7 +90,7 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
   const int half = blockIdx.z;
   const bool live = tid < tile.tgt_count;
   const int j = tile.tgt_start + (live ? tid : tile.tgt_count - 1);
-  const double xj = pos[3 * j], yj = pos[3 * j + 1];
+  const double xj = pos[3 * j] + shift.x, yj = pos[3 * j + 1] + shift.y;     // shift.z must be 0 for this kernel
 
   // this block's chunk of the window's sources
   const int per = (tile.src_count + gridDim.y - 1) / gridDim.y;
@@ -125,7 +130,7 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
       if (LOCKSTEP) __syncthreads();
       const double dx = xj - s_px[s], dy = yj - s_py[s];        // d = x_dest - x_source (reading R3)
       const double r2 = dx * dx + dy * dy;
-      const double rinv = r2 > 0.0 ? rsqrt(r2) : 0.0;           // self pair -> h_q = 0 -> contributes nothing
+      const double rinv = (r2 > 0.0 && !(shift.on && s0 + s == j)) ? rsqrt(r2) : 0.0;   // self pair -> h_q = 0 -> nothing
       const double r = r2 * rinv;
       R cm[LMAX + 1], sm[LMAX + 1];
       cm[0] = R(1); sm[0] = R(0);
@@ -308,7 +313,7 @@ template <typename R, int LMAX, int TJ, int SS>
 __global__ void __launch_bounds__(TJ)
 k_allpairs_sym3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
                  const TmTile* __restrict__ tiles, int n_scat, double k_over_pi, double inv_k,
-                 const int* __restrict__ n_active) {
+                 const int* __restrict__ n_active, TmShift shift) {
   constexpr int L = 2 * LMAX * (LMAX + 2);
   constexpr int NS = L / 2;                 // slots per sector
   constexpr int NQ = 2 * LMAX + 1;
@@ -329,7 +334,7 @@ k_allpairs_sym3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
   const int sct = blockIdx.z;
   const bool live = tid < tile.tgt_count;
   const int j = tile.tgt_start + (live ? tid : tile.tgt_count - 1);
-  const double xj = pos[3 * j], yj = pos[3 * j + 1], zj = pos[3 * j + 2];
+  const double xj = pos[3 * j] + shift.x, yj = pos[3 * j + 1] + shift.y, zj = pos[3 * j + 2] + shift.z;
   const int per = (tile.src_count + gridDim.y - 1) / gridDim.y;
   const int c0 = tile.src_start + blockIdx.y * per;
   const int c1 = min(tile.src_start + tile.src_count, c0 + per);
@@ -368,7 +373,7 @@ k_allpairs_sym3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
     for (int s = 0; s < ns; ++s) {
       const double dx = xj - s_px[s], dy = yj - s_py[s], dz = zj - s_pz[s];   // d = x_dest - x_source (reading R3)
       const double rho2 = dx * dx + dy * dy, r2 = rho2 + dz * dz;
-      const double rinv = r2 > 0.0 ? rsqrt(r2) : 0.0;          // self pair -> h_q = 0 -> contributes nothing
+      const double rinv = (r2 > 0.0 && !(shift.on && s0 + s == j)) ? rsqrt(r2) : 0.0;   // self pair -> h_q = 0 -> nothing
       const double rhoinv = rho2 > 0.0 ? rsqrt(rho2) : 0.0;
       const double r = r2 * rinv;
       R cm[LMAX + 1], sm[LMAX + 1];

@@ -46,6 +46,7 @@ struct tm_ctx {
   std::vector<int> win_ptr;
   bool coplanar = false;
   int kernel_req = TM_KERNEL_AUTO, kernel = TM_KERNEL_GENERAL;
+  TmShift shift{0.0, 0.0, 0.0, 0};      // target displacement (tm_grad_positions only)
   int cop_tj = 128, cop_lockstep = 0;   // coplanar kernel launch shape (env TM_COP_TJ / TM_COP_LOCKSTEP override)
 
   double* d_pos = nullptr;
@@ -186,7 +187,7 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
     grid.z = 2;                                         // mirror-parity half: slowest grid dimension
 #define TM_LAUNCH_COP2(LM, TJ, LS)                                                                          \
   k_allpairs_coplanar<R, LM, TJ, COP_SS, LS><<<grid, TJ, 0, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat, \
-                                                                         k_over_pi, inv_k, n_active)
+                                                                         k_over_pi, inv_k, n_active, c->shift)
 #define TM_LAUNCH_COP(LM)                                                                                   \
   do {                                                                                                      \
     if (c->cop_tj == 256) { if (c->cop_lockstep) TM_LAUNCH_COP2(LM, 256, true); else TM_LAUNCH_COP2(LM, 256, false); } \
@@ -206,7 +207,7 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
     const size_t sm = Sym3dSmem<R, LM, SYM3D_TJ, SYM3D_SS>::bytes;                                              \
     cudaFuncSetAttribute(k_allpairs_sym3d<R, LM, SYM3D_TJ, SYM3D_SS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
     k_allpairs_sym3d<R, LM, SYM3D_TJ, SYM3D_SS><<<grid, SYM3D_TJ, sm, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat, \
-                                                                                   k_over_pi, inv_k, n_active); \
+                                                                                   k_over_pi, inv_k, n_active, c->shift); \
   }
     switch (c->lmax) {
       case 1: TM_LAUNCH_S3(1) break;
@@ -1084,6 +1085,80 @@ int tm_grad_tmatrix(tm_ctx* ctx, const tm_c64* dT, const tm_c64* lambda, const t
   cudaFree(d_dT); cudaFree(d_tmp); cudaFree(d_out);
   TM_CUDA(e);
   return TM_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+template <typename R>
+int grad_positions_typed(tm_ctx* ctx, const tm_c64* lambda, const tm_c64* s, const tm_c64* dp, double h, tm_c64* out) {
+  const size_t n = ctx->n, vb = n * sizeof(Cx<R>);
+  const int L = ctx->L, N = ctx->n_scat;
+  Cx<R>*S = vec<R>(ctx, 0), *Y = vec<R>(ctx, 1), *LAM = vec<R>(ctx, 2);
+  Cx<R>*PMU = nullptr, *D = nullptr; double2 *d_out = nullptr, *d_dp = nullptr;
+  auto cleanup = [&]() { cudaFree(PMU); cudaFree(D); cudaFree(d_out); cudaFree(d_dp); ctx->shift = TmShift{0.0, 0.0, 0.0, 0}; };
+#define TM_G(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { cleanup(); return fail(ctx, TM_E_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); } } while (0)
+  TM_G(cudaMalloc(&PMU, vb)); TM_G(cudaMalloc(&D, vb)); TM_G(cudaMalloc(&d_out, (size_t)N * 3 * sizeof(double2)));
+  TM_G(cudaMemsetAsync(d_out, 0, (size_t)N * 3 * sizeof(double2), ctx->stream));
+  TM_G(load_c64<R>(ctx, s, S));
+  TM_G(load_c64<R>(ctx, lambda, LAM));
+  TM_G(launch_tapply<R>(ctx, 4, LAM, PMU, nullptr));                 // P mu = P T^T lambda
+  const int gb = (N + 3) / 4;
+  for (int alpha = 0; alpha < 3; ++alpha) {
+    for (int which = 0; which < 2; ++which) {
+      const Cx<R>* vecx = which == 0 ? S : PMU;                       // d_alpha A s   /   d_alpha A (P mu)
+      const Cx<R>* left = which == 0 ? PMU : S;                       // mu = P(P mu)  /   P s
+      const double hs[4] = {0.5 * h, -0.5 * h, h, -h};
+      const double cf[4] = {4.0 / (3.0 * h), -4.0 / (3.0 * h), -1.0 / (6.0 * h), 1.0 / (6.0 * h)};
+      for (int t = 0; t < 4; ++t) {
+        ctx->shift = TmShift{alpha == 0 ? hs[t] : 0.0, alpha == 1 ? hs[t] : 0.0, alpha == 2 ? hs[t] : 0.0, 1};
+        TM_G(launch_allpairs<R>(ctx, vecx, nullptr));
+        TM_G(launch_tapply<R>(ctx, 2, vecx, Y, nullptr));
+        k_acc_scaled<R><<<grid_for(n, 256), 256, 0, ctx->stream>>>(D, Y, cf[t], n, t == 0 ? 1 : 0);
+      }
+      k_bilinear_rows<R, R><<<gb, 128, 0, ctx->stream>>>(L, N, left, D, (size_t)L, ctx->d_const, d_out + alpha, 3);
+      ctx->total_launches += 5;
+      TM_G(cudaGetLastError());
+    }
+  }
+  ctx->shift = TmShift{0.0, 0.0, 0.0, 0};
+  if (dp) {                                                          // incident part: mu_j^T dp_j[alpha]
+    TM_G(cudaMalloc(&d_dp, n * 3 * sizeof(double2)));
+    TM_G(copy_in(d_dp, dp, n * 3 * sizeof(double2), ctx->stream));
+    for (int alpha = 0; alpha < 3; ++alpha)
+      k_bilinear_rows<R, double><<<gb, 128, 0, ctx->stream>>>(L, N, PMU, reinterpret_cast<const Cx<double>*>(d_dp) + (size_t)alpha * L,
+                                                             (size_t)3 * L, ctx->d_const, d_out + alpha, 3);
+    TM_G(cudaGetLastError());
+  }
+  TM_G(copy_out(out, d_out, (size_t)N * 3 * sizeof(double2), ctx->stream));
+  TM_G(cudaStreamSynchronize(ctx->stream));
+#undef TM_G
+  cleanup();
+  return TM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tm_grad_positions(tm_ctx* ctx, const tm_c64* lambda, const tm_c64* s, const tm_c64* dp, double h, tm_c64* out) {
+  if (!ctx) return TM_E_INVALID;
+  if (!lambda || !s || !out) return fail(ctx, TM_E_INVALID, "NULL argument");
+  if (!ctx->has_T) return fail(ctx, TM_E_STATE, "tm_set_tmatrices must be called first");
+  if (ctx->lmax > 3) return fail(ctx, TM_E_INVALID, "position sensitivities are built for lmax <= 3");
+  if (h < 0.0 || !std::isfinite(h)) return fail(ctx, TM_E_INVALID, "h must be >= 0");
+  if (h == 0.0) h = 2e-4 * 2.0 * M_PI / ctx->k;
+  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  const int saved = ctx->kernel_req;
+  ctx->kernel_req = TM_KERNEL_SYM3D;                      // displaced targets are not coplanar with the sources (alpha = z)
+  int rc = configure_kernel(ctx);
+  if (rc == TM_OK)
+    rc = ctx->precision == TM_FP64 ? grad_positions_typed<double>(ctx, lambda, s, dp, h, out)
+                                   : grad_positions_typed<float>(ctx, lambda, s, dp, h, out);
+  ctx->kernel_req = saved;
+  const int rc2 = configure_kernel(ctx);
+  return rc != TM_OK ? rc : rc2;
 }
 
 int tm_mie_tmatrix(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64* out);

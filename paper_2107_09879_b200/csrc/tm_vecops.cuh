@@ -314,3 +314,31 @@ k_grad_tmatrix(int L, int n_scat, const Cx<R>* __restrict__ as, const double2* _
   sr = warp_sum(sr); si = warp_sum(si);
   if (lane == 0) out[j] = make_double2(sr, si);
 }
+
+// acc = (init ? 0 : acc) + c * y
+template <typename R>
+__global__ void k_acc_scaled(Cx<R>* __restrict__ acc, const Cx<R>* __restrict__ y, double c, size_t n, int init) {
+  for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+    const double ar = init ? 0.0 : (double)acc[e].re, ai = init ? 0.0 : (double)acc[e].im;
+    acc[e] = cx<R>((R)(ar + c * (double)y[e].re), (R)(ai + c * (double)y[e].im));
+  }
+}
+
+// out[j * out_stride] += sum_a left_j[perm a] * D_j[a]   (bilinear, no conjugation; P = the m -> -m permutation).
+// D_j starts at D + j * d_stride.  One warp per scatterer.
+template <typename R, typename RD>
+__global__ void __launch_bounds__(128)
+k_bilinear_rows(int L, int n_scat, const Cx<R>* __restrict__ left, const Cx<RD>* __restrict__ D, size_t d_stride,
+                const TmConst* __restrict__ cst, double2* __restrict__ out, int out_stride) {
+  const int j = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (j >= n_scat) return;
+  double sr = 0.0, si = 0.0;
+  for (int a = lane; a < L; a += 32) {
+    const Cx<R> l = left[(size_t)j * L + cst->perm_neg_m[a]];
+    const Cx<RD> d = D[(size_t)j * d_stride + a];
+    sr += (double)l.re * (double)d.re - (double)l.im * (double)d.im;
+    si += (double)l.re * (double)d.im + (double)l.im * (double)d.re;
+  }
+  sr = warp_sum(sr); si = warp_sum(si);
+  if (lane == 0) { out[(size_t)j * out_stride].x += sr; out[(size_t)j * out_stride].y += si; }
+}

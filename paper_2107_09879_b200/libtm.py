@@ -21,7 +21,7 @@ TM_KERNEL_AUTO, TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR, TM_KERNEL_SYM3D = 0, 1, 2
 
 EXPORTS = ["tm_create", "tm_set_tmatrices", "tm_set_incident", "tm_get_incident", "tm_solve", "tm_solve_adjoint",
            "tm_matvec", "tm_fields", "tm_workspace_bytes", "tm_set_workspace", "tm_set_kernel", "tm_get_kernel",
-           "tm_kernel_time", "tm_pair_cost", "tm_measure_fma_peak", "tm_grad_tmatrix", "tm_mie_tmatrix_dR", "tm_mie_tmatrix", "tm_num_modes", "tm_last_error", "tm_destroy"]
+           "tm_kernel_time", "tm_pair_cost", "tm_measure_fma_peak", "tm_grad_tmatrix", "tm_grad_positions", "tm_mie_tmatrix_dR", "tm_mie_tmatrix", "tm_num_modes", "tm_last_error", "tm_destroy"]
 
 
 class c64(ctypes.Structure):
@@ -88,6 +88,7 @@ def lib():
         L.tm_kernel_time.argtypes = [vp, ci, ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(ctypes.c_longlong)]
         L.tm_mie_tmatrix.argtypes = [ci, cd, cd, c64, vp]
         L.tm_grad_tmatrix.argtypes = [vp, vp, vp, vp, vp]
+        L.tm_grad_positions.argtypes = [vp, vp, vp, vp, cd, vp]
         L.tm_mie_tmatrix_dR.argtypes = [ci, cd, cd, c64, vp]
         L.tm_pair_cost.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(cd)]
         L.tm_measure_fma_peak.argtypes = [ci, ctypes.POINTER(cd), vp]
@@ -287,6 +288,16 @@ class Solver:
         s = np.ascontiguousarray(s, dtype=np.complex128) if isinstance(s, np.ndarray) else s
         out = np.empty(self.n_scat, dtype=np.complex128) if out is None else out
         self._check(lib().tm_grad_tmatrix(self._h, _ptr(dT), _ptr(lam), _ptr(s), _ptr(out)))
+        return out
+
+    def grad_positions(self, lam, s, dp=None, h=0.0, out=None):
+        """out[j, alpha] = lambda^T T (dA/dx_{j,alpha}) s (+ mu_j^T dp[j, alpha])  (tm_grad_positions; PAPER.md Eqs. IV3-IV9)."""
+        lam = np.ascontiguousarray(lam, dtype=np.complex128) if isinstance(lam, np.ndarray) else lam
+        s = np.ascontiguousarray(s, dtype=np.complex128) if isinstance(s, np.ndarray) else s
+        if dp is not None and isinstance(dp, np.ndarray):
+            dp = np.ascontiguousarray(dp, dtype=np.complex128)
+        out = np.empty((self.n_scat, 3), dtype=np.complex128) if out is None else out
+        self._check(lib().tm_grad_positions(self._h, _ptr(lam), _ptr(s), _ptr(dp), float(h), _ptr(out)))
         return out
 
     def kernel_time(self, reset=False):

@@ -145,3 +145,33 @@ def test_adjoint_radius_sensitivities(tm):
         fd = gradient.fd_radius(lmax, W.K_B, pos, radii, 4.0, p, v, j)
         assert abs(g[j] - fd) <= 1e-6 * abs(fd)
     s.close()
+
+
+def test_adjoint_position_sensitivities(tm):
+    """NEXT-2 (position half): dJ/dx_{j,alpha} for every scatterer and direction from ONE adjoint solve (Eqs. IV3-IV9),
+    3-D cloud and a planar layout (z-derivatives need the 3-D kernel), against the oracle."""
+    from oracle import gradient, incident
+    rng = np.random.default_rng(22)
+    lmax, beta, alpha = 2, 0.4, -0.5
+    kv = W.K_B * np.array([np.sin(beta) * np.cos(alpha), np.sin(beta) * np.sin(alpha), np.cos(beta)])
+    for planar in (False, True):
+        pos = W.random_cloud(5, seed=8, planar=planar)
+        radii = rng.uniform(0.12, 0.2, 5)
+        inc = lambda q: incident.plane_wave_incident(lmax, W.K_B, q, beta, alpha, 0.7, 0.2j)
+        v = rand_x((5, 16), 23)
+        g_ref, s_ref, lam_ref = gradient.adjoint_position_gradient(lmax, W.K_B, pos, radii, 4.0, inc, v)
+        s = tm.Solver(pos, lmax, W.K_B)
+        T = np.stack([tm.mie_tmatrix(lmax, W.K_B, r, 4.0) for r in radii])
+        s.set_tmatrices(T, np.arange(5, dtype=np.int32), True)
+        s.set_incident_plane(beta, alpha, 0.7, 0.2j)
+        kern = s.get_kernel()
+        sol, _, rc = s.solve(1e-12, 60, 600)
+        lam, _, rc2 = s.solve_adjoint(v, 1e-12, 60, 600)
+        p = s.get_incident()
+        dp = 1j * kv[None, :, None] * p[:, None, :]                     # plane wave: d p_j / d x_j = i k p_j
+        g = s.grad_positions(lam, sol, dp=dp)
+        assert s.get_kernel() == kern                                    # the kernel choice is restored
+        assert np.abs(g - g_ref).max() <= 2e-7 * np.abs(g_ref).max()
+        fd = gradient.fd_position(lmax, W.K_B, pos, radii, 4.0, inc, v, 2, 2)
+        assert abs(g[2, 2] - fd) <= 1e-6 * np.abs(g_ref).max()
+        s.close()

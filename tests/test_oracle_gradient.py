@@ -23,3 +23,15 @@ def test_adjoint_radius_gradient_matches_finite_differences():
     dT = np.stack([gradient.mie_dT_dR(2, K, r, 4.0) for r in radii])
     wrong = np.sum(lam * dT * p, axis=1)
     assert np.abs(wrong - g).max() > 1e-3 * np.abs(g).max()
+
+
+def test_adjoint_position_gradient_matches_finite_differences():
+    rng = np.random.default_rng(21)
+    pos = W.random_cloud(4, seed=6)
+    radii = rng.uniform(0.12, 0.2, 4)
+    inc = lambda q: incident.plane_wave_incident(2, K, q, 0.4, -0.5, 0.7, 0.2j)
+    v = rng.standard_normal((4, 16)) + 1j * rng.standard_normal((4, 16))
+    g, s, lam = gradient.adjoint_position_gradient(2, K, pos, radii, 4.0, inc, v)
+    for (j, a) in ((0, 0), (1, 2), (3, 1)):
+        fd = gradient.fd_position(2, K, pos, radii, 4.0, inc, v, j, a)
+        assert abs(g[j, a] - fd) <= 1e-6 * np.abs(g).max()
