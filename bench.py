@@ -380,6 +380,39 @@ def run_nyquist(args, w):
     print(json.dumps(out), flush=True)
 
 
+def run_gradient(args, w):
+    """Recorded run of the adjoint sensitivities (NEXT-2; not the contract line): forward solve, adjoint solve, then ALL radius
+    and position derivatives of J = w^T s from tm_grad_tmatrix / tm_grad_positions."""
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2107_09879_b200 import libtm
+    assert w["t_kind"] in ("mie_types", "mie_sites") and w["inc_kind"] == "plane"
+    s = libtm.solver_for_workload(w)
+    N, L = s.n_scat, s.L
+    tol = args.tol or w["tol"]
+    wv = adjoint_weight(w)
+    t0 = time.perf_counter()
+    sol, i1, rc1 = s.solve(tol, w["restart"], args.max_iter or w["max_iter"])
+    lam, i2, rc2 = s.solve_adjoint(wv, tol, w["restart"], args.max_iter or w["max_iter"])
+    t1 = time.perf_counter()
+    dT = np.stack([libtm.mie_tmatrix_dR(w["lmax"], w["k"], r, w["eps_r"]) for r in w["radii"]])
+    t2 = time.perf_counter()
+    gR = s.grad_tmatrix(dT, lam, sol)
+    t3 = time.perf_counter()
+    p = s.get_incident()
+    kv = w["k"] * np.array([np.sin(w["beta"]) * np.cos(w["alpha"]), np.sin(w["beta"]) * np.sin(w["alpha"]), np.cos(w["beta"])])
+    dp = 1j * kv[None, :, None] * p[:, None, :]
+    t4 = time.perf_counter()
+    gX = s.grad_positions(lam, sol, dp=dp)
+    t5 = time.perf_counter()
+    print(json.dumps({"mode": "gradient", "workload": w["name"], "n_scat": N, "L": L, "design_variables": int(N + 3 * N),
+                      "solves_seconds": t1 - t0, "forward_iterations": i1[0].iterations, "adjoint_iterations": i2[0].iterations,
+                      "converged": rc1 == 0 and rc2 == 0, "grad_tmatrix_seconds": t3 - t2, "grad_positions_seconds": t5 - t4,
+                      "grad_positions_allpairs_launches": 24, "norm_grad_R": float(np.linalg.norm(gR)),
+                      "norm_grad_x": float(np.linalg.norm(gX))}), flush=True)
+    s.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -387,7 +420,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2")
-    ap.add_argument("--mode", default="full", choices=["full", "matvec", "nyquist"],
+    ap.add_argument("--mode", default="full", choices=["full", "matvec", "nyquist", "gradient"],
                     help="matvec: time operator applications only; nyquist: recorded run of the window decomposition")
     ap.add_argument("--group", type=int, default=16, help="nyquist mode: samples per group side")
     ap.add_argument("--padding", type=float, default=4.0, help="nyquist mode: padding in wavelengths")
@@ -413,6 +446,9 @@ def main():
     if args.mode == "nyquist":
         if rank == 0:
             run_nyquist(args, w)
+    elif args.mode == "gradient":
+        if rank == 0:
+            run_gradient(args, w)
     elif args.impl == "reference":
         run_reference(args, w, rank, world)
     else:
