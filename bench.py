@@ -59,15 +59,15 @@ def adjoint_weight(w):
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
 
-    def __init__(self, index):
-        self.rows, self.proc, self.index = [], None, index
+    def __init__(self, index, interval_ms=250):
+        self.rows, self.proc, self.index, self.interval_ms = [], None, index, interval_ms
 
     def start(self):
         q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                          "-lms", str(self.interval_ms)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except OSError:
@@ -245,7 +245,7 @@ def run_ours(args, w, rank, world, local_rank):
                 dist.barrier()
             return [a.elapsed_time(b) for a, b in ev], res
 
-        clocks = ClockSampler(local_rank)
+        clocks = ClockSampler(local_rank, args.clock_interval_ms)
         clocks.start()
         ms_list, (info, info2, rc, rc2) = timed(step_matvec if args.mode == "matvec" else step_resident, args.warmup, args.steps)
         ap_ms, ap_launches, tot_launches = s.kernel_time(reset=False)
@@ -430,6 +430,7 @@ def main():
     ap.add_argument("--max-iter", type=int, default=None)
     ap.add_argument("--tol", type=float, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--clock-interval-ms", type=int, default=250, help="nvidia-smi sampling period during the timed region")
     ap.add_argument("--forward-only", action="store_true", help="recorded big-config runs: skip the adjoint solve (not the contract step)")
     ap.add_argument("--profile", action="store_true", help="for ncu: 1 warm-up, no e2e leg, no CPU baseline (not a bench value)")
     args = ap.parse_args()
