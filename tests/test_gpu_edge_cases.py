@@ -175,3 +175,16 @@ def test_adjoint_position_sensitivities(tm):
         fd = gradient.fd_position(lmax, W.K_B, pos, radii, 4.0, inc, v, 2, 2)
         assert abs(g[2, 2] - fd) <= 1e-6 * np.abs(g_ref).max()
         s.close()
+
+
+def test_fp32_precision_floor_stops_the_restart_loop(tm):
+    """A tolerance below what an fp32 operator can reach: the solver must notice (estimated residual met, true residual
+    stuck) and return the soft status after a few cycles instead of burning max_iter."""
+    w = W.config(2, scale=12)
+    ref = driver.solve(w)
+    s = tm.solver_for_workload(w, precision=tm.TM_FP32)
+    sol, info, rc = s.solve(1e-9, 50, 100000)
+    assert rc == tm.TM_NOT_CONVERGED and info[0].rel_residual < 1e-5
+    assert info[0].matvecs < 3000                        # not the 100000-iteration budget
+    assert rel(sol, ref["s"]) <= 1e-4
+    s.close()

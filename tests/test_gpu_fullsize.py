@@ -94,3 +94,25 @@ def test_cfg4_windows_are_independent_at_full_size(tm):
     assert rel(sol1, sol[lo:hi]) <= 1e-10
     assert info1[0].iterations == info[5].iterations
     s.close(); s1.close()
+
+
+def test_sym3d_kernel_on_a_large_3d_cloud(tm):
+    """Generated 3-D kernel at scale (2e4 scatterers in a slab: 157 target tiles, many source chunks): sampled oracle rows."""
+    rng = np.random.default_rng(91)
+    n = 20000
+    side = 40.0
+    # jittered grid in a slab of thickness 3 wavelengths: minimum separation stays > 0.3
+    g = int(np.ceil(np.sqrt(n / 3)))
+    ix, iy, iz = np.meshgrid(np.arange(g), np.arange(g), np.arange(3), indexing="ij")
+    pos = np.stack([ix.ravel(), iy.ravel(), iz.ravel()], axis=1)[:n].astype(float)
+    pos[:, :2] *= side / g
+    pos += rng.uniform(-0.1, 0.1, pos.shape)
+    x = rand_x((n, 30), 92)
+    s = tm.Solver(pos, 3, W.K_B)
+    assert s.get_kernel() == tm.TM_KERNEL_SYM3D
+    u = s.matvec(x, transpose=2)
+    rows = np.sort(rng.choice(n, 12, replace=False)).astype(np.int32)
+    rows[0], rows[-1] = 0, n - 1
+    ref = omv.matvec_rows(3, W.K_B, pos, x, rows=rows)
+    assert rel(u[rows], ref) <= 1e-12
+    s.close()
