@@ -427,25 +427,11 @@ def emit_general_sym(lmaxes, path):
     with open(path, "w") as f:
         f.write("// GENERATED by gen_tables.py - do not edit.\n")
         f.write("// General 3-D translation apply in the frame rotated about z onto the pair's azimuth, one y'-mirror SECTOR per call\n")
-        f.write("// (DESIGN.md, kernel K2s).  Slots as in tm_coplanar_gen.cuh; P[q(q+1)/2+mu] = Pbar_q^mu(cos theta).\n#pragma once\n\n")
+        f.write("// (DESIGN.md, kernel K2s).  Slots as in tm_coplanar_gen.cuh; Pq_mu = Pbar_q^mu(cos theta), normalised, no Condon-Shortley phase.\n#pragma once\n\n")
         for lmax in lmaxes:
             md = modes(lmax)
             idx = {t: i for i, t in enumerate(md)}
             nq = 2 * lmax + 1
-            # normalised Legendre functions Pbar_q^mu(ct), st = sin(theta) >= 0, no Condon-Shortley phase (R2)
-            f.write(f"template <typename R>\n__device__ __forceinline__ void tm_pbar_all_L{lmax}(R ct, R st, R* P) {{\n")
-            pi = lambda q, mu: q * (q + 1) // 2 + mu
-            f.write(f"  P[0] = R({lit(mp.sqrt(mp.mpf(1) / 2))});\n")
-            for mu in range(0, nq):
-                if mu > 0:
-                    f.write(f"  P[{pi(mu, mu)}] = R({lit(mp.sqrt(mp.mpf(2 * mu + 1) / (2 * mu)))}) * st * P[{pi(mu - 1, mu - 1)}];\n")
-                if mu + 1 < nq:
-                    f.write(f"  P[{pi(mu + 1, mu)}] = R({lit(mp.sqrt(mp.mpf(2 * mu + 3)))}) * ct * P[{pi(mu, mu)}];\n")
-                for q in range(mu + 2, nq):
-                    a_ = mp.sqrt(mp.mpf(4 * q * q - 1) / (q * q - mu * mu))
-                    b_ = mp.sqrt(mp.mpf((q - 1) ** 2 - mu * mu) / (4 * (q - 1) ** 2 - 1))
-                    f.write(f"  P[{pi(q, mu)}] = R({lit(a_)}) * (ct * P[{pi(q - 1, mu)}] - R({lit(b_)}) * P[{pi(q - 2, mu)}]);\n")
-            f.write("}\n")
             cost = [0, 0]
             for sct, (slots, rows) in enumerate(general_sym(lmax)):
                 n = len(slots)

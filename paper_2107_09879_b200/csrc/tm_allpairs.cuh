@@ -68,10 +68,8 @@ TM_COP_SPEC(1, 0) TM_COP_SPEC(1, 1) TM_COP_SPEC(2, 0) TM_COP_SPEC(2, 1) TM_COP_S
 // two-halves-per-block version stalled on instruction fetch: profiles/r01_allpairs_cfg3_v1.md).
 // Thread t handles target tile.tgt_start + t.  Sources of the tile's window are split into n_chunk contiguous
 // chunks (blockIdx.y) so that small problems still fill 148 SMs; each chunk is streamed through shared memory
-// SS sources at a time (positions + this half's coefficients in the tilde basis x~ = i^p x).
-// LOCKSTEP: a __syncthreads() per source keeps the block's warps on the same instructions (the two warps
-// that share an SM sub-partition then hit in its L0 instruction cache).
-template <typename R, int LMAX, int TJ, int SS, bool LOCKSTEP>
+// SS sources at a time (positions + this half's d-values in the tilde basis x~ = i^p x).
+template <typename R, int LMAX, int TJ, int SS>
 __global__ void __launch_bounds__(TJ)
 k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
                     const TmTile* __restrict__ tiles, int n_scat, double k_over_pi, double inv_k,
@@ -127,7 +125,6 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
     __syncthreads();
 #pragma unroll 1
     for (int s = 0; s < ns; ++s) {
-      if (LOCKSTEP) __syncthreads();
       const double dx = xj - s_px[s], dy = yj - s_py[s];        // d = x_dest - x_source (reading R3)
       const double r2 = dx * dx + dy * dy;
       const double rinv = (r2 > 0.0 && !(shift.on && s0 + s == j)) ? rsqrt(r2) : 0.0;   // self pair -> h_q = 0 -> nothing

@@ -47,7 +47,7 @@ struct tm_ctx {
   bool coplanar = false;
   int kernel_req = TM_KERNEL_AUTO, kernel = TM_KERNEL_GENERAL;
   TmShift shift{0.0, 0.0, 0.0, 0};      // target displacement (tm_grad_positions only)
-  int cop_tj = 128, cop_lockstep = 0;   // coplanar kernel launch shape (env TM_COP_TJ / TM_COP_LOCKSTEP override)
+  int cop_tj = 128;                     // coplanar kernel: targets per block (env TM_COP_TJ=256 for experiments)
 
   double* d_pos = nullptr;
   int* d_win_of = nullptr;
@@ -185,14 +185,11 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
   tick(c, true);
   if (c->kernel == TM_KERNEL_COPLANAR) {
     grid.z = 2;                                         // mirror-parity half: slowest grid dimension
-#define TM_LAUNCH_COP2(LM, TJ, LS)                                                                          \
-  k_allpairs_coplanar<R, LM, TJ, COP_SS, LS><<<grid, TJ, 0, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat, \
-                                                                         k_over_pi, inv_k, n_active, c->shift)
+#define TM_LAUNCH_COP2(LM, TJ)                                                                              \
+  k_allpairs_coplanar<R, LM, TJ, COP_SS><<<grid, TJ, 0, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat,    \
+                                                                     k_over_pi, inv_k, n_active, c->shift)
 #define TM_LAUNCH_COP(LM)                                                                                   \
-  do {                                                                                                      \
-    if (c->cop_tj == 256) { if (c->cop_lockstep) TM_LAUNCH_COP2(LM, 256, true); else TM_LAUNCH_COP2(LM, 256, false); } \
-    else { if (c->cop_lockstep) TM_LAUNCH_COP2(LM, 128, true); else TM_LAUNCH_COP2(LM, 128, false); }       \
-  } while (0)
+  do { if (c->cop_tj == 256) TM_LAUNCH_COP2(LM, 256); else TM_LAUNCH_COP2(LM, 128); } while (0)
     switch (c->lmax) {
       case 1: TM_LAUNCH_COP(1); break;
       case 2: TM_LAUNCH_COP(2); break;
@@ -478,7 +475,6 @@ int configure_kernel(tm_ctx* ctx) {
   if (want == TM_KERNEL_SYM3D && ctx->lmax > 3) return fail(ctx, TM_E_INVALID, "generated 3-D kernel needs lmax <= 3");
   ctx->kernel = want;
   if (const char* e = std::getenv("TM_COP_TJ")) ctx->cop_tj = std::atoi(e) == 256 ? 256 : 128;
-  if (const char* e = std::getenv("TM_COP_LOCKSTEP")) ctx->cop_lockstep = std::atoi(e) != 0;
   int tgt_per_tile;
   const bool gen = want == TM_KERNEL_COPLANAR || want == TM_KERNEL_SYM3D;      // generated kernels: thread = target
   switch (gen ? 0 : ctx->lmax) {
