@@ -84,7 +84,7 @@ typedef struct {
  *   win_ptr   HOST pointer [n_win+1], monotone, win_ptr[0] = 0, win_ptr[n_win] = n_scat; NULL (with
  *             n_win = 1) => one window.  Scatterers interact only inside their window (reading R16;
  *             independent Nyquist windows batched on one GPU).
- *   lmax      1..6 (generated kernels for lmax <= 3: coplanar when all z are equal, else 3-D; table-driven kernel above)
+ *   lmax      1..6 (generated kernels: coplanar for any lmax when all z are equal, 3-D for lmax <= 3; table-driven otherwise)
  *   k_b       background wavenumber (wavelength 1 => 2 pi)
  *   precision TM_FP64 or TM_FP32 (API data stays fp64)
  *   cuda_stream  a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) or NULL for the default stream
@@ -135,10 +135,11 @@ size_t tm_workspace_bytes(const tm_ctx *ctx, const tm_solve_opts *opts);
 int tm_set_workspace(tm_ctx *ctx, void *dev_ptr, size_t bytes);
 
 /* Force the all-pairs kernel variant (TM_KERNEL_*):
- *   COPLANAR  generated code, all z equal and lmax <= 3 (refused with TM_E_INVALID otherwise)
+ *   COPLANAR  generated code, all z equal (refused with TM_E_INVALID otherwise); two parity halves for lmax <= 3,
+ *             four mirror sectors with shared-memory accumulators for lmax 4..6
  *   SYM3D     generated code, arbitrary 3-D positions, lmax <= 3 (refused otherwise)
  *   GENERAL   table-driven, arbitrary positions, lmax <= 6
- * Default AUTO = COPLANAR if applicable, else SYM3D if lmax <= 3, else GENERAL. */
+ * Default AUTO = COPLANAR if all z are equal, else SYM3D if lmax <= 3, else GENERAL. */
 int tm_set_kernel(tm_ctx *ctx, int kernel);
 /* Which variant is active (TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR or TM_KERNEL_SYM3D). */
 int tm_get_kernel(const tm_ctx *ctx);

@@ -545,11 +545,152 @@ def emit_general_sym(lmaxes, path):
             f.write(f"#define TM_G3D_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")
 
 
+# ----------------------------------------------------------------------------- coplanar, four sectors (lmax 4..6)
+def coplanar_sectors(lmax):
+    """Coplanar operator split by BOTH mirrors into four uncoupled sectors z = 2 h + t:
+    h = z-mirror parity (l+m+p) mod 2, t = y'-mirror sector (t = 0: {p=0: '0','+'; p=1: '-'}, t = 1: the rest).
+    Returns {z: (slots, rows)} with rows[r][q] = [(c, value)]:  u^new_r = sum_q h_q sum_c value x^new_c."""
+    md = modes(lmax)
+    idx = {t_: i for i, t_ in enumerate(md)}
+    nq = 2 * lmax + 1
+    rows0 = coplanar_rows(lmax)
+    Kd = {}
+    for b in range(len(md)):
+        for q in range(nq):
+            for (a, v) in rows0[b][q]:
+                Kd[(q, b, a)] = Kd.get((q, b, a), mp.mpf(0)) + v
+    out = {}
+    for h in (0, 1):
+        for t in (0, 1):
+            slots = []
+            for p in (0, 1):
+                for l in range(1, lmax + 1):
+                    for am in range(0, l + 1):
+                        if (l + am + p) % 2 != h:
+                            continue
+                        for kind in (["0"] if am == 0 else ["+", "-"]):
+                            in0 = (p == 0 and kind in "0+") or (p == 1 and kind == "-")
+                            if in0 == (t == 0):
+                                slots.append((l, am, p, kind))
+            rows = [[[] for _ in range(nq)] for _ in slots]
+            for r, (lr, mr, pr, kr) in enumerate(slots):
+                rws = [(idx[(lr, mr, pr)], 1)] if kr == "0" else [(idx[(lr, mr, pr)], 1), (idx[(lr, -mr, pr)], 1 if kr == "+" else -1)]
+                for c, (lc, mc, pc, kc) in enumerate(slots):
+                    cls = ([(idx[(lc, mc, pc)], mp.mpf(1))] if kc == "0" else
+                           [(idx[(lc, mc, pc)], mp.mpf(1) / 2), (idx[(lc, -mc, pc)], (mp.mpf(1) if kc == "+" else -mp.mpf(1)) / 2)])
+                    for q in range(nq):
+                        v = mp.mpf(0)
+                        for (b, sb) in rws:
+                            for (a_, sa) in cls:
+                                if (q, b, a_) in Kd:
+                                    v += sb * sa * Kd[(q, b, a_)]
+                        if abs(v) > mp.mpf(10) ** -30:
+                            rows[r][q].append((c, v))
+            out[2 * h + t] = (slots, rows)
+    return out
+
+
+def emit_coplanar4(lmaxes, path):
+    with open(path, "w") as f:
+        f.write("// GENERATED by gen_tables.py - do not edit.\n")
+        f.write("// Coplanar translation apply for lmax 4..6, one of FOUR uncoupled sectors (z-mirror parity x y'-mirror sector) per call\n")
+        f.write("// (DESIGN.md, kernel K2c4).  xs: [own slots | partner slots] d-values; ar/ai: [own | partner] accumulators, stride AS.\n#pragma once\n\n")
+        for lmax in lmaxes:
+            md = modes(lmax)
+            idx = {t_: i for i, t_ in enumerate(md)}
+            nq = 2 * lmax + 1
+            half_l = len(md) // 2
+            cost = [0, 0]
+            nmax = 0
+            secs = coplanar_sectors(lmax)
+            for z in range(4):
+                slots, rows = secs[z]
+                n = len(slots)
+                nmax = max(nmax, n)
+                f.write(f"// lmax={lmax} sector z={z}: slots (l,|m|,p,kind) {slots}\n")
+                f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
+                        f"tm_cop4_pair_L{lmax}_Z{z}(const R* __restrict__ xs, const R* cm, const R* sm, const R* hr, const R* hi, R* ar, R* ai) {{\n")
+                n_pairs = n_zero = 0
+                for k, (l, am, p, kind) in enumerate(slots):
+                    if kind == "0":
+                        f.write(f"  const R xr{k} = xs[{2 * k}], xi{k} = xs[{2 * k + 1}];\n")
+                        n_zero += 1
+                    else:      # x^own = c d^own + i s d^partner
+                        f.write(f"  const R xr{k} = xs[{2 * k}] * cm[{am}] - xs[{2 * (n + k) + 1}] * sm[{am}], "
+                                f"xi{k} = xs[{2 * k + 1}] * cm[{am}] + xs[{2 * (n + k)}] * sm[{am}];\n")
+                        n_pairs += 1
+                nterm = nrowq = 0
+                for r, (l, am, p, kind) in enumerate(slots):
+                    f.write("  {\n    R ur = R(0), ui = R(0), yr, yi;\n")
+                    for q in range(nq):
+                        terms = rows[r][q]
+                        if not terms:
+                            continue
+                        nrowq += 1
+                        for t_, (c, v) in enumerate(terms):
+                            nterm += 1
+                            if t_ == 0:
+                                f.write(f"    yr = R({lit(v)}) * xr{c}; yi = R({lit(v)}) * xi{c};\n")
+                            else:
+                                f.write(f"    yr = fma(R({lit(v)}), xr{c}, yr); yi = fma(R({lit(v)}), xi{c}, yi);\n")
+                        f.write(f"    ur = fma(hr[{q}], yr, ur); ur = fma(-hi[{q}], yi, ur); ui = fma(hr[{q}], yi, ui); ui = fma(hi[{q}], yr, ui);\n")
+                    if kind == "0":
+                        f.write(f"    ar[{r} * AS] += ur; ai[{r} * AS] += ui;\n")
+                    else:      # A^own += c u ;  A^partner += -i s u
+                        f.write(f"    ar[{r} * AS] = fma(ur, cm[{am}], ar[{r} * AS]); ai[{r} * AS] = fma(ui, cm[{am}], ai[{r} * AS]);\n")
+                        f.write(f"    ar[{n + r} * AS] = fma(ui, sm[{am}], ar[{n + r} * AS]); ai[{n + r} * AS] = fma(-ur, sm[{am}], ai[{n + r} * AS]);\n")
+                    f.write("  }\n")
+                f.write("}\n")
+                inst = 2 * nterm + 4 * nrowq + 8 * n_pairs + 2 * n_zero
+                flop = (2 * nrowq + 4 * (nterm - nrowq)) + 8 * nrowq + (6 + 8) * n_pairs + 2 * n_zero
+                cost[0] += inst
+                cost[1] += flop
+                print(f"lmax={lmax} sector z={z}: n={n} terms={nterm} (row,q)={nrowq} -> {inst} FP instructions, {flop} flop", file=sys.stderr)
+                sa, sb, ss = [], [], []
+                for (l, am, p, kind) in slots:
+                    sa.append(idx[(l, am, p)]); sb.append(idx[(l, -am, p)]); ss.append({"0": 0, "+": 1, "-": -1}[kind])
+                for (l, am, p, kind) in slots:
+                    sa.append(idx[(l, am, p)]); sb.append(idx[(l, -am, p)]); ss.append({"0": 0, "+": -1, "-": 1}[kind])
+                f.write(f"__device__ __constant__ int tm_cop4_sa_L{lmax}_Z{z}[{2 * n}] = {{{', '.join(map(str, sa))}}};\n")
+                f.write(f"__device__ __constant__ int tm_cop4_sb_L{lmax}_Z{z}[{2 * n}] = {{{', '.join(map(str, sb))}}};\n")
+                f.write(f"__device__ __constant__ int tm_cop4_ss_L{lmax}_Z{z}[{2 * n}] = {{{', '.join(map(str, ss))}}};\n")
+                f.write(f"#define TM_COP4_N_L{lmax}_Z{z} {n}\n")
+                # unmix: this sector's share of u~ for the modes of its parity half (the partner sector z^1 adds the rest)
+                f.write("template <typename R, typename C, int AS>\n__device__ __forceinline__ void "
+                        f"tm_cop4_unmix_L{lmax}_Z{z}(const R* ar, const R* ai, C* out) {{\n")
+
+                def store(i_flat, re, im):
+                    if i_flat >= half_l:
+                        f.write(f"  out[{i_flat}].re = {im}; out[{i_flat}].im = -({re});\n")
+                    else:
+                        f.write(f"  out[{i_flat}].re = {re}; out[{i_flat}].im = {im};\n")
+                covered = set()
+                for r, (l, am, p, kind) in enumerate(slots):
+                    if kind == "0":
+                        store(idx[(l, 0, p)], f"ar[{r} * AS]", f"ai[{r} * AS]")
+                        covered.add(idx[(l, 0, p)])
+                    else:
+                        pr_, pi_ = (f"ar[{r} * AS]", f"ai[{r} * AS]") if kind == "+" else (f"ar[{n + r} * AS]", f"ai[{n + r} * AS]")
+                        mr_, mi_ = (f"ar[{n + r} * AS]", f"ai[{n + r} * AS]") if kind == "+" else (f"ar[{r} * AS]", f"ai[{r} * AS]")
+                        store(idx[(l, am, p)], f"R(0.5) * ({pr_} + {mr_})", f"R(0.5) * ({pi_} + {mi_})")
+                        store(idx[(l, -am, p)], f"R(0.5) * ({pr_} - {mr_})", f"R(0.5) * ({pi_} - {mi_})")
+                        covered.add(idx[(l, am, p)]); covered.add(idx[(l, -am, p)])
+                hpar = z // 2
+                for i_flat, (l, m, p) in enumerate(md):
+                    if (l + m + p) % 2 == hpar and i_flat not in covered:    # m = 0 modes owned by the partner sector
+                        f.write(f"  out[{i_flat}].re = R(0); out[{i_flat}].im = R(0);\n")
+                f.write("}\n")
+            f.write(f"#define TM_COP4_NMAX_L{lmax} {nmax}\n")
+            f.write(f"#define TM_COP4_FPINST_L{lmax} {cost[0]}   // FP instructions per ordered pair (all four sectors)\n")
+            f.write(f"#define TM_COP4_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")
+
+
 def main():
     os.makedirs(OUT, exist_ok=True)
     emit_tables([1, 2, 3, 4, 5, 6], os.path.join(OUT, "tm_tables_gen.h"))
     emit_coplanar([1, 2, 3], os.path.join(OUT, "tm_coplanar_gen.cuh"))
     emit_general_sym([1, 2, 3], os.path.join(OUT, "tm_general3d_gen.cuh"))
+    emit_coplanar4([4, 5, 6], os.path.join(OUT, "tm_coplanar4_gen.cuh"))
 
 
 if __name__ == "__main__":

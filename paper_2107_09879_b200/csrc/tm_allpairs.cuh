@@ -397,3 +397,137 @@ k_allpairs_sym3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
     else          G3dPair<R, LMAX, 1>::template unmix<TJ>(ar, ai, out);
   }
 }
+
+// ---------------------------------------------------------------------------------------------------
+// Coplanar kernel for lmax 4..6 (the paper's truncation is lmax = 6).  Same mathematics as
+// k_allpairs_coplanar, but the two mirrors split the operator into FOUR uncoupled sectors (blockIdx.z = 2 h + t,
+// slowest grid dimension), the accumulators (own sector + the partner sector's share from the output rotation) live in
+// shared memory [slot][thread], and only the sector's own x^new (<= 24 complex at lmax 6) and h_q stay in registers.
+// At lmax 6 a sector's straight-line code is ~120 KB, far beyond the instruction caches: the kernel is
+// instruction-fetch bound there, still an order of magnitude ahead of the table-driven kernel.
+#include "generated/tm_coplanar4_gen.cuh"
+
+template <typename R, int LMAX, int Z> struct Cop4;
+#define TM_COP4_SPEC(LM, ZZ)                                                                             \
+  template <typename R> struct Cop4<R, LM, ZZ> {                                                         \
+    static constexpr int n = TM_COP4_N_L##LM##_Z##ZZ;                                                    \
+    template <int AS>                                                                                    \
+    static __device__ __forceinline__ void run(const R* xs, const R* cm, const R* sm, const R* hr,       \
+                                               const R* hi, R* ar, R* ai) {                              \
+      tm_cop4_pair_L##LM##_Z##ZZ<R, AS>(xs, cm, sm, hr, hi, ar, ai);                                     \
+    }                                                                                                    \
+    template <int AS>                                                                                    \
+    static __device__ __forceinline__ void unmix(const R* ar, const R* ai, Cx<R>* out) {                 \
+      tm_cop4_unmix_L##LM##_Z##ZZ<R, Cx<R>, AS>(ar, ai, out);                                            \
+    }                                                                                                    \
+    static __device__ __forceinline__ void stage_entry(int k, int& a, int& b, int& sg) {                 \
+      a = tm_cop4_sa_L##LM##_Z##ZZ[k]; b = tm_cop4_sb_L##LM##_Z##ZZ[k]; sg = tm_cop4_ss_L##LM##_Z##ZZ[k]; \
+    }                                                                                                    \
+  };
+TM_COP4_SPEC(4, 0) TM_COP4_SPEC(4, 1) TM_COP4_SPEC(4, 2) TM_COP4_SPEC(4, 3)
+TM_COP4_SPEC(5, 0) TM_COP4_SPEC(5, 1) TM_COP4_SPEC(5, 2) TM_COP4_SPEC(5, 3)
+TM_COP4_SPEC(6, 0) TM_COP4_SPEC(6, 1) TM_COP4_SPEC(6, 2) TM_COP4_SPEC(6, 3)
+#undef TM_COP4_SPEC
+
+template <int LMAX> struct Cop4Max;
+template <> struct Cop4Max<4> { static constexpr int n = TM_COP4_NMAX_L4; };
+template <> struct Cop4Max<5> { static constexpr int n = TM_COP4_NMAX_L5; };
+template <> struct Cop4Max<6> { static constexpr int n = TM_COP4_NMAX_L6; };
+
+template <typename R, int LMAX, int TJ, int SS> struct Cop4Smem {
+  static constexpr int NM = Cop4Max<LMAX>::n;
+  static constexpr size_t bytes = sizeof(double) * 2 * SS + sizeof(R) * (size_t)(SS * 2 * NM * 2 + 2 * 2 * NM * TJ) + sizeof(int) * 3 * 2 * NM;
+};
+
+template <typename R, int LMAX, int Z, int TJ, int SS>
+__device__ __forceinline__ void cop4_sector(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
+                                            const TmTile tile, int n_scat, double k_over_pi, double inv_k, TmShift shift,
+                                            unsigned char* smem_raw) {
+  using S = Cop4<R, LMAX, Z>;
+  constexpr int L = 2 * LMAX * (LMAX + 2);
+  constexpr int NQ = 2 * LMAX + 1;
+  constexpr int NM = Cop4Max<LMAX>::n;
+  constexpr int n = S::n;
+  double* s_px = reinterpret_cast<double*>(smem_raw);
+  double* s_py = s_px + SS;
+  R* s_x = reinterpret_cast<R*>(s_py + SS);          // [source][2 n] complex: own slots then partner slots
+  R* s_acc = s_x + SS * 2 * NM * 2;                  // [re/im][2 n][TJ]
+  int* s_sa = reinterpret_cast<int*>(s_acc + 2 * 2 * NM * TJ);
+  int* s_sb = s_sa + 2 * NM;
+  int* s_ss = s_sb + 2 * NM;
+  const int tid = threadIdx.x;
+  const bool live = tid < tile.tgt_count;
+  const int j = tile.tgt_start + (live ? tid : tile.tgt_count - 1);
+  const double xj = pos[3 * j] + shift.x, yj = pos[3 * j + 1] + shift.y;
+  const int per = (tile.src_count + gridDim.y - 1) / gridDim.y;
+  const int c0 = tile.src_start + blockIdx.y * per;
+  const int c1 = min(tile.src_start + tile.src_count, c0 + per);
+  if (tid < 2 * n) {
+    int a, b, sg;
+    S::stage_entry(tid, a, b, sg);
+    s_sa[tid] = a; s_sb[tid] = b; s_ss[tid] = sg;
+  }
+  R* ar = s_acc + tid;
+  R* ai = s_acc + 2 * NM * TJ + tid;
+#pragma unroll
+  for (int b = 0; b < 2 * n; ++b) { ar[b * TJ] = R(0); ai[b * TJ] = R(0); }
+  for (int s0 = c0; s0 < c1; s0 += SS) {
+    const int ns = min(SS, c1 - s0);
+    __syncthreads();
+    for (int e = tid; e < ns; e += TJ) { s_px[e] = pos[3 * (s0 + e)]; s_py[e] = pos[3 * (s0 + e) + 1]; }
+    for (int e = tid; e < ns * 2 * n; e += TJ) {
+      const int src = e / (2 * n), kk = e - src * 2 * n;
+      const Cx<R>* xrow = x + (size_t)(s0 + src) * L;
+      const int ia = s_sa[kk], sg = s_ss[kk];
+      Cx<R> v = xrow[ia];
+      if (sg != 0) {
+        const Cx<R> o = xrow[s_sb[kk]];
+        v = sg > 0 ? cadd(v, o) : csub(v, o);
+      }
+      if (ia >= L / 2) v = cx<R>(-v.im, v.re);         // tilde basis: multiply p = 1 modes by i
+      s_x[2 * e] = v.re;
+      s_x[2 * e + 1] = v.im;
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int s = 0; s < ns; ++s) {
+      const double dx = xj - s_px[s], dy = yj - s_py[s];
+      const double r2 = dx * dx + dy * dy;
+      const double rinv = (r2 > 0.0 && !(shift.on && s0 + s == j)) ? rsqrt(r2) : 0.0;
+      const double r = r2 * rinv;
+      R cm[LMAX + 1], sm[LMAX + 1];
+      cm[0] = R(1); sm[0] = R(0);
+      cm[1] = r2 > 0.0 ? (R)(dx * rinv) : R(1); sm[1] = (R)(dy * rinv);
+#pragma unroll
+      for (int m = 2; m <= LMAX; ++m) {
+        cm[m] = cm[m - 1] * cm[1] - sm[m - 1] * sm[1];
+        sm[m] = sm[m - 1] * cm[1] + cm[m - 1] * sm[1];
+      }
+      R ck, sk;
+      phase_kr<R>(k_over_pi, r, ck, sk);
+      R hr[NQ], hi[NQ];
+      hankel_up<R, NQ>((R)(rinv * inv_k), ck, sk, hr, hi);
+      S::template run<TJ>(&s_x[s * 2 * n * 2], cm, sm, hr, hi, ar, ai);
+    }
+  }
+  if (live) {
+    Cx<R>* out = u_part + ((size_t)(blockIdx.y * 2 + (Z & 1)) * n_scat + j) * L;
+    S::template unmix<TJ>(ar, ai, out);
+  }
+}
+
+template <typename R, int LMAX, int TJ, int SS>
+__global__ void __launch_bounds__(TJ)
+k_allpairs_coplanar4(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
+                     const TmTile* __restrict__ tiles, int n_scat, double k_over_pi, double inv_k,
+                     const int* __restrict__ n_active, TmShift shift) {
+  if (n_active != nullptr && *n_active == 0) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const TmTile tile = tiles[blockIdx.x];
+  switch (blockIdx.z) {
+    case 0: cop4_sector<R, LMAX, 0, TJ, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, shift, smem_raw); break;
+    case 1: cop4_sector<R, LMAX, 1, TJ, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, shift, smem_raw); break;
+    case 2: cop4_sector<R, LMAX, 2, TJ, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, shift, smem_raw); break;
+    default: cop4_sector<R, LMAX, 3, TJ, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, shift, smem_raw); break;
+  }
+}

@@ -26,6 +26,8 @@ std::string g_create_error;
 constexpr int COP_SS = 64;       // coplanar kernel: sources per shared-memory stage
 constexpr int SYM3D_TJ = 128;    // generated 3-D kernel: targets per block
 constexpr int SYM3D_SS = 32;     // generated 3-D kernel: sources per stage
+constexpr int COP4_TJ = 128;     // four-sector coplanar kernel (lmax 4..6): targets per block
+constexpr int COP4_SS = 16;      // ... sources per stage
 constexpr int MAX_RESTART = 300;
 
 struct Gmres {                   // device scalars of the Krylov solver, sized for `restart`
@@ -183,7 +185,22 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
   Cx<R>* up = reinterpret_cast<Cx<R>*>(c->d_upart);
   dim3 grid(c->n_tiles, c->n_chunk);
   tick(c, true);
-  if (c->kernel == TM_KERNEL_COPLANAR) {
+  if (c->kernel == TM_KERNEL_COPLANAR && c->lmax > 3) {
+    grid.z = 4;                                         // (z-mirror parity, y'-mirror sector): slowest grid dimension
+#define TM_LAUNCH_C4(LM)                                                                                        \
+  {                                                                                                             \
+    const size_t sm = Cop4Smem<R, LM, COP4_TJ, COP4_SS>::bytes;                                                 \
+    cudaFuncSetAttribute(k_allpairs_coplanar4<R, LM, COP4_TJ, COP4_SS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
+    k_allpairs_coplanar4<R, LM, COP4_TJ, COP4_SS><<<grid, COP4_TJ, sm, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat, \
+                                                                                    k_over_pi, inv_k, n_active, c->shift); \
+  }
+    switch (c->lmax) {
+      case 4: TM_LAUNCH_C4(4) break;
+      case 5: TM_LAUNCH_C4(5) break;
+      default: TM_LAUNCH_C4(6) break;
+    }
+#undef TM_LAUNCH_C4
+  } else if (c->kernel == TM_KERNEL_COPLANAR) {
     grid.z = 2;                                         // mirror-parity half: slowest grid dimension
 #define TM_LAUNCH_COP2(LM, TJ)                                                                              \
   k_allpairs_coplanar<R, LM, TJ, COP_SS><<<grid, TJ, 0, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat,    \
@@ -469,16 +486,16 @@ void fill_const(tm_ctx* c) {
 int configure_kernel(tm_ctx* ctx) {
   int want = ctx->kernel_req;
   if (want == TM_KERNEL_AUTO)
-    want = (ctx->coplanar && ctx->lmax <= 3) ? TM_KERNEL_COPLANAR : (ctx->lmax <= 3 ? TM_KERNEL_SYM3D : TM_KERNEL_GENERAL);
-  if (want == TM_KERNEL_COPLANAR && !(ctx->coplanar && ctx->lmax <= 3))
-    return fail(ctx, TM_E_INVALID, "coplanar kernel needs all z equal and lmax <= 3");
+    want = ctx->coplanar ? TM_KERNEL_COPLANAR : (ctx->lmax <= 3 ? TM_KERNEL_SYM3D : TM_KERNEL_GENERAL);
+  if (want == TM_KERNEL_COPLANAR && !ctx->coplanar)
+    return fail(ctx, TM_E_INVALID, "coplanar kernel needs all z equal");
   if (want == TM_KERNEL_SYM3D && ctx->lmax > 3) return fail(ctx, TM_E_INVALID, "generated 3-D kernel needs lmax <= 3");
   ctx->kernel = want;
   if (const char* e = std::getenv("TM_COP_TJ")) ctx->cop_tj = std::atoi(e) == 256 ? 256 : 128;
   int tgt_per_tile;
   const bool gen = want == TM_KERNEL_COPLANAR || want == TM_KERNEL_SYM3D;      // generated kernels: thread = target
   switch (gen ? 0 : ctx->lmax) {
-    case 0: tgt_per_tile = want == TM_KERNEL_SYM3D ? SYM3D_TJ : ctx->cop_tj; break;
+    case 0: tgt_per_tile = want == TM_KERNEL_SYM3D ? SYM3D_TJ : (ctx->lmax > 3 ? COP4_TJ : ctx->cop_tj); break;
     case 1: case 2: case 3: tgt_per_tile = 4; break;
     default: tgt_per_tile = 2; break;
   }
@@ -494,8 +511,9 @@ int configure_kernel(tm_ctx* ctx) {
   // small problems fill the 148 SMs (2 resident 128-thread blocks each at 255 registers) and large ones end
   // without a long tail; bounded by 64 chunks, >= 32 sources per chunk and 2 GB of partial sums.
   const long long slots = 148LL * (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj : (want == TM_KERNEL_SYM3D ? 2 : 4));
-  const long long blocks1 = (long long)ctx->n_tiles * (gen ? 2 : 1);
-  const int part_mult = want == TM_KERNEL_SYM3D ? 2 : 1;        // SYM3D: one partial buffer per (chunk, sector)
+  const bool cop4 = want == TM_KERNEL_COPLANAR && ctx->lmax > 3;   // four-sector coplanar kernel (lmax 4..6)
+  const long long blocks1 = (long long)ctx->n_tiles * (cop4 ? 4 : (gen ? 2 : 1));
+  const int part_mult = (want == TM_KERNEL_SYM3D || cop4) ? 2 : 1;   // one partial buffer per (chunk, y'-sector)
   int max_win = 1;
   for (int w = 0; w < ctx->n_win; ++w) max_win = std::max(max_win, ctx->win_ptr[w + 1] - ctx->win_ptr[w]);
   const size_t vec_bytes = ctx->n * elem_bytes(ctx);
@@ -1259,8 +1277,8 @@ int tm_pair_cost(const tm_ctx* ctx, double* fp_instructions, double* flop) {
   if (!ctx) return TM_E_INVALID;
   double inst = 0.0, fl = 0.0;
   if (ctx->kernel == TM_KERNEL_COPLANAR) {
-    const int I[4] = {0, TM_COP_FPINST_L1, TM_COP_FPINST_L2, TM_COP_FPINST_L3};
-    const int F[4] = {0, TM_COP_FLOP_L1, TM_COP_FLOP_L2, TM_COP_FLOP_L3};
+    const int I[7] = {0, TM_COP_FPINST_L1, TM_COP_FPINST_L2, TM_COP_FPINST_L3, TM_COP4_FPINST_L4, TM_COP4_FPINST_L5, TM_COP4_FPINST_L6};
+    const int F[7] = {0, TM_COP_FLOP_L1, TM_COP_FLOP_L2, TM_COP_FLOP_L3, TM_COP4_FLOP_L4, TM_COP4_FLOP_L5, TM_COP4_FLOP_L6};
     inst = I[ctx->lmax]; fl = F[ctx->lmax];
   } else if (ctx->kernel == TM_KERNEL_SYM3D) {
     const int I[4] = {0, TM_G3D_FPINST_L1, TM_G3D_FPINST_L2, TM_G3D_FPINST_L3};

@@ -47,6 +47,21 @@ def test_generated_3d_pair_code_matches_oracle_block(lmax, tmp_path):
         assert np.abs(u - ref).max() <= 2e-13 * np.abs(ref).max()
 
 
+@pytest.mark.parametrize("lmax", [4, 5, 6])
+def test_generated_four_sector_coplanar_code_matches_oracle_block(lmax, tmp_path):
+    exe = str(tmp_path / f"hostcheck4_{lmax}")
+    subprocess.check_call(["g++", "-O0", f"-DLMAX={lmax}", "-o", exe, os.path.join(ROOT, "tests", "hostcheck_coplanar4.cpp")])
+    rng = np.random.default_rng(60 + lmax)
+    L = n_modes(lmax)
+    for d in ([0.5, 0.0], [0.0, -0.5], rng.uniform(-20, 20, 2)):
+        x = rng.standard_normal(L) + 1j * rng.standard_normal(L)
+        inp = f"{float(d[0])!r} {float(d[1])!r}\n" + "\n".join(f"{float(z.real)!r} {float(z.imag)!r}" for z in x) + "\n"
+        out = subprocess.run([exe], input=inp, capture_output=True, text=True, check=True).stdout
+        u = np.array([complex(*map(float, ln.split())) for ln in out.strip().splitlines()])
+        ref = tr.block(lmax, K, np.array([d[0], d[1], 0.0]), np.zeros(3)) @ x
+        assert np.abs(u - ref).max() <= 5e-13 * np.abs(ref).max()
+
+
 def _parse_table(text, name, conv):
     m = re.search(name + r"\[\d+\] = \{(.*?)\};", text, flags=re.S)
     return [conv(t) for t in m.group(1).replace("\n", " ").split(",") if t.strip()]

@@ -101,7 +101,7 @@ def test_lmax6_solve_small(tm):
     w = W.cloud_workload(8, seed=66, lmax=6, planar=True)
     ref = driver.solve(w)
     s = tm.solver_for_workload(w)
-    assert s.get_kernel() == tm.TM_KERNEL_GENERAL        # planar but lmax > 3
+    assert s.get_kernel() == tm.TM_KERNEL_COPLANAR       # planar: four-sector generated kernel for lmax > 3
     p = s.get_incident()
     assert rel(p, ref["p"]) <= 1e-13
     sol, info, rc = s.solve(1e-11, 60, 600)
@@ -187,4 +187,26 @@ def test_fp32_precision_floor_stops_the_restart_loop(tm):
     assert rc == tm.TM_NOT_CONVERGED and info[0].rel_residual < 1e-5
     assert info[0].matvecs < 3000                        # not the 100000-iteration budget
     assert rel(sol, ref["s"]) <= 1e-4
+    s.close()
+
+
+@pytest.mark.parametrize("lmax", [4, 5, 6])
+def test_four_sector_coplanar_kernel(tm, lmax):
+    """lmax 4..6 on planar layouts (lmax = 6 is the paper's truncation): several 128-target tiles with a ragged tail,
+    source chunks, ragged windows, against the oracle and against the table-driven kernel; fp32 too."""
+    pos = W.lattice(13, 11 if lmax == 6 else 14)
+    pos = pos + np.random.default_rng(lmax).uniform(-0.05, 0.05, pos.shape) * [1, 1, 0]      # not a perfect lattice
+    N, L = pos.shape[0], W.n_modes(lmax)
+    wp = np.array([0, 40, 41, N], dtype=np.int32)
+    x = rand_x((N, L), 70 + lmax)
+    ref = omv.matvec_rows(lmax, W.K_B, pos, x, win_ptr=wp)
+    s = tm.Solver(pos, lmax, W.K_B, win_ptr=wp)
+    assert s.get_kernel() == tm.TM_KERNEL_COPLANAR
+    u = s.matvec(x, transpose=2)
+    assert rel(u, ref) <= 1e-12 and np.all(u[40] == 0)
+    s.set_kernel(tm.TM_KERNEL_GENERAL)
+    assert rel(s.matvec(x, transpose=2), u) <= 1e-12
+    s.close()
+    s = tm.Solver(pos, lmax, W.K_B, win_ptr=wp, precision=tm.TM_FP32)
+    assert rel(s.matvec(x, transpose=2), ref) <= 2e-5
     s.close()
