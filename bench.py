@@ -425,6 +425,7 @@ def main():
     ap.add_argument("--group", type=int, default=16, help="nyquist mode: samples per group side")
     ap.add_argument("--padding", type=float, default=4.0, help="nyquist mode: padding in wavelengths")
     ap.add_argument("--kernel", default="auto", choices=["auto", "general", "coplanar", "sym3d"], help="force the all-pairs kernel variant")
+    ap.add_argument("--lmax", type=int, default=None, help="override the VSWF truncation of a Mie config (lmax 6 = the paper's, PAPER.md:271)")
     ap.add_argument("--scale", type=int, default=None, help="lattice side override (parity-size runs)")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
     ap.add_argument("--max-iter", type=int, default=None)
@@ -444,6 +445,12 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     name = args.workload[3:] if args.workload.startswith("cfg") else args.workload
     w = W.config(name if name == "3b" else int(name), scale=args.scale)
+    if args.lmax is not None:
+        assert w["t_kind"] != "full_types", "--lmax needs a Mie config"
+        w["lmax"] = args.lmax
+        w["name"] += f"_lmax{args.lmax}"
+        if "w_adj" in w:
+            del w["w_adj"]
     if args.mode == "nyquist":
         if rank == 0:
             run_nyquist(args, w)
