@@ -925,7 +925,6 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
     TM_CUDA(e);
   } else if (kind == TM_INC_GAUSS || kind == TM_INC_JINC) {
     // both are angular-spectrum sources (Eqs. II9-II17): per window a list of source centres with transverse amplitudes
-    if (lmax > 3) return fail(ctx, TM_E_INVALID, "beam / jinc-source expansion is built for lmax <= 3");
     std::vector<double> hsrc;
     std::vector<double2> hamp;
     std::vector<int> hptr(ctx->n_win + 1);
@@ -961,7 +960,7 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
     gauss_legendre(nb, xg, wg);
     for (int q = 0; q < nb; ++q) { beta[q] = 0.5 * bmax * (xg[q] + 1.0); wq[q] = 0.5 * bmax * wg[q]; }
     double *d_beta = nullptr, *d_wq = nullptr, *d_src = nullptr; double2* d_amp = nullptr; int* d_ptr = nullptr; void* d_nodes = nullptr;
-    const size_t node_bytes = lmax == 1 ? sizeof(GaussNode<1>) : lmax == 2 ? sizeof(GaussNode<2>) : sizeof(GaussNode<3>);
+    const size_t node_bytes = sizeof(GaussNode<TM_MAX_LMAX>);      // upper bound for every lmax
     cudaError_t e = cudaMalloc(&d_beta, nb * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&d_wq, nb * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&d_src, std::max<size_t>(1, nsrc) * 3 * sizeof(double));
@@ -978,7 +977,14 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
   k_gauss_nodes<LM><<<(nb + 127) / 128, 128, 0, ctx->stream>>>(d_beta, d_wq, nb, kw, static_cast<GaussNode<LM>*>(d_nodes)); \
   k_incident_gauss<LM><<<ctx->n_scat, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->d_win_of, d_src, d_amp, d_ptr,            \
                                                             static_cast<GaussNode<LM>*>(d_nodes), nb, ctx->k, ctx->d_p)
-      if (lmax == 1) { TM_GAUSS(1); } else if (lmax == 2) { TM_GAUSS(2); } else { TM_GAUSS(3); }
+      switch (lmax) {
+        case 1: TM_GAUSS(1); break;
+        case 2: TM_GAUSS(2); break;
+        case 3: TM_GAUSS(3); break;
+        case 4: TM_GAUSS(4); break;
+        case 5: TM_GAUSS(5); break;
+        default: TM_GAUSS(6); break;
+      }
 #undef TM_GAUSS
       ctx->total_launches += 2;
       e = cudaGetLastError();
@@ -1037,7 +1043,6 @@ int tm_fields(tm_ctx* ctx, int n_pts, const double* pts, const tm_c64* s, int wh
   if (!ctx) return TM_E_INVALID;
   if (n_pts < 1 || !pts || !s || !out) return fail(ctx, TM_E_INVALID, "bad arguments");
   if (which != TM_FIELD_E_SCA && which != TM_FIELD_H_SCA) return fail(ctx, TM_E_INVALID, "unknown field id");
-  if (ctx->lmax > 3) return fail(ctx, TM_E_INVALID, "field evaluation is built for lmax <= 3");
   const int nchunk = std::max(1, std::min(64, (int)(148LL * 8 * 128 / std::max(1, n_pts))));
   const int nch = std::min(nchunk, std::max(1, ctx->n_scat / 32));
   double* d_pts = nullptr; double2 *d_part = nullptr, *d_out = nullptr;
@@ -1050,9 +1055,16 @@ int tm_fields(tm_ctx* ctx, int n_pts, const double* pts, const tm_c64* s, int wh
   if (e == cudaSuccess) {
     dim3 grid((n_pts + 127) / 128, nch);
     const int swap = which == TM_FIELD_H_SCA ? 1 : 0;
-    if (ctx->lmax == 1) k_fields<1><<<grid, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->n_scat, ctx->d_io, d_pts, n_pts, ctx->k, swap, d_part);
-    else if (ctx->lmax == 2) k_fields<2><<<grid, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->n_scat, ctx->d_io, d_pts, n_pts, ctx->k, swap, d_part);
-    else k_fields<3><<<grid, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->n_scat, ctx->d_io, d_pts, n_pts, ctx->k, swap, d_part);
+#define TM_FIELDS(LM) k_fields<LM><<<grid, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->n_scat, ctx->d_io, d_pts, n_pts, ctx->k, swap, d_part)
+    switch (ctx->lmax) {
+      case 1: TM_FIELDS(1); break;
+      case 2: TM_FIELDS(2); break;
+      case 3: TM_FIELDS(3); break;
+      case 4: TM_FIELDS(4); break;
+      case 5: TM_FIELDS(5); break;
+      default: TM_FIELDS(6); break;
+    }
+#undef TM_FIELDS
     k_fields_reduce<<<(unsigned)((nout + 255) / 256), 256, 0, ctx->stream>>>(d_part, nch, nout, d_out);
     ctx->total_launches += 2;
     e = cudaGetLastError();

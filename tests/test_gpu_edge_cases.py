@@ -210,3 +210,25 @@ def test_four_sector_coplanar_kernel(tm, lmax):
     s = tm.Solver(pos, lmax, W.K_B, win_ptr=wp, precision=tm.TM_FP32)
     assert rel(s.matvec(x, transpose=2), ref) <= 2e-5
     s.close()
+
+
+@pytest.mark.parametrize("lmax", [4, 6])
+def test_incident_and_fields_at_high_lmax(tm, lmax):
+    """Beam / jinc expansion and field evaluation for lmax up to 6 (the paper's truncation)."""
+    from oracle import fields, incident
+    pos = W.random_cloud(6, seed=50 + lmax)
+    s = tm.Solver(pos, lmax, W.K_B)
+    focus = np.array([[0.2, -0.1, 0.3]])
+    s.set_incident_gauss(focus, 2.0, 0.8, 0.3 - 0.4j)
+    ref = incident.gaussian_beam_incident(lmax, W.K_B, pos, focus[0], 2.0, 0.8, 0.3 - 0.4j)
+    assert rel(s.get_incident(), ref) <= 1e-10
+    src = np.array([[0.5, 0.5, -2.0], [-1.0, 0.2, -2.0]])
+    amp = np.array([[1.0, 0.2j], [0.3, -0.7]])
+    s.set_incident_jinc(src, amp)
+    assert rel(s.get_incident(), incident.jinc_sources_incident(lmax, W.K_B, pos, src, amp)) <= 1e-10
+    coef = rand_x((6, W.n_modes(lmax)), lmax)
+    pts = np.random.default_rng(lmax).uniform(-4, 4, (40, 3))
+    pts = pts[np.linalg.norm(pts[:, None, :] - pos[None], axis=2).min(axis=1) > 0.4]
+    assert rel(s.fields(pts, coef, tm.TM_FIELD_E_SCA), fields.e_sca(lmax, W.K_B, pos, coef, pts)) <= 1e-12
+    assert rel(s.fields(pts, coef, tm.TM_FIELD_H_SCA), fields.zh_sca(lmax, W.K_B, pos, coef, pts)) <= 1e-12
+    s.close()
