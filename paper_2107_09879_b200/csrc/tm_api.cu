@@ -366,7 +366,13 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
     last_mc = mc;
     for (int j = 0; j < mc; ++j) {
       Cx<R>* Vj = V + (size_t)j * n;
-      TM_CUDA(apply_operator<R>(ctx, transpose, Vj, W, Z, S.n_active));
+      const bool fuse_t = coop && ctx->diag;       // T application folded into the cooperative step
+      if (fuse_t) {
+        if (transpose == 1 && j == 0) TM_CUDA(launch_tapply<R>(ctx, 4, Vj, Z, S.n_active));   // z = P T^T v_0
+        TM_CUDA(launch_allpairs<R>(ctx, transpose == 1 ? Z : Vj, S.n_active));
+      } else {
+        TM_CUDA(apply_operator<R>(ctx, transpose, Vj, W, Z, S.n_active));
+      }
       matvecs++;
       // split the basis vectors of a dot-product pass over gridDim.y when there are few chunks
       const int G = std::max(1, std::min((j + 1 + 7) / 8, (148 * 4 + nc - 1) / nc));
@@ -390,7 +396,9 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
         const Cx<R>* Vc = V; size_t nn = n; int jj = j, ncc = nc, nww = nw; double tl = o.tol;
         Cx<R>* Wc = W; const TmChunk* chk = ctx->d_chunks; double2* prt = ctx->gm.part; double* npt = ctx->gm.normpart;
         const int* wcp = ctx->d_win_chunk_ptr; TmGmresDev Sc = S;
-        void* args[] = {&Vc, &nn, &jj, &Wc, &chk, &ncc, &prt, &npt, &wcp, &Sc, &nww, &tl};
+        TmFuseT<R> ft{fuse_t ? (transpose == 1 ? 2 : 1) : 0, Vj, reinterpret_cast<const Cx<R>*>(ctx->d_upart), ctx->n_part, n,
+                      reinterpret_cast<const Cx<R>*>(ctx->d_T), ctx->d_type_of, ctx->d_const->perm_neg_m, ctx->L, Z};
+        void* args[] = {&Vc, &nn, &jj, &Wc, &chk, &ncc, &prt, &npt, &wcp, &Sc, &nww, &tl, &ft};
         const void* fn = ctx->ept == 1 ? (const void*)k_arnoldi_fused<R, 1> : (const void*)k_arnoldi_fused<R, 4>;
         TM_CUDA(cudaLaunchCooperativeKernel(fn, dim3(nc), dim3(TM_VT), args, std::max(sm_a, sm_g), st));
         ctx->total_launches += 1;
