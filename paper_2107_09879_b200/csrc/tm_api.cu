@@ -29,6 +29,7 @@ constexpr int SYM3D_SS = 32;     // generated 3-D kernel: sources per stage
 constexpr int COP4_TJ = 128;     // four-sector coplanar kernel (lmax 4..6): targets per block
 constexpr int COP4_SS = 16;      // ... sources per stage
 constexpr int MAX_RESTART = 300;
+static_assert(MAX_RESTART + 1 <= TM_MAX_LDH, "k_gmres_solve_y keeps y in shared memory");
 
 struct Gmres {                   // device scalars of the Krylov solver, sized for `restart`
   int restart = 0;
@@ -415,7 +416,7 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
 #undef TM_AXPY
     }
     // x += V y ; r = b - M x
-    k_gmres_solve_y<<<wb, 64, 0, st>>>(S, nw);
+    k_gmres_solve_y<<<nw, 32, 0, st>>>(S, nw);
     if (ctx->ept == 1) k_axpy<R, 1><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr, nc, ctx->d_win_chunk_ptr, nullptr);
     else k_axpy<R, 4><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr, nc, ctx->d_win_chunk_ptr, nullptr);
     TM_CUDA(apply_operator<R>(ctx, transpose, X, W, Z, nullptr));

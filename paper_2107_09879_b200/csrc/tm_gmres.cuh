@@ -113,23 +113,33 @@ k_gmres_givens(TmGmresDev S, int n_win, int j, double tol, const double* __restr
   givens_body(S, w, j, tol, normpart, win_chunk_ptr, threadIdx.x, s_givens);
 }
 
-// y = R^{-1} g over the accepted columns.
-__global__ void k_gmres_solve_y(TmGmresDev S, int n_win) {
-  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+// y = R^{-1} g over the accepted columns.  One warp per window (grid = n_win, block = 32): each row's dot product is
+// split over the lanes (parallel loads of the rotated Hessenberg row, fixed summation order), y is kept in shared memory.
+#define TM_MAX_LDH 304
+__global__ void __launch_bounds__(32) k_gmres_solve_y(TmGmresDev S, int n_win) {
+  const int w = blockIdx.x, lane = threadIdx.x;
   if (w >= n_win) return;
+  __shared__ double2 s_y[TM_MAX_LDH];
   const int ldh = S.ldh, k = S.kcols[w];
   double2* y = S.y + (size_t)w * ldh;
-  const double2* g = S.g + (size_t)w * ldh;
-  for (int i = 0; i < ldh; ++i) y[i] = make_double2(0.0, 0.0);
+  for (int i = lane; i < ldh; i += 32) { s_y[i] = i < k ? S.g[(size_t)w * ldh + i] : make_double2(0.0, 0.0); y[i] = make_double2(0.0, 0.0); }
+  __syncwarp();
   for (int i = k - 1; i >= 0; --i) {
-    double2 acc = g[i];
-    for (int c = i + 1; c < k; ++c) {
-      const double2 t = d2mul(S.Rm[((size_t)w * S.m + c) * ldh + i], y[c]);
-      acc.x -= t.x; acc.y -= t.y;
+    double ar = 0.0, ai = 0.0;
+    for (int c = i + 1 + lane; c < k; c += 32) {
+      const double2 t = d2mul(S.Rm[((size_t)w * S.m + c) * ldh + i], s_y[c]);       // s_y[c] holds y[c] for c > i
+      ar += t.x; ai += t.y;
     }
-    const double2 d = S.Rm[((size_t)w * S.m + i) * ldh + i];
-    const double dd = d.x * d.x + d.y * d.y;
-    if (dd > 0.0) y[i] = make_double2((acc.x * d.x + acc.y * d.y) / dd, (acc.y * d.x - acc.x * d.y) / dd);
+    ar = warp_sum(ar); ai = warp_sum(ai);
+    if (lane == 0) {
+      const double2 d = S.Rm[((size_t)w * S.m + i) * ldh + i];
+      const double dd = d.x * d.x + d.y * d.y;
+      const double nr = s_y[i].x - ar, ni = s_y[i].y - ai;
+      const double2 yi = dd > 0.0 ? make_double2((nr * d.x + ni * d.y) / dd, (ni * d.x - nr * d.y) / dd) : make_double2(0.0, 0.0);
+      s_y[i] = yi;
+      y[i] = yi;
+    }
+    __syncwarp();
   }
 }
 
