@@ -469,7 +469,6 @@ void fill_const(tm_ctx* c) {
   TmConst& t = c->h_const;
   std::memset(&t, 0, sizeof(t));
   const int lmax = c->lmax, L = c->L, LH = L / 2;
-  int cnt[2] = {0, 0};
   for (int p = 0; p < 2; ++p)
     for (int l = 1; l <= lmax; ++l)
       for (int m = -l; m <= l; ++m) {
@@ -477,10 +476,6 @@ void fill_const(tm_ctx* c) {
         t.mode_l[idx] = l; t.mode_m[idx] = m; t.mode_p[idx] = p;
         t.perm_neg_m[idx] = p * LH + l * (l + 1) - 1 - m;
       }
-  for (int idx = 0; idx < L; ++idx) {                    // flat order within each mirror-parity half
-    const int h = (t.mode_l[idx] + t.mode_m[idx] + t.mode_p[idx]) & 1;
-    t.cop_slot[idx] = h * LH + cnt[h]++;
-  }
   for (int q = 0; q <= TM_MAX_NQ; ++q)
     for (int mu = 0; mu <= q && mu <= TM_MAX_NQ; ++mu) {
       if (q > mu) {

@@ -47,7 +47,6 @@ struct TmTile { int tgt_start, tgt_count, src_start, src_count; };
 struct TmConst {
   int perm_neg_m[96];          // flat index of (l,-m,p)               (structural identity S3)
   int mode_l[96], mode_m[96], mode_p[96];
-  int cop_slot[96];            // coplanar kernel: flat idx -> half*NH + position in half
   double leg_a[TM_MAX_NQ + 1][TM_MAX_NQ + 1];   // normalised Legendre recurrence Pbar_q^mu = a (ct Pbar_{q-1}^mu - b Pbar_{q-2}^mu)
   double leg_b[TM_MAX_NQ + 1][TM_MAX_NQ + 1];
   double leg_d[TM_MAX_NQ + 1];                  // Pbar_mu^mu = d[mu] * sin(theta) * Pbar_{mu-1}^{mu-1}
