@@ -42,8 +42,7 @@ __device__ __forceinline__ double warp_sum(double v) {
 // Work item of the all-pairs kernels: a tile of consecutive targets inside one window.
 struct TmTile { int tgt_start, tgt_count, src_start, src_count; };
 
-// Small constant tables (set once per context; identical for all contexts of the same lmax, which is
-// why they can live in __constant__: they only depend on lmax).
+// Small per-lmax tables, one device copy per context (tm_ctx::d_const).
 struct TmConst {
   int perm_neg_m[96];          // flat index of (l,-m,p)               (structural identity S3)
   int mode_l[96], mode_m[96], mode_p[96];

@@ -62,18 +62,43 @@ def build_batch(pos, src, amp, plans):
                 src=np.ascontiguousarray(src[sord]), amp=np.ascontiguousarray(amp[sord]), src_ptr=src_ptr)
 
 
+def partition_plans(plans, rank, world):
+    """Multi-GPU split: windows are independent, so rank r takes the windows r, r + world, ...; nothing is
+    exchanged during the solves.  Greedy balance is unnecessary: every window holds about the same number of pairs."""
+    return [p for i, p in enumerate(plans) if i % world == rank]
+
+
+def sum_fields(E_local, dist=None):
+    """The one communication step of the strategy ("consolidate the electric field data"): sum the detector
+    fields of all ranks.  E_local: numpy complex array (M, 3); dist: an initialised torch.distributed module or None."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return E_local
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(np.stack([E_local.real, E_local.imag], axis=0)))
+    if dist.get_backend() == "nccl":
+        t = t.cuda()
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    t = t.cpu().numpy()
+    return t[0] + 1j * t[1]
+
+
 def simulate(w, src, amp, grid_index, group, padding, pts, tol=1e-8, restart=50, max_iter=5000, precision=libtm.TM_FP64,
-             stream=None):
+             stream=None, rank=0, world=1, dist=None):
     """Distributed simulation of workload `w` (global layout: pos, lmax, k, Mie radii per site or per type) driven by the
     jinc sources (src, amp): plan windows, batch them, solve once, sum the scattered E fields of all windows at `pts`.
     group = None: one window with every scatterer and every source (the undistributed reference).
+    rank / world / dist: multi-GPU replicas - each rank solves its share of the windows, one all_reduce sums the fields.
     Returns (E (M,3), info dict)."""
     pos = w["pos"]
     if group is None:
         plans = [(np.arange(src.shape[0]), np.arange(pos.shape[0]))]
     else:
-        plans = plan_windows(pos, src, grid_index, group, padding)
+        plans = partition_plans(plan_windows(pos, src, grid_index, group, padding), rank, world)
     b = build_batch(pos, src, amp, plans)
+    if b["pos"].shape[0] == 0:                          # a rank without windows still joins the field sum
+        E = sum_fields(np.zeros((np.asarray(pts).shape[0], 3), dtype=complex), dist)
+        return E, dict(n_windows=0, n_batched_scatterers=0, rc=0, iterations=0, seconds=0.0, max_rel_residual=0.0, batch=b,
+                       solution=np.zeros((0, libtm.lib().tm_num_modes(w["lmax"])), dtype=complex))
     s = libtm.Solver(b["pos"], w["lmax"], w["k"], win_ptr=b["win_ptr"], precision=precision, stream=stream)
     type_of = np.asarray(w["type_of"])[b["scat_index"]]
     if w["t_kind"] in ("mie_types", "mie_sites"):
@@ -85,7 +110,7 @@ def simulate(w, src, amp, grid_index, group, padding, pts, tol=1e-8, restart=50,
         s.set_tmatrices(w["t_full"], type_of.astype(np.int32), False)
     s.set_incident_jinc(b["src"], b["amp"], b["src_ptr"])
     sol, info, rc = s.solve(tol, restart, max_iter)
-    E = s.fields(np.ascontiguousarray(pts, dtype=np.float64), sol, libtm.TM_FIELD_E_SCA)
+    E = sum_fields(s.fields(np.ascontiguousarray(pts, dtype=np.float64), sol, libtm.TM_FIELD_E_SCA), dist)
     out = dict(n_windows=len(b["win_ptr"]) - 1, n_batched_scatterers=int(b["pos"].shape[0]), rc=rc,
                iterations=max(i.iterations for i in info), seconds=info[0].seconds,
                max_rel_residual=max(i.rel_residual for i in info), batch=b, solution=sol)

@@ -53,3 +53,33 @@ def test_reference_arm_runs_on_rank0_only():
     line = json.loads(out.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "cMAC/s"
+
+
+def _nyq_worker(rank, world, port, out_dir):
+    sys.path.insert(0, ROOT)
+    import numpy as np
+    from paper_2107_09879_b200 import nyquist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    plans = [(np.array([i]), np.array([i, i + 1])) for i in range(5)]
+    mine = nyquist.partition_plans(plans, rank, world)
+    # a stand-in for the per-window field (the solver needs a GPU): window i contributes (i + 1) at every detector point
+    E_local = np.zeros((4, 3), dtype=complex)
+    for sidx, _ in mine:
+        E_local += (sidx[0] + 1) * (1.0 + 0.5j)
+    E = nyquist.sum_fields(E_local, dist)
+    np.save(os.path.join(out_dir, f"E{rank}.npy"), E)
+    with open(os.path.join(out_dir, f"n{rank}.txt"), "w") as f:
+        f.write(str(len(mine)))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_nyquist_windows_split_over_ranks_and_field_sum_gloo(tmp_path):
+    """The strategy's only communication: windows are dealt to the ranks, the detector fields are summed once."""
+    import numpy as np
+    port = 31500 + os.getpid() % 2000
+    mp.spawn(_nyq_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    E0, E1 = np.load(tmp_path / "E0.npy"), np.load(tmp_path / "E1.npy")
+    assert np.array_equal(E0, E1) and np.allclose(E0, 15 * (1.0 + 0.5j))        # 1 + 2 + 3 + 4 + 5
+    assert int(open(tmp_path / "n0.txt").read()) == 3 and int(open(tmp_path / "n1.txt").read()) == 2
