@@ -177,7 +177,7 @@ def run_ours(args, w, rank, world, local_rank):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    prec = libtm.TM_FP32 if args.precision == "fp32" else libtm.TM_FP64
+    prec = {"fp32": libtm.TM_FP32, "mixed": libtm.TM_MIXED}.get(args.precision, libtm.TM_FP64)
     st = torch.cuda.Stream()
     N, L = w["pos"].shape[0], W.n_modes(w["lmax"])
     pairs = n_pairs(w)
@@ -317,7 +317,7 @@ def run_ours(args, w, rank, world, local_rank):
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": t_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64" if prec == libtm.TM_FP64 else "f32", "data": "synthetic",
+            "dtype": {libtm.TM_FP64: "f64", libtm.TM_FP32: "f32"}.get(prec, "f32 cycles + f64 residual/iterate"), "data": "synthetic",
             "config": {"workload": w["name"], "n_scat": N, "lmax": w["lmax"], "L": L, "n_windows": len(w["win_ptr"]) - 1,
                        "ordered_pairs": pairs, "tol": tol, "restart": w["restart"],
                        "step": ("one operator application y = (I - T A) x (matvec-only mode)" if args.mode == "matvec" else
@@ -427,7 +427,8 @@ def main():
     ap.add_argument("--kernel", default="auto", choices=["auto", "general", "coplanar", "sym3d"], help="force the all-pairs kernel variant")
     ap.add_argument("--lmax", type=int, default=None, help="override the VSWF truncation of a Mie config (lmax 6 = the paper's, PAPER.md:271)")
     ap.add_argument("--scale", type=int, default=None, help="lattice side override (parity-size runs)")
-    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"],
+                    help="mixed: GMRES with iterative refinement (fp32 Krylov cycles, fp64 iterate and true residual)")
     ap.add_argument("--max-iter", type=int, default=None)
     ap.add_argument("--tol", type=float, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -34,7 +34,10 @@ extern "C" {
 typedef struct tm_ctx tm_ctx;
 typedef struct { double re, im; } tm_c64;
 
-enum { TM_FP64 = 0, TM_FP32 = 1 };                       /* internal compute precision of the solver */
+enum { TM_FP64 = 0, TM_FP32 = 1, TM_MIXED = 2 };         /* internal compute precision of the solver:
+   TM_MIXED = GMRES with iterative refinement: Krylov cycles (all-pairs kernel, basis, orthogonalisation) in fp32, the
+   iterate, the right-hand side and the TRUE residual of every restart in fp64 - fp64-accurate solutions at close to the
+   fp32 kernel's speed; everything outside tm_solve / tm_solve_adjoint runs in fp64 */
 enum { TM_OK = 0, TM_NOT_CONVERGED = 1,
        TM_E_INVALID = -1, TM_E_OVERLAP = -2, TM_E_STATE = -3, TM_E_CUDA = -4, TM_E_NOMEM = -5 };
 enum { TM_INC_PLANE = 0, TM_INC_GAUSS = 1, TM_INC_COEFFS = 2, TM_INC_JINC = 3 };

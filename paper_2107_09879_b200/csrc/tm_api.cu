@@ -7,6 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "tm_allpairs.cuh"
@@ -56,6 +57,7 @@ struct tm_ctx {
   int* d_win_of = nullptr;
   int* d_type_of = nullptr;
   void* d_T = nullptr;           // Cx<R> [n_types][L] or [n_types][L][L]
+  void* d_T32 = nullptr;         // TM_MIXED only: fp32 copy of T for the inner Krylov cycles
   int n_types = 0, diag = 1;
   bool has_T = false, has_inc = false;
   double2* d_p = nullptr;        // incident coefficients, fp64 [n]
@@ -112,7 +114,8 @@ cudaError_t copy_out(void* dst, const void* src_dev, size_t bytes, cudaStream_t 
   return cudaMemcpyAsync(dst, src_dev, bytes, is_device_ptr(dst) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s);
 }
 
-size_t elem_bytes(const tm_ctx* c) { return c->precision == TM_FP64 ? sizeof(Cx<double>) : sizeof(Cx<float>); }
+// bytes of one element of the context's main vectors / T: fp64 in TM_FP64 and TM_MIXED, fp32 in TM_FP32
+size_t elem_bytes(const tm_ctx* c) { return c->precision == TM_FP32 ? sizeof(Cx<float>) : sizeof(Cx<double>); }
 
 // ---------------------------------------------------------------------------------------- host math
 // Gauss-Legendre nodes/weights on [-1, 1] by Newton iteration on P_n.
@@ -169,6 +172,10 @@ void sph_yn_real(int lmax, double x, std::vector<double>& y) {
 namespace {
 
 template <typename R> Cx<R>* vec(tm_ctx* c, int i) { return reinterpret_cast<Cx<R>*>(c->d_v[i]); }
+// T in precision R: in TM_MIXED the context holds an fp64 copy (d_T) and an fp32 copy (d_T32)
+template <typename R> const Cx<R>* Tptr(const tm_ctx* c) {
+  return reinterpret_cast<const Cx<R>*>((sizeof(R) == 4 && c->precision == TM_MIXED) ? c->d_T32 : c->d_T);
+}
 
 int grid_for(size_t n, int block) { return (int)std::min<size_t>((n + block - 1) / block, 148 * 32); }
 
@@ -259,7 +266,7 @@ cudaError_t launch_tapply(tm_ctx* c, int mode, const Cx<R>* x, Cx<R>* y, const i
   constexpr int JB = 8;
   const int grid = (c->n_scat + JB - 1) / JB;
   k_tapply<R, JB><<<grid, 256, 0, c->stream>>>(mode, c->L, c->n_scat, c->n_part, x, reinterpret_cast<Cx<R>*>(c->d_upart), y,
-                                               reinterpret_cast<Cx<R>*>(c->d_T), c->diag, c->d_type_of, c->d_const, n_active);
+                                               Tptr<R>(c), c->diag, c->d_type_of, c->d_const, n_active);
   c->total_launches++;
   return cudaGetLastError();
 }
@@ -295,21 +302,31 @@ cudaError_t store_c64(tm_ctx* c, const Cx<R>* src, tm_c64* dst) {
 }
 
 // ---------------------------------------------------------------------------------------- GMRES driver
-template <typename R>
+// R  = precision of the Krylov cycles (all-pairs kernel, basis V, work vector W, orthogonalisation),
+// RX = precision of the iterate x, the right-hand side b and the TRUE residual recomputed at every restart.
+// R == RX: plain restarted GMRES.  R = float, RX = double (TM_MIXED): GMRES with iterative refinement - every cycle
+// solves the correction equation M d = r for the fp64 residual r in fp32 and adds d to the fp64 iterate.
+template <typename R, typename RX>
 int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_info* info) {
   // on entry: d_v[1] = right-hand side b; on exit d_v[0] = x.
-  Cx<R>* X = vec<R>(ctx, 0); Cx<R>* B = vec<R>(ctx, 1); Cx<R>* Z = vec<R>(ctx, 2);
+  constexpr bool mixed = !std::is_same<R, RX>::value;
+  Cx<RX>* X = vec<RX>(ctx, 0); Cx<RX>* B = vec<RX>(ctx, 1); Cx<RX>* ZX = vec<RX>(ctx, 2);
   const size_t n = ctx->n;
   const int m = o.restart, nw = ctx->n_win, nc = ctx->n_chunks;
   Cx<R>* V = reinterpret_cast<Cx<R>*>(ctx->ws);
   Cx<R>* W = V + (size_t)(m + 1) * n;
+  // scratch of the transposed operator in the cycle precision, and the vector that receives M x / the true residual
+  Cx<R>* ZV = mixed ? W + n : reinterpret_cast<Cx<R>*>(ZX);
+  Cx<RX>* RXv = mixed ? reinterpret_cast<Cx<RX>*>((reinterpret_cast<uintptr_t>(ZV + n) + 255) & ~(uintptr_t)255)
+                      : reinterpret_cast<Cx<RX>*>(W);
   TmGmresDev& S = ctx->gm.dev;
+  S.inner_floor = mixed ? 1e-5 : 0.0;                 // an fp32 cycle cannot usefully reduce its residual further
   cudaStream_t st = ctx->stream;
   const int wb = (nw + 63) / 64;
   cudaEvent_t e0, e1;
   TM_CUDA(cudaEventCreate(&e0)); TM_CUDA(cudaEventCreate(&e1));
   TM_CUDA(cudaEventRecord(e0, st));
-  TM_CUDA(cudaMemsetAsync(X, 0, n * sizeof(Cx<R>), st));
+  TM_CUDA(cudaMemsetAsync(X, 0, n * sizeof(Cx<RX>), st));
   TM_CUDA(cudaMemsetAsync(V, 0, (size_t)(m + 2) * n * sizeof(Cx<R>), st));   // basis vectors must be finite (k_axpy)
 
   std::vector<int> h_k(nw), h_done(nw), iters(nw, 0), restarts(nw, 0);
@@ -331,10 +348,10 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
     coop = can && (long long)per_sm * n_sm >= nc;
     (void)fn;
   }
-  const Cx<R>* resid_vec = B;                         // first cycle: x0 = 0 so r = b
+  const Cx<RX>* resid_vec = B;                        // first cycle: x0 = 0 so r = b
   while (true) {
     // beta = ||r|| per window
-    k_norm2<R><<<nc, TM_VT, 0, st>>>(resid_vec, ctx->d_chunks, ctx->gm.normpart);
+    k_norm2<RX><<<nc, TM_VT, 0, st>>>(resid_vec, ctx->d_chunks, ctx->gm.normpart);
     k_reduce_norm<<<nw, 64, 0, st>>>(ctx->gm.normpart, ctx->d_win_chunk_ptr, S.normw);
     if (cycle > 0) {
       k_gmres_true_resid<<<wb, 64, 0, st>>>(S, nw);
@@ -361,7 +378,7 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
     }
     TM_CUDA(cudaMemsetAsync(S.n_active, 0, sizeof(int), st));
     k_gmres_init_cycle<<<wb, 64, 0, st>>>(S, nw, cycle == 0 ? 1 : 0, o.tol);
-    k_scale_or_sub<R><<<nc, TM_VT, 0, st>>>(resid_vec, nullptr, S.inv_norm, V, ctx->d_chunks, nullptr);   // V_0 = r / beta
+    k_scale_or_sub<RX, R><<<nc, TM_VT, 0, st>>>(resid_vec, nullptr, S.inv_norm, V, ctx->d_chunks, nullptr);   // V_0 = r / beta
     ctx->total_launches += 4;
     const int mc = std::min(m, o.max_iter - total);
     last_mc = mc;
@@ -369,10 +386,10 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
       Cx<R>* Vj = V + (size_t)j * n;
       const bool fuse_t = coop && ctx->diag;       // T application folded into the cooperative step
       if (fuse_t) {
-        if (transpose == 1 && j == 0) TM_CUDA(launch_tapply<R>(ctx, 4, Vj, Z, S.n_active));   // z = P T^T v_0
-        TM_CUDA(launch_allpairs<R>(ctx, transpose == 1 ? Z : Vj, S.n_active));
+        if (transpose == 1 && j == 0) TM_CUDA(launch_tapply<R>(ctx, 4, Vj, ZV, S.n_active));   // z = P T^T v_0
+        TM_CUDA(launch_allpairs<R>(ctx, transpose == 1 ? ZV : Vj, S.n_active));
       } else {
-        TM_CUDA(apply_operator<R>(ctx, transpose, Vj, W, Z, S.n_active));
+        TM_CUDA(apply_operator<R>(ctx, transpose, Vj, W, ZV, S.n_active));
       }
       matvecs++;
       // split the basis vectors of a dot-product pass over gridDim.y when there are few chunks
@@ -398,7 +415,7 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
         Cx<R>* Wc = W; const TmChunk* chk = ctx->d_chunks; double2* prt = ctx->gm.part; double* npt = ctx->gm.normpart;
         const int* wcp = ctx->d_win_chunk_ptr; TmGmresDev Sc = S;
         TmFuseT<R> ft{fuse_t ? (transpose == 1 ? 2 : 1) : 0, Vj, reinterpret_cast<const Cx<R>*>(ctx->d_upart), ctx->n_part, n,
-                      reinterpret_cast<const Cx<R>*>(ctx->d_T), ctx->d_type_of, ctx->d_const->perm_neg_m, ctx->L, Z};
+                      Tptr<R>(ctx), ctx->d_type_of, ctx->d_const->perm_neg_m, ctx->L, ZV};
         void* args[] = {&Vc, &nn, &jj, &Wc, &chk, &ncc, &prt, &npt, &wcp, &Sc, &nww, &tl, &ft};
         const void* fn = ctx->ept == 1 ? (const void*)k_arnoldi_fused<R, 1> : (const void*)k_arnoldi_fused<R, 4>;
         TM_CUDA(cudaLaunchCooperativeKernel(fn, dim3(nc), dim3(TM_VT), args, std::max(sm_a, sm_g), st));
@@ -417,14 +434,14 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
     }
     // x += V y ; r = b - M x
     k_gmres_solve_y<<<nw, 32, 0, st>>>(S, nw);
-    if (ctx->ept == 1) k_axpy<R, 1><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr, nc, ctx->d_win_chunk_ptr, nullptr);
-    else k_axpy<R, 4><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr, nc, ctx->d_win_chunk_ptr, nullptr);
-    TM_CUDA(apply_operator<R>(ctx, transpose, X, W, Z, nullptr));
+    if (ctx->ept == 1) k_axpy<R, 1, RX><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr, nc, ctx->d_win_chunk_ptr, nullptr);
+    else k_axpy<R, 4, RX><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr, nc, ctx->d_win_chunk_ptr, nullptr);
+    TM_CUDA(apply_operator<RX>(ctx, transpose, X, RXv, ZX, nullptr));                       // in the iterate's precision
     matvecs++;
-    k_scale_or_sub<R><<<nc, TM_VT, 0, st>>>(B, W, nullptr, W, ctx->d_chunks, nullptr);      // W = b - M x
+    k_scale_or_sub<RX, RX><<<nc, TM_VT, 0, st>>>(B, RXv, nullptr, RXv, ctx->d_chunks, nullptr);   // r = b - M x
     ctx->total_launches += 3;
     TM_CUDA(cudaGetLastError());
-    resid_vec = W;
+    resid_vec = RXv;
     cycle++;
   }
   TM_CUDA(cudaEventRecord(e1, st));
@@ -553,7 +570,7 @@ int ensure_gmres(tm_ctx* ctx, int restart) {
   auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) / 256 * 256; return o; };
   const size_t o_h1 = take(nw * ldh * 16), o_h2 = take(nw * ldh * 16), o_R = take(nw * m * ldh * 16), o_cs = take(nw * m * 8),
                o_sn = take(nw * m * 16), o_g = take(nw * ldh * 16), o_y = take(nw * ldh * 16), o_nw = take(nw * 8),
-               o_bn = take(nw * 8), o_in = take(nw * 8), o_rs = take(nw * 8), o_k = take(nw * 4), o_d = take(nw * 4),
+               o_bn = take(nw * 8), o_in = take(nw * 8), o_b0 = take(nw * 8), o_rs = take(nw * 8), o_k = take(nw * 4), o_d = take(nw * 4),
                o_na = take(4), o_part = take(ldh * nc * 16), o_np = take(nc * 8);
   TM_CUDA(cudaMalloc(&ctx->gm.blob, off));
   TM_CUDA(cudaMemset(ctx->gm.blob, 0, off));
@@ -561,15 +578,19 @@ int ensure_gmres(tm_ctx* ctx, int restart) {
   TmGmresDev& S = ctx->gm.dev;
   S.h1 = (double2*)(b + o_h1); S.h2 = (double2*)(b + o_h2); S.Rm = (double2*)(b + o_R); S.cs = (double*)(b + o_cs);
   S.sn = (double2*)(b + o_sn); S.g = (double2*)(b + o_g); S.y = (double2*)(b + o_y); S.normw = (double*)(b + o_nw);
-  S.bnorm = (double*)(b + o_bn); S.inv_norm = (double*)(b + o_in); S.resid = (double*)(b + o_rs); S.kcols = (int*)(b + o_k);
+  S.bnorm = (double*)(b + o_bn); S.inv_norm = (double*)(b + o_in); S.beta0 = (double*)(b + o_b0); S.resid = (double*)(b + o_rs); S.kcols = (int*)(b + o_k);
   S.done = (int*)(b + o_d); S.n_active = (int*)(b + o_na);
-  S.ldh = (int)ldh; S.m = (int)m;
+  S.ldh = (int)ldh; S.m = (int)m; S.inner_floor = 0.0;
   ctx->gm.part = (double2*)(b + o_part); ctx->gm.normpart = (double*)(b + o_np);
   ctx->gm.restart = restart;
   return TM_OK;
 }
 
-size_t ws_bytes_for(const tm_ctx* c, int restart) { return (size_t)(restart + 2) * c->n * elem_bytes(c) + 256; }
+size_t ws_bytes_for(const tm_ctx* c, int restart) {
+  if (c->precision == TM_MIXED)     // fp32 basis + work vector + fp32 scratch, fp64 residual vector
+    return (size_t)(restart + 3) * c->n * sizeof(Cx<float>) + c->n * sizeof(Cx<double>) + 1024;
+  return (size_t)(restart + 2) * c->n * elem_bytes(c) + 256;
+}
 
 int ensure_workspace(tm_ctx* ctx, int restart) {
   const size_t need = ws_bytes_for(ctx, restart);
@@ -601,7 +622,7 @@ const char* tm_last_error(const tm_ctx* ctx) { return ctx ? ctx->err.c_str() : g
 void tm_destroy(tm_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
-  cudaFree(c->d_pos); cudaFree(c->d_win_of); cudaFree(c->d_type_of); cudaFree(c->d_T); cudaFree(c->d_p);
+  cudaFree(c->d_pos); cudaFree(c->d_win_of); cudaFree(c->d_type_of); cudaFree(c->d_T); cudaFree(c->d_T32); cudaFree(c->d_p);
   cudaFree(c->d_const); cudaFree(c->d_rowptr); cudaFree(c->d_col); cudaFree(c->d_widx); cudaFree(c->d_imag);
   cudaFree(c->d_coef); cudaFree(c->d_tiles); cudaFree(c->d_upart); cudaFree(c->d_chunks); cudaFree(c->d_win_chunk_ptr);
   for (int i = 0; i < 3; ++i) cudaFree(c->d_v[i]);
@@ -620,7 +641,8 @@ int tm_create(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const 
   if (n_scat < 1 || !pos_xyz) return fail(ctx, TM_E_INVALID, "need n_scat >= 1 and positions");
   if (lmax < 1 || lmax > tm_max_table_lmax) return fail(ctx, TM_E_INVALID, "lmax must be in 1..6");
   if (!(k_b > 0.0) || !std::isfinite(k_b)) return fail(ctx, TM_E_INVALID, "k_b must be positive and finite");
-  if (precision != TM_FP64 && precision != TM_FP32) return fail(ctx, TM_E_INVALID, "precision must be TM_FP64 or TM_FP32");
+  if (precision != TM_FP64 && precision != TM_FP32 && precision != TM_MIXED)
+    return fail(ctx, TM_E_INVALID, "precision must be TM_FP64, TM_FP32 or TM_MIXED");
   if (n_win < 1) return fail(ctx, TM_E_INVALID, "n_win must be >= 1");
   std::vector<int> wp;
   if (win_ptr) {
@@ -795,14 +817,14 @@ int tm_kernel_time(tm_ctx* ctx, int reset, double* allpairs_ms, long long* allpa
 namespace {
 
 template <typename R>
-int set_T_typed(tm_ctx* ctx, size_t count, const tm_c64* T) {
+int set_T_typed(tm_ctx* ctx, size_t count, const tm_c64* T, void* dst) {
   // stage fp64 -> Cx<R>
   double2* tmp = nullptr;
   TM_CUDA(cudaMalloc(&tmp, count * sizeof(double2)));
   cudaError_t e = copy_in(tmp, T, count * sizeof(double2), ctx->stream);
   if (e == cudaSuccess) {
     k_from_c64<R><<<grid_for(count, 256), 256, 0, ctx->stream>>>(reinterpret_cast<const double*>(tmp),
-                                                                 reinterpret_cast<Cx<R>*>(ctx->d_T), count);
+                                                                 reinterpret_cast<Cx<R>*>(dst), count);
     e = cudaGetLastError();
   }
   if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
@@ -820,7 +842,7 @@ int matvec_typed(tm_ctx* ctx, int transpose, const tm_c64* x, tm_c64* y) {
   return TM_OK;
 }
 
-template <typename R>
+template <typename RV, typename R>
 int solve_typed(tm_ctx* ctx, int adjoint, const tm_c64* w, const tm_solve_opts& o, tm_c64* out, tm_solve_info* info) {
   if (adjoint) {
     TM_CUDA(load_c64<R>(ctx, w, vec<R>(ctx, 1)));                           // b = w
@@ -830,7 +852,7 @@ int solve_typed(tm_ctx* ctx, int adjoint, const tm_c64* w, const tm_solve_opts& 
     TM_CUDA(launch_tapply<R>(ctx, 3, vec<R>(ctx, 2), vec<R>(ctx, 1), nullptr));   // b = T p   (Eq. I25)
     ctx->total_launches++;
   }
-  const int rc = gmres_solve<R>(ctx, adjoint ? 1 : 0, o, info);
+  const int rc = gmres_solve<RV, R>(ctx, adjoint ? 1 : 0, o, info);
   if (rc < 0) return rc;
   TM_CUDA(store_c64<R>(ctx, vec<R>(ctx, 0), out));
   TM_CUDA(cudaStreamSynchronize(ctx->stream));
@@ -873,7 +895,13 @@ int tm_set_tmatrices(tm_ctx* ctx, int n_types, int diag_only, const tm_c64* T, c
   TM_CUDA(cudaMalloc(&newT, count * elem_bytes(ctx)));
   void* oldT = ctx->d_T;
   ctx->d_T = newT;
-  const int rc = ctx->precision == TM_FP64 ? set_T_typed<double>(ctx, count, T) : set_T_typed<float>(ctx, count, T);
+  int rc = ctx->precision != TM_FP32 ? set_T_typed<double>(ctx, count, T, newT) : set_T_typed<float>(ctx, count, T, newT);
+  if (rc == TM_OK && ctx->precision == TM_MIXED) {            // fp32 copy for the inner Krylov cycles
+    void* new32 = nullptr;
+    if (cudaMalloc(&new32, count * sizeof(Cx<float>)) != cudaSuccess) rc = fail(ctx, TM_E_NOMEM, "cudaMalloc(T fp32)");
+    else if ((rc = set_T_typed<float>(ctx, count, T, new32)) == TM_OK) { cudaFree(ctx->d_T32); ctx->d_T32 = new32; }
+    else cudaFree(new32);
+  }
   if (rc != TM_OK) { cudaFree(newT); ctx->d_T = oldT; return rc; }
   cudaFree(oldT);
   TM_CUDA(cudaMemcpy(ctx->d_type_of, ht.data(), ht.size() * sizeof(int), cudaMemcpyHostToDevice));
@@ -1016,7 +1044,7 @@ int tm_matvec(tm_ctx* ctx, int transpose, const tm_c64* x, tm_c64* y) {
   if (!ctx) return TM_E_INVALID;
   if (!x || !y || transpose < 0 || transpose > 2) return fail(ctx, TM_E_INVALID, "bad arguments");
   if (transpose != 2 && !ctx->has_T) return fail(ctx, TM_E_STATE, "tm_set_tmatrices has not been called");
-  return ctx->precision == TM_FP64 ? matvec_typed<double>(ctx, transpose, x, y) : matvec_typed<float>(ctx, transpose, x, y);
+  return ctx->precision != TM_FP32 ? matvec_typed<double>(ctx, transpose, x, y) : matvec_typed<float>(ctx, transpose, x, y);
 }
 
 int tm_solve(tm_ctx* ctx, const tm_solve_opts* opts, tm_c64* s_out, tm_solve_info* info) {
@@ -1027,8 +1055,9 @@ int tm_solve(tm_ctx* ctx, const tm_solve_opts* opts, tm_c64* s_out, tm_solve_inf
   if (!ctx->has_T || !ctx->has_inc) return fail(ctx, TM_E_STATE, "tm_set_tmatrices and tm_set_incident must be called first");
   if ((rc = ensure_workspace(ctx, opts->restart)) != TM_OK) return rc;
   if ((rc = ensure_gmres(ctx, opts->restart)) != TM_OK) return rc;
-  return ctx->precision == TM_FP64 ? solve_typed<double>(ctx, 0, nullptr, *opts, s_out, info)
-                                   : solve_typed<float>(ctx, 0, nullptr, *opts, s_out, info);
+  if (ctx->precision == TM_MIXED) return solve_typed<float, double>(ctx, 0, nullptr, *opts, s_out, info);
+  return ctx->precision == TM_FP64 ? solve_typed<double, double>(ctx, 0, nullptr, *opts, s_out, info)
+                                   : solve_typed<float, float>(ctx, 0, nullptr, *opts, s_out, info);
 }
 
 int tm_solve_adjoint(tm_ctx* ctx, const tm_c64* w, const tm_solve_opts* opts, tm_c64* lambda_out, tm_solve_info* info) {
@@ -1039,8 +1068,9 @@ int tm_solve_adjoint(tm_ctx* ctx, const tm_c64* w, const tm_solve_opts* opts, tm
   if (!ctx->has_T) return fail(ctx, TM_E_STATE, "tm_set_tmatrices must be called first");
   if ((rc = ensure_workspace(ctx, opts->restart)) != TM_OK) return rc;
   if ((rc = ensure_gmres(ctx, opts->restart)) != TM_OK) return rc;
-  return ctx->precision == TM_FP64 ? solve_typed<double>(ctx, 1, w, *opts, lambda_out, info)
-                                   : solve_typed<float>(ctx, 1, w, *opts, lambda_out, info);
+  if (ctx->precision == TM_MIXED) return solve_typed<float, double>(ctx, 1, w, *opts, lambda_out, info);
+  return ctx->precision == TM_FP64 ? solve_typed<double, double>(ctx, 1, w, *opts, lambda_out, info)
+                                   : solve_typed<float, float>(ctx, 1, w, *opts, lambda_out, info);
 }
 
 int tm_fields(tm_ctx* ctx, int n_pts, const double* pts, const tm_c64* s, int which, tm_c64* out) {
@@ -1090,7 +1120,7 @@ int tm_grad_tmatrix(tm_ctx* ctx, const tm_c64* dT, const tm_c64* lambda, const t
   if (e == cudaSuccess) e = cudaMalloc(&d_tmp, count * sizeof(double2));
   if (e == cudaSuccess) e = cudaMalloc(&d_out, (size_t)ctx->n_scat * sizeof(double2));
   if (e == cudaSuccess) e = copy_in(d_tmp, dT, count * sizeof(double2), ctx->stream);
-  const bool f64 = ctx->precision == TM_FP64;
+  const bool f64 = ctx->precision != TM_FP32;
   if (e == cudaSuccess) {
     if (f64) k_from_c64<double><<<grid_for(count, 256), 256, 0, ctx->stream>>>(reinterpret_cast<const double*>(d_tmp), reinterpret_cast<Cx<double>*>(d_dT), count);
     else k_from_c64<float><<<grid_for(count, 256), 256, 0, ctx->stream>>>(reinterpret_cast<const double*>(d_tmp), reinterpret_cast<Cx<float>*>(d_dT), count);
@@ -1184,7 +1214,7 @@ int tm_grad_positions(tm_ctx* ctx, const tm_c64* lambda, const tm_c64* s, const 
   ctx->kernel_req = TM_KERNEL_SYM3D;                      // displaced targets are not coplanar with the sources (alpha = z)
   int rc = configure_kernel(ctx);
   if (rc == TM_OK)
-    rc = ctx->precision == TM_FP64 ? grad_positions_typed<double>(ctx, lambda, s, dp, h, out)
+    rc = ctx->precision != TM_FP32 ? grad_positions_typed<double>(ctx, lambda, s, dp, h, out)
                                    : grad_positions_typed<float>(ctx, lambda, s, dp, h, out);
   ctx->kernel_req = saved;
   const int rc2 = configure_kernel(ctx);

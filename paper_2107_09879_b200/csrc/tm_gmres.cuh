@@ -16,12 +16,14 @@ struct TmGmresDev {
   double*  normw;     // [n_win]        sqrt(sum |w|^2) of the current vector
   double*  bnorm;     // [n_win]
   double*  inv_norm;  // [n_win]
+  double*  beta0;     // [n_win]        ||r|| at the start of the cycle
   double*  resid;     // [n_win]        current estimate / true relative residual
   int*     kcols;     // [n_win]        Krylov columns accepted in this cycle
   int*     done;      // [n_win]
   int*     n_active;  // [1]            windows still iterating in this cycle
   int ldh;            // restart + 1
   int m;              // restart
+  double inner_floor; // mixed precision: a cycle also ends once the estimate has dropped by this factor (0: off)
 };
 
 __device__ __forceinline__ double2 d2mul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
@@ -32,6 +34,7 @@ __global__ void k_gmres_init_cycle(TmGmresDev S, int n_win, int first, double to
   const int w = blockIdx.x * blockDim.x + threadIdx.x;
   if (w >= n_win) return;
   const double beta = S.normw[w];
+  S.beta0[w] = beta;
   if (first) S.bnorm[w] = beta;
   const double bn = S.bnorm[w];
   S.kcols[w] = 0;
@@ -99,7 +102,7 @@ __device__ __forceinline__ void givens_body(const TmGmresDev& S, int w, int j, d
   S.kcols[w] = j + 1;
   const double bn = S.bnorm[w];
   S.resid[w] = est / bn;
-  const bool fin = !(est > tol * bn) || !(hn > 0.0);
+  const bool fin = !(est > fmax(tol * bn, S.inner_floor * S.beta0[w])) || !(hn > 0.0);
   if (fin) { S.done[w] = 1; S.inv_norm[w] = 0.0; atomicSub(S.n_active, 1); }
   else S.inv_norm[w] = 1.0 / hn;
 }

@@ -156,9 +156,10 @@ __global__ void k_reduce_h(const double2* __restrict__ part, int n_chunks, const
 // deterministic); the block owning the window's first chunk then also stores them to coef for the Givens kernel.
 // Basis vectors must hold finite numbers (the workspace is zeroed at the start of a solve): a zero coefficient
 // multiplies whatever is there.
-template <typename R, int EPT>
+// (R: precision of the basis vectors, RW: precision of the updated vector - they differ in mixed-precision solves)
+template <typename R, int EPT, typename RW = R>
 __device__ __forceinline__ void axpy_body(const Cx<R>* __restrict__ V, size_t stride, int nvec, double2* __restrict__ coef, int ldc,
-                                          double sign, Cx<R>* __restrict__ w, const TmChunk ch, int cidx,
+                                          double sign, Cx<RW>* __restrict__ w, const TmChunk ch, int cidx,
                                           double* __restrict__ normpart, const double2* __restrict__ part, int n_chunks,
                                           const int* __restrict__ win_chunk_ptr, double2* s_c, double* s_n) {
   if (part != nullptr) {
@@ -202,7 +203,7 @@ __device__ __forceinline__ void axpy_body(const Cx<R>* __restrict__ V, size_t st
         ar += c.x * (double)v.re - c.y * (double)v.im;
         ai += c.x * (double)v.im + c.y * (double)v.re;
       }
-      w[g] = cx<R>((R)ar, (R)ai);
+      w[g] = cx<RW>((RW)ar, (RW)ai);
       nrm += ar * ar + ai * ai;
     }
   }
@@ -219,17 +220,17 @@ __device__ __forceinline__ void axpy_body(const Cx<R>* __restrict__ V, size_t st
   }
 }
 
-template <typename R, int EPT>
+template <typename R, int EPT, typename RW = R>
 __global__ void __launch_bounds__(TM_VT)
 k_axpy(const Cx<R>* __restrict__ V, size_t stride, int nvec, double2* __restrict__ coef, int ldc, double sign,
-       Cx<R>* __restrict__ w, const TmChunk* __restrict__ chunks, double* __restrict__ normpart,
+       Cx<RW>* __restrict__ w, const TmChunk* __restrict__ chunks, double* __restrict__ normpart,
        const double2* __restrict__ part, int n_chunks, const int* __restrict__ win_chunk_ptr,
        const int* __restrict__ n_active) {
   if (n_active != nullptr && *n_active == 0) return;
   extern __shared__ double2 s_c[];                   // [nvec]
   __shared__ double s_n[TM_VT / 32];
-  axpy_body<R, EPT>(V, stride, nvec, coef, ldc, sign, w, chunks[blockIdx.x], blockIdx.x, normpart, part, n_chunks,
-                    win_chunk_ptr, s_c, s_n);
+  axpy_body<R, EPT, RW>(V, stride, nvec, coef, ldc, sign, w, chunks[blockIdx.x], blockIdx.x, normpart, part, n_chunks,
+                        win_chunk_ptr, s_c, s_n);
 }
 
 // normpart[c] = sum |v|^2 over chunk c
@@ -267,18 +268,19 @@ __global__ void k_reduce_norm(const double* __restrict__ normpart, const int* __
   if (threadIdx.x == 0) out[w] = sqrt(sh[0] + sh[1]);
 }
 
-// dst = a * scale[win]  (V_{j+1} = w / h_{j+1,j});  dst = a - b when b != nullptr (scale ignored)
-template <typename R>
+// dst = a * scale[win]  (V_{j+1} = w / h_{j+1,j});  dst = a - b when b != nullptr (scale ignored).
+// R: precision of a and b, RD: precision of dst (mixed-precision solves normalise an fp64 residual into an fp32 basis).
+template <typename R, typename RD = R>
 __global__ void __launch_bounds__(TM_VT)
 k_scale_or_sub(const Cx<R>* __restrict__ a, const Cx<R>* __restrict__ b, const double* __restrict__ scale,
-               Cx<R>* __restrict__ dst, const TmChunk* __restrict__ chunks, const int* __restrict__ n_active) {
+               Cx<RD>* __restrict__ dst, const TmChunk* __restrict__ chunks, const int* __restrict__ n_active) {
   if (n_active != nullptr && *n_active == 0) return;
   const TmChunk ch = chunks[blockIdx.x];
   const double sc = (b == nullptr) ? scale[ch.win] : 1.0;
   for (int e = threadIdx.x; e < ch.count; e += TM_VT) {
     const size_t g = (size_t)ch.start + e;
-    if (b == nullptr) dst[g] = cx<R>((R)(sc * (double)a[g].re), (R)(sc * (double)a[g].im));
-    else dst[g] = csub(a[g], b[g]);
+    if (b == nullptr) dst[g] = cx<RD>((RD)(sc * (double)a[g].re), (RD)(sc * (double)a[g].im));
+    else dst[g] = cx<RD>((RD)((double)a[g].re - (double)b[g].re), (RD)((double)a[g].im - (double)b[g].im));
   }
 }
 

@@ -232,3 +232,29 @@ def test_incident_and_fields_at_high_lmax(tm, lmax):
     assert rel(s.fields(pts, coef, tm.TM_FIELD_E_SCA), fields.e_sca(lmax, W.K_B, pos, coef, pts)) <= 1e-12
     assert rel(s.fields(pts, coef, tm.TM_FIELD_H_SCA), fields.zh_sca(lmax, W.K_B, pos, coef, pts)) <= 1e-12
     s.close()
+
+
+def test_mixed_precision_iterative_refinement(tm):
+    """TM_MIXED: fp32 Krylov cycles, fp64 iterate / right-hand side / true residual: fp64-level parity with the oracle.
+    Covers the cooperative path (small), diagonal and full T, windows, forward and adjoint."""
+    w = W.config(2, scale=12)
+    ref = driver.solve(w)
+    s = tm.solver_for_workload(w, precision=tm.TM_MIXED)
+    sol, info, rc = s.solve(1e-10, 50, 5000)
+    assert rc == 0 and info[0].rel_residual <= 1e-10 and rel(sol, ref["s"]) <= 1e-9
+    x = rand_x(sol.shape, 5)                              # everything outside the solves runs in fp64
+    assert rel(s.matvec(x, 0).reshape(-1), ref["M"] @ x.reshape(-1)) <= 1e-12
+    s.close()
+    w = W.config(4, scale=6)
+    ref = driver.solve(w, adjoint_w=w["w_adj"])
+    s = tm.solver_for_workload(w, precision=tm.TM_MIXED)
+    sol, info, rc = s.solve(1e-11, 50, 5000)
+    lam, info2, rc2 = s.solve_adjoint(w["w_adj"], 1e-11, 50, 5000)
+    assert rc == 0 and rc2 == 0 and rel(sol, ref["s"]) <= 1e-9 and rel(lam, ref["lam"]) <= 1e-9
+    s.close()
+    w = W.config("3b", scale=8)
+    ref = driver.solve(w)
+    s = tm.solver_for_workload(w, precision=tm.TM_MIXED)
+    sol, info, rc = s.solve(1e-11, 50, 5000)
+    assert rc == 0 and rel(sol, ref["s"]) <= 1e-9
+    s.close()
