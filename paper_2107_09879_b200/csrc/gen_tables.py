@@ -685,12 +685,101 @@ def emit_coplanar4(lmaxes, path):
             f.write(f"#define TM_COP4_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")
 
 
+# ----------------------------------------------------------------------------- coplanar, fp32 packed (FFMA2)
+def emit_coplanar_f2(lmaxes, path):
+    """fp32 build of the coplanar pair code on Blackwell's packed FP32 instructions (FFMA2 / FMUL2: two FMAs per issue
+    slot, immediate and register operands broadcast, LO_HI swap and per-half negation are operand modifiers).  A complex
+    number is one float2; real x complex = 1 FFMA2, complex x complex = 2 FFMA2.  Same mathematics as emit_coplanar."""
+    f2 = lambda a, b: f"make_float2({a}, {b})"
+    with open(path, "w") as f:
+        f.write("// GENERATED by gen_tables.py - do not edit.\n")
+        f.write("// fp32 coplanar pair code with packed FFMA2 arithmetic (one float2 per complex number); see tm_coplanar_gen.cuh.\n")
+        f.write("// xs: d-values of this half; a: accumulators A^0 / A^+- of this half.\n#pragma once\n\n")
+        f.write("__device__ __forceinline__ float2 tm_swap2(float2 v) { return make_float2(v.y, v.x); }\n\n")
+        for lmax in lmaxes:
+            md = modes(lmax)
+            idx = {t: i for i, t in enumerate(md)}
+            sym = coplanar_sym(lmax)
+            half_l = len(md) // 2
+            for h in (0, 1):
+                slots, Knew = sym[h]
+                n = len(slots)
+                nq = 2 * lmax + 1
+                f.write("__device__ __forceinline__ void "
+                        f"tm_cop_pair_f2_L{lmax}_H{h}(const float2* __restrict__ xs, const float* cm, const float* sm, const float* hr, const float* hi, float2* a) {{\n")
+                k = 0
+                while k < n:
+                    l, am, p, kind = slots[k]
+                    if kind == "0":
+                        f.write(f"  const float2 x{k} = xs[{k}];\n")
+                        k += 1
+                    else:      # x^+ = c d^+ + i s d^- ,  x^- = c d^- + i s d^+   (i s d = s (-d.y, d.x))
+                        kp, km = k, k + 1
+                        f.write(f"  const float2 x{kp} = __ffma2_rn({f2(f'-sm[{am}]', f'sm[{am}]')}, tm_swap2(xs[{km}]), __fmul2_rn({f2(f'cm[{am}]', f'cm[{am}]')}, xs[{kp}]));\n")
+                        f.write(f"  const float2 x{km} = __ffma2_rn({f2(f'-sm[{am}]', f'sm[{am}]')}, tm_swap2(xs[{kp}]), __fmul2_rn({f2(f'cm[{am}]', f'cm[{am}]')}, xs[{km}]));\n")
+                        k += 2
+
+                def row_code(r):
+                    f.write(f"    float2 u{r} = make_float2(0.f, 0.f);\n")
+                    for q in range(nq):
+                        terms = Knew[q][r]
+                        if not terms:
+                            continue
+                        for t, (c, v) in enumerate(terms):
+                            kk = lit(v) + "f"
+                            if t == 0:
+                                f.write(f"    y = __fmul2_rn({f2(kk, kk)}, x{c});\n")
+                            else:
+                                f.write(f"    y = __ffma2_rn({f2(kk, kk)}, x{c}, y);\n")
+                        # u += h_q y :  (hr yr - hi yi, hr yi + hi yr)
+                        f.write(f"    u{r} = __ffma2_rn({f2(f'hr[{q}]', f'hr[{q}]')}, y, u{r}); u{r} = __ffma2_rn({f2(f'-hi[{q}]', f'hi[{q}]')}, tm_swap2(y), u{r});\n")
+
+                k = 0
+                while k < n:
+                    l, am, p, kind = slots[k]
+                    f.write("  {\n    float2 y;\n")
+                    if kind == "0":
+                        row_code(k)
+                        f.write(f"    a[{k}] = __fadd2_rn(a[{k}], u{k});\n")
+                        k += 1
+                    else:      # A^+ += c u^+ - i s u^- ;  A^- += c u^- - i s u^+    (-i s u = s (u.y, -u.x))
+                        kp, km = k, k + 1
+                        row_code(kp)
+                        row_code(km)
+                        f.write(f"    a[{kp}] = __ffma2_rn({f2(f'cm[{am}]', f'cm[{am}]')}, u{kp}, a[{kp}]); a[{kp}] = __ffma2_rn({f2(f'sm[{am}]', f'-sm[{am}]')}, tm_swap2(u{km}), a[{kp}]);\n")
+                        f.write(f"    a[{km}] = __ffma2_rn({f2(f'cm[{am}]', f'cm[{am}]')}, u{km}, a[{km}]); a[{km}] = __ffma2_rn({f2(f'sm[{am}]', f'-sm[{am}]')}, tm_swap2(u{kp}), a[{km}]);\n")
+                        k += 2
+                    f.write("  }\n")
+                f.write("}\n")
+                f.write("template <typename C>\n__device__ __forceinline__ void "
+                        f"tm_cop_unmix_f2_L{lmax}_H{h}(const float2* a, C* out) {{\n")
+                k = 0
+                while k < n:
+                    l, am, p, kind = slots[k]
+
+                    def store(i_flat, re, im):
+                        if i_flat >= half_l:      # p = 1: multiply by -i
+                            f.write(f"  out[{i_flat}].re = {im}; out[{i_flat}].im = -({re});\n")
+                        else:
+                            f.write(f"  out[{i_flat}].re = {re}; out[{i_flat}].im = {im};\n")
+                    if kind == "0":
+                        store(idx[(l, 0, p)], f"a[{k}].x", f"a[{k}].y")
+                        k += 1
+                    else:
+                        kp, km = k, k + 1
+                        store(idx[(l, am, p)], f"0.5f * (a[{kp}].x + a[{km}].x)", f"0.5f * (a[{kp}].y + a[{km}].y)")
+                        store(idx[(l, -am, p)], f"0.5f * (a[{kp}].x - a[{km}].x)", f"0.5f * (a[{kp}].y - a[{km}].y)")
+                        k += 2
+                f.write("}\n\n")
+
+
 def main():
     os.makedirs(OUT, exist_ok=True)
     emit_tables([1, 2, 3, 4, 5, 6], os.path.join(OUT, "tm_tables_gen.h"))
     emit_coplanar([1, 2, 3], os.path.join(OUT, "tm_coplanar_gen.cuh"))
     emit_general_sym([1, 2, 3], os.path.join(OUT, "tm_general3d_gen.cuh"))
     emit_coplanar4([4, 5, 6], os.path.join(OUT, "tm_coplanar4_gen.cuh"))
+    emit_coplanar_f2([1, 2, 3], os.path.join(OUT, "tm_coplanar_f2_gen.cuh"))
 
 
 if __name__ == "__main__":

@@ -11,6 +11,7 @@
 #pragma once
 #include "tm_common.cuh"
 #include "generated/tm_coplanar_gen.cuh"
+#include "generated/tm_coplanar_f2_gen.cuh"
 
 // ---------------------------------------------------------------------------------------------------
 // h_q^(1)(x), q = 0..NQ-1, by upward recurrence from h_{-1} = e^{ix}/x, h_0 = -i e^{ix}/x  (stable upward for
@@ -44,15 +45,46 @@ template <> __device__ __forceinline__ void phase_kr<float>(double k_over_pi, do
 // excluded by index instead.
 struct TmShift { double x, y, z; int on; };
 
+// Accumulators of one parity half: two real arrays in fp64; one float2 per complex number in fp32, where the generated
+// code uses Blackwell's packed FFMA2 arithmetic (generated/tm_coplanar_f2_gen.cuh) to halve the FP issue slots.
+template <typename R, int NH> struct CopAcc {
+  R ar[NH], ai[NH];
+  __device__ __forceinline__ void clear() {
+#pragma unroll
+    for (int b = 0; b < NH; ++b) { ar[b] = R(0); ai[b] = R(0); }
+  }
+};
+template <int NH> struct CopAcc<float, NH> {
+  float2 a[NH];
+  __device__ __forceinline__ void clear() {
+#pragma unroll
+    for (int b = 0; b < NH; ++b) a[b] = make_float2(0.f, 0.f);
+  }
+};
+
 template <typename R, int LMAX, int H> struct CopPair;
 #define TM_COP_SPEC(LM, HH)                                                                              \
-  template <typename R> struct CopPair<R, LM, HH> {                                                      \
-    static __device__ __forceinline__ void run(const R* xs, const R* cm, const R* sm, const R* hr,       \
-                                               const R* hi, R* ar, R* ai) {                              \
-      tm_cop_pair_L##LM##_H##HH<R>(xs, cm, sm, hr, hi, ar, ai);                                          \
+  template <> struct CopPair<double, LM, HH> {                                                           \
+    static constexpr int NH = TM_COP_NH_L##LM;                                                           \
+    static __device__ __forceinline__ void run(const double* xs, const double* cm, const double* sm,     \
+                                               const double* hr, const double* hi, CopAcc<double, NH>& A) { \
+      tm_cop_pair_L##LM##_H##HH<double>(xs, cm, sm, hr, hi, A.ar, A.ai);                                 \
     }                                                                                                    \
-    static __device__ __forceinline__ void unmix(const R* ar, const R* ai, Cx<R>* out) {                 \
-      tm_cop_unmix_L##LM##_H##HH<R, Cx<R>>(ar, ai, out);                                                 \
+    static __device__ __forceinline__ void unmix(const CopAcc<double, NH>& A, Cx<double>* out) {         \
+      tm_cop_unmix_L##LM##_H##HH<double, Cx<double>>(A.ar, A.ai, out);                                   \
+    }                                                                                                    \
+    static __device__ __forceinline__ void stage_entry(int k, int& a, int& b, int& sg) {                 \
+      a = tm_cop_sa_L##LM##_H##HH[k]; b = tm_cop_sb_L##LM##_H##HH[k]; sg = tm_cop_ss_L##LM##_H##HH[k];   \
+    }                                                                                                    \
+  };                                                                                                     \
+  template <> struct CopPair<float, LM, HH> {                                                            \
+    static constexpr int NH = TM_COP_NH_L##LM;                                                           \
+    static __device__ __forceinline__ void run(const float* xs, const float* cm, const float* sm,        \
+                                               const float* hr, const float* hi, CopAcc<float, NH>& A) { \
+      tm_cop_pair_f2_L##LM##_H##HH(reinterpret_cast<const float2*>(xs), cm, sm, hr, hi, A.a);            \
+    }                                                                                                    \
+    static __device__ __forceinline__ void unmix(const CopAcc<float, NH>& A, Cx<float>* out) {           \
+      tm_cop_unmix_f2_L##LM##_H##HH<Cx<float>>(A.a, out);                                                \
     }                                                                                                    \
     static __device__ __forceinline__ void stage_entry(int k, int& a, int& b, int& sg) {                 \
       a = tm_cop_sa_L##LM##_H##HH[k]; b = tm_cop_sb_L##LM##_H##HH[k]; sg = tm_cop_ss_L##LM##_H##HH[k];   \
@@ -101,9 +133,8 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
     s_sa[tid] = a; s_sb[tid] = b; s_ss[tid] = sg;
   }
 
-  R ar[NH], ai[NH];
-#pragma unroll
-  for (int b = 0; b < NH; ++b) { ar[b] = R(0); ai[b] = R(0); }
+  CopAcc<R, NH> acc;
+  acc.clear();
 
   for (int s0 = c0; s0 < c1; s0 += SS) {
     const int ns = min(SS, c1 - s0);
@@ -143,8 +174,8 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
       R hr[NQ], hi[NQ];
       hankel_up<R, NQ>((R)(rinv * inv_k), ck, sk, hr, hi);
       const R* xs = &s_x[s * NH * 2];
-      if (half == 0) CopPair<R, LMAX, 0>::run(xs, cm, sm, hr, hi, ar, ai);
-      else           CopPair<R, LMAX, 1>::run(xs, cm, sm, hr, hi, ar, ai);
+      if (half == 0) CopPair<R, LMAX, 0>::run(xs, cm, sm, hr, hi, acc);
+      else           CopPair<R, LMAX, 1>::run(xs, cm, sm, hr, hi, acc);
     }
   }
 
@@ -152,8 +183,8 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
   // u~_{l,+-m,p} = (A^+ +- A^-)/2,  u_b = (-i)^{p_b} u~_b
   if (live) {
     Cx<R>* out = u_part + ((size_t)blockIdx.y * n_scat + j) * L;
-    if (half == 0) CopPair<R, LMAX, 0>::unmix(ar, ai, out);
-    else           CopPair<R, LMAX, 1>::unmix(ar, ai, out);
+    if (half == 0) CopPair<R, LMAX, 0>::unmix(acc, out);
+    else           CopPair<R, LMAX, 1>::unmix(acc, out);
   }
 }
 
