@@ -63,6 +63,8 @@ class ClockSampler:
         self.rows, self.proc, self.index, self.interval_ms = [], None, index, interval_ms
 
     def start(self):
+        if self.interval_ms <= 0:
+            return
         q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
         try:
@@ -70,6 +72,11 @@ class ClockSampler:
                                           "-lms", str(self.interval_ms)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
+            # nvidia-smi's start-up (NVML initialisation) briefly stalls kernel launches: let it finish before the warm-up,
+            # so that the hiccup cannot land in the timed region (seen as a 2-3x outlier in the first timed step)
+            t0 = time.perf_counter()
+            while not self.rows and time.perf_counter() - t0 < 10.0:
+                time.sleep(0.05)
         except OSError:
             self.proc = None
 
@@ -228,6 +235,9 @@ def run_ours(args, w, rank, world, local_rank):
         def timed(fn, n_warm, n_steps):
             ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_steps)]
             res = None
+            import gc
+            gc.collect()
+            gc.disable()                                    # no collector pauses between the ~2000 launches of a step
             for it in range(n_warm + n_steps):
                 flush.fill_(it & 0xff)                      # L2 flush between iterations (outside the timed bracket)
                 if it == n_warm:
@@ -241,6 +251,7 @@ def run_ours(args, w, rank, world, local_rank):
                 if it >= n_warm:
                     ev[it - n_warm][1].record(st)
             torch.cuda.synchronize()
+            gc.enable()
             if dist is not None:
                 dist.barrier()
             return [a.elapsed_time(b) for a, b in ev], res

@@ -83,6 +83,8 @@ struct tm_ctx {
   size_t ev_used = 0;
   long long allpairs_launches = 0, total_launches = 0;
 
+  cudaEvent_t sync_ev = nullptr; // blocking-sync event: the host thread sleeps instead of spinning while the GPU works
+
   std::string err;
 };
 
@@ -115,6 +117,18 @@ cudaError_t copy_out(void* dst, const void* src_dev, size_t bytes, cudaStream_t 
 }
 
 // bytes of one element of the context's main vectors / T: fp64 in TM_FP64 and TM_MIXED, fp32 in TM_FP32
+// Wait for the context's stream without spinning (a spinning host thread burns the container's CPU quota during
+// multi-second solves; seen as occasional 2-3x outlier steps on shared hosts).
+cudaError_t stream_wait(tm_ctx* c) {
+  if (c->sync_ev == nullptr) {
+    cudaError_t e = cudaEventCreateWithFlags(&c->sync_ev, cudaEventBlockingSync | cudaEventDisableTiming);
+    if (e != cudaSuccess) { c->sync_ev = nullptr; return cudaStreamSynchronize(c->stream); }
+  }
+  cudaError_t e = cudaEventRecord(c->sync_ev, c->stream);
+  if (e != cudaSuccess) return e;
+  return cudaEventSynchronize(c->sync_ev);
+}
+
 size_t elem_bytes(const tm_ctx* c) { return c->precision == TM_FP32 ? sizeof(Cx<float>) : sizeof(Cx<double>); }
 
 // ---------------------------------------------------------------------------------------- host math
@@ -357,7 +371,7 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
       k_gmres_true_resid<<<wb, 64, 0, st>>>(S, nw);
       TM_CUDA(cudaMemcpyAsync(h_res.data(), S.resid, nw * sizeof(double), cudaMemcpyDeviceToHost, st));
       TM_CUDA(cudaMemcpyAsync(h_k.data(), S.kcols, nw * sizeof(int), cudaMemcpyDeviceToHost, st));
-      TM_CUDA(cudaStreamSynchronize(st));
+      TM_CUDA(stream_wait(ctx));
       int kmax = 0;
       all_ok = true;
       for (int w = 0; w < nw; ++w) {
@@ -630,6 +644,7 @@ void tm_destroy(tm_ctx* c) {
   if (c->ws_owned) cudaFree(c->ws);
   cudaFree(c->gm.blob);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  if (c->sync_ev) cudaEventDestroy(c->sync_ev);
   delete c;
 }
 
@@ -764,7 +779,7 @@ int tm_set_kernel(tm_ctx* ctx, int kernel) {
   if (kernel < TM_KERNEL_AUTO || kernel > TM_KERNEL_SYM3D) return fail(ctx, TM_E_INVALID, "unknown kernel id");
   const int old = ctx->kernel_req;
   ctx->kernel_req = kernel;
-  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  TM_CUDA(stream_wait(ctx));
   const int rc = configure_kernel(ctx);
   if (rc != TM_OK) { ctx->kernel_req = old; configure_kernel(ctx); }
   return rc;
@@ -781,7 +796,7 @@ int tm_set_workspace(tm_ctx* ctx, void* dev_ptr, size_t bytes) {
   if (!ctx) return TM_E_INVALID;
   if (dev_ptr && (!is_device_ptr(dev_ptr) || (reinterpret_cast<uintptr_t>(dev_ptr) & 255)))
     return fail(ctx, TM_E_INVALID, "workspace must be 256-byte aligned device memory");
-  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  TM_CUDA(stream_wait(ctx));
   if (ctx->ws && ctx->ws_owned) cudaFree(ctx->ws);
   ctx->ws = dev_ptr; ctx->ws_bytes = dev_ptr ? bytes : 0; ctx->ws_owned = false;
   return TM_OK;
@@ -789,7 +804,7 @@ int tm_set_workspace(tm_ctx* ctx, void* dev_ptr, size_t bytes) {
 
 int tm_kernel_time(tm_ctx* ctx, int reset, double* allpairs_ms, long long* allpairs_launches, long long* total_launches) {
   if (!ctx) return TM_E_INVALID;
-  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  TM_CUDA(stream_wait(ctx));
   double ms = 0.0;
   for (size_t i = 0; i + 1 < ctx->ev_used; i += 2) {
     float t = 0.f;
@@ -827,7 +842,7 @@ int set_T_typed(tm_ctx* ctx, size_t count, const tm_c64* T, void* dst) {
                                                                  reinterpret_cast<Cx<R>*>(dst), count);
     e = cudaGetLastError();
   }
-  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  if (e == cudaSuccess) e = stream_wait(ctx);
   cudaFree(tmp);
   TM_CUDA(e);
   return TM_OK;
@@ -838,7 +853,7 @@ int matvec_typed(tm_ctx* ctx, int transpose, const tm_c64* x, tm_c64* y) {
   TM_CUDA(load_c64<R>(ctx, x, vec<R>(ctx, 0)));
   TM_CUDA(apply_operator<R>(ctx, transpose, vec<R>(ctx, 0), vec<R>(ctx, 1), vec<R>(ctx, 2), nullptr));
   TM_CUDA(store_c64<R>(ctx, vec<R>(ctx, 1), y));
-  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  TM_CUDA(stream_wait(ctx));
   return TM_OK;
 }
 
@@ -855,7 +870,7 @@ int solve_typed(tm_ctx* ctx, int adjoint, const tm_c64* w, const tm_solve_opts& 
   const int rc = gmres_solve<RV, R>(ctx, adjoint ? 1 : 0, o, info);
   if (rc < 0) return rc;
   TM_CUDA(store_c64<R>(ctx, vec<R>(ctx, 0), out));
-  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  TM_CUDA(stream_wait(ctx));
   return rc;
 }
 
@@ -869,7 +884,7 @@ int tm_set_tmatrices(tm_ctx* ctx, int n_types, int diag_only, const tm_c64* T, c
   std::vector<int> ht(ctx->n_scat);
   TM_CUDA(cudaMemcpy(ht.data(), type_of, ht.size() * sizeof(int), is_device_ptr(type_of) ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost));
   for (int v : ht) if (v < 0 || v >= n_types) return fail(ctx, TM_E_INVALID, "type_of out of range");
-  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  TM_CUDA(stream_wait(ctx));
   if (r_enclosing) {
     for (int t = 0; t < n_types; ++t)
       if (!(r_enclosing[t] >= 0.0)) return fail(ctx, TM_E_INVALID, "negative enclosing radius");
@@ -917,7 +932,7 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
     const tm_coeffs_desc* d = static_cast<const tm_coeffs_desc*>(desc);
     if (!d->p) return fail(ctx, TM_E_INVALID, "p is NULL");
     TM_CUDA(copy_in(ctx->d_p, d->p, ctx->n * sizeof(double2), ctx->stream));
-    TM_CUDA(cudaStreamSynchronize(ctx->stream));
+    TM_CUDA(stream_wait(ctx));
   } else if (kind == TM_INC_PLANE) {
     // Eq. II7 (explicit right-hand forms, reading R9b):
     //   a_{l,m,0} = -4 i^l     e^{-i m alpha} c_l [ i m pibar A_beta + taubar A_alpha ]
@@ -952,7 +967,7 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
       ctx->total_launches++;
       e = cudaGetLastError();
     }
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e == cudaSuccess) e = stream_wait(ctx);
     cudaFree(d_a);
     TM_CUDA(e);
   } else if (kind == TM_INC_GAUSS || kind == TM_INC_JINC) {
@@ -1021,7 +1036,7 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
       ctx->total_launches += 2;
       e = cudaGetLastError();
     }
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);   // the host vectors above must outlive the copies
+    if (e == cudaSuccess) e = stream_wait(ctx);   // the host vectors above must outlive the copies
     cudaFree(d_beta); cudaFree(d_wq); cudaFree(d_src); cudaFree(d_amp); cudaFree(d_ptr); cudaFree(d_nodes);
     TM_CUDA(e);
   } else {
@@ -1036,7 +1051,7 @@ int tm_get_incident(tm_ctx* ctx, tm_c64* p_out) {
   if (!ctx->has_inc) return fail(ctx, TM_E_STATE, "tm_set_incident has not been called");
   if (!p_out) return fail(ctx, TM_E_INVALID, "p_out is NULL");
   TM_CUDA(copy_out(p_out, ctx->d_p, ctx->n * sizeof(double2), ctx->stream));
-  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  TM_CUDA(stream_wait(ctx));
   return TM_OK;
 }
 
@@ -1104,7 +1119,7 @@ int tm_fields(tm_ctx* ctx, int n_pts, const double* pts, const tm_c64* s, int wh
     e = cudaGetLastError();
   }
   if (e == cudaSuccess) e = copy_out(out, d_out, nout * sizeof(double2), ctx->stream);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  if (e == cudaSuccess) e = stream_wait(ctx);
   cudaFree(d_pts); cudaFree(d_part); cudaFree(d_out);
   TM_CUDA(e);
   return TM_OK;
@@ -1141,7 +1156,7 @@ int tm_grad_tmatrix(tm_ctx* ctx, const tm_c64* dT, const tm_c64* lambda, const t
     e = cudaGetLastError();
   }
   if (e == cudaSuccess) e = copy_out(out, d_out, (size_t)ctx->n_scat * sizeof(double2), ctx->stream);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  if (e == cudaSuccess) e = stream_wait(ctx);
   cudaFree(d_dT); cudaFree(d_tmp); cudaFree(d_out);
   TM_CUDA(e);
   return TM_OK;
@@ -1192,7 +1207,7 @@ int grad_positions_typed(tm_ctx* ctx, const tm_c64* lambda, const tm_c64* s, con
     TM_G(cudaGetLastError());
   }
   TM_G(copy_out(out, d_out, (size_t)N * 3 * sizeof(double2), ctx->stream));
-  TM_G(cudaStreamSynchronize(ctx->stream));
+  TM_G(stream_wait(ctx));
 #undef TM_G
   cleanup();
   return TM_OK;
@@ -1209,7 +1224,7 @@ int tm_grad_positions(tm_ctx* ctx, const tm_c64* lambda, const tm_c64* s, const 
   if (ctx->lmax > 3) return fail(ctx, TM_E_INVALID, "position sensitivities are built for lmax <= 3");
   if (h < 0.0 || !std::isfinite(h)) return fail(ctx, TM_E_INVALID, "h must be >= 0");
   if (h == 0.0) h = 2e-4 * 2.0 * M_PI / ctx->k;
-  TM_CUDA(cudaStreamSynchronize(ctx->stream));
+  TM_CUDA(stream_wait(ctx));
   const int saved = ctx->kernel_req;
   ctx->kernel_req = TM_KERNEL_SYM3D;                      // displaced targets are not coplanar with the sources (alpha = z)
   int rc = configure_kernel(ctx);
