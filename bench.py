@@ -222,13 +222,18 @@ def run_ours(args, w, rank, world, local_rank):
             zero = libtm.SolveInfo(0, 0, 1, 0, 0.0, 0.0)
             return [one], [zero], 0, 0
 
+        solve_log = []
+
         def step_resident():
             set_inc(s)
             _, info, rc = s.solve(tol, w["restart"], max_iter, out=d_s)
+            solve_log.append(round(1e3 * info[0].seconds, 2))
             if args.forward_only:
                 info2, rc2 = [libtm.SolveInfo(0, 0, 1, 0, 0.0, 0.0)], 0
             else:
                 _, info2, rc2 = s.solve_adjoint(d_w, tol, w["restart"], max_iter, out=d_lam)
+            if not args.forward_only:
+                solve_log.append(round(1e3 * info2[0].seconds, 2))
             s.fields(d_pts, d_s, libtm.TM_FIELD_E_SCA, out=d_E)
             return info, info2, rc, rc2
 
@@ -374,6 +379,7 @@ def run_ours(args, w, rank, world, local_rank):
                          "pipe_frac": (pairs * fpinst / (ap_avg_ms * 1e-3)) / (peak * 1e12 / 2) if ap_launches else None,
                          "pairs_per_s": pairs / (ap_avg_ms * 1e-3) if ap_launches else None, "traffic": traffic},
             "clocks": clk, "ms_steps": [round(v, 3) for v in ms_list],
+            "solve_ms_log": solve_log[-2 * args.steps:] if args.mode == "full" else [],
         }
         if mixed is not None:
             out["mixed_precision"] = mixed

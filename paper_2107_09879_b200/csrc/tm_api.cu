@@ -83,6 +83,11 @@ struct tm_ctx {
   size_t ev_used = 0;
   long long allpairs_launches = 0, total_launches = 0;
 
+  // cached device scratch of the per-call paths (tm_set_incident, tm_fields): cudaMalloc / cudaFree synchronise the device and
+  // occasionally take hundreds of ms on a busy host, so nothing on the per-step path allocates
+  void* scratch[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  size_t scratch_cap[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  cudaEvent_t t0_ev = nullptr, t1_ev = nullptr;   // solve timing
   cudaEvent_t sync_ev = nullptr; // blocking-sync event: the host thread sleeps instead of spinning while the GPU works
 
   std::string err;
@@ -119,6 +124,20 @@ cudaError_t copy_out(void* dst, const void* src_dev, size_t bytes, cudaStream_t 
 // bytes of one element of the context's main vectors / T: fp64 in TM_FP64 and TM_MIXED, fp32 in TM_FP32
 // Wait for the context's stream without spinning (a spinning host thread burns the container's CPU quota during
 // multi-second solves; seen as occasional 2-3x outlier steps on shared hosts).
+// Device scratch slot `i` of at least `bytes` bytes (grown on demand, freed in tm_destroy).
+cudaError_t scratch_get(tm_ctx* c, int i, size_t bytes, void** out) {
+  if (c->scratch_cap[i] < bytes) {
+    if (c->scratch[i]) cudaFree(c->scratch[i]);
+    c->scratch[i] = nullptr; c->scratch_cap[i] = 0;
+    const size_t cap = bytes + bytes / 4 + 256;
+    cudaError_t e = cudaMalloc(&c->scratch[i], cap);
+    if (e != cudaSuccess) return e;
+    c->scratch_cap[i] = cap;
+  }
+  *out = c->scratch[i];
+  return cudaSuccess;
+}
+
 cudaError_t stream_wait(tm_ctx* c) {
   if (c->sync_ev == nullptr) {
     cudaError_t e = cudaEventCreateWithFlags(&c->sync_ev, cudaEventBlockingSync | cudaEventDisableTiming);
@@ -337,8 +356,8 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
   S.inner_floor = mixed ? 1e-5 : 0.0;                 // an fp32 cycle cannot usefully reduce its residual further
   cudaStream_t st = ctx->stream;
   const int wb = (nw + 63) / 64;
-  cudaEvent_t e0, e1;
-  TM_CUDA(cudaEventCreate(&e0)); TM_CUDA(cudaEventCreate(&e1));
+  if (!ctx->t0_ev) { TM_CUDA(cudaEventCreate(&ctx->t0_ev)); TM_CUDA(cudaEventCreate(&ctx->t1_ev)); }
+  cudaEvent_t e0 = ctx->t0_ev, e1 = ctx->t1_ev;
   TM_CUDA(cudaEventRecord(e0, st));
   TM_CUDA(cudaMemsetAsync(X, 0, n * sizeof(Cx<RX>), st));
   TM_CUDA(cudaMemsetAsync(V, 0, (size_t)(m + 2) * n * sizeof(Cx<R>), st));   // basis vectors must be finite (k_axpy)
@@ -462,7 +481,6 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
   TM_CUDA(cudaEventSynchronize(e1));
   float ms = 0.f;
   cudaEventElapsedTime(&ms, e0, e1);
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
   if (info)
     for (int w = 0; w < nw; ++w) {
       info[w].iterations = iters[w]; info[w].restarts = restarts[w]; info[w].converged = h_res[w] <= o.tol ? 1 : 0;
@@ -645,6 +663,9 @@ void tm_destroy(tm_ctx* c) {
   cudaFree(c->gm.blob);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
   if (c->sync_ev) cudaEventDestroy(c->sync_ev);
+  if (c->t0_ev) cudaEventDestroy(c->t0_ev);
+  if (c->t1_ev) cudaEventDestroy(c->t1_ev);
+  for (int i = 0; i < 8; ++i) cudaFree(c->scratch[i]);
   delete c;
 }
 
@@ -957,7 +978,7 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
       }
     }
     double2* d_a = nullptr;
-    TM_CUDA(cudaMalloc(&d_a, L * sizeof(double2)));
+    TM_CUDA(scratch_get(ctx, 0, L * sizeof(double2), reinterpret_cast<void**>(&d_a)));
     cudaError_t e = cudaMemcpyAsync(d_a, a.data(), L * sizeof(double2), cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) {
       const double sb = std::sin(d->beta);
@@ -968,7 +989,6 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
       e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = stream_wait(ctx);
-    cudaFree(d_a);
     TM_CUDA(e);
   } else if (kind == TM_INC_GAUSS || kind == TM_INC_JINC) {
     // both are angular-spectrum sources (Eqs. II9-II17): per window a list of source centres with transverse amplitudes
@@ -1096,9 +1116,9 @@ int tm_fields(tm_ctx* ctx, int n_pts, const double* pts, const tm_c64* s, int wh
   const int nch = std::min(nchunk, std::max(1, ctx->n_scat / 32));
   double* d_pts = nullptr; double2 *d_part = nullptr, *d_out = nullptr;
   const size_t nout = (size_t)n_pts * 3;
-  cudaError_t e = cudaMalloc(&d_pts, nout * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc(&d_part, nout * nch * sizeof(double2));
-  if (e == cudaSuccess) e = cudaMalloc(&d_out, nout * sizeof(double2));
+  cudaError_t e = scratch_get(ctx, 1, nout * sizeof(double), reinterpret_cast<void**>(&d_pts));
+  if (e == cudaSuccess) e = scratch_get(ctx, 2, nout * nch * sizeof(double2), reinterpret_cast<void**>(&d_part));
+  if (e == cudaSuccess) e = scratch_get(ctx, 3, nout * sizeof(double2), reinterpret_cast<void**>(&d_out));
   if (e == cudaSuccess) e = copy_in(d_pts, pts, nout * sizeof(double), ctx->stream);
   if (e == cudaSuccess) e = copy_in(ctx->d_io, s, ctx->n * sizeof(double2), ctx->stream);
   if (e == cudaSuccess) {
@@ -1120,7 +1140,6 @@ int tm_fields(tm_ctx* ctx, int n_pts, const double* pts, const tm_c64* s, int wh
   }
   if (e == cudaSuccess) e = copy_out(out, d_out, nout * sizeof(double2), ctx->stream);
   if (e == cudaSuccess) e = stream_wait(ctx);
-  cudaFree(d_pts); cudaFree(d_part); cudaFree(d_out);
   TM_CUDA(e);
   return TM_OK;
 }
