@@ -41,7 +41,7 @@ enum { TM_FP64 = 0, TM_FP32 = 1, TM_MIXED = 2 };         /* internal compute pre
 enum { TM_OK = 0, TM_NOT_CONVERGED = 1,
        TM_E_INVALID = -1, TM_E_OVERLAP = -2, TM_E_STATE = -3, TM_E_CUDA = -4, TM_E_NOMEM = -5 };
 enum { TM_INC_PLANE = 0, TM_INC_GAUSS = 1, TM_INC_COEFFS = 2, TM_INC_JINC = 3 };
-enum { TM_FIELD_E_SCA = 0, TM_FIELD_H_SCA = 1 };           /* H is returned as Z_b * H (reading R10) */
+enum { TM_FIELD_E_SCA = 0, TM_FIELD_H_SCA = 1, TM_FIELD_E_INC = 2 };   /* H is returned as Z_b * H (reading R10) */
 enum { TM_KERNEL_AUTO = 0, TM_KERNEL_GENERAL = 1, TM_KERNEL_COPLANAR = 2, TM_KERNEL_SYM3D = 3 };
 
 /* Plane wave travelling along (beta = polar angle from +z, alpha = azimuth) with amplitude
@@ -128,7 +128,10 @@ int tm_matvec(tm_ctx *ctx, int transpose, const tm_c64 *x, tm_c64 *y);
 /* Scattered fields at detector points (Eqs. I13/I24):
  *   E_sca(x) = sum_i sum_{lmp} s_{lmp;i} Phi_{lmp}(k_b (x - x_i)),  Z_b H_sca = -i sum s Phi_{l,m,1-p} (reading R10).
  *   pts [n_pts][3] doubles, s [n_scat][L], out [n_pts][3] Cartesian complex; all windows are summed
- *   (the paper sums the sub-region fields).  Points must not coincide with a scatterer centre. */
+ *   (the paper sums the sub-region fields).  Points must not coincide with a scatterer centre.
+ *   TM_FIELD_E_INC: the incident E field of the last tm_set_incident (plane wave, Gaussian beams or jinc sources; all
+ *   sources of all windows summed; s is ignored and may be NULL; TM_E_STATE after TM_INC_COEFFS or before tm_set_incident),
+ *   so that E_total = E_INC + E_SCA. */
 int tm_fields(tm_ctx *ctx, int n_pts, const double *pts, const tm_c64 *s, int which, tm_c64 *out);
 
 /* Device scratch.  tm_workspace_bytes: bytes tm_solve / tm_solve_adjoint need for these options (Krylov

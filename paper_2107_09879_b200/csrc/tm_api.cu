@@ -61,6 +61,11 @@ struct tm_ctx {
   int n_types = 0, diag = 1;
   bool has_T = false, has_inc = false;
   double2* d_p = nullptr;        // incident coefficients, fp64 [n]
+  // description of the last tm_set_incident (for TM_FIELD_E_INC)
+  int inc_kind = -1;
+  double inc_kvec[3] = {0, 0, 0}; double2 inc_e0[3] = {};            // plane wave
+  std::vector<double> inc_src; std::vector<double2> inc_amp;         // beams / jinc sources (all windows)
+  double inc_kw = -1.0, inc_bmax = 0.0; int inc_nb = 0;
   TmConst* d_const = nullptr;
   TmConst h_const{};
   int* d_rowptr = nullptr; uint8_t* d_col = nullptr; uint8_t* d_widx = nullptr; uint8_t* d_imag = nullptr; double* d_coef = nullptr;
@@ -982,6 +987,12 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
     cudaError_t e = cudaMemcpyAsync(d_a, a.data(), L * sizeof(double2), cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) {
       const double sb = std::sin(d->beta);
+      const double cbt = std::cos(d->beta), ca = std::cos(d->alpha), sa = std::sin(d->alpha);
+      ctx->inc_kvec[0] = ctx->k * sb * ca; ctx->inc_kvec[1] = ctx->k * sb * sa; ctx->inc_kvec[2] = ctx->k * cbt;
+      // E0 = A_beta beta_hat + A_alpha alpha_hat,  beta_hat = (cb ca, cb sa, -sb), alpha_hat = (-sa, ca, 0)
+      const cd ex = Ab * (cbt * ca) - Aa * sa, ey = Ab * (cbt * sa) + Aa * ca, ez = -Ab * sb;
+      ctx->inc_e0[0] = make_double2(ex.real(), ex.imag()); ctx->inc_e0[1] = make_double2(ey.real(), ey.imag());
+      ctx->inc_e0[2] = make_double2(ez.real(), ez.imag());
       const size_t tot = ctx->n;
       k_incident_plane<<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(ctx->d_pos, ctx->n_scat, L, d_a,
           ctx->k * sb * std::cos(d->alpha), ctx->k * sb * std::sin(d->alpha), ctx->k * std::cos(d->beta), ctx->d_p);
@@ -1023,6 +1034,7 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
     }
     const int nb = nb_req > 0 ? nb_req : 400;
     const size_t nsrc = hsrc.size() / 3;
+    ctx->inc_src = hsrc; ctx->inc_amp = hamp; ctx->inc_kw = kw; ctx->inc_bmax = bmax; ctx->inc_nb = nb;
     std::vector<double> xg, wg, beta(nb), wq(nb);
     gauss_legendre(nb, xg, wg);
     for (int q = 0; q < nb; ++q) { beta[q] = 0.5 * bmax * (xg[q] + 1.0); wq[q] = 0.5 * bmax * wg[q]; }
@@ -1063,6 +1075,7 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
     return fail(ctx, TM_E_INVALID, "unknown incident kind");
   }
   ctx->has_inc = true;
+  ctx->inc_kind = kind;
   return TM_OK;
 }
 
@@ -1110,6 +1123,49 @@ int tm_solve_adjoint(tm_ctx* ctx, const tm_c64* w, const tm_solve_opts* opts, tm
 
 int tm_fields(tm_ctx* ctx, int n_pts, const double* pts, const tm_c64* s, int which, tm_c64* out) {
   if (!ctx) return TM_E_INVALID;
+  if (which == TM_FIELD_E_INC) {
+    if (n_pts < 1 || !pts || !out) return fail(ctx, TM_E_INVALID, "bad arguments");
+    if (!ctx->has_inc || ctx->inc_kind == TM_INC_COEFFS || ctx->inc_kind < 0)
+      return fail(ctx, TM_E_STATE, "TM_FIELD_E_INC needs a plane-wave, Gaussian-beam or jinc incident field");
+    const size_t nout = (size_t)n_pts * 3;
+    double* d_pts = nullptr; double2* d_out = nullptr;
+    cudaError_t e = scratch_get(ctx, 1, nout * sizeof(double), reinterpret_cast<void**>(&d_pts));
+    if (e == cudaSuccess) e = scratch_get(ctx, 3, nout * sizeof(double2), reinterpret_cast<void**>(&d_out));
+    if (e == cudaSuccess) e = copy_in(d_pts, pts, nout * sizeof(double), ctx->stream);
+    if (e == cudaSuccess && ctx->inc_kind == TM_INC_PLANE) {
+      k_inc_field_plane<<<(n_pts + 127) / 128, 128, 0, ctx->stream>>>(d_pts, n_pts, ctx->inc_kvec[0], ctx->inc_kvec[1], ctx->inc_kvec[2],
+                                                                      ctx->inc_e0[0], ctx->inc_e0[1], ctx->inc_e0[2], d_out);
+      e = cudaGetLastError();
+    } else if (e == cudaSuccess) {
+      const int nb = ctx->inc_nb;
+      const size_t nsrc = ctx->inc_src.size() / 3;
+      std::vector<double> xg, wg, tab(3 * (size_t)nb);          // [w G sin | cos | sin]
+      gauss_legendre(nb, xg, wg);
+      for (int q = 0; q < nb; ++q) {
+        const double b = 0.5 * ctx->inc_bmax * (xg[q] + 1.0), sbq = std::sin(b), kw = ctx->inc_kw;
+        tab[q] = 0.5 * ctx->inc_bmax * wg[q] * (kw > 0.0 ? 0.5 * kw * kw * std::exp(-0.25 * kw * kw * sbq * sbq) : 1.0) * sbq;
+        tab[nb + q] = std::cos(b); tab[2 * (size_t)nb + q] = sbq;
+      }
+      double *d_tab = nullptr, *d_src = nullptr; double2* d_amp = nullptr;
+      e = scratch_get(ctx, 4, tab.size() * sizeof(double), reinterpret_cast<void**>(&d_tab));
+      if (e == cudaSuccess) e = scratch_get(ctx, 5, std::max<size_t>(1, nsrc) * 3 * sizeof(double), reinterpret_cast<void**>(&d_src));
+      if (e == cudaSuccess) e = scratch_get(ctx, 6, std::max<size_t>(1, nsrc) * 2 * sizeof(double2), reinterpret_cast<void**>(&d_amp));
+      if (e == cudaSuccess) e = cudaMemcpyAsync(d_tab, tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
+      if (e == cudaSuccess && nsrc) e = cudaMemcpyAsync(d_src, ctx->inc_src.data(), nsrc * 3 * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
+      if (e == cudaSuccess && nsrc) e = cudaMemcpyAsync(d_amp, ctx->inc_amp.data(), nsrc * 2 * sizeof(double2), cudaMemcpyHostToDevice, ctx->stream);
+      if (e == cudaSuccess) {
+        k_inc_field_beams<<<(n_pts + 127) / 128, 128, 0, ctx->stream>>>(d_pts, n_pts, d_src, d_amp, (int)nsrc, d_tab, d_tab + nb,
+                                                                        d_tab + 2 * (size_t)nb, nb, ctx->k, d_out);
+        e = cudaGetLastError();
+      }
+      if (e == cudaSuccess) e = stream_wait(ctx);             // tab must outlive the copy
+    }
+    ctx->total_launches += 1;
+    if (e == cudaSuccess) e = copy_out(out, d_out, nout * sizeof(double2), ctx->stream);
+    if (e == cudaSuccess) e = stream_wait(ctx);
+    TM_CUDA(e);
+    return TM_OK;
+  }
   if (n_pts < 1 || !pts || !s || !out) return fail(ctx, TM_E_INVALID, "bad arguments");
   if (which != TM_FIELD_E_SCA && which != TM_FIELD_H_SCA) return fail(ctx, TM_E_INVALID, "unknown field id");
   const int nchunk = std::max(1, std::min(64, (int)(148LL * 8 * 128 / std::max(1, n_pts))));

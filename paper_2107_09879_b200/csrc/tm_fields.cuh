@@ -93,3 +93,55 @@ __global__ void k_fields_reduce(const double2* __restrict__ part, int n_chunk, s
   for (int c = 1; c < n_chunk; ++c) { a.x += part[(size_t)c * n + e].x; a.y += part[(size_t)c * n + e].y; }
   out[e] = a;
 }
+
+// ------------------------------------------------------------------------------------------------ incident field
+// Plane wave (Eq. II6): E_inc(x) = E0 exp(i k . x),  E0 = A_beta beta_hat + A_alpha alpha_hat (Cartesian, complex).
+__global__ void k_inc_field_plane(const double* __restrict__ pts, int n_pts, double kx, double ky, double kz,
+                                  double2 e0x, double2 e0y, double2 e0z, double2* __restrict__ out) {
+  const int ip = blockIdx.x * blockDim.x + threadIdx.x;
+  if (ip >= n_pts) return;
+  double s, c;
+  sincos(kx * pts[3 * ip] + ky * pts[3 * ip + 1] + kz * pts[3 * ip + 2], &s, &c);
+  out[3 * ip] = make_double2(e0x.x * c - e0x.y * s, e0x.x * s + e0x.y * c);
+  out[3 * ip + 1] = make_double2(e0y.x * c - e0y.y * s, e0y.x * s + e0y.y * c);
+  out[3 * ip + 2] = make_double2(e0z.x * c - e0z.y * s, e0z.x * s + e0z.y * c);
+}
+
+// Angular-spectrum sources (Gaussian beams: reading R9; jinc sources: Eqs. II3-II5), all sources of all windows summed:
+//   E(x) = (1/2pi) int A(beta,alpha) exp(i k.(x - x0)) G(beta) sin(beta) cos(beta) dalpha dbeta,
+//   A = A^T - z_hat tan(beta) (Ax cos(alpha) + Ay sin(alpha))                                           (Eq. II5)
+// with the alpha integral in closed form (Jacobi-Anger): transverse part J_0(rho), z part i J_1(rho) (Ax cos xi + Ay sin xi),
+// rho = k rho_T sin(beta), (rho_T, xi) = polar coordinates of x^T - x0^T, and the same Gauss-Legendre nodes in beta as the
+// coefficient kernel (wq[q] already holds w_q G(beta_q) sin(beta_q)).  One thread per detector point.
+__global__ void __launch_bounds__(128)
+k_inc_field_beams(const double* __restrict__ pts, int n_pts, const double* __restrict__ src, const double2* __restrict__ amp,
+                  int n_src, const double* __restrict__ wq, const double* __restrict__ cb, const double* __restrict__ sb,
+                  int n_beta, double k, double2* __restrict__ out) {
+  const int ip = blockIdx.x * blockDim.x + threadIdx.x;
+  if (ip >= n_pts) return;
+  const double px = pts[3 * ip], py = pts[3 * ip + 1], pz = pts[3 * ip + 2];
+  double exr = 0, exi = 0, eyr = 0, eyi = 0, ezr = 0, ezi = 0;
+  for (int s = 0; s < n_src; ++s) {
+    const double rx = px - src[3 * s], ry = py - src[3 * s + 1], rz = pz - src[3 * s + 2];
+    const double rhoT = sqrt(rx * rx + ry * ry);
+    const double cxi = rhoT > 0.0 ? rx / rhoT : 1.0, sxi = rhoT > 0.0 ? ry / rhoT : 0.0;
+    const double2 Ax = amp[2 * s], Ay = amp[2 * s + 1];
+    double tr = 0, ti = 0, zr = 0, zi = 0;           // int w cos(b) J0 e^{ikz cos b},  int w sin(b) J1 e^{ikz cos b}
+    for (int q = 0; q < n_beta; ++q) {
+      double J[2];
+      bessel_j_all<1>(k * rhoT * sb[q], J);
+      double sz, cz;
+      sincos(k * rz * cb[q], &sz, &cz);
+      const double wt = wq[q] * cb[q] * J[0], wz = wq[q] * sb[q] * J[1];
+      tr += wt * cz; ti += wt * sz;
+      zr += wz * cz; zi += wz * sz;
+    }
+    exr += Ax.x * tr - Ax.y * ti; exi += Ax.x * ti + Ax.y * tr;
+    eyr += Ay.x * tr - Ay.y * ti; eyi += Ay.x * ti + Ay.y * tr;
+    // E_z = -i (Ax cos xi + Ay sin xi) (zr + i zi)
+    const double gr = Ax.x * cxi + Ay.x * sxi, gi = Ax.y * cxi + Ay.y * sxi;
+    const double mr = gr * zr - gi * zi, mi = gr * zi + gi * zr;
+    ezr += mi; ezi += -mr;
+  }
+  out[3 * ip] = make_double2(exr, exi); out[3 * ip + 1] = make_double2(eyr, eyi); out[3 * ip + 2] = make_double2(ezr, ezi);
+}

@@ -16,7 +16,7 @@ TM_FP64, TM_FP32, TM_MIXED = 0, 1, 2
 TM_OK, TM_NOT_CONVERGED = 0, 1
 TM_E_INVALID, TM_E_OVERLAP, TM_E_STATE, TM_E_CUDA, TM_E_NOMEM = -1, -2, -3, -4, -5
 TM_INC_PLANE, TM_INC_GAUSS, TM_INC_COEFFS, TM_INC_JINC = 0, 1, 2, 3
-TM_FIELD_E_SCA, TM_FIELD_H_SCA = 0, 1
+TM_FIELD_E_SCA, TM_FIELD_H_SCA, TM_FIELD_E_INC = 0, 1, 2
 TM_KERNEL_AUTO, TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR, TM_KERNEL_SYM3D = 0, 1, 2, 3
 
 EXPORTS = ["tm_create", "tm_set_tmatrices", "tm_set_incident", "tm_get_incident", "tm_solve", "tm_solve_adjoint",
@@ -264,7 +264,7 @@ class Solver:
 
     def fields(self, pts, s, which=TM_FIELD_E_SCA, out=None):
         pts = np.ascontiguousarray(pts, dtype=np.float64) if isinstance(pts, np.ndarray) else pts
-        s = np.ascontiguousarray(s, dtype=np.complex128) if isinstance(s, np.ndarray) else s
+        s = np.ascontiguousarray(s, dtype=np.complex128) if isinstance(s, np.ndarray) else s      # None for TM_FIELD_E_INC
         n_pts = int(pts.shape[0])
         if out is None:
             if isinstance(pts, np.ndarray):

@@ -258,3 +258,33 @@ def test_mixed_precision_iterative_refinement(tm):
     sol, info, rc = s.solve(1e-11, 50, 5000)
     assert rc == 0 and rel(sol, ref["s"]) <= 1e-9
     s.close()
+
+
+def test_incident_field_at_detector_points(tm):
+    """TM_FIELD_E_INC: plane wave (closed form), Gaussian beams and jinc sources (direct 2-D quadrature of Eq. II4 in the
+    oracle), all sources of all windows summed."""
+    from oracle import incident
+    pos = W.random_cloud(6, seed=71)
+    pts = np.random.default_rng(72).uniform(-2, 2, (9, 3))
+    s = tm.Solver(pos, 2, W.K_B, win_ptr=np.array([0, 2, 6], dtype=np.int32))
+    with pytest.raises(tm.TmError) as e:
+        s.fields(pts, None, tm.TM_FIELD_E_INC)
+    assert e.value.code == tm.TM_E_STATE
+    beta, alpha, Ab, Aa = 0.5, -0.7, 0.8, 0.3 - 0.4j
+    s.set_incident_plane(beta, alpha, Ab, Aa)
+    kv = W.K_B * np.array([np.sin(beta) * np.cos(alpha), np.sin(beta) * np.sin(alpha), np.cos(beta)])
+    bh = np.array([np.cos(beta) * np.cos(alpha), np.cos(beta) * np.sin(alpha), -np.sin(beta)])
+    ah = np.array([-np.sin(alpha), np.cos(alpha), 0.0])
+    ref = (Ab * bh + Aa * ah)[None, :] * np.exp(1j * pts @ kv)[:, None]
+    assert rel(s.fields(pts, None, tm.TM_FIELD_E_INC), ref) <= 1e-13
+    focus = np.array([[0.2, -0.1, -0.5], [-0.6, 0.4, -0.5]])
+    s.set_incident_gauss(focus, 1.5, 0.8, 0.3 - 0.4j)
+    ref = np.array([sum(incident.gaussian_beam_field_direct(W.K_B, p, f, 1.5, 0.8, 0.3 - 0.4j, n_beta=300, n_alpha=512) for f in focus)
+                    for p in pts])
+    assert rel(s.fields(pts, None, tm.TM_FIELD_E_INC), ref) <= 1e-8
+    src = np.array([[0.5, 0.5, -1.0], [-1.0, 0.2, -1.0], [0.0, 0.0, -1.0]])
+    amp = np.array([[1.0, 0.2j], [0.3, -0.7], [0.5j, 0.1]])
+    s.set_incident_jinc(src, amp, np.array([0, 1, 3], dtype=np.int32))
+    ref = np.array([sum(incident.jinc_field_direct(W.K_B, p, src[i], amp[i, 0], amp[i, 1]) for i in range(3)) for p in pts])
+    assert rel(s.fields(pts, None, tm.TM_FIELD_E_INC), ref) <= 1e-7
+    s.close()
