@@ -590,98 +590,134 @@ def coplanar_sectors(lmax):
     return out
 
 
+COP4_GROUPS = {4: 1, 5: 2, 6: 4}     # row groups per sector: keeps one block's straight-line code near the 32 KB L1.5 I-cache
+
+
 def emit_coplanar4(lmaxes, path):
     with open(path, "w") as f:
         f.write("// GENERATED by gen_tables.py - do not edit.\n")
-        f.write("// Coplanar translation apply for lmax 4..6, one of FOUR uncoupled sectors (z-mirror parity x y'-mirror sector) per call\n")
-        f.write("// (DESIGN.md, kernel K2c4).  xs: [own slots | partner slots] d-values; ar/ai: [own | partner] accumulators, stride AS.\n#pragma once\n\n")
+        f.write("// Coplanar translation apply for lmax 4..6: FOUR uncoupled sectors (z-mirror parity x y'-mirror sector), each split into\n")
+        f.write("// G row groups so that one block's straight-line code stays near the instruction-cache size (DESIGN.md, kernel K2c4).\n")
+        f.write("// xs: [own slots | partner slots] d-values of the sector; ar/ai: [own rows of the group | their partner share], stride AS.\n#pragma once\n\n")
         for lmax in lmaxes:
             md = modes(lmax)
             idx = {t_: i for i, t_ in enumerate(md)}
             nq = 2 * lmax + 1
             half_l = len(md) // 2
+            G = COP4_GROUPS[lmax]
             cost = [0, 0]
             nmax = 0
+            rmax = 0
             secs = coplanar_sectors(lmax)
             for z in range(4):
                 slots, rows = secs[z]
                 n = len(slots)
                 nmax = max(nmax, n)
-                f.write(f"// lmax={lmax} sector z={z}: slots (l,|m|,p,kind) {slots}\n")
-                f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
-                        f"tm_cop4_pair_L{lmax}_Z{z}(const R* __restrict__ xs, const R* cm, const R* sm, const R* hr, const R* hi, R* ar, R* ai) {{\n")
-                n_pairs = n_zero = 0
-                for k, (l, am, p, kind) in enumerate(slots):
-                    if kind == "0":
-                        f.write(f"  const R xr{k} = xs[{2 * k}], xi{k} = xs[{2 * k + 1}];\n")
-                        n_zero += 1
-                    else:      # x^own = c d^own + i s d^partner
-                        f.write(f"  const R xr{k} = xs[{2 * k}] * cm[{am}] - xs[{2 * (n + k) + 1}] * sm[{am}], "
-                                f"xi{k} = xs[{2 * k + 1}] * cm[{am}] + xs[{2 * (n + k)}] * sm[{am}];\n")
-                        n_pairs += 1
-                nterm = nrowq = 0
-                for r, (l, am, p, kind) in enumerate(slots):
-                    f.write("  {\n    R ur = R(0), ui = R(0), yr, yi;\n")
-                    for q in range(nq):
-                        terms = rows[r][q]
-                        if not terms:
-                            continue
-                        nrowq += 1
-                        for t_, (c, v) in enumerate(terms):
-                            nterm += 1
-                            if t_ == 0:
-                                f.write(f"    yr = R({lit(v)}) * xr{c}; yi = R({lit(v)}) * xi{c};\n")
-                            else:
-                                f.write(f"    yr = fma(R({lit(v)}), xr{c}, yr); yi = fma(R({lit(v)}), xi{c}, yi);\n")
-                        f.write(f"    ur = fma(hr[{q}], yr, ur); ur = fma(-hi[{q}], yi, ur); ui = fma(hr[{q}], yi, ui); ui = fma(hi[{q}], yr, ui);\n")
-                    if kind == "0":
-                        f.write(f"    ar[{r} * AS] += ur; ai[{r} * AS] += ui;\n")
-                    else:      # A^own += c u ;  A^partner += -i s u
-                        f.write(f"    ar[{r} * AS] = fma(ur, cm[{am}], ar[{r} * AS]); ai[{r} * AS] = fma(ui, cm[{am}], ai[{r} * AS]);\n")
-                        f.write(f"    ar[{n + r} * AS] = fma(ui, sm[{am}], ar[{n + r} * AS]); ai[{n + r} * AS] = fma(-ur, sm[{am}], ai[{n + r} * AS]);\n")
-                    f.write("  }\n")
-                f.write("}\n")
-                inst = 2 * nterm + 4 * nrowq + 8 * n_pairs + 2 * n_zero
-                flop = (2 * nrowq + 4 * (nterm - nrowq)) + 8 * nrowq + (6 + 8) * n_pairs + 2 * n_zero
-                cost[0] += inst
-                cost[1] += flop
-                print(f"lmax={lmax} sector z={z}: n={n} terms={nterm} (row,q)={nrowq} -> {inst} FP instructions, {flop} flop", file=sys.stderr)
+                # staging tables of the sector: own slots then partner slots
                 sa, sb, ss = [], [], []
                 for (l, am, p, kind) in slots:
                     sa.append(idx[(l, am, p)]); sb.append(idx[(l, -am, p)]); ss.append({"0": 0, "+": 1, "-": -1}[kind])
                 for (l, am, p, kind) in slots:
                     sa.append(idx[(l, am, p)]); sb.append(idx[(l, -am, p)]); ss.append({"0": 0, "+": -1, "-": 1}[kind])
+                f.write(f"// lmax={lmax} sector z={z}: slots (l,|m|,p,kind) {slots}\n")
                 f.write(f"__device__ __constant__ int tm_cop4_sa_L{lmax}_Z{z}[{2 * n}] = {{{', '.join(map(str, sa))}}};\n")
                 f.write(f"__device__ __constant__ int tm_cop4_sb_L{lmax}_Z{z}[{2 * n}] = {{{', '.join(map(str, sb))}}};\n")
                 f.write(f"__device__ __constant__ int tm_cop4_ss_L{lmax}_Z{z}[{2 * n}] = {{{', '.join(map(str, ss))}}};\n")
                 f.write(f"#define TM_COP4_N_L{lmax}_Z{z} {n}\n")
-                # unmix: this sector's share of u~ for the modes of its parity half (the partner sector z^1 adds the rest)
-                f.write("template <typename R, typename C, int AS>\n__device__ __forceinline__ void "
-                        f"tm_cop4_unmix_L{lmax}_Z{z}(const R* ar, const R* ai, C* out) {{\n")
-
-                def store(i_flat, re, im):
-                    if i_flat >= half_l:
-                        f.write(f"  out[{i_flat}].re = {im}; out[{i_flat}].im = -({re});\n")
-                    else:
-                        f.write(f"  out[{i_flat}].re = {re}; out[{i_flat}].im = {im};\n")
-                covered = set()
-                for r, (l, am, p, kind) in enumerate(slots):
-                    if kind == "0":
-                        store(idx[(l, 0, p)], f"ar[{r} * AS]", f"ai[{r} * AS]")
-                        covered.add(idx[(l, 0, p)])
-                    else:
-                        pr_, pi_ = (f"ar[{r} * AS]", f"ai[{r} * AS]") if kind == "+" else (f"ar[{n + r} * AS]", f"ai[{n + r} * AS]")
-                        mr_, mi_ = (f"ar[{n + r} * AS]", f"ai[{n + r} * AS]") if kind == "+" else (f"ar[{r} * AS]", f"ai[{r} * AS]")
-                        store(idx[(l, am, p)], f"R(0.5) * ({pr_} + {mr_})", f"R(0.5) * ({pi_} + {mi_})")
-                        store(idx[(l, -am, p)], f"R(0.5) * ({pr_} - {mr_})", f"R(0.5) * ({pi_} - {mi_})")
-                        covered.add(idx[(l, am, p)]); covered.add(idx[(l, -am, p)])
+                # row groups: contiguous, balanced by term count
+                work = [sum(len(rows[r][q]) for q in range(nq)) + 4 for r in range(n)]
+                bounds = [0]
+                acc_w, target = 0, sum(work) / G
+                for r in range(n):
+                    acc_w += work[r]
+                    if len(bounds) < G and acc_w >= target * len(bounds) and r + 1 < n:
+                        bounds.append(r + 1)
+                while len(bounds) < G:
+                    bounds.append(n)
+                bounds.append(n)
                 hpar = z // 2
-                for i_flat, (l, m, p) in enumerate(md):
-                    if (l + m + p) % 2 == hpar and i_flat not in covered:    # m = 0 modes owned by the partner sector
-                        f.write(f"  out[{i_flat}].re = R(0); out[{i_flat}].im = R(0);\n")
-                f.write("}\n")
+                covered_sector = set()
+                for (l, am, p, kind) in slots:
+                    covered_sector.add(idx[(l, am, p)]); covered_sector.add(idx[(l, -am, p)])
+                for g in range(G):
+                    r0, r1 = bounds[g], bounds[g + 1]
+                    nr = r1 - r0
+                    rmax = max(rmax, nr)
+                    used_cols = sorted({c for r in range(r0, r1) for q in range(nq) for (c, _) in rows[r][q]})
+                    f.write(f"// lmax={lmax} z={z} group={g}: rows {r0}..{r1 - 1}\n")
+                    f.write(f"#define TM_COP4_NR_L{lmax}_Z{z}_G{g} {nr}\n")
+                    f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
+                            f"tm_cop4_pair_L{lmax}_Z{z}_G{g}(const R* __restrict__ xs, const R* cm, const R* sm, const R* hr, const R* hi, R* ar, R* ai) {{\n")
+                    n_pairs = n_zero = 0
+                    for k in used_cols:
+                        l, am, p, kind = slots[k]
+                        if kind == "0":
+                            f.write(f"  const R xr{k} = xs[{2 * k}], xi{k} = xs[{2 * k + 1}];\n")
+                            n_zero += 1
+                        else:      # x^own = c d^own + i s d^partner
+                            f.write(f"  const R xr{k} = xs[{2 * k}] * cm[{am}] - xs[{2 * (n + k) + 1}] * sm[{am}], "
+                                    f"xi{k} = xs[{2 * k + 1}] * cm[{am}] + xs[{2 * (n + k)}] * sm[{am}];\n")
+                            n_pairs += 1
+                    nterm = nrowq = 0
+                    for r in range(r0, r1):
+                        l, am, p, kind = slots[r]
+                        lr = r - r0
+                        f.write("  {\n    R ur = R(0), ui = R(0), yr, yi;\n")
+                        for q in range(nq):
+                            terms = rows[r][q]
+                            if not terms:
+                                continue
+                            nrowq += 1
+                            for t_, (c, v) in enumerate(terms):
+                                nterm += 1
+                                if t_ == 0:
+                                    f.write(f"    yr = R({lit(v)}) * xr{c}; yi = R({lit(v)}) * xi{c};\n")
+                                else:
+                                    f.write(f"    yr = fma(R({lit(v)}), xr{c}, yr); yi = fma(R({lit(v)}), xi{c}, yi);\n")
+                            f.write(f"    ur = fma(hr[{q}], yr, ur); ur = fma(-hi[{q}], yi, ur); ui = fma(hr[{q}], yi, ui); ui = fma(hi[{q}], yr, ui);\n")
+                        if kind == "0":
+                            f.write(f"    ar[{lr} * AS] += ur; ai[{lr} * AS] += ui;\n")
+                        else:      # A^own += c u ;  A^partner += -i s u
+                            f.write(f"    ar[{lr} * AS] = fma(ur, cm[{am}], ar[{lr} * AS]); ai[{lr} * AS] = fma(ui, cm[{am}], ai[{lr} * AS]);\n")
+                            f.write(f"    ar[({nr + lr}) * AS] = fma(ui, sm[{am}], ar[({nr + lr}) * AS]); ai[({nr + lr}) * AS] = fma(-ur, sm[{am}], ai[({nr + lr}) * AS]);\n")
+                        f.write("  }\n")
+                    f.write("}\n")
+                    nrp = sum(1 for r in range(r0, r1) if slots[r][3] != "0")
+                    inst = 2 * nterm + 4 * nrowq + 4 * n_pairs + 4 * nrp + 2 * (nr - nrp)
+                    flop = (2 * nrowq + 4 * (nterm - nrowq)) + 8 * nrowq + 6 * n_pairs + 8 * nrp + 2 * (nr - nrp)
+                    cost[0] += inst
+                    cost[1] += flop
+                    print(f"lmax={lmax} z={z} g={g}: rows={nr} cols={len(used_cols)} terms={nterm} (row,q)={nrowq} -> {inst} FP instructions", file=sys.stderr)
+                    # unmix of the group's rows (+ the zero fill of the partner-owned m = 0 modes, done by group 0)
+                    f.write("template <typename R, typename C, int AS>\n__device__ __forceinline__ void "
+                            f"tm_cop4_unmix_L{lmax}_Z{z}_G{g}(const R* ar, const R* ai, C* out) {{\n")
+
+                    def store(i_flat, re, im):
+                        if i_flat >= half_l:
+                            f.write(f"  out[{i_flat}].re = {im}; out[{i_flat}].im = -({re});\n")
+                        else:
+                            f.write(f"  out[{i_flat}].re = {re}; out[{i_flat}].im = {im};\n")
+                    for r in range(r0, r1):
+                        l, am, p, kind = slots[r]
+                        lr = r - r0
+                        own_r, own_i = f"ar[{lr} * AS]", f"ai[{lr} * AS]"
+                        par_r, par_i = f"ar[({nr + lr}) * AS]", f"ai[({nr + lr}) * AS]"
+                        if kind == "0":
+                            store(idx[(l, 0, p)], own_r, own_i)
+                        else:
+                            pr_, pi_ = (own_r, own_i) if kind == "+" else (par_r, par_i)
+                            mr_, mi_ = (par_r, par_i) if kind == "+" else (own_r, own_i)
+                            store(idx[(l, am, p)], f"R(0.5) * ({pr_} + {mr_})", f"R(0.5) * ({pi_} + {mi_})")
+                            store(idx[(l, -am, p)], f"R(0.5) * ({pr_} - {mr_})", f"R(0.5) * ({pi_} - {mi_})")
+                    if g == 0:
+                        for i_flat, (l, m, p) in enumerate(md):
+                            if (l + m + p) % 2 == hpar and i_flat not in covered_sector:
+                                f.write(f"  out[{i_flat}].re = R(0); out[{i_flat}].im = R(0);\n")
+                    f.write("}\n")
             f.write(f"#define TM_COP4_NMAX_L{lmax} {nmax}\n")
-            f.write(f"#define TM_COP4_FPINST_L{lmax} {cost[0]}   // FP instructions per ordered pair (all four sectors)\n")
+            f.write(f"#define TM_COP4_G_L{lmax} {G}\n")
+            f.write(f"#define TM_COP4_NRMAX_L{lmax} {rmax}\n")
+            f.write(f"#define TM_COP4_FPINST_L{lmax} {cost[0]}   // FP instructions per ordered pair (all sectors and row groups)\n")
             f.write(f"#define TM_COP4_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")
 
 

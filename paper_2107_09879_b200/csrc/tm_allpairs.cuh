@@ -438,52 +438,58 @@ k_allpairs_sym3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
 // instruction-fetch bound there, still an order of magnitude ahead of the table-driven kernel.
 #include "generated/tm_coplanar4_gen.cuh"
 
-template <typename R, int LMAX, int Z> struct Cop4;
-#define TM_COP4_SPEC(LM, ZZ)                                                                             \
-  template <typename R> struct Cop4<R, LM, ZZ> {                                                         \
+template <typename R, int LMAX, int Z, int G> struct Cop4;
+#define TM_COP4_SPEC(LM, ZZ, GG)                                                                         \
+  template <typename R> struct Cop4<R, LM, ZZ, GG> {                                                     \
     static constexpr int n = TM_COP4_N_L##LM##_Z##ZZ;                                                    \
+    static constexpr int nr = TM_COP4_NR_L##LM##_Z##ZZ##_G##GG;                                          \
     template <int AS>                                                                                    \
     static __device__ __forceinline__ void run(const R* xs, const R* cm, const R* sm, const R* hr,       \
                                                const R* hi, R* ar, R* ai) {                              \
-      tm_cop4_pair_L##LM##_Z##ZZ<R, AS>(xs, cm, sm, hr, hi, ar, ai);                                     \
+      tm_cop4_pair_L##LM##_Z##ZZ##_G##GG<R, AS>(xs, cm, sm, hr, hi, ar, ai);                             \
     }                                                                                                    \
     template <int AS>                                                                                    \
     static __device__ __forceinline__ void unmix(const R* ar, const R* ai, Cx<R>* out) {                 \
-      tm_cop4_unmix_L##LM##_Z##ZZ<R, Cx<R>, AS>(ar, ai, out);                                            \
+      tm_cop4_unmix_L##LM##_Z##ZZ##_G##GG<R, Cx<R>, AS>(ar, ai, out);                                    \
     }                                                                                                    \
     static __device__ __forceinline__ void stage_entry(int k, int& a, int& b, int& sg) {                 \
       a = tm_cop4_sa_L##LM##_Z##ZZ[k]; b = tm_cop4_sb_L##LM##_Z##ZZ[k]; sg = tm_cop4_ss_L##LM##_Z##ZZ[k]; \
     }                                                                                                    \
   };
-TM_COP4_SPEC(4, 0) TM_COP4_SPEC(4, 1) TM_COP4_SPEC(4, 2) TM_COP4_SPEC(4, 3)
-TM_COP4_SPEC(5, 0) TM_COP4_SPEC(5, 1) TM_COP4_SPEC(5, 2) TM_COP4_SPEC(5, 3)
-TM_COP4_SPEC(6, 0) TM_COP4_SPEC(6, 1) TM_COP4_SPEC(6, 2) TM_COP4_SPEC(6, 3)
+#define TM_COP4_SPEC_Z(LM, GG) TM_COP4_SPEC(LM, 0, GG) TM_COP4_SPEC(LM, 1, GG) TM_COP4_SPEC(LM, 2, GG) TM_COP4_SPEC(LM, 3, GG)
+TM_COP4_SPEC_Z(4, 0)
+TM_COP4_SPEC_Z(5, 0) TM_COP4_SPEC_Z(5, 1)
+TM_COP4_SPEC_Z(6, 0) TM_COP4_SPEC_Z(6, 1) TM_COP4_SPEC_Z(6, 2) TM_COP4_SPEC_Z(6, 3)
+#undef TM_COP4_SPEC_Z
 #undef TM_COP4_SPEC
 
-template <int LMAX> struct Cop4Max;
-template <> struct Cop4Max<4> { static constexpr int n = TM_COP4_NMAX_L4; };
-template <> struct Cop4Max<5> { static constexpr int n = TM_COP4_NMAX_L5; };
-template <> struct Cop4Max<6> { static constexpr int n = TM_COP4_NMAX_L6; };
+template <int LMAX> struct Cop4Max;      // n: slots of the largest sector; nr: rows of the largest row group; ng: row groups per sector
+template <> struct Cop4Max<4> { static constexpr int n = TM_COP4_NMAX_L4, nr = TM_COP4_NRMAX_L4, ng = TM_COP4_G_L4; };
+template <> struct Cop4Max<5> { static constexpr int n = TM_COP4_NMAX_L5, nr = TM_COP4_NRMAX_L5, ng = TM_COP4_G_L5; };
+template <> struct Cop4Max<6> { static constexpr int n = TM_COP4_NMAX_L6, nr = TM_COP4_NRMAX_L6, ng = TM_COP4_G_L6; };
 
 template <typename R, int LMAX, int TJ, int SS> struct Cop4Smem {
   static constexpr int NM = Cop4Max<LMAX>::n;
-  static constexpr size_t bytes = sizeof(double) * 2 * SS + sizeof(R) * (size_t)(SS * 2 * NM * 2 + 2 * 2 * NM * TJ) + sizeof(int) * 3 * 2 * NM;
+  static constexpr int NR = Cop4Max<LMAX>::nr;
+  static constexpr size_t bytes = sizeof(double) * 2 * SS + sizeof(R) * (size_t)(SS * 2 * NM * 2 + 2 * 2 * NR * TJ) + sizeof(int) * 3 * 2 * NM;
 };
 
-template <typename R, int LMAX, int Z, int TJ, int SS>
+template <typename R, int LMAX, int Z, int G, int TJ, int SS>
 __device__ __forceinline__ void cop4_sector(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
                                             const TmTile tile, int n_scat, double k_over_pi, double inv_k, TmShift shift,
                                             unsigned char* smem_raw) {
-  using S = Cop4<R, LMAX, Z>;
+  using S = Cop4<R, LMAX, Z, G>;
   constexpr int L = 2 * LMAX * (LMAX + 2);
   constexpr int NQ = 2 * LMAX + 1;
   constexpr int NM = Cop4Max<LMAX>::n;
+  constexpr int NR = Cop4Max<LMAX>::nr;
   constexpr int n = S::n;
+  constexpr int nr = S::nr;
   double* s_px = reinterpret_cast<double*>(smem_raw);
   double* s_py = s_px + SS;
   R* s_x = reinterpret_cast<R*>(s_py + SS);          // [source][2 n] complex: own slots then partner slots
-  R* s_acc = s_x + SS * 2 * NM * 2;                  // [re/im][2 n][TJ]
-  int* s_sa = reinterpret_cast<int*>(s_acc + 2 * 2 * NM * TJ);
+  R* s_acc = s_x + SS * 2 * NM * 2;                  // [re/im][2 nr][TJ]: the group's own rows, then their partner share
+  int* s_sa = reinterpret_cast<int*>(s_acc + 2 * 2 * NR * TJ);
   int* s_sb = s_sa + 2 * NM;
   int* s_ss = s_sb + 2 * NM;
   const int tid = threadIdx.x;
@@ -499,9 +505,9 @@ __device__ __forceinline__ void cop4_sector(const double* __restrict__ pos, cons
     s_sa[tid] = a; s_sb[tid] = b; s_ss[tid] = sg;
   }
   R* ar = s_acc + tid;
-  R* ai = s_acc + 2 * NM * TJ + tid;
+  R* ai = s_acc + 2 * NR * TJ + tid;
 #pragma unroll
-  for (int b = 0; b < 2 * n; ++b) { ar[b * TJ] = R(0); ai[b * TJ] = R(0); }
+  for (int b = 0; b < 2 * nr; ++b) { ar[b * TJ] = R(0); ai[b * TJ] = R(0); }
   for (int s0 = c0; s0 < c1; s0 += SS) {
     const int ns = min(SS, c1 - s0);
     __syncthreads();
@@ -547,6 +553,16 @@ __device__ __forceinline__ void cop4_sector(const double* __restrict__ pos, cons
   }
 }
 
+// blockIdx.z = z * NG + g (sector-major, slowest grid dimension: co-resident blocks run the same code)
+template <typename R, int LMAX, int ZG, int TJ, int SS>
+__device__ __forceinline__ void cop4_dispatch(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
+                                              const TmTile tile, int n_scat, double k_over_pi, double inv_k, TmShift shift,
+                                              unsigned char* smem_raw) {
+  constexpr int NG = Cop4Max<LMAX>::ng;
+  if (blockIdx.z == ZG) cop4_sector<R, LMAX, ZG / NG, ZG % NG, TJ, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, shift, smem_raw);
+  else if constexpr (ZG + 1 < 4 * NG) cop4_dispatch<R, LMAX, ZG + 1, TJ, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, shift, smem_raw);
+}
+
 template <typename R, int LMAX, int TJ, int SS>
 __global__ void __launch_bounds__(TJ)
 k_allpairs_coplanar4(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
@@ -555,10 +571,5 @@ k_allpairs_coplanar4(const double* __restrict__ pos, const Cx<R>* __restrict__ x
   if (n_active != nullptr && *n_active == 0) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const TmTile tile = tiles[blockIdx.x];
-  switch (blockIdx.z) {
-    case 0: cop4_sector<R, LMAX, 0, TJ, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, shift, smem_raw); break;
-    case 1: cop4_sector<R, LMAX, 1, TJ, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, shift, smem_raw); break;
-    case 2: cop4_sector<R, LMAX, 2, TJ, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, shift, smem_raw); break;
-    default: cop4_sector<R, LMAX, 3, TJ, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, shift, smem_raw); break;
-  }
+  cop4_dispatch<R, LMAX, 0, TJ, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, shift, smem_raw);
 }

@@ -232,7 +232,8 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
   dim3 grid(c->n_tiles, c->n_chunk);
   tick(c, true);
   if (c->kernel == TM_KERNEL_COPLANAR && c->lmax > 3) {
-    grid.z = 4;                                         // (z-mirror parity, y'-mirror sector): slowest grid dimension
+    // (z-mirror parity, y'-mirror sector) x row group: slowest grid dimension
+    grid.z = 4 * (c->lmax == 4 ? Cop4Max<4>::ng : (c->lmax == 5 ? Cop4Max<5>::ng : Cop4Max<6>::ng));
 #define TM_LAUNCH_C4(LM)                                                                                        \
   {                                                                                                             \
     const size_t sm = Cop4Smem<R, LM, COP4_TJ, COP4_SS>::bytes;                                                 \
@@ -570,7 +571,8 @@ int configure_kernel(tm_ctx* ctx) {
   // without a long tail; bounded by 64 chunks, >= 32 sources per chunk and 2 GB of partial sums.
   const long long slots = 148LL * (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj : (want == TM_KERNEL_SYM3D ? 2 : 4));
   const bool cop4 = want == TM_KERNEL_COPLANAR && ctx->lmax > 3;   // four-sector coplanar kernel (lmax 4..6)
-  const long long blocks1 = (long long)ctx->n_tiles * (cop4 ? 4 : (gen ? 2 : 1));
+  const int cop4_z = !cop4 ? 0 : 4 * (ctx->lmax == 4 ? Cop4Max<4>::ng : (ctx->lmax == 5 ? Cop4Max<5>::ng : Cop4Max<6>::ng));
+  const long long blocks1 = (long long)ctx->n_tiles * (cop4 ? cop4_z : (gen ? 2 : 1));
   const int part_mult = (want == TM_KERNEL_SYM3D || cop4) ? 2 : 1;   // one partial buffer per (chunk, y'-sector)
   int max_win = 1;
   for (int w = 0; w < ctx->n_win; ++w) max_win = std::max(max_win, ctx->win_ptr[w + 1] - ctx->win_ptr[w]);
