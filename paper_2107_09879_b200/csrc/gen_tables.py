@@ -590,7 +590,7 @@ def coplanar_sectors(lmax):
     return out
 
 
-COP4_GROUPS = {4: 1, 5: 2, 6: 4}     # row groups per sector: keeps one block's straight-line code near the 32 KB L1.5 I-cache
+COP4_GROUPS = {4: 1, 5: 4, 6: 4}     # row groups per sector: keeps one block's straight-line code near the 32 KB L1.5 I-cache
 
 
 def emit_coplanar4(lmaxes, path):
@@ -716,6 +716,8 @@ def emit_coplanar4(lmaxes, path):
                     f.write("}\n")
             f.write(f"#define TM_COP4_NMAX_L{lmax} {nmax}\n")
             f.write(f"#define TM_COP4_G_L{lmax} {G}\n")
+            for gg in (2, 4, 8):       # TM_COP4_IFn_Lx(code): code if the sector has at least n row groups
+                f.write(f"#define TM_COP4_IF{gg}_L{lmax}(...) {'__VA_ARGS__' if G >= gg else ''}\n")
             f.write(f"#define TM_COP4_NRMAX_L{lmax} {rmax}\n")
             f.write(f"#define TM_COP4_FPINST_L{lmax} {cost[0]}   // FP instructions per ordered pair (all sectors and row groups)\n")
             f.write(f"#define TM_COP4_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")

@@ -457,9 +457,13 @@ template <typename R, int LMAX, int Z, int G> struct Cop4;
     }                                                                                                    \
   };
 #define TM_COP4_SPEC_Z(LM, GG) TM_COP4_SPEC(LM, 0, GG) TM_COP4_SPEC(LM, 1, GG) TM_COP4_SPEC(LM, 2, GG) TM_COP4_SPEC(LM, 3, GG)
-TM_COP4_SPEC_Z(4, 0)
-TM_COP4_SPEC_Z(5, 0) TM_COP4_SPEC_Z(5, 1)
-TM_COP4_SPEC_Z(6, 0) TM_COP4_SPEC_Z(6, 1) TM_COP4_SPEC_Z(6, 2) TM_COP4_SPEC_Z(6, 3)
+#define TM_COP4_SPEC_L(LM)                                                            \
+  TM_COP4_SPEC_Z(LM, 0) TM_COP4_SPEC_G2(LM) TM_COP4_SPEC_G4(LM) TM_COP4_SPEC_G8(LM)
+#define TM_COP4_SPEC_G2(LM) TM_COP4_IF2_L##LM(TM_COP4_SPEC_Z(LM, 1))
+#define TM_COP4_SPEC_G4(LM) TM_COP4_IF4_L##LM(TM_COP4_SPEC_Z(LM, 2) TM_COP4_SPEC_Z(LM, 3))
+#define TM_COP4_SPEC_G8(LM) TM_COP4_IF8_L##LM(TM_COP4_SPEC_Z(LM, 4) TM_COP4_SPEC_Z(LM, 5) TM_COP4_SPEC_Z(LM, 6) TM_COP4_SPEC_Z(LM, 7))
+TM_COP4_SPEC_L(4) TM_COP4_SPEC_L(5) TM_COP4_SPEC_L(6)
+#undef TM_COP4_SPEC_L
 #undef TM_COP4_SPEC_Z
 #undef TM_COP4_SPEC
 

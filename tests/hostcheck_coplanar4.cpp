@@ -36,6 +36,9 @@ SECZ(1)
 #if NGROUPS > 2
 SECZ(2) SECZ(3)
 #endif
+#if NGROUPS > 4
+SECZ(4) SECZ(5) SECZ(6) SECZ(7)
+#endif
 // one (sector, row group) block of the kernel: stage, accumulate the group's rows, unmix into the group's output modes
 template <int Z, int G>
 void run(const C* x, const double* cm, const double* sm, const double* hr, const double* hi, C* u, int L) {
@@ -82,6 +85,10 @@ int main() {
 #endif
 #if NGROUPS > 2
   run_group<2>(x.data(), cm, sm, hr, hi, u.data(), L); run_group<3>(x.data(), cm, sm, hr, hi, u.data(), L);
+#endif
+#if NGROUPS > 4
+  run_group<4>(x.data(), cm, sm, hr, hi, u.data(), L); run_group<5>(x.data(), cm, sm, hr, hi, u.data(), L);
+  run_group<6>(x.data(), cm, sm, hr, hi, u.data(), L); run_group<7>(x.data(), cm, sm, hr, hi, u.data(), L);
 #endif
   for (int i = 0; i < L; ++i) printf("%.17g %.17g\n", u[i].re, u[i].im);
   return 0;
