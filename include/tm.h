@@ -70,7 +70,15 @@ typedef struct { const tm_c64 *p; } tm_coeffs_desc;
 /* GMRES options (reading R13): x0 = 0, restarted GMRES(restart) with CGS2 orthogonalisation on
  * (I - T A) s = T p; stop when ||b - M x|| / ||b|| <= tol per window (true residual, recomputed at every
  * restart and at exit); at most max_iter Arnoldi steps per window. */
-typedef struct { double tol; int restart; int max_iter; } tm_solve_opts;
+typedef struct {
+  double tol;
+  int    restart;
+  int    max_iter;
+  int    warm_start;      /* 0: start from x0 = 0.  1: the output array (s_out / lambda_out) holds an initial guess x0 on
+                             entry - e.g. the solution of the previous optimisation step (the design
+                             changes little between steps); the first residual is b - M x0, the stopping rule still
+                             refers to ||b||.  Costs one extra operator application. */
+} tm_solve_opts;
 
 /* Per-window report. */
 typedef struct {

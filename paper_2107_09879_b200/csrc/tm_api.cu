@@ -347,7 +347,7 @@ cudaError_t store_c64(tm_ctx* c, const Cx<R>* src, tm_c64* dst) {
 // solves the correction equation M d = r for the fp64 residual r in fp32 and adds d to the fp64 iterate.
 template <typename R, typename RX>
 int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_info* info) {
-  // on entry: d_v[1] = right-hand side b; on exit d_v[0] = x.
+  // on entry: d_v[1] = right-hand side b (and, with o.warm_start, d_v[0] = initial guess x0); on exit d_v[0] = x.
   constexpr bool mixed = !std::is_same<R, RX>::value;
   Cx<RX>* X = vec<RX>(ctx, 0); Cx<RX>* B = vec<RX>(ctx, 1); Cx<RX>* ZX = vec<RX>(ctx, 2);
   const size_t n = ctx->n;
@@ -365,7 +365,8 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
   if (!ctx->t0_ev) { TM_CUDA(cudaEventCreate(&ctx->t0_ev)); TM_CUDA(cudaEventCreate(&ctx->t1_ev)); }
   cudaEvent_t e0 = ctx->t0_ev, e1 = ctx->t1_ev;
   TM_CUDA(cudaEventRecord(e0, st));
-  TM_CUDA(cudaMemsetAsync(X, 0, n * sizeof(Cx<RX>), st));
+  const bool warm = o.warm_start != 0;
+  if (!warm) TM_CUDA(cudaMemsetAsync(X, 0, n * sizeof(Cx<RX>), st));
   TM_CUDA(cudaMemsetAsync(V, 0, (size_t)(m + 2) * n * sizeof(Cx<R>), st));   // basis vectors must be finite (k_axpy)
 
   std::vector<int> h_k(nw), h_done(nw), iters(nw, 0), restarts(nw, 0);
@@ -388,6 +389,15 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
     (void)fn;
   }
   const Cx<RX>* resid_vec = B;                        // first cycle: x0 = 0 so r = b
+  if (warm) {                                         // ||b|| is the reference norm; r0 = b - M x0 starts the first cycle
+    k_norm2<RX><<<nc, TM_VT, 0, st>>>(B, ctx->d_chunks, ctx->gm.normpart);
+    k_reduce_norm<<<nw, 64, 0, st>>>(ctx->gm.normpart, ctx->d_win_chunk_ptr, S.bnorm);
+    TM_CUDA(apply_operator<RX>(ctx, transpose, X, RXv, ZX, nullptr));
+    matvecs++;
+    k_scale_or_sub<RX, RX><<<nc, TM_VT, 0, st>>>(B, RXv, nullptr, RXv, ctx->d_chunks, nullptr);
+    ctx->total_launches += 3;
+    resid_vec = RXv;
+  }
   while (true) {
     // beta = ||r|| per window
     k_norm2<RX><<<nc, TM_VT, 0, st>>>(resid_vec, ctx->d_chunks, ctx->gm.normpart);
@@ -416,7 +426,7 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
       if (stagnant >= 2) break;
     }
     TM_CUDA(cudaMemsetAsync(S.n_active, 0, sizeof(int), st));
-    k_gmres_init_cycle<<<wb, 64, 0, st>>>(S, nw, cycle == 0 ? 1 : 0, o.tol);
+    k_gmres_init_cycle<<<wb, 64, 0, st>>>(S, nw, (cycle == 0 && !warm) ? 1 : 0, o.tol);
     k_scale_or_sub<RX, R><<<nc, TM_VT, 0, st>>>(resid_vec, nullptr, S.inv_norm, V, ctx->d_chunks, nullptr);   // V_0 = r / beta
     ctx->total_launches += 4;
     const int mc = std::min(m, o.max_iter - total);
@@ -895,6 +905,7 @@ int solve_typed(tm_ctx* ctx, int adjoint, const tm_c64* w, const tm_solve_opts& 
     TM_CUDA(launch_tapply<R>(ctx, 3, vec<R>(ctx, 2), vec<R>(ctx, 1), nullptr));   // b = T p   (Eq. I25)
     ctx->total_launches++;
   }
+  if (o.warm_start) TM_CUDA(load_c64<R>(ctx, out, vec<R>(ctx, 0)));        // x0 = caller's guess (read from the output array)
   const int rc = gmres_solve<RV, R>(ctx, adjoint ? 1 : 0, o, info);
   if (rc < 0) return rc;
   TM_CUDA(store_c64<R>(ctx, vec<R>(ctx, 0), out));

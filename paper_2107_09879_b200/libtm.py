@@ -46,7 +46,7 @@ class CoeffsDesc(ctypes.Structure):
 
 
 class SolveOpts(ctypes.Structure):
-    _fields_ = [("tol", ctypes.c_double), ("restart", ctypes.c_int), ("max_iter", ctypes.c_int)]
+    _fields_ = [("tol", ctypes.c_double), ("restart", ctypes.c_int), ("max_iter", ctypes.c_int), ("warm_start", ctypes.c_int)]
 
 
 class SolveInfo(ctypes.Structure):
@@ -224,7 +224,7 @@ class Solver:
         return lib().tm_get_kernel(self._h)
 
     def workspace_bytes(self, restart):
-        o = SolveOpts(1e-6, int(restart), 1)
+        o = SolveOpts(1e-6, int(restart), 1, 0)
         return int(lib().tm_workspace_bytes(self._h, ctypes.byref(o)))
 
     def set_workspace(self, tensor):
@@ -247,17 +247,22 @@ class Solver:
         import torch
         return torch.empty((self.n_scat, self.L), dtype=torch.complex128, device=x.device)
 
-    def solve(self, tol, restart, max_iter, out=None):
+    def solve(self, tol, restart, max_iter, out=None, warm_start=False):
+        """warm_start: `out` holds the initial guess on entry (tm_solve_opts.warm_start)."""
+        if warm_start and out is None:
+            raise ValueError("warm_start needs the initial guess in `out`")
         out = np.empty((self.n_scat, self.L), dtype=np.complex128) if out is None else out
-        o = SolveOpts(float(tol), int(restart), int(max_iter))
+        o = SolveOpts(float(tol), int(restart), int(max_iter), 1 if warm_start else 0)
         info = (SolveInfo * self.n_win)()
         rc = self._check(lib().tm_solve(self._h, ctypes.byref(o), _ptr(out), ctypes.addressof(info)))
         return out, list(info), rc
 
-    def solve_adjoint(self, w, tol, restart, max_iter, out=None):
+    def solve_adjoint(self, w, tol, restart, max_iter, out=None, warm_start=False):
         w = np.ascontiguousarray(w, dtype=np.complex128) if isinstance(w, np.ndarray) else w
+        if warm_start and out is None:
+            raise ValueError("warm_start needs the initial guess in `out`")
         out = self._like(w) if out is None else out
-        o = SolveOpts(float(tol), int(restart), int(max_iter))
+        o = SolveOpts(float(tol), int(restart), int(max_iter), 1 if warm_start else 0)
         info = (SolveInfo * self.n_win)()
         rc = self._check(lib().tm_solve_adjoint(self._h, _ptr(w), ctypes.byref(o), _ptr(out), ctypes.addressof(info)))
         return out, list(info), rc

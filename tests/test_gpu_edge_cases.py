@@ -288,3 +288,38 @@ def test_incident_field_at_detector_points(tm):
     ref = np.array([sum(incident.jinc_field_direct(W.K_B, p, src[i], amp[i, 0], amp[i, 1]) for i in range(3)) for p in pts])
     assert rel(s.fields(pts, None, tm.TM_FIELD_E_INC), ref) <= 1e-7
     s.close()
+
+
+@pytest.mark.parametrize("precision", ["fp64", "mixed"])
+def test_warm_start(tm, precision):
+    """tm_solve_opts.warm_start (optimisation loop): starting from the exact solution takes no Arnoldi
+    step; starting from the solution of a slightly different design takes fewer steps than a cold start and reaches the
+    same solution (oracle: dense LU of the perturbed design); the adjoint solve honours it too."""
+    prec = tm.TM_FP64 if precision == "fp64" else tm.TM_MIXED
+    w = W.cloud_workload(40, seed=11, lmax=2, planar=True)
+    ref = driver.solve(w)
+    s = tm.solver_for_workload(w, precision=prec)
+    cold, ic, rc = s.solve(1e-10, 30, 2000)
+    assert rc == 0 and rel(cold, ref["s"]) <= 1e-9
+    again = cold.copy()
+    again, ia, rc = s.solve(1e-10, 30, 2000, out=again, warm_start=True)
+    assert rc == 0 and ia[0].iterations == 0 and ia[0].rel_residual <= 1e-10 and rel(again, ref["s"]) <= 1e-9
+    # design step: every radius grows by 0.5 %
+    w2 = dict(w)
+    w2["radii"] = np.asarray(w["radii"]) * 1.005
+    ref2 = driver.solve(w2)
+    T2 = np.stack([tm.mie_tmatrix(w["lmax"], w["k"], r, w["eps_r"]) for r in w2["radii"]])
+    s.set_tmatrices(T2, np.asarray(w["type_of"], dtype=np.int32), True)
+    cold2, ic2, rc = s.solve(1e-10, 30, 2000)
+    assert rc == 0 and rel(cold2, ref2["s"]) <= 1e-9
+    warm2 = cold.copy()
+    warm2, iw2, rc = s.solve(1e-10, 30, 2000, out=warm2, warm_start=True)
+    assert rc == 0 and rel(warm2, ref2["s"]) <= 1e-9
+    assert iw2[0].iterations < ic2[0].iterations
+    # adjoint
+    wv = rand_x(cold.shape, 5)
+    lam, il, rc = s.solve_adjoint(wv, 1e-10, 30, 2000)
+    lam2 = lam.copy()
+    lam2, il2, rc2 = s.solve_adjoint(wv, 1e-10, 30, 2000, out=lam2, warm_start=True)
+    assert rc == 0 and rc2 == 0 and il2[0].iterations == 0 and rel(lam2, lam) <= 1e-9
+    s.close()
