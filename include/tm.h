@@ -204,6 +204,13 @@ int tm_measure_fma_peak(int precision, double *tflops, void *cuda_stream);
  * T_{l,p=0} = -b_l, T_{l,p=1} = -a_l), out[L] in flat mode order.  eps_r complex relative permittivity. */
 int tm_mie_tmatrix(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64 *out);
 
+/* Memory (the solver state is what limits the problem size on one GPU).  All device memory of the
+ * library comes from the current device's stream-ordered pool (cudaMallocAsync) with the release threshold raised, so a
+ * context created and destroyed once per optimisation step re-uses the same physical memory.  This call hands the cached,
+ * unused memory back to the driver (e.g. before another library needs it); live contexts are not affected.
+ * Returns TM_OK or TM_E_CUDA. */
+int tm_release_cached_memory(void);
+
 int tm_num_modes(int lmax);                    /* L = 2 lmax (lmax + 2) */
 const char *tm_last_error(const tm_ctx *ctx);  /* ctx may be NULL: last error of tm_create */
 void tm_destroy(tm_ctx *ctx);

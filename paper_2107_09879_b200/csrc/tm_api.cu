@@ -24,6 +24,39 @@ namespace {
 
 std::string g_create_error;
 
+// Device memory comes from the device's stream-ordered pool with an unlimited release threshold: a context that is
+// created and destroyed once per step (an optimisation loop, the end-to-end bench leg) gets the same physical memory
+// back instead of paying the driver's map / unmap on every cudaMalloc / cudaFree (measured: 1-60 ms per call, at
+// random).  tm_release_cached_memory() returns the cached memory to the driver.
+template <typename T>
+cudaError_t tm_dev_alloc(T** p, size_t bytes) {
+  *p = nullptr;
+  if (bytes == 0) return cudaSuccess;
+  static bool pool_set[64] = {};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev >= 0 && dev < 64 && !pool_set[dev]) {
+    cudaMemPool_t pool;
+    unsigned long long keep = ~0ULL;
+    if ((e = cudaDeviceGetDefaultMemPool(&pool, dev)) != cudaSuccess) return e;
+    if ((e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep)) != cudaSuccess) return e;
+    pool_set[dev] = true;
+  }
+  void* q = nullptr;
+  if ((e = cudaMallocAsync(&q, bytes, (cudaStream_t)0)) != cudaSuccess) return e;
+  *p = static_cast<T*>(q);
+  return cudaStreamSynchronize((cudaStream_t)0);      // usable from any stream on return
+}
+
+// Like cudaFree: every kernel that may still use the block has finished before it goes back to the pool.
+inline cudaError_t tm_dev_free(void* p) {
+  if (!p) return cudaSuccess;
+  cudaError_t e = cudaDeviceSynchronize();
+  const cudaError_t f = cudaFreeAsync(p, (cudaStream_t)0);
+  return e != cudaSuccess ? e : f;
+}
+
 constexpr int COP_SS = 64;       // coplanar kernel: sources per shared-memory stage
 constexpr int SYM3D_TJ = 128;    // generated 3-D kernel: targets per block
 constexpr int SYM3D_SS = 32;     // generated 3-D kernel: sources per stage
@@ -132,10 +165,10 @@ cudaError_t copy_out(void* dst, const void* src_dev, size_t bytes, cudaStream_t 
 // Device scratch slot `i` of at least `bytes` bytes (grown on demand, freed in tm_destroy).
 cudaError_t scratch_get(tm_ctx* c, int i, size_t bytes, void** out) {
   if (c->scratch_cap[i] < bytes) {
-    if (c->scratch[i]) cudaFree(c->scratch[i]);
+    if (c->scratch[i]) tm_dev_free(c->scratch[i]);
     c->scratch[i] = nullptr; c->scratch_cap[i] = 0;
     const size_t cap = bytes + bytes / 4 + 256;
-    cudaError_t e = cudaMalloc(&c->scratch[i], cap);
+    cudaError_t e = tm_dev_alloc(&c->scratch[i], cap);
     if (e != cudaSuccess) return e;
     c->scratch_cap[i] = cap;
   }
@@ -596,15 +629,15 @@ int configure_kernel(tm_ctx* ctx) {
     if (cost < best * 0.995) { best = cost; nchunk = cnd; }
   }
   ctx->n_chunk = (int)std::max<long long>(1, nchunk);
-  if (ctx->d_tiles) cudaFree(ctx->d_tiles);
-  TM_CUDA(cudaMalloc(&ctx->d_tiles, tiles.size() * sizeof(TmTile)));
+  if (ctx->d_tiles) tm_dev_free(ctx->d_tiles);
+  TM_CUDA(tm_dev_alloc(&ctx->d_tiles, tiles.size() * sizeof(TmTile)));
   TM_CUDA(cudaMemcpy(ctx->d_tiles, tiles.data(), tiles.size() * sizeof(TmTile), cudaMemcpyHostToDevice));
   ctx->n_part = ctx->n_chunk * part_mult;
   const size_t need = (size_t)ctx->n_part * vec_bytes;
   if (need > ctx->upart_bytes) {
-    if (ctx->d_upart) cudaFree(ctx->d_upart);
+    if (ctx->d_upart) tm_dev_free(ctx->d_upart);
     ctx->d_upart = nullptr; ctx->upart_bytes = 0;
-    TM_CUDA(cudaMalloc(&ctx->d_upart, need));
+    TM_CUDA(tm_dev_alloc(&ctx->d_upart, need));
     ctx->upart_bytes = need;
   }
   return TM_OK;
@@ -612,7 +645,7 @@ int configure_kernel(tm_ctx* ctx) {
 
 int ensure_gmres(tm_ctx* ctx, int restart) {
   if (ctx->gm.restart >= restart && ctx->gm.blob) { ctx->gm.dev.ldh = restart + 1; ctx->gm.dev.m = restart; return TM_OK; }
-  if (ctx->gm.blob) cudaFree(ctx->gm.blob);
+  if (ctx->gm.blob) tm_dev_free(ctx->gm.blob);
   ctx->gm = Gmres{};
   const size_t nw = ctx->n_win, ldh = restart + 1, m = restart, nc = ctx->n_chunks;
   size_t off = 0;
@@ -621,7 +654,7 @@ int ensure_gmres(tm_ctx* ctx, int restart) {
                o_sn = take(nw * m * 16), o_g = take(nw * ldh * 16), o_y = take(nw * ldh * 16), o_nw = take(nw * 8),
                o_bn = take(nw * 8), o_in = take(nw * 8), o_b0 = take(nw * 8), o_rs = take(nw * 8), o_k = take(nw * 4), o_d = take(nw * 4),
                o_na = take(4), o_part = take(ldh * nc * 16), o_np = take(nc * 8);
-  TM_CUDA(cudaMalloc(&ctx->gm.blob, off));
+  TM_CUDA(tm_dev_alloc(&ctx->gm.blob, off));
   TM_CUDA(cudaMemset(ctx->gm.blob, 0, off));
   char* b = reinterpret_cast<char*>(ctx->gm.blob);
   TmGmresDev& S = ctx->gm.dev;
@@ -645,9 +678,9 @@ int ensure_workspace(tm_ctx* ctx, int restart) {
   const size_t need = ws_bytes_for(ctx, restart);
   if (ctx->ws && ctx->ws_bytes >= need) return TM_OK;
   if (ctx->ws && !ctx->ws_owned) return fail(ctx, TM_E_NOMEM, "caller workspace too small: see tm_workspace_bytes");
-  if (ctx->ws) cudaFree(ctx->ws);
+  if (ctx->ws) tm_dev_free(ctx->ws);
   ctx->ws = nullptr; ctx->ws_bytes = 0;
-  TM_CUDA(cudaMalloc(&ctx->ws, need));
+  TM_CUDA(tm_dev_alloc(&ctx->ws, need));
   ctx->ws_bytes = need; ctx->ws_owned = true;
   return TM_OK;
 }
@@ -671,18 +704,18 @@ const char* tm_last_error(const tm_ctx* ctx) { return ctx ? ctx->err.c_str() : g
 void tm_destroy(tm_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
-  cudaFree(c->d_pos); cudaFree(c->d_win_of); cudaFree(c->d_type_of); cudaFree(c->d_T); cudaFree(c->d_T32); cudaFree(c->d_p);
-  cudaFree(c->d_const); cudaFree(c->d_rowptr); cudaFree(c->d_col); cudaFree(c->d_widx); cudaFree(c->d_imag);
-  cudaFree(c->d_coef); cudaFree(c->d_tiles); cudaFree(c->d_upart); cudaFree(c->d_chunks); cudaFree(c->d_win_chunk_ptr);
-  for (int i = 0; i < 3; ++i) cudaFree(c->d_v[i]);
-  cudaFree(c->d_io);
-  if (c->ws_owned) cudaFree(c->ws);
-  cudaFree(c->gm.blob);
+  tm_dev_free(c->d_pos); tm_dev_free(c->d_win_of); tm_dev_free(c->d_type_of); tm_dev_free(c->d_T); tm_dev_free(c->d_T32); tm_dev_free(c->d_p);
+  tm_dev_free(c->d_const); tm_dev_free(c->d_rowptr); tm_dev_free(c->d_col); tm_dev_free(c->d_widx); tm_dev_free(c->d_imag);
+  tm_dev_free(c->d_coef); tm_dev_free(c->d_tiles); tm_dev_free(c->d_upart); tm_dev_free(c->d_chunks); tm_dev_free(c->d_win_chunk_ptr);
+  for (int i = 0; i < 3; ++i) tm_dev_free(c->d_v[i]);
+  tm_dev_free(c->d_io);
+  if (c->ws_owned) tm_dev_free(c->ws);
+  tm_dev_free(c->gm.blob);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
   if (c->sync_ev) cudaEventDestroy(c->sync_ev);
   if (c->t0_ev) cudaEventDestroy(c->t0_ev);
   if (c->t1_ev) cudaEventDestroy(c->t1_ev);
-  for (int i = 0; i < 8; ++i) cudaFree(c->scratch[i]);
+  for (int i = 0; i < 8; ++i) tm_dev_free(c->scratch[i]);
   delete c;
 }
 
@@ -739,15 +772,15 @@ int tm_create(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const 
       return code_;                                                                           \
     }                                                                                         \
   } while (0)
-  TM_CREATE_CUDA(cudaMalloc(&c->d_pos, hpos.size() * sizeof(double)));
+  TM_CREATE_CUDA(tm_dev_alloc(&c->d_pos, hpos.size() * sizeof(double)));
   TM_CREATE_CUDA(cudaMemcpy(c->d_pos, hpos.data(), hpos.size() * sizeof(double), cudaMemcpyHostToDevice));
   std::vector<int> win_of(n_scat);
   for (int w = 0; w < n_win; ++w) for (int i = wp[w]; i < wp[w + 1]; ++i) win_of[i] = w;
-  TM_CREATE_CUDA(cudaMalloc(&c->d_win_of, n_scat * sizeof(int)));
+  TM_CREATE_CUDA(tm_dev_alloc(&c->d_win_of, n_scat * sizeof(int)));
   TM_CREATE_CUDA(cudaMemcpy(c->d_win_of, win_of.data(), n_scat * sizeof(int), cudaMemcpyHostToDevice));
-  TM_CREATE_CUDA(cudaMalloc(&c->d_type_of, n_scat * sizeof(int)));
+  TM_CREATE_CUDA(tm_dev_alloc(&c->d_type_of, n_scat * sizeof(int)));
   fill_const(c);
-  TM_CREATE_CUDA(cudaMalloc(&c->d_const, sizeof(TmConst)));
+  TM_CREATE_CUDA(tm_dev_alloc(&c->d_const, sizeof(TmConst)));
   TM_CREATE_CUDA(cudaMemcpy(c->d_const, &c->h_const, sizeof(TmConst), cudaMemcpyHostToDevice));
   {   // general-kernel term table of this lmax
     const TmTermTable& t = tm_term_tables[lmax - 1];
@@ -762,12 +795,12 @@ int tm_create(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const 
         imag[q] = t.ipow[q] & 1;
         coef[q] = (t.ipow[q] & 2) ? -t.val[q] : t.val[q];
       }
-    TM_CREATE_CUDA(cudaMalloc(&c->d_rowptr, (L + 1) * sizeof(int)));
+    TM_CREATE_CUDA(tm_dev_alloc(&c->d_rowptr, (L + 1) * sizeof(int)));
     TM_CREATE_CUDA(cudaMemcpy(c->d_rowptr, t.row_ptr, (L + 1) * sizeof(int), cudaMemcpyHostToDevice));
-    TM_CREATE_CUDA(cudaMalloc(&c->d_col, nt)); TM_CREATE_CUDA(cudaMemcpy(c->d_col, t.col, nt, cudaMemcpyHostToDevice));
-    TM_CREATE_CUDA(cudaMalloc(&c->d_widx, nt)); TM_CREATE_CUDA(cudaMemcpy(c->d_widx, widx.data(), nt, cudaMemcpyHostToDevice));
-    TM_CREATE_CUDA(cudaMalloc(&c->d_imag, nt)); TM_CREATE_CUDA(cudaMemcpy(c->d_imag, imag.data(), nt, cudaMemcpyHostToDevice));
-    TM_CREATE_CUDA(cudaMalloc(&c->d_coef, nt * sizeof(double)));
+    TM_CREATE_CUDA(tm_dev_alloc(&c->d_col, nt)); TM_CREATE_CUDA(cudaMemcpy(c->d_col, t.col, nt, cudaMemcpyHostToDevice));
+    TM_CREATE_CUDA(tm_dev_alloc(&c->d_widx, nt)); TM_CREATE_CUDA(cudaMemcpy(c->d_widx, widx.data(), nt, cudaMemcpyHostToDevice));
+    TM_CREATE_CUDA(tm_dev_alloc(&c->d_imag, nt)); TM_CREATE_CUDA(cudaMemcpy(c->d_imag, imag.data(), nt, cudaMemcpyHostToDevice));
+    TM_CREATE_CUDA(tm_dev_alloc(&c->d_coef, nt * sizeof(double)));
     TM_CREATE_CUDA(cudaMemcpy(c->d_coef, coef.data(), nt * sizeof(double), cudaMemcpyHostToDevice));
   }
   {   // vector chunks: every chunk inside one window
@@ -783,23 +816,23 @@ int tm_create(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const 
     }
     if (c->n > (size_t)0x7fffffff) { g_create_error = "problem too large (n_scat * L must fit in int32)"; tm_destroy(c); return TM_E_INVALID; }
     c->n_chunks = (int)ch.size();
-    TM_CREATE_CUDA(cudaMalloc(&c->d_chunks, ch.size() * sizeof(TmChunk)));
+    TM_CREATE_CUDA(tm_dev_alloc(&c->d_chunks, ch.size() * sizeof(TmChunk)));
     TM_CREATE_CUDA(cudaMemcpy(c->d_chunks, ch.data(), ch.size() * sizeof(TmChunk), cudaMemcpyHostToDevice));
-    TM_CREATE_CUDA(cudaMalloc(&c->d_win_chunk_ptr, (n_win + 1) * sizeof(int)));
+    TM_CREATE_CUDA(tm_dev_alloc(&c->d_win_chunk_ptr, (n_win + 1) * sizeof(int)));
     TM_CREATE_CUDA(cudaMemcpy(c->d_win_chunk_ptr, wcp.data(), (n_win + 1) * sizeof(int), cudaMemcpyHostToDevice));
   }
-  for (int i = 0; i < 3; ++i) TM_CREATE_CUDA(cudaMalloc(&c->d_v[i], c->n * elem_bytes(c)));
-  TM_CREATE_CUDA(cudaMalloc(&c->d_io, c->n * sizeof(double2)));
-  TM_CREATE_CUDA(cudaMalloc(&c->d_p, c->n * sizeof(double2)));
+  for (int i = 0; i < 3; ++i) TM_CREATE_CUDA(tm_dev_alloc(&c->d_v[i], c->n * elem_bytes(c)));
+  TM_CREATE_CUDA(tm_dev_alloc(&c->d_io, c->n * sizeof(double2)));
+  TM_CREATE_CUDA(tm_dev_alloc(&c->d_p, c->n * sizeof(double2)));
   {   // coincident centres are always an error (h_q diverges)
     int* d_flag = nullptr; int* d_wp = nullptr; int h_flag = 0;
-    TM_CREATE_CUDA(cudaMalloc(&d_flag, sizeof(int)));
+    TM_CREATE_CUDA(tm_dev_alloc(&d_flag, sizeof(int)));
     TM_CREATE_CUDA(cudaMemset(d_flag, 0, sizeof(int)));
-    TM_CREATE_CUDA(cudaMalloc(&d_wp, (n_win + 1) * sizeof(int)));
+    TM_CREATE_CUDA(tm_dev_alloc(&d_wp, (n_win + 1) * sizeof(int)));
     TM_CREATE_CUDA(cudaMemcpy(d_wp, wp.data(), (n_win + 1) * sizeof(int), cudaMemcpyHostToDevice));
     k_check_overlap<<<(n_scat + 127) / 128, 128>>>(c->d_pos, c->d_win_of, d_wp, nullptr, nullptr, n_scat, d_flag);
     cudaError_t e = cudaMemcpy(&h_flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost);
-    cudaFree(d_flag); cudaFree(d_wp);
+    tm_dev_free(d_flag); tm_dev_free(d_wp);
     TM_CREATE_CUDA(e);
     if (h_flag) { g_create_error = "two scatterers of one window share a centre"; tm_destroy(c); return TM_E_INVALID; }
   }
@@ -835,7 +868,7 @@ int tm_set_workspace(tm_ctx* ctx, void* dev_ptr, size_t bytes) {
   if (dev_ptr && (!is_device_ptr(dev_ptr) || (reinterpret_cast<uintptr_t>(dev_ptr) & 255)))
     return fail(ctx, TM_E_INVALID, "workspace must be 256-byte aligned device memory");
   TM_CUDA(stream_wait(ctx));
-  if (ctx->ws && ctx->ws_owned) cudaFree(ctx->ws);
+  if (ctx->ws && ctx->ws_owned) tm_dev_free(ctx->ws);
   ctx->ws = dev_ptr; ctx->ws_bytes = dev_ptr ? bytes : 0; ctx->ws_owned = false;
   return TM_OK;
 }
@@ -873,7 +906,7 @@ template <typename R>
 int set_T_typed(tm_ctx* ctx, size_t count, const tm_c64* T, void* dst) {
   // stage fp64 -> Cx<R>
   double2* tmp = nullptr;
-  TM_CUDA(cudaMalloc(&tmp, count * sizeof(double2)));
+  TM_CUDA(tm_dev_alloc(&tmp, count * sizeof(double2)));
   cudaError_t e = copy_in(tmp, T, count * sizeof(double2), ctx->stream);
   if (e == cudaSuccess) {
     k_from_c64<R><<<grid_for(count, 256), 256, 0, ctx->stream>>>(reinterpret_cast<const double*>(tmp),
@@ -881,7 +914,7 @@ int set_T_typed(tm_ctx* ctx, size_t count, const tm_c64* T, void* dst) {
     e = cudaGetLastError();
   }
   if (e == cudaSuccess) e = stream_wait(ctx);
-  cudaFree(tmp);
+  tm_dev_free(tmp);
   TM_CUDA(e);
   return TM_OK;
 }
@@ -928,36 +961,36 @@ int tm_set_tmatrices(tm_ctx* ctx, int n_types, int diag_only, const tm_c64* T, c
     for (int t = 0; t < n_types; ++t)
       if (!(r_enclosing[t] >= 0.0)) return fail(ctx, TM_E_INVALID, "negative enclosing radius");
     int *d_flag = nullptr, *d_wp = nullptr, *d_ty = nullptr; double* d_r = nullptr; int h_flag = 0;
-    cudaError_t e = cudaMalloc(&d_flag, sizeof(int));
+    cudaError_t e = tm_dev_alloc(&d_flag, sizeof(int));
     if (e == cudaSuccess) e = cudaMemset(d_flag, 0, sizeof(int));
-    if (e == cudaSuccess) e = cudaMalloc(&d_wp, (ctx->n_win + 1) * sizeof(int));
+    if (e == cudaSuccess) e = tm_dev_alloc(&d_wp, (ctx->n_win + 1) * sizeof(int));
     if (e == cudaSuccess) e = cudaMemcpy(d_wp, ctx->win_ptr.data(), (ctx->n_win + 1) * sizeof(int), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMalloc(&d_ty, ht.size() * sizeof(int));
+    if (e == cudaSuccess) e = tm_dev_alloc(&d_ty, ht.size() * sizeof(int));
     if (e == cudaSuccess) e = cudaMemcpy(d_ty, ht.data(), ht.size() * sizeof(int), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMalloc(&d_r, n_types * sizeof(double));
+    if (e == cudaSuccess) e = tm_dev_alloc(&d_r, n_types * sizeof(double));
     if (e == cudaSuccess) e = cudaMemcpy(d_r, r_enclosing, n_types * sizeof(double), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) {
       k_check_overlap<<<(ctx->n_scat + 127) / 128, 128>>>(ctx->d_pos, ctx->d_win_of, d_wp, d_ty, d_r, ctx->n_scat, d_flag);
       e = cudaMemcpy(&h_flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost);
     }
-    cudaFree(d_flag); cudaFree(d_wp); cudaFree(d_ty); cudaFree(d_r);
+    tm_dev_free(d_flag); tm_dev_free(d_wp); tm_dev_free(d_ty); tm_dev_free(d_r);
     TM_CUDA(e);
     if (h_flag) return fail(ctx, TM_E_OVERLAP, "enclosing spheres of two scatterers intersect (PAPER.md:275)");
   }
   const size_t count = (size_t)n_types * ctx->L * (diag_only ? 1 : ctx->L);
   void* newT = nullptr;
-  TM_CUDA(cudaMalloc(&newT, count * elem_bytes(ctx)));
+  TM_CUDA(tm_dev_alloc(&newT, count * elem_bytes(ctx)));
   void* oldT = ctx->d_T;
   ctx->d_T = newT;
   int rc = ctx->precision != TM_FP32 ? set_T_typed<double>(ctx, count, T, newT) : set_T_typed<float>(ctx, count, T, newT);
   if (rc == TM_OK && ctx->precision == TM_MIXED) {            // fp32 copy for the inner Krylov cycles
     void* new32 = nullptr;
-    if (cudaMalloc(&new32, count * sizeof(Cx<float>)) != cudaSuccess) rc = fail(ctx, TM_E_NOMEM, "cudaMalloc(T fp32)");
-    else if ((rc = set_T_typed<float>(ctx, count, T, new32)) == TM_OK) { cudaFree(ctx->d_T32); ctx->d_T32 = new32; }
-    else cudaFree(new32);
+    if (tm_dev_alloc(&new32, count * sizeof(Cx<float>)) != cudaSuccess) rc = fail(ctx, TM_E_NOMEM, "tm_dev_alloc(T fp32)");
+    else if ((rc = set_T_typed<float>(ctx, count, T, new32)) == TM_OK) { tm_dev_free(ctx->d_T32); ctx->d_T32 = new32; }
+    else tm_dev_free(new32);
   }
-  if (rc != TM_OK) { cudaFree(newT); ctx->d_T = oldT; return rc; }
-  cudaFree(oldT);
+  if (rc != TM_OK) { tm_dev_free(newT); ctx->d_T = oldT; return rc; }
+  tm_dev_free(oldT);
   TM_CUDA(cudaMemcpy(ctx->d_type_of, ht.data(), ht.size() * sizeof(int), cudaMemcpyHostToDevice));
   ctx->n_types = n_types; ctx->diag = diag_only ? 1 : 0; ctx->has_T = true;
   return TM_OK;
@@ -1053,12 +1086,12 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
     for (int q = 0; q < nb; ++q) { beta[q] = 0.5 * bmax * (xg[q] + 1.0); wq[q] = 0.5 * bmax * wg[q]; }
     double *d_beta = nullptr, *d_wq = nullptr, *d_src = nullptr; double2* d_amp = nullptr; int* d_ptr = nullptr; void* d_nodes = nullptr;
     const size_t node_bytes = sizeof(GaussNode<TM_MAX_LMAX>);      // upper bound for every lmax
-    cudaError_t e = cudaMalloc(&d_beta, nb * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc(&d_wq, nb * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc(&d_src, std::max<size_t>(1, nsrc) * 3 * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc(&d_amp, std::max<size_t>(1, nsrc) * 2 * sizeof(double2));
-    if (e == cudaSuccess) e = cudaMalloc(&d_ptr, (ctx->n_win + 1) * sizeof(int));
-    if (e == cudaSuccess) e = cudaMalloc(&d_nodes, nb * node_bytes);
+    cudaError_t e = tm_dev_alloc(&d_beta, nb * sizeof(double));
+    if (e == cudaSuccess) e = tm_dev_alloc(&d_wq, nb * sizeof(double));
+    if (e == cudaSuccess) e = tm_dev_alloc(&d_src, std::max<size_t>(1, nsrc) * 3 * sizeof(double));
+    if (e == cudaSuccess) e = tm_dev_alloc(&d_amp, std::max<size_t>(1, nsrc) * 2 * sizeof(double2));
+    if (e == cudaSuccess) e = tm_dev_alloc(&d_ptr, (ctx->n_win + 1) * sizeof(int));
+    if (e == cudaSuccess) e = tm_dev_alloc(&d_nodes, nb * node_bytes);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_beta, beta.data(), nb * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_wq, wq.data(), nb * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess && nsrc) e = cudaMemcpyAsync(d_src, hsrc.data(), nsrc * 3 * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
@@ -1082,7 +1115,7 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
       e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = stream_wait(ctx);   // the host vectors above must outlive the copies
-    cudaFree(d_beta); cudaFree(d_wq); cudaFree(d_src); cudaFree(d_amp); cudaFree(d_ptr); cudaFree(d_nodes);
+    tm_dev_free(d_beta); tm_dev_free(d_wq); tm_dev_free(d_src); tm_dev_free(d_amp); tm_dev_free(d_ptr); tm_dev_free(d_nodes);
     TM_CUDA(e);
   } else {
     return fail(ctx, TM_E_INVALID, "unknown incident kind");
@@ -1219,9 +1252,9 @@ int tm_grad_tmatrix(tm_ctx* ctx, const tm_c64* dT, const tm_c64* lambda, const t
   if (!ctx->has_T || !ctx->has_inc) return fail(ctx, TM_E_STATE, "tm_set_tmatrices and tm_set_incident must be called first");
   const size_t count = (size_t)ctx->n_types * ctx->L * (ctx->diag ? 1 : ctx->L);
   void* d_dT = nullptr; double2* d_tmp = nullptr; double2* d_out = nullptr;
-  cudaError_t e = cudaMalloc(&d_dT, count * elem_bytes(ctx));
-  if (e == cudaSuccess) e = cudaMalloc(&d_tmp, count * sizeof(double2));
-  if (e == cudaSuccess) e = cudaMalloc(&d_out, (size_t)ctx->n_scat * sizeof(double2));
+  cudaError_t e = tm_dev_alloc(&d_dT, count * elem_bytes(ctx));
+  if (e == cudaSuccess) e = tm_dev_alloc(&d_tmp, count * sizeof(double2));
+  if (e == cudaSuccess) e = tm_dev_alloc(&d_out, (size_t)ctx->n_scat * sizeof(double2));
   if (e == cudaSuccess) e = copy_in(d_tmp, dT, count * sizeof(double2), ctx->stream);
   const bool f64 = ctx->precision != TM_FP32;
   if (e == cudaSuccess) {
@@ -1245,7 +1278,7 @@ int tm_grad_tmatrix(tm_ctx* ctx, const tm_c64* dT, const tm_c64* lambda, const t
   }
   if (e == cudaSuccess) e = copy_out(out, d_out, (size_t)ctx->n_scat * sizeof(double2), ctx->stream);
   if (e == cudaSuccess) e = stream_wait(ctx);
-  cudaFree(d_dT); cudaFree(d_tmp); cudaFree(d_out);
+  tm_dev_free(d_dT); tm_dev_free(d_tmp); tm_dev_free(d_out);
   TM_CUDA(e);
   return TM_OK;
 }
@@ -1260,9 +1293,9 @@ int grad_positions_typed(tm_ctx* ctx, const tm_c64* lambda, const tm_c64* s, con
   const int L = ctx->L, N = ctx->n_scat;
   Cx<R>*S = vec<R>(ctx, 0), *Y = vec<R>(ctx, 1), *LAM = vec<R>(ctx, 2);
   Cx<R>*PMU = nullptr, *D = nullptr; double2 *d_out = nullptr, *d_dp = nullptr;
-  auto cleanup = [&]() { cudaFree(PMU); cudaFree(D); cudaFree(d_out); cudaFree(d_dp); ctx->shift = TmShift{0.0, 0.0, 0.0, 0}; };
+  auto cleanup = [&]() { tm_dev_free(PMU); tm_dev_free(D); tm_dev_free(d_out); tm_dev_free(d_dp); ctx->shift = TmShift{0.0, 0.0, 0.0, 0}; };
 #define TM_G(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { cleanup(); return fail(ctx, TM_E_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); } } while (0)
-  TM_G(cudaMalloc(&PMU, vb)); TM_G(cudaMalloc(&D, vb)); TM_G(cudaMalloc(&d_out, (size_t)N * 3 * sizeof(double2)));
+  TM_G(tm_dev_alloc(&PMU, vb)); TM_G(tm_dev_alloc(&D, vb)); TM_G(tm_dev_alloc(&d_out, (size_t)N * 3 * sizeof(double2)));
   TM_G(cudaMemsetAsync(d_out, 0, (size_t)N * 3 * sizeof(double2), ctx->stream));
   TM_G(load_c64<R>(ctx, s, S));
   TM_G(load_c64<R>(ctx, lambda, LAM));
@@ -1287,7 +1320,7 @@ int grad_positions_typed(tm_ctx* ctx, const tm_c64* lambda, const tm_c64* s, con
   }
   ctx->shift = TmShift{0.0, 0.0, 0.0, 0};
   if (dp) {                                                          // incident part: mu_j^T dp_j[alpha]
-    TM_G(cudaMalloc(&d_dp, n * 3 * sizeof(double2)));
+    TM_G(tm_dev_alloc(&d_dp, n * 3 * sizeof(double2)));
     TM_G(copy_in(d_dp, dp, n * 3 * sizeof(double2), ctx->stream));
     for (int alpha = 0; alpha < 3; ++alpha)
       k_bilinear_rows<R, double><<<gb, 128, 0, ctx->stream>>>(L, N, PMU, reinterpret_cast<const Cx<double>*>(d_dp) + (size_t)alpha * L,
@@ -1398,7 +1431,7 @@ __global__ void __launch_bounds__(256) k_fma_peak(R* out, int iters, R a, R b) {
 template <typename R>
 int fma_peak_typed(double* tflops, cudaStream_t st) {
   R* d = nullptr;
-  if (cudaMalloc(&d, sizeof(R)) != cudaSuccess) return TM_E_CUDA;
+  if (tm_dev_alloc(&d, sizeof(R)) != cudaSuccess) return TM_E_CUDA;
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0); cudaEventCreate(&e1);
   const int blocks = 148 * 8, iters = 4096;
@@ -1407,13 +1440,13 @@ int fma_peak_typed(double* tflops, cudaStream_t st) {
     cudaEventRecord(e0, st);
     k_fma_peak<R><<<blocks, 256, 0, st>>>(d, iters, R(0.999999), R(1e-7));
     cudaEventRecord(e1, st);
-    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return TM_E_CUDA; }
+    if (cudaEventSynchronize(e1) != cudaSuccess) { tm_dev_free(d); return TM_E_CUDA; }
     float ms = 0.f;
     cudaEventElapsedTime(&ms, e0, e1);
     const double fl = 2.0 * 8 * 16 * (double)iters * 256.0 * blocks;
     if (rep > 0) best = std::max(best, fl / (ms * 1e-3) * 1e-12);
   }
-  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+  cudaEventDestroy(e0); cudaEventDestroy(e1); tm_dev_free(d);
   *tflops = best;
   return TM_OK;
 }
@@ -1440,6 +1473,14 @@ int tm_pair_cost(const tm_ctx* ctx, double* fp_instructions, double* flop) {
   if (fp_instructions) *fp_instructions = inst;
   if (flop) *flop = fl;
   return TM_OK;
+}
+
+int tm_release_cached_memory(void) {
+  int dev = 0;
+  cudaMemPool_t pool;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetDefaultMemPool(&pool, dev) != cudaSuccess) return TM_E_CUDA;
+  if (cudaDeviceSynchronize() != cudaSuccess) return TM_E_CUDA;
+  return cudaMemPoolTrimTo(pool, 0) == cudaSuccess ? TM_OK : TM_E_CUDA;
 }
 
 int tm_measure_fma_peak(int precision, double* tflops, void* cuda_stream) {

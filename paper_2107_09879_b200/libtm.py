@@ -21,7 +21,8 @@ TM_KERNEL_AUTO, TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR, TM_KERNEL_SYM3D = 0, 1, 2
 
 EXPORTS = ["tm_create", "tm_set_tmatrices", "tm_set_incident", "tm_get_incident", "tm_solve", "tm_solve_adjoint",
            "tm_matvec", "tm_fields", "tm_workspace_bytes", "tm_set_workspace", "tm_set_kernel", "tm_get_kernel",
-           "tm_kernel_time", "tm_pair_cost", "tm_measure_fma_peak", "tm_grad_tmatrix", "tm_grad_positions", "tm_mie_tmatrix_dR", "tm_mie_tmatrix", "tm_num_modes", "tm_last_error", "tm_destroy"]
+           "tm_kernel_time", "tm_pair_cost", "tm_measure_fma_peak", "tm_grad_tmatrix", "tm_grad_positions", "tm_mie_tmatrix_dR", "tm_mie_tmatrix",
+           "tm_release_cached_memory", "tm_num_modes", "tm_last_error", "tm_destroy"]
 
 
 class c64(ctypes.Structure):
@@ -141,6 +142,13 @@ def measure_fma_peak(precision=TM_FP64, stream=None):
     if rc != TM_OK:
         raise TmError(rc, "tm_measure_fma_peak failed (no CUDA device?)")
     return v.value
+
+
+def release_cached_memory():
+    """Hand the library's cached, unused device memory back to the driver (tm_release_cached_memory)."""
+    rc = lib().tm_release_cached_memory()
+    if rc != TM_OK:
+        raise TmError(rc, "tm_release_cached_memory failed")
 
 
 class Solver:

@@ -38,13 +38,28 @@ def test_num_modes_and_enums(libtm):
         assert m and int(m.group(1)) == getattr(libtm, name), name
 
 
-def test_struct_layouts(libtm):
-    assert ctypes.sizeof(libtm.c64) == 16
-    assert ctypes.sizeof(libtm.PlaneDesc) == 48
-    assert ctypes.sizeof(libtm.SolveOpts) == 16
-    assert ctypes.sizeof(libtm.SolveInfo) == 32
-    assert ctypes.sizeof(libtm.GaussDesc) == 56
-    assert ctypes.sizeof(libtm.JincDesc) == 40
+def test_struct_layouts(libtm, tmp_path):
+    """The ctypes mirrors have the layout the C compiler gives include/tm.h (sizes and the offset of every field)."""
+    import subprocess
+    pairs = [("tm_c64", libtm.c64), ("tm_plane_desc", libtm.PlaneDesc), ("tm_gauss_desc", libtm.GaussDesc),
+             ("tm_jinc_desc", libtm.JincDesc), ("tm_coeffs_desc", libtm.CoeffsDesc), ("tm_solve_opts", libtm.SolveOpts),
+             ("tm_solve_info", libtm.SolveInfo)]
+    lines = ['#include <stddef.h>', '#include <stdio.h>', '#include "tm.h"', "int main(void) {"]
+    for cname, ct in pairs:
+        lines.append(f'  printf("{cname} %zu\\n", sizeof({cname}));')
+        for fname, _ in ct._fields_:
+            lines.append(f'  printf("{cname}.{fname} %zu\\n", offsetof({cname}, {fname}));')
+    lines += ["  return 0;", "}"]
+    src = tmp_path / "layout.c"
+    src.write_text("\n".join(lines))
+    exe = tmp_path / "layout"
+    subprocess.run(["gcc", "-std=c99", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
+    got = dict(l.split() for l in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.splitlines())
+    for cname, ct in pairs:
+        assert int(got[cname]) == ctypes.sizeof(ct), cname
+        for fname, _ in ct._fields_:
+            assert int(got[f"{cname}.{fname}"]) == getattr(ct, fname).offset, f"{cname}.{fname}"
+    assert ctypes.sizeof(libtm.SolveOpts) == 24 and libtm.SolveOpts.warm_start.offset == 16
 
 
 def test_mie_host_helper_lossless_and_argument_checks(libtm):
