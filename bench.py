@@ -192,6 +192,8 @@ def run_ours(args, w, rank, world, local_rank):
     wadj = adjoint_weight(w)
     max_iter = args.max_iter or w["max_iter"]
     tol = args.tol or w["tol"]
+    if args.restart:
+        w["restart"] = args.restart
 
     with torch.cuda.stream(st):
         peak = libtm.measure_fma_peak(prec, st.cuda_stream)
@@ -471,6 +473,7 @@ def main():
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"],
                     help="mixed: GMRES with iterative refinement (fp32 Krylov cycles, fp64 iterate and true residual)")
     ap.add_argument("--max-iter", type=int, default=None)
+    ap.add_argument("--restart", type=int, default=None, help="override the GMRES restart length of the workload (<= 300)")
     ap.add_argument("--tol", type=float, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--clock-interval-ms", type=int, default=250, help="nvidia-smi sampling period during the timed region")
