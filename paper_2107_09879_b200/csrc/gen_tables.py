@@ -249,10 +249,291 @@ def coplanar_sym(lmax):
     return out
 
 
+# ----------------------------------------------------------------------------- coplanar: rotation - axial translation - rotation
+# In the pair frame F' (x' along the pair, z' the layout normal) the translation mixes all m.  In the frame F'' whose z''
+# axis is the pair axis (x'' = -z', y'' = y', z'' = x': F' turned by +90 degrees about y') it is diagonal in m'' (theta = 0:
+# Pbar_q^mu(1) = 0 for mu > 0 in Eq. I16).  The frame change acts on the coefficients of every (l, p) with the same real
+# (2l+1) x (2l+1) matrix Dl, because Phi_{l,m,p} are built from Ybar_{l,m} = Pbar_l^{|m|}(cos theta) e^{i m phi} by
+# coordinate-free operators.  Dl is obtained numerically (40 digits) from its definition
+#   Ybar_{l,m'}(direction in F') = sum_{m''} Dl[m'', m'] Ybar_{l,m''}(same direction in F''),
+# so no phase convention enters; coplanar_axial() asserts K_q = D^-1 Z_q D for every q against coplanar_rows().
+def pbar_general(l, m, x):
+    """Pbar_l^m(x), m >= 0, no Condon-Shortley phase (R2): sqrt((2l+1)/2 (l-m)!/(l+m)!) (1-x^2)^{m/2} d^m P_l/dx^m."""
+    s = mp.mpf(0)
+    for k in range(0, l // 2 + 1):
+        e = l - 2 * k
+        if e - m < 0:
+            continue
+        c = Fraction((-1) ** k * comb(l, k) * comb(2 * l - 2 * k, l), 2 ** l) * Fraction(factorial(e), factorial(e - m))
+        s += mp.mpf(c.numerator) / mp.mpf(c.denominator) * mp.mpf(x) ** (e - m)
+    n2 = Fraction((2 * l + 1) * factorial(l - m), 2 * factorial(l + m))
+    return s * mp.sqrt(1 - mp.mpf(x) ** 2) ** m * mp.sqrt(mp.mpf(n2.numerator) / mp.mpf(n2.denominator))
+
+
+_rot_cache = {}
+
+
+def frame_rotation(l):
+    """Dl (real, (2l+1) x (2l+1), rows m'' = -l..l, columns m' = -l..l) for F' -> F''."""
+    if l in _rot_cache:
+        return _rot_cache[l]
+    N = 2 * l + 1
+    pts = []
+    for i in range(N + 3):          # fixed, well spread directions (golden-angle spiral)
+        z = mp.mpf(2 * i + 1) / (N + 3) - 1
+        ph = i * mp.pi * (3 - mp.sqrt(5))
+        r = mp.sqrt(1 - z * z)
+        pts.append((r * mp.cos(ph), r * mp.sin(ph), z))
+
+    def ybar(m, v):
+        return pbar_general(l, abs(m), v[2]) * mp.e ** (1j * m * mp.atan2(v[1], v[0]))
+    Yp = mp.matrix(len(pts), N)
+    Ypp = mp.matrix(len(pts), N)
+    for i, v in enumerate(pts):
+        vpp = (-v[2], v[1], v[0])
+        for j, m in enumerate(range(-l, l + 1)):
+            Yp[i, j] = ybar(m, v)
+            Ypp[i, j] = ybar(m, vpp)
+    D = mp.inverse(Ypp[:N, :]) * Yp[:N, :]
+    assert mp.norm(Ypp * D - Yp) < mp.mpf(10) ** -30, "frame rotation: projection does not reproduce the extra directions"
+    assert max(abs(mp.im(D[i, j])) for i in range(N) for j in range(N)) < mp.mpf(10) ** -30
+    D = D.apply(mp.re)
+    _rot_cache[l] = D
+    return D
+
+
+_axial_cache = {}
+
+
+def _axial_operators(lmax):
+    """(Rm, Rinv, Z, all2, S2, S2inv, pm_matrices) of one lmax: block rotation, tilde-basis axial operator per q, F'' slots."""
+    if lmax in _axial_cache:
+        return _axial_cache[lmax]
+    md = modes(lmax)
+    L = len(md)
+    nq = 2 * lmax + 1
+    idx = {t: i for i, t in enumerate(md)}
+    eps = mp.mpf(10) ** -30
+    Rm = mp.matrix(L, L)
+    for p in (0, 1):
+        for l in range(1, lmax + 1):
+            D = frame_rotation(l)
+            for i, m2 in enumerate(range(-l, l + 1)):
+                for j, m1 in enumerate(range(-l, l + 1)):
+                    Rm[idx[(l, m2, p)], idx[(l, m1, p)]] = D[i, j]
+    Rinv = mp.inverse(Rm)
+    # tilde-basis axial operator (theta = 0): only m_a = m_b, Pbar_q^0(1) = sqrt((2q+1)/2)
+    Z = [mp.matrix(L, L) for _ in range(nq)]
+    for b, (lp, mp_, pp) in enumerate(md):
+        for a, (l, m, p) in enumerate(md):
+            if m != mp_:
+                continue
+            for q in range(nq):
+                ip, v = coupling(l, m, p, lp, mp_, pp, q)
+                if v == 0:
+                    continue
+                tot = (ip + (pp - p)) % 4
+                assert tot % 2 == 0
+                v = v * mp.sqrt(mp.mpf(2 * q + 1) / 2)
+                Z[q][b, a] = v if tot == 0 else -v
+    rows = coplanar_rows(lmax)
+    for q in range(nq):                      # the identity the whole factorisation rests on
+        Kd = mp.matrix(L, L)
+        for b in range(L):
+            for (a, v) in rows[b][q]:
+                Kd[b, a] += v
+        assert mp.norm(Kd - Rinv * Z[q] * Rm) < eps, "rotation - axial translation - rotation identity violated"
+
+    def pm_matrices(slots):
+        S = mp.matrix(len(slots), L)
+        Sinv = mp.matrix(L, len(slots))
+        for k, (l, am, p, kind) in enumerate(slots):
+            if kind == "0":
+                S[k, idx[(l, 0, p)]] = 1
+                Sinv[idx[(l, 0, p)], k] = 1
+            else:
+                sg = 1 if kind == "+" else -1
+                S[k, idx[(l, am, p)]] = 1
+                S[k, idx[(l, -am, p)]] = sg
+                Sinv[idx[(l, am, p)], k] = mp.mpf(1) / 2
+                Sinv[idx[(l, -am, p)], k] = mp.mpf(sg) / 2
+        return S, Sinv
+    all2 = []
+    for p in (0, 1):
+        for l in range(1, lmax + 1):
+            for am in range(0, l + 1):
+                all2 += [(l, 0, p, "0")] if am == 0 else [(l, am, p, "+"), (l, am, p, "-")]
+    S2, S2inv = pm_matrices(all2)
+    Zc = [S2 * Z[q] * S2inv for q in range(nq)]
+    _axial_cache[lmax] = (Rm, Rinv, Zc, all2, S2, S2inv, pm_matrices)
+    return _axial_cache[lmax]
+
+
+def axial_factorise(lmax, slots, Kdirect):
+    """Factorisation  K_q = Gout Z''_q G  of the pair-frame operator restricted to the +- slots `slots` (a subspace the
+    operator does not leave).  Kdirect(q) -> {(row, col): value} is the direct operator, used only for the final check.
+    Returns (slots, slots2, G, entries, Gout):
+      slots2  the F'' slots (l, |m''|, p, kind) reached from this subspace (same count)
+      G       rows over slots2: [(col slot, value)]        x'' = G x'
+      entries {(row2, col2): [(q, value)]}                 u''_row = sum_col (sum_q value h_q) x''_col   (same |m''| only)
+      Gout    rows over slots: [(col2, value)]             u' = Gout u''"""
+    Rm, Rinv, Zc, all2, S2, S2inv, pm_matrices = _axial_operators(lmax)
+    L = len(all2)
+    nq = 2 * lmax + 1
+    eps = mp.mpf(10) ** -30
+    n = len(slots)
+    S, Sinv = pm_matrices(slots)
+    Gf = S2 * Rm * Sinv                  # L x n
+    sel = [r for r in range(L) if any(abs(Gf[r, c]) > eps for c in range(n))]
+    assert len(sel) == n, "the subspace must map onto as many F'' slots"
+    sel.sort(key=lambda r: (all2[r][1], r))          # group by |m''|
+    pos = {r: i for i, r in enumerate(sel)}
+    Go_f = S * Rinv * S2inv              # n x L
+    G = [[(c, Gf[r, c]) for c in range(n) if abs(Gf[r, c]) > eps] for r in sel]
+    Gout = [[(j, Go_f[i, r]) for j, r in enumerate(sel) if abs(Go_f[i, r]) > eps] for i in range(n)]
+    entries = {}
+    for q in range(nq):
+        for i, r in enumerate(sel):
+            for c in range(L):
+                if abs(Zc[q][r, c]) > eps:
+                    assert c in pos and all2[c][1] == all2[r][1], "axial operator must stay inside the subspace and inside |m''|"
+                    entries.setdefault((i, pos[c]), []).append((q, Zc[q][r, c]))
+    Gm = mp.matrix(n, n)
+    Gom = mp.matrix(n, n)
+    for i, row in enumerate(G):
+        for (c, v) in row:
+            Gm[i, c] = v
+    for i, row in enumerate(Gout):
+        for (c, v) in row:
+            Gom[i, c] = v
+    for q in range(nq):                  # end-to-end check against the direct operator
+        M = mp.matrix(n, n)
+        for (i, j), lst in entries.items():
+            for (qq, v) in lst:
+                if qq == q:
+                    M[i, j] = v
+        Kq = mp.matrix(n, n)
+        for (r, c), v in Kdirect(q).items():
+            Kq[r, c] = v
+        assert mp.norm(Kq - Gom * M * Gm) < eps, "factorised operator differs from the direct one"
+    return slots, [all2[r] for r in sel], G, entries, Gout
+
+
+def coplanar_axial(lmax):
+    """Per z-mirror half of coplanar_sym(): the factorisation of axial_factorise()."""
+    out = []
+    for (slots, Knew) in coplanar_sym(lmax):
+        out.append(axial_factorise(lmax, slots, lambda q, Knew=Knew: {(r, c): v for r in range(len(Knew[q])) for (c, v) in Knew[q][r]}))
+    return out
+
+
+def coplanar_sectors_axial(lmax):
+    """Per sector of coplanar_sectors(): the factorisation of axial_factorise()."""
+    out = {}
+    for z, (slots, rows) in coplanar_sectors(lmax).items():
+        out[z] = axial_factorise(lmax, slots, lambda q, rows=rows: {(r, c): v for r in range(len(rows)) for (c, v) in rows[r][q]})
+    return out
+
+
+COPLANAR_AXIAL = True      # False: direct pair-frame operator (sum over (row, col, q) terms), the round's first version
+
+
+def emit_axial_core(f, fac):
+    """Straight-line code  u' = Gout (sum_q h_q Z''_q) G x'  for one half; x' in xr{k}/xi{k}, result in ur{k}/ui{k}.
+    Returns (FP instructions, flop)."""
+    slots, slots2, G, entries, Gout = fac
+    n = len(slots)
+    inst = flop = 0
+
+    # x'' = G x'
+    f.write("  // frame change F' -> F'' (z'' = pair axis)\n")
+    for i, row in enumerate(G):
+        for part in ("r", "i"):
+            expr = None
+            for t, (c, v) in enumerate(row):
+                if t == 0:
+                    if abs(v) == 1:
+                        expr = f"{'-' if v < 0 else ''}x{part}{c}"
+                    else:
+                        expr = f"R({lit(v)}) * x{part}{c}"
+                        inst += 1
+                        flop += 1
+                else:
+                    expr = f"fma(R({lit(v)}), x{part}{c}, {expr})"
+                    inst += 1
+                    flop += 2
+            f.write(f"  const R w{part}{i} = {expr};\n")
+    # axial translation, one |m''| block after the other; identical radial sums are formed once
+    f.write("  // axial translation along z'': diagonal in m''\n")
+    known = {}
+    by_row = {}
+    for (i, j), lst in sorted(entries.items()):
+        by_row.setdefault(i, []).append((j, lst))
+    for i in range(n):
+        first = True
+        for (j, lst) in by_row.get(i, []):
+            s0 = 1 if lst[0][1] > 0 else -1
+            key = tuple((q, mp.nstr(s0 * v, 30)) for (q, v) in lst)
+            if key not in known:
+                e = len(known)
+                known[key] = e
+                for part, hh in (("r", "hr"), ("i", "hi")):
+                    expr = None
+                    for t, (q, v) in enumerate(lst):
+                        vv = s0 * v
+                        if t == 0 and abs(vv) == 1:
+                            expr = f"{'-' if vv < 0 else ''}{hh}[{q}]"
+                        elif t == 0:
+                            expr = f"R({lit(vv)}) * {hh}[{q}]"
+                            inst += 1
+                            flop += 1
+                        else:
+                            expr = f"fma(R({lit(vv)}), {hh}[{q}], {expr})"
+                            inst += 1
+                            flop += 2
+                    f.write(f"  const R e{part}{e} = {expr};\n")
+            e = known[key]
+            sg = "" if s0 > 0 else "-"
+            ng = "-" if s0 > 0 else ""
+            if first:
+                f.write(f"  R tr{i} = {sg}er{e} * wr{j}; tr{i} = fma({ng}ei{e}, wi{j}, tr{i}); "
+                        f"R ti{i} = {sg}er{e} * wi{j}; ti{i} = fma({sg}ei{e}, wr{j}, ti{i});\n")
+                inst += 4
+                flop += 6
+                first = False
+            else:
+                f.write(f"  tr{i} = fma({sg}er{e}, wr{j}, tr{i}); tr{i} = fma({ng}ei{e}, wi{j}, tr{i}); "
+                        f"ti{i} = fma({sg}er{e}, wi{j}, ti{i}); ti{i} = fma({sg}ei{e}, wr{j}, ti{i});\n")
+                inst += 4
+                flop += 8
+        assert not first, "every F'' slot receives something"
+    # u' = Gout u''
+    f.write("  // frame change back F'' -> F'\n")
+    for r, row in enumerate(Gout):
+        for part in ("r", "i"):
+            expr = None
+            for t, (c, v) in enumerate(row):
+                if t == 0:
+                    if abs(v) == 1:
+                        expr = f"{'-' if v < 0 else ''}t{part}{c}"
+                    else:
+                        expr = f"R({lit(v)}) * t{part}{c}"
+                        inst += 1
+                        flop += 1
+                else:
+                    expr = f"fma(R({lit(v)}), t{part}{c}, {expr})"
+                    inst += 1
+                    flop += 2
+            f.write(f"  const R u{part}{r} = {expr};\n")
+    return inst, flop, len(known), sum(len(k) for k in known)
+
+
 def emit_coplanar(lmaxes, path):
     with open(path, "w") as f:
         f.write("// GENERATED by gen_tables.py - do not edit.\n")
-        f.write("// Coplanar (theta = pi/2) translation apply in the pair frame, one z-mirror-parity half per call, reduced by\n")
+        f.write("// Coplanar (theta = pi/2) translation apply, one z-mirror-parity half per call: phase rotation onto the pair frame,\n")
+        f.write("// fixed real frame change onto the pair AXIS, m''-diagonal axial translation, and back (gen_tables.py: coplanar_axial).\n")
+        f.write("// Interface and +- bases as in the direct version: pair frame, one z-mirror-parity half per call, reduced by\n")
         f.write("// the pair's y'-mirror symmetry (DESIGN.md, kernel K2c).  Basis of a half (\"slots\"): for every (l, |m|, p):\n")
         f.write("// d^0 = x~_{l,0,p};  d^+- = x~_{l,m,p} +- x~_{l,-m,p}  (x~ = i^p x), staged by the kernel with the tables below.\n")
         f.write("// xs: interleaved (re,im) d-values of this half; cm/sm: cos/sin(m phi); hr/hi: Re/Im h_q^(1)(kr);\n")
@@ -261,6 +542,7 @@ def emit_coplanar(lmaxes, path):
             md = modes(lmax)
             idx = {t: i for i, t in enumerate(md)}
             sym = coplanar_sym(lmax)
+            axial = coplanar_axial(lmax) if COPLANAR_AXIAL else None
             cost = [0, 0]
             for h in (0, 1):
                 slots, Knew = sym[h]
@@ -288,8 +570,14 @@ def emit_coplanar(lmaxes, path):
                         n_pairs += 1
                         k += 2
 
+                core = None
+                if COPLANAR_AXIAL:
+                    core = emit_axial_core(f, axial[h])
+
                 def row_code(r):
                     nonlocal nterm, nrowq
+                    if COPLANAR_AXIAL:
+                        return
                     f.write(f"    R ur{r} = R(0), ui{r} = R(0);\n")
                     first_q = True
                     for q in range(nq):
@@ -312,7 +600,7 @@ def emit_coplanar(lmaxes, path):
                 k = 0
                 while k < n:
                     l, am, p, kind = slots[k]
-                    f.write("  {\n    R yr, yi;\n")
+                    f.write("  {\n" if COPLANAR_AXIAL else "  {\n    R yr, yi;\n")
                     if kind == "0":
                         row_code(k)
                         f.write(f"    ar[{k}] += ur{k}; ai[{k}] += ui{k};\n")
@@ -333,10 +621,16 @@ def emit_coplanar(lmaxes, path):
                 #   input rotation per +- pair: 4 MUL + 4 FMA; output per pair: 8 FMA; m = 0 rows: 2 ADD
                 inst = 2 * nterm + 4 * nrowq + 8 * n_pairs + 8 * n_pairs + 2 * n_zero
                 flop = (2 * nrowq + 4 * (nterm - nrowq)) + (8 * nrowq - 2 * n) + (4 + 8) * n_pairs + 16 * n_pairs + 2 * n_zero
+                if COPLANAR_AXIAL:      # frame changes + radial sums + m''-diagonal apply, plus the phase rotations in and out
+                    inst = core[0] + 16 * n_pairs + 2 * n_zero
+                    flop = core[1] + (4 + 8) * n_pairs + 16 * n_pairs + 2 * n_zero
+                    print(f"lmax={lmax} half={h}: n={n} axial: {core[2]} distinct radial sums ({core[3]} terms) "
+                          f"-> {inst} FP instructions, {flop} flop per pair-half", file=sys.stderr)
+                else:
+                    print(f"lmax={lmax} half={h}: n={n} sym terms={nterm} (row,q) combos={nrowq} "
+                          f"-> {inst} FP instructions, {flop} flop per pair-half", file=sys.stderr)
                 cost[0] += inst
                 cost[1] += flop
-                print(f"lmax={lmax} half={h}: n={n} sym terms={nterm} (row,q) combos={nrowq} "
-                      f"-> {inst} FP instructions, {flop} flop per pair-half", file=sys.stderr)
                 # staging tables: d_k = x~[sa] + ss * x~[sb]
                 sa, sb, ss = [], [], []
                 for (l, am, p, kind) in slots:
@@ -593,6 +887,9 @@ def coplanar_sectors(lmax):
 COP4_GROUPS = {4: 1, 5: 4, 6: 4}     # row groups per sector: keeps one block's straight-line code near the 32 KB L1.5 I-cache
 
 
+COP4_AXIAL = True        # False: direct pair-frame operator cut into row groups
+
+
 def emit_coplanar4(lmaxes, path):
     with open(path, "w") as f:
         f.write("// GENERATED by gen_tables.py - do not edit.\n")
@@ -604,11 +901,12 @@ def emit_coplanar4(lmaxes, path):
             idx = {t_: i for i, t_ in enumerate(md)}
             nq = 2 * lmax + 1
             half_l = len(md) // 2
-            G = COP4_GROUPS[lmax]
+            G = 1 if COP4_AXIAL else COP4_GROUPS[lmax]
             cost = [0, 0]
             nmax = 0
             rmax = 0
             secs = coplanar_sectors(lmax)
+            secs_axial = coplanar_sectors_axial(lmax) if COP4_AXIAL else None
             for z in range(4):
                 slots, rows = secs[z]
                 n = len(slots)
@@ -643,7 +941,7 @@ def emit_coplanar4(lmaxes, path):
                     r0, r1 = bounds[g], bounds[g + 1]
                     nr = r1 - r0
                     rmax = max(rmax, nr)
-                    used_cols = sorted({c for r in range(r0, r1) for q in range(nq) for (c, _) in rows[r][q]})
+                    used_cols = list(range(n)) if COP4_AXIAL else sorted({c for r in range(r0, r1) for q in range(nq) for (c, _) in rows[r][q]})
                     f.write(f"// lmax={lmax} z={z} group={g}: rows {r0}..{r1 - 1}\n")
                     f.write(f"#define TM_COP4_NR_L{lmax}_Z{z}_G{g} {nr}\n")
                     f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
@@ -659,13 +957,17 @@ def emit_coplanar4(lmaxes, path):
                                     f"xi{k} = xs[{2 * k + 1}] * cm[{am}] + xs[{2 * (n + k)}] * sm[{am}];\n")
                             n_pairs += 1
                     nterm = nrowq = 0
+                    core = emit_axial_core(f, secs_axial[z]) if COP4_AXIAL else None
                     for r in range(r0, r1):
                         l, am, p, kind = slots[r]
                         lr = r - r0
-                        f.write("  {\n    R ur = R(0), ui = R(0), yr, yi;\n")
+                        if COP4_AXIAL:
+                            f.write(f"  {{\n    const R ur = ur{r}, ui = ui{r};\n")
+                        else:
+                            f.write("  {\n    R ur = R(0), ui = R(0), yr, yi;\n")
                         for q in range(nq):
                             terms = rows[r][q]
-                            if not terms:
+                            if not terms or COP4_AXIAL:
                                 continue
                             nrowq += 1
                             for t_, (c, v) in enumerate(terms):
@@ -685,9 +987,14 @@ def emit_coplanar4(lmaxes, path):
                     nrp = sum(1 for r in range(r0, r1) if slots[r][3] != "0")
                     inst = 2 * nterm + 4 * nrowq + 4 * n_pairs + 4 * nrp + 2 * (nr - nrp)
                     flop = (2 * nrowq + 4 * (nterm - nrowq)) + 8 * nrowq + 6 * n_pairs + 8 * nrp + 2 * (nr - nrp)
+                    if COP4_AXIAL:
+                        inst = core[0] + 4 * n_pairs + 4 * nrp + 2 * (nr - nrp)
+                        flop = core[1] + 6 * n_pairs + 8 * nrp + 2 * (nr - nrp)
+                        print(f"lmax={lmax} z={z}: n={n} axial: {core[2]} distinct radial sums ({core[3]} terms) -> {inst} FP instructions, {flop} flop", file=sys.stderr)
+                    else:
+                        print(f"lmax={lmax} z={z} g={g}: rows={nr} cols={len(used_cols)} terms={nterm} (row,q)={nrowq} -> {inst} FP instructions", file=sys.stderr)
                     cost[0] += inst
                     cost[1] += flop
-                    print(f"lmax={lmax} z={z} g={g}: rows={nr} cols={len(used_cols)} terms={nterm} (row,q)={nrowq} -> {inst} FP instructions", file=sys.stderr)
                     # unmix of the group's rows (+ the zero fill of the partner-owned m = 0 modes, done by group 0)
                     f.write("template <typename R, typename C, int AS>\n__device__ __forceinline__ void "
                             f"tm_cop4_unmix_L{lmax}_Z{z}_G{g}(const R* ar, const R* ai, C* out) {{\n")
