@@ -1031,6 +1031,52 @@ def emit_coplanar4(lmaxes, path):
 
 
 # ----------------------------------------------------------------------------- coplanar, fp32 packed (FFMA2)
+def emit_axial_core_f2(f, fac):
+    """Packed-fp32 version of emit_axial_core: x' in float2 x{k}, result in float2 u{k}; real x complex = 1 FFMA2,
+    complex x complex = 2 FFMA2; h{q} = (Re, Im) h_q must be in scope."""
+    slots, slots2, G, entries, Gout = fac
+    n = len(slots)
+    f2 = lambda a, b: f"make_float2({a}, {b})"
+
+    def lincomb(dst, src, rows):
+        for i, row in enumerate(rows):
+            expr = None
+            for t, (c, v) in enumerate(row):
+                kk = lit(v) + "f"
+                if t == 0 and v == 1:
+                    expr = f"{src}{c}"
+                else:
+                    expr = f"__fmul2_rn({f2(kk, kk)}, {src}{c})" if t == 0 else f"__ffma2_rn({f2(kk, kk)}, {src}{c}, {expr})"
+            f.write(f"  const float2 {dst}{i} = {expr};\n")
+    lincomb("w", "x", G)
+    known = {}
+    by_row = {}
+    for (i, j), lst in sorted(entries.items()):
+        by_row.setdefault(i, []).append((j, lst))
+    for i in range(n):
+        first = True
+        for (j, lst) in by_row.get(i, []):
+            s0 = 1 if lst[0][1] > 0 else -1
+            key = tuple((q, mp.nstr(s0 * v, 30)) for (q, v) in lst)
+            if key not in known:
+                e = len(known)
+                known[key] = e
+                expr = None
+                for t, (q, v) in enumerate(lst):
+                    kk = lit(s0 * v) + "f"
+                    expr = f"__fmul2_rn({f2(kk, kk)}, h{q})" if t == 0 else f"__ffma2_rn({f2(kk, kk)}, h{q}, {expr})"
+                f.write(f"  const float2 e{e} = {expr};\n")
+            e = known[key]
+            a_re = f2(f"e{e}.x", f"e{e}.x") if s0 > 0 else f2(f"-e{e}.x", f"-e{e}.x")
+            a_im = f2(f"-e{e}.y", f"e{e}.y") if s0 > 0 else f2(f"e{e}.y", f"-e{e}.y")
+            if first:
+                f.write(f"  float2 t{i} = __fmul2_rn({a_re}, w{j}); t{i} = __ffma2_rn({a_im}, tm_swap2(w{j}), t{i});\n")
+                first = False
+            else:
+                f.write(f"  t{i} = __ffma2_rn({a_re}, w{j}, t{i}); t{i} = __ffma2_rn({a_im}, tm_swap2(w{j}), t{i});\n")
+    lincomb("u", "t", Gout)
+
+
 def emit_coplanar_f2(lmaxes, path):
     """fp32 build of the coplanar pair code on Blackwell's packed FP32 instructions (FFMA2 / FMUL2: two FMAs per issue
     slot, immediate and register operands broadcast, LO_HI swap and per-half negation are operand modifiers).  A complex
@@ -1045,6 +1091,7 @@ def emit_coplanar_f2(lmaxes, path):
             md = modes(lmax)
             idx = {t: i for i, t in enumerate(md)}
             sym = coplanar_sym(lmax)
+            axial = coplanar_axial(lmax) if COPLANAR_AXIAL else None
             half_l = len(md) // 2
             for h in (0, 1):
                 slots, Knew = sym[h]
@@ -1064,7 +1111,14 @@ def emit_coplanar_f2(lmaxes, path):
                         f.write(f"  const float2 x{km} = __ffma2_rn({f2(f'-sm[{am}]', f'sm[{am}]')}, tm_swap2(xs[{kp}]), __fmul2_rn({f2(f'cm[{am}]', f'cm[{am}]')}, xs[{km}]));\n")
                         k += 2
 
+                if COPLANAR_AXIAL:
+                    for q in range(nq):
+                        f.write(f"  const float2 h{q} = make_float2(hr[{q}], hi[{q}]);\n")
+                    emit_axial_core_f2(f, axial[h])
+
                 def row_code(r):
+                    if COPLANAR_AXIAL:
+                        return
                     f.write(f"    float2 u{r} = make_float2(0.f, 0.f);\n")
                     for q in range(nq):
                         terms = Knew[q][r]
@@ -1082,7 +1136,7 @@ def emit_coplanar_f2(lmaxes, path):
                 k = 0
                 while k < n:
                     l, am, p, kind = slots[k]
-                    f.write("  {\n    float2 y;\n")
+                    f.write("  {\n" if COPLANAR_AXIAL else "  {\n    float2 y;\n")
                     if kind == "0":
                         row_code(k)
                         f.write(f"    a[{k}] = __fadd2_rn(a[{k}], u{k});\n")

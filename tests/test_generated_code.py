@@ -89,3 +89,64 @@ def test_generated_general_term_table_matches_oracle_block(lmax):
             B[b, a] += (1j) ** ip[t] * val[t] * h[qq[t]] * sp.pbar(qq[t], abs(mu), np.cos(th)) * np.exp(1j * mu * ph)
     ref = tr.block(lmax, K, d, np.zeros(3))
     assert np.abs(B - ref).max() <= 1e-13 * np.abs(ref).max()
+
+
+def _load_generator():
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("tm_gen_tables", os.path.join(ROOT, "paper_2107_09879_b200", "csrc", "gen_tables.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    return mod
+
+
+def test_frame_rotation_is_a_quarter_turn():
+    """The generator's frame change F' -> F'' (z'' = pair axis): real, orthogonal (all Ybar_lm have the same norm), four
+    applications give the identity, and it carries the direction x' onto z'': Ybar_l0 of the pole is the only non-zero
+    harmonic there, so column m' must reproduce Ybar_{l,m'}(x') = Pbar_l^{|m'|}(0) up to the pole value sqrt((2l+1)/2)."""
+    g = _load_generator()
+    for l in (1, 2, 3, 6):
+        D = np.array(g.frame_rotation(l).tolist(), dtype=float)
+        n = 2 * l + 1
+        assert np.abs(D @ D.T - np.eye(n)).max() < 1e-14
+        assert np.abs(np.linalg.matrix_power(D, 4) - np.eye(n)).max() < 1e-13
+        pole = np.sqrt((2 * l + 1) / 2.0)
+        for j, m in enumerate(range(-l, l + 1)):
+            want = float(sp.pbar(l, abs(m), 0.0))
+            assert abs(D[l, j] * pole - want) < 1e-14          # row m'' = 0
+
+
+@pytest.mark.parametrize("lmax", [1, 2, 3])
+def test_axial_factorisation_reproduces_the_oracle_block(lmax):
+    """u = A x for an in-plane pair through the generator's factorisation  K_q = Gout Z''_q G  (numpy evaluation of the
+    returned sparse factors, both halves, with the kernel's +- staging and phase rotation) against the oracle block."""
+    g = _load_generator()
+    md = g.modes(lmax)
+    idx = {t: i for i, t in enumerate(md)}
+    L = len(md)
+    rng = np.random.default_rng(70 + lmax)
+    ipow = np.array([1j ** p for (_, _, p) in md])
+    for d in ([0.5, 0.0], [-1.7, 2.9], rng.uniform(-6, 6, 2)):
+        x = rng.standard_normal(L) + 1j * rng.standard_normal(L)
+        r = float(np.hypot(d[0], d[1]))
+        phi = float(np.arctan2(d[1], d[0]))
+        hq = np.array([complex(sp.sph_h1(q, K * r)) for q in range(2 * lmax + 1)])
+        xt = ipow * x * np.exp(1j * np.array([m for (_, m, _) in md]) * phi)        # x~' = e^{i m phi} i^p x
+        ut = np.zeros(L, dtype=complex)
+        for (slots, slots2, G, entries, Gout) in g.coplanar_axial(lmax):
+            n = len(slots)
+            xs = np.array([xt[idx[(l, am, p)]] + {"0": 0, "+": 1, "-": -1}[k] * xt[idx[(l, -am, p)]] for (l, am, p, k) in slots])
+            w = np.array([sum(float(v) * xs[c] for (c, v) in row) for row in G])
+            t = np.zeros(n, dtype=complex)
+            for (i, j), lst in entries.items():
+                t[i] += sum(float(v) * hq[q] for (q, v) in lst) * w[j]
+            u = np.array([sum(float(v) * t[c] for (c, v) in row) for row in Gout])
+            for k_, (l, am, p, kind) in enumerate(slots):
+                if kind == "0":
+                    ut[idx[(l, 0, p)]] += u[k_]
+                else:
+                    sg = 1 if kind == "+" else -1
+                    ut[idx[(l, am, p)]] += 0.5 * u[k_]
+                    ut[idx[(l, -am, p)]] += 0.5 * sg * u[k_]
+        u_full = np.conj(ipow) * np.exp(-1j * np.array([m for (_, m, _) in md]) * phi) * ut
+        ref = tr.block(lmax, K, np.array([d[0], d[1], 0.0]), np.zeros(3)) @ x
+        assert np.abs(u_full - ref).max() <= 2e-13 * np.abs(ref).max()
