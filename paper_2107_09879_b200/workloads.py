@@ -132,3 +132,51 @@ def cloud_workload(n, seed, lmax=3, planar=False, full_t=False, n_win=1):
     cuts = np.linspace(0, n, n_win + 1).round().astype(np.int32)
     w["win_ptr"] = cuts
     return w
+
+
+# ---- surfaces of revolution for the null-field T-matrix ("numerical discretization ... for evaluating
+# these surface integrals").  A generatrix is the discretised surface r = r(theta) about the z axis: arrays
+# (theta, r, dr, w) with dr = dr/dtheta and Gauss-Legendre weights w in theta, one panel per smooth piece.
+# Geometry only: none of the method's arithmetic.
+
+def _panels(edges, n_per_panel):
+    x, w = np.polynomial.legendre.leggauss(n_per_panel)
+    th, wt = [], []
+    for a, b in zip(edges[:-1], edges[1:]):
+        th.append(0.5 * (b - a) * x + 0.5 * (a + b))
+        wt.append(0.5 * (b - a) * w)
+    return np.concatenate(th), np.concatenate(wt)
+
+
+def generatrix_sphere(radius, n=48, offset=0.0):
+    """Sphere of the given radius whose centre sits at z = offset (|offset| < radius), seen from the origin."""
+    th, w = _panels([0.0, np.pi], n)
+    root = np.sqrt(radius ** 2 - (offset * np.sin(th)) ** 2)
+    r = offset * np.cos(th) + root
+    dr = -offset * np.sin(th) - offset ** 2 * np.sin(th) * np.cos(th) / root
+    return th, r, dr, w
+
+
+def generatrix_cylinder(radius, height, n_per_panel=48):
+    """Finite circular cylinder (the paper's meta-atom shape) centred on the origin, axis z:
+    top cap, side wall, bottom cap (three smooth panels)."""
+    hh = 0.5 * height
+    tc = np.arctan2(radius, hh)
+    th, w = _panels([0.0, tc, np.pi - tc, np.pi], n_per_panel)
+    r, dr = np.empty_like(th), np.empty_like(th)
+    top, bot = th < tc, th > np.pi - tc
+    side = ~(top | bot)
+    r[top] = hh / np.cos(th[top]);       dr[top] = hh * np.sin(th[top]) / np.cos(th[top]) ** 2
+    r[bot] = -hh / np.cos(th[bot]);      dr[bot] = -hh * np.sin(th[bot]) / np.cos(th[bot]) ** 2
+    r[side] = radius / np.sin(th[side]); dr[side] = -radius * np.cos(th[side]) / np.sin(th[side]) ** 2
+    return th, r, dr, w
+
+
+def generatrix_spheroid(a_xy, c_z, n=64):
+    """Spheroid x^2/a^2 + y^2/a^2 + z^2/c^2 = 1."""
+    th, w = _panels([0.0, np.pi], n)
+    s, c = np.sin(th), np.cos(th)
+    q = (s / a_xy) ** 2 + (c / c_z) ** 2
+    r = q ** -0.5
+    dr = -0.5 * q ** -1.5 * 2.0 * s * c * (1.0 / a_xy ** 2 - 1.0 / c_z ** 2)
+    return th, r, dr, w
