@@ -456,6 +456,38 @@ def run_gradient(args, w):
     s.close()
 
 
+def run_nullfield(args):
+    """Recorded run of NEXT-4 (not the contract line): null-field T-matrices of a library of cylinders (the paper's meta-atom
+    library) at the paper's truncation lmax 6 in ONE tm_nullfield_tmatrix call; the oracle's literal
+    surface quadrature timed on one shape beside it."""
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2107_09879_b200 import libtm
+    lmax = args.lmax or 6
+    n_shapes, n_panel = 256, 64
+    radii = np.linspace(0.10, 0.24, n_shapes)
+    gens = [W.generatrix_cylinder(r, 0.3, n_panel) for r in radii]
+    libtm.nullfield_tmatrix(lmax, W.K_B, 4.0, gens[:2])                     # warm-up (module load, pool)
+    ts = []
+    for _ in range(5):
+        t0 = time.perf_counter()
+        T = libtm.nullfield_tmatrix(lmax, W.K_B, 4.0, gens)
+        ts.append(time.perf_counter() - t0)
+    n = T.shape[1]
+    S = np.eye(n)[None] + 2.0 * T
+    unit = float(np.abs(S @ np.conj(np.swapaxes(S, 1, 2)) - np.eye(n)[None]).max())
+    out = {"mode": "nullfield", "lmax": lmax, "L": n, "n_shapes": n_shapes, "nodes_per_shape": 3 * n_panel,
+           "call_ms_median_incl_copies": 1e3 * float(np.median(ts)), "shapes_per_s": n_shapes / float(np.median(ts)),
+           "max_unitarity_defect": unit}
+    if not args.no_cpu_baseline:
+        from oracle import nullfield as onf
+        t0 = time.perf_counter()
+        ref = onf.nullfield_tmatrix(lmax, W.K_B, 4.0, gens[100])
+        out.update(oracle_seconds_per_shape=time.perf_counter() - t0,
+                   max_rel_error_vs_oracle=float(np.abs(T[100] - ref).max() / np.abs(ref).max()))
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -463,7 +495,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2")
-    ap.add_argument("--mode", default="full", choices=["full", "matvec", "nyquist", "gradient"],
+    ap.add_argument("--mode", default="full", choices=["full", "matvec", "nyquist", "gradient", "nullfield"],
                     help="matvec: time operator applications only; nyquist: recorded run of the window decomposition")
     ap.add_argument("--group", type=int, default=16, help="nyquist mode: samples per group side")
     ap.add_argument("--padding", type=float, default=4.0, help="nyquist mode: padding in wavelengths")
@@ -496,7 +528,10 @@ def main():
         w["name"] += f"_lmax{args.lmax}"
         if "w_adj" in w:
             del w["w_adj"]
-    if args.mode == "nyquist":
+    if args.mode == "nullfield":
+        if rank == 0:
+            run_nullfield(args)
+    elif args.mode == "nyquist":
         if rank == 0:
             run_nyquist(args, w)
     elif args.mode == "gradient":

@@ -16,6 +16,7 @@
 #include "tm_fields.cuh"
 #include "tm_gmres.cuh"
 #include "tm_incident.cuh"
+#include "tm_nullfield.cuh"
 #include "tm_special.cuh"
 #include "tm_vecops.cuh"
 #include "generated/tm_tables_gen.h"
@@ -1481,6 +1482,43 @@ int tm_release_cached_memory(void) {
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetDefaultMemPool(&pool, dev) != cudaSuccess) return TM_E_CUDA;
   if (cudaDeviceSynchronize() != cudaSuccess) return TM_E_CUDA;
   return cudaMemPoolTrimTo(pool, 0) == cudaSuccess ? TM_OK : TM_E_CUDA;
+}
+
+int tm_nullfield_tmatrix(int lmax, double k_b, double eps_r, int n_shapes, int n_nodes, const double* theta, const double* r,
+                         const double* dr_dtheta, const double* weight, tm_c64* T_out, void* cuda_stream) {
+  if (lmax < 1 || lmax > TM_MAX_LMAX || !(k_b > 0.0) || !(eps_r > 0.0) || !std::isfinite(eps_r) || n_shapes < 1 || n_nodes < 1 ||
+      !theta || !r || !dr_dtheta || !weight || !T_out)
+    return TM_E_INVALID;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return TM_E_CUDA; }
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const size_t nn = (size_t)n_shapes * n_nodes, L = (size_t)tm_num_modes(lmax);
+  {   // the surface must be star-shaped about the origin with finite nodes: r > 0, 0 < theta < pi
+    std::vector<double> hr(nn), ht(nn);
+    if (cudaMemcpy(hr.data(), r, nn * sizeof(double), is_device_ptr(r) ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost) != cudaSuccess ||
+        cudaMemcpy(ht.data(), theta, nn * sizeof(double), is_device_ptr(theta) ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost) != cudaSuccess) {
+      cudaGetLastError(); return TM_E_CUDA;
+    }
+    for (size_t i = 0; i < nn; ++i)
+      if (!(hr[i] > 0.0) || !std::isfinite(hr[i]) || !(ht[i] > 0.0) || !(ht[i] < 3.14159265358979324)) return TM_E_INVALID;
+  }
+  double* d_in = nullptr; double2* d_T = nullptr;
+  if (tm_dev_alloc(&d_in, 4 * nn * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return TM_E_NOMEM; }
+  if (tm_dev_alloc(&d_T, n_shapes * L * L * sizeof(double2)) != cudaSuccess) { cudaGetLastError(); tm_dev_free(d_in); return TM_E_NOMEM; }
+  const double* src[4] = {theta, r, dr_dtheta, weight};
+  cudaError_t e = cudaSuccess;
+  for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = copy_in(d_in + i * nn, src[i], nn * sizeof(double), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_T, 0, n_shapes * L * L * sizeof(double2), st);
+  if (e == cudaSuccess) {
+    nullfield::k_nullfield<<<dim3(n_shapes, 2 * lmax + 1), 256, 0, st>>>(lmax, k_b, k_b * std::sqrt(eps_r), n_nodes, d_in, d_in + nn,
+                                                                         d_in + 2 * nn, d_in + 3 * nn, d_T);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = copy_out(T_out, d_T, n_shapes * L * L * sizeof(double2), st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  tm_dev_free(d_in); tm_dev_free(d_T);
+  if (e != cudaSuccess) { cudaGetLastError(); return TM_E_CUDA; }
+  return TM_OK;
 }
 
 int tm_measure_fma_peak(int precision, double* tflops, void* cuda_stream) {

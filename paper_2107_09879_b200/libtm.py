@@ -22,6 +22,7 @@ TM_KERNEL_AUTO, TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR, TM_KERNEL_SYM3D = 0, 1, 2
 EXPORTS = ["tm_create", "tm_set_tmatrices", "tm_set_incident", "tm_get_incident", "tm_solve", "tm_solve_adjoint",
            "tm_matvec", "tm_fields", "tm_workspace_bytes", "tm_set_workspace", "tm_set_kernel", "tm_get_kernel",
            "tm_kernel_time", "tm_pair_cost", "tm_measure_fma_peak", "tm_grad_tmatrix", "tm_grad_positions", "tm_mie_tmatrix_dR", "tm_mie_tmatrix",
+           "tm_nullfield_tmatrix",
            "tm_release_cached_memory", "tm_num_modes", "tm_last_error", "tm_destroy"]
 
 
@@ -91,6 +92,7 @@ def lib():
         L.tm_grad_tmatrix.argtypes = [vp, vp, vp, vp, vp]
         L.tm_grad_positions.argtypes = [vp, vp, vp, vp, cd, vp]
         L.tm_mie_tmatrix_dR.argtypes = [ci, cd, cd, c64, vp]
+        L.tm_nullfield_tmatrix.argtypes = [ci, cd, cd, ci, ci, vp, vp, vp, vp, vp, vp]
         L.tm_pair_cost.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(cd)]
         L.tm_measure_fma_peak.argtypes = [ci, ctypes.POINTER(cd), vp]
         L.tm_num_modes.argtypes = [ci]
@@ -133,6 +135,23 @@ def mie_tmatrix_dR(lmax, k_b, radius, eps_r):
     if rc != TM_OK:
         raise TmError(rc, "tm_mie_tmatrix_dR: invalid arguments")
     return out
+
+
+def nullfield_tmatrix(lmax, k_b, eps_r, generatrices, stream=None):
+    """Null-field T-matrices of bodies of revolution (tm_nullfield_tmatrix).  `generatrices`: one (theta, r, dr, w) tuple
+    or a list of them with equal node counts (workloads.generatrix_*).  Returns (L, L) or (n_shapes, L, L) complex128."""
+    single = not isinstance(generatrices, list)
+    gens = [generatrices] if single else generatrices
+    arr = [np.ascontiguousarray(np.stack([np.asarray(g[i], dtype=np.float64) for g in gens])) for i in range(4)]
+    n_shapes, n_nodes = arr[0].shape
+    L = lib().tm_num_modes(lmax)
+    out = np.zeros((n_shapes, L, L), dtype=np.complex128)
+    rc = lib().tm_nullfield_tmatrix(int(lmax), float(k_b), float(eps_r), n_shapes, n_nodes, arr[0].ctypes.data, arr[1].ctypes.data,
+                                    arr[2].ctypes.data, arr[3].ctypes.data, out.ctypes.data,
+                                    ctypes.c_void_p(stream) if stream else None)
+    if rc != TM_OK:
+        raise TmError(rc, "tm_nullfield_tmatrix failed")
+    return out[0] if single else out
 
 
 def measure_fma_peak(precision=TM_FP64, stream=None):

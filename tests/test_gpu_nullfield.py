@@ -1,0 +1,83 @@
+"""NEXT-4: null-field T-matrices of bodies of revolution on the device (tm_nullfield_tmatrix) against the oracle's literal
+two-dimensional surface quadrature (oracle/nullfield.py), and through the coupled solve."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from oracle import nullfield as onf, system, tmatrix, incident  # noqa: E402
+from paper_2107_09879_b200 import workloads as W  # noqa: E402
+
+K = W.K_B
+
+
+@pytest.fixture(scope="module")
+def tm():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2107_09879_b200 import libtm
+    libtm.lib()
+    return libtm
+
+
+def maxrel(a, b):
+    return np.abs(np.asarray(a) - np.asarray(b)).max() / np.abs(b).max()
+
+
+@pytest.mark.parametrize("lmax", [1, 2, 3, 4, 6])
+def test_sphere_is_mie(tm, lmax):
+    T = tm.nullfield_tmatrix(lmax, K, 4.0, W.generatrix_sphere(0.2, 48))
+    assert maxrel(T, np.diag(tmatrix.mie_tmatrix_diag(lmax, K, 0.2, 4.0))) <= 1e-12
+
+
+@pytest.mark.parametrize("name,lmax,gen", [
+    ("cylinder", 3, W.generatrix_cylinder(0.15, 0.3, 32)),
+    ("cylinder", 6, W.generatrix_cylinder(0.12, 0.35, 43)),          # 129 nodes: three stages, ragged tail
+    ("spheroid", 4, W.generatrix_spheroid(0.15, 0.22, 64)),
+    ("offset sphere", 5, W.generatrix_sphere(0.2, 70, offset=0.05)),   # no mirror symmetry: full (l, p) blocks
+])
+def test_matches_oracle_surface_quadrature(tm, name, lmax, gen):
+    T = tm.nullfield_tmatrix(lmax, K, 4.0, gen)
+    ref = onf.nullfield_tmatrix(lmax, K, 4.0, gen)
+    assert maxrel(T, ref) <= 1e-9
+
+
+def test_library_of_shapes_in_one_call(tm):
+    radii = [0.10, 0.14, 0.18, 0.22]
+    gens = [W.generatrix_cylinder(r, 0.3, 24) for r in radii]
+    Ts = tm.nullfield_tmatrix(3, K, 4.0, gens)
+    assert Ts.shape == (4, 30, 30)
+    for T, g in zip(Ts, gens):
+        assert maxrel(T, onf.nullfield_tmatrix(3, K, 4.0, g)) <= 1e-9
+        assert maxrel(T, tm.nullfield_tmatrix(3, K, 4.0, g)) == 0.0          # batch = single, bit for bit
+
+
+def test_invalid_arguments(tm):
+    g = W.generatrix_sphere(0.2, 8)
+    for bad in ((0, K, 4.0, g), (7, K, 4.0, g), (3, K, -1.0, g), (3, K, 4.0, (g[0], -g[1], g[2], g[3])),
+                (3, K, 4.0, (g[0] + 4.0, g[1], g[2], g[3]))):
+        with pytest.raises(tm.TmError):
+            tm.nullfield_tmatrix(*bad)
+
+
+def test_cylinder_lattice_solve_vs_dense_lu(tm):
+    """6x6 lattice of cylinders from a 4-radius library: device T-matrices -> tm_set_tmatrices (full) -> GMRES, against the
+    oracle's T-matrices -> dense LU."""
+    lmax = 3
+    rng = np.random.default_rng(11)
+    pos = W.lattice(6, 6)
+    radii = [0.10, 0.13, 0.16, 0.19]
+    gens = [W.generatrix_cylinder(r, 0.3, 32) for r in radii]
+    type_of = rng.integers(0, 4, len(pos)).astype(np.int32)
+    t_dev = tm.nullfield_tmatrix(lmax, K, 4.0, gens)
+    t_ref = np.stack([onf.nullfield_tmatrix(lmax, K, 4.0, g) for g in gens])
+    p = incident.plane_wave_incident(lmax, K, pos, 0.0, 0.0, 1.0, 0.0)
+    M = system.assemble_M(lmax, K, pos, t_ref, type_of, False)
+    ref = system.solve_forward(M, t_ref, type_of, False, p)
+    s = tm.Solver(pos, lmax, K)
+    s.set_tmatrices(t_dev, type_of, False)
+    s.set_incident_plane(0.0, 0.0, 1.0, 0.0)
+    sol, info, rc = s.solve(1e-11, 50, 500)
+    assert rc == 0
+    assert np.linalg.norm(sol - ref) / np.linalg.norm(ref) <= 1e-9
+    s.close()
