@@ -196,7 +196,9 @@ def run_ours(args, w, rank, world, local_rank):
         w["restart"] = args.restart
 
     with torch.cuda.stream(st):
-        peak = libtm.measure_fma_peak(prec, st.cuda_stream)
+        # TM_MIXED: all but one all-pairs launch per restart cycle run on the FP32 pipe, so that pipe's peak is the denominator
+        peak_prec = libtm.TM_FP64 if prec == libtm.TM_FP64 else libtm.TM_FP32
+        peak = libtm.measure_fma_peak(peak_prec, st.cuda_stream)
         kern_req = {"auto": libtm.TM_KERNEL_AUTO, "general": libtm.TM_KERNEL_GENERAL, "coplanar": libtm.TM_KERNEL_COPLANAR,
                     "sym3d": libtm.TM_KERNEL_SYM3D}[args.kernel]
         s = libtm.solver_for_workload(w, precision=prec, stream=st.cuda_stream, kernel=kern_req)
@@ -270,6 +272,17 @@ def run_ours(args, w, rank, world, local_rank):
         clk = clocks.stop()
         matvecs = info[0].matvecs + info2[0].matvecs
         total_ms = float(sum(ms_list))
+        # physics self-check of the timed solution (outside the timed region, one extra all-pairs product): lossless scatterers
+        # scatter what they extinguish,  -Re p^H s = |s|^2 + Re s^H A s  (SURVEY.md 8(c) O9 / identity S4b); holds at any size
+        energy = None
+        if args.mode == "full":
+            s.matvec(d_s, 2, out=d_y)                                       # u = A s
+            d_p = torch.empty_like(d_s)
+            s.get_incident(out=d_p)
+            ext = -float(torch.vdot(d_p.reshape(-1), d_s.reshape(-1)).real)
+            sca = float(torch.vdot(d_s.reshape(-1), d_s.reshape(-1)).real + torch.vdot(d_s.reshape(-1), d_y.reshape(-1)).real)
+            energy = {"extinction": ext, "scattering": sca, "rel_defect": abs(ext - sca) / abs(ext),
+                      "note": "coefficient units (x pi/k^2 = cross-section for a unit plane wave); lossless T: defect ~ solver residual"}
 
         # end to end through the C ABI with HOST buffers: context creation (uploads positions, T, types), incident,
         # both solves and the field evaluation, every result copied back to host memory
@@ -376,11 +389,12 @@ def run_ours(args, w, rank, world, local_rank):
             "roofline": {"bound": "alu", "kernel": {libtm.TM_KERNEL_COPLANAR: "k_allpairs_coplanar", libtm.TM_KERNEL_SYM3D: "k_allpairs_sym3d"}.get(kern, "k_allpairs_general"),
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": (achieved / peak) if achieved else None,
                          "peak_source": "measured live: tm_measure_fma_peak (register-resident FMA chains, this GPU, this run)",
+                         "peak_pipe": "fp64" if peak_prec == libtm.TM_FP64 else "fp32",
                          "flop_per_pair": flop, "fp_instr_per_pair": fpinst, "pairs_per_launch": pairs,
                          "avg_launch_ms": ap_avg_ms, "launches": int(ap_launches), "share_of_step": ap_ms / total_ms if total_ms else None,
                          "pipe_frac": (pairs * fpinst / (ap_avg_ms * 1e-3)) / (peak * 1e12 / 2) if ap_launches else None,
                          "pairs_per_s": pairs / (ap_avg_ms * 1e-3) if ap_launches else None, "traffic": traffic},
-            "clocks": clk, "ms_steps": [round(v, 3) for v in ms_list],
+            "energy_balance": energy, "clocks": clk, "ms_steps": [round(v, 3) for v in ms_list],
             "solve_ms_log": solve_log[-2 * args.steps:] if args.mode == "full" else [],
         }
         if mixed is not None:

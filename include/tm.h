@@ -223,6 +223,15 @@ int tm_mie_tmatrix(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64 *ou
 int tm_nullfield_tmatrix(int lmax, double k_b, double eps_r, int n_shapes, int n_nodes, const double *theta, const double *r,
                          const double *dr_dtheta, const double *weight, tm_c64 *T_out, void *cuda_stream);
 
+/* d T / d(shape parameter) of the null-field T-matrix ("T_j depends on the geometry parameters of scatterer
+ * j"; the `dT` of tm_grad_tmatrix).  The caller hands over, per shape, FOUR generatrices - the surface at parameter values
+ * p + h, p - h, p + h/2, p - h/2, in this order - laid out [n_shapes][4][n_nodes]; the library computes the four T-matrices in
+ * the same launch as tm_nullfield_tmatrix and combines them on the device into the Richardson-extrapolated central
+ * difference (4 D(h/2) - D(h)) / 3, D(h) = (T(p+h) - T(p-h)) / 2h  (error O(h^4)).  A stated deviation from an analytic
+ * dT/dp, like tm_mie_tmatrix_dR.  dT_out [n_shapes][L][L], host or device.  Errors as tm_nullfield_tmatrix, and h <= 0. */
+int tm_nullfield_dtmatrix(int lmax, double k_b, double eps_r, int n_shapes, int n_nodes, const double *theta, const double *r,
+                          const double *dr_dtheta, const double *weight, double h, tm_c64 *dT_out, void *cuda_stream);
+
 /* Memory (the solver state is what limits the problem size on one GPU).  All device memory of the
  * library comes from the current device's stream-ordered pool (cudaMallocAsync) with the release threshold raised, so a
  * context created and destroyed once per optimisation step re-uses the same physical memory.  This call hands the cached,

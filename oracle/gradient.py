@@ -76,3 +76,22 @@ def adjoint_position_gradient(lmax, k, pos, radii, eps_r, inc_fn, v, h=1e-5):
             dp = (inc_fn(pp) - inc_fn(pm)) / (2 * h)
             out[j, alpha] = mu @ (dA @ s.reshape(-1)) + mu @ dp.reshape(-1)
     return out, s, lam
+
+
+# ------------------------------------------------------------------------------ shape parameters of null-field T-matrices
+def _solve_J_shapes(lmax, k, pos, gen_fn, params, type_of, eps_r, p_inc, v):
+    from . import nullfield
+    t = np.stack([nullfield.nullfield_tmatrix(lmax, k, eps_r, gen_fn(p)) for p in params])
+    M = system.assemble_M(lmax, k, pos, t, type_of, False)
+    return np.sum(v * system.solve_forward(M, t, type_of, False, p_inc))
+
+
+def fd_shape_parameter(lmax, k, pos, gen_fn, params, type_of, eps_r, p_inc, v, which, h=1e-5):
+    """dJ/dp_which, J = v^T s, for a library of bodies of revolution gen_fn(p) (a geometry parameter enters only
+    through T): central difference of the full dense solve with the null-field T-matrices rebuilt at p +- h - the plain
+    definition of the derivative, no adjoint formula."""
+    pp, pm = np.array(params, dtype=float), np.array(params, dtype=float)
+    pp[which] += h
+    pm[which] -= h
+    return (_solve_J_shapes(lmax, k, pos, gen_fn, pp, type_of, eps_r, p_inc, v)
+            - _solve_J_shapes(lmax, k, pos, gen_fn, pm, type_of, eps_r, p_inc, v)) / (2 * h)

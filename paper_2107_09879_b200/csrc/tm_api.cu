@@ -1484,15 +1484,25 @@ int tm_release_cached_memory(void) {
   return cudaMemPoolTrimTo(pool, 0) == cudaSuccess ? TM_OK : TM_E_CUDA;
 }
 
-int tm_nullfield_tmatrix(int lmax, double k_b, double eps_r, int n_shapes, int n_nodes, const double* theta, const double* r,
-                         const double* dr_dtheta, const double* weight, tm_c64* T_out, void* cuda_stream) {
-  if (lmax < 1 || lmax > TM_MAX_LMAX || !(k_b > 0.0) || !(eps_r > 0.0) || !std::isfinite(eps_r) || n_shapes < 1 || n_nodes < 1 ||
-      !theta || !r || !dr_dtheta || !weight || !T_out)
-    return TM_E_INVALID;
-  int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return TM_E_CUDA; }
-  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
-  const size_t nn = (size_t)n_shapes * n_nodes, L = (size_t)tm_num_modes(lmax);
+}  // extern "C"
+
+namespace {
+// Richardson-extrapolated central difference of four T-matrices per shape: T(+h), T(-h), T(+h/2), T(-h/2)
+__global__ void k_nullfield_richardson(const double2* __restrict__ T4, double2* __restrict__ dT, size_t LL, size_t total, double inv_h) {
+  const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const size_t shape = i / LL, e = i % LL;
+  const double2* t = T4 + shape * 4 * LL + e;
+  const double2 a = t[0], b = t[LL], c = t[2 * LL], d = t[3 * LL];
+  // (4 D(h/2) - D(h)) / 3,  D(h) = (T(+h) - T(-h)) / 2h
+  dT[i] = make_double2((4.0 * (c.x - d.x) - 0.5 * (a.x - b.x)) * inv_h / 3.0, (4.0 * (c.y - d.y) - 0.5 * (a.y - b.y)) * inv_h / 3.0);
+}
+
+int nullfield_run(int lmax, double k_b, double eps_r, int n_shapes, int n_nodes, const double* theta, const double* r,
+                  const double* dr_dtheta, const double* weight, tm_c64* out, cudaStream_t st, double richardson_h) {
+  const bool deriv = richardson_h > 0.0;
+  const int n_gen = deriv ? 4 * n_shapes : n_shapes;
+  const size_t nn = (size_t)n_gen * n_nodes, L = (size_t)tm_num_modes(lmax), LL = L * L;
   {   // the surface must be star-shaped about the origin with finite nodes: r > 0, 0 < theta < pi
     std::vector<double> hr(nn), ht(nn);
     if (cudaMemcpy(hr.data(), r, nn * sizeof(double), is_device_ptr(r) ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost) != cudaSuccess ||
@@ -1502,23 +1512,56 @@ int tm_nullfield_tmatrix(int lmax, double k_b, double eps_r, int n_shapes, int n
     for (size_t i = 0; i < nn; ++i)
       if (!(hr[i] > 0.0) || !std::isfinite(hr[i]) || !(ht[i] > 0.0) || !(ht[i] < 3.14159265358979324)) return TM_E_INVALID;
   }
-  double* d_in = nullptr; double2* d_T = nullptr;
+  double* d_in = nullptr; double2* d_T = nullptr; double2* d_dT = nullptr;
   if (tm_dev_alloc(&d_in, 4 * nn * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return TM_E_NOMEM; }
-  if (tm_dev_alloc(&d_T, n_shapes * L * L * sizeof(double2)) != cudaSuccess) { cudaGetLastError(); tm_dev_free(d_in); return TM_E_NOMEM; }
+  if (tm_dev_alloc(&d_T, n_gen * LL * sizeof(double2)) != cudaSuccess) { cudaGetLastError(); tm_dev_free(d_in); return TM_E_NOMEM; }
+  if (deriv && tm_dev_alloc(&d_dT, n_shapes * LL * sizeof(double2)) != cudaSuccess) {
+    cudaGetLastError(); tm_dev_free(d_in); tm_dev_free(d_T); return TM_E_NOMEM;
+  }
   const double* src[4] = {theta, r, dr_dtheta, weight};
   cudaError_t e = cudaSuccess;
   for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = copy_in(d_in + i * nn, src[i], nn * sizeof(double), st);
-  if (e == cudaSuccess) e = cudaMemsetAsync(d_T, 0, n_shapes * L * L * sizeof(double2), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_T, 0, n_gen * LL * sizeof(double2), st);
   if (e == cudaSuccess) {
-    nullfield::k_nullfield<<<dim3(n_shapes, 2 * lmax + 1), 256, 0, st>>>(lmax, k_b, k_b * std::sqrt(eps_r), n_nodes, d_in, d_in + nn,
-                                                                         d_in + 2 * nn, d_in + 3 * nn, d_T);
+    nullfield::k_nullfield<<<dim3(n_gen, 2 * lmax + 1), 256, 0, st>>>(lmax, k_b, k_b * std::sqrt(eps_r), n_nodes, d_in, d_in + nn,
+                                                                      d_in + 2 * nn, d_in + 3 * nn, d_T);
     e = cudaGetLastError();
   }
-  if (e == cudaSuccess) e = copy_out(T_out, d_T, n_shapes * L * L * sizeof(double2), st);
+  if (e == cudaSuccess && deriv) {
+    const size_t total = n_shapes * LL;
+    k_nullfield_richardson<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(d_T, d_dT, LL, total, 1.0 / richardson_h);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = copy_out(out, deriv ? d_dT : d_T, n_shapes * LL * sizeof(double2), st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  tm_dev_free(d_in); tm_dev_free(d_T);
+  tm_dev_free(d_in); tm_dev_free(d_T); tm_dev_free(d_dT);
   if (e != cudaSuccess) { cudaGetLastError(); return TM_E_CUDA; }
   return TM_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int tm_nullfield_tmatrix(int lmax, double k_b, double eps_r, int n_shapes, int n_nodes, const double* theta, const double* r,
+                         const double* dr_dtheta, const double* weight, tm_c64* T_out, void* cuda_stream) {
+  if (lmax < 1 || lmax > TM_MAX_LMAX || !(k_b > 0.0) || !(eps_r > 0.0) || !std::isfinite(eps_r) || n_shapes < 1 || n_nodes < 1 ||
+      !theta || !r || !dr_dtheta || !weight || !T_out)
+    return TM_E_INVALID;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return TM_E_CUDA; }
+  return nullfield_run(lmax, k_b, eps_r, n_shapes, n_nodes, theta, r, dr_dtheta, weight, T_out,
+                       reinterpret_cast<cudaStream_t>(cuda_stream), 0.0);
+}
+
+int tm_nullfield_dtmatrix(int lmax, double k_b, double eps_r, int n_shapes, int n_nodes, const double* theta, const double* r,
+                          const double* dr_dtheta, const double* weight, double h, tm_c64* dT_out, void* cuda_stream) {
+  if (lmax < 1 || lmax > TM_MAX_LMAX || !(k_b > 0.0) || !(eps_r > 0.0) || !std::isfinite(eps_r) || n_shapes < 1 || n_nodes < 1 ||
+      !theta || !r || !dr_dtheta || !weight || !dT_out || !(h > 0.0) || !std::isfinite(h))
+    return TM_E_INVALID;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return TM_E_CUDA; }
+  return nullfield_run(lmax, k_b, eps_r, n_shapes, n_nodes, theta, r, dr_dtheta, weight, dT_out,
+                       reinterpret_cast<cudaStream_t>(cuda_stream), h);
 }
 
 int tm_measure_fma_peak(int precision, double* tflops, void* cuda_stream) {

@@ -22,7 +22,7 @@ TM_KERNEL_AUTO, TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR, TM_KERNEL_SYM3D = 0, 1, 2
 EXPORTS = ["tm_create", "tm_set_tmatrices", "tm_set_incident", "tm_get_incident", "tm_solve", "tm_solve_adjoint",
            "tm_matvec", "tm_fields", "tm_workspace_bytes", "tm_set_workspace", "tm_set_kernel", "tm_get_kernel",
            "tm_kernel_time", "tm_pair_cost", "tm_measure_fma_peak", "tm_grad_tmatrix", "tm_grad_positions", "tm_mie_tmatrix_dR", "tm_mie_tmatrix",
-           "tm_nullfield_tmatrix",
+           "tm_nullfield_tmatrix", "tm_nullfield_dtmatrix",
            "tm_release_cached_memory", "tm_num_modes", "tm_last_error", "tm_destroy"]
 
 
@@ -93,6 +93,7 @@ def lib():
         L.tm_grad_positions.argtypes = [vp, vp, vp, vp, cd, vp]
         L.tm_mie_tmatrix_dR.argtypes = [ci, cd, cd, c64, vp]
         L.tm_nullfield_tmatrix.argtypes = [ci, cd, cd, ci, ci, vp, vp, vp, vp, vp, vp]
+        L.tm_nullfield_dtmatrix.argtypes = [ci, cd, cd, ci, ci, vp, vp, vp, vp, cd, vp, vp]
         L.tm_pair_cost.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(cd)]
         L.tm_measure_fma_peak.argtypes = [ci, ctypes.POINTER(cd), vp]
         L.tm_num_modes.argtypes = [ci]
@@ -152,6 +153,22 @@ def nullfield_tmatrix(lmax, k_b, eps_r, generatrices, stream=None):
     if rc != TM_OK:
         raise TmError(rc, "tm_nullfield_tmatrix failed")
     return out[0] if single else out
+
+
+def nullfield_dtmatrix(lmax, k_b, eps_r, generatrix_fn, params, h, stream=None):
+    """dT/dp of null-field T-matrices (tm_nullfield_dtmatrix).  generatrix_fn(p) -> (theta, r, dr, w) for parameter value p;
+    params: the parameter value of every shape.  Returns (n_shapes, L, L) complex128."""
+    gens = [generatrix_fn(p + d) for p in params for d in (h, -h, 0.5 * h, -0.5 * h)]
+    arr = [np.ascontiguousarray(np.stack([np.asarray(g[i], dtype=np.float64) for g in gens])) for i in range(4)]
+    n_nodes = arr[0].shape[1]
+    L = lib().tm_num_modes(lmax)
+    out = np.zeros((len(params), L, L), dtype=np.complex128)
+    rc = lib().tm_nullfield_dtmatrix(int(lmax), float(k_b), float(eps_r), len(params), n_nodes, arr[0].ctypes.data, arr[1].ctypes.data,
+                                     arr[2].ctypes.data, arr[3].ctypes.data, float(h), out.ctypes.data,
+                                     ctypes.c_void_p(stream) if stream else None)
+    if rc != TM_OK:
+        raise TmError(rc, "tm_nullfield_dtmatrix failed")
+    return out
 
 
 def measure_fma_peak(precision=TM_FP64, stream=None):

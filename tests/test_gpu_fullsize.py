@@ -81,6 +81,24 @@ def test_cfg2_full_solve_vs_dense_lu_golden(tm):
     s.close()
 
 
+@pytest.mark.parametrize("cfg,scale", [(2, None), (5, 64)])
+def test_energy_conservation_of_the_gpu_solution(tm, cfg, scale):
+    """Property that holds at any size (no oracle values): lossless Mie spheres under a unit plane wave scatter exactly what they
+    extinguish, C_ext = -(pi/k^2) Re p^H s = C_sca = (pi/k^2) (|s|^2 + Re s^H A s)  (Re s^H A s = s^H RgA s
+    because the Neumann part of A is Hermitian, identity S4b pinned in tests/test_oracle_vswf_translation.py).  The operator
+    product A s is the GPU all-pairs kernel; a wrong block, sign or missing pair breaks the balance at O(1)."""
+    w = W.config(cfg, scale=scale)
+    s = tm.solver_for_workload(w)
+    sol, info, rc = s.solve(1e-10, w["restart"], 4000)
+    assert rc == 0
+    p = s.get_incident()
+    u = s.matvec(sol, transpose=2)                                   # u = A s
+    c_ext = -(np.pi / w["k"] ** 2) * np.real(np.vdot(p, sol))
+    c_sca = (np.pi / w["k"] ** 2) * (np.real(np.vdot(sol, sol)) + np.real(np.vdot(sol, u)))
+    assert c_ext > 0 and abs(c_ext - c_sca) <= 1e-8 * c_ext
+    s.close()
+
+
 def test_cfg4_windows_are_independent_at_full_size(tm):
     """One 64x64 window solved alone vs. inside the 64-window batch: a few GMRES cycles give identical iterates."""
     w = W.config(4)

@@ -81,3 +81,40 @@ def test_cylinder_lattice_solve_vs_dense_lu(tm):
     assert rc == 0
     assert np.linalg.norm(sol - ref) / np.linalg.norm(ref) <= 1e-9
     s.close()
+
+
+def test_dtmatrix_against_differences_of_the_oracle(tm):
+    """tm_nullfield_dtmatrix (device Richardson difference of four generatrices) vs. the same derivative taken from the ORACLE's
+    T-matrices with another step (central difference, h = 1e-5: truncation ~1e-8 relative)."""
+    lmax, radii = 3, [0.12, 0.18]
+    fn = lambda r: W.generatrix_cylinder(r, 0.3, 32)           # noqa: E731
+    dT = tm.nullfield_dtmatrix(lmax, K, 4.0, fn, radii, 2e-3)
+    for d, r in zip(dT, radii):
+        ref = (onf.nullfield_tmatrix(lmax, K, 4.0, fn(r + 1e-5)) - onf.nullfield_tmatrix(lmax, K, 4.0, fn(r - 1e-5))) / 2e-5
+        assert maxrel(d, ref) <= 1e-6
+
+
+def test_cylinder_radius_gradient_through_the_adjoint_solve(tm):
+    """The paper's optimisation chain for its own meta-atoms: cylinder radii -> null-field T and dT/dR on
+    the device -> forward + adjoint GMRES -> tm_grad_tmatrix, against central differences of the oracle's dense solve."""
+    from oracle import gradient
+    lmax = 2
+    rng = np.random.default_rng(5)
+    pos = W.lattice(4, 4)
+    radii = np.array([0.11, 0.15, 0.19])
+    fn = lambda r: W.generatrix_cylinder(r, 0.3, 24)           # noqa: E731
+    type_of = rng.integers(0, 3, len(pos)).astype(np.int32)
+    v = W.complex_normal((len(pos), W.n_modes(lmax)), rng)
+    s = tm.Solver(pos, lmax, K)
+    s.set_tmatrices(tm.nullfield_tmatrix(lmax, K, 4.0, [fn(r) for r in radii]), type_of, False)
+    s.set_incident_plane(0.0, 0.0, 1.0, 0.0)
+    sol, _, rc = s.solve(1e-12, 50, 500)
+    lam, _, rc2 = s.solve_adjoint(v, 1e-12, 50, 500)
+    assert rc == 0 and rc2 == 0
+    g_site = s.grad_tmatrix(tm.nullfield_dtmatrix(lmax, K, 4.0, fn, radii, 2e-3), lam, sol)
+    p = incident.plane_wave_incident(lmax, K, pos, 0.0, 0.0, 1.0, 0.0)
+    for t in range(3):
+        g = np.sum(g_site[type_of == t])
+        ref = gradient.fd_shape_parameter(lmax, K, pos, fn, radii, type_of, 4.0, p, v, t)
+        assert abs(g - ref) <= 1e-6 * abs(ref)
+    s.close()

@@ -35,3 +35,18 @@ def test_adjoint_position_gradient_matches_finite_differences():
     for (j, a) in ((0, 0), (1, 2), (3, 1)):
         fd = gradient.fd_position(2, K, pos, radii, 4.0, inc, v, j, a)
         assert abs(g[j, a] - fd) <= 1e-6 * np.abs(g).max()
+
+
+def test_shape_parameter_derivative_reduces_to_the_mie_radius_derivative():
+    """fd_shape_parameter with spheres as the bodies of revolution = fd_radius with the closed-form Mie T-matrix (two
+    independent routes to T: null-field surface integrals vs. Lorenz-Mie)."""
+    rng = np.random.default_rng(3)
+    pos = W.random_cloud(3, seed=9)
+    radii = np.array([0.12, 0.2, 0.16])
+    p = incident.plane_wave_incident(2, K, pos, 0.2, 0.1, 1.0, 0.0)
+    v = rng.standard_normal(p.shape) + 1j * rng.standard_normal(p.shape)
+    fn = lambda r: W.generatrix_sphere(r, 32)                  # noqa: E731
+    for j in range(3):
+        a = gradient.fd_shape_parameter(2, K, pos, fn, radii, np.arange(3), 4.0, p, v, j, h=1e-6)
+        b = gradient.fd_radius(2, K, pos, radii, 4.0, p, v, j, h=1e-6)
+        assert abs(a - b) <= 1e-6 * abs(b)

@@ -111,6 +111,9 @@ def test_block_symmetries_S1_S2_S3_S4():
         Rg = tr.block(lmax, K, d, np.zeros(3), regular=True)
         Rgm = tr.block(lmax, K, -d, np.zeros(3), regular=True)
         assert np.abs(Rgm - Rg.conj().T).max() < 1e-13 * np.abs(Rg).max()          # S4: RgA_ij = RgA_ji^H
+        Ng, Ngm = (B - Rg) / 1j, (Bm - Rgm) / 1j                                   # A = RgA + i NgA (y_q in place of j_q)
+        assert np.abs(Ngm - Ng.conj().T).max() < 1e-13 * np.abs(Ng).max()          # S4b: NgA is Hermitian too, hence
+        #      Re(s^H A s) = s^H RgA s for the assembled operator: C_sca needs only the OUTGOING matvec (full-size GPU check)
         # S2: coplanar sparsity counts
         dc = np.array([0.7, -0.4, 0.0])
         Bc = tr.block(lmax, K, dc, np.zeros(3))
