@@ -12,7 +12,7 @@
 // and the wavefunctions in spherical components at phi = 0 (Eq. I6):
 //   Psi_{l,m,0} = g_l z_l [ i m pibar theta_hat - taubar phi_hat ] ,
 //   Psi_{l,m,1} = g_l { l(l+1) z_l/(kr) Pbar r_hat + [kr z_l]'/(kr) ( taubar theta_hat + i m pibar phi_hat ) } ,  g_l = [2l(l+1)]^{-1/2}.
-// One block per (shape, m): the node quantities are staged through shared memory 64 nodes at a time (thread = node), then
+// One block per (shape, m): the node quantities are staged through shared memory 32 nodes at a time (thread = node), then
 // thread = matrix entry accumulates B_rg and the Neumann part B_y (B_out = B_rg + i B_y) in registers in node order
 // (deterministic), and the block solves its (<= 12 x 12) system by Gauss-Jordan elimination with row equilibration and
 // partial pivoting.  Own code: shares nothing with oracle/nullfield.py, which integrates over the whole surface in 2-D.
@@ -22,7 +22,7 @@
 
 namespace nullfield {
 
-constexpr int NC = 64;                 // nodes per shared-memory stage
+constexpr int NC = 32;                 // nodes per shared-memory stage
 constexpr int NLM = TM_MAX_LMAX;       // l values per block (l0..lmax)
 constexpr int NBM = 2 * NLM;           // block dimension (l, p)
 
@@ -50,8 +50,40 @@ __device__ inline void sph_jy(int lmax, double x, double* j, double* y) {
   for (int q = 1; q < top; ++q) y[q + 1] = (2 * q + 1) * ix * y[q] - y[q - 1];
 }
 
+// j_l(z), l = 0..lmax+1, for complex z = k_s r (lossy scatterer medium): the same downward recurrence in complex arithmetic.
+__device__ __forceinline__ Cx<double> cdivd(Cx<double> a, Cx<double> b) {
+  if (fabs(b.re) >= fabs(b.im)) {                      // Smith's algorithm: no overflow / underflow of |b|^2
+    const double t = b.im / b.re, inv = 1.0 / (b.re + b.im * t);
+    return cx<double>((a.re + a.im * t) * inv, (a.im - a.re * t) * inv);
+  }
+  const double t = b.re / b.im, inv = 1.0 / (b.re * t + b.im);
+  return cx<double>((a.re * t + a.im) * inv, (a.im * t - a.re) * inv);
+}
+__device__ inline void sph_j_complex(int lmax, Cx<double> z, Cx<double>* j) {
+  const int top = lmax + 1;
+  const Cx<double> iz = cdivd(cx<double>(1.0, 0.0), z);
+  const double sa = sin(z.re), ca = cos(z.re), ch = cosh(z.im), sh = sinh(z.im);
+  const Cx<double> s = cx<double>(sa * ch, ca * sh), c = cx<double>(ca * ch, -sa * sh);
+  const Cx<double> j0 = cmul(s, iz), j1 = cmul(csub(cmul(s, iz), c), iz);
+  const int N = top + 24 + (int)sqrt(z.re * z.re + z.im * z.im);
+  Cx<double> fp1 = cx<double>(0.0, 0.0), f = cx<double>(1e-100, 0.0);
+  for (int n = N; n >= 1; --n) {
+    const Cx<double> t = cmul(iz, f);
+    const Cx<double> fm1 = cx<double>((2 * n + 1) * t.re - fp1.re, (2 * n + 1) * t.im - fp1.im);
+    fp1 = f; f = fm1;
+    if (n - 1 <= top) j[n - 1] = f;
+    if (fabs(f.re) + fabs(f.im) > 1e100) {
+      f.re *= 1e-100; f.im *= 1e-100; fp1.re *= 1e-100; fp1.im *= 1e-100;
+      for (int q = n - 1; q <= top; ++q) { j[q].re *= 1e-100; j[q].im *= 1e-100; }
+    }
+  }
+  const bool use0 = j0.re * j0.re + j0.im * j0.im >= j1.re * j1.re + j1.im * j1.im;
+  const Cx<double> scale = use0 ? cdivd(j0, j[0]) : cdivd(j1, j[1]);
+  for (int q = 0; q <= top; ++q) j[q] = cmul(j[q], scale);
+}
+
 struct Node {                          // per (node, l): radial triples (z, [x z]'/x, z/x) and angular functions at |m|
-  double jS[NLM], dS[NLM], qS[NLM];    // regular, scatterer medium   (x = k_s r)
+  Cx<double> jS[NLM], dS[NLM], qS[NLM];   // regular, scatterer medium (z = k_s r, complex for a lossy medium)
   double jB[NLM], dB[NLM], qB[NLM];    // regular, background         (x = k_b r)
   double yB[NLM], eB[NLM], pB[NLM];    // Neumann part of the outgoing function, background
   double P[NLM], PI[NLM], TAU[NLM];
@@ -80,8 +112,25 @@ __device__ __forceinline__ void comps(int l, int m, int p, double z, double d, d
   }
 }
 
+// the same with a complex radial triple (internal field of a lossy medium)
+__device__ __forceinline__ void comps_c(int l, int m, int p, Cx<double> z, Cx<double> d, Cx<double> q, double P, double PI, double TAU,
+                                        Cx<double>* out) {
+  const double g = rsqrt(2.0 * l * (l + 1));
+  if (p == 0) {
+    const double a = g * m * PI, b = -g * TAU;
+    out[0] = cx<double>(0.0, 0.0);
+    out[1] = cx<double>(-a * z.im, a * z.re);
+    out[2] = cx<double>(b * z.re, b * z.im);
+  } else {
+    const double a = g * l * (l + 1) * P, b = g * TAU, c = g * m * PI;
+    out[0] = cx<double>(a * q.re, a * q.im);
+    out[1] = cx<double>(b * d.re, b * d.im);
+    out[2] = cx<double>(-c * d.im, c * d.re);
+  }
+}
+
 __global__ void __launch_bounds__(256)
-k_nullfield(int lmax, double k_b, double k_s, int n_nodes, const double* __restrict__ theta, const double* __restrict__ rad,
+k_nullfield(int lmax, double k_b, Cx<double> k_s, int n_nodes, const double* __restrict__ theta, const double* __restrict__ rad,
             const double* __restrict__ drad, const double* __restrict__ wgt, double2* __restrict__ T_out) {
   __shared__ Node node[NC];
   __shared__ Cx<double> aug[NBM][2 * NBM];
@@ -94,7 +143,7 @@ k_nullfield(int lmax, double k_b, double k_s, int n_nodes, const double* __restr
   const bool is_entry = e < nb * nb;
   const int ra = is_entry ? e / nb : 0, cb = is_entry ? e % nb : 0;
   const int l_row = l0 + ra % nl, p_row = ra / nl, l_col = l0 + cb % nl, p_col = cb / nl;
-  const double ratio = k_s / k_b;
+  const Cx<double> ratio = cx<double>(k_s.re / k_b, k_s.im / k_b);
   Cx<double> b_rg = cx<double>(0.0, 0.0), b_y = cx<double>(0.0, 0.0);
   const size_t base = (size_t)shape * n_nodes;
 
@@ -107,14 +156,17 @@ k_nullfield(int lmax, double k_b, double k_s, int n_nodes, const double* __restr
       sincos(th, &st, &ct);
       double P[TM_MAX_LMAX + 1][TM_MAX_LMAX + 1], PI[TM_MAX_LMAX + 1][TM_MAX_LMAX + 1], TAU[TM_MAX_LMAX + 1][TM_MAX_LMAX + 1];
       ang_functions<TM_MAX_LMAX>(ct, st, P, PI, TAU);
-      double js[TM_MAX_LMAX + 2], ys[TM_MAX_LMAX + 2], jb[TM_MAX_LMAX + 2], yb[TM_MAX_LMAX + 2];
-      const double xs = k_s * r, xb = k_b * r;
-      sph_jy(lmax, xs, js, ys);
+      Cx<double> js[TM_MAX_LMAX + 2];
+      double jb[TM_MAX_LMAX + 2], yb[TM_MAX_LMAX + 2];
+      const Cx<double> xs = cx<double>(k_s.re * r, k_s.im * r);
+      const double xb = k_b * r;
+      sph_j_complex(lmax, xs, js);
       sph_jy(lmax, xb, jb, yb);
       Node& nd = node[e];
       for (int a = 0; a < nl; ++a) {
         const int l = l0 + a;
-        nd.jS[a] = js[l]; nd.dS[a] = js[l - 1] - l * js[l] / xs; nd.qS[a] = js[l] / xs;      // [x z_l]'/x = z_{l-1} - l z_l / x
+        const Cx<double> qs = cdivd(js[l], xs);
+        nd.jS[a] = js[l]; nd.dS[a] = cx<double>(js[l - 1].re - l * qs.re, js[l - 1].im - l * qs.im); nd.qS[a] = qs;   // [x z_l]'/x = z_{l-1} - l z_l / x
         nd.jB[a] = jb[l]; nd.dB[a] = jb[l - 1] - l * jb[l] / xb; nd.qB[a] = jb[l] / xb;
         nd.yB[a] = yb[l]; nd.eB[a] = yb[l - 1] - l * yb[l] / xb; nd.pB[a] = yb[l] / xb;
         nd.P[a] = P[l][am]; nd.PI[a] = PI[l][am]; nd.TAU[a] = TAU[l][am];
@@ -128,16 +180,17 @@ k_nullfield(int lmax, double k_b, double k_s, int n_nodes, const double* __restr
       for (int i = 0; i < cnt; ++i) {
         const Node& nd = node[i];
         Cx<double> U[3], Us[3], W[3], Ws[3];
-        comps(l_col, m, p_col, nd.jS[b], nd.dS[b], nd.qS[b], nd.P[b], nd.PI[b], nd.TAU[b], U);         // RPhi_{l'm p'}(k_s)
-        comps(l_col, m, 1 - p_col, nd.jS[b], nd.dS[b], nd.qS[b], nd.P[b], nd.PI[b], nd.TAU[b], Us);    // RPhi_{l'm 1-p'}(k_s)
+        comps_c(l_col, m, p_col, nd.jS[b], nd.dS[b], nd.qS[b], nd.P[b], nd.PI[b], nd.TAU[b], U);         // RPhi_{l'm p'}(k_s)
+        comps_c(l_col, m, 1 - p_col, nd.jS[b], nd.dS[b], nd.qS[b], nd.P[b], nd.PI[b], nd.TAU[b], Us);    // RPhi_{l'm 1-p'}(k_s)
         comps(l_row, -m, p_row, nd.jB[a], nd.dB[a], nd.qB[a], nd.P[a], nd.PI[a], nd.TAU[a], W);        // RPhi_{l,-m,p}(k_b)
         comps(l_row, -m, 1 - p_row, nd.jB[a], nd.dB[a], nd.qB[a], nd.P[a], nd.PI[a], nd.TAU[a], Ws);
         Cx<double> t1 = cross_dot_n(U, Ws, nd.n_r, nd.n_th), t2 = cross_dot_n(Us, W, nd.n_r, nd.n_th);
-        b_rg.re += t1.re + ratio * t2.re; b_rg.im += t1.im + ratio * t2.im;
+        t2 = cmul(ratio, t2);
+        b_rg.re += t1.re + t2.re; b_rg.im += t1.im + t2.im;
         comps(l_row, -m, p_row, nd.yB[a], nd.eB[a], nd.pB[a], nd.P[a], nd.PI[a], nd.TAU[a], W);        // Neumann part
         comps(l_row, -m, 1 - p_row, nd.yB[a], nd.eB[a], nd.pB[a], nd.P[a], nd.PI[a], nd.TAU[a], Ws);
-        t1 = cross_dot_n(U, Ws, nd.n_r, nd.n_th); t2 = cross_dot_n(Us, W, nd.n_r, nd.n_th);
-        b_y.re += t1.re + ratio * t2.re; b_y.im += t1.im + ratio * t2.im;
+        t1 = cross_dot_n(U, Ws, nd.n_r, nd.n_th); t2 = cmul(ratio, cross_dot_n(Us, W, nd.n_r, nd.n_th));
+        b_y.re += t1.re + t2.re; b_y.im += t1.im + t2.im;
       }
     }
   }

@@ -92,8 +92,8 @@ def lib():
         L.tm_grad_tmatrix.argtypes = [vp, vp, vp, vp, vp]
         L.tm_grad_positions.argtypes = [vp, vp, vp, vp, cd, vp]
         L.tm_mie_tmatrix_dR.argtypes = [ci, cd, cd, c64, vp]
-        L.tm_nullfield_tmatrix.argtypes = [ci, cd, cd, ci, ci, vp, vp, vp, vp, vp, vp]
-        L.tm_nullfield_dtmatrix.argtypes = [ci, cd, cd, ci, ci, vp, vp, vp, vp, cd, vp, vp]
+        L.tm_nullfield_tmatrix.argtypes = [ci, cd, c64, ci, ci, vp, vp, vp, vp, vp, vp]
+        L.tm_nullfield_dtmatrix.argtypes = [ci, cd, c64, ci, ci, vp, vp, vp, vp, cd, vp, vp]
         L.tm_pair_cost.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(cd)]
         L.tm_measure_fma_peak.argtypes = [ci, ctypes.POINTER(cd), vp]
         L.tm_num_modes.argtypes = [ci]
@@ -147,7 +147,7 @@ def nullfield_tmatrix(lmax, k_b, eps_r, generatrices, stream=None):
     n_shapes, n_nodes = arr[0].shape
     L = lib().tm_num_modes(lmax)
     out = np.zeros((n_shapes, L, L), dtype=np.complex128)
-    rc = lib().tm_nullfield_tmatrix(int(lmax), float(k_b), float(eps_r), n_shapes, n_nodes, arr[0].ctypes.data, arr[1].ctypes.data,
+    rc = lib().tm_nullfield_tmatrix(int(lmax), float(k_b), _c64(eps_r), n_shapes, n_nodes, arr[0].ctypes.data, arr[1].ctypes.data,
                                     arr[2].ctypes.data, arr[3].ctypes.data, out.ctypes.data,
                                     ctypes.c_void_p(stream) if stream else None)
     if rc != TM_OK:
@@ -163,7 +163,7 @@ def nullfield_dtmatrix(lmax, k_b, eps_r, generatrix_fn, params, h, stream=None):
     n_nodes = arr[0].shape[1]
     L = lib().tm_num_modes(lmax)
     out = np.zeros((len(params), L, L), dtype=np.complex128)
-    rc = lib().tm_nullfield_dtmatrix(int(lmax), float(k_b), float(eps_r), len(params), n_nodes, arr[0].ctypes.data, arr[1].ctypes.data,
+    rc = lib().tm_nullfield_dtmatrix(int(lmax), float(k_b), _c64(eps_r), len(params), n_nodes, arr[0].ctypes.data, arr[1].ctypes.data,
                                      arr[2].ctypes.data, arr[3].ctypes.data, float(h), out.ctypes.data,
                                      ctypes.c_void_p(stream) if stream else None)
     if rc != TM_OK:

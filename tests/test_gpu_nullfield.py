@@ -30,6 +30,18 @@ def test_sphere_is_mie(tm, lmax):
     assert maxrel(T, np.diag(tmatrix.mie_tmatrix_diag(lmax, K, 0.2, 4.0))) <= 1e-12
 
 
+def test_lossy_medium(tm):
+    """Complex permittivity (Im eps_r > 0, e^{-i omega t}): complex k_s, Bessel functions of complex argument."""
+    eps = 12.0 + 0.8j
+    T = tm.nullfield_tmatrix(4, K, eps, W.generatrix_sphere(0.15, 48))
+    assert maxrel(T, np.diag(tmatrix.mie_tmatrix_diag(4, K, 0.15, eps))) <= 1e-12
+    assert maxrel(T, np.diag(tm.mie_tmatrix(4, K, 0.15, eps))) <= 1e-12
+    g = W.generatrix_cylinder(0.1, 0.25, 40)
+    assert maxrel(tm.nullfield_tmatrix(5, K, eps, g), onf.nullfield_tmatrix(5, K, eps, g)) <= 1e-9
+    g = W.generatrix_spheroid(0.12, 0.18, 64)
+    assert maxrel(tm.nullfield_tmatrix(3, K, 2.0 + 3.0j, g), onf.nullfield_tmatrix(3, K, 2.0 + 3.0j, g)) <= 1e-9
+
+
 @pytest.mark.parametrize("name,lmax,gen", [
     ("cylinder", 3, W.generatrix_cylinder(0.15, 0.3, 32)),
     ("cylinder", 6, W.generatrix_cylinder(0.12, 0.35, 43)),          # 129 nodes: three stages, ragged tail
@@ -54,7 +66,7 @@ def test_library_of_shapes_in_one_call(tm):
 
 def test_invalid_arguments(tm):
     g = W.generatrix_sphere(0.2, 8)
-    for bad in ((0, K, 4.0, g), (7, K, 4.0, g), (3, K, -1.0, g), (3, K, 4.0, (g[0], -g[1], g[2], g[3])),
+    for bad in ((0, K, 4.0, g), (7, K, 4.0, g), (3, K, -1.0, g), (3, K, 0.0, g), (3, K, 4.0 - 1.0j, g), (3, K, 4.0, (g[0], -g[1], g[2], g[3])),
                 (3, K, 4.0, (g[0] + 4.0, g[1], g[2], g[3]))):
         with pytest.raises(tm.TmError):
             tm.nullfield_tmatrix(*bad)

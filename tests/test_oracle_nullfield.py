@@ -26,6 +26,17 @@ def test_sphere_reproduces_lorenz_mie():
         assert np.abs(T - np.diag(d)).max() <= 1e-12 * np.abs(d).max()
 
 
+def test_lossy_sphere_reproduces_lorenz_mie_and_absorbs():
+    eps = 12.0 + 0.8j
+    T = nf.nullfield_tmatrix(3, K, eps, W.generatrix_sphere(0.15, 48))
+    d = tmatrix.mie_tmatrix_diag(3, K, 0.15, eps)
+    assert np.abs(T - np.diag(d)).max() <= 1e-12 * np.abs(d).max()
+    Tc = nf.nullfield_tmatrix(6, K, eps, W.generatrix_spheroid(0.12, 0.18, 64))
+    S = np.eye(len(Tc)) + 2.0 * Tc
+    ev = np.linalg.eigvalsh(np.eye(len(Tc)) - S.conj().T @ S)        # absorbed power is non-negative for every incident field
+    assert ev.min() >= -1e-6 and ev.max() > 1e-3
+
+
 def test_printed_forms_fail_the_mie_limit():
     """Reading R18: the printed minus sign; reading R19: T = -P Q^{-1} with P the OUTGOING matrix as printed."""
     gen = W.generatrix_sphere(0.2, 48)
