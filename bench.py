@@ -485,21 +485,71 @@ def run_nullfield(args):
     ts = []
     for _ in range(5):
         t0 = time.perf_counter()
-        T = libtm.nullfield_tmatrix(lmax, W.K_B, 4.0, gens)
+        T = libtm.nullfield_tmatrix(lmax, W.K_B, 4.0, gens, lmax_internal=args.lmax_internal)
         ts.append(time.perf_counter() - t0)
     n = T.shape[1]
     S = np.eye(n)[None] + 2.0 * T
     unit = float(np.abs(S @ np.conj(np.swapaxes(S, 1, 2)) - np.eye(n)[None]).max())
-    out = {"mode": "nullfield", "lmax": lmax, "L": n, "n_shapes": n_shapes, "nodes_per_shape": 3 * n_panel,
+    out = {"mode": "nullfield", "lmax": lmax, "lmax_internal": args.lmax_internal or lmax, "L": n, "n_shapes": n_shapes, "nodes_per_shape": 3 * n_panel,
            "call_ms_median_incl_copies": 1e3 * float(np.median(ts)), "shapes_per_s": n_shapes / float(np.median(ts)),
            "max_unitarity_defect": unit}
     if not args.no_cpu_baseline:
         from oracle import nullfield as onf
         t0 = time.perf_counter()
-        ref = onf.nullfield_tmatrix(lmax, W.K_B, 4.0, gens[100])
+        ref = onf.nullfield_tmatrix(lmax, W.K_B, 4.0, gens[100], lmax_internal=args.lmax_internal or None)
         out.update(oracle_seconds_per_shape=time.perf_counter() - t0,
                    max_rel_error_vs_oracle=float(np.abs(T[100] - ref).max() / np.abs(ref).max()))
     print(json.dumps(out), flush=True)
+
+
+def run_paper_case(args):
+    """Recorded run (not the contract line): the paper's own largest single-GPU case end to end on its own kind of meta-atom
+    (workloads.paper_lens: 56 x 56 silicon cylinders, lmax 6; 1-1.5 h on a V100): null-field T-matrices of the
+    radius library -> coupled solve to the paper's residual 1e-6 -> E field on the focal plane."""
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2107_09879_b200 import libtm
+    lmax = args.lmax or 6
+    w = W.paper_lens(args.scale or 56)
+    N = w["pos"].shape[0]
+    prec = {"fp64": libtm.TM_FP64, "fp32": libtm.TM_FP32, "mixed": libtm.TM_MIXED}[args.precision]
+    libtm.nullfield_tmatrix(lmax, w["k"], w["eps_r"], W.generatrix_cylinder(w["radii"][0], w["height"], 8))      # module load
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    gens = [W.generatrix_cylinder(r, w["height"], 64) for r in w["radii"]]
+    T = libtm.nullfield_tmatrix(lmax, w["k"], w["eps_r"], gens, lmax_internal=args.lmax_internal)
+    t1 = time.perf_counter()
+    s = libtm.Solver(w["pos"], lmax, w["k"], precision=prec)
+    r_enc = np.sqrt(w["radii"] ** 2 + (0.5 * w["height"]) ** 2)
+    s.set_tmatrices(T, w["type_of"], False, r_enclosing=r_enc)
+    s.set_incident_plane(0.0, 0.0, 1.0, 0.0)
+    t2 = time.perf_counter()
+    sol, info, rc = s.solve(args.tol or 1e-6, args.restart or 50, args.max_iter or 5000)
+    t3 = time.perf_counter()
+    g = (np.arange(64) - 31.5) * (10.0 / 64)
+    X, Y = np.meshgrid(g, g)
+    pts = np.stack([X.ravel(), Y.ravel(), np.full(X.size, w["focal"])], axis=1)
+    E = s.fields(pts, sol) + s.fields(pts, sol, libtm.TM_FIELD_E_INC)
+    t4 = time.perf_counter()
+    u = s.matvec(sol, transpose=2)
+    p = s.get_incident()
+    ext = -float(np.real(np.vdot(p, sol)))
+    sca = float(np.real(np.vdot(sol, sol)) + np.real(np.vdot(sol, u)))
+    n = T.shape[1]
+    S = np.eye(n)[None] + 2.0 * T
+    I2 = np.sum(np.abs(E) ** 2, axis=1).reshape(64, 64)
+    ap_ms, ap_launches, _ = s.kernel_time(reset=False)
+    print(json.dumps({"mode": "paper_case", "workload": w["name"], "n_scat": N, "lmax": lmax, "L": n, "n_types": len(gens),
+                      "lmax_internal": args.lmax_internal or lmax, "precision": args.precision, "tmatrix_seconds": t1 - t0, "setup_seconds": t2 - t1, "solve_seconds": t3 - t2,
+                      "fields_seconds": t4 - t3, "total_seconds": t4 - t0, "iterations": info[0].iterations,
+                      "matvecs": info[0].matvecs, "rel_residual": info[0].rel_residual, "converged": rc == 0,
+                      "allpairs_ms_per_launch": ap_ms / max(1, ap_launches), "kernel": s.get_kernel(),
+                      "library_unitarity_defect": float(np.abs(S @ np.conj(np.swapaxes(S, 1, 2)) - np.eye(n)[None]).max()),
+                      "energy_balance": {"extinction": ext, "scattering": sca, "rel_defect": abs(ext - sca) / abs(ext)},
+                      "focal_plane": {"peak_intensity_over_incident": float(I2.max()),
+                                      "peak_offset_wavelengths": [float(X.ravel()[I2.argmax()]), float(Y.ravel()[I2.argmax()])]}}),
+          flush=True)
+    s.close()
 
 
 def main():
@@ -509,12 +559,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2")
-    ap.add_argument("--mode", default="full", choices=["full", "matvec", "nyquist", "gradient", "nullfield"],
+    ap.add_argument("--mode", default="full", choices=["full", "matvec", "nyquist", "gradient", "nullfield", "paper_case"],
                     help="matvec: time operator applications only; nyquist: recorded run of the window decomposition")
     ap.add_argument("--group", type=int, default=16, help="nyquist mode: samples per group side")
     ap.add_argument("--padding", type=float, default=4.0, help="nyquist mode: padding in wavelengths")
     ap.add_argument("--kernel", default="auto", choices=["auto", "general", "coplanar", "sym3d"], help="force the all-pairs kernel variant")
     ap.add_argument("--lmax", type=int, default=None, help="override the VSWF truncation of a Mie config (lmax 6 = the paper's, PAPER.md:271)")
+    ap.add_argument("--lmax-internal", type=int, default=0,
+                    help="paper_case / nullfield modes: internal truncation of the null-field method (0 = lmax, the paper's setting)")
     ap.add_argument("--scale", type=int, default=None, help="lattice side override (parity-size runs)")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"],
                     help="mixed: GMRES with iterative refinement (fp32 Krylov cycles, fp64 iterate and true residual)")
@@ -545,6 +597,9 @@ def main():
     if args.mode == "nullfield":
         if rank == 0:
             run_nullfield(args)
+    elif args.mode == "paper_case":
+        if rank == 0:
+            run_paper_case(args)
     elif args.mode == "nyquist":
         if rank == 0:
             run_nyquist(args, w)

@@ -215,13 +215,17 @@ int tm_mie_tmatrix(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64 *ou
  * discretization" of the surface integrals: per shape n_nodes quadrature nodes theta[i] in (0, pi), r[i] > 0,
  * dr_dtheta[i] and the quadrature weight[i] in theta (e.g. Gauss-Legendre per smooth panel of the generatrix; the phi
  * integral is done analytically: T is block diagonal in m).  All four arrays [n_shapes][n_nodes], host or device.
+ *   lmax_internal  truncation of the field expansions INSIDE the method (surface-field and test functions): the block
+ *              systems are built and solved with l <= lmax_internal and the rows / columns with l <= lmax are returned.
+ *              0 or lmax = the paper's setting (everything at lmax = 6); up to 12.  For the paper's tall
+ *              silicon cylinders the lmax-6 result is far from converged near resonances
  *   eps_r      complex relative permittivity of the scatterer against the background, as in tm_mie_tmatrix (time convention
  *              e^{-i omega t}: Im eps_r >= 0 is a lossy medium; negative real eps_r and Im eps_r < 0 are refused)
  *   T_out      [n_shapes][L][L] row-major, s = T a, flat mode order R1 - the `T` of tm_set_tmatrices(diag_only = 0);
  *              host or device, fully written (zeros outside the m = m' blocks)
  * One launch for all shapes (a library of radii / heights is one call); synchronises cuda_stream before returning.
- * Errors: TM_E_INVALID (sizes, lmax > 6, eps_r = 0 / negative real / Im < 0, r <= 0, theta outside (0, pi)), TM_E_CUDA, TM_E_NOMEM. */
-int tm_nullfield_tmatrix(int lmax, double k_b, tm_c64 eps_r, int n_shapes, int n_nodes, const double *theta, const double *r,
+ * Errors: TM_E_INVALID (sizes, lmax > 6, lmax_internal not 0 and outside [lmax, 12], eps_r = 0 / negative real / Im < 0, r <= 0, theta outside (0, pi)), TM_E_CUDA, TM_E_NOMEM. */
+int tm_nullfield_tmatrix(int lmax, int lmax_internal, double k_b, tm_c64 eps_r, int n_shapes, int n_nodes, const double *theta, const double *r,
                          const double *dr_dtheta, const double *weight, tm_c64 *T_out, void *cuda_stream);
 
 /* d T / d(shape parameter) of the null-field T-matrix ("T_j depends on the geometry parameters of scatterer
@@ -230,7 +234,7 @@ int tm_nullfield_tmatrix(int lmax, double k_b, tm_c64 eps_r, int n_shapes, int n
  * the same launch as tm_nullfield_tmatrix and combines them on the device into the Richardson-extrapolated central
  * difference (4 D(h/2) - D(h)) / 3, D(h) = (T(p+h) - T(p-h)) / 2h  (error O(h^4)).  A stated deviation from an analytic
  * dT/dp, like tm_mie_tmatrix_dR.  dT_out [n_shapes][L][L], host or device.  Errors as tm_nullfield_tmatrix, and h <= 0. */
-int tm_nullfield_dtmatrix(int lmax, double k_b, tm_c64 eps_r, int n_shapes, int n_nodes, const double *theta, const double *r,
+int tm_nullfield_dtmatrix(int lmax, int lmax_internal, double k_b, tm_c64 eps_r, int n_shapes, int n_nodes, const double *theta, const double *r,
                           const double *dr_dtheta, const double *weight, double h, tm_c64 *dT_out, void *cuda_stream);
 
 /* Memory (the solver state is what limits the problem size on one GPU).  All device memory of the

@@ -62,14 +62,18 @@ def surface_matrices(lmax, k_b, k_s, gen, n_phi=None, printed=False):
     return out[0], out[1]
 
 
-def nullfield_tmatrix(lmax, k_b, eps_r, gen, n_phi=None, printed=False):
+def nullfield_tmatrix(lmax, k_b, eps_r, gen, n_phi=None, printed=False, lmax_internal=None):
     """T (L, L) of a homogeneous non-magnetic scatterer of relative permittivity eps_r (vs. the background) bounded by
-    the surface of revolution `gen`; s = T a in flat mode order (reading R1)."""
+    the surface of revolution `gen`; s = T a in flat mode order (reading R1).  lmax_internal > lmax: the method is run
+    with all expansions truncated at lmax_internal and the block of the modes l <= lmax is returned (the paper uses
+    lmax_internal = lmax = 6, PAPER.md:271)."""
     k_s = k_b * np.sqrt(eps_r + 0j)
     if abs(k_s.imag) == 0.0:
         k_s = k_s.real
-    b_rg, b_out = surface_matrices(lmax, k_b, k_s, gen, n_phi, printed)
-    return -np.linalg.solve(b_out.T, b_rg.T).T
+    li = lmax_internal or lmax
+    b_rg, b_out = surface_matrices(li, k_b, k_s, gen, n_phi, printed)
+    t = -np.linalg.solve(b_out.T, b_rg.T).T
+    return t if li == lmax else sub_block(t, li, lmax)
 
 
 def sub_block(t, lmax_from, lmax_to):

@@ -1498,7 +1498,7 @@ __global__ void k_nullfield_richardson(const double2* __restrict__ T4, double2* 
   dT[i] = make_double2((4.0 * (c.x - d.x) - 0.5 * (a.x - b.x)) * inv_h / 3.0, (4.0 * (c.y - d.y) - 0.5 * (a.y - b.y)) * inv_h / 3.0);
 }
 
-int nullfield_run(int lmax, double k_b, tm_c64 eps_r, int n_shapes, int n_nodes, const double* theta, const double* r,
+int nullfield_run(int lmax, int l_int, double k_b, tm_c64 eps_r, int n_shapes, int n_nodes, const double* theta, const double* r,
                   const double* dr_dtheta, const double* weight, tm_c64* out, cudaStream_t st, double richardson_h) {
   const bool deriv = richardson_h > 0.0;
   const int n_gen = deriv ? 4 * n_shapes : n_shapes;
@@ -1524,7 +1524,7 @@ int nullfield_run(int lmax, double k_b, tm_c64 eps_r, int n_shapes, int n_nodes,
   if (e == cudaSuccess) e = cudaMemsetAsync(d_T, 0, n_gen * LL * sizeof(double2), st);
   if (e == cudaSuccess) {
     const cd ks = k_b * std::sqrt(cd(eps_r.re, eps_r.im));              // principal root: Im k_s >= 0 for a lossy medium
-    nullfield::k_nullfield<<<dim3(n_gen, 2 * lmax + 1), 256, 0, st>>>(lmax, k_b, cx<double>(ks.real(), ks.imag()), n_nodes, d_in, d_in + nn,
+    nullfield::k_nullfield<<<dim3(n_gen, 2 * lmax + 1), nullfield::NT, 0, st>>>(lmax, l_int, k_b, cx<double>(ks.real(), ks.imag()), n_nodes, d_in, d_in + nn,
                                                                       d_in + 2 * nn, d_in + 3 * nn, d_T);
     e = cudaGetLastError();
   }
@@ -1543,27 +1543,29 @@ int nullfield_run(int lmax, double k_b, tm_c64 eps_r, int n_shapes, int n_nodes,
 
 extern "C" {
 
-int tm_nullfield_tmatrix(int lmax, double k_b, tm_c64 eps_r, int n_shapes, int n_nodes, const double* theta, const double* r,
+int tm_nullfield_tmatrix(int lmax, int lmax_internal, double k_b, tm_c64 eps_r, int n_shapes, int n_nodes, const double* theta, const double* r,
                          const double* dr_dtheta, const double* weight, tm_c64* T_out, void* cuda_stream) {
-  if (lmax < 1 || lmax > TM_MAX_LMAX || !(k_b > 0.0) || !std::isfinite(eps_r.re) || !std::isfinite(eps_r.im) || (eps_r.re == 0.0 && eps_r.im == 0.0) || eps_r.im < 0.0 ||
+  if (lmax < 1 || lmax > TM_MAX_LMAX || (lmax_internal != 0 && (lmax_internal < lmax || lmax_internal > nullfield::NF_MAX_L)) ||
+      !(k_b > 0.0) || !std::isfinite(eps_r.re) || !std::isfinite(eps_r.im) || (eps_r.re == 0.0 && eps_r.im == 0.0) || eps_r.im < 0.0 ||
       (eps_r.im == 0.0 && eps_r.re < 0.0) || n_shapes < 1 || n_nodes < 1 ||
       !theta || !r || !dr_dtheta || !weight || !T_out)
     return TM_E_INVALID;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return TM_E_CUDA; }
-  return nullfield_run(lmax, k_b, eps_r, n_shapes, n_nodes, theta, r, dr_dtheta, weight, T_out,
+  return nullfield_run(lmax, lmax_internal > 0 ? lmax_internal : lmax, k_b, eps_r, n_shapes, n_nodes, theta, r, dr_dtheta, weight, T_out,
                        reinterpret_cast<cudaStream_t>(cuda_stream), 0.0);
 }
 
-int tm_nullfield_dtmatrix(int lmax, double k_b, tm_c64 eps_r, int n_shapes, int n_nodes, const double* theta, const double* r,
+int tm_nullfield_dtmatrix(int lmax, int lmax_internal, double k_b, tm_c64 eps_r, int n_shapes, int n_nodes, const double* theta, const double* r,
                           const double* dr_dtheta, const double* weight, double h, tm_c64* dT_out, void* cuda_stream) {
-  if (lmax < 1 || lmax > TM_MAX_LMAX || !(k_b > 0.0) || !std::isfinite(eps_r.re) || !std::isfinite(eps_r.im) || (eps_r.re == 0.0 && eps_r.im == 0.0) || eps_r.im < 0.0 ||
+  if (lmax < 1 || lmax > TM_MAX_LMAX || (lmax_internal != 0 && (lmax_internal < lmax || lmax_internal > nullfield::NF_MAX_L)) ||
+      !(k_b > 0.0) || !std::isfinite(eps_r.re) || !std::isfinite(eps_r.im) || (eps_r.re == 0.0 && eps_r.im == 0.0) || eps_r.im < 0.0 ||
       (eps_r.im == 0.0 && eps_r.re < 0.0) || n_shapes < 1 || n_nodes < 1 ||
       !theta || !r || !dr_dtheta || !weight || !dT_out || !(h > 0.0) || !std::isfinite(h))
     return TM_E_INVALID;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return TM_E_CUDA; }
-  return nullfield_run(lmax, k_b, eps_r, n_shapes, n_nodes, theta, r, dr_dtheta, weight, dT_out,
+  return nullfield_run(lmax, lmax_internal > 0 ? lmax_internal : lmax, k_b, eps_r, n_shapes, n_nodes, theta, r, dr_dtheta, weight, dT_out,
                        reinterpret_cast<cudaStream_t>(cuda_stream), h);
 }
 

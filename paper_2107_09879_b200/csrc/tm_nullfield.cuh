@@ -12,9 +12,9 @@
 // and the wavefunctions in spherical components at phi = 0 (Eq. I6):
 //   Psi_{l,m,0} = g_l z_l [ i m pibar theta_hat - taubar phi_hat ] ,
 //   Psi_{l,m,1} = g_l { l(l+1) z_l/(kr) Pbar r_hat + [kr z_l]'/(kr) ( taubar theta_hat + i m pibar phi_hat ) } ,  g_l = [2l(l+1)]^{-1/2}.
-// One block per (shape, m): the node quantities are staged through shared memory 32 nodes at a time (thread = node), then
+// One block per (shape, m): the node quantities are staged through shared memory 16 nodes at a time (thread = node), then
 // thread = matrix entry accumulates B_rg and the Neumann part B_y (B_out = B_rg + i B_y) in registers in node order
-// (deterministic), and the block solves its (<= 12 x 12) system by Gauss-Jordan elimination with row equilibration and
+// (deterministic), and the block solves its (<= 24 x 24) system by Gauss-Jordan elimination with row equilibration and
 // partial pivoting.  Own code: shares nothing with oracle/nullfield.py, which integrates over the whole surface in 2-D.
 #pragma once
 #include "tm_common.cuh"
@@ -22,9 +22,11 @@
 
 namespace nullfield {
 
-constexpr int NC = 32;                 // nodes per shared-memory stage
-constexpr int NLM = TM_MAX_LMAX;       // l values per block (l0..lmax)
+constexpr int NF_MAX_L = 12;           // largest INTERNAL truncation (the retained lmax is <= TM_MAX_LMAX)
+constexpr int NC = 16;                 // nodes per shared-memory stage
+constexpr int NLM = NF_MAX_L;          // l values per block (l0..l_int)
 constexpr int NBM = 2 * NLM;           // block dimension (l, p)
+constexpr int NT = NBM * NBM;          // threads per block = matrix entries of the largest block (576)
 
 // j_l(x), y_l(x), l = 0..lmax+1 (x > 0): j by Miller's downward recurrence normalised with the larger of j_0 / j_1
 // (upward recurrence loses j_l for x < l), y upward (stable).
@@ -129,15 +131,17 @@ __device__ __forceinline__ void comps_c(int l, int m, int p, Cx<double> z, Cx<do
   }
 }
 
-__global__ void __launch_bounds__(256)
-k_nullfield(int lmax, double k_b, Cx<double> k_s, int n_nodes, const double* __restrict__ theta, const double* __restrict__ rad,
+// The surface integrals are truncated at l_int >= lmax (the INTERNAL truncation: field expansions inside the method); the
+// block system is solved at that size and the rows / columns with l <= lmax are written.  l_int = lmax is the paper's setting.
+__global__ void __launch_bounds__(NT)
+k_nullfield(int lmax, int l_int, double k_b, Cx<double> k_s, int n_nodes, const double* __restrict__ theta, const double* __restrict__ rad,
             const double* __restrict__ drad, const double* __restrict__ wgt, double2* __restrict__ T_out) {
   __shared__ Node node[NC];
   __shared__ Cx<double> aug[NBM][2 * NBM];
   __shared__ Cx<double> fac[NBM];
   __shared__ int piv;
   const int shape = blockIdx.x, m = (int)blockIdx.y - lmax, am = m < 0 ? -m : m;
-  const int l0 = am > 1 ? am : 1, nl = lmax - l0 + 1, nb = 2 * nl;
+  const int l0 = am > 1 ? am : 1, nl = l_int - l0 + 1, nb = 2 * nl;
   const int L = 2 * lmax * (lmax + 2), LH = L / 2;
   const int e = threadIdx.x;
   const bool is_entry = e < nb * nb;
@@ -154,14 +158,14 @@ k_nullfield(int lmax, double k_b, Cx<double> k_s, int n_nodes, const double* __r
       const double th = theta[base + c0 + e], r = rad[base + c0 + e], dr = drad[base + c0 + e], w = wgt[base + c0 + e];
       double st, ct;
       sincos(th, &st, &ct);
-      double P[TM_MAX_LMAX + 1][TM_MAX_LMAX + 1], PI[TM_MAX_LMAX + 1][TM_MAX_LMAX + 1], TAU[TM_MAX_LMAX + 1][TM_MAX_LMAX + 1];
-      ang_functions<TM_MAX_LMAX>(ct, st, P, PI, TAU);
-      Cx<double> js[TM_MAX_LMAX + 2];
-      double jb[TM_MAX_LMAX + 2], yb[TM_MAX_LMAX + 2];
+      double P[NF_MAX_L + 1][NF_MAX_L + 1], PI[NF_MAX_L + 1][NF_MAX_L + 1], TAU[NF_MAX_L + 1][NF_MAX_L + 1];
+      ang_functions<NF_MAX_L>(ct, st, P, PI, TAU);
+      Cx<double> js[NF_MAX_L + 2];
+      double jb[NF_MAX_L + 2], yb[NF_MAX_L + 2];
       const Cx<double> xs = cx<double>(k_s.re * r, k_s.im * r);
       const double xb = k_b * r;
-      sph_j_complex(lmax, xs, js);
-      sph_jy(lmax, xb, jb, yb);
+      sph_j_complex(l_int, xs, js);
+      sph_jy(l_int, xb, jb, yb);
       Node& nd = node[e];
       for (int a = 0; a < nl; ++a) {
         const int l = l0 + a;
@@ -237,7 +241,7 @@ k_nullfield(int lmax, double k_b, Cx<double> k_s, int n_nodes, const double* __r
     }
     __syncthreads();
   }
-  if (is_entry) {                                                          // T[ra][cb] = X^T[cb][ra] / pivot
+  if (is_entry && l_row <= lmax && l_col <= lmax) {                        // T[ra][cb] = X^T[cb][ra] / pivot
     const Cx<double> d = aug[cb][cb], x = aug[cb][nb + ra];
     const double inv = 1.0 / (d.re * d.re + d.im * d.im);
     const int row = p_row * LH + l_row * (l_row + 1) - 1 + m, col = p_col * LH + l_col * (l_col + 1) - 1 + m;

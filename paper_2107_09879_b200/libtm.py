@@ -92,8 +92,8 @@ def lib():
         L.tm_grad_tmatrix.argtypes = [vp, vp, vp, vp, vp]
         L.tm_grad_positions.argtypes = [vp, vp, vp, vp, cd, vp]
         L.tm_mie_tmatrix_dR.argtypes = [ci, cd, cd, c64, vp]
-        L.tm_nullfield_tmatrix.argtypes = [ci, cd, c64, ci, ci, vp, vp, vp, vp, vp, vp]
-        L.tm_nullfield_dtmatrix.argtypes = [ci, cd, c64, ci, ci, vp, vp, vp, vp, cd, vp, vp]
+        L.tm_nullfield_tmatrix.argtypes = [ci, ci, cd, c64, ci, ci, vp, vp, vp, vp, vp, vp]
+        L.tm_nullfield_dtmatrix.argtypes = [ci, ci, cd, c64, ci, ci, vp, vp, vp, vp, cd, vp, vp]
         L.tm_pair_cost.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(cd)]
         L.tm_measure_fma_peak.argtypes = [ci, ctypes.POINTER(cd), vp]
         L.tm_num_modes.argtypes = [ci]
@@ -138,7 +138,7 @@ def mie_tmatrix_dR(lmax, k_b, radius, eps_r):
     return out
 
 
-def nullfield_tmatrix(lmax, k_b, eps_r, generatrices, stream=None):
+def nullfield_tmatrix(lmax, k_b, eps_r, generatrices, stream=None, lmax_internal=0):
     """Null-field T-matrices of bodies of revolution (tm_nullfield_tmatrix).  `generatrices`: one (theta, r, dr, w) tuple
     or a list of them with equal node counts (workloads.generatrix_*).  Returns (L, L) or (n_shapes, L, L) complex128."""
     single = not isinstance(generatrices, list)
@@ -147,7 +147,7 @@ def nullfield_tmatrix(lmax, k_b, eps_r, generatrices, stream=None):
     n_shapes, n_nodes = arr[0].shape
     L = lib().tm_num_modes(lmax)
     out = np.zeros((n_shapes, L, L), dtype=np.complex128)
-    rc = lib().tm_nullfield_tmatrix(int(lmax), float(k_b), _c64(eps_r), n_shapes, n_nodes, arr[0].ctypes.data, arr[1].ctypes.data,
+    rc = lib().tm_nullfield_tmatrix(int(lmax), int(lmax_internal), float(k_b), _c64(eps_r), n_shapes, n_nodes, arr[0].ctypes.data, arr[1].ctypes.data,
                                     arr[2].ctypes.data, arr[3].ctypes.data, out.ctypes.data,
                                     ctypes.c_void_p(stream) if stream else None)
     if rc != TM_OK:
@@ -155,7 +155,7 @@ def nullfield_tmatrix(lmax, k_b, eps_r, generatrices, stream=None):
     return out[0] if single else out
 
 
-def nullfield_dtmatrix(lmax, k_b, eps_r, generatrix_fn, params, h, stream=None):
+def nullfield_dtmatrix(lmax, k_b, eps_r, generatrix_fn, params, h, stream=None, lmax_internal=0):
     """dT/dp of null-field T-matrices (tm_nullfield_dtmatrix).  generatrix_fn(p) -> (theta, r, dr, w) for parameter value p;
     params: the parameter value of every shape.  Returns (n_shapes, L, L) complex128."""
     gens = [generatrix_fn(p + d) for p in params for d in (h, -h, 0.5 * h, -0.5 * h)]
@@ -163,7 +163,7 @@ def nullfield_dtmatrix(lmax, k_b, eps_r, generatrix_fn, params, h, stream=None):
     n_nodes = arr[0].shape[1]
     L = lib().tm_num_modes(lmax)
     out = np.zeros((len(params), L, L), dtype=np.complex128)
-    rc = lib().tm_nullfield_dtmatrix(int(lmax), float(k_b), _c64(eps_r), len(params), n_nodes, arr[0].ctypes.data, arr[1].ctypes.data,
+    rc = lib().tm_nullfield_dtmatrix(int(lmax), int(lmax_internal), float(k_b), _c64(eps_r), len(params), n_nodes, arr[0].ctypes.data, arr[1].ctypes.data,
                                      arr[2].ctypes.data, arr[3].ctypes.data, float(h), out.ctypes.data,
                                      ctypes.c_void_p(stream) if stream else None)
     if rc != TM_OK:

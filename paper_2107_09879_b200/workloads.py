@@ -180,3 +180,21 @@ def generatrix_spheroid(a_xy, c_z, n=64):
     r = q ** -0.5
     dr = -0.5 * q ** -1.5 * 2.0 * s * c * (1.0 / a_xy ** 2 - 1.0 / c_z ** 2)
     return th, r, dr, w
+
+
+def paper_lens(n_side=56, n_types=32, focal_um=25.0):
+    """Stand-in for the paper's own single-GPU workload: silicon cylinders (n = 3.48) of height 940 nm
+    and radius 50-250 nm on a square lattice of period 1070 nm in air at wavelength 1550 nm; 56 x 56 sites = 60 um x 60 um,
+    "the largest single-GPU simulation" (1-1.5 h on a V100).  Lengths in wavelengths.  The paper picks each radius from the
+    phase curve of its periodic library (not available); here the hyperbolic lens phase -k (sqrt(rho^2 + f^2) - f) mod 2 pi
+    is mapped linearly onto the sorted radius library, which gives the same kind of layout (concentric zones of growing
+    radius).  Returns a dict with pos, type_of, radii, height, eps_r, pitch."""
+    lam_nm = 1550.0
+    pitch, height = 1070.0 / lam_nm, 940.0 / lam_nm
+    radii = np.linspace(50.0, 250.0, n_types) / lam_nm
+    pos = lattice(n_side, n_side, pitch)
+    f = focal_um * 1000.0 / lam_nm
+    phase = np.mod(-K_B * (np.sqrt(pos[:, 0] ** 2 + pos[:, 1] ** 2 + f * f) - f), 2.0 * np.pi)
+    type_of = np.minimum((phase / (2.0 * np.pi) * n_types).astype(np.int32), n_types - 1)
+    return dict(name=f"paper_lens{n_side}", k=K_B, pos=pos, type_of=type_of, radii=radii, height=height, eps_r=3.48 ** 2,
+                pitch=pitch, focal=f)

@@ -54,6 +54,19 @@ def test_matches_oracle_surface_quadrature(tm, name, lmax, gen):
     assert maxrel(T, ref) <= 1e-9
 
 
+@pytest.mark.parametrize("lmax,lint", [(2, 6), (3, 8), (6, 10), (6, 12), (1, 12)])
+def test_internal_truncation(tm, lmax, lint):
+    """Expansions inside the method carried to lmax_internal > lmax (blocks up to 24 x 24), block l <= lmax returned; the case
+    is the paper's own meta-atom: a silicon cylinder 940 nm tall, radius 205 nm at 1550 nm, where lmax 6 alone is far from
+    converged."""
+    g = W.generatrix_cylinder(204.84 / 1550, 940.0 / 1550, 48)
+    T = tm.nullfield_tmatrix(lmax, K, 3.48 ** 2, g, lmax_internal=lint)
+    ref = onf.nullfield_tmatrix(lmax, K, 3.48 ** 2, g, lmax_internal=lint)
+    assert maxrel(T, ref) <= 1e-8
+    if lmax == 6:
+        assert maxrel(T, onf.nullfield_tmatrix(6, K, 3.48 ** 2, g)) > 0.1       # the lmax-6-only result is a different matrix
+
+
 def test_library_of_shapes_in_one_call(tm):
     radii = [0.10, 0.14, 0.18, 0.22]
     gens = [W.generatrix_cylinder(r, 0.3, 24) for r in radii]
@@ -70,6 +83,9 @@ def test_invalid_arguments(tm):
                 (3, K, 4.0, (g[0] + 4.0, g[1], g[2], g[3]))):
         with pytest.raises(tm.TmError):
             tm.nullfield_tmatrix(*bad)
+    for li in (2, 13, -1):
+        with pytest.raises(tm.TmError):
+            tm.nullfield_tmatrix(3, K, 4.0, g, lmax_internal=li)
 
 
 def test_cylinder_lattice_solve_vs_dense_lu(tm):

@@ -61,6 +61,19 @@ def test_displaced_sphere_equals_translated_mie():
     assert np.abs(a - b).max() <= 1e-9
 
 
+def test_internal_truncation_converges_to_the_translated_mie_block():
+    """lmax_internal: the l <= 2 block of the displaced sphere computed with expansions up to 2 is off by the coupling to
+    higher orders; with the expansions carried to 6 it reproduces the exact (translated Lorenz-Mie) block."""
+    off, radius = 0.08, 0.2
+    gen = W.generatrix_sphere(radius, 64, offset=off)
+    c, o = np.array([0.0, 0.0, off]), np.zeros(3)
+    exact = nf.sub_block(translation.block(6, K, o, c, regular=True) @ np.diag(tmatrix.mie_tmatrix_diag(6, K, radius, 4.0))
+                         @ translation.block(6, K, c, o, regular=True), 6, 2)
+    coarse = np.abs(nf.nullfield_tmatrix(2, K, 4.0, gen) - exact).max()
+    fine = np.abs(nf.nullfield_tmatrix(2, K, 4.0, gen, lmax_internal=6) - exact).max()
+    assert coarse > 1e-4 and fine <= 1e-7 and fine < 1e-3 * coarse
+
+
 def test_spheroid_is_lossless_reciprocal_and_mirror_symmetric():
     lmax = 6
     T = nf.nullfield_tmatrix(lmax, K, 4.0, W.generatrix_spheroid(0.15, 0.22, 64))
