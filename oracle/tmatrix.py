@@ -1,7 +1,7 @@
 """Per-scatterer transition matrices (TEST INFRASTRUCTURE ONLY - see oracle/__init__.py).
 
 PAPER.md:254 (Eq. I9): s = T a.  The paper computes T by the null-field method for cylinders
-(out of scope); BASELINE.json's configs use homogeneous spheres, whose T is the
+(oracle/nullfield.py); BASELINE.json's configs use homogeneous spheres, whose T is the
 closed-form Lorenz-Mie result (reading R11): diagonal, independent of m,
     T_{l,p=0} = -b_l ,   T_{l,p=1} = -a_l ,
 with the Bohren-Huffman coefficients (size parameter x = k_b R, relative index m_r = sqrt(eps_r)):
