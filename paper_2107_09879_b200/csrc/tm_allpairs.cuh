@@ -101,8 +101,11 @@ TM_COP_SPEC(1, 0) TM_COP_SPEC(1, 1) TM_COP_SPEC(2, 0) TM_COP_SPEC(2, 1) TM_COP_S
 // Thread t handles target tile.tgt_start + t.  Sources of the tile's window are split into n_chunk contiguous
 // chunks (blockIdx.y) so that small problems still fill 148 SMs; each chunk is streamed through shared memory
 // SS sources at a time (positions + this half's d-values in the tilde basis x~ = i^p x).
+#ifndef TM_COP_MINBLOCKS
+#define TM_COP_MINBLOCKS 1       // resident blocks per SM the register allocation is asked to allow (experiments: 3)
+#endif
 template <typename R, int LMAX, int TJ, int SS>
-__global__ void __launch_bounds__(TJ)
+__global__ void __launch_bounds__(TJ, TM_COP_MINBLOCKS)
 k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
                     const TmTile* __restrict__ tiles, int n_scat, double k_over_pi, double inv_k,
                     const int* __restrict__ n_active, TmShift shift) {
