@@ -654,7 +654,7 @@ int ensure_gmres(tm_ctx* ctx, int restart) {
   const size_t o_h1 = take(nw * ldh * 16), o_h2 = take(nw * ldh * 16), o_R = take(nw * m * ldh * 16), o_cs = take(nw * m * 8),
                o_sn = take(nw * m * 16), o_g = take(nw * ldh * 16), o_y = take(nw * ldh * 16), o_nw = take(nw * 8),
                o_bn = take(nw * 8), o_in = take(nw * 8), o_b0 = take(nw * 8), o_rs = take(nw * 8), o_k = take(nw * 4), o_d = take(nw * 4),
-               o_na = take(4), o_part = take(ldh * nc * 16), o_np = take(nc * 8);
+               o_na = take(4), o_part = take(2 * ldh * nc * 16) /* two buffers: k_arnoldi_fused */, o_np = take(nc * 8);
   TM_CUDA(tm_dev_alloc(&ctx->gm.blob, off));
   TM_CUDA(cudaMemset(ctx->gm.blob, 0, off));
   char* b = reinterpret_cast<char*>(ctx->gm.blob);

@@ -46,13 +46,17 @@ k_arnoldi_fused(const Cx<R>* __restrict__ V, size_t stride, int j, Cx<R>* __rest
     }
     __syncthreads();
   }
+  // CGS2 with three grid barriers: the second projection of a chunk needs only that chunk of w after the first update, so
+  // it follows the update without a barrier; its partial sums go to a second buffer because slower blocks may still be
+  // reducing the first one.
+  double2* part2 = part + (size_t)S.ldh * n_chunks;
   dots_body<R, EPT>(V, stride, nvec, W, ch, c, n_chunks, part, 0, 1, s_w);
   grid.sync();
   axpy_body<R, EPT>(V, stride, nvec, S.h1, S.ldh, -1.0, W, ch, c, nullptr, part, n_chunks, win_chunk_ptr, s_dyn, s_n);
+  __syncthreads();
+  dots_body<R, EPT>(V, stride, nvec, W, ch, c, n_chunks, part2, 0, 1, s_w);
   grid.sync();
-  dots_body<R, EPT>(V, stride, nvec, W, ch, c, n_chunks, part, 0, 1, s_w);
-  grid.sync();
-  axpy_body<R, EPT>(V, stride, nvec, S.h2, S.ldh, -1.0, W, ch, c, normpart, part, n_chunks, win_chunk_ptr, s_dyn, s_n);
+  axpy_body<R, EPT>(V, stride, nvec, S.h2, S.ldh, -1.0, W, ch, c, normpart, part2, n_chunks, win_chunk_ptr, s_dyn, s_n);
   grid.sync();
   // Givens update (one warp per window) runs alongside the normalisation: every block recomputes its window's norm
   // from the chunk norms (same fixed order as the Givens warp), so no further barrier is needed.  A window that
