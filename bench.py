@@ -587,6 +587,17 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.workload == "paper_lens":        # the paper's own kind of layout (silicon cylinders, null-field T-matrices): nyquist mode
+        assert args.mode == "nyquist", "--workload paper_lens is for --mode nyquist (or use --mode paper_case)"
+        if rank == 0:
+            from paper_2107_09879_b200 import libtm
+            w = W.paper_lens(args.scale or 56)
+            lmax = args.lmax or 6
+            gens = [W.generatrix_cylinder(r, w["height"], 64) for r in w["radii"]]
+            w.update(lmax=lmax, t_kind="full_types", win_ptr=np.array([0, w["pos"].shape[0]], dtype=np.int32),
+                     t_full=libtm.nullfield_tmatrix(lmax, w["k"], w["eps_r"], gens, lmax_internal=args.lmax_internal or 10))
+            run_nyquist(args, w)
+        return
     name = args.workload[3:] if args.workload.startswith("cfg") else args.workload
     w = W.config(name if name == "3b" else int(name), scale=args.scale)
     if args.lmax is not None:
