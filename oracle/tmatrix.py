@@ -46,9 +46,3 @@ def mie_tmatrix_diag(lmax, k_b, radius, eps_r):
         a, b = mie_ab(l, x, m_r)
         t[idx] = -b if p == 0 else -a
     return t
-
-
-def random_unitary_s_tmatrix(U):
-    """Config 3 (BASELINE.json; reading R12): T = (S - I)/2 with S = U U^T for a given unitary U."""
-    S = U @ U.T
-    return (S - np.eye(U.shape[0])) / 2.0

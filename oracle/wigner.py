@@ -2,8 +2,9 @@
 
 PAPER.md:327 (Eq. I19).  The oracle uses the Racah single-sum formula with exact integer
 factorials (python ints / Fractions) and takes one square root at the end.  (The paper
-cites a recursion; the CUDA path's host tables use that recursion, the oracle
-deliberately does not.)
+cites a recursion, which neither side uses: the CUDA path's build-time generator
+csrc/gen_tables.py has its own, separately typed Racah sum in binomial form with mpmath square
+roots; nothing is shared or imported between the two.)
 """
 from fractions import Fraction
 from functools import lru_cache

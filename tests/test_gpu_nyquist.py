@@ -18,8 +18,7 @@ def tm():
     return libtm
 
 
-def rel(a, b):
-    return np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(b)
+from parity_metric import rel  # noqa: E402  (L2 AND per-(l,p)-block / per-point max error)
 
 
 def test_jinc_incident_matches_oracle(tm):

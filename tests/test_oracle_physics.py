@@ -192,7 +192,7 @@ def test_windows_are_independent():
 
 def test_c_matvec_against_dense():
     rng = np.random.default_rng(17)
-    for lmax, n, nw in [(1, 12, 1), (2, 30, 2), (3, 40, 3)]:
+    for lmax, n, nw in [(1, 12, 1), (2, 30, 2), (3, 40, 3), (4, 14, 2), (5, 10, 1), (6, 9, 2)]:
         w = W.cloud_workload(n, seed=18 + lmax, lmax=lmax, n_win=nw)
         L = n_modes(lmax)
         x = W.complex_normal((n, L), rng)
@@ -207,3 +207,38 @@ def test_c_matvec_against_dense():
     x = W.complex_normal((36, 30), rng)
     A = system.assemble_A(3, K, w["pos"])
     assert np.abs((A @ x.reshape(-1)).reshape(36, 30) - matvec.matvec_rows(3, K, w["pos"], x)).max() < 1e-12
+
+
+def test_H_field_is_the_curl_of_E():
+    """Pin of oracle/fields.py::zh_sca (reading R10; PAPER.md:284 Eq. I13 with curl Phi_p = k Phi_{1-p}, PAPER.md:230-234
+    Eq. I6b): Maxwell's curl E = i omega mu H = i k (Z_b H), with the curl of the ORACLE's own e_sca taken numerically
+    (4th-order central differences) near a 3-scatterer cloud.  A wrong sign of the -i, a missing p <-> 1-p swap, or a
+    wrong sum fails it."""
+    rng = np.random.default_rng(41)
+    lmax = 3
+    L = n_modes(lmax)
+    pos = np.array([[0.0, 0.0, 0.0], [0.7, 0.2, -0.3], [-0.4, 0.8, 0.5]])
+    s = W.complex_normal((3, L), rng)
+    h = 2e-3
+
+    def curl_E(x):
+        J = np.zeros((3, 3), dtype=complex)          # J[a, b] = d E_a / d x_b
+        for b in range(3):
+            e = np.zeros(3)
+            e[b] = h
+            f = lambda t: fields.e_sca(lmax, K, pos, s, x + t * e)[0]
+            J[:, b] = (8 * (f(1) - f(-1)) - (f(2) - f(-2))) / (12 * h)
+        return np.array([J[2, 1] - J[1, 2], J[0, 2] - J[2, 0], J[1, 0] - J[0, 1]])
+
+    swap = np.concatenate([np.arange(L // 2, L), np.arange(0, L // 2)])
+    for _ in range(4):
+        x = rng.uniform(-1.5, 1.5, 3) + np.array([0.3, -0.2, 1.9])
+        zh = fields.zh_sca(lmax, K, pos, s, x)[0]
+        ref = curl_E(x) / (1j * K)
+        scale = np.abs(ref).max()
+        assert np.abs(zh - ref).max() < 1e-6 * scale
+        assert np.abs(-zh - ref).max() > 0.5 * scale                      # the +i variant fails
+        # without the p <-> 1-p swap (-i sum s Phi_{lmp} = -i E) it fails too
+        assert np.abs(-1j * fields.e_sca(lmax, K, pos, s, x)[0] - ref).max() > 1e-2 * scale
+        # and it is the same sum as E with the coefficient halves exchanged: Z H[s] = -i E[s with p <-> 1-p]
+        assert np.abs(zh + 1j * fields.e_sca(lmax, K, pos, s[:, swap], x)[0]).max() < 1e-13 * scale

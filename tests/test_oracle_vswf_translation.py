@@ -81,6 +81,27 @@ def test_addition_theorem_pointwise():
         assert _addition_error(xw, 3, 12, xs, xd, pt) > 1e-2
 
 
+def test_addition_theorem_pointwise_source_rows_to_lmax6():
+    """Entries with BOTH l >= 4 and l' >= 4 (Eqs. I16-I18; the paper's truncation is lmax = 6,
+    PAPER.md:271): every source row l <= 6 of the translation matrix, expanded over destination columns l' <= 14,
+    must reproduce the outgoing wavefunction pointwise.  The entries (l, l') in [4, 6]^2 carry 1.5e-2 of a row's
+    value at this distance (asserted below), so a slip in a5 / b5 / the 3j symbols at high order fails the 1e-11 bound."""
+    rng = np.random.default_rng(55)
+    xs = rng.uniform(-1, 1, 3)
+    xd = xs + 0.9 * _unit(rng)
+    pt = xd + 0.05 * _unit(rng)
+    xi = tr.xi_matrix(14, K, xd - xs)
+    assert _addition_error(xi, 6, 14, xs, xd, pt) < 1e-11
+    # the high-order entries matter: zeroing the block l, l' in [4, 6] must break it
+    big = mode_list(14)
+    hi = np.array([4 <= l <= 6 for (l, m, p) in big])
+    xz = xi.copy()
+    xz[np.ix_(hi, hi)] = 0.0
+    assert _addition_error(xz, 6, 14, xs, xd, pt) > 1e-3
+    xr = tr.xi_matrix(14, K, xd - xs, regular=True)
+    assert _addition_error(xr, 6, 14, xs, xd, pt, regular_lhs=True) < 1e-11
+
+
 def _unit(rng):
     v = rng.standard_normal(3)
     return v / np.linalg.norm(v)
@@ -97,7 +118,7 @@ def test_printed_forms_fail():
 
 def test_block_symmetries_S1_S2_S3_S4():
     rng = np.random.default_rng(6)
-    for lmax in (2, 3):
+    for lmax in (2, 3, 4, 5, 6):
         L = n_modes(lmax)
         modes = mode_list(lmax)
         d = rng.uniform(0.6, 2.0) * _unit(rng)
@@ -118,7 +139,8 @@ def test_block_symmetries_S1_S2_S3_S4():
         dc = np.array([0.7, -0.4, 0.0])
         Bc = tr.block(lmax, K, dc, np.zeros(3))
         nz = int(np.sum(np.abs(Bc) > 1e-12 * np.abs(Bc).max()))
-        assert nz == {2: 124, 3: 442}[lmax]
+        if lmax <= 3:
+            assert nz == {2: 124, 3: 442}[lmax]
         par = np.array([(-1) ** (l + m + p) for (l, m, p) in modes])
         assert np.all((np.abs(Bc) > 1e-12 * np.abs(Bc).max()) <= (par[:, None] == par[None, :]))
         # axial displacement couples only m = m'
@@ -132,7 +154,7 @@ def test_blocks_many_equals_literal_block():
     D = rng.uniform(-2, 2, (6, 3))
     D[0] = [0.5, 0.0, 0.0]
     D[1] = [0.0, 0.0, -0.7]
-    for lmax in (1, 2, 3):
+    for lmax in (1, 2, 3, 5, 6):
         Bm = tr.blocks_many(lmax, K, D)
         for t in range(len(D)):
             B = tr.block(lmax, K, D[t], np.zeros(3))
