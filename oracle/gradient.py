@@ -57,10 +57,26 @@ def fd_position(lmax, k, pos, radii, eps_r, inc_fn, v, j, alpha, h=1e-5):
     return (_solve_J(lmax, k, pp, radii, eps_r, inc_fn(pp), v)[0] - _solve_J(lmax, k, pm, radii, eps_r, inc_fn(pm), v)[0]) / (2 * h)
 
 
+def dA_dposition(lmax, k, pos, j):
+    """d A / d x_{j,alpha}, alpha = x, y, z, assembled densely: (3, N L, N L).  Only the block row j (A_ji depends on
+    x_j - x_i) and the block column j (A_ij depends on x_i - x_j, hence the minus sign) are non-zero; the blocks are the
+    ANALYTIC derivative of the translation coefficients (translation.d_block)."""
+    from . import translation as tr
+    N, L = len(pos), n_modes(lmax)
+    out = np.zeros((3, N * L, N * L), dtype=complex)
+    for i in range(N):
+        if i == j:
+            continue
+        out[:, j * L:(j + 1) * L, i * L:(i + 1) * L] = tr.d_block(lmax, k, pos[j], pos[i])
+        out[:, i * L:(i + 1) * L, j * L:(j + 1) * L] = -tr.d_block(lmax, k, pos[i], pos[j])
+    return out
+
+
 def adjoint_position_gradient(lmax, k, pos, radii, eps_r, inc_fn, v, h=1e-5):
     """All dJ/dx_{j,alpha} through ONE adjoint solve: lambda^T T (dA/dx_{j,alpha}) s + lambda^T T da^(0)/dx_{j,alpha}
-    (Eq. IV6 with Omega = T^{-1} M; dOmega/dq = -dA/dq).  dA/dq and da^(0)/dq by central differences of the oracle's own
-    dense assembly (the paper differentiates Eq. I23 analytically; numerically the same matrix).  Returns (N, 3)."""
+    (Eq. IV6 with Omega = T^{-1} M; dOmega/dq = -dA/dq).  dA/dq is the analytic derivative of Eq. I23's off-diagonal blocks
+    (dA_dposition; "can be computed analytically"); da^(0)/dq, which is not part of Omega, by central
+    differences of inc_fn.  Returns (N, 3).  Pinned by fd_position (central differences of the whole dense solve)."""
     p_inc = inc_fn(pos)
     J, s, M, t = _solve_J(lmax, k, pos, radii, eps_r, p_inc, v)
     lam = system.solve_adjoint(M, v)
@@ -68,13 +84,13 @@ def adjoint_position_gradient(lmax, k, pos, radii, eps_r, inc_fn, v, h=1e-5):
     mu = (t * lam).reshape(-1)                                     # T^T lambda (T diagonal)
     out = np.zeros((N, 3), dtype=complex)
     for j in range(N):
+        dA = dA_dposition(lmax, k, pos, j)
         for alpha in range(3):
             pp, pm = np.array(pos, dtype=float), np.array(pos, dtype=float)
             pp[j, alpha] += h
             pm[j, alpha] -= h
-            dA = (system.assemble_A(lmax, k, pp) - system.assemble_A(lmax, k, pm)) / (2 * h)
             dp = (inc_fn(pp) - inc_fn(pm)) / (2 * h)
-            out[j, alpha] = mu @ (dA @ s.reshape(-1)) + mu @ dp.reshape(-1)
+            out[j, alpha] = mu @ (dA[alpha] @ s.reshape(-1)) + mu @ dp.reshape(-1)
     return out, s, lam
 
 

@@ -37,6 +37,16 @@ def sph_h1_rd(l, x):
     return sph_h1(l, x) / x + spherical_jn(l, x, derivative=True) + 1j * spherical_yn(l, x, derivative=True)
 
 
+def sph_jn_d(l, x):
+    """d j_l(x) / dx."""
+    return spherical_jn(l, x, derivative=True)
+
+
+def sph_h1_d(l, x):
+    """d h_l^(1)(x) / dx."""
+    return spherical_jn(l, x, derivative=True) + 1j * spherical_yn(l, x, derivative=True)
+
+
 def _norm(l, m):
     return sqrt((2 * l + 1) / 2.0 * factorial(l - m) / factorial(l + m))
 

@@ -78,6 +78,55 @@ def xi_matrix(lmax, k, d, regular=False):
     return xi
 
 
+def d_xi_matrix(lmax, k, d, regular=False):
+    """Gradient of xi_matrix with respect to the displacement d, analytically: (3, L, L), [alpha, source mode, destination mode].
+
+    PAPER.md:517-546 (App. IV, Eqs. IV2-IV6) needs dOmega/dq_i for a scatterer position q_i, and PAPER.md:560 (observation b)
+    notes that it "can be computed analytically": Omega depends on the positions only through xi(k(x_j - x_i)) (Eq. I23).
+    Chain rule on Eq. I17 in the spherical coordinates (r, theta, phi) of d,
+        d/d d_alpha = r_hat_alpha d/dr + (theta_hat_alpha / r) d/dtheta + (phi_hat_alpha / (r sin theta)) d/dphi ,
+    applied term by term to  e^{i mu phi} h_q(k r) Pbar_q^{|mu|}(cos theta),  mu = m - m':
+        d/dr     -> k h_q'(k r)
+        d/dtheta -> taubar_q^{|mu|}(theta)                       (= d Pbar_q^{|mu|}(cos theta) / d theta, Eq. II7 notation)
+        d/dphi   -> i mu ;  Pbar_q^{|mu|} / sin theta = pibar_q^{|mu|}(theta)   (regular at the poles; absent for mu = 0)."""
+    from .vswf import sph_unit_vectors
+    r, theta, phi = cart_to_sph(np.asarray(d, dtype=float))
+    r, theta, phi = float(r), float(theta), float(phi)
+    kr = k * r
+    ct = float(np.cos(theta))
+    rh, th, ph = sph_unit_vectors(theta, phi)
+    modes = mode_list(lmax)
+    L = n_modes(lmax)
+    nq = 2 * lmax + 1
+    zq = [(sp.sph_jn(q, kr) + 0j) if regular else sp.sph_h1(q, kr) for q in range(nq)]
+    dzq = [(sp.sph_jn_d(q, kr) + 0j) if regular else sp.sph_h1_d(q, kr) for q in range(nq)]
+    pq = {(q, mu): float(sp.pbar(q, mu, ct)) for q in range(nq) for mu in range(q + 1)}
+    tq = {(q, mu): float(sp.taubar(q, mu, theta)) for q in range(nq) for mu in range(q + 1)}
+    piq = {(q, mu): float(sp.pibar(q, mu, theta)) for q in range(nq) for mu in range(q + 1)}
+    out = np.zeros((3, L, L), dtype=complex)
+    for a, (l, m, p) in enumerate(modes):
+        for b, (lp, mp, pp) in enumerate(modes):
+            mu = m - mp
+            am = abs(mu)
+            s_r = s_t = s_p = 0.0
+            q0 = abs(l - lp) + (0 if p == pp else 1)
+            for q in range(q0, l + lp + 1):
+                if q < am:
+                    continue
+                c = a5(l, m, lp, mp, q) if p == pp else b5(l, m, lp, mp, q)
+                s_r += c * k * dzq[q] * pq[(q, am)]
+                s_t += c * zq[q] * tq[(q, am)] / r
+                s_p += c * zq[q] * (1j * mu) * piq[(q, am)] / r
+            out[:, a, b] = np.exp(1j * mu * phi) * (rh * s_r + th * s_t + ph * s_p)
+    return out
+
+
+def d_block(lmax, k, x_dst, x_src, regular=False):
+    """d A_ji / d x_j (= - d A_ji / d x_i): (3, L, L) with destination rows, source columns (see block())."""
+    d = np.asarray(x_dst, dtype=float) - np.asarray(x_src, dtype=float)
+    return np.transpose(d_xi_matrix(lmax, k, d, regular), (0, 2, 1))
+
+
 def block(lmax, k, x_dst, x_src, regular=False):
     """A_{ji} = xi^T(x_j, x_i): [A_ji]_{(lmp),(l'm'p')} = xi_{l'm'p';lmp}(k(x_j - x_i))  (Eq. I21, PAPER.md:336).
     Destination modes index rows, source modes index columns."""

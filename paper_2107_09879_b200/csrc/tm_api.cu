@@ -85,7 +85,7 @@ struct tm_ctx {
   bool coplanar = false;
   int kernel_req = TM_KERNEL_AUTO, kernel = TM_KERNEL_GENERAL;
   TmShift shift{0.0, 0.0, 0.0, 0};      // target displacement (tm_grad_positions only)
-  int cop_tj = 128;                     // coplanar kernel: targets per block (env TM_COP_TJ=256 for experiments)
+  int cop_tj = 128;                     // coplanar kernel: targets per block (-DTM_COP_TJ=256 for experiments)
 
   double* d_pos = nullptr;
   int* d_win_of = nullptr;
@@ -410,7 +410,8 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
   bool all_ok = false;
   // cooperative single-launch Arnoldi step: only when every chunk's block can be resident at once
   bool coop = false;
-  if (ctx->max_chunks_per_win <= 512 && !std::getenv("TM_NO_COOP")) {
+#ifndef TM_NO_COOP                 // build switch (-DTM_NO_COOP): multi-kernel Arnoldi step everywhere, for A/B measurements
+  if (ctx->max_chunks_per_win <= 512) {
     int per_sm = 0, dev = 0, n_sm = 0, can = 0;
     const void* fn = ctx->ept == 1 ? (const void*)k_arnoldi_fused<R, 1> : (const void*)k_arnoldi_fused<R, 4>;
     const size_t sm_max = (size_t)(2 * m + 2) * sizeof(double2) + (size_t)(m + 1) * sizeof(double);
@@ -422,6 +423,7 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
     coop = can && (long long)per_sm * n_sm >= nc;
     (void)fn;
   }
+#endif
   const Cx<RX>* resid_vec = B;                        // first cycle: x0 = 0 so r = b
   if (warm) {                                         // ||b|| is the reference norm; r0 = b - M x0 starts the first cycle
     k_norm2<RX><<<nc, TM_VT, 0, st>>>(B, ctx->d_chunks, ctx->gm.normpart);
@@ -594,7 +596,9 @@ int configure_kernel(tm_ctx* ctx) {
     return fail(ctx, TM_E_INVALID, "coplanar kernel needs all z equal");
   if (want == TM_KERNEL_SYM3D && ctx->lmax > 3) return fail(ctx, TM_E_INVALID, "generated 3-D kernel needs lmax <= 3");
   ctx->kernel = want;
-  if (const char* e = std::getenv("TM_COP_TJ")) ctx->cop_tj = std::atoi(e) == 256 ? 256 : 128;
+#ifdef TM_COP_TJ                   // build switch (-DTM_COP_TJ=256): 256 targets per block (measured +-1 %)
+  ctx->cop_tj = TM_COP_TJ == 256 ? 256 : 128;
+#endif
   int tgt_per_tile;
   const bool gen = want == TM_KERNEL_COPLANAR || want == TM_KERNEL_SYM3D;      // generated kernels: thread = target
   switch (gen ? 0 : ctx->lmax) {

@@ -37,6 +37,33 @@ def test_adjoint_position_gradient_matches_finite_differences():
         assert abs(g[j, a] - fd) <= 1e-6 * np.abs(g).max()
 
 
+def test_analytic_translation_derivative_matches_central_differences():
+    """Pin of oracle/translation.py::d_xi_matrix (PAPER.md:517-546, 560): the analytic gradient of the translation
+    coefficients against 4th-order central differences of xi_matrix itself, for a general displacement, the two polar
+    directions (phi undefined, pibar limit), a coplanar one, and the regular (j_q) variant; lmax up to 6 (the paper's
+    truncation).  A wrong sign of any of the three spherical components, a missing 1/r or a wrong h_q' fails it."""
+    from oracle import translation as tr
+    rng = np.random.default_rng(31)
+    cases = [(3, rng.uniform(-1, 1, 3) + 0.3), (3, np.array([0.0, 0.0, 0.9])), (3, np.array([0.0, 0.0, -0.7])),
+             (3, np.array([0.6, -0.3, 0.0])), (6, np.array([0.5, 0.4, -0.6])), (4, np.array([-0.7, 0.2, 0.0]))]
+    h = 1e-4
+    for lmax, d in cases:
+        for regular in ((False, True) if lmax == 3 else (False,)):
+            an = tr.d_xi_matrix(lmax, K, d, regular)
+            f = lambda x: tr.xi_matrix(lmax, K, x, regular)
+            for al in range(3):
+                e = np.zeros(3)
+                e[al] = h
+                fd = (8 * (f(d + e) - f(d - e)) - (f(d + 2 * e) - f(d - 2 * e))) / (12 * h)
+                assert np.abs(an[al] - fd).max() <= 1e-8 * np.abs(fd).max(), (lmax, d, al)
+    # d_block: destination rows, source columns, d = x_dst - x_src; moving the SOURCE flips the sign
+    xd, xs = np.array([0.2, 0.5, -0.1]), np.array([-0.4, 0.1, 0.6])
+    an = tr.d_block(2, K, xd, xs)
+    e = np.array([0.0, h, 0.0])
+    assert np.abs(an[1] - (tr.block(2, K, xd + e, xs) - tr.block(2, K, xd - e, xs)) / (2 * h)).max() <= 1e-6 * np.abs(an[1]).max()
+    assert np.abs(an[1] + (tr.block(2, K, xd, xs + e) - tr.block(2, K, xd, xs - e)) / (2 * h)).max() <= 1e-6 * np.abs(an[1]).max()
+
+
 def test_shape_parameter_derivative_reduces_to_the_mie_radius_derivative():
     """fd_shape_parameter with spheres as the bodies of revolution = fd_radius with the closed-form Mie T-matrix (two
     independent routes to T: null-field surface integrals vs. Lorenz-Mie)."""
