@@ -388,13 +388,13 @@ def measure(args, w, mode, steps, warmup, rank, world, local_rank, dist, st, pea
     sm_max = (clk.get("sm_max_mhz") or 1965.0) * 1e6
     nominal = 148 * NOMINAL_LANES[pipe] * 2 * sm_max * 1e-12
     cfg = config_record(w, args, mode)
-    cfg.update(kernel={libtm.TM_KERNEL_COPLANAR: "coplanar", libtm.TM_KERNEL_SYM3D: "sym3d"}.get(kern, "general"),
-               parallelism="replicas" if world > 1 else "single")
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
         "ms_per_step": t_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": {libtm.TM_FP64: "f64", libtm.TM_FP32: "f32"}.get(prec, "f32 cycles + f64 residual/iterate"), "data": "synthetic",
         "config": cfg,
+        "launch": {"kernel": {libtm.TM_KERNEL_COPLANAR: "coplanar", libtm.TM_KERNEL_SYM3D: "sym3d"}.get(kern, "general"),
+                   "parallelism": "replicas" if world > 1 else "single"},
         "solve": {"forward_iterations": max(i.iterations for i in info), "adjoint_iterations": max(i.iterations for i in info2),
                   "forward_rel_residual": max(i.rel_residual for i in info), "adjoint_rel_residual": max(i.rel_residual for i in info2),
                   "forward_seconds": info[0].seconds, "adjoint_seconds": info2[0].seconds, "converged": bool(rc == 0 and rc2 == 0),
@@ -510,7 +510,7 @@ def run_gradient(args, w):
     print(json.dumps({"mode": "gradient", "workload": w["name"], "n_scat": N, "L": L, "design_variables": int(N + 3 * N),
                       "solves_seconds": t1 - t0, "forward_iterations": i1[0].iterations, "adjoint_iterations": i2[0].iterations,
                       "converged": rc1 == 0 and rc2 == 0, "grad_tmatrix_seconds": t3 - t2, "grad_positions_seconds": t5 - t4,
-                      "grad_positions_allpairs_launches": 24, "norm_grad_R": float(np.linalg.norm(gR)),
+                      "grad_positions_allpairs_launches": 2, "grad_positions_lmax_of_products": w["lmax"] + 1, "norm_grad_R": float(np.linalg.norm(gR)),
                       "norm_grad_x": float(np.linalg.norm(gX))}), flush=True)
     s.close()
 

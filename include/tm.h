@@ -178,12 +178,14 @@ int tm_grad_tmatrix(tm_ctx *ctx, const tm_c64 *dT, const tm_c64 *lambda, const t
  * scatterer's own waves - is the caller's, it does not involve the solver).  Identity S3 folds the row-block and
  * column-block parts of dA/dx_j into two all-pairs products with the DERIVATIVE of the translation operator,
  *   G_j = mu_j^T (d_alpha A s)_j + (P s_j)^T (d_alpha A P mu)_j ,  mu = T^T lambda,
- * and d_alpha A is taken by Richardson-extrapolated central differences of the on-the-fly operator in its displacement
- * argument (targets displaced rigidly by +-h, +-h/2; error O((k h)^4); h in the units of the positions, 0 -> 2e-4
- * wavelengths) - a stated deviation from the paper's analytic dOmega/dq.  24 all-pairs launches.
- *   lambda, s [n_scat][L]; dp [n_scat][3][L] or NULL (plane wave: dp = i k_alpha p); out [n_scat][3] complex.
- * lmax <= 3 (uses the generated 3-D kernel for all three directions). */
-int tm_grad_positions(tm_ctx *ctx, const tm_c64 *lambda, const tm_c64 *s, const tm_c64 *dp, double h, tm_c64 *out);
+ * and d_alpha A is ANALYTIC ("can be computed analytically"): differentiating the addition theorem with
+ * respect to the destination centre gives  dA(d)/dd_alpha = k_b D^alpha A^ext(d),  A^ext = the translation operator with
+ * destination rows up to lmax + 1 and D^alpha three constant sparse matrices (the gradient ladder of the regular
+ * wavefunctions, generated at build time).  Cost: TWO all-pairs products at lmax + 1 for all 3 n_scat derivatives, on an
+ * auxiliary context created at the first call and kept; planar layouts stay on the coplanar kernels (the z-derivative
+ * sits in the constant matrix).  Every lmax of the API (1..6), any layout, every precision.
+ *   lambda, s [n_scat][L]; dp [n_scat][3][L] or NULL (plane wave: dp = i k_alpha p); out [n_scat][3] complex. */
+int tm_grad_positions(tm_ctx *ctx, const tm_c64 *lambda, const tm_c64 *s, const tm_c64 *dp, tm_c64 *out);
 
 /* Host helper: d(diag T)/dR of the Mie T-matrix of tm_mie_tmatrix (Richardson-extrapolated central differences of the
  * closed form, relative accuracy ~1e-10), out[L]. */

@@ -72,24 +72,30 @@ def dA_dposition(lmax, k, pos, j):
     return out
 
 
-def adjoint_position_gradient(lmax, k, pos, radii, eps_r, inc_fn, v, h=1e-5):
+def adjoint_position_gradient(lmax, k, pos, radii, eps_r, inc_fn, v, h=1e-5, dinc_fn=None):
     """All dJ/dx_{j,alpha} through ONE adjoint solve: lambda^T T (dA/dx_{j,alpha}) s + lambda^T T da^(0)/dx_{j,alpha}
     (Eq. IV6 with Omega = T^{-1} M; dOmega/dq = -dA/dq).  dA/dq is the analytic derivative of Eq. I23's off-diagonal blocks
     (dA_dposition; "can be computed analytically"); da^(0)/dq, which is not part of Omega, by central
-    differences of inc_fn.  Returns (N, 3).  Pinned by fd_position (central differences of the whole dense solve)."""
+    differences of inc_fn, or exactly from dinc_fn(pos) -> (N, 3, L) = d a^(0)_j / d x_{j,alpha} when given (plane wave:
+    i k_alpha a^(0)_j, Eq. II6).  Returns (N, 3).  Pinned by fd_position (central differences of the whole dense solve)."""
     p_inc = inc_fn(pos)
     J, s, M, t = _solve_J(lmax, k, pos, radii, eps_r, p_inc, v)
     lam = system.solve_adjoint(M, v)
     N, L = s.shape
     mu = (t * lam).reshape(-1)                                     # T^T lambda (T diagonal)
     out = np.zeros((N, 3), dtype=complex)
+    dinc = dinc_fn(pos) if dinc_fn is not None else None
     for j in range(N):
         dA = dA_dposition(lmax, k, pos, j)
         for alpha in range(3):
-            pp, pm = np.array(pos, dtype=float), np.array(pos, dtype=float)
-            pp[j, alpha] += h
-            pm[j, alpha] -= h
-            dp = (inc_fn(pp) - inc_fn(pm)) / (2 * h)
+            if dinc is not None:
+                dp = np.zeros((N, L), dtype=complex)
+                dp[j] = dinc[j, alpha]
+            else:
+                pp, pm = np.array(pos, dtype=float), np.array(pos, dtype=float)
+                pp[j, alpha] += h
+                pm[j, alpha] -= h
+                dp = (inc_fn(pp) - inc_fn(pm)) / (2 * h)
             out[j, alpha] = mu @ (dA[alpha] @ s.reshape(-1)) + mu @ dp.reshape(-1)
     return out, s, lam
 

@@ -22,11 +22,24 @@ def _mtime(p):
     return os.path.getmtime(p) if os.path.exists(p) else 0.0
 
 
+def _gen_hash():
+    import hashlib
+    return hashlib.sha256(open(os.path.join(CSRC, "gen_tables.py"), "rb").read()).hexdigest()
+
+
 def generate(force=False):
+    """(Re)write csrc/generated/ when it does not belong to the current gen_tables.py.  Staleness is decided by the
+    generator's content hash recorded in generated/GENERATOR_SHA256 (file times mean nothing after a git checkout, and a
+    full generation takes minutes of 40-digit arithmetic)."""
     gen_py = os.path.join(CSRC, "gen_tables.py")
-    outs = [os.path.join(GEN, "tm_tables_gen.h"), os.path.join(GEN, "tm_coplanar_gen.cuh")]
-    if force or any(_mtime(o) < _mtime(gen_py) for o in outs):
+    stamp = os.path.join(GEN, "GENERATOR_SHA256")
+    outs = [os.path.join(GEN, f) for f in ("tm_tables_gen.h", "tm_coplanar_gen.cuh", "tm_coplanar_f2_gen.cuh",
+                                           "tm_general3d_gen.cuh", "tm_coplanar4_gen.cuh")]
+    have = open(stamp).read().strip() if os.path.exists(stamp) else ""
+    if force or have != _gen_hash() or not all(os.path.exists(o) for o in outs):
         subprocess.check_call([sys.executable, gen_py])
+        with open(stamp, "w") as f:
+            f.write(_gen_hash() + "\n")
 
 
 def sources():

@@ -152,12 +152,63 @@ def emit_tables(lmaxes, path):
                 f.write("  " + ", ".join(lit(t[4]) for t in terms[s:s + 6]) + ",\n")
             f.write("};\n\n")
             print(f"lmax={lmax}: L={L} general terms={len(terms)}", file=sys.stderr)
+        emit_gradient_tables(f, [l for l in lmaxes if l + 1 in lmaxes])
         f.write(f"static const int tm_max_table_lmax = {max(lmaxes)};\n")
         f.write("static const TmTermTable tm_term_tables[] = {\n")
         for lmax in lmaxes:
             tag = f"L{lmax}"
             f.write(f"  {{{lmax}, (int)(sizeof(tm_col_{tag})), tm_rowptr_{tag}, tm_col_{tag}, tm_q_{tag}, tm_ipow_{tag}, tm_val_{tag}}},\n")
         f.write("};\n")
+
+
+# ----------------------------------------------------------------------------- gradient of the translation operator
+def gradient_entries(lmax):
+    """Constant matrices of the analytic position derivative (PAPER.md:517-546 Eqs. IV2-IV6, :560 "can be computed
+    analytically").  The regular wavefunctions obey  d/dx_alpha RPhi_b = k sum_b' D^alpha[b', b] RPhi_b'  with
+    D^alpha = (1/k) d RgA(eps)/d eps_alpha at eps = 0, and only the q = 1 term of Eq. I17 is linear in eps:
+        j_1(k eps) Pbar_1^0(cos theta) -> (k/3) sqrt(3/2) eps_z ,   j_1(k eps) Pbar_1^1 e^{+-i phi} -> (k/3) (sqrt(3)/2) (eps_x +- i eps_y).
+    Differentiating  Phi_a(x - x_i) = sum_b A_ba(x_j - x_i) RPhi_b(x - x_j)  with respect to x_j gives
+        d A(d) / d d_alpha = k D^alpha A^ext(d),
+    A^ext = the translation operator with destination rows up to lmax + 1: the derivative of the operator is ONE ordinary
+    all-pairs product at lmax + 1 followed by a constant sparse matrix per direction.
+    Returns [(alpha, row b' in modes(lmax), col b in modes(lmax+1), complex value D^alpha[b', b])]."""
+    md, mde = modes(lmax), modes(lmax + 1)
+    cz = mp.sqrt(mp.mpf(3) / 2) / 3
+    cx = mp.sqrt(mp.mpf(3)) / 2 / 3
+    out = []
+    for bp, (lp, mp_, pp) in enumerate(md):            # destination b'
+        for b, (l, m, p) in enumerate(mde):             # source b
+            ip, v = coupling(l, m, p, lp, mp_, pp, 1)
+            if v == 0:
+                continue
+            c = (mp.mpc(0, 1) ** ip) * v
+            mu = m - mp_
+            if mu == 0:
+                out.append((2, bp, b, c * cz))
+            elif abs(mu) == 1:
+                out.append((0, bp, b, c * cx))
+                out.append((1, bp, b, c * cx * mp.mpc(0, mu)))
+    return out
+
+
+def emit_gradient_tables(f, lmaxes):
+    f.write("// Gradient of the translation operator (gen_tables.py: gradient_entries):  dA/dd_alpha = k D^alpha A^ext,\n")
+    f.write("// entry e: D^{alpha[e]}[row[e] (flat index at lmax), col[e] (flat index at lmax + 1)] = (re[e], im[e]).\n")
+    f.write("struct TmGradTable { int lmax; int n; const uint8_t* alpha; const uint8_t* row; const uint8_t* col; const double* re; const double* im; };\n")
+    for lmax in lmaxes:
+        ent = gradient_entries(lmax)
+        tag = f"L{lmax}"
+        f.write(f"static const uint8_t tm_grad_alpha_{tag}[{len(ent)}] = {{{', '.join(str(e[0]) for e in ent)}}};\n")
+        f.write(f"static const uint8_t tm_grad_row_{tag}[{len(ent)}] = {{{', '.join(str(e[1]) for e in ent)}}};\n")
+        f.write(f"static const uint8_t tm_grad_col_{tag}[{len(ent)}] = {{{', '.join(str(e[2]) for e in ent)}}};\n")
+        f.write(f"static const double tm_grad_re_{tag}[{len(ent)}] = {{{', '.join(lit(mp.re(e[3])) for e in ent)}}};\n")
+        f.write(f"static const double tm_grad_im_{tag}[{len(ent)}] = {{{', '.join(lit(mp.im(e[3])) for e in ent)}}};\n")
+        print(f"lmax={lmax}: gradient entries={len(ent)}", file=sys.stderr)
+    f.write("static const TmGradTable tm_grad_tables[] = {\n")
+    for lmax in lmaxes:
+        tag = f"L{lmax}"
+        f.write(f"  {{{lmax}, (int)(sizeof(tm_grad_alpha_{tag})), tm_grad_alpha_{tag}, tm_grad_row_{tag}, tm_grad_col_{tag}, tm_grad_re_{tag}, tm_grad_im_{tag}}},\n")
+    f.write("};\n\n")
 
 
 # ----------------------------------------------------------------------------- coplanar specialisation
@@ -884,7 +935,7 @@ def coplanar_sectors(lmax):
     return out
 
 
-COP4_GROUPS = {4: 1, 5: 4, 6: 4}     # row groups per sector: keeps one block's straight-line code near the 32 KB L1.5 I-cache
+COP4_GROUPS = {4: 1, 5: 4, 6: 4, 7: 4}     # row groups per sector: keeps one block's straight-line code near the 32 KB L1.5 I-cache
 
 
 COP4_AXIAL = True        # False: direct pair-frame operator cut into row groups
@@ -1174,10 +1225,10 @@ def emit_coplanar_f2(lmaxes, path):
 
 def main():
     os.makedirs(OUT, exist_ok=True)
-    emit_tables([1, 2, 3, 4, 5, 6], os.path.join(OUT, "tm_tables_gen.h"))
+    emit_tables([1, 2, 3, 4, 5, 6, 7], os.path.join(OUT, "tm_tables_gen.h"))     # 7: internal (gradient at lmax 6)
     emit_coplanar([1, 2, 3], os.path.join(OUT, "tm_coplanar_gen.cuh"))
     emit_general_sym([1, 2, 3], os.path.join(OUT, "tm_general3d_gen.cuh"))
-    emit_coplanar4([4, 5, 6], os.path.join(OUT, "tm_coplanar4_gen.cuh"))
+    emit_coplanar4([4, 5, 6, 7], os.path.join(OUT, "tm_coplanar4_gen.cuh"))     # 7: internal (gradient at lmax 6)
     emit_coplanar_f2([1, 2, 3], os.path.join(OUT, "tm_coplanar_f2_gen.cuh"))
 
 

@@ -465,7 +465,7 @@ template <typename R, int LMAX, int Z, int G> struct Cop4;
 #define TM_COP4_SPEC_G2(LM) TM_COP4_IF2_L##LM(TM_COP4_SPEC_Z(LM, 1))
 #define TM_COP4_SPEC_G4(LM) TM_COP4_IF4_L##LM(TM_COP4_SPEC_Z(LM, 2) TM_COP4_SPEC_Z(LM, 3))
 #define TM_COP4_SPEC_G8(LM) TM_COP4_IF8_L##LM(TM_COP4_SPEC_Z(LM, 4) TM_COP4_SPEC_Z(LM, 5) TM_COP4_SPEC_Z(LM, 6) TM_COP4_SPEC_Z(LM, 7))
-TM_COP4_SPEC_L(4) TM_COP4_SPEC_L(5) TM_COP4_SPEC_L(6)
+TM_COP4_SPEC_L(4) TM_COP4_SPEC_L(5) TM_COP4_SPEC_L(6) TM_COP4_SPEC_L(7)
 #undef TM_COP4_SPEC_L
 #undef TM_COP4_SPEC_Z
 #undef TM_COP4_SPEC
@@ -474,6 +474,7 @@ template <int LMAX> struct Cop4Max;      // n: slots of the largest sector; nr: 
 template <> struct Cop4Max<4> { static constexpr int n = TM_COP4_NMAX_L4, nr = TM_COP4_NRMAX_L4, ng = TM_COP4_G_L4; };
 template <> struct Cop4Max<5> { static constexpr int n = TM_COP4_NMAX_L5, nr = TM_COP4_NRMAX_L5, ng = TM_COP4_G_L5; };
 template <> struct Cop4Max<6> { static constexpr int n = TM_COP4_NMAX_L6, nr = TM_COP4_NRMAX_L6, ng = TM_COP4_G_L6; };
+template <> struct Cop4Max<7> { static constexpr int n = TM_COP4_NMAX_L7, nr = TM_COP4_NRMAX_L7, ng = TM_COP4_G_L7; };
 
 template <typename R, int LMAX, int TJ, int SS> struct Cop4Smem {
   static constexpr int NM = Cop4Max<LMAX>::n;

@@ -64,6 +64,9 @@ constexpr int SYM3D_SS = 32;     // generated 3-D kernel: sources per stage
 constexpr int COP4_TJ = 128;     // four-sector coplanar kernel (lmax 4..6): targets per block
 constexpr int COP4_SS = 16;      // ... sources per stage
 constexpr int MAX_RESTART = 300;
+inline int cop4_groups(int lmax) {   // row groups per sector of the four-sector coplanar kernel
+  return lmax == 4 ? Cop4Max<4>::ng : (lmax == 5 ? Cop4Max<5>::ng : (lmax == 6 ? Cop4Max<6>::ng : Cop4Max<7>::ng));
+}
 static_assert(MAX_RESTART + 1 <= TM_MAX_LDH, "k_gmres_solve_y keeps y in shared memory");
 
 struct Gmres {                   // device scalars of the Krylov solver, sized for `restart`
@@ -84,7 +87,9 @@ struct tm_ctx {
   std::vector<int> win_ptr;
   bool coplanar = false;
   int kernel_req = TM_KERNEL_AUTO, kernel = TM_KERNEL_GENERAL;
-  TmShift shift{0.0, 0.0, 0.0, 0};      // target displacement (tm_grad_positions only)
+  TmShift shift{0.0, 0.0, 0.0, 0};      // target displacement (unused by the library: kept for A/B experiments)
+  tm_ctx* grad_aux = nullptr;           // tm_grad_positions: the same layout at lmax + 1 (all-pairs product A^ext)
+  void* d_grad_tab = nullptr; TmGradDev grad_tab{};
   int cop_tj = 128;                     // coplanar kernel: targets per block (-DTM_COP_TJ=256 for experiments)
 
   double* d_pos = nullptr;
@@ -267,7 +272,7 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
   tick(c, true);
   if (c->kernel == TM_KERNEL_COPLANAR && c->lmax > 3) {
     // (z-mirror parity, y'-mirror sector) x row group: slowest grid dimension
-    grid.z = 4 * (c->lmax == 4 ? Cop4Max<4>::ng : (c->lmax == 5 ? Cop4Max<5>::ng : Cop4Max<6>::ng));
+    grid.z = 4 * cop4_groups(c->lmax);
 #define TM_LAUNCH_C4(LM)                                                                                        \
   {                                                                                                             \
     const size_t sm = Cop4Smem<R, LM, COP4_TJ, COP4_SS>::bytes;                                                 \
@@ -278,7 +283,8 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
     switch (c->lmax) {
       case 4: TM_LAUNCH_C4(4) break;
       case 5: TM_LAUNCH_C4(5) break;
-      default: TM_LAUNCH_C4(6) break;
+      case 6: TM_LAUNCH_C4(6) break;
+      default: TM_LAUNCH_C4(7) break;
     }
 #undef TM_LAUNCH_C4
   } else if (c->kernel == TM_KERNEL_COPLANAR) {
@@ -325,7 +331,8 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
       case 3: TM_LAUNCH_GEN(3) break;
       case 4: TM_LAUNCH_GEN(4) break;
       case 5: TM_LAUNCH_GEN(5) break;
-      default: TM_LAUNCH_GEN(6) break;
+      case 6: TM_LAUNCH_GEN(6) break;
+      default: TM_LAUNCH_GEN(7) break;
     }
 #undef TM_LAUNCH_GEN
   }
@@ -619,7 +626,7 @@ int configure_kernel(tm_ctx* ctx) {
   // without a long tail; bounded by 64 chunks, >= 32 sources per chunk and 2 GB of partial sums.
   const long long slots = 148LL * (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj : (want == TM_KERNEL_SYM3D ? 2 : 4));
   const bool cop4 = want == TM_KERNEL_COPLANAR && ctx->lmax > 3;   // four-sector coplanar kernel (lmax 4..6)
-  const int cop4_z = !cop4 ? 0 : 4 * (ctx->lmax == 4 ? Cop4Max<4>::ng : (ctx->lmax == 5 ? Cop4Max<5>::ng : Cop4Max<6>::ng));
+  const int cop4_z = !cop4 ? 0 : 4 * cop4_groups(ctx->lmax);
   const long long blocks1 = (long long)ctx->n_tiles * (cop4 ? cop4_z : (gen ? 2 : 1));
   const int part_mult = (want == TM_KERNEL_SYM3D || cop4) ? 2 : 1;   // one partial buffer per (chunk, y'-sector)
   int max_win = 1;
@@ -709,6 +716,8 @@ const char* tm_last_error(const tm_ctx* ctx) { return ctx ? ctx->err.c_str() : g
 void tm_destroy(tm_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
+  if (c->grad_aux) tm_destroy(c->grad_aux);
+  tm_dev_free(c->d_grad_tab);
   tm_dev_free(c->d_pos); tm_dev_free(c->d_win_of); tm_dev_free(c->d_type_of); tm_dev_free(c->d_T); tm_dev_free(c->d_T32); tm_dev_free(c->d_p);
   tm_dev_free(c->d_const); tm_dev_free(c->d_rowptr); tm_dev_free(c->d_col); tm_dev_free(c->d_widx); tm_dev_free(c->d_imag);
   tm_dev_free(c->d_coef); tm_dev_free(c->d_tiles); tm_dev_free(c->d_upart); tm_dev_free(c->d_chunks); tm_dev_free(c->d_win_chunk_ptr);
@@ -724,13 +733,19 @@ void tm_destroy(tm_ctx* c) {
   delete c;
 }
 
-int tm_create(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const int* win_ptr, int lmax, double k_b,
-              int precision, void* cuda_stream) {
+}  // extern "C"
+
+namespace {
+// tm_create with the truncation limit as a parameter: the public entry point allows lmax <= TM_MAX_LMAX, the position
+// gradient builds its auxiliary context at lmax + 1 <= TM_INT_LMAX.
+int create_ctx(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const int* win_ptr, int lmax, double k_b,
+               int precision, void* cuda_stream, int lmax_limit) {
   tm_ctx* ctx = nullptr;                                  // errors before allocation go to g_create_error
   if (!out) return fail(ctx, TM_E_INVALID, "out is NULL");
   *out = nullptr;
   if (n_scat < 1 || !pos_xyz) return fail(ctx, TM_E_INVALID, "need n_scat >= 1 and positions");
-  if (lmax < 1 || lmax > tm_max_table_lmax) return fail(ctx, TM_E_INVALID, "lmax must be in 1..6");
+  static_assert(tm_max_table_lmax == TM_INT_LMAX, "term tables must reach the internal truncation");
+  if (lmax < 1 || lmax > lmax_limit) return fail(ctx, TM_E_INVALID, "lmax must be in 1..6");
   if (!(k_b > 0.0) || !std::isfinite(k_b)) return fail(ctx, TM_E_INVALID, "k_b must be positive and finite");
   if (precision != TM_FP64 && precision != TM_FP32 && precision != TM_MIXED)
     return fail(ctx, TM_E_INVALID, "precision must be TM_FP64, TM_FP32 or TM_MIXED");
@@ -848,6 +863,14 @@ int tm_create(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const 
 #undef TM_CREATE_CUDA
   *out = c;
   return TM_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int tm_create(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const int* win_ptr, int lmax, double k_b,
+              int precision, void* cuda_stream) {
+  return create_ctx(out, n_scat, pos_xyz, n_win, win_ptr, lmax, k_b, precision, cuda_stream, TM_MAX_LMAX);
 }
 
 int tm_set_kernel(tm_ctx* ctx, int kernel) {
@@ -1292,38 +1315,36 @@ int tm_grad_tmatrix(tm_ctx* ctx, const tm_c64* dT, const tm_c64* lambda, const t
 
 namespace {
 
+// Analytic position gradient (PAPER.md:517-546 Eqs. IV2-IV6; :560 "can be computed analytically").  With
+// dA/dd_alpha = k D^alpha A^ext (gen_tables.py: gradient_entries) the two products with the derivative of the translation
+// operator become two ORDINARY all-pairs products at lmax + 1 on the auxiliary context `ax` (same positions and windows),
+// each followed by the constant sparse contraction k_grad_contract for the three directions at once.
 template <typename R>
-int grad_positions_typed(tm_ctx* ctx, const tm_c64* lambda, const tm_c64* s, const tm_c64* dp, double h, tm_c64* out) {
+int grad_positions_typed(tm_ctx* ctx, tm_ctx* ax, const tm_c64* lambda, const tm_c64* s, const tm_c64* dp, tm_c64* out) {
   const size_t n = ctx->n, vb = n * sizeof(Cx<R>);
-  const int L = ctx->L, N = ctx->n_scat;
-  Cx<R>*S = vec<R>(ctx, 0), *Y = vec<R>(ctx, 1), *LAM = vec<R>(ctx, 2);
-  Cx<R>*PMU = nullptr, *D = nullptr; double2 *d_out = nullptr, *d_dp = nullptr;
-  auto cleanup = [&]() { tm_dev_free(PMU); tm_dev_free(D); tm_dev_free(d_out); tm_dev_free(d_dp); ctx->shift = TmShift{0.0, 0.0, 0.0, 0}; };
+  const int L = ctx->L, Le = ax->L, N = ctx->n_scat;
+  Cx<R>*S = vec<R>(ctx, 0), *LAM = vec<R>(ctx, 2);
+  Cx<R>*XP = vec<R>(ax, 0), *V = vec<R>(ax, 1);
+  Cx<R>* PMU = nullptr; double2 *d_out = nullptr, *d_dp = nullptr;
+  auto cleanup = [&]() { tm_dev_free(PMU); tm_dev_free(d_out); tm_dev_free(d_dp); };
 #define TM_G(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { cleanup(); return fail(ctx, TM_E_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); } } while (0)
-  TM_G(tm_dev_alloc(&PMU, vb)); TM_G(tm_dev_alloc(&D, vb)); TM_G(tm_dev_alloc(&d_out, (size_t)N * 3 * sizeof(double2)));
+  TM_G(tm_dev_alloc(&PMU, vb)); TM_G(tm_dev_alloc(&d_out, (size_t)N * 3 * sizeof(double2)));
   TM_G(cudaMemsetAsync(d_out, 0, (size_t)N * 3 * sizeof(double2), ctx->stream));
   TM_G(load_c64<R>(ctx, s, S));
   TM_G(load_c64<R>(ctx, lambda, LAM));
   TM_G(launch_tapply<R>(ctx, 4, LAM, PMU, nullptr));                 // P mu = P T^T lambda
   const int gb = (N + 3) / 4;
-  for (int alpha = 0; alpha < 3; ++alpha) {
-    for (int which = 0; which < 2; ++which) {
-      const Cx<R>* vecx = which == 0 ? S : PMU;                       // d_alpha A s   /   d_alpha A (P mu)
-      const Cx<R>* left = which == 0 ? PMU : S;                       // mu = P(P mu)  /   P s
-      const double hs[4] = {0.5 * h, -0.5 * h, h, -h};
-      const double cf[4] = {4.0 / (3.0 * h), -4.0 / (3.0 * h), -1.0 / (6.0 * h), 1.0 / (6.0 * h)};
-      for (int t = 0; t < 4; ++t) {
-        ctx->shift = TmShift{alpha == 0 ? hs[t] : 0.0, alpha == 1 ? hs[t] : 0.0, alpha == 2 ? hs[t] : 0.0, 1};
-        TM_G(launch_allpairs<R>(ctx, vecx, nullptr));
-        TM_G(launch_tapply<R>(ctx, 2, vecx, Y, nullptr));
-        k_acc_scaled<R><<<grid_for(n, 256), 256, 0, ctx->stream>>>(D, Y, cf[t], n, t == 0 ? 1 : 0);
-      }
-      k_bilinear_rows<R, R><<<gb, 128, 0, ctx->stream>>>(L, N, left, D, (size_t)L, ctx->d_const, d_out + alpha, 3);
-      ctx->total_launches += 5;
-      TM_G(cudaGetLastError());
-    }
+  for (int which = 0; which < 2; ++which) {
+    const Cx<R>* vecx = which == 0 ? S : PMU;                         // dA s   /   dA (P mu)
+    const Cx<R>* left = which == 0 ? PMU : S;                         // mu = P(P mu)  /   P s   (k_grad_contract applies P)
+    TM_G(cudaMemsetAsync(XP, 0, ax->n * sizeof(Cx<R>), ctx->stream));
+    k_pad_modes<R><<<grid_for(n, 256), 256, 0, ctx->stream>>>(vecx, XP, L, Le, n);
+    TM_G(launch_allpairs<R>(ax, XP, nullptr));                        // A^ext (padded vector): rows l' <= lmax + 1
+    TM_G(launch_tapply<R>(ax, 2, XP, V, nullptr));
+    k_grad_contract<R><<<gb, 128, 0, ctx->stream>>>(L, Le, N, left, V, ctx->d_const, ctx->grad_tab, ctx->k, d_out);
+    ctx->total_launches += 4; ctx->allpairs_launches++;
+    TM_G(cudaGetLastError());
   }
-  ctx->shift = TmShift{0.0, 0.0, 0.0, 0};
   if (dp) {                                                          // incident part: mu_j^T dp_j[alpha]
     TM_G(tm_dev_alloc(&d_dp, n * 3 * sizeof(double2)));
     TM_G(copy_in(d_dp, dp, n * 3 * sizeof(double2), ctx->stream));
@@ -1343,23 +1364,30 @@ int grad_positions_typed(tm_ctx* ctx, const tm_c64* lambda, const tm_c64* s, con
 
 extern "C" {
 
-int tm_grad_positions(tm_ctx* ctx, const tm_c64* lambda, const tm_c64* s, const tm_c64* dp, double h, tm_c64* out) {
+int tm_grad_positions(tm_ctx* ctx, const tm_c64* lambda, const tm_c64* s, const tm_c64* dp, tm_c64* out) {
   if (!ctx) return TM_E_INVALID;
   if (!lambda || !s || !out) return fail(ctx, TM_E_INVALID, "NULL argument");
   if (!ctx->has_T) return fail(ctx, TM_E_STATE, "tm_set_tmatrices must be called first");
-  if (ctx->lmax > 3) return fail(ctx, TM_E_INVALID, "position sensitivities are built for lmax <= 3");
-  if (h < 0.0 || !std::isfinite(h)) return fail(ctx, TM_E_INVALID, "h must be >= 0");
-  if (h == 0.0) h = 2e-4 * 2.0 * M_PI / ctx->k;
   TM_CUDA(stream_wait(ctx));
-  const int saved = ctx->kernel_req;
-  ctx->kernel_req = TM_KERNEL_SYM3D;                      // displaced targets are not coplanar with the sources (alpha = z)
-  int rc = configure_kernel(ctx);
-  if (rc == TM_OK)
-    rc = ctx->precision != TM_FP32 ? grad_positions_typed<double>(ctx, lambda, s, dp, h, out)
-                                   : grad_positions_typed<float>(ctx, lambda, s, dp, h, out);
-  ctx->kernel_req = saved;
-  const int rc2 = configure_kernel(ctx);
-  return rc != TM_OK ? rc : rc2;
+  if (!ctx->grad_aux) {            // the same layout at lmax + 1 (kept for later calls of an optimisation loop)
+    const int rc = create_ctx(&ctx->grad_aux, ctx->n_scat, ctx->d_pos, ctx->n_win, ctx->win_ptr.data(), ctx->lmax + 1, ctx->k,
+                              ctx->precision == TM_FP32 ? TM_FP32 : TM_FP64, ctx->stream, TM_INT_LMAX);
+    if (rc != TM_OK) return fail(ctx, rc, "auxiliary lmax + 1 context: " + g_create_error);
+  }
+  if (!ctx->d_grad_tab) {          // D^alpha entries of this lmax
+    const TmGradTable& t = tm_grad_tables[ctx->lmax - 1];
+    const size_t nn = (size_t)t.n, off_re = (3 * nn + 255) / 256 * 256, bytes = off_re + 2 * nn * sizeof(double);
+    std::vector<unsigned char> h(bytes, 0);
+    std::memcpy(h.data(), t.alpha, nn); std::memcpy(h.data() + nn, t.row, nn); std::memcpy(h.data() + 2 * nn, t.col, nn);
+    std::memcpy(h.data() + off_re, t.re, nn * sizeof(double)); std::memcpy(h.data() + off_re + nn * sizeof(double), t.im, nn * sizeof(double));
+    TM_CUDA(tm_dev_alloc(&ctx->d_grad_tab, bytes));
+    TM_CUDA(cudaMemcpy(ctx->d_grad_tab, h.data(), bytes, cudaMemcpyHostToDevice));
+    const unsigned char* b = static_cast<const unsigned char*>(ctx->d_grad_tab);
+    ctx->grad_tab = TmGradDev{t.n, b, b + nn, b + 2 * nn, reinterpret_cast<const double*>(b + off_re),
+                              reinterpret_cast<const double*>(b + off_re) + nn};
+  }
+  return ctx->precision != TM_FP32 ? grad_positions_typed<double>(ctx, ctx->grad_aux, lambda, s, dp, out)
+                                   : grad_positions_typed<float>(ctx, ctx->grad_aux, lambda, s, dp, out);
 }
 
 int tm_mie_tmatrix(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64* out);
@@ -1464,8 +1492,8 @@ int tm_pair_cost(const tm_ctx* ctx, double* fp_instructions, double* flop) {
   if (!ctx) return TM_E_INVALID;
   double inst = 0.0, fl = 0.0;
   if (ctx->kernel == TM_KERNEL_COPLANAR) {
-    const int I[7] = {0, TM_COP_FPINST_L1, TM_COP_FPINST_L2, TM_COP_FPINST_L3, TM_COP4_FPINST_L4, TM_COP4_FPINST_L5, TM_COP4_FPINST_L6};
-    const int F[7] = {0, TM_COP_FLOP_L1, TM_COP_FLOP_L2, TM_COP_FLOP_L3, TM_COP4_FLOP_L4, TM_COP4_FLOP_L5, TM_COP4_FLOP_L6};
+    const int I[8] = {0, TM_COP_FPINST_L1, TM_COP_FPINST_L2, TM_COP_FPINST_L3, TM_COP4_FPINST_L4, TM_COP4_FPINST_L5, TM_COP4_FPINST_L6, TM_COP4_FPINST_L7};
+    const int F[8] = {0, TM_COP_FLOP_L1, TM_COP_FLOP_L2, TM_COP_FLOP_L3, TM_COP4_FLOP_L4, TM_COP4_FLOP_L5, TM_COP4_FLOP_L6, TM_COP4_FLOP_L7};
     inst = I[ctx->lmax]; fl = F[ctx->lmax];
   } else if (ctx->kernel == TM_KERNEL_SYM3D) {
     const int I[4] = {0, TM_G3D_FPINST_L1, TM_G3D_FPINST_L2, TM_G3D_FPINST_L3};

@@ -4,8 +4,10 @@
 #include <cstdint>
 #include <cstdio>
 
-#define TM_MAX_LMAX 6
-#define TM_MAX_NQ (2 * TM_MAX_LMAX + 1)
+#define TM_MAX_LMAX 6                                      // largest truncation of the public API (the paper's)
+#define TM_INT_LMAX 7                                      // internal: the position gradient at lmax runs one all-pairs product at lmax + 1
+#define TM_MAX_NQ (2 * TM_INT_LMAX + 1)
+#define TM_MAX_MODES (2 * TM_INT_LMAX * (TM_INT_LMAX + 2))  // 126
 
 template <typename R> struct Cx;                       // interleaved complex of the compute precision
 template <> struct __align__(16) Cx<double> { double re, im; };
@@ -44,8 +46,8 @@ struct TmTile { int tgt_start, tgt_count, src_start, src_count; };
 
 // Small per-lmax tables, one device copy per context (tm_ctx::d_const).
 struct TmConst {
-  int perm_neg_m[96];          // flat index of (l,-m,p)               (structural identity S3)
-  int mode_l[96], mode_m[96], mode_p[96];
+  int perm_neg_m[TM_MAX_MODES];          // flat index of (l,-m,p)               (structural identity S3)
+  int mode_l[TM_MAX_MODES], mode_m[TM_MAX_MODES], mode_p[TM_MAX_MODES];
   double leg_a[TM_MAX_NQ + 1][TM_MAX_NQ + 1];   // normalised Legendre recurrence Pbar_q^mu = a (ct Pbar_{q-1}^mu - b Pbar_{q-2}^mu)
   double leg_b[TM_MAX_NQ + 1][TM_MAX_NQ + 1];
   double leg_d[TM_MAX_NQ + 1];                  // Pbar_mu^mu = d[mu] * sin(theta) * Pbar_{mu-1}^{mu-1}

@@ -37,7 +37,7 @@ k_tapply(int mode, int L, int n_scat, int n_chunk, const Cx<R>* __restrict__ x, 
          Cx<R>* __restrict__ y, const Cx<R>* __restrict__ T, int diag, const int* __restrict__ type_of,
          const TmConst* __restrict__ cst, const int* __restrict__ n_active) {
   if (n_active != nullptr && *n_active == 0) return;
-  __shared__ Cx<R> s_v[JB * 96];
+  __shared__ Cx<R> s_v[JB * TM_MAX_MODES];
   const int j0 = blockIdx.x * JB;
   const int nj = min(JB, n_scat - j0);
   const int ne = nj * L;
@@ -343,4 +343,44 @@ k_bilinear_rows(int L, int n_scat, const Cx<R>* __restrict__ left, const Cx<RD>*
   }
   sr = warp_sum(sr); si = warp_sum(si);
   if (lane == 0) { out[(size_t)j * out_stride].x += sr; out[(size_t)j * out_stride].y += si; }
+}
+
+// ------------------------------------------------------------------------------------------------ analytic position gradient
+// dA/dd_alpha = k D^alpha A^ext (gen_tables.py: gradient_entries).  k_pad_modes embeds a coefficient
+// vector of truncation lmax into the mode order of lmax + 1 (zeros for l = lmax + 1; xp is cleared by the caller);
+// k_grad_contract adds  out[j][alpha] += k * sum_e left_j[perm(row_e)] D_e v_j[col_e]  (alpha = alpha_e), v = A^ext (padded x).
+struct TmGradDev { int n; const uint8_t* alpha; const uint8_t* row; const uint8_t* col; const double* re; const double* im; };
+
+template <typename R>
+__global__ void k_pad_modes(const Cx<R>* __restrict__ x, Cx<R>* __restrict__ xp, int L, int Le, size_t n) {
+  const size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+  if (e >= n) return;
+  const size_t j = e / L;
+  const int a = (int)(e - j * L);
+  const int ae = a < L / 2 ? a : a - L / 2 + Le / 2;            // flat index p * (L/2) + l (l + 1) - 1 + m (reading R1)
+  xp[j * Le + ae] = x[e];
+}
+
+template <typename R>
+__global__ void __launch_bounds__(128)
+k_grad_contract(int L, int Le, int n_scat, const Cx<R>* __restrict__ left, const Cx<R>* __restrict__ v,
+                const TmConst* __restrict__ cst, TmGradDev tab, double k, double2* __restrict__ out) {
+  const int j = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (j >= n_scat) return;
+  double sr[3] = {0.0, 0.0, 0.0}, si[3] = {0.0, 0.0, 0.0};
+  for (int e = lane; e < tab.n; e += 32) {
+    const Cx<R> l = left[(size_t)j * L + cst->perm_neg_m[tab.row[e]]];
+    const Cx<R> w = v[(size_t)j * Le + tab.col[e]];
+    const double dr = tab.re[e], di = tab.im[e];
+    const double tr = dr * (double)w.re - di * (double)w.im, ti = dr * (double)w.im + di * (double)w.re;      // D_e v
+    const double pr = (double)l.re * tr - (double)l.im * ti, pi = (double)l.re * ti + (double)l.im * tr;
+    const int a = tab.alpha[e];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) if (a == q) { sr[q] += pr; si[q] += pi; }
+  }
+#pragma unroll
+  for (int q = 0; q < 3; ++q) {
+    const double a = warp_sum(sr[q]), b = warp_sum(si[q]);
+    if (lane == 0) { out[(size_t)j * 3 + q].x += k * a; out[(size_t)j * 3 + q].y += k * b; }
+  }
 }

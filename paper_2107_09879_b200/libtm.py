@@ -90,7 +90,7 @@ def lib():
         L.tm_kernel_time.argtypes = [vp, ci, ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(ctypes.c_longlong)]
         L.tm_mie_tmatrix.argtypes = [ci, cd, cd, c64, vp]
         L.tm_grad_tmatrix.argtypes = [vp, vp, vp, vp, vp]
-        L.tm_grad_positions.argtypes = [vp, vp, vp, vp, cd, vp]
+        L.tm_grad_positions.argtypes = [vp, vp, vp, vp, vp]
         L.tm_mie_tmatrix_dR.argtypes = [ci, cd, cd, c64, vp]
         L.tm_nullfield_tmatrix.argtypes = [ci, ci, cd, c64, ci, ci, vp, vp, vp, vp, vp, vp]
         L.tm_nullfield_dtmatrix.argtypes = [ci, ci, cd, c64, ci, ci, vp, vp, vp, vp, cd, vp, vp]
@@ -339,14 +339,14 @@ class Solver:
         self._check(lib().tm_grad_tmatrix(self._h, _ptr(dT), _ptr(lam), _ptr(s), _ptr(out)))
         return out
 
-    def grad_positions(self, lam, s, dp=None, h=0.0, out=None):
+    def grad_positions(self, lam, s, dp=None, out=None):
         """out[j, alpha] = lambda^T T (dA/dx_{j,alpha}) s (+ mu_j^T dp[j, alpha])  (tm_grad_positions; PAPER.md Eqs. IV3-IV9)."""
         lam = np.ascontiguousarray(lam, dtype=np.complex128) if isinstance(lam, np.ndarray) else lam
         s = np.ascontiguousarray(s, dtype=np.complex128) if isinstance(s, np.ndarray) else s
         if dp is not None and isinstance(dp, np.ndarray):
             dp = np.ascontiguousarray(dp, dtype=np.complex128)
         out = np.empty((self.n_scat, 3), dtype=np.complex128) if out is None else out
-        self._check(lib().tm_grad_positions(self._h, _ptr(lam), _ptr(s), _ptr(dp), float(h), _ptr(out)))
+        self._check(lib().tm_grad_positions(self._h, _ptr(lam), _ptr(s), _ptr(dp), _ptr(out)))
         return out
 
     def kernel_time(self, reset=False):

@@ -150,3 +150,30 @@ def test_axial_factorisation_reproduces_the_oracle_block(lmax):
         u_full = np.conj(ipow) * np.exp(-1j * np.array([m for (_, m, _) in md]) * phi) * ut
         ref = tr.block(lmax, K, np.array([d[0], d[1], 0.0]), np.zeros(3)) @ x
         assert np.abs(u_full - ref).max() <= 2e-13 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("lmax", [1, 2, 3, 5])
+def test_generated_gradient_tables_match_oracle_derivative(lmax):
+    """The product's analytic position derivative  dA/dd_alpha = k D^alpha A^ext  (gen_tables.py: gradient_entries; one
+    all-pairs product at lmax + 1 and a constant sparse matrix) against the oracle's chain-rule derivative of Eq. I17
+    (oracle/translation.py: d_block, itself pinned by central differences): two independent routes to the same matrix."""
+    text = open(os.path.join(GEN, "tm_tables_gen.h")).read()
+    tag = f"L{lmax}"
+    al = _parse_table(text, f"tm_grad_alpha_{tag}", int)
+    row = _parse_table(text, f"tm_grad_row_{tag}", int)
+    col = _parse_table(text, f"tm_grad_col_{tag}", int)
+    re_ = _parse_table(text, f"tm_grad_re_{tag}", float)
+    im_ = _parse_table(text, f"tm_grad_im_{tag}", float)
+    L, Le = n_modes(lmax), n_modes(lmax + 1)
+    D = np.zeros((3, L, Le), dtype=complex)
+    for a, r, c, x, y in zip(al, row, col, re_, im_):
+        D[a, r, c] += x + 1j * y
+    ext = mode_list(lmax + 1)
+    cols = np.array([ext.index(t) for t in mode_list(lmax)])           # the lmax modes inside the lmax + 1 ordering
+    rng = np.random.default_rng(80 + lmax)
+    for d in (rng.uniform(-2, 2, 3), np.array([0.7, -0.2, 0.0]), np.array([0.0, 0.0, 0.9])):
+        Aext = tr.block(lmax + 1, K, d, np.zeros(3))[:, cols]          # rows l' <= lmax + 1, source columns l <= lmax
+        ref = tr.d_block(lmax, K, d, np.zeros(3))
+        for a in range(3):
+            got = K * D[a] @ Aext
+            assert np.abs(got - ref[a]).max() <= 1e-12 * np.abs(ref[a]).max(), (lmax, a)

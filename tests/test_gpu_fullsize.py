@@ -22,7 +22,7 @@ def tm():
     return libtm
 
 
-from parity_metric import rel  # noqa: E402  (L2 AND per-(l,p)-block / per-point max error)
+from parity_metric import rel, rel_solve  # noqa: E402,F401  (L2 AND per-(l,p)-block / per-point max error; solutions: L2 AND max norm)
 
 
 def rand_x(shape, seed):
@@ -75,7 +75,7 @@ def test_cfg2_full_solve_vs_dense_lu_golden(tm):
     s = tm.solver_for_workload(w)
     sol, info, rc = s.solve(w["tol"], w["restart"], w["max_iter"])
     assert rc == 0 and info[0].rel_residual <= w["tol"]
-    assert rel(sol, ref) <= 1e-9
+    assert rel_solve(sol, ref) <= 1e-9
     s.close()
 
 
@@ -107,7 +107,7 @@ def test_cfg4_windows_are_independent_at_full_size(tm):
               type_of=np.arange(hi - lo, dtype=np.int32), focus=w["focus"][5:6])
     s1 = tm.solver_for_workload(w1)
     sol1, info1, rc1 = s1.solve(1e-3, 20, 20)
-    assert rel(sol1, sol[lo:hi]) <= 1e-10
+    assert rel_solve(sol1, sol[lo:hi]) <= 1e-10
     assert info1[0].iterations == info[5].iterations
     s.close(); s1.close()
 

@@ -18,7 +18,7 @@ def tm():
     return libtm
 
 
-from parity_metric import rel  # noqa: E402  (L2 AND per-(l,p)-block / per-point max error)
+from parity_metric import rel, rel_solve  # noqa: E402,F401  (L2 AND per-(l,p)-block / per-point max error; solutions: L2 AND max norm)
 
 
 def test_jinc_incident_matches_oracle(tm):

@@ -20,7 +20,7 @@ def tm():
     return libtm
 
 
-from parity_metric import rel  # noqa: E402  (L2 AND per-(l,p)-block / per-point max error)
+from parity_metric import rel, rel_solve  # noqa: E402,F401  (L2 AND per-(l,p)-block / per-point max error; solutions: L2 AND max norm)
 
 
 def rand_x(shape, seed):
@@ -189,7 +189,7 @@ def test_solve_cfg1(tm):
     s = tm.solver_for_workload(w)
     sol, info, rc = s.solve(w["tol"], w["restart"], w["max_iter"])
     assert rc == 0 and info[0].converged and info[0].rel_residual <= w["tol"]
-    assert rel(sol, ref["s"]) <= 1e-9
+    assert rel_solve(sol, ref["s"]) <= 1e-9
     cext, csca = fields.cross_sections(w["lmax"], w["k"], w["pos"], sol, s.get_incident())
     assert abs(cext - csca) <= 1e-8 * abs(cext)          # lossless spheres: extinction = scattering
     s.close()
@@ -203,7 +203,7 @@ def test_solve_reduced_configs(tm, cfg, scale):
     s = tm.solver_for_workload(w)
     sol, info, rc = s.solve(1e-11, w["restart"], w["max_iter"])
     assert rc == 0, info[0].rel_residual
-    assert rel(sol, ref["s"]) <= 1e-9
+    assert rel_solve(sol, ref["s"]) <= 1e-9
     s.close()
 
 
@@ -215,10 +215,10 @@ def test_solve_windows_and_adjoint(tm):
     s = tm.solver_for_workload(w)
     sol, info, rc = s.solve(1e-11, 50, 2000)
     assert rc == 0 and len(info) == 4
-    assert rel(sol, ref["s"]) <= 1e-9
+    assert rel_solve(sol, ref["s"]) <= 1e-9
     lam, info2, rc2 = s.solve_adjoint(w["w_adj"], 1e-11, 50, 2000)
     assert rc2 == 0
-    assert rel(lam, ref["lam"]) <= 1e-9
+    assert rel_solve(lam, ref["lam"]) <= 1e-9
     # bilinear identity lam^T (T p) = w^T s  (exact link between forward and adjoint solves)
     t, type_of, diag = driver.tmatrices(w)
     b = system.apply_T(t, type_of, ref["p"], diag)
@@ -230,7 +230,7 @@ def test_solve_windows_and_adjoint(tm):
               type_of=np.arange(hi - lo, dtype=np.int32), focus=w["focus"][1:2])
     s1 = tm.solver_for_workload(w1)
     sol1, _, _ = s1.solve(1e-11, 50, 2000)
-    assert rel(sol1, sol[lo:hi]) <= 1e-9
+    assert rel_solve(sol1, sol[lo:hi]) <= 1e-9
     s.close(); s1.close()
     del rng
 
@@ -240,7 +240,7 @@ def test_solve_3d_cloud_full_T_general_kernel(tm):
     ref = driver.solve(w)
     s = tm.solver_for_workload(w)
     sol, info, rc = s.solve(w["tol"], w["restart"], w["max_iter"])
-    assert rc == 0 and rel(sol, ref["s"]) <= 1e-9
+    assert rc == 0 and rel_solve(sol, ref["s"]) <= 1e-9
     s.close()
 
 
@@ -249,7 +249,7 @@ def test_solve_fp32(tm):
     ref = driver.solve(w)
     s = tm.solver_for_workload(w, precision=tm.TM_FP32)
     sol, info, rc = s.solve(1e-6, 50, 2000)
-    assert rel(sol, ref["s"]) <= 1e-4
+    assert rel_solve(sol, ref["s"]) <= 1e-4
     assert info[0].rel_residual <= 5e-6
     s.close()
 

@@ -35,6 +35,10 @@ def test_adjoint_position_gradient_matches_finite_differences():
     for (j, a) in ((0, 0), (1, 2), (3, 1)):
         fd = gradient.fd_position(2, K, pos, radii, 4.0, inc, v, j, a)
         assert abs(g[j, a] - fd) <= 1e-6 * np.abs(g).max()
+    # exact incident derivative of a plane wave (d a_j / d x_j = i k a_j) instead of its central difference
+    kv = K * np.array([np.sin(0.4) * np.cos(-0.5), np.sin(0.4) * np.sin(-0.5), np.cos(0.4)])
+    g2, _, _ = gradient.adjoint_position_gradient(2, K, pos, radii, 4.0, inc, v, dinc_fn=lambda q: 1j * kv[None, :, None] * inc(q)[:, None, :])
+    assert np.abs(g2 - g).max() <= 1e-8 * np.abs(g).max()
 
 
 def test_analytic_translation_derivative_matches_central_differences():
