@@ -52,7 +52,8 @@ typedef struct { double beta, alpha; tm_c64 A_beta, A_alpha; } tm_plane_desc;
 /* Gaussian beam along +z, one focus per window (reading R9 of DESIGN.md: the angular-spectrum machinery of
  * Eqs. II9-II17, with a Gaussian spectral weight).  Transverse field on the focal plane
  * (Ax, Ay) exp(-|x_T - focus_T|^2 / w0^2).  focus: HOST pointer [n_win][3].  n_beta: Gauss-Legendre nodes in
- * the polar angle (0 -> default 400). */
+ * the polar angle; 0 -> 400 (reading R9), raised to k_b D_max beta_max / 2 + 40 when the largest source - scatterer
+ * distance D_max of a window needs more (beyond ~125 wavelengths for a jinc source); an explicit value is used as given. */
 typedef struct { const double *focus; double w0; tm_c64 Ax, Ay; int n_beta; } tm_gauss_desc;
 
 /* Superposition of jinc sources per window - the paper's Nyquist decomposition of a band-limited incident field
@@ -60,7 +61,7 @@ typedef struct { const double *focus; double w0; tm_c64 Ax, Ay; int n_beta; } tm
  * centred at src_xyz[s] = (x_0, y_0, z_0), propagating along +z, transverse field on its plane
  * (Ax_s, Ay_s) J_1(k rho)/(k rho); window w owns the sources src_ptr[w] <= s < src_ptr[w+1].
  * A field sampled on the lambda/2 grid is carried by sources of amplitude (pi/2) x sample (reading R17).
- * All pointers are HOST pointers.  n_beta: Gauss-Legendre nodes on [0, pi/2] (0 -> 400). */
+ * All pointers are HOST pointers.  n_beta: Gauss-Legendre nodes on [0, pi/2] (0 -> 400 or more, as in tm_gauss_desc). */
 typedef struct { int n_src; const double *src_xyz; const tm_c64 *amp /* [n_src][2] */; const int *src_ptr /* [n_win+1] */;
                  int n_beta; } tm_jinc_desc;
 
@@ -136,7 +137,8 @@ int tm_matvec(tm_ctx *ctx, int transpose, const tm_c64 *x, tm_c64 *y);
 /* Scattered fields at detector points (Eqs. I13/I24):
  *   E_sca(x) = sum_i sum_{lmp} s_{lmp;i} Phi_{lmp}(k_b (x - x_i)),  Z_b H_sca = -i sum s Phi_{l,m,1-p} (reading R10).
  *   pts [n_pts][3] doubles, s [n_scat][L], out [n_pts][3] Cartesian complex; all windows are summed
- *   (the paper sums the sub-region fields).  Points must not coincide with a scatterer centre.
+ *   (the paper sums the sub-region fields).  The outgoing waves of a scatterer are singular at its own centre:
+ *   for a point that coincides with a centre that scatterer's term is left out (the field of all the others is returned).
  *   TM_FIELD_E_INC: the incident E field of the last tm_set_incident (plane wave, Gaussian beams or jinc sources; all
  *   sources of all windows summed; s is ignored and may be NULL; TM_E_STATE after TM_INC_COEFFS or before tm_set_incident),
  *   so that E_total = E_INC + E_SCA. */
@@ -159,7 +161,10 @@ int tm_set_kernel(tm_ctx *ctx, int kernel);
 int tm_get_kernel(const tm_ctx *ctx);
 
 /* Device time (ms, CUDA events on the context's stream) of the all-pairs kernel launches since the last
- * call with reset != 0, and their count: lets a caller attribute time without a profiler. */
+ * call with reset > 0, and their count: lets a caller attribute time without a profiler.  reset > 0 (re)starts TIMING MODE:
+ * an event pair around every all-pairs launch; in timing mode a restart cycle is issued launch by launch.  reset < 0
+ * leaves timing mode (the default) and zeroes the launch counters: the solvers then replay each full restart cycle of a window-sized problem as one CUDA
+ * graph (windows of ~31^2 scatterers are launch-bound), and only the launch counts are maintained. */
 int tm_kernel_time(tm_ctx *ctx, int reset, double *allpairs_ms, long long *allpairs_launches,
                    long long *total_launches);
 
@@ -188,7 +193,8 @@ int tm_grad_tmatrix(tm_ctx *ctx, const tm_c64 *dT, const tm_c64 *lambda, const t
 int tm_grad_positions(tm_ctx *ctx, const tm_c64 *lambda, const tm_c64 *s, const tm_c64 *dp, tm_c64 *out);
 
 /* Host helper: d(diag T)/dR of the Mie T-matrix of tm_mie_tmatrix (Richardson-extrapolated central differences of the
- * closed form, relative accuracy ~1e-10), out[L]. */
+ * closed form with the RELATIVE step 1e-3 R, so the accuracy - about 1e-10 relative - does not depend on the length
+ * unit), out[L]. */
 int tm_mie_tmatrix_dR(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64 *out);
 
 /* Executed floating-point work of the active all-pairs kernel per ORDERED pair:

@@ -489,8 +489,11 @@ def coplanar_sectors_axial(lmax):
 COPLANAR_AXIAL = True      # False: direct pair-frame operator (sum over (row, col, q) terms), the round's first version
 
 
-def emit_axial_core(f, fac):
+def emit_axial_core(f, fac, sync_tag=None):
     """Straight-line code  u' = Gout (sum_q h_q Z''_q) G x'  for one half; x' in xr{k}/xi{k}, result in ur{k}/ui{k}.
+    sync_tag: emit TM_PHASE_SYNC(tag, k) after the frame change (k = 0) and after every |m''| block of the axial translation
+    (k = 1, 2, ...): block-wide barriers that keep the warps of a block inside one phase of the straight-line code, so that
+    the phase - not the whole loop body - has to fit the 32 KB instruction cache (lmax >= 5; a no-op elsewhere).
     Returns (FP instructions, flop)."""
     slots, slots2, G, entries, Gout = fac
     n = len(slots)
@@ -515,12 +518,18 @@ def emit_axial_core(f, fac):
                     flop += 2
             f.write(f"  const R w{part}{i} = {expr};\n")
     # axial translation, one |m''| block after the other; identical radial sums are formed once
+    if sync_tag is not None:
+        f.write(f"  TM_PHASE_SYNC({sync_tag}, 0);\n")
     f.write("  // axial translation along z'': diagonal in m''\n")
     known = {}
     by_row = {}
+    n_sync = 1
     for (i, j), lst in sorted(entries.items()):
         by_row.setdefault(i, []).append((j, lst))
     for i in range(n):
+        if sync_tag is not None and i > 0 and slots2[i][1] != slots2[i - 1][1]:
+            f.write(f"  TM_PHASE_SYNC({sync_tag}, {n_sync});\n")
+            n_sync += 1
         first = True
         for (j, lst) in by_row.get(i, []):
             s0 = 1 if lst[0][1] > 0 else -1
@@ -559,6 +568,8 @@ def emit_axial_core(f, fac):
                 flop += 8
         assert not first, "every F'' slot receives something"
     # u' = Gout u''
+    if sync_tag is not None:
+        f.write(f"  TM_PHASE_SYNC({sync_tag}, {n_sync});\n")
     f.write("  // frame change back F'' -> F'\n")
     for r, row in enumerate(Gout):
         for part in ("r", "i"):
@@ -947,6 +958,7 @@ def emit_coplanar4(lmaxes, path):
         f.write("// Coplanar translation apply for lmax 4..6: FOUR uncoupled sectors (z-mirror parity x y'-mirror sector), each split into\n")
         f.write("// G row groups so that one block's straight-line code stays near the instruction-cache size (DESIGN.md, kernel K2c4).\n")
         f.write("// xs: [own slots | partner slots] d-values of the sector; ar/ai: [own rows of the group | their partner share], stride AS.\n#pragma once\n\n")
+        f.write("#ifndef TM_PHASE_SYNC\n#define TM_PHASE_SYNC(lmax, k)      // device build: block-wide barrier between code phases (tm_allpairs.cuh)\n#endif\n\n")
         for lmax in lmaxes:
             md = modes(lmax)
             idx = {t_: i for i, t_ in enumerate(md)}
@@ -1008,7 +1020,7 @@ def emit_coplanar4(lmaxes, path):
                                     f"xi{k} = xs[{2 * k + 1}] * cm[{am}] + xs[{2 * (n + k)}] * sm[{am}];\n")
                             n_pairs += 1
                     nterm = nrowq = 0
-                    core = emit_axial_core(f, secs_axial[z]) if COP4_AXIAL else None
+                    core = emit_axial_core(f, secs_axial[z], sync_tag=lmax) if COP4_AXIAL else None
                     for r in range(r0, r1):
                         l, am, p, kind = slots[r]
                         lr = r - r0

@@ -439,6 +439,21 @@ k_allpairs_sym3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
 // shared memory [slot][thread], and only the sector's own x^new (<= 24 complex at lmax 6) and h_q stay in registers.
 // At lmax 6 a sector's straight-line code is ~120 KB, far beyond the instruction caches: the kernel is
 // instruction-fetch bound there, still an order of magnitude ahead of the table-driven kernel.
+// Phase barriers inside the generated pair code (gen_tables.py: emit_axial_core): bit k of TM_COP4_SYNC_L<lmax> enables
+// barrier k.  All threads of a block run the same straight-line code with a uniform trip count, so the barriers are legal.
+#ifndef TM_COP4_SYNC_L4
+#define TM_COP4_SYNC_L4 0
+#endif
+#ifndef TM_COP4_SYNC_L5
+#define TM_COP4_SYNC_L5 0
+#endif
+#ifndef TM_COP4_SYNC_L6
+#define TM_COP4_SYNC_L6 0
+#endif
+#ifndef TM_COP4_SYNC_L7
+#define TM_COP4_SYNC_L7 0
+#endif
+#define TM_PHASE_SYNC(lmax, k) do { if ((TM_COP4_SYNC_L##lmax >> (k)) & 1) __syncthreads(); } while (0)
 #include "generated/tm_coplanar4_gen.cuh"
 
 template <typename R, int LMAX, int Z, int G> struct Cop4;

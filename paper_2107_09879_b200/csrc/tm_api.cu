@@ -61,7 +61,11 @@ inline cudaError_t tm_dev_free(void* p) {
 constexpr int COP_SS = 64;       // coplanar kernel: sources per shared-memory stage
 constexpr int SYM3D_TJ = 128;    // generated 3-D kernel: targets per block
 constexpr int SYM3D_SS = 32;     // generated 3-D kernel: sources per stage
-constexpr int COP4_TJ = 128;     // four-sector coplanar kernel (lmax 4..6): targets per block
+constexpr int COP4_TJ = 128;     // four-sector coplanar kernel (lmax 4, 5, 7): targets per block
+constexpr int COP4_TJ_L6 = 256;  // lmax 6: ONE 8-warp block per SM, so that all warps of an SM run the same sector's code (a sector's
+                                 // loop body is 42 KB > the 32 KB L1.5 instruction cache; two co-resident 4-warp blocks of
+                                 // DIFFERENT sectors double the footprint; measured 6.80 -> 6.50 ms on the 56x56 lattice)
+inline int cop4_tj(int lmax) { return lmax == 6 ? COP4_TJ_L6 : COP4_TJ; }
 constexpr int COP4_SS = 16;      // ... sources per stage
 constexpr int MAX_RESTART = 300;
 inline int cop4_groups(int lmax) {   // row groups per sector of the four-sector coplanar kernel
@@ -93,6 +97,7 @@ struct tm_ctx {
   int cop_tj = 128;                     // coplanar kernel: targets per block (-DTM_COP_TJ=256 for experiments)
 
   double* d_pos = nullptr;
+  std::vector<double> h_pos;      // host copy (quadrature sizing of the angular-spectrum sources)
   int* d_win_of = nullptr;
   int* d_type_of = nullptr;
   void* d_T = nullptr;           // Cx<R> [n_types][L] or [n_types][L][L]
@@ -120,6 +125,17 @@ struct tm_ctx {
 
   void* ws = nullptr; size_t ws_bytes = 0; bool ws_owned = false;
   Gmres gm;
+
+  // One restart cycle (all-pairs + fused Arnoldi step, m times) as a CUDA graph: window-sized problems are launch-bound
+  // (the paper's windows are ~31^2 scatterers).  Keyed on everything the captured launches bake in.
+  struct CycleGraph {
+    cudaGraphExec_t exec = nullptr;
+    int transpose = -1, m = 0, rbytes = 0, n_part = 0, kernel = 0, launches = 0;
+    double tol = 0.0;
+    const void *ws = nullptr, *T = nullptr, *upart = nullptr, *blob = nullptr, *tiles = nullptr;
+  } cyc[2];
+  bool graphs_ok = true;          // cleared when a capture fails (direct launches from then on)
+  bool capturing = false;
 
   // timing of the all-pairs kernel
   bool time_kernels = false;
@@ -257,7 +273,7 @@ template <typename R> const Cx<R>* Tptr(const tm_ctx* c) {
 int grid_for(size_t n, int block) { return (int)std::min<size_t>((n + block - 1) / block, 148 * 32); }
 
 void tick(tm_ctx* c, bool allpairs_begin) {
-  if (!c->time_kernels) return;
+  if (!c->time_kernels || c->capturing) return;
   if (c->ev_used + 2 > c->ev.size()) return;
   if (allpairs_begin) cudaEventRecord(c->ev[c->ev_used], c->stream);
   else { cudaEventRecord(c->ev[c->ev_used + 1], c->stream); c->ev_used += 2; }
@@ -273,18 +289,18 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
   if (c->kernel == TM_KERNEL_COPLANAR && c->lmax > 3) {
     // (z-mirror parity, y'-mirror sector) x row group: slowest grid dimension
     grid.z = 4 * cop4_groups(c->lmax);
-#define TM_LAUNCH_C4(LM)                                                                                        \
+#define TM_LAUNCH_C4(LM, TJ_)                                                                                   \
   {                                                                                                             \
-    const size_t sm = Cop4Smem<R, LM, COP4_TJ, COP4_SS>::bytes;                                                 \
-    cudaFuncSetAttribute(k_allpairs_coplanar4<R, LM, COP4_TJ, COP4_SS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
-    k_allpairs_coplanar4<R, LM, COP4_TJ, COP4_SS><<<grid, COP4_TJ, sm, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat, \
-                                                                                    k_over_pi, inv_k, n_active, c->shift); \
+    const size_t sm = Cop4Smem<R, LM, TJ_, COP4_SS>::bytes;                                                     \
+    cudaFuncSetAttribute(k_allpairs_coplanar4<R, LM, TJ_, COP4_SS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
+    k_allpairs_coplanar4<R, LM, TJ_, COP4_SS><<<grid, TJ_, sm, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat, \
+                                                                            k_over_pi, inv_k, n_active, c->shift); \
   }
     switch (c->lmax) {
-      case 4: TM_LAUNCH_C4(4) break;
-      case 5: TM_LAUNCH_C4(5) break;
-      case 6: TM_LAUNCH_C4(6) break;
-      default: TM_LAUNCH_C4(7) break;
+      case 4: TM_LAUNCH_C4(4, COP4_TJ) break;
+      case 5: TM_LAUNCH_C4(5, COP4_TJ) break;
+      case 6: TM_LAUNCH_C4(6, COP4_TJ_L6) break;
+      default: TM_LAUNCH_C4(7, COP4_TJ) break;
     }
 #undef TM_LAUNCH_C4
   } else if (c->kernel == TM_KERNEL_COPLANAR) {
@@ -474,7 +490,9 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
     ctx->total_launches += 4;
     const int mc = std::min(m, o.max_iter - total);
     last_mc = mc;
-    for (int j = 0; j < mc; ++j) {
+    // the Arnoldi steps of this cycle: enqueue(j0, j1) issues steps j0..j1-1 (directly or into a stream capture)
+    auto enqueue = [&](int j0, int j1) -> int {
+    for (int j = j0; j < j1; ++j) {
       Cx<R>* Vj = V + (size_t)j * n;
       const bool fuse_t = coop && ctx->diag;       // T application folded into the cooperative step
       if (fuse_t) {
@@ -483,7 +501,6 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
       } else {
         TM_CUDA(apply_operator<R>(ctx, transpose, Vj, W, ZV, S.n_active));
       }
-      matvecs++;
       // split the basis vectors of a dot-product pass over gridDim.y when there are few chunks
       const int G = std::max(1, std::min((j + 1 + 7) / 8, (148 * 4 + nc - 1) / nc));
       const size_t sm_a = (size_t)(j + 1) * sizeof(double2);
@@ -524,6 +541,48 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
 #undef TM_DOTS
 #undef TM_AXPY
     }
+    return TM_OK;
+    };
+    // CUDA graph of a full cycle (cooperative path only: small / medium problems, where the ~2 m launches of a cycle
+    // cost more in launch gaps than in work).  Timing mode (tm_kernel_time) keeps direct launches: events per launch.
+    bool launched = false;
+    if (coop && ctx->graphs_ok && !ctx->time_kernels && mc == m && m >= 4) {
+      tm_ctx::CycleGraph& G = ctx->cyc[transpose == 1 ? 1 : 0];
+      const void* Tp = Tptr<R>(ctx);
+      const bool hit = G.exec && G.transpose == transpose && G.m == m && G.rbytes == (int)sizeof(R) && G.n_part == ctx->n_part &&
+                       G.kernel == ctx->kernel && G.tol == o.tol && G.ws == ctx->ws && G.T == Tp && G.upart == ctx->d_upart &&
+                       G.blob == ctx->gm.blob && G.tiles == ctx->d_tiles;
+      if (!hit) {
+        if (G.exec) { cudaGraphExecDestroy(G.exec); G.exec = nullptr; }
+        const long long l0 = ctx->total_launches, a0 = ctx->allpairs_launches;
+        cudaGraph_t graph = nullptr;
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+          ctx->capturing = true;
+          const int rc_cap = enqueue(0, m);
+          ctx->capturing = false;
+          const cudaError_t ee = cudaStreamEndCapture(st, &graph);
+          if (rc_cap == TM_OK && ee == cudaSuccess && graph && cudaGraphInstantiate(&G.exec, graph, 0) == cudaSuccess) {
+            G.transpose = transpose; G.m = m; G.rbytes = (int)sizeof(R); G.n_part = ctx->n_part; G.kernel = ctx->kernel;
+            G.tol = o.tol; G.ws = ctx->ws; G.T = Tp; G.upart = ctx->d_upart; G.blob = ctx->gm.blob; G.tiles = ctx->d_tiles;
+            G.launches = (int)(ctx->total_launches - l0);
+          } else {
+            G.exec = nullptr; ctx->graphs_ok = false;
+          }
+          if (graph) cudaGraphDestroy(graph);
+        } else {
+          ctx->graphs_ok = false;
+        }
+        cudaGetLastError();
+        ctx->total_launches = l0; ctx->allpairs_launches = a0;       // the capture pass launched nothing
+      }
+      if (G.exec) {
+        TM_CUDA(cudaGraphLaunch(G.exec, st));
+        ctx->total_launches += G.launches; ctx->allpairs_launches += m;
+        launched = true;
+      }
+    }
+    if (!launched) { const int rc_e = enqueue(0, mc); if (rc_e != TM_OK) return rc_e; }
+    matvecs += mc;
     // x += V y ; r = b - M x
     k_gmres_solve_y<<<nw, 32, 0, st>>>(S, nw);
     if (ctx->ept == 1) k_axpy<R, 1, RX><<<nc, TM_VT, (size_t)m * sizeof(double2), st>>>(V, n, m, S.y, S.ldh, +1.0, X, ctx->d_chunks, nullptr, nullptr, nc, ctx->d_win_chunk_ptr, nullptr);
@@ -609,7 +668,7 @@ int configure_kernel(tm_ctx* ctx) {
   int tgt_per_tile;
   const bool gen = want == TM_KERNEL_COPLANAR || want == TM_KERNEL_SYM3D;      // generated kernels: thread = target
   switch (gen ? 0 : ctx->lmax) {
-    case 0: tgt_per_tile = want == TM_KERNEL_SYM3D ? SYM3D_TJ : (ctx->lmax > 3 ? COP4_TJ : ctx->cop_tj); break;
+    case 0: tgt_per_tile = want == TM_KERNEL_SYM3D ? SYM3D_TJ : (ctx->lmax > 3 ? cop4_tj(ctx->lmax) : ctx->cop_tj); break;
     case 1: case 2: case 3: tgt_per_tile = 4; break;
     default: tgt_per_tile = 2; break;
   }
@@ -624,8 +683,8 @@ int configure_kernel(tm_ctx* ctx) {
   // Source chunks: pick the chunk count that minimises (waves of resident blocks) x (sources per block), so that
   // small problems fill the 148 SMs (2 resident 128-thread blocks each at 255 registers) and large ones end
   // without a long tail; bounded by 64 chunks, >= 32 sources per chunk and 2 GB of partial sums.
-  const long long slots = 148LL * (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj : (want == TM_KERNEL_SYM3D ? 2 : 4));
   const bool cop4 = want == TM_KERNEL_COPLANAR && ctx->lmax > 3;   // four-sector coplanar kernel (lmax 4..6)
+  const long long slots = 148LL * (cop4 ? 256 / cop4_tj(ctx->lmax) : (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj : (want == TM_KERNEL_SYM3D ? 2 : 4)));
   const int cop4_z = !cop4 ? 0 : 4 * cop4_groups(ctx->lmax);
   const long long blocks1 = (long long)ctx->n_tiles * (cop4 ? cop4_z : (gen ? 2 : 1));
   const int part_mult = (want == TM_KERNEL_SYM3D || cop4) ? 2 : 1;   // one partial buffer per (chunk, y'-sector)
@@ -716,6 +775,7 @@ const char* tm_last_error(const tm_ctx* ctx) { return ctx ? ctx->err.c_str() : g
 void tm_destroy(tm_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
+  for (auto& g : c->cyc) if (g.exec) cudaGraphExecDestroy(g.exec);
   if (c->grad_aux) tm_destroy(c->grad_aux);
   tm_dev_free(c->d_grad_tab);
   tm_dev_free(c->d_pos); tm_dev_free(c->d_win_of); tm_dev_free(c->d_type_of); tm_dev_free(c->d_T); tm_dev_free(c->d_T32); tm_dev_free(c->d_p);
@@ -780,7 +840,7 @@ int create_ctx(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const
   tm_ctx* c = new tm_ctx();
   c->n_scat = n_scat; c->n_win = n_win; c->lmax = lmax; c->L = tm_num_modes(lmax); c->precision = precision;
   c->k = k_b; c->n = (size_t)n_scat * c->L; c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
-  c->win_ptr = wp; c->coplanar = coplanar;
+  c->win_ptr = wp; c->coplanar = coplanar; c->h_pos = hpos;
   ctx = c;
 #define TM_CREATE_CUDA(call)                                                                  \
   do {                                                                                        \
@@ -915,7 +975,10 @@ int tm_kernel_time(tm_ctx* ctx, int reset, double* allpairs_ms, long long* allpa
   if (allpairs_ms) *allpairs_ms = ms;
   if (allpairs_launches) *allpairs_launches = ctx->allpairs_launches;
   if (total_launches) *total_launches = ctx->total_launches;
-  if (reset) {
+  if (reset < 0) {                               // leave timing mode: restart cycles run as CUDA graphs again; counters restart
+    ctx->time_kernels = false; ctx->ev_used = 0; ctx->allpairs_launches = 0; ctx->total_launches = 0;
+  }
+  if (reset > 0) {
     if (ctx->ev.empty()) {
       ctx->ev.resize(2 * 4096);
       for (cudaEvent_t& e : ctx->ev) TM_CUDA(cudaEventCreate(&e));
@@ -1106,8 +1169,29 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
       for (int sidx = 0; sidx < 2 * d->n_src; ++sidx) hamp.push_back(make_double2(d->amp[sidx].re, d->amp[sidx].im));
       nb_req = d->n_beta;
     }
-    const int nb = nb_req > 0 ? nb_req : 400;
     const size_t nsrc = hsrc.size() / 3;
+    // Default node count: 400 (reading R9: part of the definition for the configs), raised when the geometry needs more.
+    // The integrand J_n(k rho sin b) e^{i k z cos b} turns by at most k D radians per unit of beta, D = source - scatterer
+    // distance, so [0, beta_max] holds k D beta_max / (2 pi) periods; Gauss-Legendre resolves an oscillatory integrand with
+    // about pi nodes per period plus a margin:  n >= k D_max beta_max / 2 + 40  (D_max over the pairs of each window).
+    int nb = nb_req > 0 ? nb_req : 400;
+    if (nb_req <= 0 && nsrc > 0) {
+      double dmax2 = 0.0;
+      for (int w = 0; w < ctx->n_win; ++w) {
+        const int i0 = ctx->win_ptr[w], i1 = ctx->win_ptr[w + 1];
+        if (i1 <= i0 || hptr[w + 1] <= hptr[w]) continue;
+        double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+        for (int i = i0; i < i1; ++i)
+          for (int a = 0; a < 3; ++a) { lo[a] = std::min(lo[a], ctx->h_pos[3 * (size_t)i + a]); hi[a] = std::max(hi[a], ctx->h_pos[3 * (size_t)i + a]); }
+        for (int sidx = hptr[w]; sidx < hptr[w + 1]; ++sidx) {
+          double d2 = 0.0;
+          for (int a = 0; a < 3; ++a) { const double x = hsrc[3 * (size_t)sidx + a]; const double d = std::max(std::fabs(x - lo[a]), std::fabs(x - hi[a])); d2 += d * d; }
+          dmax2 = std::max(dmax2, d2);
+        }
+      }
+      const double need = 0.5 * ctx->k * std::sqrt(dmax2) * bmax + 40.0;
+      if (need > nb) nb = (int)std::min(65536.0, std::ceil(need / 8.0) * 8.0);
+    }
     ctx->inc_src = hsrc; ctx->inc_amp = hamp; ctx->inc_kw = kw; ctx->inc_bmax = bmax; ctx->inc_nb = nb;
     std::vector<double> xg, wg, beta(nb), wq(nb);
     gauss_legendre(nb, xg, wg);
@@ -1395,8 +1479,7 @@ int tm_mie_tmatrix(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64* ou
 int tm_mie_tmatrix_dR(int lmax, double k_b, double radius, tm_c64 eps_r, tm_c64* out) {
   if (lmax < 1 || lmax > TM_MAX_LMAX || !(k_b > 0.0) || !(radius > 0.0) || !out) return TM_E_INVALID;
   const int L = tm_num_modes(lmax);
-  const double h = 1e-4 * (radius < 1.0 ? 1.0 : radius);
-  if (!(radius - h > 0.0)) return TM_E_INVALID;
+  const double h = 1e-3 * radius;            // relative step: the accuracy does not depend on the caller's length unit
   std::vector<tm_c64> a(L), b(L), c(L), d(L);
   tm_mie_tmatrix(lmax, k_b, radius + h, eps_r, a.data());
   tm_mie_tmatrix(lmax, k_b, radius - h, eps_r, b.data());

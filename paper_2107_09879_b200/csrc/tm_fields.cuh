@@ -25,6 +25,7 @@ k_fields(const double* __restrict__ pos, int n_scat, const double2* __restrict__
   for (int i = i0; i < i1; ++i) {
     const double dx = px - pos[3 * i], dy = py - pos[3 * i + 1], dz = pz - pos[3 * i + 2];
     const double rho2 = dx * dx + dy * dy, r2 = rho2 + dz * dz;
+    if (r2 == 0.0) continue;                         // point on this scatterer's centre: its own outgoing waves are singular there
     const double r = sqrt(r2), rho = sqrt(rho2);
     const double ct = dz / r, st = rho / r;
     const double cph = rho > 0.0 ? dx / rho : 1.0, sph = rho > 0.0 ? dy / rho : 0.0;

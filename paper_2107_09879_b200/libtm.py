@@ -350,8 +350,9 @@ class Solver:
         return out
 
     def kernel_time(self, reset=False):
+        """reset: True / 1 starts timing mode (events per all-pairs launch), -1 leaves it (tm_kernel_time)."""
         ms, n_ap, n_tot = ctypes.c_double(), ctypes.c_longlong(), ctypes.c_longlong()
-        self._check(lib().tm_kernel_time(self._h, 1 if reset else 0, ctypes.byref(ms), ctypes.byref(n_ap), ctypes.byref(n_tot)))
+        self._check(lib().tm_kernel_time(self._h, int(reset), ctypes.byref(ms), ctypes.byref(n_ap), ctypes.byref(n_tot)))
         return ms.value, n_ap.value, n_tot.value
 
 
