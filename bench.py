@@ -221,7 +221,7 @@ def measure(args, w, mode, steps, warmup, rank, world, local_rank, dist, st, pea
             peaks[pipe] = libtm.measure_fma_peak(peak_prec, st.cuda_stream)
         peak = peaks[pipe]
         kern_req = {"auto": libtm.TM_KERNEL_AUTO, "general": libtm.TM_KERNEL_GENERAL, "coplanar": libtm.TM_KERNEL_COPLANAR,
-                    "sym3d": libtm.TM_KERNEL_SYM3D}[args.kernel]
+                    "sym3d": libtm.TM_KERNEL_SYM3D, "rot3d": libtm.TM_KERNEL_ROT3D}[args.kernel]
         s = libtm.solver_for_workload(w, precision=prec, stream=st.cuda_stream, kernel=kern_req)
         ws = torch.empty(s.workspace_bytes(restart), dtype=torch.uint8, device="cuda")
         s.set_workspace(ws)
@@ -401,14 +401,15 @@ def measure(args, w, mode, steps, warmup, rank, world, local_rank, dist, st, pea
         "ms_per_step": t_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": {libtm.TM_FP64: "f64", libtm.TM_FP32: "f32"}.get(prec, "f32 cycles + f64 residual/iterate"), "data": "synthetic",
         "config": cfg,
-        "launch": {"kernel": {libtm.TM_KERNEL_COPLANAR: "coplanar", libtm.TM_KERNEL_SYM3D: "sym3d"}.get(kern, "general"),
+        "launch": {"kernel": {libtm.TM_KERNEL_COPLANAR: "coplanar", libtm.TM_KERNEL_SYM3D: "sym3d", libtm.TM_KERNEL_ROT3D: "rot3d"}.get(kern, "general"),
                    "parallelism": "replicas" if world > 1 else "single"},
         "solve": {"forward_iterations": max(i.iterations for i in info), "adjoint_iterations": max(i.iterations for i in info2),
                   "forward_rel_residual": max(i.rel_residual for i in info), "adjoint_rel_residual": max(i.rel_residual for i in info2),
                   "forward_seconds": info[0].seconds, "adjoint_seconds": info2[0].seconds, "converged": bool(rc == 0 and rc2 == 0),
                   "bounded": mode == "hotpath", "matvecs_per_step": matvecs, "matvecs_per_s": matvecs / (t_step * 1e-3)},
         "gpu_launches": int(tot_launches),
-        "roofline": {"bound": "alu", "kernel": {libtm.TM_KERNEL_COPLANAR: "k_allpairs_coplanar", libtm.TM_KERNEL_SYM3D: "k_allpairs_sym3d"}.get(kern, "k_allpairs_general"),
+        "roofline": {"bound": "alu", "kernel": {libtm.TM_KERNEL_COPLANAR: "k_allpairs_coplanar", libtm.TM_KERNEL_SYM3D: "k_allpairs_sym3d",
+                                                 libtm.TM_KERNEL_ROT3D: "k_allpairs_rot3d"}.get(kern, "k_allpairs_general"),
                      "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": (achieved / peak) if achieved else None,
                      "peak_source": "builder microbenchmark: tm_measure_fma_peak (register-resident FMA chains) on this GPU in this run; "
                                     "MEASURED_PEAKS.json has no FP64/FP32 FMA figure",
@@ -623,7 +624,7 @@ def main():
     ap.add_argument("--no-solve-record", action="store_true", help="hotpath mode: skip the config-2 full-solve sub-record")
     ap.add_argument("--group", type=int, default=16, help="nyquist mode: samples per group side")
     ap.add_argument("--padding", type=float, default=4.0, help="nyquist mode: padding in wavelengths")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "general", "coplanar", "sym3d"], help="force the all-pairs kernel variant")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "general", "coplanar", "sym3d", "rot3d"], help="force the all-pairs kernel variant")
     ap.add_argument("--lmax", type=int, default=None, help="override the VSWF truncation of a Mie config (lmax 6 = the paper's, PAPER.md:271)")
     ap.add_argument("--lmax-internal", type=int, default=0,
                     help="paper_case / nullfield modes: internal truncation of the null-field method (0 = lmax, the paper's setting)")

@@ -42,7 +42,7 @@ enum { TM_OK = 0, TM_NOT_CONVERGED = 1,
        TM_E_INVALID = -1, TM_E_OVERLAP = -2, TM_E_STATE = -3, TM_E_CUDA = -4, TM_E_NOMEM = -5 };
 enum { TM_INC_PLANE = 0, TM_INC_GAUSS = 1, TM_INC_COEFFS = 2, TM_INC_JINC = 3 };
 enum { TM_FIELD_E_SCA = 0, TM_FIELD_H_SCA = 1, TM_FIELD_E_INC = 2 };   /* H is returned as Z_b * H (reading R10) */
-enum { TM_KERNEL_AUTO = 0, TM_KERNEL_GENERAL = 1, TM_KERNEL_COPLANAR = 2, TM_KERNEL_SYM3D = 3 };
+enum { TM_KERNEL_AUTO = 0, TM_KERNEL_GENERAL = 1, TM_KERNEL_COPLANAR = 2, TM_KERNEL_SYM3D = 3, TM_KERNEL_ROT3D = 4 };
 
 /* Plane wave travelling along (beta = polar angle from +z, alpha = azimuth) with amplitude
  * A = A_beta * beta_hat + A_alpha * alpha_hat  (Eqs. II6-II7).
@@ -96,7 +96,7 @@ typedef struct {
  *   win_ptr   HOST pointer [n_win+1], monotone, win_ptr[0] = 0, win_ptr[n_win] = n_scat; NULL (with
  *             n_win = 1) => one window.  Scatterers interact only inside their window (reading R16;
  *             independent Nyquist windows batched on one GPU).
- *   lmax      1..6 (generated kernels: coplanar for any lmax when all z are equal, 3-D for lmax <= 3; table-driven otherwise)
+ *   lmax      1..6 (generated kernels: coplanar when all z are equal, rotation-based 3-D otherwise)
  *   k_b       background wavenumber (wavelength 1 => 2 pi)
  *   precision TM_FP64 or TM_FP32 (API data stays fp64)
  *   cuda_stream  a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) or NULL for the default stream
@@ -153,11 +153,13 @@ int tm_set_workspace(tm_ctx *ctx, void *dev_ptr, size_t bytes);
 /* Force the all-pairs kernel variant (TM_KERNEL_*):
  *   COPLANAR  generated code, all z equal (refused with TM_E_INVALID otherwise); two parity halves for lmax <= 3,
  *             four mirror sectors with shared-memory accumulators for lmax 4..6
- *   SYM3D     generated code, arbitrary 3-D positions, lmax <= 3 (refused otherwise)
- *   GENERAL   table-driven, arbitrary positions, lmax <= 6
- * Default AUTO = COPLANAR if all z are equal, else SYM3D if lmax <= 3, else GENERAL. */
+ *   ROT3D     generated code, arbitrary 3-D positions, every lmax: rotation - axial translation - rotation with the polar
+ *             rotation as constant frame change - phase rotation - constant frame change (O(L^1.5) work per pair)
+ *   SYM3D     generated code, arbitrary 3-D positions, lmax <= 3 (refused otherwise): direct pair-frame operator
+ *   GENERAL   table-driven, arbitrary positions, lmax <= 6 (correct-by-table reference)
+ * Default AUTO = COPLANAR if all z are equal, else ROT3D. */
 int tm_set_kernel(tm_ctx *ctx, int kernel);
-/* Which variant is active (TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR or TM_KERNEL_SYM3D). */
+/* Which variant is active (TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR, TM_KERNEL_SYM3D or TM_KERNEL_ROT3D). */
 int tm_get_kernel(const tm_ctx *ctx);
 
 /* Device time (ms, CUDA events on the context's stream) of the all-pairs kernel launches since the last

@@ -34,7 +34,7 @@ def generate(force=False):
     gen_py = os.path.join(CSRC, "gen_tables.py")
     stamp = os.path.join(GEN, "GENERATOR_SHA256")
     outs = [os.path.join(GEN, f) for f in ("tm_tables_gen.h", "tm_coplanar_gen.cuh", "tm_coplanar_f2_gen.cuh",
-                                           "tm_general3d_gen.cuh", "tm_coplanar4_gen.cuh")]
+                                           "tm_general3d_gen.cuh", "tm_coplanar4_gen.cuh", "tm_rot3d_gen.cuh")]
     have = open(stamp).read().strip() if os.path.exists(stamp) else ""
     if force or have != _gen_hash() or not all(os.path.exists(o) for o in outs):
         subprocess.check_call([sys.executable, gen_py])

@@ -1242,7 +1242,378 @@ def main():
     emit_general_sym([1, 2, 3], os.path.join(OUT, "tm_general3d_gen.cuh"))
     emit_coplanar4([4, 5, 6, 7], os.path.join(OUT, "tm_coplanar4_gen.cuh"))     # 7: internal (gradient at lmax 6)
     emit_coplanar_f2([1, 2, 3], os.path.join(OUT, "tm_coplanar_f2_gen.cuh"))
+    emit_rot3d([1, 2, 3, 4, 5, 6, 7], os.path.join(OUT, "tm_rot3d_gen.cuh"))      # 7: internal (gradient at lmax 6)
 
 
 if __name__ == "__main__":
     main()
+
+
+# ----------------------------------------------------------------------------- general 3-D, rotation - axial translation - rotation
+# Arbitrary pair direction (theta, phi), any lmax: rotate about z by phi (phases), then about y' by theta so that z'' is the
+# pair axis, translate along z'' (diagonal in m''), rotate back.  The theta rotation is NOT evaluated through Wigner-d
+# recurrences: with A = the fixed frame change F' -> F_y whose z axis is y' (x_y = x', y_y = -z', z_y = y'),
+#       D_l(theta) = A_l^-1 diag(e^{i m theta}) A_l ,
+# so a rotation by any theta is two applications of a CONSTANT matrix around a phase rotation - the same primitive as the
+# phi rotation.  All matrices are obtained numerically (40 digits) from the definition of the frame change (projection
+# of Ybar_lm, as frame_rotation), in +- bases in which they come out real and sparse (about 1.3 non-zeros per row), and
+# the assembled operator is asserted against the direct one (general_sym) at random angles before any code is emitted.
+def frame_rotation_axes(l, ax, _cache={}):
+    """D (rows m'' = -l..l, columns m' = -l..l): Ybar_{l,m'}(v) = sum_{m''} D[m'', m'] Ybar_{l,m''}(ax v); ax = rows of the new axes."""
+    key = (l, tuple(tuple(mp.nstr(mp.mpf(x), 30) for x in row) for row in ax))
+    if key in _cache:
+        return _cache[key]
+    N = 2 * l + 1
+    pts = []
+    for i in range(N + 3):
+        z = mp.mpf(2 * i + 1) / (N + 3) - 1
+        ph = i * mp.pi * (3 - mp.sqrt(5))
+        r = mp.sqrt(1 - z * z)
+        pts.append((r * mp.cos(ph), r * mp.sin(ph), z))
+
+    def ybar(m, v):
+        return pbar_general(l, abs(m), v[2]) * mp.e ** (1j * m * mp.atan2(v[1], v[0]))
+    Yp = mp.matrix(len(pts), N)
+    Ypp = mp.matrix(len(pts), N)
+    for i, v in enumerate(pts):
+        vpp = tuple(sum(mp.mpf(ax[a][b]) * v[b] for b in range(3)) for a in range(3))
+        for j, m in enumerate(range(-l, l + 1)):
+            Yp[i, j] = ybar(m, v)
+            Ypp[i, j] = ybar(m, vpp)
+    D = mp.inverse(Ypp[:N, :]) * Yp[:N, :]
+    assert mp.norm(Ypp * D - Yp) < mp.mpf(10) ** -28, "frame rotation: projection does not reproduce the extra directions"
+    _cache[key] = D
+    return D
+
+
+_rot3d_cache = {}
+
+
+def rot3d_sectors(lmax):
+    """Per y'-mirror sector (slots as in general_sym):
+      slots   B1 = B3 slots (l, |m|, p, kind) in the pair-azimuth frame F' / the pair-axis frame F''
+      slots2  B2 slots (l, |m_y|, p, kind, kappa) in the frame F_y (z_y = y'), kappa in {1, 1j}: the stored value is w / kappa
+      M1      rows over slots2: [(col in slots, real value)]     B2 <- B1  (and B2 <- B3)
+      M2      rows over slots:  [(col in slots2, real value)]    B3 <- B2  (and B1 <- B2)
+      pairs   [(i_plus, i_minus, m_y, form)] theta phase rotation of a (+,-) pair of slots2; form in {'cx', 'r+', 'r-'}:
+                 'cx':  a+ -> c a+ + i s a-,  a- -> c a- + i s a+        'r+': a+ -> c a+ + s a-, a- -> c a- - s a+
+                 'r-':  a+ -> c a+ - s a-,  a- -> c a- + s a+            (c, s = cos, sin(m_y theta); inverse: s -> -s)
+      entries {(row, col): [(q, value)]} axial operator in B3 (same |m''| only)."""
+    if lmax in _rot3d_cache:
+        return _rot3d_cache[lmax]
+    md = modes(lmax)
+    L = len(md)
+    nq = 2 * lmax + 1
+    idx = {t: i for i, t in enumerate(md)}
+    eps = mp.mpf(10) ** -28
+    ax_y = [[1, 0, 0], [0, 0, -1], [0, 1, 0]]
+    By = mp.matrix(L, L)
+    for p in (0, 1):
+        for l in range(1, lmax + 1):
+            A = frame_rotation_axes(l, ax_y)
+            for i, m2 in enumerate(range(-l, l + 1)):
+                for j, m1 in enumerate(range(-l, l + 1)):
+                    By[idx[(l, m2, p)], idx[(l, m1, p)]] = A[i, j]
+    Byi = mp.inverse(By)
+    Rm, Rinv, Zc, all2, S2, S2inv, pm_matrices = _axial_operators(lmax)
+    pos2 = {t: i for i, t in enumerate(all2)}
+    out = []
+    for sct, (slots, rows) in enumerate(general_sym(lmax)):
+        n = len(slots)
+        S, Sinv = pm_matrices(slots)
+        Mfull = By * Sinv                                      # F_y modes x B1
+        nzrows = [r for r in range(L) if any(abs(Mfull[r, c]) > eps for c in range(n))]
+        assert len(nzrows) == n, "a y'-sector must map onto one mirror-parity class of F_y modes"
+        combos = []
+        for p in (0, 1):
+            for l in range(1, lmax + 1):
+                for am in range(0, l + 1):
+                    if idx[(l, am, p)] not in nzrows:
+                        continue
+                    assert idx[(l, -am, p)] in nzrows
+                    combos += [(l, 0, p, "0")] if am == 0 else [(l, am, p, "+"), (l, am, p, "-")]
+        assert len(combos) == n
+        C, Cinv = pm_matrices(combos)                          # combos x L,  L x combos
+        M1c = C * Mfull                                        # B2 <- B1, complex
+        kappa = []
+        for r in range(n):
+            re = max(abs(mp.re(M1c[r, c])) for c in range(n))
+            im = max(abs(mp.im(M1c[r, c])) for c in range(n))
+            assert min(re, im) < eps and max(re, im) > eps, "rows of the frame change must be purely real or purely imaginary"
+            kappa.append(mp.mpc(1) if im < eps else mp.mpc(0, 1))
+        Kd = mp.diag(kappa)
+        Kdi = mp.diag([1 / k for k in kappa])
+        M1m = Kdi * M1c
+        M2m = S * Byi * Cinv * Kd                              # B3 <- B2
+        assert max(abs(mp.im(M1m[r, c])) for r in range(n) for c in range(n)) < eps
+        assert max(abs(mp.im(M2m[r, c])) for r in range(n) for c in range(n)) < eps
+        assert mp.norm(M2m * M1m - mp.eye(n)) < eps
+        M1 = [[(c, mp.re(M1m[r, c])) for c in range(n) if abs(M1m[r, c]) > eps] for r in range(n)]
+        M2 = [[(c, mp.re(M2m[r, c])) for c in range(n) if abs(M2m[r, c]) > eps] for r in range(n)]
+        slots2 = [(l, am, p, kind, kappa[r]) for r, (l, am, p, kind) in enumerate(combos)]
+        pairs = []
+        for r, (l, am, p, kind) in enumerate(combos):
+            if kind == "+":
+                assert combos[r + 1] == (l, am, p, "-")
+                ratio = kappa[r + 1] / kappa[r]                 # a+ -> c a+ + i s ratio a-
+                form = "cx" if abs(ratio - 1) < eps else ("r-" if abs(ratio - mp.mpc(0, 1)) < eps else "r+")
+                assert form != "r+" or abs(ratio + mp.mpc(0, 1)) < eps
+                pairs.append((r, r + 1, am, form))
+        entries = {}
+        sel = [pos2[t] for t in slots]
+        selset = {r: i for i, r in enumerate(sel)}
+        for q in range(nq):
+            for i, r in enumerate(sel):
+                for c in range(len(all2)):
+                    if abs(Zc[q][r, c]) > eps:
+                        assert c in selset and all2[c][1] == all2[r][1], "axial operator must stay inside the sector and inside |m''|"
+                        entries.setdefault((i, selset[c]), []).append((q, Zc[q][r, c]))
+        # end-to-end check against the direct operator at two random pair directions (phi = 0: the phi rotation is the kernel's)
+        for th in (mp.mpf("0.7317"), mp.mpf("2.4603")):
+            ct = mp.cos(th)
+            E = mp.matrix(n, n)
+            for r in range(n):
+                E[r, r] = 1
+            for (ip, im_, m, form) in pairs:
+                c_, s_ = mp.cos(m * th), mp.sin(m * th)
+                E[ip, ip] = c_
+                E[im_, im_] = c_
+                if form == "cx":
+                    E[ip, im_] = mp.mpc(0, 1) * s_
+                    E[im_, ip] = mp.mpc(0, 1) * s_
+                elif form == "r+":
+                    E[ip, im_] = s_
+                    E[im_, ip] = -s_
+                else:
+                    E[ip, im_] = -s_
+                    E[im_, ip] = s_
+            Ei = mp.inverse(E)
+            for q in range(nq):
+                Zq = mp.matrix(n, n)
+                for (i, j), lst in entries.items():
+                    for (qq, v) in lst:
+                        if qq == q:
+                            Zq[i, j] = v
+                Kf = M2m * Ei * M1m * Zq * M2m * E * M1m
+                Kq = mp.matrix(n, n)
+                for r in range(n):
+                    for (c, lst) in rows[r][q]:
+                        Kq[r, c] = sum(v * pbar_general(q, mu, ct) for (mu, v) in lst)
+                assert mp.norm(Kf - Kq) < mp.mpf(10) ** -25, ("rotation - axial translation - rotation differs from the direct operator", lmax, sct, q)
+        out.append((slots, slots2, M1, M2, pairs, entries))
+    _rot3d_cache[lmax] = out
+    return out
+
+
+def emit_rot3d(lmaxes, path):
+    """Straight-line code of rot3d_sectors(): one y'-mirror sector per call, three phases around a per-thread scratch vector
+    (sr/si, stride AS): A) per (l,p) block: phi rotation, frame change, theta rotation, frame change -> w (scratch);
+    B) per |m''| block: axial translation w -> t (scratch, in place); C) per (l,p) block: the way back and the accumulation."""
+    def lin(f, dst, src, rows, sel, counter):
+        """dst{r} = sum_c value * src{c} for r in sel (real constants, complex values)."""
+        for r in sel:
+            for part in ("r", "i"):
+                expr = None
+                for t, (c, v) in enumerate(rows[r]):
+                    if t == 0:
+                        if abs(v) == 1:
+                            expr = f"{'-' if v < 0 else ''}{src}{part}{c}"
+                        else:
+                            expr = f"R({lit(v)}) * {src}{part}{c}"
+                            counter[0] += 1
+                            counter[1] += 1
+                    else:
+                        expr = f"fma(R({lit(v)}), {src}{part}{c}, {expr})"
+                        counter[0] += 1
+                        counter[1] += 2
+                f.write(f"    const R {dst}{part}{r} = {expr};\n")
+
+    def theta_rot(f, src, dst, pairs, sel2, inverse, counter):
+        """phase rotation of the B2 slots in sel2: pairs get the real 2x2 rotation, m_y = 0 slots pass through."""
+        done = set()
+        for (ip, im_, m, form) in pairs:
+            if ip not in sel2:
+                continue
+            assert im_ in sel2 and form in ("r+", "r-")
+            sg = 1 if form == "r+" else -1          # a+ -> c a+ + sg s a-,  a- -> c a- - sg s a+
+            if inverse:
+                sg = -sg
+            a, b = ("", "-") if sg > 0 else ("-", "")
+            for part in ("r", "i"):
+                f.write(f"    const R {dst}{part}{ip} = fma({a}stm[{m}], {src}{part}{im_}, ctm[{m}] * {src}{part}{ip});\n")
+                f.write(f"    const R {dst}{part}{im_} = fma({b}stm[{m}], {src}{part}{ip}, ctm[{m}] * {src}{part}{im_});\n")
+            counter[0] += 8
+            counter[1] += 12
+            done.update((ip, im_))
+        for r in sel2:
+            if r not in done:
+                f.write(f"    const R {dst}r{r} = {src}r{r}, {dst}i{r} = {src}i{r};\n")
+
+    with open(path, "w") as f:
+        f.write("// GENERATED by gen_tables.py - do not edit.\n")
+        f.write("// General 3-D translation apply by rotation - axial translation - rotation for ANY pair direction (DESIGN.md, kernel K2r):\n")
+        f.write("// phi phases, constant frame change onto the frame whose z axis is y', theta phases, constant frame change back: z'' is the\n")
+        f.write("// pair axis; m''-diagonal axial translation; and the same way back.  One y'-mirror SECTOR per call (slots as in\n")
+        f.write("// tm_general3d_gen.cuh).  xs: [own | partner] d-values; cph/sph, cth/sth: cos/sin of the pair's azimuth and polar angle; hr/hi: h_q(kr);\n")
+        f.write("// sr/si: per-thread scratch (n slots, stride AS); ar/ai: accumulators [own n | partner n], stride AS.\n#pragma once\n\n")
+        for lmax in lmaxes:
+            md = modes(lmax)
+            idx = {t: i for i, t in enumerate(md)}
+            half_l = len(md) // 2
+            cost = [0, 0]
+            for sct, (slots, slots2, M1, M2, pairs, entries) in enumerate(rot3d_sectors(lmax)):
+                n = len(slots)
+                cnt = [0, 0]
+                blocks = []                 # (l, p) -> B1/B3 slot indices and B2 slot indices
+                for p in (0, 1):
+                    for l in range(1, lmax + 1):
+                        b1 = [k for k, s_ in enumerate(slots) if s_[0] == l and s_[2] == p]
+                        b2 = [k for k, s_ in enumerate(slots2) if s_[0] == l and s_[2] == p]
+                        if b1:
+                            assert len(b1) == len(b2)
+                            for r in b2:
+                                assert all(c in b1 for (c, _) in M1[r]), "frame change must be block diagonal in (l, p)"
+                            for r in b1:
+                                assert all(c in b2 for (c, _) in M2[r])
+                            blocks.append((b1, b2))
+                f.write(f"// lmax={lmax} sector={sct}: slots (l,|m|,p,kind) {slots}\n")
+                f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
+                        f"tm_r3d_pair_L{lmax}_S{sct}(const R* __restrict__ xs, R cph, R sph, R cth, R sth, "
+                        "const R* hr, const R* hi, R* sr, R* si, R* ar, R* ai) {\n")
+                phases = ("    R cm[%d], sm[%d], ctm[%d], stm[%d];\n    cm[0] = R(1); sm[0] = R(0); cm[1] = cph; sm[1] = sph; "
+                          "ctm[0] = R(1); stm[0] = R(0); ctm[1] = cth; stm[1] = sth;\n" % ((lmax + 1,) * 4))
+                for m in range(2, lmax + 1):
+                    phases += (f"    cm[{m}] = cm[{m - 1}] * cph - sm[{m - 1}] * sph; sm[{m}] = sm[{m - 1}] * cph + cm[{m - 1}] * sph; "
+                               f"ctm[{m}] = ctm[{m - 1}] * cth - stm[{m - 1}] * sth; stm[{m}] = stm[{m - 1}] * cth + ctm[{m - 1}] * sth;\n")
+                cnt[0] += 2 * 8 * max(0, lmax - 1)          # cos/sin(m phi), cos/sin(m theta) by recurrence, in phase A and again in phase C
+                cnt[1] += 2 * 12 * max(0, lmax - 1)
+                # ---- phase A
+                f.write("  // A: into the pair-axis frame, block by block in (l, p)\n  {\n" + phases)
+                for (b1, b2) in blocks:
+                    f.write("  {\n")
+                    for k in b1:
+                        l, am, p, kind = slots[k]
+                        if kind == "0":
+                            f.write(f"    const R xr{k} = xs[{2 * k}], xi{k} = xs[{2 * k + 1}];\n")
+                        else:
+                            f.write(f"    const R xr{k} = xs[{2 * k}] * cm[{am}] - xs[{2 * (n + k) + 1}] * sm[{am}], "
+                                    f"xi{k} = xs[{2 * k + 1}] * cm[{am}] + xs[{2 * (n + k)}] * sm[{am}];\n")
+                            cnt[0] += 4
+                            cnt[1] += 6
+                    lin(f, "v", "x", M1, b2, cnt)
+                    theta_rot(f, "v", "e", pairs, b2, False, cnt)
+                    lin(f, "w", "e", M2, b1, cnt)
+                    for k in b1:
+                        f.write(f"    sr[{k} * AS] = wr{k}; si[{k} * AS] = wi{k};\n")
+                    f.write("  }\n")
+                f.write("  }\n")
+                # ---- phase B
+                f.write("  // B: axial translation along z'', block by block in |m''| (scratch in place)\n")
+                for mm in sorted(set(s_[1] for s_ in slots)):
+                    grp = [k for k, s_ in enumerate(slots) if s_[1] == mm]
+                    f.write("  {\n")
+                    for k in grp:
+                        f.write(f"    const R wr{k} = sr[{k} * AS], wi{k} = si[{k} * AS];\n")
+                    known = {}
+                    for i in grp:
+                        first = True
+                        for j in grp:
+                            lst = entries.get((i, j))
+                            if not lst:
+                                continue
+                            s0 = 1 if lst[0][1] > 0 else -1
+                            key = tuple((q, mp.nstr(s0 * v, 30)) for (q, v) in lst)
+                            if key not in known:
+                                e = len(known)
+                                known[key] = e
+                                for part, hh in (("r", "hr"), ("i", "hi")):
+                                    expr = None
+                                    for t, (q, v) in enumerate(lst):
+                                        vv = s0 * v
+                                        if t == 0 and abs(vv) == 1:
+                                            expr = f"{'-' if vv < 0 else ''}{hh}[{q}]"
+                                        elif t == 0:
+                                            expr = f"R({lit(vv)}) * {hh}[{q}]"
+                                            cnt[0] += 1
+                                            cnt[1] += 1
+                                        else:
+                                            expr = f"fma(R({lit(vv)}), {hh}[{q}], {expr})"
+                                            cnt[0] += 1
+                                            cnt[1] += 2
+                                    f.write(f"    const R e{part}{e} = {expr};\n")
+                            e = known[key]
+                            sg = "" if s0 > 0 else "-"
+                            ng = "-" if s0 > 0 else ""
+                            if first:
+                                f.write(f"    R tr{i} = {sg}er{e} * wr{j}; tr{i} = fma({ng}ei{e}, wi{j}, tr{i}); "
+                                        f"R ti{i} = {sg}er{e} * wi{j}; ti{i} = fma({sg}ei{e}, wr{j}, ti{i});\n")
+                                cnt[0] += 4
+                                cnt[1] += 6
+                                first = False
+                            else:
+                                f.write(f"    tr{i} = fma({sg}er{e}, wr{j}, tr{i}); tr{i} = fma({ng}ei{e}, wi{j}, tr{i}); "
+                                        f"ti{i} = fma({sg}er{e}, wi{j}, ti{i}); ti{i} = fma({sg}ei{e}, wr{j}, ti{i});\n")
+                                cnt[0] += 4
+                                cnt[1] += 8
+                        assert not first
+                        f.write(f"    sr[{i} * AS] = tr{i}; si[{i} * AS] = ti{i};\n")     # w_i is already in a register: store t_i at once
+                    f.write("  }\n")
+                # ---- phase C
+                f.write("  // C: back into the pair-azimuth frame and accumulation (own sector: cos, partner sector: sin)\n  {\n" + phases)
+                for (b1, b2) in blocks:
+                    f.write("  {\n")
+                    for k in b1:
+                        f.write(f"    const R tr{k} = sr[{k} * AS], ti{k} = si[{k} * AS];\n")
+                    lin(f, "v", "t", M1, b2, cnt)
+                    theta_rot(f, "v", "e", pairs, b2, True, cnt)
+                    lin(f, "u", "e", M2, b1, cnt)
+                    for k in b1:
+                        l, am, p, kind = slots[k]
+                        if kind == "0":
+                            f.write(f"    ar[{k} * AS] += ur{k}; ai[{k} * AS] += ui{k};\n")
+                            cnt[0] += 2
+                            cnt[1] += 2
+                        else:
+                            f.write(f"    ar[{k} * AS] = fma(ur{k}, cm[{am}], ar[{k} * AS]); ai[{k} * AS] = fma(ui{k}, cm[{am}], ai[{k} * AS]);\n")
+                            f.write(f"    ar[{n + k} * AS] = fma(ui{k}, sm[{am}], ar[{n + k} * AS]); ai[{n + k} * AS] = fma(-ur{k}, sm[{am}], ai[{n + k} * AS]);\n")
+                            cnt[0] += 4
+                            cnt[1] += 8
+                    f.write("  }\n")
+                f.write("  }\n}\n")
+                cost[0] += cnt[0]
+                cost[1] += cnt[1]
+                print(f"lmax={lmax} rot3d sector={sct}: n={n} frame-change nnz={sum(len(r) for r in M1)}+{sum(len(r) for r in M2)} "
+                      f"axial entries={len(entries)} -> {cnt[0]} FP instructions, {cnt[1]} flop", file=sys.stderr)
+                # staging tables and unmix: as in emit_general_sym (same slots)
+                sa, sb, ss = [], [], []
+                for (l, am, p, kind) in slots:
+                    sa.append(idx[(l, am, p)]); sb.append(idx[(l, -am, p)]); ss.append({"0": 0, "+": 1, "-": -1}[kind])
+                for (l, am, p, kind) in slots:
+                    sa.append(idx[(l, am, p)]); sb.append(idx[(l, -am, p)]); ss.append({"0": 0, "+": -1, "-": 1}[kind])
+                f.write(f"__device__ __constant__ int tm_r3d_sa_L{lmax}_S{sct}[{2 * n}] = {{{', '.join(map(str, sa))}}};\n")
+                f.write(f"__device__ __constant__ int tm_r3d_sb_L{lmax}_S{sct}[{2 * n}] = {{{', '.join(map(str, sb))}}};\n")
+                f.write(f"__device__ __constant__ int tm_r3d_ss_L{lmax}_S{sct}[{2 * n}] = {{{', '.join(map(str, ss))}}};\n")
+                f.write("template <typename R, typename C, int AS>\n__device__ __forceinline__ void "
+                        f"tm_r3d_unmix_L{lmax}_S{sct}(const R* ar, const R* ai, C* out) {{\n")
+                for r, (l, am, p, kind) in enumerate(slots):
+                    def store(i_flat, re, im):
+                        if i_flat >= half_l:
+                            f.write(f"  out[{i_flat}].re = {im}; out[{i_flat}].im = -({re});\n")
+                        else:
+                            f.write(f"  out[{i_flat}].re = {re}; out[{i_flat}].im = {im};\n")
+                    if kind == "0":
+                        store(idx[(l, 0, p)], f"ar[{r} * AS]", f"ai[{r} * AS]")
+                    else:
+                        plus_r, plus_i = (f"ar[{r} * AS]", f"ai[{r} * AS]") if kind == "+" else (f"ar[{n + r} * AS]", f"ai[{n + r} * AS]")
+                        minus_r, minus_i = (f"ar[{n + r} * AS]", f"ai[{n + r} * AS]") if kind == "+" else (f"ar[{r} * AS]", f"ai[{r} * AS]")
+                        store(idx[(l, am, p)], f"R(0.5) * ({plus_r} + {minus_r})", f"R(0.5) * ({plus_i} + {minus_i})")
+                        store(idx[(l, -am, p)], f"R(0.5) * ({plus_r} - {minus_r})", f"R(0.5) * ({plus_i} - {minus_i})")
+                covered = set()
+                for (l, am, p, kind) in slots:
+                    covered.add(idx[(l, am, p)]); covered.add(idx[(l, -am, p)])
+                for i_flat in range(len(md)):
+                    if i_flat not in covered:
+                        f.write(f"  out[{i_flat}].re = R(0); out[{i_flat}].im = R(0);\n")
+                f.write("}\n")
+            f.write(f"#define TM_R3D_FPINST_L{lmax} {cost[0]}   // FP instructions per ordered pair (both sectors, generated apply code only)\n")
+            f.write(f"#define TM_R3D_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")

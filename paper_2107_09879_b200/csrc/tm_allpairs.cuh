@@ -433,6 +433,130 @@ k_allpairs_sym3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Rotation-based 3-D kernel (arbitrary positions, any lmax 1..7): rotation - axial translation - rotation with the theta
+// rotation written as  constant frame change . phase rotation . constant frame change  (gen_tables.py: rot3d_sectors), so
+// the per-pair work is O(L^1.5) for every pair direction: 1516 FP instructions per ordered pair at lmax 3 (sym3d: 4094),
+// ~7000 at lmax 6 (table-driven kernel: ~150 000).  Thread = target, one y'-mirror sector per block (blockIdx.z); the
+// sector's vector in the pair-axis frame (n = L/2 complex) lives in a per-thread shared-memory scratch [slot][thread]
+// because the frame changes are block diagonal in (l, p) and the axial translation in |m''|; accumulators (own sector +
+// partner share) in shared memory as in k_allpairs_sym3d.  Partial buffers and the finishing kernel as for sym3d.
+#include "generated/tm_rot3d_gen.cuh"
+
+template <typename R, int LMAX, int S> struct R3dPair;
+#define TM_R3D_SPEC(LM, SS_)                                                                             \
+  template <typename R> struct R3dPair<R, LM, SS_> {                                                     \
+    template <int AS>                                                                                    \
+    static __device__ __forceinline__ void run(const R* xs, R cph, R sph, R cth, R sth,                  \
+                                               const R* hr, const R* hi, R* sr, R* si, R* ar, R* ai) {   \
+      tm_r3d_pair_L##LM##_S##SS_<R, AS>(xs, cph, sph, cth, sth, hr, hi, sr, si, ar, ai);                 \
+    }                                                                                                    \
+    template <int AS>                                                                                    \
+    static __device__ __forceinline__ void unmix(const R* ar, const R* ai, Cx<R>* out) {                 \
+      tm_r3d_unmix_L##LM##_S##SS_<R, Cx<R>, AS>(ar, ai, out);                                            \
+    }                                                                                                    \
+    static __device__ __forceinline__ void stage_entry(int k, int& a, int& b, int& sg) {                 \
+      a = tm_r3d_sa_L##LM##_S##SS_[k]; b = tm_r3d_sb_L##LM##_S##SS_[k]; sg = tm_r3d_ss_L##LM##_S##SS_[k]; \
+    }                                                                                                    \
+  };
+TM_R3D_SPEC(1, 0) TM_R3D_SPEC(1, 1) TM_R3D_SPEC(2, 0) TM_R3D_SPEC(2, 1) TM_R3D_SPEC(3, 0) TM_R3D_SPEC(3, 1) TM_R3D_SPEC(4, 0)
+TM_R3D_SPEC(4, 1) TM_R3D_SPEC(5, 0) TM_R3D_SPEC(5, 1) TM_R3D_SPEC(6, 0) TM_R3D_SPEC(6, 1) TM_R3D_SPEC(7, 0) TM_R3D_SPEC(7, 1)
+#undef TM_R3D_SPEC
+
+template <typename R, int LMAX, int TJ, int SS> struct Rot3dSmem {
+  static constexpr int L = 2 * LMAX * (LMAX + 2);
+  // positions | staged d-values (own + partner = L slots) | scratch (L/2 slots) | accumulators (L slots) | staging tables
+  static constexpr size_t bytes = sizeof(double) * 3 * SS + sizeof(R) * (size_t)(SS * L * 2 + L * TJ + 2 * L * TJ) + sizeof(int) * 3 * L;
+};
+
+template <typename R, int LMAX, int TJ, int SS>
+__global__ void __launch_bounds__(TJ)
+k_allpairs_rot3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
+                 const TmTile* __restrict__ tiles, int n_scat, double k_over_pi, double inv_k,
+                 const int* __restrict__ n_active) {
+  constexpr int L = 2 * LMAX * (LMAX + 2);
+  constexpr int NS = L / 2;                 // slots per sector
+  constexpr int NQ = 2 * LMAX + 1;
+  if (n_active != nullptr && *n_active == 0) return;
+
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* s_px = reinterpret_cast<double*>(smem_raw);
+  double* s_py = s_px + SS;
+  double* s_pz = s_py + SS;
+  R* s_x = reinterpret_cast<R*>(s_pz + SS);          // [source][2 NS] complex: own slots then partner slots
+  R* s_scr = s_x + SS * L * 2;                       // [re/im][NS][TJ]
+  R* s_acc = s_scr + L * TJ;                         // [re/im][2 NS][TJ]
+  int* s_sa = reinterpret_cast<int*>(s_acc + 2 * L * TJ);
+  int* s_sb = s_sa + L;
+  int* s_ss = s_sb + L;
+
+  const TmTile tile = tiles[blockIdx.x];
+  const int tid = threadIdx.x;
+  const int sct = blockIdx.z;
+  const bool live = tid < tile.tgt_count;
+  const int j = tile.tgt_start + (live ? tid : tile.tgt_count - 1);
+  const double xj = pos[3 * j], yj = pos[3 * j + 1], zj = pos[3 * j + 2];
+  const int per = (tile.src_count + gridDim.y - 1) / gridDim.y;
+  const int c0 = tile.src_start + blockIdx.y * per;
+  const int c1 = min(tile.src_start + tile.src_count, c0 + per);
+
+  for (int e = tid; e < L; e += TJ) {
+    int a, b, sg;
+    if (sct == 0) R3dPair<R, LMAX, 0>::stage_entry(e, a, b, sg); else R3dPair<R, LMAX, 1>::stage_entry(e, a, b, sg);
+    s_sa[e] = a; s_sb[e] = b; s_ss[e] = sg;
+  }
+  R* sr = s_scr + tid;
+  R* si = s_scr + NS * TJ + tid;
+  R* ar = s_acc + tid;
+  R* ai = s_acc + L * TJ + tid;
+#pragma unroll
+  for (int b = 0; b < L; ++b) { ar[b * TJ] = R(0); ai[b * TJ] = R(0); }
+
+  for (int s0 = c0; s0 < c1; s0 += SS) {
+    const int ns = min(SS, c1 - s0);
+    __syncthreads();
+    for (int e = tid; e < ns; e += TJ) {
+      s_px[e] = pos[3 * (s0 + e)]; s_py[e] = pos[3 * (s0 + e) + 1]; s_pz[e] = pos[3 * (s0 + e) + 2];
+    }
+    for (int e = tid; e < ns * L; e += TJ) {
+      const int src = e / L, kk = e - src * L;
+      const Cx<R>* xrow = x + (size_t)(s0 + src) * L;
+      const int ia = s_sa[kk], sg = s_ss[kk];
+      Cx<R> v = xrow[ia];
+      if (sg != 0) {
+        const Cx<R> o = xrow[s_sb[kk]];
+        v = sg > 0 ? cadd(v, o) : csub(v, o);
+      }
+      if (ia >= NS) v = cx<R>(-v.im, v.re);            // tilde basis: multiply p = 1 modes by i
+      s_x[2 * e] = v.re;
+      s_x[2 * e + 1] = v.im;
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int s = 0; s < ns; ++s) {
+      const double dx = xj - s_px[s], dy = yj - s_py[s], dz = zj - s_pz[s];   // d = x_dest - x_source (reading R3)
+      const double rho2 = dx * dx + dy * dy, r2 = rho2 + dz * dz;
+      const double rinv = r2 > 0.0 ? rsqrt(r2) : 0.0;                          // self pair -> h_q = 0 -> nothing
+      const double rhoinv = rho2 > 0.0 ? rsqrt(rho2) : 0.0;
+      const double r = r2 * rinv;
+      const R cph = rho2 > 0.0 ? (R)(dx * rhoinv) : R(1), sph = (R)(dy * rhoinv);         // azimuth of d (pair along z: phi := 0)
+      const R cth = r2 > 0.0 ? (R)(dz * rinv) : R(1), sth = (R)(rho2 * rhoinv * rinv);     // polar angle of d
+      R ck, sk;
+      phase_kr<R>(k_over_pi, r, ck, sk);
+      R hr[NQ], hi[NQ];
+      hankel_up<R, NQ>((R)(rinv * inv_k), ck, sk, hr, hi);
+      const R* xs = &s_x[s * L * 2];
+      if (sct == 0) R3dPair<R, LMAX, 0>::template run<TJ>(xs, cph, sph, cth, sth, hr, hi, sr, si, ar, ai);
+      else          R3dPair<R, LMAX, 1>::template run<TJ>(xs, cph, sph, cth, sth, hr, hi, sr, si, ar, ai);
+    }
+  }
+  if (live) {
+    Cx<R>* out = u_part + ((size_t)(blockIdx.y * 2 + sct) * n_scat + j) * L;
+    if (sct == 0) R3dPair<R, LMAX, 0>::template unmix<TJ>(ar, ai, out);
+    else          R3dPair<R, LMAX, 1>::template unmix<TJ>(ar, ai, out);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Coplanar kernel for lmax 4..6 (the paper's truncation is lmax = 6).  Same mathematics as
 // k_allpairs_coplanar, but the two mirrors split the operator into FOUR uncoupled sectors (blockIdx.z = 2 h + t,
 // slowest grid dimension), the accumulators (own sector + the partner sector's share from the output rotation) live in

@@ -67,6 +67,10 @@ constexpr int COP4_TJ_L6 = 256;  // lmax 6: ONE 8-warp block per SM, so that all
                                  // DIFFERENT sectors double the footprint; measured 6.80 -> 6.50 ms on the 56x56 lattice)
 inline int cop4_tj(int lmax) { return lmax == 6 ? COP4_TJ_L6 : COP4_TJ; }
 constexpr int COP4_SS = 16;      // ... sources per stage
+// rotation-based 3-D kernel: targets per block / sources per stage (shared memory per thread grows with L: scratch L/2 +
+// accumulators L complex), chosen so that lmax <= 5 keeps two blocks per SM
+inline int rot3d_tj(int lmax) { return lmax <= 3 ? 128 : 64; }
+constexpr int ROT3D_SS_LO = 16, ROT3D_SS_HI = 4;
 constexpr int MAX_RESTART = 300;
 inline int cop4_groups(int lmax) {   // row groups per sector of the four-sector coplanar kernel
   return lmax == 4 ? Cop4Max<4>::ng : (lmax == 5 ? Cop4Max<5>::ng : (lmax == 6 ? Cop4Max<6>::ng : Cop4Max<7>::ng));
@@ -317,6 +321,25 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
     }
 #undef TM_LAUNCH_COP
 #undef TM_LAUNCH_COP2
+  } else if (c->kernel == TM_KERNEL_ROT3D) {
+    grid.z = 2;                                         // y'-mirror sector: slowest grid dimension
+#define TM_LAUNCH_R3(LM, TJ_, SS_)                                                                              \
+  {                                                                                                             \
+    const size_t sm = Rot3dSmem<R, LM, TJ_, SS_>::bytes;                                                        \
+    cudaFuncSetAttribute(k_allpairs_rot3d<R, LM, TJ_, SS_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
+    k_allpairs_rot3d<R, LM, TJ_, SS_><<<grid, TJ_, sm, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat,      \
+                                                                    k_over_pi, inv_k, n_active);                \
+  }
+    switch (c->lmax) {
+      case 1: TM_LAUNCH_R3(1, 128, ROT3D_SS_LO) break;
+      case 2: TM_LAUNCH_R3(2, 128, ROT3D_SS_LO) break;
+      case 3: TM_LAUNCH_R3(3, 128, ROT3D_SS_LO) break;
+      case 4: TM_LAUNCH_R3(4, 64, ROT3D_SS_HI) break;
+      case 5: TM_LAUNCH_R3(5, 64, ROT3D_SS_HI) break;
+      case 6: TM_LAUNCH_R3(6, 64, ROT3D_SS_HI) break;
+      default: TM_LAUNCH_R3(7, 64, ROT3D_SS_HI) break;
+    }
+#undef TM_LAUNCH_R3
   } else if (c->kernel == TM_KERNEL_SYM3D) {
     grid.z = 2;                                         // y'-mirror sector: slowest grid dimension
 #define TM_LAUNCH_S3(LM)                                                                                        \
@@ -656,8 +679,7 @@ void fill_const(tm_ctx* c) {
 
 int configure_kernel(tm_ctx* ctx) {
   int want = ctx->kernel_req;
-  if (want == TM_KERNEL_AUTO)
-    want = ctx->coplanar ? TM_KERNEL_COPLANAR : (ctx->lmax <= 3 ? TM_KERNEL_SYM3D : TM_KERNEL_GENERAL);
+  if (want == TM_KERNEL_AUTO) want = ctx->coplanar ? TM_KERNEL_COPLANAR : TM_KERNEL_ROT3D;
   if (want == TM_KERNEL_COPLANAR && !ctx->coplanar)
     return fail(ctx, TM_E_INVALID, "coplanar kernel needs all z equal");
   if (want == TM_KERNEL_SYM3D && ctx->lmax > 3) return fail(ctx, TM_E_INVALID, "generated 3-D kernel needs lmax <= 3");
@@ -666,9 +688,9 @@ int configure_kernel(tm_ctx* ctx) {
   ctx->cop_tj = TM_COP_TJ == 256 ? 256 : 128;
 #endif
   int tgt_per_tile;
-  const bool gen = want == TM_KERNEL_COPLANAR || want == TM_KERNEL_SYM3D;      // generated kernels: thread = target
+  const bool gen = want == TM_KERNEL_COPLANAR || want == TM_KERNEL_SYM3D || want == TM_KERNEL_ROT3D;   // generated kernels: thread = target
   switch (gen ? 0 : ctx->lmax) {
-    case 0: tgt_per_tile = want == TM_KERNEL_SYM3D ? SYM3D_TJ : (ctx->lmax > 3 ? cop4_tj(ctx->lmax) : ctx->cop_tj); break;
+    case 0: tgt_per_tile = want == TM_KERNEL_ROT3D ? rot3d_tj(ctx->lmax) : (want == TM_KERNEL_SYM3D ? SYM3D_TJ : (ctx->lmax > 3 ? cop4_tj(ctx->lmax) : ctx->cop_tj)); break;
     case 1: case 2: case 3: tgt_per_tile = 4; break;
     default: tgt_per_tile = 2; break;
   }
@@ -684,10 +706,11 @@ int configure_kernel(tm_ctx* ctx) {
   // small problems fill the 148 SMs (2 resident 128-thread blocks each at 255 registers) and large ones end
   // without a long tail; bounded by 64 chunks, >= 32 sources per chunk and 2 GB of partial sums.
   const bool cop4 = want == TM_KERNEL_COPLANAR && ctx->lmax > 3;   // four-sector coplanar kernel (lmax 4..6)
-  const long long slots = 148LL * (cop4 ? 256 / cop4_tj(ctx->lmax) : (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj : (want == TM_KERNEL_SYM3D ? 2 : 4)));
+  const long long slots = 148LL * (cop4 ? 256 / cop4_tj(ctx->lmax) : (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj :
+                                   (want == TM_KERNEL_SYM3D ? 2 : (want == TM_KERNEL_ROT3D ? (ctx->lmax <= 5 ? 2 : 1) : 4))));
   const int cop4_z = !cop4 ? 0 : 4 * cop4_groups(ctx->lmax);
   const long long blocks1 = (long long)ctx->n_tiles * (cop4 ? cop4_z : (gen ? 2 : 1));
-  const int part_mult = (want == TM_KERNEL_SYM3D || cop4) ? 2 : 1;   // one partial buffer per (chunk, y'-sector)
+  const int part_mult = (want == TM_KERNEL_SYM3D || want == TM_KERNEL_ROT3D || cop4) ? 2 : 1;   // one partial buffer per (chunk, y'-sector)
   int max_win = 1;
   for (int w = 0; w < ctx->n_win; ++w) max_win = std::max(max_win, ctx->win_ptr[w + 1] - ctx->win_ptr[w]);
   const size_t vec_bytes = ctx->n * elem_bytes(ctx);
@@ -935,7 +958,7 @@ int tm_create(tm_ctx** out, int n_scat, const double* pos_xyz, int n_win, const 
 
 int tm_set_kernel(tm_ctx* ctx, int kernel) {
   if (!ctx) return TM_E_INVALID;
-  if (kernel < TM_KERNEL_AUTO || kernel > TM_KERNEL_SYM3D) return fail(ctx, TM_E_INVALID, "unknown kernel id");
+  if (kernel < TM_KERNEL_AUTO || kernel > TM_KERNEL_ROT3D) return fail(ctx, TM_E_INVALID, "unknown kernel id");
   const int old = ctx->kernel_req;
   ctx->kernel_req = kernel;
   TM_CUDA(stream_wait(ctx));
@@ -1577,6 +1600,10 @@ int tm_pair_cost(const tm_ctx* ctx, double* fp_instructions, double* flop) {
   if (ctx->kernel == TM_KERNEL_COPLANAR) {
     const int I[8] = {0, TM_COP_FPINST_L1, TM_COP_FPINST_L2, TM_COP_FPINST_L3, TM_COP4_FPINST_L4, TM_COP4_FPINST_L5, TM_COP4_FPINST_L6, TM_COP4_FPINST_L7};
     const int F[8] = {0, TM_COP_FLOP_L1, TM_COP_FLOP_L2, TM_COP_FLOP_L3, TM_COP4_FLOP_L4, TM_COP4_FLOP_L5, TM_COP4_FLOP_L6, TM_COP4_FLOP_L7};
+    inst = I[ctx->lmax]; fl = F[ctx->lmax];
+  } else if (ctx->kernel == TM_KERNEL_ROT3D) {
+    const int I[8] = {0, TM_R3D_FPINST_L1, TM_R3D_FPINST_L2, TM_R3D_FPINST_L3, TM_R3D_FPINST_L4, TM_R3D_FPINST_L5, TM_R3D_FPINST_L6, TM_R3D_FPINST_L7};
+    const int F[8] = {0, TM_R3D_FLOP_L1, TM_R3D_FLOP_L2, TM_R3D_FLOP_L3, TM_R3D_FLOP_L4, TM_R3D_FLOP_L5, TM_R3D_FLOP_L6, TM_R3D_FLOP_L7};
     inst = I[ctx->lmax]; fl = F[ctx->lmax];
   } else if (ctx->kernel == TM_KERNEL_SYM3D) {
     const int I[4] = {0, TM_G3D_FPINST_L1, TM_G3D_FPINST_L2, TM_G3D_FPINST_L3};

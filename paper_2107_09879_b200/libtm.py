@@ -17,7 +17,7 @@ TM_OK, TM_NOT_CONVERGED = 0, 1
 TM_E_INVALID, TM_E_OVERLAP, TM_E_STATE, TM_E_CUDA, TM_E_NOMEM = -1, -2, -3, -4, -5
 TM_INC_PLANE, TM_INC_GAUSS, TM_INC_COEFFS, TM_INC_JINC = 0, 1, 2, 3
 TM_FIELD_E_SCA, TM_FIELD_H_SCA, TM_FIELD_E_INC = 0, 1, 2
-TM_KERNEL_AUTO, TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR, TM_KERNEL_SYM3D = 0, 1, 2, 3
+TM_KERNEL_AUTO, TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR, TM_KERNEL_SYM3D, TM_KERNEL_ROT3D = 0, 1, 2, 3, 4
 
 EXPORTS = ["tm_create", "tm_set_tmatrices", "tm_set_incident", "tm_get_incident", "tm_solve", "tm_solve_adjoint",
            "tm_matvec", "tm_fields", "tm_workspace_bytes", "tm_set_workspace", "tm_set_kernel", "tm_get_kernel",

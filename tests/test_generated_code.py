@@ -177,3 +177,21 @@ def test_generated_gradient_tables_match_oracle_derivative(lmax):
         for a in range(3):
             got = K * D[a] @ Aext
             assert np.abs(got - ref[a]).max() <= 1e-12 * np.abs(ref[a]).max(), (lmax, a)
+
+
+@pytest.mark.parametrize("lmax", [1, 2, 3, 4, 6])
+def test_generated_rotation_based_3d_pair_code_matches_oracle_block(lmax, tmp_path):
+    """Generated rotation - axial translation - rotation code for arbitrary pair directions (tm_rot3d_gen.cuh, the AUTO kernel
+    of non-planar layouts at every lmax) compiled as host C++: u = A_ji x against the oracle block, including pairs along
+    +-z (theta = 0, pi: phi undefined), in the plane, along -x (phi = pi) and far apart (k r ~ 200)."""
+    exe = str(tmp_path / f"hostcheck_rot3d_{lmax}")
+    subprocess.check_call(["g++", "-O0" if lmax > 4 else "-O1", f"-DLMAX={lmax}", "-o", exe, os.path.join(ROOT, "tests", "hostcheck_rot3d.cpp")])
+    rng = np.random.default_rng(50 + lmax)
+    L = n_modes(lmax)
+    for d in ([0.3, -0.4, 0.8], [0.0, 0.0, 1.2], [0.0, 0.0, -0.7], [1.0, 0.5, 0.0], [-0.6, 0.0, 0.0], rng.uniform(-30, 30, 3), rng.uniform(-3, 3, 3)):
+        x = rng.standard_normal(L) + 1j * rng.standard_normal(L)
+        inp = " ".join(repr(float(v)) for v in d) + "\n" + "\n".join(f"{float(z.real)!r} {float(z.imag)!r}" for z in x) + "\n"
+        out = subprocess.run([exe], input=inp, capture_output=True, text=True, check=True).stdout
+        u = np.array([complex(*map(float, ln.split())) for ln in out.strip().splitlines()])
+        ref = tr.block(lmax, K, np.array(d, dtype=float), np.zeros(3)) @ x
+        assert np.abs(u - ref).max() <= 2e-13 * np.abs(ref).max()

@@ -89,6 +89,7 @@ def test_table_kernel_at_maximum_lmax(tm, lmax):
     pos = W.random_cloud(12, seed=60 + lmax)
     x = rand_x((12, W.n_modes(lmax)), lmax)
     s = tm.Solver(pos, lmax, W.K_B)
+    s.set_kernel(tm.TM_KERNEL_GENERAL)
     assert s.get_kernel() == tm.TM_KERNEL_GENERAL
     assert rel(s.matvec(x, 2), omv.matvec_rows(lmax, W.K_B, pos, x)) <= 1e-12
     with pytest.raises(tm.TmError):

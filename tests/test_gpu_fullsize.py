@@ -112,8 +112,9 @@ def test_cfg4_windows_are_independent_at_full_size(tm):
     s.close(); s1.close()
 
 
-def test_sym3d_kernel_on_a_large_3d_cloud(tm):
-    """Generated 3-D kernel at scale (2e4 scatterers in a slab: 157 target tiles, many source chunks): sampled oracle rows."""
+@pytest.mark.parametrize("kernel", ["rot3d", "sym3d"])
+def test_3d_kernels_on_a_large_3d_cloud(tm, kernel):
+    """Generated 3-D kernels at scale (2e4 scatterers in a slab: 157 target tiles, many source chunks): sampled oracle rows."""
     rng = np.random.default_rng(91)
     n = 20000
     side = 40.0
@@ -125,7 +126,9 @@ def test_sym3d_kernel_on_a_large_3d_cloud(tm):
     pos += rng.uniform(-0.1, 0.1, pos.shape)
     x = rand_x((n, 30), 92)
     s = tm.Solver(pos, 3, W.K_B)
-    assert s.get_kernel() == tm.TM_KERNEL_SYM3D
+    assert s.get_kernel() == tm.TM_KERNEL_ROT3D
+    if kernel == "sym3d":
+        s.set_kernel(tm.TM_KERNEL_SYM3D)
     u = s.matvec(x, transpose=2)
     rows = np.sort(rng.choice(n, 12, replace=False)).astype(np.int32)
     rows[0], rows[-1] = 0, n - 1

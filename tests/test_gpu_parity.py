@@ -55,37 +55,43 @@ def test_allpairs_matvec_lattice(tm, kernel, lmax, n_side):
     s.close()
 
 
-@pytest.mark.parametrize("lmax", [1, 2, 3, 4])
+@pytest.mark.parametrize("lmax", [1, 2, 3, 4, 5, 6])
 def test_allpairs_matvec_random_3d_cloud(tm, lmax):
-    """Random non-lattice 3-D positions (PAPER.md:375 uses random positions): AUTO picks the generated 3-D kernel for
-    lmax <= 3 and the table-driven kernel above; the table-driven kernel is also checked for lmax <= 3."""
-    n = 150 if lmax <= 3 else 40
+    """Random non-lattice 3-D positions (PAPER.md:375 uses random positions; positions incl. z are design variables,
+    PAPER.md:517): AUTO picks the rotation-based generated kernel at every lmax up to the paper's 6; the direct generated
+    kernel (lmax <= 3) and the table-driven kernel are checked beside it."""
+    n = 150 if lmax <= 3 else (70 if lmax <= 5 else 40)
     pos = W.random_cloud(n, seed=20 + lmax)
-    pos[7] = pos[3] + [0.0, 0.0, 0.9]                    # a pair on a common vertical axis (theta = 0, rho = 0)
+    pos[7] = pos[3] + [0.0, 0.0, 0.9]                    # pairs on a common vertical axis (theta = 0 and pi, rho = 0)
+    pos[11] = pos[9] + [0.7, 0.0, 0.0]                   # and on a common x axis (theta = pi/2, phi = 0 and pi)
     x = rand_x((n, W.n_modes(lmax)), 30 + lmax)
     ref = omv.matvec_rows(lmax, W.K_B, pos, x)
     s = tm.Solver(pos, lmax, W.K_B)
-    assert s.get_kernel() == (tm.TM_KERNEL_SYM3D if lmax <= 3 else tm.TM_KERNEL_GENERAL)
+    assert s.get_kernel() == tm.TM_KERNEL_ROT3D
     assert rel(s.matvec(x, transpose=2), ref) <= 1e-12
-    if lmax <= 3:
-        s.set_kernel(tm.TM_KERNEL_GENERAL)
-        assert s.get_kernel() == tm.TM_KERNEL_GENERAL
+    for kern in ([tm.TM_KERNEL_SYM3D, tm.TM_KERNEL_GENERAL] if lmax <= 3 else ([tm.TM_KERNEL_GENERAL] if lmax == 4 else [])):
+        s.set_kernel(kern)
+        assert s.get_kernel() == kern
         assert rel(s.matvec(x, transpose=2), ref) <= 1e-12
     s.close()
 
 
-def test_sym3d_kernel_tiles_chunks_windows_fp32(tm):
-    """Generated 3-D kernel over several 128-target tiles, a ragged tail, several source chunks, ragged windows; fp32."""
+@pytest.mark.parametrize("kernel", ["rot3d", "sym3d"])
+def test_3d_kernels_tiles_chunks_windows_fp32(tm, kernel):
+    """Generated 3-D kernels over several 128-target tiles, a ragged tail, several source chunks, ragged windows; fp32."""
+    kid = tm.TM_KERNEL_ROT3D if kernel == "rot3d" else tm.TM_KERNEL_SYM3D
     pos = W.random_cloud(700, seed=77)
     wp = np.array([0, 300, 301, 700], dtype=np.int32)
     x = rand_x((700, 30), 78)
     ref = omv.matvec_rows(3, W.K_B, pos, x, win_ptr=wp)
     s = tm.Solver(pos, 3, W.K_B, win_ptr=wp)
-    assert s.get_kernel() == tm.TM_KERNEL_SYM3D
+    s.set_kernel(kid)
+    assert s.get_kernel() == kid
     u = s.matvec(x, transpose=2)
     assert rel(u, ref) <= 1e-12 and np.all(u[300] == 0)
     s.close()
     s = tm.Solver(pos, 3, W.K_B, win_ptr=wp, precision=tm.TM_FP32)
+    s.set_kernel(kid)
     assert rel(s.matvec(x, transpose=2), ref) <= 2e-5
     s.close()
     # a planar layout forced through the 3-D kernel must agree with the coplanar one
@@ -93,8 +99,35 @@ def test_sym3d_kernel_tiles_chunks_windows_fp32(tm):
     xp = rand_x((99, 30), 79)
     s = tm.Solver(posp, 3, W.K_B)
     a = s.matvec(xp, transpose=2)
-    s.set_kernel(tm.TM_KERNEL_SYM3D)
+    s.set_kernel(kid)
     assert rel(s.matvec(xp, transpose=2), a) <= 1e-13
+    s.close()
+
+
+def test_rot3d_kernel_lmax6_tiles_chunks_windows(tm):
+    """The rotation-based kernel at the paper's truncation on a non-planar layout: several 64-target tiles with a ragged tail,
+    source chunks, ragged windows (one scatterer, then a multiple of the tile), fp64 and fp32, against the oracle and
+    against the four-sector coplanar kernel on a planar layout."""
+    pos = W.random_cloud(230, seed=91)
+    wp = np.array([0, 1, 129, 230], dtype=np.int32)
+    L = W.n_modes(6)
+    x = rand_x((230, L), 92)
+    ref = omv.matvec_rows(6, W.K_B, pos, x, win_ptr=wp)
+    s = tm.Solver(pos, 6, W.K_B, win_ptr=wp)
+    assert s.get_kernel() == tm.TM_KERNEL_ROT3D
+    u = s.matvec(x, transpose=2)
+    assert rel(u, ref) <= 1e-12 and np.all(u[0] == 0)
+    s.close()
+    s = tm.Solver(pos, 6, W.K_B, win_ptr=wp, precision=tm.TM_FP32)
+    assert rel(s.matvec(x, transpose=2), ref) <= 2e-5
+    s.close()
+    posp = W.lattice(7, 9)
+    xp = rand_x((63, L), 93)
+    s = tm.Solver(posp, 6, W.K_B)
+    assert s.get_kernel() == tm.TM_KERNEL_COPLANAR
+    a = s.matvec(xp, transpose=2)
+    s.set_kernel(tm.TM_KERNEL_ROT3D)
+    assert rel(s.matvec(xp, transpose=2), a) <= 1e-12
     s.close()
 
 
@@ -113,7 +146,7 @@ def test_allpairs_matvec_windows(tm):
     pos = W.random_cloud(200, seed=8, planar=True)
     wp = np.array([0, 1, 70, 71, 200], dtype=np.int32)
     x = rand_x((200, 30), 9)
-    for kern in (tm.TM_KERNEL_COPLANAR, tm.TM_KERNEL_GENERAL, tm.TM_KERNEL_SYM3D):
+    for kern in (tm.TM_KERNEL_COPLANAR, tm.TM_KERNEL_GENERAL, tm.TM_KERNEL_SYM3D, tm.TM_KERNEL_ROT3D):
         s = tm.Solver(pos, 3, W.K_B, win_ptr=wp)
         s.set_kernel(kern)
         u = s.matvec(x, transpose=2)
