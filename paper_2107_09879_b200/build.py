@@ -1,8 +1,8 @@
 """Builds paper_2107_09879_b200/libtm.so (the C-ABI CUDA library, include/tm.h) in-tree (lib/libtm.so) with nvcc for sm_100a.
 
-    python -m paper_2107_09879_b200.build [--force]
+    python -m paper_2107_09879_b200.build [--force] [-v]
 
-nvcc cross-compiles without a GPU.  The generated headers under csrc/generated/ are (re)written by
+nvcc cross-compiles without a GPU; the translation units (host code + one per kernel family) compile in parallel.  The generated headers under csrc/generated/ are (re)written by
 csrc/gen_tables.py when missing or older than the generator.
 """
 import os
@@ -14,8 +14,6 @@ CSRC = os.path.join(HERE, "csrc")
 GEN = os.path.join(CSRC, "generated")
 SO = os.path.join(HERE, "lib", "libtm.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-shared", "-Xcompiler", "-fPIC", "-cudart", "static"]
 
 
 def _mtime(p):
@@ -49,13 +47,37 @@ def sources():
     return out
 
 
-def build(force=False, verbose=False):
+# Translation units: the host code and one per all-pairs kernel family (the generated straight-line code makes ptxas the
+# long pole of the build - compiled in parallel, the wall time is that of the largest family instead of their sum).
+UNITS = ["tm_api.cu", "tm_tu_coplanar.cu", "tm_tu_cop4_lo.cu", "tm_tu_cop4_hi.cu", "tm_tu_sym3d.cu", "tm_tu_rot3d_lo.cu",
+         "tm_tu_rot3d_6.cu", "tm_tu_rot3d_7.cu", "tm_tu_general.cu"]
+CFLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
+
+
+def build(force=False, verbose=False, jobs=None):
     generate()
     if not force and _mtime(SO) >= max(_mtime(s) for s in sources()):
         return SO
+    from concurrent.futures import ThreadPoolExecutor
     os.makedirs(os.path.dirname(SO), exist_ok=True)
-    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", SO, os.path.join(CSRC, "tm_api.cu")]
-    subprocess.check_call(cmd, cwd=CSRC)
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    extra = os.environ.get("TM_NVCC_EXTRA", "").split()             # e.g. -DTM_COP4_SYNC_L6=255 for A/B builds
+
+    def compile_one(unit):
+        obj = os.path.join(objdir, unit[:-3] + ".o")
+        cmd = [NVCC] + CFLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, os.path.join(CSRC, unit)]
+        r = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
+        return unit, obj, r
+    with ThreadPoolExecutor(max_workers=jobs or min(len(UNITS), os.cpu_count() or 1)) as ex:
+        results = list(ex.map(compile_one, UNITS))
+    for unit, obj, r in results:
+        if verbose or r.returncode != 0:
+            sys.stderr.write(f"== {unit}\n{r.stdout}{r.stderr}")
+        if r.returncode != 0:
+            raise subprocess.CalledProcessError(r.returncode, f"nvcc -c {unit}")
+    subprocess.check_call([NVCC, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a", "-o", SO]
+                          + [obj for _, obj, _ in results], cwd=CSRC)
     return SO
 
 

@@ -953,6 +953,7 @@ COP4_AXIAL = True        # False: direct pair-frame operator cut into row groups
 
 
 def emit_coplanar4(lmaxes, path):
+    costs = {}
     with open(path, "w") as f:
         f.write("// GENERATED by gen_tables.py - do not edit.\n")
         f.write("// Coplanar translation apply for lmax 4..6: FOUR uncoupled sectors (z-mirror parity x y'-mirror sector), each split into\n")
@@ -1091,6 +1092,12 @@ def emit_coplanar4(lmaxes, path):
             f.write(f"#define TM_COP4_NRMAX_L{lmax} {rmax}\n")
             f.write(f"#define TM_COP4_FPINST_L{lmax} {cost[0]}   // FP instructions per ordered pair (all sectors and row groups)\n")
             f.write(f"#define TM_COP4_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")
+            costs[lmax] = tuple(cost)
+    # the cost figures alone (for translation units that do not compile the four-sector code)
+    with open(os.path.join(os.path.dirname(path), "tm_coplanar4_cost.h"), "w") as f:
+        f.write("// GENERATED by gen_tables.py - do not edit.  Cost figures of tm_coplanar4_gen.cuh.\n#pragma once\n")
+        for lmax in lmaxes:
+            f.write(f"#ifndef TM_COP4_FPINST_L{lmax}\n#define TM_COP4_FPINST_L{lmax} {costs[lmax][0]}\n#define TM_COP4_FLOP_L{lmax} {costs[lmax][1]}\n#endif\n")
 
 
 # ----------------------------------------------------------------------------- coplanar, fp32 packed (FFMA2)
@@ -1235,18 +1242,6 @@ def emit_coplanar_f2(lmaxes, path):
                 f.write("}\n\n")
 
 
-def main():
-    os.makedirs(OUT, exist_ok=True)
-    emit_tables([1, 2, 3, 4, 5, 6, 7], os.path.join(OUT, "tm_tables_gen.h"))     # 7: internal (gradient at lmax 6)
-    emit_coplanar([1, 2, 3], os.path.join(OUT, "tm_coplanar_gen.cuh"))
-    emit_general_sym([1, 2, 3], os.path.join(OUT, "tm_general3d_gen.cuh"))
-    emit_coplanar4([4, 5, 6, 7], os.path.join(OUT, "tm_coplanar4_gen.cuh"))     # 7: internal (gradient at lmax 6)
-    emit_coplanar_f2([1, 2, 3], os.path.join(OUT, "tm_coplanar_f2_gen.cuh"))
-    emit_rot3d([1, 2, 3, 4, 5, 6, 7], os.path.join(OUT, "tm_rot3d_gen.cuh"))      # 7: internal (gradient at lmax 6)
-
-
-if __name__ == "__main__":
-    main()
 
 
 # ----------------------------------------------------------------------------- general 3-D, rotation - axial translation - rotation
@@ -1455,7 +1450,8 @@ def emit_rot3d(lmaxes, path):
         f.write("// phi phases, constant frame change onto the frame whose z axis is y', theta phases, constant frame change back: z'' is the\n")
         f.write("// pair axis; m''-diagonal axial translation; and the same way back.  One y'-mirror SECTOR per call (slots as in\n")
         f.write("// tm_general3d_gen.cuh).  xs: [own | partner] d-values; cph/sph, cth/sth: cos/sin of the pair's azimuth and polar angle; hr/hi: h_q(kr);\n")
-        f.write("// sr/si: per-thread scratch (n slots, stride AS); ar/ai: accumulators [own n | partner n], stride AS.\n#pragma once\n\n")
+        f.write("// sr/si: per-thread scratch (n slots, stride AS); ar/ai: accumulators of the own sector, pr/pi: the partner sector's share (n slots each, stride AS).\n#pragma once\n\n")
+        f.write("#ifndef TM_PIN\n#define TM_PIN(v)      // device build: zero-cost scheduling pin (tm_allpairs.cuh)\n#endif\n\n")
         for lmax in lmaxes:
             md = modes(lmax)
             idx = {t: i for i, t in enumerate(md)}
@@ -1479,7 +1475,7 @@ def emit_rot3d(lmaxes, path):
                 f.write(f"// lmax={lmax} sector={sct}: slots (l,|m|,p,kind) {slots}\n")
                 f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
                         f"tm_r3d_pair_L{lmax}_S{sct}(const R* __restrict__ xs, R cph, R sph, R cth, R sth, "
-                        "const R* hr, const R* hi, R* sr, R* si, R* ar, R* ai) {\n")
+                        "R* hr, R* hi, R* sr, R* si, R* ar, R* ai, R* pr, R* pi) {\n")
                 phases = ("    R cm[%d], sm[%d], ctm[%d], stm[%d];\n    cm[0] = R(1); sm[0] = R(0); cm[1] = cph; sm[1] = sph; "
                           "ctm[0] = R(1); stm[0] = R(0); ctm[1] = cth; stm[1] = sth;\n" % ((lmax + 1,) * 4))
                 for m in range(2, lmax + 1):
@@ -1517,6 +1513,21 @@ def emit_rot3d(lmaxes, path):
                     known = {}
                     for i in grp:
                         first = True
+                        # opaque pins: the radial sums depend only on h_q, so nothing stops the scheduler from forming all of a block's
+                        # sums up front (register spills at lmax >= 5); a zero-cost asm on the h_q a row's NEW sums read keeps
+                        # each sum next to its use
+                        newq = set()
+                        seen = set(known)
+                        for j in grp:
+                            lst = entries.get((i, j))
+                            if lst:
+                                s0 = 1 if lst[0][1] > 0 else -1
+                                key = tuple((q, mp.nstr(s0 * v, 30)) for (q, v) in lst)
+                                if key not in seen:
+                                    seen.add(key)
+                                    newq.update(q for (q, _) in lst)
+                        if newq:
+                            f.write("    " + " ".join(f"TM_PIN(hr[{q}]); TM_PIN(hi[{q}]);" for q in sorted(newq)) + "\n")
                         for j in grp:
                             lst = entries.get((i, j))
                             if not lst:
@@ -1575,7 +1586,7 @@ def emit_rot3d(lmaxes, path):
                             cnt[1] += 2
                         else:
                             f.write(f"    ar[{k} * AS] = fma(ur{k}, cm[{am}], ar[{k} * AS]); ai[{k} * AS] = fma(ui{k}, cm[{am}], ai[{k} * AS]);\n")
-                            f.write(f"    ar[{n + k} * AS] = fma(ui{k}, sm[{am}], ar[{n + k} * AS]); ai[{n + k} * AS] = fma(-ur{k}, sm[{am}], ai[{n + k} * AS]);\n")
+                            f.write(f"    pr[{k} * AS] = fma(ui{k}, sm[{am}], pr[{k} * AS]); pi[{k} * AS] = fma(-ur{k}, sm[{am}], pi[{k} * AS]);\n")
                             cnt[0] += 4
                             cnt[1] += 8
                     f.write("  }\n")
@@ -1594,7 +1605,7 @@ def emit_rot3d(lmaxes, path):
                 f.write(f"__device__ __constant__ int tm_r3d_sb_L{lmax}_S{sct}[{2 * n}] = {{{', '.join(map(str, sb))}}};\n")
                 f.write(f"__device__ __constant__ int tm_r3d_ss_L{lmax}_S{sct}[{2 * n}] = {{{', '.join(map(str, ss))}}};\n")
                 f.write("template <typename R, typename C, int AS>\n__device__ __forceinline__ void "
-                        f"tm_r3d_unmix_L{lmax}_S{sct}(const R* ar, const R* ai, C* out) {{\n")
+                        f"tm_r3d_unmix_L{lmax}_S{sct}(const R* ar, const R* ai, const R* pr, const R* pi, C* out) {{\n")
                 for r, (l, am, p, kind) in enumerate(slots):
                     def store(i_flat, re, im):
                         if i_flat >= half_l:
@@ -1604,8 +1615,8 @@ def emit_rot3d(lmaxes, path):
                     if kind == "0":
                         store(idx[(l, 0, p)], f"ar[{r} * AS]", f"ai[{r} * AS]")
                     else:
-                        plus_r, plus_i = (f"ar[{r} * AS]", f"ai[{r} * AS]") if kind == "+" else (f"ar[{n + r} * AS]", f"ai[{n + r} * AS]")
-                        minus_r, minus_i = (f"ar[{n + r} * AS]", f"ai[{n + r} * AS]") if kind == "+" else (f"ar[{r} * AS]", f"ai[{r} * AS]")
+                        plus_r, plus_i = (f"ar[{r} * AS]", f"ai[{r} * AS]") if kind == "+" else (f"pr[{r} * AS]", f"pi[{r} * AS]")
+                        minus_r, minus_i = (f"pr[{r} * AS]", f"pi[{r} * AS]") if kind == "+" else (f"ar[{r} * AS]", f"ai[{r} * AS]")
                         store(idx[(l, am, p)], f"R(0.5) * ({plus_r} + {minus_r})", f"R(0.5) * ({plus_i} + {minus_i})")
                         store(idx[(l, -am, p)], f"R(0.5) * ({plus_r} - {minus_r})", f"R(0.5) * ({plus_i} - {minus_i})")
                 covered = set()
@@ -1617,3 +1628,17 @@ def emit_rot3d(lmaxes, path):
                 f.write("}\n")
             f.write(f"#define TM_R3D_FPINST_L{lmax} {cost[0]}   // FP instructions per ordered pair (both sectors, generated apply code only)\n")
             f.write(f"#define TM_R3D_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")
+
+
+def main():
+    os.makedirs(OUT, exist_ok=True)
+    emit_tables([1, 2, 3, 4, 5, 6, 7], os.path.join(OUT, "tm_tables_gen.h"))     # 7: internal (gradient at lmax 6)
+    emit_coplanar([1, 2, 3], os.path.join(OUT, "tm_coplanar_gen.cuh"))
+    emit_general_sym([1, 2, 3], os.path.join(OUT, "tm_general3d_gen.cuh"))
+    emit_coplanar4([4, 5, 6, 7], os.path.join(OUT, "tm_coplanar4_gen.cuh"))     # 7: internal (gradient at lmax 6)
+    emit_coplanar_f2([1, 2, 3], os.path.join(OUT, "tm_coplanar_f2_gen.cuh"))
+    emit_rot3d([1, 2, 3, 4, 5, 6, 7], os.path.join(OUT, "tm_rot3d_gen.cuh"))      # 7: internal (gradient at lmax 6)
+
+
+if __name__ == "__main__":
+    main()

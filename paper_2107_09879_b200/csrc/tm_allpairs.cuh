@@ -10,8 +10,12 @@
 // adds the chunks in a fixed order (deterministic) and applies T.
 #pragma once
 #include "tm_common.cuh"
+// Sections (one per kernel family): a translation unit defines the TM_SEC_* it compiles (csrc/tm_tu_*.cu) so that the
+// families build in parallel; the host code (tm_api.cu) sees only the launch functions of tm_launch.h.
+#ifdef TM_SEC_COP
 #include "generated/tm_coplanar_gen.cuh"
 #include "generated/tm_coplanar_f2_gen.cuh"
+#endif
 
 // ---------------------------------------------------------------------------------------------------
 // h_q^(1)(x), q = 0..NQ-1, by upward recurrence from h_{-1} = e^{ix}/x, h_0 = -i e^{ix}/x  (stable upward for
@@ -43,8 +47,8 @@ template <> __device__ __forceinline__ void phase_kr<float>(double k_over_pi, do
 // Optional rigid displacement of all TARGETS against the sources (tm_grad_positions: numerical differentiation of the
 // translation operator in its displacement argument).  With a non-zero shift the self pair no longer has r = 0 and is
 // excluded by index instead.
-struct TmShift { double x, y, z; int on; };
 
+#ifdef TM_SEC_COP
 // Accumulators of one parity half: two real arrays in fp64; one float2 per complex number in fp32, where the generated
 // code uses Blackwell's packed FFMA2 arithmetic (generated/tm_coplanar_f2_gen.cuh) to halve the FP issue slots.
 template <typename R, int NH> struct CopAcc {
@@ -97,7 +101,7 @@ TM_COP_SPEC(1, 0) TM_COP_SPEC(1, 1) TM_COP_SPEC(2, 0) TM_COP_SPEC(2, 1) TM_COP_S
 // Coplanar kernel.  grid = (n_tiles, n_chunk, 2); block = TJ threads.  blockIdx.z selects the mirror-parity
 // half: it is the SLOWEST grid dimension, so at any time (almost) all resident blocks of an SM run the same
 // half and its ~30 KB of straight-line code stays within the 32 KB L1.5 instruction cache (ncu showed the
-// two-halves-per-block version stalled on instruction fetch: profiles/r01_allpairs_cfg3_v1.md).
+// two-halves-per-block version stalled on instruction fetch: profiles/r01_recorded_runs.md, kernel history).
 // Thread t handles target tile.tgt_start + t.  Sources of the tile's window are split into n_chunk contiguous
 // chunks (blockIdx.y) so that small problems still fill 148 SMs; each chunk is streamed through shared memory
 // SS sources at a time (positions + this half's d-values in the tilde basis x~ = i^p x).
@@ -191,12 +195,13 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
   }
 }
 
+#endif  // TM_SEC_COP
+#ifdef TM_SEC_GEN
 // ---------------------------------------------------------------------------------------------------
 // General 3-D kernel (any lmax <= 6).  Term table on the device: for destination row b, terms
 // row_ptr[b] <= t < row_ptr[b+1] with source column col[t], scalar-wave index widx[t] = q^2 + q + mu
 // (mu = m_col - m_b) and coefficient coef[t] (real part if !imag[t], imaginary part otherwise):
 //      A[b][col] += coef * h_q(kr) Pbar_q^{|mu|}(cos theta) e^{i mu phi}                 (Eq. I17)
-struct TmTermsDev { const int* row_ptr; const uint8_t* col; const uint8_t* widx; const uint8_t* imag; const double* coef; };
 
 template <int LMAX> struct GenCfg {
   static constexpr int L = 2 * LMAX * (LMAX + 2);
@@ -305,6 +310,8 @@ k_allpairs_general(const double* __restrict__ pos, const Cx<R>* __restrict__ x, 
   (void)m_b;
 }
 
+#endif  // TM_SEC_GEN
+#ifdef TM_SEC_SYM3D
 // ---------------------------------------------------------------------------------------------------
 // Generated 3-D kernel (arbitrary positions, lmax <= 3).  Same scheme as the coplanar kernel - rotate about z onto
 // the pair's azimuth, exploit the mirror y' -> -y' of the rotated pair (+- basis), never form the block:
@@ -432,6 +439,8 @@ k_allpairs_sym3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
   }
 }
 
+#endif  // TM_SEC_SYM3D
+#ifdef TM_SEC_ROT3D
 // ---------------------------------------------------------------------------------------------------
 // Rotation-based 3-D kernel (arbitrary positions, any lmax 1..7): rotation - axial translation - rotation with the theta
 // rotation written as  constant frame change . phase rotation . constant frame change  (gen_tables.py: rot3d_sectors), so
@@ -440,19 +449,23 @@ k_allpairs_sym3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
 // sector's vector in the pair-axis frame (n = L/2 complex) lives in a per-thread shared-memory scratch [slot][thread]
 // because the frame changes are block diagonal in (l, p) and the axial translation in |m''|; accumulators (own sector +
 // partner share) in shared memory as in k_allpairs_sym3d.  Partial buffers and the finishing kernel as for sym3d.
+// zero-cost scheduling pin: the compiler must treat v as modified here (keeps a value's consumers after this point)
+__device__ __forceinline__ void tm_pin(double& v) { asm volatile("" : "+d"(v)); }
+__device__ __forceinline__ void tm_pin(float& v) { asm volatile("" : "+f"(v)); }
+#define TM_PIN(v) tm_pin(v)
 #include "generated/tm_rot3d_gen.cuh"
 
 template <typename R, int LMAX, int S> struct R3dPair;
 #define TM_R3D_SPEC(LM, SS_)                                                                             \
   template <typename R> struct R3dPair<R, LM, SS_> {                                                     \
     template <int AS>                                                                                    \
-    static __device__ __forceinline__ void run(const R* xs, R cph, R sph, R cth, R sth,                  \
-                                               const R* hr, const R* hi, R* sr, R* si, R* ar, R* ai) {   \
-      tm_r3d_pair_L##LM##_S##SS_<R, AS>(xs, cph, sph, cth, sth, hr, hi, sr, si, ar, ai);                 \
+    static __device__ __forceinline__ void run(const R* xs, R cph, R sph, R cth, R sth, R* hr, R* hi,    \
+                                               R* sr, R* si, R* ar, R* ai, R* pr, R* pi) {               \
+      tm_r3d_pair_L##LM##_S##SS_<R, AS>(xs, cph, sph, cth, sth, hr, hi, sr, si, ar, ai, pr, pi);         \
     }                                                                                                    \
     template <int AS>                                                                                    \
-    static __device__ __forceinline__ void unmix(const R* ar, const R* ai, Cx<R>* out) {                 \
-      tm_r3d_unmix_L##LM##_S##SS_<R, Cx<R>, AS>(ar, ai, out);                                            \
+    static __device__ __forceinline__ void unmix(const R* ar, const R* ai, const R* pr, const R* pi, Cx<R>* out) { \
+      tm_r3d_unmix_L##LM##_S##SS_<R, Cx<R>, AS>(ar, ai, pr, pi, out);                                    \
     }                                                                                                    \
     static __device__ __forceinline__ void stage_entry(int k, int& a, int& b, int& sg) {                 \
       a = tm_r3d_sa_L##LM##_S##SS_[k]; b = tm_r3d_sb_L##LM##_S##SS_[k]; sg = tm_r3d_ss_L##LM##_S##SS_[k]; \
@@ -462,17 +475,20 @@ TM_R3D_SPEC(1, 0) TM_R3D_SPEC(1, 1) TM_R3D_SPEC(2, 0) TM_R3D_SPEC(2, 1) TM_R3D_S
 TM_R3D_SPEC(4, 1) TM_R3D_SPEC(5, 0) TM_R3D_SPEC(5, 1) TM_R3D_SPEC(6, 0) TM_R3D_SPEC(6, 1) TM_R3D_SPEC(7, 0) TM_R3D_SPEC(7, 1)
 #undef TM_R3D_SPEC
 
-template <typename R, int LMAX, int TJ, int SS> struct Rot3dSmem {
+// PG: the partner sector's share of the accumulators lives in GLOBAL memory (L2-resident, [block][re/im][slot][thread],
+// coalesced) instead of shared memory: at lmax >= 6 the three per-thread vectors (scratch, own and partner accumulators)
+// leave room for a single 2-warp block per SM; with the partner share in L2 two blocks fit and every scheduler has a warp.
+template <typename R, int LMAX, int TJ, int SS, bool PG> struct Rot3dSmem {
   static constexpr int L = 2 * LMAX * (LMAX + 2);
-  // positions | staged d-values (own + partner = L slots) | scratch (L/2 slots) | accumulators (L slots) | staging tables
-  static constexpr size_t bytes = sizeof(double) * 3 * SS + sizeof(R) * (size_t)(SS * L * 2 + L * TJ + 2 * L * TJ) + sizeof(int) * 3 * L;
+  // positions | staged d-values (own + partner = L slots) | scratch (L/2 slots) | accumulators (L or L/2 slots) | staging tables
+  static constexpr size_t bytes = sizeof(double) * 3 * SS + sizeof(R) * (size_t)(SS * L * 2 + L * TJ + (PG ? 1 : 2) * L * TJ) + sizeof(int) * 3 * L;
 };
 
-template <typename R, int LMAX, int TJ, int SS>
+template <typename R, int LMAX, int TJ, int SS, bool PG>
 __global__ void __launch_bounds__(TJ)
 k_allpairs_rot3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
                  const TmTile* __restrict__ tiles, int n_scat, double k_over_pi, double inv_k,
-                 const int* __restrict__ n_active) {
+                 const int* __restrict__ n_active, R* __restrict__ g_pacc) {
   constexpr int L = 2 * LMAX * (LMAX + 2);
   constexpr int NS = L / 2;                 // slots per sector
   constexpr int NQ = 2 * LMAX + 1;
@@ -484,8 +500,8 @@ k_allpairs_rot3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
   double* s_pz = s_py + SS;
   R* s_x = reinterpret_cast<R*>(s_pz + SS);          // [source][2 NS] complex: own slots then partner slots
   R* s_scr = s_x + SS * L * 2;                       // [re/im][NS][TJ]
-  R* s_acc = s_scr + L * TJ;                         // [re/im][2 NS][TJ]
-  int* s_sa = reinterpret_cast<int*>(s_acc + 2 * L * TJ);
+  R* s_acc = s_scr + L * TJ;                         // [re/im][NS][TJ] own sector, then (unless PG) [re/im][NS][TJ] partner share
+  int* s_sa = reinterpret_cast<int*>(s_acc + (PG ? 1 : 2) * L * TJ);
   int* s_sb = s_sa + L;
   int* s_ss = s_sb + L;
 
@@ -507,9 +523,16 @@ k_allpairs_rot3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
   R* sr = s_scr + tid;
   R* si = s_scr + NS * TJ + tid;
   R* ar = s_acc + tid;
-  R* ai = s_acc + L * TJ + tid;
+  R* ai = s_acc + NS * TJ + tid;
+  R* pr = s_acc + L * TJ + tid;
+  R* pi = s_acc + (L + NS) * TJ + tid;
+  if (PG) {
+    const size_t blk = ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    pr = g_pacc + blk * (size_t)(L * TJ) + tid;
+    pi = pr + NS * TJ;
+  }
 #pragma unroll
-  for (int b = 0; b < L; ++b) { ar[b * TJ] = R(0); ai[b * TJ] = R(0); }
+  for (int b = 0; b < NS; ++b) { ar[b * TJ] = R(0); ai[b * TJ] = R(0); pr[b * TJ] = R(0); pi[b * TJ] = R(0); }
 
   for (int s0 = c0; s0 < c1; s0 += SS) {
     const int ns = min(SS, c1 - s0);
@@ -535,7 +558,7 @@ k_allpairs_rot3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
     for (int s = 0; s < ns; ++s) {
       const double dx = xj - s_px[s], dy = yj - s_py[s], dz = zj - s_pz[s];   // d = x_dest - x_source (reading R3)
       const double rho2 = dx * dx + dy * dy, r2 = rho2 + dz * dz;
-      const double rinv = r2 > 0.0 ? rsqrt(r2) : 0.0;                          // self pair -> h_q = 0 -> nothing
+      const double rinv = r2 > 0.0 ? rsqrt(r2) : 0.0;                          // self pair -> h_q = 0 -> nothing  [rot3d]
       const double rhoinv = rho2 > 0.0 ? rsqrt(rho2) : 0.0;
       const double r = r2 * rinv;
       const R cph = rho2 > 0.0 ? (R)(dx * rhoinv) : R(1), sph = (R)(dy * rhoinv);         // azimuth of d (pair along z: phi := 0)
@@ -545,17 +568,19 @@ k_allpairs_rot3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
       R hr[NQ], hi[NQ];
       hankel_up<R, NQ>((R)(rinv * inv_k), ck, sk, hr, hi);
       const R* xs = &s_x[s * L * 2];
-      if (sct == 0) R3dPair<R, LMAX, 0>::template run<TJ>(xs, cph, sph, cth, sth, hr, hi, sr, si, ar, ai);
-      else          R3dPair<R, LMAX, 1>::template run<TJ>(xs, cph, sph, cth, sth, hr, hi, sr, si, ar, ai);
+      if (sct == 0) R3dPair<R, LMAX, 0>::template run<TJ>(xs, cph, sph, cth, sth, hr, hi, sr, si, ar, ai, pr, pi);
+      else          R3dPair<R, LMAX, 1>::template run<TJ>(xs, cph, sph, cth, sth, hr, hi, sr, si, ar, ai, pr, pi);
     }
   }
   if (live) {
     Cx<R>* out = u_part + ((size_t)(blockIdx.y * 2 + sct) * n_scat + j) * L;
-    if (sct == 0) R3dPair<R, LMAX, 0>::template unmix<TJ>(ar, ai, out);
-    else          R3dPair<R, LMAX, 1>::template unmix<TJ>(ar, ai, out);
+    if (sct == 0) R3dPair<R, LMAX, 0>::template unmix<TJ>(ar, ai, pr, pi, out);
+    else          R3dPair<R, LMAX, 1>::template unmix<TJ>(ar, ai, pr, pi, out);
   }
 }
 
+#endif  // TM_SEC_ROT3D
+#ifdef TM_SEC_COP4
 // ---------------------------------------------------------------------------------------------------
 // Coplanar kernel for lmax 4..6 (the paper's truncation is lmax = 6).  Same mathematics as
 // k_allpairs_coplanar, but the two mirrors split the operator into FOUR uncoupled sectors (blockIdx.z = 2 h + t,
@@ -723,3 +748,4 @@ k_allpairs_coplanar4(const double* __restrict__ pos, const Cx<R>* __restrict__ x
   const TmTile tile = tiles[blockIdx.x];
   cop4_dispatch<R, LMAX, 0, TJ, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, shift, smem_raw);
 }
+#endif  // TM_SEC_COP4

@@ -10,7 +10,7 @@
 #include <type_traits>
 #include <vector>
 
-#include "tm_allpairs.cuh"
+#include "tm_launch.h"
 #include "tm_arnoldi.cuh"
 #include "tm_common.cuh"
 #include "tm_fields.cuh"
@@ -58,23 +58,7 @@ inline cudaError_t tm_dev_free(void* p) {
   return e != cudaSuccess ? e : f;
 }
 
-constexpr int COP_SS = 64;       // coplanar kernel: sources per shared-memory stage
-constexpr int SYM3D_TJ = 128;    // generated 3-D kernel: targets per block
-constexpr int SYM3D_SS = 32;     // generated 3-D kernel: sources per stage
-constexpr int COP4_TJ = 128;     // four-sector coplanar kernel (lmax 4, 5, 7): targets per block
-constexpr int COP4_TJ_L6 = 256;  // lmax 6: ONE 8-warp block per SM, so that all warps of an SM run the same sector's code (a sector's
-                                 // loop body is 42 KB > the 32 KB L1.5 instruction cache; two co-resident 4-warp blocks of
-                                 // DIFFERENT sectors double the footprint; measured 6.80 -> 6.50 ms on the 56x56 lattice)
-inline int cop4_tj(int lmax) { return lmax == 6 ? COP4_TJ_L6 : COP4_TJ; }
-constexpr int COP4_SS = 16;      // ... sources per stage
-// rotation-based 3-D kernel: targets per block / sources per stage (shared memory per thread grows with L: scratch L/2 +
-// accumulators L complex), chosen so that lmax <= 5 keeps two blocks per SM
-inline int rot3d_tj(int lmax) { return lmax <= 3 ? 128 : 64; }
-constexpr int ROT3D_SS_LO = 16, ROT3D_SS_HI = 4;
 constexpr int MAX_RESTART = 300;
-inline int cop4_groups(int lmax) {   // row groups per sector of the four-sector coplanar kernel
-  return lmax == 4 ? Cop4Max<4>::ng : (lmax == 5 ? Cop4Max<5>::ng : (lmax == 6 ? Cop4Max<6>::ng : Cop4Max<7>::ng));
-}
 static_assert(MAX_RESTART + 1 <= TM_MAX_LDH, "k_gmres_solve_y keeps y in shared memory");
 
 struct Gmres {                   // device scalars of the Krylov solver, sized for `restart`
@@ -120,6 +104,7 @@ struct tm_ctx {
 
   TmTile* d_tiles = nullptr; int n_tiles = 0, n_chunk = 1, n_part = 1;   // n_part: partial-sum buffers the finishing kernel adds
   void* d_upart = nullptr; size_t upart_bytes = 0;
+  void* d_pacc = nullptr; size_t pacc_bytes = 0;       // rotation-based 3-D kernel, lmax >= 6: partner accumulators [block][L][TJ]
   TmChunk* d_chunks = nullptr; int n_chunks = 0; int* d_win_chunk_ptr = nullptr;
   int ept = 4;                   // vector kernels: elements per thread (chunk = ept * TM_VT)
   int max_chunks_per_win = 0;
@@ -286,98 +271,21 @@ void tick(tm_ctx* c, bool allpairs_begin) {
 // u_part <- A x   (all chunks)
 template <typename R>
 cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
-  const double k_over_pi = c->k / M_PI, inv_k = 1.0 / c->k;
   Cx<R>* up = reinterpret_cast<Cx<R>*>(c->d_upart);
-  dim3 grid(c->n_tiles, c->n_chunk);
+  const TmLaunch a{c->d_pos, c->d_tiles, c->n_scat, c->k / M_PI, 1.0 / c->k, n_active, c->stream, dim3(c->n_tiles, c->n_chunk), c->lmax};
   tick(c, true);
-  if (c->kernel == TM_KERNEL_COPLANAR && c->lmax > 3) {
-    // (z-mirror parity, y'-mirror sector) x row group: slowest grid dimension
-    grid.z = 4 * cop4_groups(c->lmax);
-#define TM_LAUNCH_C4(LM, TJ_)                                                                                   \
-  {                                                                                                             \
-    const size_t sm = Cop4Smem<R, LM, TJ_, COP4_SS>::bytes;                                                     \
-    cudaFuncSetAttribute(k_allpairs_coplanar4<R, LM, TJ_, COP4_SS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
-    k_allpairs_coplanar4<R, LM, TJ_, COP4_SS><<<grid, TJ_, sm, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat, \
-                                                                            k_over_pi, inv_k, n_active, c->shift); \
-  }
-    switch (c->lmax) {
-      case 4: TM_LAUNCH_C4(4, COP4_TJ) break;
-      case 5: TM_LAUNCH_C4(5, COP4_TJ) break;
-      case 6: TM_LAUNCH_C4(6, COP4_TJ_L6) break;
-      default: TM_LAUNCH_C4(7, COP4_TJ) break;
-    }
-#undef TM_LAUNCH_C4
-  } else if (c->kernel == TM_KERNEL_COPLANAR) {
-    grid.z = 2;                                         // mirror-parity half: slowest grid dimension
-#define TM_LAUNCH_COP2(LM, TJ)                                                                              \
-  k_allpairs_coplanar<R, LM, TJ, COP_SS><<<grid, TJ, 0, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat,    \
-                                                                     k_over_pi, inv_k, n_active, c->shift)
-#define TM_LAUNCH_COP(LM)                                                                                   \
-  do { if (c->cop_tj == 256) TM_LAUNCH_COP2(LM, 256); else TM_LAUNCH_COP2(LM, 128); } while (0)
-    switch (c->lmax) {
-      case 1: TM_LAUNCH_COP(1); break;
-      case 2: TM_LAUNCH_COP(2); break;
-      default: TM_LAUNCH_COP(3); break;
-    }
-#undef TM_LAUNCH_COP
-#undef TM_LAUNCH_COP2
-  } else if (c->kernel == TM_KERNEL_ROT3D) {
-    grid.z = 2;                                         // y'-mirror sector: slowest grid dimension
-#define TM_LAUNCH_R3(LM, TJ_, SS_)                                                                              \
-  {                                                                                                             \
-    const size_t sm = Rot3dSmem<R, LM, TJ_, SS_>::bytes;                                                        \
-    cudaFuncSetAttribute(k_allpairs_rot3d<R, LM, TJ_, SS_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
-    k_allpairs_rot3d<R, LM, TJ_, SS_><<<grid, TJ_, sm, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat,      \
-                                                                    k_over_pi, inv_k, n_active);                \
-  }
-    switch (c->lmax) {
-      case 1: TM_LAUNCH_R3(1, 128, ROT3D_SS_LO) break;
-      case 2: TM_LAUNCH_R3(2, 128, ROT3D_SS_LO) break;
-      case 3: TM_LAUNCH_R3(3, 128, ROT3D_SS_LO) break;
-      case 4: TM_LAUNCH_R3(4, 64, ROT3D_SS_HI) break;
-      case 5: TM_LAUNCH_R3(5, 64, ROT3D_SS_HI) break;
-      case 6: TM_LAUNCH_R3(6, 64, ROT3D_SS_HI) break;
-      default: TM_LAUNCH_R3(7, 64, ROT3D_SS_HI) break;
-    }
-#undef TM_LAUNCH_R3
-  } else if (c->kernel == TM_KERNEL_SYM3D) {
-    grid.z = 2;                                         // y'-mirror sector: slowest grid dimension
-#define TM_LAUNCH_S3(LM)                                                                                        \
-  {                                                                                                             \
-    const size_t sm = Sym3dSmem<R, LM, SYM3D_TJ, SYM3D_SS>::bytes;                                              \
-    cudaFuncSetAttribute(k_allpairs_sym3d<R, LM, SYM3D_TJ, SYM3D_SS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
-    k_allpairs_sym3d<R, LM, SYM3D_TJ, SYM3D_SS><<<grid, SYM3D_TJ, sm, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->n_scat, \
-                                                                                   k_over_pi, inv_k, n_active, c->shift); \
-  }
-    switch (c->lmax) {
-      case 1: TM_LAUNCH_S3(1) break;
-      case 2: TM_LAUNCH_S3(2) break;
-      default: TM_LAUNCH_S3(3) break;
-    }
-#undef TM_LAUNCH_S3
-  } else {
-    TmTermsDev tb{c->d_rowptr, c->d_col, c->d_widx, c->d_imag, c->d_coef};
-#define TM_LAUNCH_GEN(LM)                                                                                         \
-  {                                                                                                               \
-    const size_t sm = GenCfg<LM>::smem<R>();                                                                      \
-    cudaFuncSetAttribute(k_allpairs_general<R, LM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);        \
-    k_allpairs_general<R, LM><<<grid, 32 * GenCfg<LM>::WJ, sm, c->stream>>>(c->d_pos, x, up, c->d_tiles, c->d_const, \
-                                                                            tb, c->n_scat, k_over_pi, inv_k, n_active); \
-  }
-    switch (c->lmax) {
-      case 1: TM_LAUNCH_GEN(1) break;
-      case 2: TM_LAUNCH_GEN(2) break;
-      case 3: TM_LAUNCH_GEN(3) break;
-      case 4: TM_LAUNCH_GEN(4) break;
-      case 5: TM_LAUNCH_GEN(5) break;
-      case 6: TM_LAUNCH_GEN(6) break;
-      default: TM_LAUNCH_GEN(7) break;
-    }
-#undef TM_LAUNCH_GEN
-  }
+  cudaError_t e;
+  if (c->kernel == TM_KERNEL_COPLANAR && c->lmax > 3)
+    e = c->lmax <= 5 ? tm_launch_coplanar4_lo<R>(a, x, up, c->shift) : tm_launch_coplanar4_hi<R>(a, x, up, c->shift);
+  else if (c->kernel == TM_KERNEL_COPLANAR) e = tm_launch_coplanar<R>(a, x, up, c->cop_tj, c->shift);
+  else if (c->kernel == TM_KERNEL_ROT3D) {
+    R* pacc = reinterpret_cast<R*>(c->d_pacc);
+    e = c->lmax <= 5 ? tm_launch_rot3d_lo<R>(a, x, up, pacc) : (c->lmax == 6 ? tm_launch_rot3d_6<R>(a, x, up, pacc) : tm_launch_rot3d_7<R>(a, x, up, pacc));
+  } else if (c->kernel == TM_KERNEL_SYM3D) e = tm_launch_sym3d<R>(a, x, up, c->shift);
+  else e = tm_launch_general<R>(a, x, up, c->d_const, TmTermsDev{c->d_rowptr, c->d_col, c->d_widx, c->d_imag, c->d_coef});
   tick(c, false);
   c->allpairs_launches++; c->total_launches++;
-  return cudaGetLastError();
+  return e;
 }
 
 template <typename R>
@@ -690,9 +598,8 @@ int configure_kernel(tm_ctx* ctx) {
   int tgt_per_tile;
   const bool gen = want == TM_KERNEL_COPLANAR || want == TM_KERNEL_SYM3D || want == TM_KERNEL_ROT3D;   // generated kernels: thread = target
   switch (gen ? 0 : ctx->lmax) {
-    case 0: tgt_per_tile = want == TM_KERNEL_ROT3D ? rot3d_tj(ctx->lmax) : (want == TM_KERNEL_SYM3D ? SYM3D_TJ : (ctx->lmax > 3 ? cop4_tj(ctx->lmax) : ctx->cop_tj)); break;
-    case 1: case 2: case 3: tgt_per_tile = 4; break;
-    default: tgt_per_tile = 2; break;
+    case 0: tgt_per_tile = want == TM_KERNEL_ROT3D ? tm_rot3d_tj(ctx->lmax) : (want == TM_KERNEL_SYM3D ? TM_SYM3D_TJ : (ctx->lmax > 3 ? tm_cop4_tj(ctx->lmax) : ctx->cop_tj)); break;
+    default: tgt_per_tile = tm_general_tj(ctx->lmax); break;
   }
   std::vector<TmTile> tiles;
   int min_win = ctx->n_scat;
@@ -706,9 +613,9 @@ int configure_kernel(tm_ctx* ctx) {
   // small problems fill the 148 SMs (2 resident 128-thread blocks each at 255 registers) and large ones end
   // without a long tail; bounded by 64 chunks, >= 32 sources per chunk and 2 GB of partial sums.
   const bool cop4 = want == TM_KERNEL_COPLANAR && ctx->lmax > 3;   // four-sector coplanar kernel (lmax 4..6)
-  const long long slots = 148LL * (cop4 ? 256 / cop4_tj(ctx->lmax) : (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj :
-                                   (want == TM_KERNEL_SYM3D ? 2 : (want == TM_KERNEL_ROT3D ? (ctx->lmax <= 5 ? 2 : 1) : 4))));
-  const int cop4_z = !cop4 ? 0 : 4 * cop4_groups(ctx->lmax);
+  const long long slots = 148LL * (cop4 ? 256 / tm_cop4_tj(ctx->lmax) : (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj :
+                                   (want == TM_KERNEL_SYM3D ? 2 : (want == TM_KERNEL_ROT3D ? (ctx->lmax <= 6 ? 2 : 1) : 4))));
+  const int cop4_z = !cop4 ? 0 : 4 * tm_cop4_groups(ctx->lmax);
   const long long blocks1 = (long long)ctx->n_tiles * (cop4 ? cop4_z : (gen ? 2 : 1));
   const int part_mult = (want == TM_KERNEL_SYM3D || want == TM_KERNEL_ROT3D || cop4) ? 2 : 1;   // one partial buffer per (chunk, y'-sector)
   int max_win = 1;
@@ -726,6 +633,16 @@ int configure_kernel(tm_ctx* ctx) {
   if (ctx->d_tiles) tm_dev_free(ctx->d_tiles);
   TM_CUDA(tm_dev_alloc(&ctx->d_tiles, tiles.size() * sizeof(TmTile)));
   TM_CUDA(cudaMemcpy(ctx->d_tiles, tiles.data(), tiles.size() * sizeof(TmTile), cudaMemcpyHostToDevice));
+  if (want == TM_KERNEL_ROT3D && tm_rot3d_pg(ctx->lmax)) {
+    const size_t per_block = (size_t)ctx->L * tm_rot3d_tj(ctx->lmax) * (ctx->precision == TM_FP32 ? sizeof(float) : sizeof(double));
+    const size_t need_p = (size_t)ctx->n_tiles * ctx->n_chunk * 2 * per_block;
+    if (need_p > ctx->pacc_bytes) {
+      if (ctx->d_pacc) tm_dev_free(ctx->d_pacc);
+      ctx->d_pacc = nullptr; ctx->pacc_bytes = 0;
+      TM_CUDA(tm_dev_alloc(&ctx->d_pacc, need_p));
+      ctx->pacc_bytes = need_p;
+    }
+  }
   ctx->n_part = ctx->n_chunk * part_mult;
   const size_t need = (size_t)ctx->n_part * vec_bytes;
   if (need > ctx->upart_bytes) {
@@ -803,7 +720,7 @@ void tm_destroy(tm_ctx* c) {
   tm_dev_free(c->d_grad_tab);
   tm_dev_free(c->d_pos); tm_dev_free(c->d_win_of); tm_dev_free(c->d_type_of); tm_dev_free(c->d_T); tm_dev_free(c->d_T32); tm_dev_free(c->d_p);
   tm_dev_free(c->d_const); tm_dev_free(c->d_rowptr); tm_dev_free(c->d_col); tm_dev_free(c->d_widx); tm_dev_free(c->d_imag);
-  tm_dev_free(c->d_coef); tm_dev_free(c->d_tiles); tm_dev_free(c->d_upart); tm_dev_free(c->d_chunks); tm_dev_free(c->d_win_chunk_ptr);
+  tm_dev_free(c->d_coef); tm_dev_free(c->d_tiles); tm_dev_free(c->d_upart); tm_dev_free(c->d_pacc); tm_dev_free(c->d_chunks); tm_dev_free(c->d_win_chunk_ptr);
   for (int i = 0; i < 3; ++i) tm_dev_free(c->d_v[i]);
   tm_dev_free(c->d_io);
   if (c->ws_owned) tm_dev_free(c->ws);
@@ -1597,19 +1514,10 @@ extern "C" {
 int tm_pair_cost(const tm_ctx* ctx, double* fp_instructions, double* flop) {
   if (!ctx) return TM_E_INVALID;
   double inst = 0.0, fl = 0.0;
-  if (ctx->kernel == TM_KERNEL_COPLANAR) {
-    const int I[8] = {0, TM_COP_FPINST_L1, TM_COP_FPINST_L2, TM_COP_FPINST_L3, TM_COP4_FPINST_L4, TM_COP4_FPINST_L5, TM_COP4_FPINST_L6, TM_COP4_FPINST_L7};
-    const int F[8] = {0, TM_COP_FLOP_L1, TM_COP_FLOP_L2, TM_COP_FLOP_L3, TM_COP4_FLOP_L4, TM_COP4_FLOP_L5, TM_COP4_FLOP_L6, TM_COP4_FLOP_L7};
-    inst = I[ctx->lmax]; fl = F[ctx->lmax];
-  } else if (ctx->kernel == TM_KERNEL_ROT3D) {
-    const int I[8] = {0, TM_R3D_FPINST_L1, TM_R3D_FPINST_L2, TM_R3D_FPINST_L3, TM_R3D_FPINST_L4, TM_R3D_FPINST_L5, TM_R3D_FPINST_L6, TM_R3D_FPINST_L7};
-    const int F[8] = {0, TM_R3D_FLOP_L1, TM_R3D_FLOP_L2, TM_R3D_FLOP_L3, TM_R3D_FLOP_L4, TM_R3D_FLOP_L5, TM_R3D_FLOP_L6, TM_R3D_FLOP_L7};
-    inst = I[ctx->lmax]; fl = F[ctx->lmax];
-  } else if (ctx->kernel == TM_KERNEL_SYM3D) {
-    const int I[4] = {0, TM_G3D_FPINST_L1, TM_G3D_FPINST_L2, TM_G3D_FPINST_L3};
-    const int F[4] = {0, TM_G3D_FLOP_L1, TM_G3D_FLOP_L2, TM_G3D_FLOP_L3};
-    inst = I[ctx->lmax]; fl = F[ctx->lmax];
-  } else {   // general kernel: per (term, source): 2 MUL + 4 FMA
+  if (ctx->kernel == TM_KERNEL_COPLANAR) tm_cost_coplanar(ctx->lmax, &inst, &fl);
+  else if (ctx->kernel == TM_KERNEL_ROT3D) tm_cost_rot3d(ctx->lmax, &inst, &fl);
+  else if (ctx->kernel == TM_KERNEL_SYM3D) tm_cost_sym3d(ctx->lmax, &inst, &fl);
+  else {   // general kernel: per (term, source): 2 MUL + 4 FMA
     const double nt = tm_term_tables[ctx->lmax - 1].n_terms;
     inst = 6.0 * nt; fl = 10.0 * nt;
   }

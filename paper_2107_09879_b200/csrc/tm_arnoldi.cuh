@@ -2,7 +2,7 @@
 //   CGS2 orthogonalisation (dots -> axpy -> dots -> axpy + norm), Givens update per window, normalisation of the new
 //   basis vector - the phases of tm_vecops.cuh / tm_gmres.cuh separated by grid-wide barriers instead of kernel
 //   boundaries; for diagonal T the T application (and the transposed operator's permutations) is folded in too.  On the 32x32 lattice the seven dependent launches cost more than their work (profiles/
-//   r01_launches_cfg2_v3.md); here block c keeps chunk c for the whole step.  Used when all chunks are co-resident.
+//   r01_recorded_runs.md, kernel history); here block c keeps chunk c for the whole step.  Used when all chunks are co-resident.
 #pragma once
 #include <cooperative_groups.h>
 

@@ -44,6 +44,14 @@ __device__ __forceinline__ double warp_sum(double v) {
 // Work item of the all-pairs kernels: a tile of consecutive targets inside one window.
 struct TmTile { int tgt_start, tgt_count, src_start, src_count; };
 
+// Optional rigid displacement of all TARGETS against the sources (A/B experiments on the displacement argument of the
+// translation operator).  With a non-zero shift the self pair no longer has r = 0 and is excluded by index instead.
+struct TmShift { double x, y, z; int on; };
+
+// Term table of the table-driven kernel on the device: for destination row b, terms row_ptr[b] <= t < row_ptr[b+1] with
+// source column col[t], scalar-wave index widx[t] = q^2 + q + mu and coefficient coef[t] (real part if !imag[t]).
+struct TmTermsDev { const int* row_ptr; const uint8_t* col; const uint8_t* widx; const uint8_t* imag; const double* coef; };
+
 // Small per-lmax tables, one device copy per context (tm_ctx::d_const).
 struct TmConst {
   int perm_neg_m[TM_MAX_MODES];          // flat index of (l,-m,p)               (structural identity S3)

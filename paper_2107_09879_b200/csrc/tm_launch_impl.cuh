@@ -1,0 +1,168 @@
+// Definitions of the launch functions of tm_launch.h, one section per kernel family (selected by the TM_SEC_* / TM_RANGE_*
+// macros of the including translation unit).
+#pragma once
+#include "tm_launch.h"
+#include "tm_allpairs.cuh"
+
+#ifdef TM_SEC_COP
+template <typename R> cudaError_t tm_launch_coplanar(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, int tj, TmShift shift) {
+  dim3 grid = a.grid;
+  grid.z = 2;                                         // mirror-parity half: slowest grid dimension
+#define TM_LAUNCH_COP2(LM, TJ)                                                                              \
+  k_allpairs_coplanar<R, LM, TJ, TM_COP_SS><<<grid, TJ, 0, a.stream>>>(a.pos, x, up, a.tiles, a.n_scat,     \
+                                                                       a.k_over_pi, a.inv_k, a.n_active, shift)
+#define TM_LAUNCH_COP(LM)                                                                                   \
+  do { if (tj == 256) TM_LAUNCH_COP2(LM, 256); else TM_LAUNCH_COP2(LM, 128); } while (0)
+  switch (a.lmax) {
+    case 1: TM_LAUNCH_COP(1); break;
+    case 2: TM_LAUNCH_COP(2); break;
+    default: TM_LAUNCH_COP(3); break;
+  }
+#undef TM_LAUNCH_COP
+#undef TM_LAUNCH_COP2
+  return cudaGetLastError();
+}
+template cudaError_t tm_launch_coplanar<double>(const TmLaunch&, const Cx<double>*, Cx<double>*, int, TmShift);
+template cudaError_t tm_launch_coplanar<float>(const TmLaunch&, const Cx<float>*, Cx<float>*, int, TmShift);
+#endif
+
+#ifdef TM_SEC_COP4
+#define TM_LAUNCH_C4(LM, TJ_)                                                                                   \
+  {                                                                                                             \
+    const size_t sm = Cop4Smem<R, LM, TJ_, TM_COP4_SS>::bytes;                                                  \
+    cudaFuncSetAttribute(k_allpairs_coplanar4<R, LM, TJ_, TM_COP4_SS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
+    k_allpairs_coplanar4<R, LM, TJ_, TM_COP4_SS><<<grid, TJ_, sm, a.stream>>>(a.pos, x, up, a.tiles, a.n_scat,  \
+                                                                              a.k_over_pi, a.inv_k, a.n_active, shift); \
+  }
+#ifdef TM_RANGE_LO
+template <typename R> cudaError_t tm_launch_coplanar4_lo(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, TmShift shift) {
+  dim3 grid = a.grid;
+  grid.z = 4 * (a.lmax == 4 ? Cop4Max<4>::ng : Cop4Max<5>::ng);   // (z-mirror parity, y'-mirror sector) x row group: slowest grid dimension
+  if (a.lmax == 4) TM_LAUNCH_C4(4, 128) else TM_LAUNCH_C4(5, 128)
+  return cudaGetLastError();
+}
+template cudaError_t tm_launch_coplanar4_lo<double>(const TmLaunch&, const Cx<double>*, Cx<double>*, TmShift);
+template cudaError_t tm_launch_coplanar4_lo<float>(const TmLaunch&, const Cx<float>*, Cx<float>*, TmShift);
+int tm_cop4_groups(int lmax) {
+  return lmax == 4 ? Cop4Max<4>::ng : (lmax == 5 ? Cop4Max<5>::ng : (lmax == 6 ? Cop4Max<6>::ng : Cop4Max<7>::ng));
+}
+#endif
+#ifdef TM_RANGE_HI
+template <typename R> cudaError_t tm_launch_coplanar4_hi(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, TmShift shift) {
+  dim3 grid = a.grid;
+  grid.z = 4 * (a.lmax == 6 ? Cop4Max<6>::ng : Cop4Max<7>::ng);
+  if (a.lmax == 6) TM_LAUNCH_C4(6, 256) else TM_LAUNCH_C4(7, 128)
+  return cudaGetLastError();
+}
+template cudaError_t tm_launch_coplanar4_hi<double>(const TmLaunch&, const Cx<double>*, Cx<double>*, TmShift);
+template cudaError_t tm_launch_coplanar4_hi<float>(const TmLaunch&, const Cx<float>*, Cx<float>*, TmShift);
+#endif
+#undef TM_LAUNCH_C4
+#endif
+
+#ifdef TM_SEC_SYM3D
+template <typename R> cudaError_t tm_launch_sym3d(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, TmShift shift) {
+  dim3 grid = a.grid;
+  grid.z = 2;                                         // y'-mirror sector: slowest grid dimension
+#define TM_LAUNCH_S3(LM)                                                                                        \
+  {                                                                                                             \
+    const size_t sm = Sym3dSmem<R, LM, TM_SYM3D_TJ, TM_SYM3D_SS>::bytes;                                        \
+    cudaFuncSetAttribute(k_allpairs_sym3d<R, LM, TM_SYM3D_TJ, TM_SYM3D_SS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
+    k_allpairs_sym3d<R, LM, TM_SYM3D_TJ, TM_SYM3D_SS><<<grid, TM_SYM3D_TJ, sm, a.stream>>>(a.pos, x, up, a.tiles, a.n_scat, \
+                                                                                           a.k_over_pi, a.inv_k, a.n_active, shift); \
+  }
+  switch (a.lmax) {
+    case 1: TM_LAUNCH_S3(1) break;
+    case 2: TM_LAUNCH_S3(2) break;
+    default: TM_LAUNCH_S3(3) break;
+  }
+#undef TM_LAUNCH_S3
+  return cudaGetLastError();
+}
+template cudaError_t tm_launch_sym3d<double>(const TmLaunch&, const Cx<double>*, Cx<double>*, TmShift);
+template cudaError_t tm_launch_sym3d<float>(const TmLaunch&, const Cx<float>*, Cx<float>*, TmShift);
+void tm_cost_sym3d(int lmax, double* inst, double* flop) {
+  const int I[4] = {0, TM_G3D_FPINST_L1, TM_G3D_FPINST_L2, TM_G3D_FPINST_L3};
+  const int F[4] = {0, TM_G3D_FLOP_L1, TM_G3D_FLOP_L2, TM_G3D_FLOP_L3};
+  *inst = I[lmax]; *flop = F[lmax];
+}
+#endif
+
+#ifdef TM_SEC_ROT3D
+#define TM_LAUNCH_R3(LM, TJ_, SS_)                                                                              \
+  {                                                                                                             \
+    constexpr bool PG_ = LM >= TM_R3D_PG_FROM;                                                                  \
+    const size_t sm = Rot3dSmem<R, LM, TJ_, SS_, PG_>::bytes;                                                   \
+    cudaFuncSetAttribute(k_allpairs_rot3d<R, LM, TJ_, SS_, PG_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
+    k_allpairs_rot3d<R, LM, TJ_, SS_, PG_><<<grid, TJ_, sm, a.stream>>>(a.pos, x, up, a.tiles, a.n_scat,        \
+                                                                        a.k_over_pi, a.inv_k, a.n_active, pacc); \
+  }
+#ifdef TM_RANGE_LO
+template <typename R> cudaError_t tm_launch_rot3d_lo(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, R* pacc) {
+  dim3 grid = a.grid;
+  grid.z = 2;                                         // y'-mirror sector: slowest grid dimension
+  switch (a.lmax) {
+    case 1: TM_LAUNCH_R3(1, 128, 16) break;
+    case 2: TM_LAUNCH_R3(2, 128, 16) break;
+    case 3: TM_LAUNCH_R3(3, 128, 16) break;
+    case 4: TM_LAUNCH_R3(4, 64, 4) break;
+    default: TM_LAUNCH_R3(5, 64, 4) break;
+  }
+  return cudaGetLastError();
+}
+template cudaError_t tm_launch_rot3d_lo<double>(const TmLaunch&, const Cx<double>*, Cx<double>*, double*);
+template cudaError_t tm_launch_rot3d_lo<float>(const TmLaunch&, const Cx<float>*, Cx<float>*, float*);
+void tm_cost_rot3d(int lmax, double* inst, double* flop) {
+  const int I[8] = {0, TM_R3D_FPINST_L1, TM_R3D_FPINST_L2, TM_R3D_FPINST_L3, TM_R3D_FPINST_L4, TM_R3D_FPINST_L5, TM_R3D_FPINST_L6, TM_R3D_FPINST_L7};
+  const int F[8] = {0, TM_R3D_FLOP_L1, TM_R3D_FLOP_L2, TM_R3D_FLOP_L3, TM_R3D_FLOP_L4, TM_R3D_FLOP_L5, TM_R3D_FLOP_L6, TM_R3D_FLOP_L7};
+  *inst = I[lmax]; *flop = F[lmax];
+}
+#endif
+#ifdef TM_RANGE_6
+template <typename R> cudaError_t tm_launch_rot3d_6(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, R* pacc) {
+  dim3 grid = a.grid;
+  grid.z = 2;
+  TM_LAUNCH_R3(6, 64, 4)
+  return cudaGetLastError();
+}
+template cudaError_t tm_launch_rot3d_6<double>(const TmLaunch&, const Cx<double>*, Cx<double>*, double*);
+template cudaError_t tm_launch_rot3d_6<float>(const TmLaunch&, const Cx<float>*, Cx<float>*, float*);
+#endif
+#ifdef TM_RANGE_7
+template <typename R> cudaError_t tm_launch_rot3d_7(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, R* pacc) {
+  dim3 grid = a.grid;
+  grid.z = 2;
+  TM_LAUNCH_R3(7, 64, 4)
+  return cudaGetLastError();
+}
+template cudaError_t tm_launch_rot3d_7<double>(const TmLaunch&, const Cx<double>*, Cx<double>*, double*);
+template cudaError_t tm_launch_rot3d_7<float>(const TmLaunch&, const Cx<float>*, Cx<float>*, float*);
+#endif
+#undef TM_LAUNCH_R3
+#endif
+
+#ifdef TM_SEC_GEN
+template <typename R> cudaError_t tm_launch_general(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, const TmConst* cst, TmTermsDev tb) {
+  const dim3 grid = a.grid;
+#define TM_LAUNCH_GEN(LM)                                                                                         \
+  {                                                                                                               \
+    const size_t sm = GenCfg<LM>::template smem<R>();                                                             \
+    cudaFuncSetAttribute(k_allpairs_general<R, LM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);        \
+    k_allpairs_general<R, LM><<<grid, 32 * GenCfg<LM>::WJ, sm, a.stream>>>(a.pos, x, up, a.tiles, cst, tb, a.n_scat, \
+                                                                           a.k_over_pi, a.inv_k, a.n_active);     \
+  }
+  switch (a.lmax) {
+    case 1: TM_LAUNCH_GEN(1) break;
+    case 2: TM_LAUNCH_GEN(2) break;
+    case 3: TM_LAUNCH_GEN(3) break;
+    case 4: TM_LAUNCH_GEN(4) break;
+    case 5: TM_LAUNCH_GEN(5) break;
+    case 6: TM_LAUNCH_GEN(6) break;
+    default: TM_LAUNCH_GEN(7) break;
+  }
+#undef TM_LAUNCH_GEN
+  return cudaGetLastError();
+}
+template cudaError_t tm_launch_general<double>(const TmLaunch&, const Cx<double>*, Cx<double>*, const TmConst*, TmTermsDev);
+template cudaError_t tm_launch_general<float>(const TmLaunch&, const Cx<float>*, Cx<float>*, const TmConst*, TmTermsDev);
+#endif

@@ -44,8 +44,8 @@ int main() {
     }
     C part[L];
     for (int i = 0; i < L; ++i) part[i].re = part[i].im = 0.0;
-    if (sct == 0) { CAT(tm_r3d_pair_L, LMAX, _S, 0)<double, 1>(xs, cph, sph, cth, sth, hr, hi, sr, si, ar, ai); CAT(tm_r3d_unmix_L, LMAX, _S, 0)<double, C, 1>(ar, ai, part); }
-    else { CAT(tm_r3d_pair_L, LMAX, _S, 1)<double, 1>(xs, cph, sph, cth, sth, hr, hi, sr, si, ar, ai); CAT(tm_r3d_unmix_L, LMAX, _S, 1)<double, C, 1>(ar, ai, part); }
+    if (sct == 0) { CAT(tm_r3d_pair_L, LMAX, _S, 0)<double, 1>(xs, cph, sph, cth, sth, hr, hi, sr, si, ar, ai, ar + NS, ai + NS); CAT(tm_r3d_unmix_L, LMAX, _S, 0)<double, C, 1>(ar, ai, ar + NS, ai + NS, part); }
+    else { CAT(tm_r3d_pair_L, LMAX, _S, 1)<double, 1>(xs, cph, sph, cth, sth, hr, hi, sr, si, ar, ai, ar + NS, ai + NS); CAT(tm_r3d_unmix_L, LMAX, _S, 1)<double, C, 1>(ar, ai, ar + NS, ai + NS, part); }
     for (int i = 0; i < L; ++i) { u[i].re += part[i].re; u[i].im += part[i].im; }
   }
   for (int i = 0; i < L; ++i) printf("%.17g %.17g\n", u[i].re, u[i].im);
