@@ -464,13 +464,20 @@ def run_ours(args, w, rank, world, local_rank):
         dist.destroy_process_group()
 
 
-def run_nyquist(args, w):
+def run_nyquist(args, w, rank=0, world=1, local_rank=0):
     """Recorded run of the paper's distribution strategy (NEXT-1; not the contract line): a Gaussian beam sampled on the
     lambda/2 grid -> jinc sources -> groups + padded windows batched on one GPU -> summed fields, against the undistributed
-    solve of the same sources."""
+    solve of the same sources.  Under torchrun (--gpus N) the windows are DEALT to the ranks (nyquist.simulate(rank, world,
+    dist): rank r solves windows r, r + N, ...) and the detector fields are summed by ONE all_reduce - the only exchange step of
+    the paper's strategy; strong scaling of one fixed problem, time = max over ranks."""
     import torch
     assert torch.cuda.is_available()
+    torch.cuda.set_device(local_rank)
     from paper_2107_09879_b200 import nyquist
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     half = float(np.abs(w["pos"][:, 0]).max()) + 0.25
     w0 = half / 2.0
     field = lambda x, y: (np.exp(-(x * x + y * y) / w0 ** 2), np.zeros_like(x))
@@ -478,20 +485,31 @@ def run_nyquist(args, w):
     g = np.linspace(-half, half, 33)
     pts = np.array([[a, b, 5.0] for a in g for b in g])
     out = {"mode": "nyquist", "workload": w["name"], "n_scat": int(w["pos"].shape[0]), "n_sources": int(src.shape[0]),
-           "group_samples": args.group, "padding": args.padding, "tol": args.tol or 1e-8}
-    t0 = time.perf_counter()
-    E, inf = nyquist.simulate(w, src, amp, gi, args.group, args.padding, pts, tol=args.tol or 1e-8)
+           "group_samples": args.group, "padding": args.padding, "tol": args.tol or 1e-8, "n_gpus": world,
+           "scaling": "strong (windows dealt to the ranks, one all_reduce of the detector field)"}
+    if dist is not None:
+        dist.barrier()
     torch.cuda.synchronize()
-    out.update(distributed={"n_windows": inf["n_windows"], "batched_scatterers": inf["n_batched_scatterers"], "iterations": inf["iterations"],
-                            "solve_seconds": inf["seconds"], "wall_seconds": time.perf_counter() - t0, "max_rel_residual": inf["max_rel_residual"],
-                            "converged": inf["rc"] == 0})
     t0 = time.perf_counter()
-    E0, inf0 = nyquist.simulate(w, src, amp, gi, None, 0.0, pts, tol=args.tol or 1e-8)
+    E, inf = nyquist.simulate(w, src, amp, gi, args.group, args.padding, pts, tol=args.tol or 1e-8, rank=rank, world=world, dist=dist)
     torch.cuda.synchronize()
-    out.update(undistributed={"iterations": inf0["iterations"], "solve_seconds": inf0["seconds"], "wall_seconds": time.perf_counter() - t0,
-                              "converged": inf0["rc"] == 0},
-               field_rel_l2_error=float(np.linalg.norm(E - E0) / np.linalg.norm(E0)))
-    print(json.dumps(out), flush=True)
+    wall = time.perf_counter() - t0
+    stats = max_over_ranks([wall, inf["seconds"]], dist, "cuda")
+    out.update(distributed={"n_windows_this_rank": inf["n_windows"], "batched_scatterers_this_rank": inf["n_batched_scatterers"],
+                            "iterations": inf["iterations"], "solve_seconds_max_over_ranks": stats[1], "wall_seconds_max_over_ranks": stats[0],
+                            "max_rel_residual": inf["max_rel_residual"], "converged": inf["rc"] == 0})
+    if rank == 0 and not args.no_undistributed:
+        t0 = time.perf_counter()
+        E0, inf0 = nyquist.simulate(w, src, amp, gi, None, 0.0, pts, tol=args.tol or 1e-8)
+        torch.cuda.synchronize()
+        out.update(undistributed={"iterations": inf0["iterations"], "solve_seconds": inf0["seconds"], "wall_seconds": time.perf_counter() - t0,
+                                  "converged": inf0["rc"] == 0},
+                   field_rel_l2_error=float(np.linalg.norm(E - E0) / np.linalg.norm(E0)))
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
 
 
 def run_gradient(args, w):
@@ -624,6 +642,7 @@ def main():
     ap.add_argument("--no-solve-record", action="store_true", help="hotpath mode: skip the config-2 full-solve sub-record")
     ap.add_argument("--group", type=int, default=16, help="nyquist mode: samples per group side")
     ap.add_argument("--padding", type=float, default=4.0, help="nyquist mode: padding in wavelengths")
+    ap.add_argument("--no-undistributed", action="store_true", help="nyquist mode: skip the undistributed reference solve")
     ap.add_argument("--kernel", default="auto", choices=["auto", "general", "coplanar", "sym3d", "rot3d"], help="force the all-pairs kernel variant")
     ap.add_argument("--lmax", type=int, default=None, help="override the VSWF truncation of a Mie config (lmax 6 = the paper's, PAPER.md:271)")
     ap.add_argument("--lmax-internal", type=int, default=0,
@@ -651,14 +670,15 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.workload == "paper_lens":        # the paper's own kind of layout (silicon cylinders, null-field T-matrices): nyquist mode
         assert args.mode == "nyquist", "--workload paper_lens is for --mode nyquist (or use --mode paper_case)"
-        if rank == 0:
-            from paper_2107_09879_b200 import libtm
-            w = W.paper_lens(args.scale or 56)
-            lmax = args.lmax or 6
-            gens = [W.generatrix_cylinder(r, w["height"], 64) for r in w["radii"]]
-            w.update(lmax=lmax, t_kind="full_types", win_ptr=np.array([0, w["pos"].shape[0]], dtype=np.int32),
-                     t_full=libtm.nullfield_tmatrix(lmax, w["k"], w["eps_r"], gens, lmax_internal=args.lmax_internal or 10))
-            run_nyquist(args, w)
+        import torch
+        torch.cuda.set_device(local_rank)
+        from paper_2107_09879_b200 import libtm
+        w = W.paper_lens(args.scale or 56)
+        lmax = args.lmax or 6
+        gens = [W.generatrix_cylinder(r, w["height"], 64) for r in w["radii"]]
+        w.update(lmax=lmax, t_kind="full_types", win_ptr=np.array([0, w["pos"].shape[0]], dtype=np.int32),
+                 t_full=libtm.nullfield_tmatrix(lmax, w["k"], w["eps_r"], gens, lmax_internal=args.lmax_internal or 10))
+        run_nyquist(args, w, rank, world, local_rank)
         return
     name = args.workload[3:] if args.workload.startswith("cfg") else args.workload
     w = W.config(name if name == "3b" else int(name), scale=args.scale)
@@ -675,8 +695,7 @@ def main():
         if rank == 0:
             run_paper_case(args)
     elif args.mode == "nyquist":
-        if rank == 0:
-            run_nyquist(args, w)
+        run_nyquist(args, w, rank, world, local_rank)
     elif args.mode == "gradient":
         if rank == 0:
             run_gradient(args, w)

@@ -60,10 +60,12 @@ typedef struct { const double *focus; double w0; tm_c64 Ax, Ay; int n_beta; } tm
  * (Eqs. II1-II17; reading R17).  Source s: flat angular spectrum inside the light cone,
  * centred at src_xyz[s] = (x_0, y_0, z_0), propagating along +z, transverse field on its plane
  * (Ax_s, Ay_s) J_1(k rho)/(k rho); window w owns the sources src_ptr[w] <= s < src_ptr[w+1].
- * A field sampled on the lambda/2 grid is carried by sources of amplitude (pi/2) x sample (reading R17).
+ * amp_is_sample != 0: `amp` holds the SAMPLES (Ex, Ey)(x_s, y_s) of a band-limited field on the lambda/2 grid and the library
+ * applies the Nyquist amplitude factor of reading R17 (a sample is carried by a source of amplitude (pi/2) x sample: the
+ * ideal disc low-pass of the square lambda/2 lattice); 0: `amp` holds the source amplitudes themselves.
  * All pointers are HOST pointers.  n_beta: Gauss-Legendre nodes on [0, pi/2] (0 -> 400 or more, as in tm_gauss_desc). */
 typedef struct { int n_src; const double *src_xyz; const tm_c64 *amp /* [n_src][2] */; const int *src_ptr /* [n_win+1] */;
-                 int n_beta; } tm_jinc_desc;
+                 int n_beta; int amp_is_sample; } tm_jinc_desc;
 
 /* Caller-supplied incident coefficients p[n_scat][L] (host or device). */
 typedef struct { const tm_c64 *p; } tm_coeffs_desc;

@@ -1106,7 +1106,9 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
       if (hptr[0] != 0 || hptr[ctx->n_win] != d->n_src) return fail(ctx, TM_E_INVALID, "src_ptr must start at 0 and end at n_src");
       for (int w = 0; w < ctx->n_win; ++w) if (hptr[w + 1] < hptr[w]) return fail(ctx, TM_E_INVALID, "src_ptr must be monotone");
       hsrc.assign(d->src_xyz, d->src_xyz + (size_t)d->n_src * 3);
-      for (int sidx = 0; sidx < 2 * d->n_src; ++sidx) hamp.push_back(make_double2(d->amp[sidx].re, d->amp[sidx].im));
+      // reading R17: a sample of the band-limited field on the lambda/2 grid is carried by a jinc source of amplitude (pi/2) x sample
+      const double nyq = d->amp_is_sample ? 0.5 * M_PI : 1.0;
+      for (int sidx = 0; sidx < 2 * d->n_src; ++sidx) hamp.push_back(make_double2(nyq * d->amp[sidx].re, nyq * d->amp[sidx].im));
       nb_req = d->n_beta;
     }
     const size_t nsrc = hsrc.size() / 3;
@@ -1154,15 +1156,20 @@ int tm_set_incident(tm_ctx* ctx, int kind, const void* desc) {
   k_gauss_nodes<LM><<<(nb + 127) / 128, 128, 0, ctx->stream>>>(d_beta, d_wq, nb, kw, static_cast<GaussNode<LM>*>(d_nodes)); \
   k_incident_gauss<LM><<<ctx->n_scat, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->d_win_of, d_src, d_amp, d_ptr,            \
                                                             static_cast<GaussNode<LM>*>(d_nodes), nb, ctx->k, ctx->d_p)
+#define TM_GAUSS_MODES(LM)      /* lmax >= 4: warp per scatterer, lane per (l, m >= 0) group, factorised node sums */    \
+  k_gauss_nodes<LM><<<(nb + 127) / 128, 128, 0, ctx->stream>>>(d_beta, d_wq, nb, kw, static_cast<GaussNode<LM>*>(d_nodes)); \
+  k_incident_modes<LM><<<(ctx->n_scat + 3) / 4, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->d_win_of, d_src, d_amp, d_ptr,  \
+                                                            static_cast<GaussNode<LM>*>(d_nodes), nb, ctx->k, ctx->n_scat, ctx->d_p)
       switch (lmax) {
         case 1: TM_GAUSS(1); break;
         case 2: TM_GAUSS(2); break;
         case 3: TM_GAUSS(3); break;
-        case 4: TM_GAUSS(4); break;
-        case 5: TM_GAUSS(5); break;
-        default: TM_GAUSS(6); break;
+        case 4: TM_GAUSS_MODES(4); break;
+        case 5: TM_GAUSS_MODES(5); break;
+        default: TM_GAUSS_MODES(6); break;
       }
 #undef TM_GAUSS
+#undef TM_GAUSS_MODES
       ctx->total_launches += 2;
       e = cudaGetLastError();
     }

@@ -40,7 +40,7 @@ class GaussDesc(ctypes.Structure):
 
 class JincDesc(ctypes.Structure):
     _fields_ = [("n_src", ctypes.c_int), ("src_xyz", ctypes.c_void_p), ("amp", ctypes.c_void_p), ("src_ptr", ctypes.c_void_p),
-                ("n_beta", ctypes.c_int)]
+                ("n_beta", ctypes.c_int), ("amp_is_sample", ctypes.c_int)]
 
 
 class CoeffsDesc(ctypes.Structure):
@@ -243,12 +243,13 @@ class Solver:
         d = GaussDesc(f.ctypes.data, float(w0), _c64(Ax), _c64(Ay), int(n_beta))
         return self._check(lib().tm_set_incident(self._h, TM_INC_GAUSS, ctypes.addressof(d)))
 
-    def set_incident_jinc(self, src, amp, src_ptr=None, n_beta=0):
-        """Jinc sources (PAPER.md Eqs. II1-II17): src (S,3), amp (S,2) complex transverse amplitudes, src_ptr (n_win+1,)."""
+    def set_incident_jinc(self, src, amp, src_ptr=None, n_beta=0, samples=False):
+        """Jinc sources (PAPER.md Eqs. II1-II17): src (S,3), amp (S,2) complex transverse amplitudes - or, with samples=True,
+        the field samples on the lambda/2 grid (the library applies the Nyquist factor of reading R17) -, src_ptr (n_win+1,)."""
         src = np.ascontiguousarray(src, dtype=np.float64).reshape(-1, 3)
         amp = np.ascontiguousarray(amp, dtype=np.complex128).reshape(-1, 2)
         ptr = np.array([0, src.shape[0]], dtype=np.int32) if src_ptr is None else np.ascontiguousarray(src_ptr, dtype=np.int32)
-        d = JincDesc(int(src.shape[0]), src.ctypes.data, amp.ctypes.data, ptr.ctypes.data, int(n_beta))
+        d = JincDesc(int(src.shape[0]), src.ctypes.data, amp.ctypes.data, ptr.ctypes.data, int(n_beta), 1 if samples else 0)
         return self._check(lib().tm_set_incident(self._h, TM_INC_JINC, ctypes.addressof(d)))
 
     def set_incident_coeffs(self, p):

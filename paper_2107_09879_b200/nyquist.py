@@ -21,14 +21,14 @@ def sample_grid(k, x_range, y_range):
 
 
 def jinc_sources(k, x_range, y_range, z0, field_fn, drop_below=0.0):
-    """Sources for a transverse field field_fn(x, y) -> (Ex, Ey) sampled on the Nyquist grid at z = z0.
-    A sample E is carried by a unit jinc source (transverse profile J_1(k rho)/(k rho)) of amplitude (pi/2) E: the ideal
-    disc low-pass of the lambda/2 lattice (reading R17).  Returns src (S,3), amp (S,2) complex, grid index (S,2)."""
+    """Sources for a transverse field field_fn(x, y) -> (Ex, Ey) sampled on the Nyquist grid at z = z0: one jinc source per
+    sample.  Returns src (S,3), the SAMPLES (S,2) complex and the grid index (S,2); the sample -> source-amplitude factor of
+    the method (reading R17) is applied by the library (tm_jinc_desc.amp_is_sample), not here."""
     xs, ys = sample_grid(k, x_range, y_range)
     X, Y = np.meshgrid(xs, ys, indexing="xy")
     IX, IY = np.meshgrid(np.arange(xs.size), np.arange(ys.size), indexing="xy")
     Ex, Ey = field_fn(X.ravel(), Y.ravel())
-    amp = 0.5 * np.pi * np.stack([np.asarray(Ex, dtype=complex), np.asarray(Ey, dtype=complex)], axis=1)
+    amp = np.stack([np.asarray(Ex, dtype=complex), np.asarray(Ey, dtype=complex)], axis=1)      # samples, not amplitudes
     src = np.stack([X.ravel(), Y.ravel(), np.full(X.size, float(z0))], axis=1)
     gi = np.stack([IX.ravel(), IY.ravel()], axis=1)
     keep = np.abs(amp).max(axis=1) > drop_below
@@ -85,7 +85,8 @@ def sum_fields(E_local, dist=None):
 def simulate(w, src, amp, grid_index, group, padding, pts, tol=1e-8, restart=50, max_iter=5000, precision=libtm.TM_FP64,
              stream=None, rank=0, world=1, dist=None):
     """Distributed simulation of workload `w` (global layout: pos, lmax, k, Mie radii per site or per type) driven by the
-    jinc sources (src, amp): plan windows, batch them, solve once, sum the scattered E fields of all windows at `pts`.
+    jinc sources (src, amp = field SAMPLES as returned by jinc_sources): plan windows, batch them, solve once, sum the scattered E
+    fields of all windows at `pts`.
     group = None: one window with every scatterer and every source (the undistributed reference).
     rank / world / dist: multi-GPU replicas - each rank solves its share of the windows, one all_reduce sums the fields.
     Returns (E (M,3), info dict)."""
@@ -108,7 +109,7 @@ def simulate(w, src, amp, grid_index, group, padding, pts, tol=1e-8, restart=50,
         s.set_tmatrices(T, inv.astype(np.int32), True, r_enclosing=radii[used])
     else:
         s.set_tmatrices(w["t_full"], type_of.astype(np.int32), False)
-    s.set_incident_jinc(b["src"], b["amp"], b["src_ptr"])
+    s.set_incident_jinc(b["src"], b["amp"], b["src_ptr"], samples=True)
     sol, info, rc = s.solve(tol, restart, max_iter)
     E = sum_fields(s.fields(np.ascontiguousarray(pts, dtype=np.float64), sol, libtm.TM_FIELD_E_SCA), dist)
     out = dict(n_windows=len(b["win_ptr"]) - 1, n_batched_scatterers=int(b["pos"].shape[0]), rc=rc,

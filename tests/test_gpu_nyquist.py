@@ -34,6 +34,9 @@ def test_jinc_incident_matches_oracle(tm):
     ref = np.concatenate([incident.jinc_sources_incident(3, W.K_B, pos[wp[i]:wp[i + 1]], src[sp[i]:sp[i + 1]], amp[sp[i]:sp[i + 1]])
                           for i in range(2)])
     assert rel(s.get_incident(), ref) <= 1e-11
+    # samples instead of amplitudes: the library applies the Nyquist factor of reading R17 (oracle: incident.nyquist_sources)
+    s.set_incident_jinc(src, amp, sp, samples=True)
+    assert rel(s.get_incident(), 0.5 * np.pi * ref) <= 1e-11
     s.close()
 
 

