@@ -209,7 +209,9 @@ int tm_pair_cost(const tm_ctx *ctx, double *fp_instructions, double *flop);
 
 /* Register-resident FMA microbenchmark on the current device (no memory traffic, 8 independent chains per
  * thread): the measured peak of the plain FP64 / FP32 pipe that the all-pairs kernel is bounded by.
- * precision TM_FP64 / TM_FP32; result in TFLOP/s (FMA = 2 flop).  Needs a CUDA device. */
+ * precision TM_FP64 / TM_FP32, or TM_PEAK_FP64_TENSOR: chains of FP64 tensor-core instructions (DMMA m8n8k4), the bound a
+ * dense-block multi-right-hand-side route would have; result in TFLOP/s (FMA = 2 flop).  Needs a CUDA device. */
+enum { TM_PEAK_FP64_TENSOR = 3 };
 int tm_measure_fma_peak(int precision, double *tflops, void *cuda_stream);
 
 /* Host helper: diagonal of the Lorenz-Mie T-matrix of a homogeneous sphere (reading R11; closed form,

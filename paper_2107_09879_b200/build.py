@@ -64,9 +64,24 @@ def build(force=False, verbose=False, jobs=None):
     os.makedirs(objdir, exist_ok=True)
     extra = os.environ.get("TM_NVCC_EXTRA", "").split()             # e.g. -DTM_COP4_SYNC_L6=255 for A/B builds
 
+    flag_file = os.path.join(objdir, "FLAGS")
+    flags_now = " ".join(CFLAGS + extra)
+    same_flags = os.path.exists(flag_file) and open(flag_file).read() == flags_now
+
+    def up_to_date(obj, dep):
+        """obj is newer than every file nvcc listed as a dependency of the unit (make-style .d file)."""
+        if force or verbose or not same_flags or not (os.path.exists(obj) and os.path.exists(dep)):
+            return False
+        words = open(dep).read().replace("\\\n", " ").split()
+        return all(os.path.exists(f) and _mtime(f) <= _mtime(obj) for f in words[1:] if not f.endswith(":"))
+
     def compile_one(unit):
         obj = os.path.join(objdir, unit[:-3] + ".o")
-        cmd = [NVCC] + CFLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, os.path.join(CSRC, unit)]
+        dep = obj + ".d"
+        if up_to_date(obj, dep):
+            return unit, obj, subprocess.CompletedProcess([], 0, "", "")
+        cmd = ([NVCC] + CFLAGS + extra + (["-Xptxas", "-v"] if verbose else [])
+               + ["-MD", "-MF", dep, "-c", "-o", obj, os.path.join(CSRC, unit)])
         r = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
         return unit, obj, r
     with ThreadPoolExecutor(max_workers=jobs or min(len(UNITS), os.cpu_count() or 1)) as ex:
@@ -76,6 +91,8 @@ def build(force=False, verbose=False, jobs=None):
             sys.stderr.write(f"== {unit}\n{r.stdout}{r.stderr}")
         if r.returncode != 0:
             raise subprocess.CalledProcessError(r.returncode, f"nvcc -c {unit}")
+    with open(flag_file, "w") as f:
+        f.write(flags_now)
     subprocess.check_call([NVCC, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a", "-o", SO]
                           + [obj for _, obj, _ in results], cwd=CSRC)
     return SO

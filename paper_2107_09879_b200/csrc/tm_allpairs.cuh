@@ -478,13 +478,15 @@ TM_R3D_SPEC(4, 1) TM_R3D_SPEC(5, 0) TM_R3D_SPEC(5, 1) TM_R3D_SPEC(6, 0) TM_R3D_S
 // PG: the partner sector's share of the accumulators lives in GLOBAL memory (L2-resident, [block][re/im][slot][thread],
 // coalesced) instead of shared memory: at lmax >= 6 the three per-thread vectors (scratch, own and partner accumulators)
 // leave room for a single 2-warp block per SM; with the partner share in L2 two blocks fit and every scheduler has a warp.
-template <typename R, int LMAX, int TJ, int SS, bool PG> struct Rot3dSmem {
+// PG = 2: the own sector's accumulators too (shared memory then holds only the scratch vector: 128-thread blocks, 8 warps per SM;
+// measured at lmax 6 on the 56x56 lattice: 27.4 ms (PG 1, 64 targets) -> 24.3 ms (PG 2, 128 targets); PG 2 with 64 targets: 33.0 ms).
+template <typename R, int LMAX, int TJ, int SS, int PG> struct Rot3dSmem {
   static constexpr int L = 2 * LMAX * (LMAX + 2);
-  // positions | staged d-values (own + partner = L slots) | scratch (L/2 slots) | accumulators (L or L/2 slots) | staging tables
-  static constexpr size_t bytes = sizeof(double) * 3 * SS + sizeof(R) * (size_t)(SS * L * 2 + L * TJ + (PG ? 1 : 2) * L * TJ) + sizeof(int) * 3 * L;
+  // positions | staged d-values (own + partner = L slots) | scratch (L/2 slots) | accumulators (L, L/2 or 0 slots) | staging tables
+  static constexpr size_t bytes = sizeof(double) * 3 * SS + sizeof(R) * (size_t)(SS * L * 2 + L * TJ + (2 - PG) * L * TJ) + sizeof(int) * 3 * L;
 };
 
-template <typename R, int LMAX, int TJ, int SS, bool PG>
+template <typename R, int LMAX, int TJ, int SS, int PG>
 __global__ void __launch_bounds__(TJ)
 k_allpairs_rot3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
                  const TmTile* __restrict__ tiles, int n_scat, double k_over_pi, double inv_k,
@@ -501,7 +503,7 @@ k_allpairs_rot3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
   R* s_x = reinterpret_cast<R*>(s_pz + SS);          // [source][2 NS] complex: own slots then partner slots
   R* s_scr = s_x + SS * L * 2;                       // [re/im][NS][TJ]
   R* s_acc = s_scr + L * TJ;                         // [re/im][NS][TJ] own sector, then (unless PG) [re/im][NS][TJ] partner share
-  int* s_sa = reinterpret_cast<int*>(s_acc + (PG ? 1 : 2) * L * TJ);
+  int* s_sa = reinterpret_cast<int*>(s_acc + (2 - PG) * L * TJ);
   int* s_sb = s_sa + L;
   int* s_ss = s_sb + L;
 
@@ -526,10 +528,11 @@ k_allpairs_rot3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
   R* ai = s_acc + NS * TJ + tid;
   R* pr = s_acc + L * TJ + tid;
   R* pi = s_acc + (L + NS) * TJ + tid;
-  if (PG) {
+  if (PG >= 1) {
     const size_t blk = ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
-    pr = g_pacc + blk * (size_t)(L * TJ) + tid;
+    pr = g_pacc + blk * (size_t)(PG * L * TJ) + tid;
     pi = pr + NS * TJ;
+    if (PG >= 2) { ar = pr + L * TJ; ai = ar + NS * TJ; }
   }
 #pragma unroll
   for (int b = 0; b < NS; ++b) { ar[b * TJ] = R(0); ai[b * TJ] = R(0); pr[b * TJ] = R(0); pi[b * TJ] = R(0); }

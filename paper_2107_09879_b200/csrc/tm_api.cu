@@ -121,7 +121,8 @@ struct tm_ctx {
     cudaGraphExec_t exec = nullptr;
     int transpose = -1, m = 0, rbytes = 0, n_part = 0, kernel = 0, launches = 0;
     double tol = 0.0;
-    const void *ws = nullptr, *T = nullptr, *upart = nullptr, *blob = nullptr, *tiles = nullptr;
+    const void *ws = nullptr, *T = nullptr, *upart = nullptr, *blob = nullptr, *tiles = nullptr, *pacc = nullptr;
+    int n_tiles = 0, n_chunk = 0, diag = -1;
   } cyc[2];
   bool graphs_ok = true;          // cleared when a capture fails (direct launches from then on)
   bool capturing = false;
@@ -482,7 +483,8 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
       const void* Tp = Tptr<R>(ctx);
       const bool hit = G.exec && G.transpose == transpose && G.m == m && G.rbytes == (int)sizeof(R) && G.n_part == ctx->n_part &&
                        G.kernel == ctx->kernel && G.tol == o.tol && G.ws == ctx->ws && G.T == Tp && G.upart == ctx->d_upart &&
-                       G.blob == ctx->gm.blob && G.tiles == ctx->d_tiles;
+                       G.blob == ctx->gm.blob && G.tiles == ctx->d_tiles && G.pacc == ctx->d_pacc && G.n_tiles == ctx->n_tiles &&
+                       G.n_chunk == ctx->n_chunk && G.diag == ctx->diag;
       if (!hit) {
         if (G.exec) { cudaGraphExecDestroy(G.exec); G.exec = nullptr; }
         const long long l0 = ctx->total_launches, a0 = ctx->allpairs_launches;
@@ -494,7 +496,7 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
           const cudaError_t ee = cudaStreamEndCapture(st, &graph);
           if (rc_cap == TM_OK && ee == cudaSuccess && graph && cudaGraphInstantiate(&G.exec, graph, 0) == cudaSuccess) {
             G.transpose = transpose; G.m = m; G.rbytes = (int)sizeof(R); G.n_part = ctx->n_part; G.kernel = ctx->kernel;
-            G.tol = o.tol; G.ws = ctx->ws; G.T = Tp; G.upart = ctx->d_upart; G.blob = ctx->gm.blob; G.tiles = ctx->d_tiles;
+            G.tol = o.tol; G.ws = ctx->ws; G.T = Tp; G.upart = ctx->d_upart; G.blob = ctx->gm.blob; G.tiles = ctx->d_tiles; G.pacc = ctx->d_pacc; G.n_tiles = ctx->n_tiles; G.n_chunk = ctx->n_chunk; G.diag = ctx->diag;
             G.launches = (int)(ctx->total_launches - l0);
           } else {
             G.exec = nullptr; ctx->graphs_ok = false;
@@ -634,7 +636,7 @@ int configure_kernel(tm_ctx* ctx) {
   TM_CUDA(tm_dev_alloc(&ctx->d_tiles, tiles.size() * sizeof(TmTile)));
   TM_CUDA(cudaMemcpy(ctx->d_tiles, tiles.data(), tiles.size() * sizeof(TmTile), cudaMemcpyHostToDevice));
   if (want == TM_KERNEL_ROT3D && tm_rot3d_pg(ctx->lmax)) {
-    const size_t per_block = (size_t)ctx->L * tm_rot3d_tj(ctx->lmax) * (ctx->precision == TM_FP32 ? sizeof(float) : sizeof(double));
+    const size_t per_block = (size_t)tm_rot3d_pg(ctx->lmax) * ctx->L * tm_rot3d_tj(ctx->lmax) * (ctx->precision == TM_FP32 ? sizeof(float) : sizeof(double));
     const size_t need_p = (size_t)ctx->n_tiles * ctx->n_chunk * 2 * per_block;
     if (need_p > ctx->pacc_bytes) {
       if (ctx->d_pacc) tm_dev_free(ctx->d_pacc);
@@ -1491,6 +1493,47 @@ __global__ void __launch_bounds__(256) k_fma_peak(R* out, int iters, R a, R b) {
   if (s == R(123.456)) out[0] = s;                      // never true; keeps the chains alive
 }
 
+// FP64 tensor-core (DMMA m8n8k4) chains: the number the multi-RHS dense-block route would be bounded by.
+__global__ void __launch_bounds__(256) k_dmma_peak(double* out, int iters, double a, double b) {
+  double c[8][2];
+#pragma unroll
+  for (int u = 0; u < 8; ++u) { c[u][0] = threadIdx.x * 1e-3 + u; c[u][1] = threadIdx.x * 2e-3 - u; }
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+      for (int u = 0; u < 8; ++u)
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                     : "+d"(c[u][0]), "+d"(c[u][1]) : "d"(a), "d"(b));
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int u = 0; u < 8; ++u) s += c[u][0] + c[u][1];
+  if (s == 123.456) out[0] = s;
+}
+
+int dmma_peak(double* tflops, cudaStream_t st) {
+  double* d = nullptr;
+  if (tm_dev_alloc(&d, sizeof(double)) != cudaSuccess) return TM_E_CUDA;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int blocks = 148 * 8, iters = 2048;
+  double best = 0.0;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0, st);
+    k_dmma_peak<<<blocks, 256, 0, st>>>(d, iters, 0.999999, 1e-7);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { tm_dev_free(d); return TM_E_CUDA; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double fl = 2.0 * 8 * 8 * 4 * 8.0 * 4.0 * (double)iters * (256.0 / 32.0) * blocks;   // m8n8k4 = 256 FMA per warp instruction
+    if (rep > 0) best = std::max(best, fl / (ms * 1e-3) * 1e-12);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); tm_dev_free(d);
+  *tflops = best;
+  return TM_OK;
+}
+
 template <typename R>
 int fma_peak_typed(double* tflops, cudaStream_t st) {
   R* d = nullptr;
@@ -1631,6 +1674,7 @@ int tm_measure_fma_peak(int precision, double* tflops, void* cuda_stream) {
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return TM_E_CUDA; }
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  if (precision == TM_PEAK_FP64_TENSOR) return dmma_peak(tflops, st);
   return precision == TM_FP32 ? fma_peak_typed<float>(tflops, st) : fma_peak_typed<double>(tflops, st);
 }
 

@@ -19,11 +19,19 @@ constexpr int TM_COP4_SS = 16;       // four-sector coplanar kernel (lmax 4..7):
 // of DIFFERENT sectors double the footprint; measured 6.80 -> 6.50 ms on the 56x56 lattice)
 inline int tm_cop4_tj(int lmax) { return lmax == 6 ? 256 : 128; }
 // rotation-based 3-D kernel: targets per block (shared memory per thread grows with L: scratch L/2 + accumulators L complex)
-inline int tm_rot3d_tj(int lmax) { return lmax <= 3 ? 128 : 64; }
 #ifndef TM_R3D_PG_FROM
-#define TM_R3D_PG_FROM 6             // lmax from which the partner share of the accumulators lives in global memory (L2)
+#define TM_R3D_PG_FROM 6             // lmax from which accumulators live in global memory (L2-resident)
 #endif
-inline bool tm_rot3d_pg(int lmax) { return lmax >= TM_R3D_PG_FROM; }
+#ifndef TM_R3D_PG_LEVEL
+#define TM_R3D_PG_LEVEL 2            // 1: the partner sector's share; 2: the own sector's accumulators too
+#endif
+#ifndef TM_R3D_TJ6
+#define TM_R3D_TJ6 128               // targets per block at lmax 6 (64 with PG level 1: shared memory)
+#endif
+inline int tm_rot3d_tj(int lmax) { return lmax <= 3 ? 128 : (lmax == 6 ? TM_R3D_TJ6 : 64); }
+// lmax 7 (internal: the gradient at lmax 6) stays at level 1 with 64-target blocks: at level 2 its compile time explodes
+constexpr int tm_rot3d_pg_level(int lmax) { return lmax < TM_R3D_PG_FROM ? 0 : (lmax == 6 ? TM_R3D_PG_LEVEL : 1); }
+inline int tm_rot3d_pg(int lmax) { return tm_rot3d_pg_level(lmax); }
 inline int tm_general_tj(int lmax) { return lmax <= 3 ? 4 : 2; }      // table-driven kernel: targets (warps) per block
 
 template <typename R> cudaError_t tm_launch_coplanar(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, int tj, TmShift shift);   // lmax 1..3

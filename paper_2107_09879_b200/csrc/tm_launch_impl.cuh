@@ -91,7 +91,7 @@ void tm_cost_sym3d(int lmax, double* inst, double* flop) {
 #ifdef TM_SEC_ROT3D
 #define TM_LAUNCH_R3(LM, TJ_, SS_)                                                                              \
   {                                                                                                             \
-    constexpr bool PG_ = LM >= TM_R3D_PG_FROM;                                                                  \
+    constexpr int PG_ = tm_rot3d_pg_level(LM);                                                                  \
     const size_t sm = Rot3dSmem<R, LM, TJ_, SS_, PG_>::bytes;                                                   \
     cudaFuncSetAttribute(k_allpairs_rot3d<R, LM, TJ_, SS_, PG_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
     k_allpairs_rot3d<R, LM, TJ_, SS_, PG_><<<grid, TJ_, sm, a.stream>>>(a.pos, x, up, a.tiles, a.n_scat,        \
@@ -122,7 +122,7 @@ void tm_cost_rot3d(int lmax, double* inst, double* flop) {
 template <typename R> cudaError_t tm_launch_rot3d_6(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, R* pacc) {
   dim3 grid = a.grid;
   grid.z = 2;
-  TM_LAUNCH_R3(6, 64, 4)
+  TM_LAUNCH_R3(6, TM_R3D_TJ6, 4)
   return cudaGetLastError();
 }
 template cudaError_t tm_launch_rot3d_6<double>(const TmLaunch&, const Cx<double>*, Cx<double>*, double*);

@@ -13,6 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "lib", "libtm.so")
 
 TM_FP64, TM_FP32, TM_MIXED = 0, 1, 2
+TM_PEAK_FP64_TENSOR = 3
 TM_OK, TM_NOT_CONVERGED = 0, 1
 TM_E_INVALID, TM_E_OVERLAP, TM_E_STATE, TM_E_CUDA, TM_E_NOMEM = -1, -2, -3, -4, -5
 TM_INC_PLANE, TM_INC_GAUSS, TM_INC_COEFFS, TM_INC_JINC = 0, 1, 2, 3

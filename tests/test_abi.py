@@ -33,7 +33,7 @@ def test_num_modes_and_enums(libtm):
     hdr = open(os.path.join(ROOT, "include", "tm.h")).read()
     for name in ("TM_FP64", "TM_FP32", "TM_OK", "TM_NOT_CONVERGED", "TM_E_INVALID", "TM_E_OVERLAP", "TM_E_STATE",
                  "TM_E_CUDA", "TM_E_NOMEM", "TM_INC_PLANE", "TM_INC_GAUSS", "TM_INC_COEFFS", "TM_INC_JINC", "TM_FIELD_E_SCA",
-                 "TM_FIELD_H_SCA", "TM_FIELD_E_INC", "TM_MIXED", "TM_KERNEL_AUTO", "TM_KERNEL_GENERAL", "TM_KERNEL_COPLANAR", "TM_KERNEL_SYM3D", "TM_KERNEL_ROT3D"):
+                 "TM_FIELD_H_SCA", "TM_FIELD_E_INC", "TM_MIXED", "TM_KERNEL_AUTO", "TM_KERNEL_GENERAL", "TM_KERNEL_COPLANAR", "TM_KERNEL_SYM3D", "TM_KERNEL_ROT3D", "TM_PEAK_FP64_TENSOR"):
         m = re.search(name + r"\s*=\s*(-?\d+)", hdr)
         assert m and int(m.group(1)) == getattr(libtm, name), name
 

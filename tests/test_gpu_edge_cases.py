@@ -333,3 +333,30 @@ def test_warm_start(tm, precision):
     lam2, il2, rc2 = s.solve_adjoint(wv, 1e-10, 30, 2000, out=lam2, warm_start=True)
     assert rc == 0 and rc2 == 0 and il2[0].iterations == 0 and rel_solve(lam2, lam) <= 1e-9
     s.close()
+
+
+def test_cuda_graph_cycles_equal_launch_by_launch_cycles(tm):
+    """Window-sized problems replay a full restart cycle as one CUDA graph: same kernels, same arguments, so the
+    iterates must equal - bit for bit - those of the launch-by-launch path (the library's timing mode), forward and transposed,
+    also after the T-matrices were replaced (the captured nodes bake the T pointer: the cache key must notice) and in TM_MIXED."""
+    w = W.config(2, scale=14)
+    for prec in (tm.TM_FP64, tm.TM_MIXED):
+        s = tm.solver_for_workload(w, precision=prec)
+        wv = rand_x((196, 30), 5)
+        s.kernel_time(reset=-1)                                          # production mode: graphs
+        a, ia, rca = s.solve(1e-10, 12, 600)                             # several cycles of restart 12
+        la, _, _ = s.solve_adjoint(wv, 1e-10, 12, 600)
+        a2, _, _ = s.solve(1e-10, 12, 600)                               # replay of the cached graph
+        s.kernel_time(reset=True)                                        # timing mode: launch by launch
+        b, ib, rcb = s.solve(1e-10, 12, 600)
+        lb, _, _ = s.solve_adjoint(wv, 1e-10, 12, 600)
+        assert rca == 0 and rcb == 0 and ia[0].iterations == ib[0].iterations and ia[0].restarts > 2
+        assert np.array_equal(a, b) and np.array_equal(a, a2) and np.array_equal(la, lb)
+        s.kernel_time(reset=-1)
+        # new T-matrices on the same context
+        w2 = dict(w, radii=np.asarray(w["radii"]) * 0.9)
+        T2 = np.stack([tm.mie_tmatrix(3, W.K_B, r, 4.0) for r in w2["radii"]])
+        s.set_tmatrices(T2, w["type_of"], True)
+        c, _, rcc = s.solve(1e-11, 12, 900)
+        assert rcc == 0 and rel_solve(c, driver.solve(w2)["s"]) <= 1e-9
+        s.close()
