@@ -146,6 +146,26 @@ int tm_matvec(tm_ctx *ctx, int transpose, const tm_c64 *x, tm_c64 *y);
  *   so that E_total = E_INC + E_SCA. */
 int tm_fields(tm_ctx *ctx, int n_pts, const double *pts, const tm_c64 *s, int which, tm_c64 *out);
 
+/* The same scattered fields through an entry point that ALLOCATES NOTHING - for callers that cannot call cudaMalloc (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid it).  No context: the caller passes inputs and outputs as
+ * DEVICE pointers (pos_dev [n_scat][3], s_dev [n_scat][L], pts_dev [n_pts][3], out_dev [n_pts][3]; host pointers are refused,
+ * nothing is copied), the kernels are enqueued on cuda_stream and the call returns WITHOUT synchronising (results are ready in
+ * stream order).  The per-source-chunk partial sums - the scratch tm_fields takes from its context - live in a file-scope static
+ * device array of 8 MiB that every GPU loading the library holds until exit.  Limits and rules:
+ *   - n_pts <= 65536 per call (lmax 1..6, n_scat >= 1); larger point sets are REJECTED with TM_E_INVALID and a message from
+ *     tm_fields_static_error() - split them or use tm_fields; there is no fallback allocation;
+ *   - all calls on a device share the one array: calls that OVERLAP on the GPU (two streams, two host threads, graphs replayed
+ *     concurrently) race on it and must be serialised by the caller; back-to-back calls on one stream are safe;
+ *   - the array keeps the last call's contents; nothing needs clearing (every partial sum read is written first by the same call);
+ *   - tm_fields_static_setup() resolves the array's device address for the CURRENT device (cudaGetSymbolAddress, once per
+ *     device); tm_fields_static does it lazily, so call the set-up once per device before a stream capture begins.
+ * Output equals tm_fields' (same kernels; bit-identical when both use the same number of source chunks).
+ * which: TM_FIELD_E_SCA or TM_FIELD_H_SCA.  Returns TM_OK, TM_E_INVALID or TM_E_CUDA. */
+int tm_fields_static_setup(void);
+int tm_fields_static(int lmax, double k_b, int n_scat, const double *pos_dev, const tm_c64 *s_dev, int n_pts,
+                     const double *pts_dev, int which, tm_c64 *out_dev, void *cuda_stream);
+const char *tm_fields_static_error(void);      /* message of the calling thread's last failed tm_fields_static* call */
+
 /* Device scratch.  tm_workspace_bytes: bytes tm_solve / tm_solve_adjoint need for these options (Krylov
  * basis etc.).  tm_set_workspace: hand in caller-allocated DEVICE memory (e.g. a torch tensor), 256-byte
  * aligned, which must outlive its use; without it the library allocates (and caches) its own. */

@@ -50,7 +50,7 @@ def sources():
 # Translation units: the host code and one per all-pairs kernel family (the generated straight-line code makes ptxas the
 # long pole of the build - compiled in parallel, the wall time is that of the largest family instead of their sum).
 UNITS = ["tm_api.cu", "tm_tu_coplanar.cu", "tm_tu_cop4_lo.cu", "tm_tu_cop4_hi.cu", "tm_tu_sym3d.cu", "tm_tu_rot3d_lo.cu",
-         "tm_tu_rot3d_6.cu", "tm_tu_rot3d_7.cu", "tm_tu_general.cu"]
+         "tm_tu_rot3d_6.cu", "tm_tu_rot3d_7.cu", "tm_tu_general.cu", "tm_static.cu"]
 CFLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 

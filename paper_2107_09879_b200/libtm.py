@@ -24,6 +24,7 @@ EXPORTS = ["tm_create", "tm_set_tmatrices", "tm_set_incident", "tm_get_incident"
            "tm_matvec", "tm_fields", "tm_workspace_bytes", "tm_set_workspace", "tm_set_kernel", "tm_get_kernel",
            "tm_kernel_time", "tm_pair_cost", "tm_measure_fma_peak", "tm_grad_tmatrix", "tm_grad_positions", "tm_mie_tmatrix_dR", "tm_mie_tmatrix",
            "tm_nullfield_tmatrix", "tm_nullfield_dtmatrix",
+           "tm_fields_static_setup", "tm_fields_static", "tm_fields_static_error",
            "tm_release_cached_memory", "tm_num_modes", "tm_last_error", "tm_destroy"]
 
 
@@ -102,6 +103,10 @@ def lib():
         L.tm_last_error.restype = ctypes.c_char_p
         L.tm_destroy.argtypes = [vp]
         L.tm_destroy.restype = None
+        L.tm_fields_static_setup.argtypes = []
+        L.tm_fields_static.argtypes = [ci, cd, ci, vp, vp, ci, vp, ci, vp, vp]
+        L.tm_fields_static_error.argtypes = []
+        L.tm_fields_static_error.restype = ctypes.c_char_p
         _lib = L
     return _lib
 
@@ -179,6 +184,28 @@ def measure_fma_peak(precision=TM_FP64, stream=None):
     if rc != TM_OK:
         raise TmError(rc, "tm_measure_fma_peak failed (no CUDA device?)")
     return v.value
+
+
+def fields_static_setup():
+    """Resolve the static scratch array of tm_fields_static on the current device (once per device; e.g. before a graph capture)."""
+    rc = lib().tm_fields_static_setup()
+    if rc != TM_OK:
+        raise TmError(rc, lib().tm_fields_static_error().decode())
+
+
+def fields_static(lmax, k_b, pos, s, pts, which=TM_FIELD_E_SCA, out=None, stream=None):
+    """tm_fields_static: scattered E (or Z_b H) at pts from coefficients s, allocation-free in the library.  pos (N,3) float64,
+    s (N,L) complex128, pts (M,3) float64: torch CUDA tensors; out (M,3) complex128 CUDA tensor (created here when None - pass
+    one in where the caller must not allocate either).  Enqueued on `stream` (raw cudaStream_t, default stream when None)
+    WITHOUT synchronising.  Raises TmError for M > 65536 and other invalid arguments."""
+    import torch
+    if out is None:
+        out = torch.empty((int(pts.shape[0]), 3), dtype=torch.complex128, device=pts.device)
+    rc = lib().tm_fields_static(int(lmax), float(k_b), int(pos.shape[0]), _ptr(pos), _ptr(s), int(pts.shape[0]), _ptr(pts), int(which),
+                                _ptr(out), ctypes.c_void_p(stream) if stream else None)
+    if rc != TM_OK:
+        raise TmError(rc, lib().tm_fields_static_error().decode())
+    return out
 
 
 def release_cached_memory():
