@@ -83,6 +83,7 @@ struct tm_ctx {
   tm_ctx* grad_aux = nullptr;           // tm_grad_positions: the same layout at lmax + 1 (all-pairs product A^ext)
   void* d_grad_tab = nullptr; TmGradDev grad_tab{};
   int cop_tj = 128;                     // coplanar kernel: targets per block (-DTM_COP_TJ=256 for experiments)
+  int cop_cl = 1;                       // coplanar kernel: cluster size along the chunk dimension (chunk partials reduced in DSMEM)
 
   double* d_pos = nullptr;
   std::vector<double> h_pos;      // host copy (quadrature sizing of the angular-spectrum sources)
@@ -278,7 +279,7 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
   cudaError_t e;
   if (c->kernel == TM_KERNEL_COPLANAR && c->lmax > 3)
     e = c->lmax <= 5 ? tm_launch_coplanar4_lo<R>(a, x, up, c->shift) : tm_launch_coplanar4_hi<R>(a, x, up, c->shift);
-  else if (c->kernel == TM_KERNEL_COPLANAR) e = tm_launch_coplanar<R>(a, x, up, c->cop_tj, c->shift);
+  else if (c->kernel == TM_KERNEL_COPLANAR) e = tm_launch_coplanar<R>(a, x, up, c->cop_tj, c->cop_cl, c->shift);
   else if (c->kernel == TM_KERNEL_ROT3D) {
     R* pacc = reinterpret_cast<R*>(c->d_pacc);
     e = c->lmax <= 5 ? tm_launch_rot3d_lo<R>(a, x, up, pacc) : (c->lmax == 6 ? tm_launch_rot3d_6<R>(a, x, up, pacc) : tm_launch_rot3d_7<R>(a, x, up, pacc));
@@ -645,7 +646,19 @@ int configure_kernel(tm_ctx* ctx) {
       ctx->pacc_bytes = need_p;
     }
   }
-  ctx->n_part = ctx->n_chunk * part_mult;
+  // Optional (build switch, OFF by default): on large planar problems (lmax <= 3) clusters of 4 or 2 chunk blocks sum their partials
+  // through distributed shared memory, so only n_chunk / cl partial buffers are written and read back.  Measured on config 5
+  // (8 chunks; profiles/r02_cluster_reduction.md): DRAM traffic of the launch 572 MB -> 177 MB (clusters of 2) / 64 MB (clusters
+  // of 4), launch time 132.6 -> 134.6 / 142.4 ms - the launch is ALU-bound, the traffic costs nothing, and only 71 of the 74
+  // clusters of 4 that the 296 block slots could hold are co-resident.  Parity with clusters on: 1e-12 (same tests).
+#ifndef TM_COP_CLUSTER
+#define TM_COP_CLUSTER 0              // largest cluster size: 4, 2, or 0 = never launch clusters
+#endif
+  ctx->cop_cl = 1;
+  if (TM_COP_CLUSTER >= 2 && want == TM_KERNEL_COPLANAR && !cop4 && ctx->cop_tj == 128 && ctx->n_chunk > 1 &&
+      (size_t)ctx->n_chunk * vec_bytes >= ((size_t)32 << 20))
+    ctx->cop_cl = (TM_COP_CLUSTER >= 4 && ctx->n_chunk % 4 == 0) ? 4 : (ctx->n_chunk % 2 == 0 ? 2 : 1);
+  ctx->n_part = ctx->n_chunk * part_mult / ctx->cop_cl;
   const size_t need = (size_t)ctx->n_part * vec_bytes;
   if (need > ctx->upart_bytes) {
     if (ctx->d_upart) tm_dev_free(ctx->d_upart);

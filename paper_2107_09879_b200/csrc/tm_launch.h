@@ -34,7 +34,8 @@ constexpr int tm_rot3d_pg_level(int lmax) { return lmax < TM_R3D_PG_FROM ? 0 : (
 inline int tm_rot3d_pg(int lmax) { return tm_rot3d_pg_level(lmax); }
 inline int tm_general_tj(int lmax) { return lmax <= 3 ? 4 : 2; }      // table-driven kernel: targets (warps) per block
 
-template <typename R> cudaError_t tm_launch_coplanar(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, int tj, TmShift shift);   // lmax 1..3
+// cl: cluster size along the chunk dimension (1: none; 2 or 4: chunk partials reduced through distributed shared memory, grid.y / cl partial buffers)
+template <typename R> cudaError_t tm_launch_coplanar(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, int tj, int cl, TmShift shift);   // lmax 1..3
 template <typename R> cudaError_t tm_launch_coplanar4_lo(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, TmShift shift);      // lmax 4, 5
 template <typename R> cudaError_t tm_launch_coplanar4_hi(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, TmShift shift);      // lmax 6, 7
 template <typename R> cudaError_t tm_launch_sym3d(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, TmShift shift);             // lmax 1..3

@@ -5,9 +5,34 @@
 #include "tm_allpairs.cuh"
 
 #ifdef TM_SEC_COP
-template <typename R> cudaError_t tm_launch_coplanar(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, int tj, TmShift shift) {
+// cluster launch of the coplanar kernel: CL blocks along the chunk dimension reduce their partials through distributed shared memory
+template <typename R, int LM, int CL>
+cudaError_t launch_coplanar_cluster(const TmLaunch& a, dim3 grid, const Cx<R>* x, Cx<R>* up, TmShift shift) {
+  constexpr int L = 2 * LM * (LM + 2);
+  const size_t sm = sizeof(Cx<R>) * (size_t)128 * L;  // staging rows [128 targets][L]
+  auto kern = k_allpairs_coplanar<R, LM, 128, TM_COP_SS, CL>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+  if (e != cudaSuccess) return e;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = sm; cfg.stream = a.stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = 1; at[0].val.clusterDim.y = CL; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, a.pos, x, up, a.tiles, a.n_scat, a.k_over_pi, a.inv_k, a.n_active, shift);
+}
+
+template <typename R> cudaError_t tm_launch_coplanar(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, int tj, int cl, TmShift shift) {
   dim3 grid = a.grid;
   grid.z = 2;                                         // mirror-parity half: slowest grid dimension
+  if (cl > 1 && tj == 128 && grid.y % cl == 0) {
+    cudaError_t e;
+    if (cl == 4) e = a.lmax == 1 ? launch_coplanar_cluster<R, 1, 4>(a, grid, x, up, shift)
+                   : (a.lmax == 2 ? launch_coplanar_cluster<R, 2, 4>(a, grid, x, up, shift) : launch_coplanar_cluster<R, 3, 4>(a, grid, x, up, shift));
+    else e = a.lmax == 1 ? launch_coplanar_cluster<R, 1, 2>(a, grid, x, up, shift)
+             : (a.lmax == 2 ? launch_coplanar_cluster<R, 2, 2>(a, grid, x, up, shift) : launch_coplanar_cluster<R, 3, 2>(a, grid, x, up, shift));
+    return e != cudaSuccess ? e : cudaGetLastError();
+  }
 #define TM_LAUNCH_COP2(LM, TJ)                                                                              \
   k_allpairs_coplanar<R, LM, TJ, TM_COP_SS><<<grid, TJ, 0, a.stream>>>(a.pos, x, up, a.tiles, a.n_scat,     \
                                                                        a.k_over_pi, a.inv_k, a.n_active, shift)
@@ -22,8 +47,8 @@ template <typename R> cudaError_t tm_launch_coplanar(const TmLaunch& a, const Cx
 #undef TM_LAUNCH_COP2
   return cudaGetLastError();
 }
-template cudaError_t tm_launch_coplanar<double>(const TmLaunch&, const Cx<double>*, Cx<double>*, int, TmShift);
-template cudaError_t tm_launch_coplanar<float>(const TmLaunch&, const Cx<float>*, Cx<float>*, int, TmShift);
+template cudaError_t tm_launch_coplanar<double>(const TmLaunch&, const Cx<double>*, Cx<double>*, int, int, TmShift);
+template cudaError_t tm_launch_coplanar<float>(const TmLaunch&, const Cx<float>*, Cx<float>*, int, int, TmShift);
 #endif
 
 #ifdef TM_SEC_COP4
