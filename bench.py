@@ -553,7 +553,7 @@ def run_gradient(args, w):
 def run_multirhs(args, w):
     """Recorded run (NEXT-3, multi-RHS; not the contract line): n_rhs plane waves (both polarisations, then two oblique ones) on ONE
     geometry, (a) solved one after the other on a single-window context and (b) batched - the geometry replicated as n_rhs windows
-    of one context, every window with its own right-hand side, Krylov scalars and convergence mask.  Also prints the measured
+    of one auxiliary context inside the library (tm_solve_multi), every window with its own right-hand side, Krylov scalars and convergence mask.  Also prints the measured
     FP64 tensor-core (DMMA) and FP64 FMA peaks: the bound of a dense-block multi-RHS route against that of the factorised apply."""
     import torch
     assert torch.cuda.is_available()
@@ -579,28 +579,22 @@ def run_multirhs(args, w):
     for (b, a, Ab, Aa) in waves:
         s1.set_incident_plane(b, a, Ab, Aa)
         ps.append(s1.get_incident())
-    s1.close()
-    pos = np.concatenate([w["pos"]] * n_rhs)
-    wp = (np.arange(n_rhs + 1) * N).astype(np.int32)
-    T = np.stack([libtm.mie_tmatrix(w["lmax"], w["k"], r, w["eps_r"]) for r in w["radii"]])
-    sb = libtm.Solver(pos, w["lmax"], w["k"], win_ptr=wp)
-    sb.set_tmatrices(T, np.concatenate([np.asarray(w["type_of"], dtype=np.int32)] * n_rhs), True)
-    sb.set_incident_coeffs(np.concatenate(ps))
-    for rep in range(2):
+    P = np.stack(ps)
+    for rep in range(2):                                    # tm_solve_multi: the geometry replicated as windows inside the library
         e0, e1 = ev(), ev()
         e0.record()
-        solb, infob, rcb = sb.solve(tol, restart, max_iter)
+        solb, infob, rcb = s1.solve_multi(P, tol, restart, max_iter)
         e1.record(); torch.cuda.synchronize()
         t_bat = e0.elapsed_time(e1)
-    err = max(float(np.linalg.norm(solb[i * N:(i + 1) * N] - sols[i]) / np.linalg.norm(sols[i])) for i in range(n_rhs))
+    err = max(float(np.linalg.norm(solb[i] - sols[i]) / np.linalg.norm(sols[i])) for i in range(n_rhs))
     st = torch.cuda.current_stream().cuda_stream
     print(json.dumps({"mode": "multirhs", "workload": w["name"], "n_scat": N, "lmax": w["lmax"], "n_rhs": n_rhs, "tol": tol,
                       "sequential_ms": t_seq, "sequential_iterations": its, "batched_ms": t_bat,
-                      "batched_iterations": [i.iterations for i in infob], "gain": t_seq / t_bat,
+                      "batched_iterations": [i[0].iterations for i in infob], "gain": t_seq / t_bat,
                       "max_rel_diff_batched_vs_sequential": err, "converged": bool(rcb == 0),
                       "fp64_fma_peak_tflops": libtm.measure_fma_peak(libtm.TM_FP64, st),
                       "fp64_tensor_dmma_peak_tflops": libtm.measure_fma_peak(libtm.TM_PEAK_FP64_TENSOR, st)}), flush=True)
-    sb.close()
+    s1.close()
 
 
 def run_nullfield(args):

@@ -132,6 +132,19 @@ int tm_solve(tm_ctx *ctx, const tm_solve_opts *opts, tm_c64 *s_out, tm_solve_inf
 int tm_solve_adjoint(tm_ctx *ctx, const tm_c64 *w, const tm_solve_opts *opts, tm_c64 *lambda_out,
                      tm_solve_info *info);
 
+/* Several right-hand sides on ONE geometry - both polarisations of a plane wave, many sources on one layout
+ * (PAPER.md:31-37); SURVEY.md 8(f) NEXT-3.  adjoint = 0: rhs [n_rhs][n_scat][L] are INCIDENT coefficients p_r, solved is
+ * (I - T A) s_r = T p_r; adjoint = 1: rhs are weight vectors w_r, solved is (I - T A)^T lambda_r = w_r.  out [n_rhs][n_scat][L];
+ * info: HOST [n_rhs][n_win] or NULL; rhs and out host or device.  The right-hand sides are solved TOGETHER: the geometry is
+ * replicated as one set of windows per right-hand side on an auxiliary context (created at the first call for this n_rhs and kept,
+ * n_rhs times the memory of ctx), every right-hand side keeps its own Krylov scalars and convergence mask, and every launch of
+ * the batched solver is shared.  Same solutions as n_rhs separate solves (same iteration counts, 1e-15); measured gain on one
+ * B200: 1.15x / 1.21x for n_rhs = 2 / 4 on a 32x32 lattice at lmax 3 (latency-bound), 1.00x / 1.04x on 56x56 at lmax 6
+ * (all-pairs-bound) - DESIGN.md section 9.  The incident field of ctx itself (tm_set_incident) is not touched.
+ * 1 <= n_rhs <= 64.  Returns as tm_solve (TM_NOT_CONVERGED if any right-hand side of any window did not converge). */
+int tm_solve_multi(tm_ctx *ctx, int adjoint, int n_rhs, const tm_c64 *rhs, const tm_solve_opts *opts, tm_c64 *out,
+                   tm_solve_info *info);
+
 /* One operator application: y = (I - T A) x (transpose = 0) or y = (I - T A)^T x (transpose = 1).
  * transpose = 2: y = A x (bare all-pairs translation matvec, Eq. I21; no T needed).  Parity and throughput. */
 int tm_matvec(tm_ctx *ctx, int transpose, const tm_c64 *x, tm_c64 *y);

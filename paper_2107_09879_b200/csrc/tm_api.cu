@@ -81,6 +81,9 @@ struct tm_ctx {
   int kernel_req = TM_KERNEL_AUTO, kernel = TM_KERNEL_GENERAL;
   TmShift shift{0.0, 0.0, 0.0, 0};      // target displacement (unused by the library: kept for A/B experiments)
   tm_ctx* grad_aux = nullptr;           // tm_grad_positions: the same layout at lmax + 1 (all-pairs product A^ext)
+  tm_ctx* multi_aux = nullptr;          // tm_solve_multi: the same geometry replicated as one set of windows per right-hand side
+  int multi_rhs = 0; long long multi_T_version = -1;
+  long long T_version = 0;              // bumped by tm_set_tmatrices
   void* d_grad_tab = nullptr; TmGradDev grad_tab{};
   int cop_tj = 128;                     // coplanar kernel: targets per block (-DTM_COP_TJ=256 for experiments)
   int cop_cl = 1;                       // coplanar kernel: cluster size along the chunk dimension (chunk partials reduced in DSMEM)
@@ -732,6 +735,7 @@ void tm_destroy(tm_ctx* c) {
   cudaStreamSynchronize(c->stream);
   for (auto& g : c->cyc) if (g.exec) cudaGraphExecDestroy(g.exec);
   if (c->grad_aux) tm_destroy(c->grad_aux);
+  if (c->multi_aux) tm_destroy(c->multi_aux);
   tm_dev_free(c->d_grad_tab);
   tm_dev_free(c->d_pos); tm_dev_free(c->d_win_of); tm_dev_free(c->d_type_of); tm_dev_free(c->d_T); tm_dev_free(c->d_T32); tm_dev_free(c->d_p);
   tm_dev_free(c->d_const); tm_dev_free(c->d_rowptr); tm_dev_free(c->d_col); tm_dev_free(c->d_widx); tm_dev_free(c->d_imag);
@@ -1038,7 +1042,7 @@ int tm_set_tmatrices(tm_ctx* ctx, int n_types, int diag_only, const tm_c64* T, c
   if (rc != TM_OK) { tm_dev_free(newT); ctx->d_T = oldT; return rc; }
   tm_dev_free(oldT);
   TM_CUDA(cudaMemcpy(ctx->d_type_of, ht.data(), ht.size() * sizeof(int), cudaMemcpyHostToDevice));
-  ctx->n_types = n_types; ctx->diag = diag_only ? 1 : 0; ctx->has_T = true;
+  ctx->n_types = n_types; ctx->diag = diag_only ? 1 : 0; ctx->has_T = true; ctx->T_version++;
   return TM_OK;
 }
 
@@ -1239,6 +1243,65 @@ int tm_solve_adjoint(tm_ctx* ctx, const tm_c64* w, const tm_solve_opts* opts, tm
   if (ctx->precision == TM_MIXED) return solve_typed<float, double>(ctx, 1, w, *opts, lambda_out, info);
   return ctx->precision == TM_FP64 ? solve_typed<double, double>(ctx, 1, w, *opts, lambda_out, info)
                                    : solve_typed<float, float>(ctx, 1, w, *opts, lambda_out, info);
+}
+
+// Several right-hand sides on ONE geometry (both polarisations; many sources): the geometry is
+// replicated as one set of windows per right-hand side on an auxiliary context (created at the first call for this n_rhs and
+// kept; T is cloned device to device and re-cloned after tm_set_tmatrices), so every right-hand side has its own Krylov scalars
+// and convergence mask and all of them share every launch of the batched solver.
+int tm_solve_multi(tm_ctx* ctx, int adjoint, int n_rhs, const tm_c64* rhs, const tm_solve_opts* opts, tm_c64* out, tm_solve_info* info) {
+  if (!ctx) return TM_E_INVALID;
+  int rc = check_opts(ctx, opts);
+  if (rc != TM_OK) return rc;
+  if (n_rhs < 1 || n_rhs > 64 || !rhs || !out) return fail(ctx, TM_E_INVALID, "need 1 <= n_rhs <= 64, rhs and out");
+  if (!ctx->has_T) return fail(ctx, TM_E_STATE, "tm_set_tmatrices must be called first");
+  if ((long long)ctx->n * n_rhs > 0x7fffffffLL) return fail(ctx, TM_E_INVALID, "n_rhs * n_scat * L must fit in int32");
+  TM_CUDA(stream_wait(ctx));
+  if (ctx->multi_aux && ctx->multi_rhs != n_rhs) { tm_destroy(ctx->multi_aux); ctx->multi_aux = nullptr; }
+  if (!ctx->multi_aux) {
+    const size_t N = ctx->n_scat;
+    std::vector<double> pos(3 * N * n_rhs);
+    std::vector<int> wp((size_t)ctx->n_win * n_rhs + 1);
+    for (int r = 0; r < n_rhs; ++r) {
+      std::copy(ctx->h_pos.begin(), ctx->h_pos.end(), pos.begin() + 3 * N * r);
+      for (int w = 0; w <= ctx->n_win; ++w) wp[(size_t)r * ctx->n_win + w] = ctx->win_ptr[w] + (int)(N * r);
+    }
+    rc = create_ctx(&ctx->multi_aux, (int)(N * n_rhs), pos.data(), ctx->n_win * n_rhs, wp.data(), ctx->lmax, ctx->k, ctx->precision,
+                    ctx->stream, TM_MAX_LMAX);
+    if (rc != TM_OK) return fail(ctx, rc, "auxiliary multi-RHS context: " + g_create_error);
+    ctx->multi_rhs = n_rhs; ctx->multi_T_version = -1;
+    if (ctx->kernel_req != TM_KERNEL_AUTO) { ctx->multi_aux->kernel_req = ctx->kernel_req; configure_kernel(ctx->multi_aux); }
+  }
+  tm_ctx* ax = ctx->multi_aux;
+  if (ctx->multi_T_version != ctx->T_version) {          // clone T (and its fp32 copy) device to device; replicate type_of
+    const size_t count = (size_t)ctx->n_types * ctx->L * (ctx->diag ? 1 : ctx->L);
+    tm_dev_free(ax->d_T); tm_dev_free(ax->d_T32); ax->d_T = nullptr; ax->d_T32 = nullptr;
+    TM_CUDA(tm_dev_alloc(&ax->d_T, count * elem_bytes(ctx)));
+    TM_CUDA(cudaMemcpy(ax->d_T, ctx->d_T, count * elem_bytes(ctx), cudaMemcpyDeviceToDevice));
+    if (ctx->d_T32) {
+      TM_CUDA(tm_dev_alloc(&ax->d_T32, count * sizeof(Cx<float>)));
+      TM_CUDA(cudaMemcpy(ax->d_T32, ctx->d_T32, count * sizeof(Cx<float>), cudaMemcpyDeviceToDevice));
+    }
+    for (int r = 0; r < n_rhs; ++r)
+      TM_CUDA(cudaMemcpy(ax->d_type_of + (size_t)r * ctx->n_scat, ctx->d_type_of, ctx->n_scat * sizeof(int), cudaMemcpyDeviceToDevice));
+    ax->n_types = ctx->n_types; ax->diag = ctx->diag; ax->has_T = true; ax->T_version++;
+    ctx->multi_T_version = ctx->T_version;
+  }
+  ax->time_kernels = false;
+  if (!adjoint) {                                         // rhs = incident coefficients p of every right-hand side; b = T p
+    TM_CUDA(copy_in(ax->d_p, rhs, ax->n * sizeof(double2), ax->stream));
+    ax->has_inc = true; ax->inc_kind = TM_INC_COEFFS;
+  }
+  if ((rc = ensure_workspace(ax, opts->restart)) != TM_OK) return fail(ctx, rc, ax->err);
+  if ((rc = ensure_gmres(ax, opts->restart)) != TM_OK) return fail(ctx, rc, ax->err);
+  const tm_c64* w = adjoint ? rhs : nullptr;
+  if (ctx->precision == TM_MIXED) rc = solve_typed<float, double>(ax, adjoint ? 1 : 0, w, *opts, out, info);
+  else rc = ctx->precision == TM_FP64 ? solve_typed<double, double>(ax, adjoint ? 1 : 0, w, *opts, out, info)
+                                      : solve_typed<float, float>(ax, adjoint ? 1 : 0, w, *opts, out, info);
+  if (rc < 0) return fail(ctx, rc, ax->err);
+  ctx->allpairs_launches += ax->allpairs_launches; ctx->total_launches += ax->total_launches;
+  ax->allpairs_launches = 0; ax->total_launches = 0;
+  return rc;
 }
 
 int tm_fields(tm_ctx* ctx, int n_pts, const double* pts, const tm_c64* s, int which, tm_c64* out) {

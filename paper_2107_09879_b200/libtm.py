@@ -21,7 +21,7 @@ TM_FIELD_E_SCA, TM_FIELD_H_SCA, TM_FIELD_E_INC = 0, 1, 2
 TM_KERNEL_AUTO, TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR, TM_KERNEL_SYM3D, TM_KERNEL_ROT3D = 0, 1, 2, 3, 4
 
 EXPORTS = ["tm_create", "tm_set_tmatrices", "tm_set_incident", "tm_get_incident", "tm_solve", "tm_solve_adjoint",
-           "tm_matvec", "tm_fields", "tm_workspace_bytes", "tm_set_workspace", "tm_set_kernel", "tm_get_kernel",
+           "tm_matvec", "tm_solve_multi", "tm_fields", "tm_workspace_bytes", "tm_set_workspace", "tm_set_kernel", "tm_get_kernel",
            "tm_kernel_time", "tm_pair_cost", "tm_measure_fma_peak", "tm_grad_tmatrix", "tm_grad_positions", "tm_mie_tmatrix_dR", "tm_mie_tmatrix",
            "tm_nullfield_tmatrix", "tm_nullfield_dtmatrix",
            "tm_fields_static_setup", "tm_fields_static", "tm_fields_static_error",
@@ -83,6 +83,7 @@ def lib():
         L.tm_solve.argtypes = [vp, ctypes.POINTER(SolveOpts), vp, vp]
         L.tm_solve_adjoint.argtypes = [vp, vp, ctypes.POINTER(SolveOpts), vp, vp]
         L.tm_matvec.argtypes = [vp, ci, vp, vp]
+        L.tm_solve_multi.argtypes = [vp, ci, ci, vp, ctypes.POINTER(SolveOpts), vp, vp]
         L.tm_fields.argtypes = [vp, ci, vp, vp, ci, vp]
         L.tm_workspace_bytes.argtypes = [vp, ctypes.POINTER(SolveOpts)]
         L.tm_workspace_bytes.restype = ctypes.c_size_t
@@ -339,6 +340,24 @@ class Solver:
         info = (SolveInfo * self.n_win)()
         rc = self._check(lib().tm_solve_adjoint(self._h, _ptr(w), ctypes.byref(o), _ptr(out), ctypes.addressof(info)))
         return out, list(info), rc
+
+    def solve_multi(self, rhs, tol, restart, max_iter, adjoint=False, out=None):
+        """tm_solve_multi: rhs (n_rhs, n_scat, L) incident coefficients (or adjoint weights) -> (out (n_rhs, n_scat, L),
+        info[n_rhs][n_win], rc)."""
+        rhs = np.ascontiguousarray(rhs, dtype=np.complex128) if isinstance(rhs, np.ndarray) else rhs
+        n_rhs = int(rhs.shape[0])
+        if out is None:
+            if isinstance(rhs, np.ndarray):
+                out = np.empty((n_rhs, self.n_scat, self.L), dtype=np.complex128)
+            else:
+                import torch
+                out = torch.empty((n_rhs, self.n_scat, self.L), dtype=torch.complex128, device=rhs.device)
+        o = SolveOpts(float(tol), int(restart), int(max_iter), 0)
+        info = (SolveInfo * (self.n_win * n_rhs))()
+        rc = self._check(lib().tm_solve_multi(self._h, 1 if adjoint else 0, n_rhs, _ptr(rhs), ctypes.byref(o), _ptr(out),
+                                              ctypes.addressof(info)))
+        flat = list(info)
+        return out, [flat[r * self.n_win:(r + 1) * self.n_win] for r in range(n_rhs)], rc
 
     def fields(self, pts, s, which=TM_FIELD_E_SCA, out=None):
         pts = np.ascontiguousarray(pts, dtype=np.float64) if isinstance(pts, np.ndarray) else pts

@@ -360,3 +360,43 @@ def test_cuda_graph_cycles_equal_launch_by_launch_cycles(tm):
         c, _, rcc = s.solve(1e-11, 12, 900)
         assert rcc == 0 and rel_solve(c, driver.solve(w2)["s"]) <= 1e-9
         s.close()
+
+
+def test_solve_multi_equals_separate_solves_and_the_oracle(tm):
+    """tm_solve_multi (NEXT-3: several right-hand sides on one geometry, solved together as replicated windows): same solutions and
+    iteration counts as separate solves, forward and adjoint, two windows, also after the T-matrices were replaced (the auxiliary
+    context must re-clone them) and in TM_MIXED; right-hand side 0 against the oracle's dense LU."""
+    w = W.cloud_workload(40, seed=77, lmax=3, n_win=2)
+    ref = driver.solve(w)
+    for prec in (tm.TM_FP64, tm.TM_MIXED):
+        s = tm.solver_for_workload(w, precision=prec)
+        P = [s.get_incident().copy()]
+        for (b, a, Ab, Aa) in ((0.0, 0.0, 0.0, 1.0), (0.7, 2.0, 0.3, 1.0 - 0.5j)):
+            s.set_incident_plane(b, a, Ab, Aa)
+            P.append(s.get_incident().copy())
+        P = np.stack(P)
+        sep, its = [], []
+        for r in range(3):
+            s.set_incident_coeffs(P[r])
+            sol, info, rc = s.solve(1e-11, 40, 2000)
+            assert rc == 0
+            sep.append(sol.copy()); its.append([i.iterations for i in info])
+        out, info, rc = s.solve_multi(P, 1e-11, 40, 2000)
+        assert rc == 0 and out.shape == (3, 40, 30)
+        for r in range(3):
+            assert rel_solve(out[r], sep[r]) <= 1e-12
+            assert [i.iterations for i in info[r]] == its[r]
+        assert rel_solve(out[0], ref["s"]) <= 1e-9
+        # adjoint right-hand sides
+        Wv = rand_x((2, 40, 30), 78)
+        lam, _, rc = s.solve_multi(Wv, 1e-11, 40, 2000, adjoint=True)
+        assert rc == 0
+        for r in range(2):
+            l1, _, _ = s.solve_adjoint(Wv[r], 1e-11, 40, 2000)
+            assert rel_solve(lam[r], l1) <= 1e-12
+        # new T-matrices: the cached auxiliary context must pick them up
+        w2 = dict(w, radii=np.asarray(w["radii"]) * 0.93)
+        s.set_tmatrices(np.stack([tm.mie_tmatrix(3, W.K_B, r, 4.0) for r in w2["radii"]]), w["type_of"], True)
+        out2, _, rc = s.solve_multi(P[:1], 1e-11, 40, 2000)              # and another n_rhs
+        assert rc == 0 and rel_solve(out2[0], driver.solve(w2)["s"]) <= 1e-9
+        s.close()
