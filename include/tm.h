@@ -189,7 +189,8 @@ int tm_set_workspace(tm_ctx *ctx, void *dev_ptr, size_t bytes);
  *   COPLANAR  generated code, all z equal (refused with TM_E_INVALID otherwise); two parity halves for lmax <= 3,
  *             four mirror sectors with shared-memory accumulators for lmax 4..6
  *   ROT3D     generated code, arbitrary 3-D positions, every lmax: rotation - axial translation - rotation with the polar
- *             rotation as constant frame change - phase rotation - constant frame change (O(L^1.5) work per pair)
+ *             rotation as constant frame change - phase rotation - constant frame change (O(L^1.5) work per pair);
+ *             lmax 4..6: warp-split organisation (register accumulators, instruction stream shared by the warps)
  *   SYM3D     generated code, arbitrary 3-D positions, lmax <= 3 (refused otherwise): direct pair-frame operator
  *   GENERAL   table-driven, arbitrary positions, lmax <= 6 (correct-by-table reference)
  * Default AUTO = COPLANAR if all z are equal, else ROT3D. */

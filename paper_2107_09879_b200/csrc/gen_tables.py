@@ -1630,6 +1630,270 @@ def emit_rot3d(lmaxes, path):
             f.write(f"#define TM_R3D_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")
 
 
+# ----------------------------------------------------------------------------- rot3d, warp-split (lmax >= 4)
+# Same mathematics as emit_rot3d.  The NP warps of a block share ONE target per lane.  Phases A (into the pair-axis frame) and B
+# (axial translation) touch no accumulator, so in a round every warp runs them - the SAME code, hence a shared instruction stream -
+# for a DIFFERENT source of the lane's target and leaves t in its own shared-memory scratch vector [slot][lane]; after a block
+# barrier, warp g runs phase C (back into the pair-azimuth frame and accumulation) of the (l, p) blocks it OWNS for each of the NP
+# sources of the round.  A thread accumulates only its own blocks' rows - n / NP slots, own sector + partner share - which fits
+# its registers: nothing is re-read per pair (the one-thread-per-target version rewrote 1.5 KB of accumulators per pair and
+# sector at lmax 6 and was memory-bound; splitting ALL phases over the warps made every warp stream its own code and was
+# instruction-fetch-bound, profiles/r02_rot3d.md).
+def _r3_lin(f, dst, src, rows, sel, counter):
+    for r in sel:
+        for part in ("r", "i"):
+            expr = None
+            for t, (c, v) in enumerate(rows[r]):
+                if t == 0:
+                    if abs(v) == 1:
+                        expr = f"{'-' if v < 0 else ''}{src}{part}{c}"
+                    else:
+                        expr = f"R({lit(v)}) * {src}{part}{c}"
+                        counter[0] += 1
+                        counter[1] += 1
+                else:
+                    expr = f"fma(R({lit(v)}), {src}{part}{c}, {expr})"
+                    counter[0] += 1
+                    counter[1] += 2
+            f.write(f"    const R {dst}{part}{r} = {expr};\n")
+
+
+def _r3_theta(f, src, dst, pairs, sel2, inverse, counter):
+    done = set()
+    for (ip, im_, m, form) in pairs:
+        if ip not in sel2:
+            continue
+        assert im_ in sel2 and form in ("r+", "r-")
+        sg = 1 if form == "r+" else -1
+        if inverse:
+            sg = -sg
+        a, b = ("", "-") if sg > 0 else ("-", "")
+        for part in ("r", "i"):
+            f.write(f"    const R {dst}{part}{ip} = fma({a}stm[{m}], {src}{part}{im_}, ctm[{m}] * {src}{part}{ip});\n")
+            f.write(f"    const R {dst}{part}{im_} = fma({b}stm[{m}], {src}{part}{ip}, ctm[{m}] * {src}{part}{im_});\n")
+        counter[0] += 8
+        counter[1] += 12
+        done.update((ip, im_))
+    for r in sel2:
+        if r not in done:
+            f.write(f"    const R {dst}r{r} = {src}r{r}, {dst}i{r} = {src}i{r};\n")
+
+
+def rot3d_ws_partition(lmax, sector, NP):
+    """-> (blocks, part_blocks, part_rows): (l,p) blocks [(b1, b2)], block indices per part (LPT on the frame-change work),
+    B3 rows per part (contiguous in |m''| order, balanced on the axial work)."""
+    slots, slots2, M1, M2, pairs, entries = sector
+    n = len(slots)
+    blocks = []
+    for p in (0, 1):
+        for l in range(1, lmax + 1):
+            b1 = [k for k, s_ in enumerate(slots) if s_[0] == l and s_[2] == p]
+            b2 = [k for k, s_ in enumerate(slots2) if s_[0] == l and s_[2] == p]
+            if b1:
+                blocks.append((b1, b2))
+    cost = [sum(len(M1[r]) for r in b2) + sum(len(M2[r]) for r in b1) + 3 * len(b1) for (b1, b2) in blocks]
+    part_blocks = [[] for _ in range(NP)]
+    load = [0] * NP
+    for bi in sorted(range(len(blocks)), key=lambda i: -cost[i]):
+        g = min(range(NP), key=lambda q: load[q])
+        part_blocks[g].append(bi)
+        load[g] += cost[bi]
+    for g in range(NP):
+        part_blocks[g].sort()
+    order = sorted(range(n), key=lambda k: (slots[k][1], k))           # rows by |m''|
+    rcost = [sum(4 + 2 * len(entries[(i, j)]) / 3.0 for j in range(n) if (i, j) in entries) for i in range(n)]
+    total = sum(rcost)
+    part_rows = [[] for _ in range(NP)]
+    acc, g = 0.0, 0
+    for i in order:
+        if g < NP - 1 and acc + 0.5 * rcost[i] > total * (g + 1) / NP:
+            g += 1
+        part_rows[g].append(i)
+        acc += rcost[i]
+    return blocks, part_blocks, part_rows
+
+
+def emit_rot3d_ws(lmaxes, path, NP=4):
+    with open(path, "w") as f:
+        f.write("// GENERATED by gen_tables.py - do not edit.\n")
+        f.write("// Rotation - axial translation - rotation for any pair direction, WARP-SPLIT (DESIGN.md, kernel K2r at lmax >= 4): one y'-mirror\n")
+        f.write("// sector per block, one target per lane.  A_*: phi rotation, frame change, theta rotation, frame change of ALL (l, p) blocks -> w\n")
+        f.write("// (scratch wr/wi, [slot * AS]);  B_*: axial translation of ALL rows, w -> t (in place when tr = wr: a |m''| group is read before its rows\n")
+        f.write(f"// are written);  C_*_P<g>: the way back of the (l, p) blocks OWNED by part g (one of {NP}) and the accumulation into that part's REGISTER\n")
+        f.write("// accumulators (ar/ai own sector, pr/pi partner share; local slot order);  unmix_*_P<g>: the part's share of u.\n#pragma once\n\n")
+        f.write("#ifndef TM_PIN\n#define TM_PIN(v)\n#endif\n\n")
+        for lmax in lmaxes:
+            md = modes(lmax)
+            idx = {t: i for i, t in enumerate(md)}
+            half_l = len(md) // 2
+            cost = [0, 0]
+            nslmax = 0
+            phases = ("    R cm[%d], sm[%d], ctm[%d], stm[%d];\n    cm[0] = R(1); sm[0] = R(0); cm[1] = cph; sm[1] = sph; "
+                      "ctm[0] = R(1); stm[0] = R(0); ctm[1] = cth; stm[1] = sth;\n" % ((lmax + 1,) * 4))
+            for m in range(2, lmax + 1):
+                phases += (f"    cm[{m}] = cm[{m - 1}] * cph - sm[{m - 1}] * sph; sm[{m}] = sm[{m - 1}] * cph + cm[{m - 1}] * sph; "
+                           f"ctm[{m}] = ctm[{m - 1}] * cth - stm[{m - 1}] * sth; stm[{m}] = stm[{m - 1}] * cth + ctm[{m - 1}] * sth;\n")
+            nph = (8 * max(0, lmax - 1), 12 * max(0, lmax - 1))
+            for sct, sector in enumerate(rot3d_sectors(lmax)):
+                slots, slots2, M1, M2, pairs, entries = sector
+                n = len(slots)
+                blocks, part_blocks, _ = rot3d_ws_partition(lmax, sector, NP)
+                sa, sb, ss = [], [], []
+                for (l, am, p, kind) in slots:
+                    sa.append(idx[(l, am, p)]); sb.append(idx[(l, -am, p)]); ss.append({"0": 0, "+": 1, "-": -1}[kind])
+                for (l, am, p, kind) in slots:
+                    sa.append(idx[(l, am, p)]); sb.append(idx[(l, -am, p)]); ss.append({"0": 0, "+": -1, "-": 1}[kind])
+                f.write(f"// lmax={lmax} sector={sct}: slots (l,|m|,p,kind) {slots}\n")
+                f.write(f"__device__ __constant__ int tm_r3w_sa_L{lmax}_S{sct}[{2 * n}] = {{{', '.join(map(str, sa))}}};\n")
+                f.write(f"__device__ __constant__ int tm_r3w_sb_L{lmax}_S{sct}[{2 * n}] = {{{', '.join(map(str, sb))}}};\n")
+                f.write(f"__device__ __constant__ int tm_r3w_ss_L{lmax}_S{sct}[{2 * n}] = {{{', '.join(map(str, ss))}}};\n")
+                covered = set()
+                for (l, am, p, kind) in slots:
+                    covered.add(idx[(l, am, p)]); covered.add(idx[(l, -am, p)])
+                cnt = [0, 0]
+                tagS = f"L{lmax}_S{sct}"
+                # ---- A: all (l, p) blocks
+                f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
+                        f"tm_r3w_A_{tagS}(const R* __restrict__ xs, R cph, R sph, R cth, R sth, R* wr, R* wi) {{\n" + phases)
+                cnt[0] += nph[0]; cnt[1] += nph[1]
+                for (b1, b2) in blocks:
+                    f.write("  {\n")
+                    for k in b1:
+                        l, am, p, kind = slots[k]
+                        if kind == "0":
+                            f.write(f"    const R xr{k} = xs[{2 * k}], xi{k} = xs[{2 * k + 1}];\n")
+                        else:
+                            f.write(f"    const R xr{k} = xs[{2 * k}] * cm[{am}] - xs[{2 * (n + k) + 1}] * sm[{am}], "
+                                    f"xi{k} = xs[{2 * k + 1}] * cm[{am}] + xs[{2 * (n + k)}] * sm[{am}];\n")
+                            cnt[0] += 4; cnt[1] += 6
+                    _r3_lin(f, "v", "x", M1, b2, cnt)
+                    _r3_theta(f, "v", "e", pairs, b2, False, cnt)
+                    _r3_lin(f, "w", "e", M2, b1, cnt)
+                    for k in b1:
+                        f.write(f"    wr[{k} * AS] = wr{k}; wi[{k} * AS] = wi{k};\n")
+                    f.write("  }\n")
+                f.write("}\n")
+                # ---- B: all rows, one |m''| group after the other
+                f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
+                        f"tm_r3w_B_{tagS}(R* hr, R* hi, const R* wr, const R* wi, R* tr, R* ti) {{\n")
+                for mm in sorted(set(s_[1] for s_ in slots)):
+                    grp = [k for k, s_ in enumerate(slots) if s_[1] == mm]
+                    f.write("  {\n")
+                    for j in grp:
+                        f.write(f"    const R wr{j} = wr[{j} * AS], wi{j} = wi[{j} * AS];\n")
+                    known = {}
+                    for i in grp:
+                        first = True
+                        newq, seen = set(), set(known)
+                        for j in grp:
+                            lst = entries.get((i, j))
+                            if lst:
+                                s0 = 1 if lst[0][1] > 0 else -1
+                                key = tuple((q, mp.nstr(s0 * v, 30)) for (q, v) in lst)
+                                if key not in seen:
+                                    seen.add(key)
+                                    newq.update(q for (q, _) in lst)
+                        if newq:
+                            f.write("    " + " ".join(f"TM_PIN(hr[{q}]); TM_PIN(hi[{q}]);" for q in sorted(newq)) + "\n")
+                        for j in grp:
+                            lst = entries.get((i, j))
+                            if not lst:
+                                continue
+                            s0 = 1 if lst[0][1] > 0 else -1
+                            key = tuple((q, mp.nstr(s0 * v, 30)) for (q, v) in lst)
+                            if key not in known:
+                                e = len(known)
+                                known[key] = e
+                                for part, hh in (("r", "hr"), ("i", "hi")):
+                                    expr = None
+                                    for t, (q, v) in enumerate(lst):
+                                        vv = s0 * v
+                                        if t == 0 and abs(vv) == 1:
+                                            expr = f"{'-' if vv < 0 else ''}{hh}[{q}]"
+                                        elif t == 0:
+                                            expr = f"R({lit(vv)}) * {hh}[{q}]"
+                                            cnt[0] += 1; cnt[1] += 1
+                                        else:
+                                            expr = f"fma(R({lit(vv)}), {hh}[{q}], {expr})"
+                                            cnt[0] += 1; cnt[1] += 2
+                                    f.write(f"    const R e{part}{e} = {expr};\n")
+                            e = known[key]
+                            sg = "" if s0 > 0 else "-"
+                            ng = "-" if s0 > 0 else ""
+                            if first:
+                                f.write(f"    R tr{i} = {sg}er{e} * wr{j}; tr{i} = fma({ng}ei{e}, wi{j}, tr{i}); "
+                                        f"R ti{i} = {sg}er{e} * wi{j}; ti{i} = fma({sg}ei{e}, wr{j}, ti{i});\n")
+                                cnt[0] += 4; cnt[1] += 6
+                                first = False
+                            else:
+                                f.write(f"    tr{i} = fma({sg}er{e}, wr{j}, tr{i}); tr{i} = fma({ng}ei{e}, wi{j}, tr{i}); "
+                                        f"ti{i} = fma({sg}er{e}, wi{j}, ti{i}); ti{i} = fma({sg}ei{e}, wr{j}, ti{i});\n")
+                                cnt[0] += 4; cnt[1] += 8
+                        assert not first
+                        f.write(f"    tr[{i} * AS] = tr{i}; ti[{i} * AS] = ti{i};\n")
+                    f.write("  }\n")
+                f.write("}\n")
+                # ---- C and unmix per owning part
+                for g in range(NP):
+                    myslots = [k for bi in part_blocks[g] for k in blocks[bi][0]]
+                    loc = {k: i for i, k in enumerate(myslots)}
+                    nslmax = max(nslmax, len(myslots))
+                    tag = f"{tagS}_P{g}"
+                    f.write(f"// part {g} owns the (l,p) blocks {[(slots[blocks[bi][0][0]][0], slots[blocks[bi][0][0]][2]) for bi in part_blocks[g]]}\n"
+                            f"#define TM_R3W_NSL_{tag} {len(myslots)}\n")
+                    f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
+                            f"tm_r3w_C_{tag}(R cph, R sph, R cth, R sth, const R* tr, const R* ti, R* ar, R* ai, R* pr, R* pi) {{\n" + phases)
+                    cnt[0] += nph[0]; cnt[1] += nph[1]
+                    for bi in part_blocks[g]:
+                        b1, b2 = blocks[bi]
+                        f.write("  {\n")
+                        for k in b1:
+                            f.write(f"    const R tr{k} = tr[{k} * AS], ti{k} = ti[{k} * AS];\n")
+                        _r3_lin(f, "v", "t", M1, b2, cnt)
+                        _r3_theta(f, "v", "e", pairs, b2, True, cnt)
+                        _r3_lin(f, "u", "e", M2, b1, cnt)
+                        for k in b1:
+                            l, am, p, kind = slots[k]
+                            li = loc[k]
+                            if kind == "0":
+                                f.write(f"    ar[{li}] += ur{k}; ai[{li}] += ui{k};\n")
+                                cnt[0] += 2; cnt[1] += 2
+                            else:
+                                f.write(f"    ar[{li}] = fma(ur{k}, cm[{am}], ar[{li}]); ai[{li}] = fma(ui{k}, cm[{am}], ai[{li}]);\n")
+                                f.write(f"    pr[{li}] = fma(ui{k}, sm[{am}], pr[{li}]); pi[{li}] = fma(-ur{k}, sm[{am}], pi[{li}]);\n")
+                                cnt[0] += 4; cnt[1] += 8
+                        f.write("  }\n")
+                    f.write("}\n")
+                    f.write("template <typename R, typename C>\n__device__ __forceinline__ void "
+                            f"tm_r3w_unmix_{tag}(const R* ar, const R* ai, const R* pr, const R* pi, C* out) {{\n")
+
+                    def store(i_flat, re, im):
+                        if i_flat >= half_l:
+                            f.write(f"  out[{i_flat}].re = {im}; out[{i_flat}].im = -({re});\n")
+                        else:
+                            f.write(f"  out[{i_flat}].re = {re}; out[{i_flat}].im = {im};\n")
+                    for k in myslots:
+                        l, am, p, kind = slots[k]
+                        li = loc[k]
+                        if kind == "0":
+                            store(idx[(l, 0, p)], f"ar[{li}]", f"ai[{li}]")
+                        else:
+                            plus_r, plus_i = (f"ar[{li}]", f"ai[{li}]") if kind == "+" else (f"pr[{li}]", f"pi[{li}]")
+                            minus_r, minus_i = (f"pr[{li}]", f"pi[{li}]") if kind == "+" else (f"ar[{li}]", f"ai[{li}]")
+                            store(idx[(l, am, p)], f"R(0.5) * ({plus_r} + {minus_r})", f"R(0.5) * ({plus_i} + {minus_i})")
+                            store(idx[(l, -am, p)], f"R(0.5) * ({plus_r} - {minus_r})", f"R(0.5) * ({plus_i} - {minus_i})")
+                    if g == 0:
+                        for i_flat in range(len(md)):
+                            if i_flat not in covered:
+                                f.write(f"  out[{i_flat}].re = R(0); out[{i_flat}].im = R(0);\n")
+                    f.write("}\n")
+                cost[0] += cnt[0]; cost[1] += cnt[1]
+                print(f"lmax={lmax} rot3d-ws sector={sct}: n={n} -> {cnt[0]} FP instructions, {cnt[1]} flop", file=sys.stderr)
+            f.write(f"#define TM_R3W_NSLMAX_L{lmax} {nslmax}\n")
+            f.write(f"#define TM_R3W_FPINST_L{lmax} {cost[0]}   // FP instructions per ordered pair (both sectors, all parts)\n")
+            f.write(f"#define TM_R3W_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")
+
+
 def main():
     os.makedirs(OUT, exist_ok=True)
     emit_tables([1, 2, 3, 4, 5, 6, 7], os.path.join(OUT, "tm_tables_gen.h"))     # 7: internal (gradient at lmax 6)
@@ -1638,6 +1902,7 @@ def main():
     emit_coplanar4([4, 5, 6, 7], os.path.join(OUT, "tm_coplanar4_gen.cuh"))     # 7: internal (gradient at lmax 6)
     emit_coplanar_f2([1, 2, 3], os.path.join(OUT, "tm_coplanar_f2_gen.cuh"))
     emit_rot3d([1, 2, 3, 4, 5, 6, 7], os.path.join(OUT, "tm_rot3d_gen.cuh"))      # 7: internal (gradient at lmax 6)
+    emit_rot3d_ws([4, 5, 6], os.path.join(OUT, "tm_rot3d_ws_gen.cuh"))
 
 
 if __name__ == "__main__":

@@ -490,9 +490,11 @@ k_allpairs_sym3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
 // because the frame changes are block diagonal in (l, p) and the axial translation in |m''|; accumulators (own sector +
 // partner share) in shared memory as in k_allpairs_sym3d.  Partial buffers and the finishing kernel as for sym3d.
 // zero-cost scheduling pin: the compiler must treat v as modified here (keeps a value's consumers after this point)
+#ifndef TM_PIN
 __device__ __forceinline__ void tm_pin(double& v) { asm volatile("" : "+d"(v)); }
 __device__ __forceinline__ void tm_pin(float& v) { asm volatile("" : "+f"(v)); }
 #define TM_PIN(v) tm_pin(v)
+#endif
 #include "generated/tm_rot3d_gen.cuh"
 
 template <typename R, int LMAX, int S> struct R3dPair;
@@ -623,6 +625,186 @@ k_allpairs_rot3d(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx
 }
 
 #endif  // TM_SEC_ROT3D
+#ifdef TM_SEC_ROT3DW
+// ---------------------------------------------------------------------------------------------------
+// Rotation-based 3-D kernel, WARP-SPLIT (lmax 4..6; gen_tables.py: emit_rot3d_ws).  Block = 4 warps x 32 targets: lane = target.
+// A round handles 4 sources: warp g runs phases A + B (into the pair-axis frame, axial translation) - the SAME straight-line code
+// in all warps, so the instruction stream is shared - for source s + g of its lane's target and leaves t in ITS scratch vector
+// [slot][lane]; block barrier; warp g then runs phase C (back into the pair-azimuth frame, accumulation) of the (l, p) blocks it
+// OWNS for each of the 4 sources, into REGISTER accumulators (n / 4 slots, own sector + partner share); block barrier.
+// The pair angles travel with t (4 values per lane and source in shared memory).
+#ifndef TM_PIN
+__device__ __forceinline__ void tm_pin(double& v) { asm volatile("" : "+d"(v)); }
+__device__ __forceinline__ void tm_pin(float& v) { asm volatile("" : "+f"(v)); }
+#define TM_PIN(v) tm_pin(v)
+#endif
+#include "generated/tm_rot3d_ws_gen.cuh"
+
+template <int LMAX, int S> struct R3wTab;
+#define TM_R3W_TAB(LM, SS_)                                                                               \
+  template <> struct R3wTab<LM, SS_> {                                                                    \
+    static __device__ __forceinline__ void entry(int k, int& a, int& b, int& sg) {                        \
+      a = tm_r3w_sa_L##LM##_S##SS_[k]; b = tm_r3w_sb_L##LM##_S##SS_[k]; sg = tm_r3w_ss_L##LM##_S##SS_[k]; \
+    }                                                                                                     \
+  };
+TM_R3W_TAB(4, 0) TM_R3W_TAB(4, 1) TM_R3W_TAB(5, 0) TM_R3W_TAB(5, 1) TM_R3W_TAB(6, 0) TM_R3W_TAB(6, 1)
+#undef TM_R3W_TAB
+
+template <typename R, int LMAX, int S> struct R3wSec;
+#define TM_R3W_SEC(LM, SS_)                                                                               \
+  template <typename R> struct R3wSec<R, LM, SS_> {                                                       \
+    template <int AS> static __device__ __forceinline__ void A(const R* xs, R cph, R sph, R cth, R sth, R* wr, R* wi) { \
+      tm_r3w_A_L##LM##_S##SS_<R, AS>(xs, cph, sph, cth, sth, wr, wi);                                     \
+    }                                                                                                     \
+    template <int AS> static __device__ __forceinline__ void B(R* hr, R* hi, R* wr, R* wi) {              \
+      tm_r3w_B_L##LM##_S##SS_<R, AS>(hr, hi, wr, wi, wr, wi);                                             \
+    }                                                                                                     \
+  };
+TM_R3W_SEC(4, 0) TM_R3W_SEC(4, 1) TM_R3W_SEC(5, 0) TM_R3W_SEC(5, 1) TM_R3W_SEC(6, 0) TM_R3W_SEC(6, 1)
+#undef TM_R3W_SEC
+template <typename R, int LMAX, int S, int P> struct R3wPart;
+#define TM_R3W_SPEC(LM, SS_, PP)                                                                          \
+  template <typename R> struct R3wPart<R, LM, SS_, PP> {                                                  \
+    template <int AS> static __device__ __forceinline__ void Cc(R cph, R sph, R cth, R sth, const R* tr, const R* ti, \
+                                                                R* ar, R* ai, R* pr, R* pi) {             \
+      tm_r3w_C_L##LM##_S##SS_##_P##PP<R, AS>(cph, sph, cth, sth, tr, ti, ar, ai, pr, pi);                 \
+    }                                                                                                     \
+    static __device__ __forceinline__ void unmix(const R* ar, const R* ai, const R* pr, const R* pi, Cx<R>* out) { \
+      tm_r3w_unmix_L##LM##_S##SS_##_P##PP<R, Cx<R>>(ar, ai, pr, pi, out);                                 \
+    }                                                                                                     \
+  };
+#define TM_R3W_SPEC_S(LM, SS_) TM_R3W_SPEC(LM, SS_, 0) TM_R3W_SPEC(LM, SS_, 1) TM_R3W_SPEC(LM, SS_, 2) TM_R3W_SPEC(LM, SS_, 3)
+TM_R3W_SPEC_S(4, 0) TM_R3W_SPEC_S(4, 1) TM_R3W_SPEC_S(5, 0) TM_R3W_SPEC_S(5, 1) TM_R3W_SPEC_S(6, 0) TM_R3W_SPEC_S(6, 1)
+#undef TM_R3W_SPEC_S
+#undef TM_R3W_SPEC
+template <int LMAX> struct R3wMax;
+template <> struct R3wMax<4> { static constexpr int nsl = TM_R3W_NSLMAX_L4; };
+template <> struct R3wMax<5> { static constexpr int nsl = TM_R3W_NSLMAX_L5; };
+template <> struct R3wMax<6> { static constexpr int nsl = TM_R3W_NSLMAX_L6; };
+
+template <typename R, int LMAX, int SS> struct Rot3dWsSmem {
+  static constexpr int L = 2 * LMAX * (LMAX + 2);
+  // positions | staged d-values (own + partner = L slots per source) | 4 scratch vectors ([re/im][L/2 slots][32 lanes], one per warp) |
+  // pair angles [warp][4][32 lanes] | staging tables
+  static constexpr size_t bytes = sizeof(double) * 3 * SS + sizeof(R) * (size_t)(SS * L * 2 + 4 * L * 32 + 4 * 4 * 32) + sizeof(int) * 3 * L;
+};
+
+// one sector (compile time) of the warp-split kernel; `warp` selects the part at run time (warp-uniform branch)
+template <typename R, int LMAX, int S, int SS>
+__device__ __forceinline__ void rot3d_ws_sector(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
+                                                const TmTile tile, int n_scat, double k_over_pi, double inv_k, unsigned char* smem_raw) {
+  constexpr int L = 2 * LMAX * (LMAX + 2), NS = L / 2, NQ = 2 * LMAX + 1, TJ = 32, NT = 128, NSL = R3wMax<LMAX>::nsl;
+  double* s_px = reinterpret_cast<double*>(smem_raw);
+  double* s_py = s_px + SS;
+  double* s_pz = s_py + SS;
+  R* s_x = reinterpret_cast<R*>(s_pz + SS);          // [source][2 NS] complex: own slots then partner slots
+  R* s_scr = s_x + SS * L * 2;                       // [warp][re/im][NS][TJ]: t of the warp's source of the round
+  R* s_ang = s_scr + 4 * L * TJ;                     // [warp][4][TJ]: cos / sin of the pair's azimuth and polar angle
+  int* s_sa = reinterpret_cast<int*>(s_ang + 4 * 4 * TJ);
+  int* s_sb = s_sa + L;
+  int* s_ss = s_sb + L;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const bool live = lane < tile.tgt_count;
+  const int j = tile.tgt_start + (live ? lane : tile.tgt_count - 1);
+  const double xj = pos[3 * j], yj = pos[3 * j + 1], zj = pos[3 * j + 2];
+  const int per = (tile.src_count + gridDim.y - 1) / gridDim.y;
+  const int c0 = tile.src_start + blockIdx.y * per;
+  const int c1 = min(tile.src_start + tile.src_count, c0 + per);
+  for (int e = tid; e < L; e += NT) {
+    int a, b, sg;
+    R3wTab<LMAX, S>::entry(e, a, b, sg);
+    s_sa[e] = a; s_sb[e] = b; s_ss[e] = sg;
+  }
+  R* wr = s_scr + (size_t)warp * L * TJ + lane;      // this warp's scratch vector
+  R* wi = wr + NS * TJ;
+  R ar[NSL], ai[NSL], pr[NSL], pi[NSL];
+#pragma unroll
+  for (int q = 0; q < NSL; ++q) { ar[q] = R(0); ai[q] = R(0); pr[q] = R(0); pi[q] = R(0); }
+
+  for (int s0 = c0; s0 < c1; s0 += SS) {
+    const int ns = min(SS, c1 - s0);
+    __syncthreads();                                   // previous stage consumed (also orders the staging tables)
+    for (int e = tid; e < ns; e += NT) {
+      s_px[e] = pos[3 * (s0 + e)]; s_py[e] = pos[3 * (s0 + e) + 1]; s_pz[e] = pos[3 * (s0 + e) + 2];
+    }
+    for (int e = tid; e < ns * L; e += NT) {
+      const int src = e / L, kk = e - src * L;
+      const Cx<R>* xrow = x + (size_t)(s0 + src) * L;
+      const int ia = s_sa[kk], sg = s_ss[kk];
+      Cx<R> v = xrow[ia];
+      if (sg != 0) {
+        const Cx<R> o = xrow[s_sb[kk]];
+        v = sg > 0 ? cadd(v, o) : csub(v, o);
+      }
+      if (ia >= NS) v = cx<R>(-v.im, v.re);            // tilde basis: multiply p = 1 modes by i
+      s_x[2 * e] = v.re;
+      s_x[2 * e + 1] = v.im;
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int s = 0; s < ns; s += 4) {
+      const int sg = s + warp;                       // this warp's source of the round
+      if (sg < ns) {
+        const double dx = xj - s_px[sg], dy = yj - s_py[sg], dz = zj - s_pz[sg];   // d = x_dest - x_source (reading R3)
+        const double rho2 = dx * dx + dy * dy, r2 = rho2 + dz * dz;
+        const double rinv = r2 > 0.0 ? rsqrt(r2) : 0.0;                            // self pair -> h_q = 0 -> t = 0
+        const double rhoinv = rho2 > 0.0 ? rsqrt(rho2) : 0.0;
+        const double r = r2 * rinv;
+        const R cph = rho2 > 0.0 ? (R)(dx * rhoinv) : R(1), sph = (R)(dy * rhoinv);
+        const R cth = r2 > 0.0 ? (R)(dz * rinv) : R(1), sth = (R)(rho2 * rhoinv * rinv);
+        R* ang = s_ang + (size_t)warp * 4 * TJ + lane;
+        ang[0] = cph; ang[TJ] = sph; ang[2 * TJ] = cth; ang[3 * TJ] = sth;
+        R3wSec<R, LMAX, S>::template A<TJ>(&s_x[sg * L * 2], cph, sph, cth, sth, wr, wi);
+        R ck, sk;
+        phase_kr<R>(k_over_pi, r, ck, sk);
+        R hr[NQ], hi[NQ];
+        hankel_up<R, NQ>((R)(rinv * inv_k), ck, sk, hr, hi);
+        R3wSec<R, LMAX, S>::template B<TJ>(hr, hi, wr, wi);
+      }
+      __syncthreads();                               // the round's t vectors are complete
+      const int nq = min(4, ns - s);
+#pragma unroll 1
+      for (int q = 0; q < nq; ++q) {
+        const R* ang = s_ang + (size_t)q * 4 * TJ + lane;
+        const R cph = ang[0], sph = ang[TJ], cth = ang[2 * TJ], sth = ang[3 * TJ];
+        const R* tr = s_scr + (size_t)q * L * TJ + lane;
+        const R* ti = tr + NS * TJ;
+        switch (warp) {
+          case 0: R3wPart<R, LMAX, S, 0>::template Cc<TJ>(cph, sph, cth, sth, tr, ti, ar, ai, pr, pi); break;
+          case 1: R3wPart<R, LMAX, S, 1>::template Cc<TJ>(cph, sph, cth, sth, tr, ti, ar, ai, pr, pi); break;
+          case 2: R3wPart<R, LMAX, S, 2>::template Cc<TJ>(cph, sph, cth, sth, tr, ti, ar, ai, pr, pi); break;
+          default: R3wPart<R, LMAX, S, 3>::template Cc<TJ>(cph, sph, cth, sth, tr, ti, ar, ai, pr, pi); break;
+        }
+      }
+      __syncthreads();                               // every owner has consumed the round before the scratch is rewritten
+    }
+  }
+  if (live) {
+    Cx<R>* out = u_part + ((size_t)(blockIdx.y * 2 + S) * n_scat + j) * L;
+    switch (warp) {
+      case 0: R3wPart<R, LMAX, S, 0>::unmix(ar, ai, pr, pi, out); break;
+      case 1: R3wPart<R, LMAX, S, 1>::unmix(ar, ai, pr, pi, out); break;
+      case 2: R3wPart<R, LMAX, S, 2>::unmix(ar, ai, pr, pi, out); break;
+      default: R3wPart<R, LMAX, S, 3>::unmix(ar, ai, pr, pi, out); break;
+    }
+  }
+}
+
+#ifndef TM_R3W_MINBLOCKS
+#define TM_R3W_MINBLOCKS 2
+#endif
+template <typename R, int LMAX, int SS>
+__global__ void __launch_bounds__(128, TM_R3W_MINBLOCKS)
+k_allpairs_rot3d_ws(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
+                    const TmTile* __restrict__ tiles, int n_scat, double k_over_pi, double inv_k,
+                    const int* __restrict__ n_active) {
+  if (n_active != nullptr && *n_active == 0) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const TmTile tile = tiles[blockIdx.x];
+  if (blockIdx.z == 0) rot3d_ws_sector<R, LMAX, 0, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, smem_raw);
+  else                 rot3d_ws_sector<R, LMAX, 1, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, smem_raw);
+}
+#endif  // TM_SEC_ROT3DW
 #ifdef TM_SEC_COP4
 // ---------------------------------------------------------------------------------------------------
 // Coplanar kernel for lmax 4..6 (the paper's truncation is lmax = 6).  Same mathematics as

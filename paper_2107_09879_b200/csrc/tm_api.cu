@@ -285,7 +285,8 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
   else if (c->kernel == TM_KERNEL_COPLANAR) e = tm_launch_coplanar<R>(a, x, up, c->cop_tj, c->cop_cl, c->shift);
   else if (c->kernel == TM_KERNEL_ROT3D) {
     R* pacc = reinterpret_cast<R*>(c->d_pacc);
-    e = c->lmax <= 5 ? tm_launch_rot3d_lo<R>(a, x, up, pacc) : (c->lmax == 6 ? tm_launch_rot3d_6<R>(a, x, up, pacc) : tm_launch_rot3d_7<R>(a, x, up, pacc));
+    if (tm_rot3d_ws(c->lmax)) e = tm_launch_rot3d_ws<R>(a, x, up);
+    else e = c->lmax <= 5 ? tm_launch_rot3d_lo<R>(a, x, up, pacc) : (c->lmax == 6 ? tm_launch_rot3d_6<R>(a, x, up, pacc) : tm_launch_rot3d_7<R>(a, x, up, pacc));
   } else if (c->kernel == TM_KERNEL_SYM3D) e = tm_launch_sym3d<R>(a, x, up, c->shift);
   else e = tm_launch_general<R>(a, x, up, c->d_const, TmTermsDev{c->d_rowptr, c->d_col, c->d_widx, c->d_imag, c->d_coef});
   tick(c, false);
@@ -604,7 +605,7 @@ int configure_kernel(tm_ctx* ctx) {
   int tgt_per_tile;
   const bool gen = want == TM_KERNEL_COPLANAR || want == TM_KERNEL_SYM3D || want == TM_KERNEL_ROT3D;   // generated kernels: thread = target
   switch (gen ? 0 : ctx->lmax) {
-    case 0: tgt_per_tile = want == TM_KERNEL_ROT3D ? tm_rot3d_tj(ctx->lmax) : (want == TM_KERNEL_SYM3D ? TM_SYM3D_TJ : (ctx->lmax > 3 ? tm_cop4_tj(ctx->lmax) : ctx->cop_tj)); break;
+    case 0: tgt_per_tile = want == TM_KERNEL_ROT3D ? (tm_rot3d_ws(ctx->lmax) ? 32 : tm_rot3d_tj(ctx->lmax)) : (want == TM_KERNEL_SYM3D ? TM_SYM3D_TJ : (ctx->lmax > 3 ? tm_cop4_tj(ctx->lmax) : ctx->cop_tj)); break;
     default: tgt_per_tile = tm_general_tj(ctx->lmax); break;
   }
   std::vector<TmTile> tiles;
@@ -620,7 +621,7 @@ int configure_kernel(tm_ctx* ctx) {
   // without a long tail; bounded by 64 chunks, >= 32 sources per chunk and 2 GB of partial sums.
   const bool cop4 = want == TM_KERNEL_COPLANAR && ctx->lmax > 3;   // four-sector coplanar kernel (lmax 4..6)
   const long long slots = 148LL * (cop4 ? 256 / tm_cop4_tj(ctx->lmax) : (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj :
-                                   (want == TM_KERNEL_SYM3D ? 2 : (want == TM_KERNEL_ROT3D ? (ctx->lmax <= 6 ? 2 : 1) : 4))));
+                                   (want == TM_KERNEL_SYM3D ? 2 : (want == TM_KERNEL_ROT3D ? (tm_rot3d_ws(ctx->lmax) ? 2 : (ctx->lmax <= 6 ? 2 : 1)) : 4))));
   const int cop4_z = !cop4 ? 0 : 4 * tm_cop4_groups(ctx->lmax);
   const long long blocks1 = (long long)ctx->n_tiles * (cop4 ? cop4_z : (gen ? 2 : 1));
   const int part_mult = (want == TM_KERNEL_SYM3D || want == TM_KERNEL_ROT3D || cop4) ? 2 : 1;   // one partial buffer per (chunk, y'-sector)
@@ -639,7 +640,7 @@ int configure_kernel(tm_ctx* ctx) {
   if (ctx->d_tiles) tm_dev_free(ctx->d_tiles);
   TM_CUDA(tm_dev_alloc(&ctx->d_tiles, tiles.size() * sizeof(TmTile)));
   TM_CUDA(cudaMemcpy(ctx->d_tiles, tiles.data(), tiles.size() * sizeof(TmTile), cudaMemcpyHostToDevice));
-  if (want == TM_KERNEL_ROT3D && tm_rot3d_pg(ctx->lmax)) {
+  if (want == TM_KERNEL_ROT3D && tm_rot3d_pg(ctx->lmax) && !tm_rot3d_ws(ctx->lmax)) {
     const size_t per_block = (size_t)tm_rot3d_pg(ctx->lmax) * ctx->L * tm_rot3d_tj(ctx->lmax) * (ctx->precision == TM_FP32 ? sizeof(float) : sizeof(double));
     const size_t need_p = (size_t)ctx->n_tiles * ctx->n_chunk * 2 * per_block;
     if (need_p > ctx->pacc_bytes) {
@@ -1641,6 +1642,7 @@ int tm_pair_cost(const tm_ctx* ctx, double* fp_instructions, double* flop) {
   if (!ctx) return TM_E_INVALID;
   double inst = 0.0, fl = 0.0;
   if (ctx->kernel == TM_KERNEL_COPLANAR) tm_cost_coplanar(ctx->lmax, &inst, &fl);
+  else if (ctx->kernel == TM_KERNEL_ROT3D && tm_rot3d_ws(ctx->lmax)) tm_cost_rot3d_ws(ctx->lmax, &inst, &fl);
   else if (ctx->kernel == TM_KERNEL_ROT3D) tm_cost_rot3d(ctx->lmax, &inst, &fl);
   else if (ctx->kernel == TM_KERNEL_SYM3D) tm_cost_sym3d(ctx->lmax, &inst, &fl);
   else {   // general kernel: per (term, source): 2 MUL + 4 FMA

@@ -42,6 +42,13 @@ template <typename R> cudaError_t tm_launch_sym3d(const TmLaunch& a, const Cx<R>
 template <typename R> cudaError_t tm_launch_rot3d_lo(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, R* pacc);                // lmax 1..5
 template <typename R> cudaError_t tm_launch_rot3d_6(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, R* pacc);
 template <typename R> cudaError_t tm_launch_rot3d_7(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, R* pacc);
+// warp-split rotation-based kernel (lmax 4..6): 32 targets per tile, 4 warps = 4 parts of the sector's code
+#ifndef TM_R3D_WS
+#define TM_R3D_WS 1                  // build switch: 0 = keep the one-thread-per-target rotation-based kernel at lmax 4..6
+#endif
+inline bool tm_rot3d_ws(int lmax) { return TM_R3D_WS && lmax >= 4 && lmax <= 6; }
+template <typename R> cudaError_t tm_launch_rot3d_ws(const TmLaunch& a, const Cx<R>* x, Cx<R>* up);
+void tm_cost_rot3d_ws(int lmax, double* inst, double* flop);
 template <typename R> cudaError_t tm_launch_general(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, const TmConst* cst, TmTermsDev tb);   // lmax 1..7
 
 int tm_cop4_groups(int lmax);                                  // row groups per sector (generated constant)

@@ -195,3 +195,21 @@ def test_generated_rotation_based_3d_pair_code_matches_oracle_block(lmax, tmp_pa
         u = np.array([complex(*map(float, ln.split())) for ln in out.strip().splitlines()])
         ref = tr.block(lmax, K, np.array(d, dtype=float), np.zeros(3)) @ x
         assert np.abs(u - ref).max() <= 2e-13 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("lmax", [4, 5, 6])
+def test_generated_warp_split_3d_pair_code_matches_oracle_block(lmax, tmp_path):
+    """Generated warp-split rotation-based code (tm_rot3d_ws_gen.cuh: the AUTO kernel of non-planar layouts at lmax 4..6) compiled as
+    host C++ - phase A, phase B in place, then every owner part's phase C and unmix - against the oracle block, including pairs along
+    +-z, in the plane, along -x and far apart."""
+    exe = str(tmp_path / f"hostcheck_rot3d_ws_{lmax}")
+    subprocess.check_call(["g++", "-O0", f"-DLMAX={lmax}", "-o", exe, os.path.join(ROOT, "tests", "hostcheck_rot3d_ws.cpp")])
+    rng = np.random.default_rng(50 + lmax)
+    L = n_modes(lmax)
+    for d in ([0.3, -0.4, 0.8], [0.0, 0.0, 1.2], [0.0, 0.0, -0.7], [1.0, 0.5, 0.0], [-0.6, 0.0, 0.0], rng.uniform(-30, 30, 3), rng.uniform(-3, 3, 3)):
+        x = rng.standard_normal(L) + 1j * rng.standard_normal(L)
+        inp = " ".join(repr(float(v)) for v in d) + "\n" + "\n".join(f"{float(z.real)!r} {float(z.imag)!r}" for z in x) + "\n"
+        out = subprocess.run([exe], input=inp, capture_output=True, text=True, check=True).stdout
+        u = np.array([complex(*map(float, ln.split())) for ln in out.strip().splitlines()])
+        ref = tr.block(lmax, K, np.array(d, dtype=float), np.zeros(3)) @ x
+        assert np.abs(u - ref).max() <= 2e-13 * np.abs(ref).max()
