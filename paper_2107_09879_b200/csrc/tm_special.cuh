@@ -41,6 +41,10 @@ __host__ __device__ inline void ang_functions(double ct, double st, double (*P)[
 
 // Cylindrical Bessel J_0..J_nmax(x), x >= 0, by Miller's backward recurrence normalised with
 // 1 = J_0 + 2 sum_{k>=1} J_2k  (absolute accuracy ~1e-15, uniform in x; used for Eq. II11).
+// The recurrence J_{n-1} = (2n/x) J_n - J_{n+1} starts at an even N = x + 18 x^{1/3} + 30 with J_{N+1} = 0, J_N = 1e-250.  Two steps per
+// loop iteration down to the orders that are needed (no stores, no parity test; the coefficient 2n/x is formed from an exact
+// double counter), then a fully unrolled tail that stores J_0..J_NMAX.  No rescaling: from 1e-250 the unnormalised values grow by
+// at most ~1e100 for the arguments that occur (k rho sin(beta) <= a few hundred), far from overflow.
 template <int NMAX>
 __host__ __device__ inline void bessel_j_all(double x, double* J) {
   if (x < 1e-8) {
@@ -49,23 +53,31 @@ __host__ __device__ inline void bessel_j_all(double x, double* J) {
     for (int n = 1; n <= NMAX; ++n) { t *= 0.5 * x / n; J[n] = t; }
     return;
   }
+  constexpr int NSTOP = (NMAX + 3) & ~1;             // smallest even number >= NMAX + 2
   int N = (int)(x + 18.0 * cbrt(x > 1.0 ? x : 1.0)) + 30;
   N += (N & 1);                                      // even start
+  if (N < NSTOP) N = NSTOP;
   const double tx = 2.0 / x;
-  double jp1 = 0.0, jn = 1e-250, sum = 0.0;
-  for (int n = N; n >= 1; --n) {                     // jn holds J_n (unnormalised)
-    const double jm1 = n * tx * jn - jp1;
-    jp1 = jn; jn = jm1;                              // now jn = J_{n-1}
-    if (n - 1 <= NMAX) J[n - 1] = jn;
-    if (n <= NMAX) { /* J[n] was stored one step earlier */ }
-    if (((n - 1) & 1) == 0 && n - 1 > 0) sum += 2.0 * jn;
-    if (fabs(jn) > 1e200) {                          // rescale
-      const double sc = 1e-200;
-      jn *= sc; jp1 *= sc; sum *= sc;
-      for (int k = n - 1; k <= NMAX; ++k) J[k] *= sc;
-    }
+  double jp1 = 0.0, jn = 1e-250, sum = 0.0;          // J_{n+1}, J_n (unnormalised), n = N
+  double dn = (double)N;
+  for (int n = N; n > NSTOP; n -= 2) {
+    const double jm1 = fma(dn * tx, jn, -jp1);       // J_{n-1}
+    dn -= 1.0;
+    const double jm2 = fma(dn * tx, jm1, -jn);       // J_{n-2}, n - 2 even and > 0
+    dn -= 1.0;
+    sum = fma(2.0, jm2, sum);
+    jp1 = jm1; jn = jm2;
+  }
+#pragma unroll
+  for (int m = NSTOP; m >= 1; --m) {                 // jn = J_m -> J_{m-1}
+    const double jm1 = fma(dn * tx, jn, -jp1);
+    dn -= 1.0;
+    jp1 = jn; jn = jm1;
+    if (m - 1 <= NMAX) J[m - 1] = jn;
+    if (((m - 1) & 1) == 0 && m - 1 > 0) sum = fma(2.0, jn, sum);
   }
   sum += jn;                                         // J_0 term
   const double inv = 1.0 / sum;
+#pragma unroll
   for (int n = 0; n <= NMAX; ++n) J[n] *= inv;
 }
