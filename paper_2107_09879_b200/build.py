@@ -32,7 +32,7 @@ def generate(force=False):
     gen_py = os.path.join(CSRC, "gen_tables.py")
     stamp = os.path.join(GEN, "GENERATOR_SHA256")
     outs = [os.path.join(GEN, f) for f in ("tm_tables_gen.h", "tm_coplanar_gen.cuh", "tm_coplanar_f2_gen.cuh",
-                                           "tm_general3d_gen.cuh", "tm_coplanar4_gen.cuh", "tm_rot3d_gen.cuh", "tm_rot3d_ws_gen.cuh", "tm_coplanar4_ws_gen.cuh")]
+                                           "tm_general3d_gen.cuh", "tm_coplanar4_gen.cuh", "tm_rot3d_gen.cuh", "tm_rot3d_ws_gen.cuh")]
     have = open(stamp).read().strip() if os.path.exists(stamp) else ""
     if force or have != _gen_hash() or not all(os.path.exists(o) for o in outs):
         subprocess.check_call([sys.executable, gen_py])
@@ -50,7 +50,7 @@ def sources():
 # Translation units: the host code and one per all-pairs kernel family (the generated straight-line code makes ptxas the
 # long pole of the build - compiled in parallel, the wall time is that of the largest family instead of their sum).
 UNITS = ["tm_api.cu", "tm_tu_coplanar.cu", "tm_tu_cop4_lo.cu", "tm_tu_cop4_hi.cu", "tm_tu_sym3d.cu", "tm_tu_rot3d_lo.cu",
-         "tm_tu_rot3d_6.cu", "tm_tu_rot3d_7.cu", "tm_tu_general.cu", "tm_tu_rot3d_ws.cu", "tm_tu_cop4_ws.cu", "tm_static.cu"]
+         "tm_tu_rot3d_6.cu", "tm_tu_rot3d_7.cu", "tm_tu_general.cu", "tm_tu_rot3d_ws.cu", "tm_static.cu"]
 CFLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 

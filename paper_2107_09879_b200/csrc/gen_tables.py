@@ -1894,221 +1894,6 @@ def emit_rot3d_ws(lmaxes, path, NP=4):
             f.write(f"#define TM_R3W_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")
 
 
-# ----------------------------------------------------------------------------- coplanar four sectors, warp-split (lmax 4..6)
-# The planar kernel in the organisation of emit_rot3d_ws: per mirror sector (z-parity x y'-sector, coplanar_sectors_axial),
-#   A: phi rotation of the staged d-values and the constant frame change G onto the pair axis      -> w  (all (l, p) blocks)
-#   B: m''-diagonal axial translation                                                               -> t  (in place per |m''| group)
-#   C: frame change back Gout and the accumulation with the output rotation, per OWNING part of the (l, p) blocks, into registers.
-# A + B are one instruction stream shared by the 4 warps of a block (about 30 KB at lmax 6 against 43 KB for the whole sector loop of
-# emit_coplanar4, which misses the 32 KB instruction cache); C is a quarter of the rest per warp and loops over the 4 sources of a round.
-_cop4_axial_results = {}
-
-
-def coplanar_sectors_axial_cached(lmax):
-    if lmax not in _cop4_axial_results:
-        _cop4_axial_results[lmax] = coplanar_sectors_axial(lmax)
-    return _cop4_axial_results[lmax]
-
-
-def emit_coplanar4_ws(lmaxes, path, NP=4):
-    with open(path, "w") as f:
-        f.write("// GENERATED by gen_tables.py - do not edit.\n")
-        f.write("// Coplanar translation apply for lmax 4..6, four mirror sectors, WARP-SPLIT (DESIGN.md, kernel K2c4-ws): A_* phi rotation + frame change\n")
-        f.write("// of all (l, p) blocks -> w (scratch [slot * AS]);  B_* axial translation, in place per |m''| group;  C_*_P<g> frame change back and\n")
-        f.write(f"// accumulation of the (l, p) blocks OWNED by part g (one of {NP}) into that part's register accumulators;  unmix_*_P<g> its share of u.\n")
-        f.write("// xs: [own slots | partner slots] d-values of the sector.\n#pragma once\n\n")
-        f.write("#ifndef TM_PIN\n#define TM_PIN(v)\n#endif\n\n")
-        for lmax in lmaxes:
-            md = modes(lmax)
-            idx = {t_: i for i, t_ in enumerate(md)}
-            half_l = len(md) // 2
-            cost = [0, 0]
-            nslmax = nmax = 0
-            secs = coplanar_sectors_axial_cached(lmax)
-            for z in range(4):
-                slots, slots2, G, entries, Gout = secs[z]
-                n = len(slots)
-                nmax = max(nmax, n)
-                hpar = z // 2
-                sa, sb, ss = [], [], []
-                for (l, am, p, kind) in slots:
-                    sa.append(idx[(l, am, p)]); sb.append(idx[(l, -am, p)]); ss.append({"0": 0, "+": 1, "-": -1}[kind])
-                for (l, am, p, kind) in slots:
-                    sa.append(idx[(l, am, p)]); sb.append(idx[(l, -am, p)]); ss.append({"0": 0, "+": -1, "-": 1}[kind])
-                tagS = f"L{lmax}_Z{z}"
-                f.write(f"// lmax={lmax} sector z={z}: slots (l,|m|,p,kind) {slots}\n")
-                f.write(f"__device__ __constant__ int tm_c4w_sa_{tagS}[{2 * n}] = {{{', '.join(map(str, sa))}}};\n")
-                f.write(f"__device__ __constant__ int tm_c4w_sb_{tagS}[{2 * n}] = {{{', '.join(map(str, sb))}}};\n")
-                f.write(f"__device__ __constant__ int tm_c4w_ss_{tagS}[{2 * n}] = {{{', '.join(map(str, ss))}}};\n")
-                f.write(f"#define TM_C4W_N_{tagS} {n}\n")
-                covered = set()
-                for (l, am, p, kind) in slots:
-                    covered.add(idx[(l, am, p)]); covered.add(idx[(l, -am, p)])
-                # (l, p) blocks: b1 = pair-frame slots, b3 = pair-axis-frame slots (index space of w / t)
-                blocks = []
-                for p in (0, 1):
-                    for l in range(1, lmax + 1):
-                        b1 = [k for k, s_ in enumerate(slots) if s_[0] == l and s_[2] == p]
-                        b3 = [k for k, s_ in enumerate(slots2) if s_[0] == l and s_[2] == p]
-                        if b1 or b3:
-                            assert len(b1) == len(b3)
-                            for i in b3:
-                                assert all(c in b1 for (c, _) in G[i]), "frame change must be block diagonal in (l, p)"
-                            for r in b1:
-                                assert all(j in b3 for (j, _) in Gout[r])
-                            blocks.append((b1, b3))
-                bcost = [sum(len(Gout[r]) for r in b1) + 3 * len(b1) for (b1, b3) in blocks]
-                part_blocks = [[] for _ in range(NP)]
-                load = [0] * NP
-                for bi in sorted(range(len(blocks)), key=lambda i: -bcost[i]):
-                    g = min(range(NP), key=lambda q: load[q])
-                    part_blocks[g].append(bi)
-                    load[g] += bcost[bi]
-                for g in range(NP):
-                    part_blocks[g].sort()
-                cnt = [0, 0]
-                phases = "    R cm[%d], sm[%d];\n    cm[0] = R(1); sm[0] = R(0); cm[1] = cph; sm[1] = sph;\n" % (lmax + 1, lmax + 1)
-                for m in range(2, lmax + 1):
-                    phases += f"    cm[{m}] = cm[{m - 1}] * cph - sm[{m - 1}] * sph; sm[{m}] = sm[{m - 1}] * cph + cm[{m - 1}] * sph;\n"
-                nph = (4 * max(0, lmax - 1), 6 * max(0, lmax - 1))
-                # ---- A
-                f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
-                        f"tm_c4w_A_{tagS}(const R* __restrict__ xs, R cph, R sph, R* wr, R* wi) {{\n" + phases)
-                cnt[0] += nph[0]; cnt[1] += nph[1]
-                for (b1, b3) in blocks:
-                    f.write("  {\n")
-                    for k in b1:
-                        l, am, p, kind = slots[k]
-                        if kind == "0":
-                            f.write(f"    const R xr{k} = xs[{2 * k}], xi{k} = xs[{2 * k + 1}];\n")
-                        else:
-                            f.write(f"    const R xr{k} = xs[{2 * k}] * cm[{am}] - xs[{2 * (n + k) + 1}] * sm[{am}], "
-                                    f"xi{k} = xs[{2 * k + 1}] * cm[{am}] + xs[{2 * (n + k)}] * sm[{am}];\n")
-                            cnt[0] += 4; cnt[1] += 6
-                    _r3_lin(f, "w", "x", G, b3, cnt)
-                    for i in b3:
-                        f.write(f"    wr[{i} * AS] = wr{i}; wi[{i} * AS] = wi{i};\n")
-                    f.write("  }\n")
-                f.write("}\n")
-                # ---- B
-                f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
-                        f"tm_c4w_B_{tagS}(R* hr, R* hi, const R* wr, const R* wi, R* tr, R* ti) {{\n")
-                for mm in sorted(set(s_[1] for s_ in slots2)):
-                    grp = [k for k, s_ in enumerate(slots2) if s_[1] == mm]
-                    f.write("  {\n")
-                    for j in grp:
-                        f.write(f"    const R wr{j} = wr[{j} * AS], wi{j} = wi[{j} * AS];\n")
-                    known = {}
-                    for i in grp:
-                        first = True
-                        newq, seen = set(), set(known)          # scheduling pins: keep each radial sum next to its first use
-                        for j in grp:
-                            lst = entries.get((i, j))
-                            if lst:
-                                s0 = 1 if lst[0][1] > 0 else -1
-                                key = tuple((q, mp.nstr(s0 * v, 30)) for (q, v) in lst)
-                                if key not in seen:
-                                    seen.add(key)
-                                    newq.update(q for (q, _) in lst)
-                        if newq:
-                            f.write("    " + " ".join(f"TM_PIN(hr[{q}]); TM_PIN(hi[{q}]);" for q in sorted(newq)) + "\n")
-                        for j in grp:
-                            lst = entries.get((i, j))
-                            if not lst:
-                                continue
-                            s0 = 1 if lst[0][1] > 0 else -1
-                            key = tuple((q, mp.nstr(s0 * v, 30)) for (q, v) in lst)
-                            if key not in known:
-                                e = len(known)
-                                known[key] = e
-                                for part, hh in (("r", "hr"), ("i", "hi")):
-                                    expr = None
-                                    for t, (q, v) in enumerate(lst):
-                                        vv = s0 * v
-                                        if t == 0 and abs(vv) == 1:
-                                            expr = f"{'-' if vv < 0 else ''}{hh}[{q}]"
-                                        elif t == 0:
-                                            expr = f"R({lit(vv)}) * {hh}[{q}]"
-                                            cnt[0] += 1; cnt[1] += 1
-                                        else:
-                                            expr = f"fma(R({lit(vv)}), {hh}[{q}], {expr})"
-                                            cnt[0] += 1; cnt[1] += 2
-                                    f.write(f"    const R e{part}{e} = {expr};\n")
-                            e = known[key]
-                            sg = "" if s0 > 0 else "-"
-                            ng = "-" if s0 > 0 else ""
-                            if first:
-                                f.write(f"    R tr{i} = {sg}er{e} * wr{j}; tr{i} = fma({ng}ei{e}, wi{j}, tr{i}); "
-                                        f"R ti{i} = {sg}er{e} * wi{j}; ti{i} = fma({sg}ei{e}, wr{j}, ti{i});\n")
-                                cnt[0] += 4; cnt[1] += 6
-                                first = False
-                            else:
-                                f.write(f"    tr{i} = fma({sg}er{e}, wr{j}, tr{i}); tr{i} = fma({ng}ei{e}, wi{j}, tr{i}); "
-                                        f"ti{i} = fma({sg}er{e}, wi{j}, ti{i}); ti{i} = fma({sg}ei{e}, wr{j}, ti{i});\n")
-                                cnt[0] += 4; cnt[1] += 8
-                        assert not first
-                        f.write(f"    tr[{i} * AS] = tr{i}; ti[{i} * AS] = ti{i};\n")
-                    f.write("  }\n")
-                f.write("}\n")
-                # ---- C and unmix per owning part
-                for g in range(NP):
-                    myslots = [k for bi in part_blocks[g] for k in blocks[bi][0]]
-                    loc = {k: i for i, k in enumerate(myslots)}
-                    nslmax = max(nslmax, len(myslots))
-                    tag = f"{tagS}_P{g}"
-                    f.write(f"#define TM_C4W_NSL_{tag} {len(myslots)}\n")
-                    f.write("template <typename R, int AS>\n__device__ __forceinline__ void "
-                            f"tm_c4w_C_{tag}(R cph, R sph, const R* tr, const R* ti, R* ar, R* ai, R* pr, R* pi) {{\n" + phases)
-                    cnt[0] += nph[0]; cnt[1] += nph[1]
-                    for bi in part_blocks[g]:
-                        b1, b3 = blocks[bi]
-                        f.write("  {\n")
-                        for j in b3:
-                            f.write(f"    const R tr{j} = tr[{j} * AS], ti{j} = ti[{j} * AS];\n")
-                        _r3_lin(f, "u", "t", Gout, b1, cnt)
-                        for k in b1:
-                            l, am, p, kind = slots[k]
-                            li = loc[k]
-                            if kind == "0":
-                                f.write(f"    ar[{li}] += ur{k}; ai[{li}] += ui{k};\n")
-                                cnt[0] += 2; cnt[1] += 2
-                            else:
-                                f.write(f"    ar[{li}] = fma(ur{k}, cm[{am}], ar[{li}]); ai[{li}] = fma(ui{k}, cm[{am}], ai[{li}]);\n")
-                                f.write(f"    pr[{li}] = fma(ui{k}, sm[{am}], pr[{li}]); pi[{li}] = fma(-ur{k}, sm[{am}], pi[{li}]);\n")
-                                cnt[0] += 4; cnt[1] += 8
-                        f.write("  }\n")
-                    f.write("}\n")
-                    f.write("template <typename R, typename C>\n__device__ __forceinline__ void "
-                            f"tm_c4w_unmix_{tag}(const R* ar, const R* ai, const R* pr, const R* pi, C* out) {{\n")
-
-                    def store(i_flat, re, im):
-                        if i_flat >= half_l:
-                            f.write(f"  out[{i_flat}].re = {im}; out[{i_flat}].im = -({re});\n")
-                        else:
-                            f.write(f"  out[{i_flat}].re = {re}; out[{i_flat}].im = {im};\n")
-                    for k in myslots:
-                        l, am, p, kind = slots[k]
-                        li = loc[k]
-                        if kind == "0":
-                            store(idx[(l, 0, p)], f"ar[{li}]", f"ai[{li}]")
-                        else:
-                            plus_r, plus_i = (f"ar[{li}]", f"ai[{li}]") if kind == "+" else (f"pr[{li}]", f"pi[{li}]")
-                            minus_r, minus_i = (f"pr[{li}]", f"pi[{li}]") if kind == "+" else (f"ar[{li}]", f"ai[{li}]")
-                            store(idx[(l, am, p)], f"R(0.5) * ({plus_r} + {minus_r})", f"R(0.5) * ({plus_i} + {minus_i})")
-                            store(idx[(l, -am, p)], f"R(0.5) * ({plus_r} - {minus_r})", f"R(0.5) * ({plus_i} - {minus_i})")
-                    if g == 0:        # m = 0 modes of this z-parity that the partner y'-sector owns: this sector contributes nothing
-                        for i_flat, (l, m, p) in enumerate(md):
-                            if (l + m + p) % 2 == hpar and i_flat not in covered:
-                                f.write(f"  out[{i_flat}].re = R(0); out[{i_flat}].im = R(0);\n")
-                    f.write("}\n")
-                cost[0] += cnt[0]; cost[1] += cnt[1]
-                print(f"lmax={lmax} cop4-ws z={z}: n={n} -> {cnt[0]} FP instructions, {cnt[1]} flop", file=sys.stderr)
-            f.write(f"#define TM_C4W_NMAX_L{lmax} {nmax}\n")
-            f.write(f"#define TM_C4W_NSLMAX_L{lmax} {nslmax}\n")
-            f.write(f"#define TM_C4W_FPINST_L{lmax} {cost[0]}   // FP instructions per ordered pair (all four sectors)\n")
-            f.write(f"#define TM_C4W_FLOP_L{lmax} {cost[1]}     // flop per ordered pair (FMA = 2)\n\n")
-
-
 def main():
     os.makedirs(OUT, exist_ok=True)
     emit_tables([1, 2, 3, 4, 5, 6, 7], os.path.join(OUT, "tm_tables_gen.h"))     # 7: internal (gradient at lmax 6)
@@ -2118,7 +1903,6 @@ def main():
     emit_coplanar_f2([1, 2, 3], os.path.join(OUT, "tm_coplanar_f2_gen.cuh"))
     emit_rot3d([1, 2, 3, 4, 5, 6, 7], os.path.join(OUT, "tm_rot3d_gen.cuh"))      # 7: internal (gradient at lmax 6)
     emit_rot3d_ws([4, 5, 6], os.path.join(OUT, "tm_rot3d_ws_gen.cuh"))
-    emit_coplanar4_ws([4, 5, 6], os.path.join(OUT, "tm_coplanar4_ws_gen.cuh"))
 
 
 if __name__ == "__main__":

@@ -974,176 +974,3 @@ k_allpairs_coplanar4(const double* __restrict__ pos, const Cx<R>* __restrict__ x
   cop4_dispatch<R, LMAX, 0, TJ, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, shift, smem_raw);
 }
 #endif  // TM_SEC_COP4
-#ifdef TM_SEC_COP4W
-// ---------------------------------------------------------------------------------------------------
-// Four-sector coplanar kernel, WARP-SPLIT (lmax 4..6; gen_tables.py: emit_coplanar4_ws) - the organisation of k_allpairs_rot3d_ws on
-// the planar factorisation.  Block = 4 warps x 32 targets, lane = target, blockIdx.z = mirror sector (z-parity x y'-sector).  A round
-// handles 4 sources: warp g runs phases A + B (phi rotation, frame change onto the pair axis, axial translation) - the same code in
-// all warps - for source s + g of its lane's target into ITS scratch vector; block barrier; warp g then runs phase C (frame change
-// back, output rotation, accumulation) of the (l, p) blocks it owns for each of the 4 sources into REGISTER accumulators; barrier.
-#ifndef TM_PIN
-__device__ __forceinline__ void tm_pin(double& v) { asm volatile("" : "+d"(v)); }
-__device__ __forceinline__ void tm_pin(float& v) { asm volatile("" : "+f"(v)); }
-#define TM_PIN(v) tm_pin(v)
-#endif
-#include "generated/tm_coplanar4_ws_gen.cuh"
-
-template <typename R, int LMAX, int Z> struct C4wSec;
-template <typename R, int LMAX, int Z, int P> struct C4wPart;
-#define TM_C4W_SEC(LM, ZZ)                                                                                 \
-  template <typename R> struct C4wSec<R, LM, ZZ> {                                                         \
-    static constexpr int n = TM_C4W_N_L##LM##_Z##ZZ;                                                       \
-    template <int AS> static __device__ __forceinline__ void A(const R* xs, R cph, R sph, R* wr, R* wi) {  \
-      tm_c4w_A_L##LM##_Z##ZZ<R, AS>(xs, cph, sph, wr, wi);                                                 \
-    }                                                                                                      \
-    template <int AS> static __device__ __forceinline__ void B(R* hr, R* hi, R* wr, R* wi) {               \
-      tm_c4w_B_L##LM##_Z##ZZ<R, AS>(hr, hi, wr, wi, wr, wi);                                               \
-    }                                                                                                      \
-    static __device__ __forceinline__ void entry(int k, int& a, int& b, int& sg) {                         \
-      a = tm_c4w_sa_L##LM##_Z##ZZ[k]; b = tm_c4w_sb_L##LM##_Z##ZZ[k]; sg = tm_c4w_ss_L##LM##_Z##ZZ[k];     \
-    }                                                                                                      \
-  };
-#define TM_C4W_PART(LM, ZZ, PP)                                                                            \
-  template <typename R> struct C4wPart<R, LM, ZZ, PP> {                                                    \
-    template <int AS> static __device__ __forceinline__ void Cc(R cph, R sph, const R* tr, const R* ti, R* ar, R* ai, R* pr, R* pi) { \
-      tm_c4w_C_L##LM##_Z##ZZ##_P##PP<R, AS>(cph, sph, tr, ti, ar, ai, pr, pi);                             \
-    }                                                                                                      \
-    static __device__ __forceinline__ void unmix(const R* ar, const R* ai, const R* pr, const R* pi, Cx<R>* out) { \
-      tm_c4w_unmix_L##LM##_Z##ZZ##_P##PP<R, Cx<R>>(ar, ai, pr, pi, out);                                   \
-    }                                                                                                      \
-  };
-#define TM_C4W_ALL(LM, ZZ) TM_C4W_SEC(LM, ZZ) TM_C4W_PART(LM, ZZ, 0) TM_C4W_PART(LM, ZZ, 1) TM_C4W_PART(LM, ZZ, 2) TM_C4W_PART(LM, ZZ, 3)
-#define TM_C4W_L(LM) TM_C4W_ALL(LM, 0) TM_C4W_ALL(LM, 1) TM_C4W_ALL(LM, 2) TM_C4W_ALL(LM, 3)
-TM_C4W_L(4) TM_C4W_L(5) TM_C4W_L(6)
-#undef TM_C4W_L
-#undef TM_C4W_ALL
-#undef TM_C4W_PART
-#undef TM_C4W_SEC
-template <int LMAX> struct C4wMax;
-template <> struct C4wMax<4> { static constexpr int n = TM_C4W_NMAX_L4, nsl = TM_C4W_NSLMAX_L4; };
-template <> struct C4wMax<5> { static constexpr int n = TM_C4W_NMAX_L5, nsl = TM_C4W_NSLMAX_L5; };
-template <> struct C4wMax<6> { static constexpr int n = TM_C4W_NMAX_L6, nsl = TM_C4W_NSLMAX_L6; };
-
-template <typename R, int LMAX, int SS> struct Cop4WsSmem {
-  static constexpr int NM = C4wMax<LMAX>::n;
-  // positions | staged d-values (own + partner = 2 n slots per source) | 4 scratch vectors ([re/im][n slots][32 lanes]) | pair angles
-  // [warp][2][32] | staging tables
-  static constexpr size_t bytes = sizeof(double) * 2 * SS + sizeof(R) * (size_t)(SS * 2 * NM * 2 + 4 * 2 * NM * 32 + 4 * 2 * 32) + sizeof(int) * 3 * 2 * NM;
-};
-
-template <typename R, int LMAX, int Z, int SS>
-__device__ __forceinline__ void cop4_ws_sector(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
-                                               const TmTile tile, int n_scat, double k_over_pi, double inv_k, unsigned char* smem_raw) {
-  using S = C4wSec<R, LMAX, Z>;
-  constexpr int L = 2 * LMAX * (LMAX + 2), NQ = 2 * LMAX + 1, TJ = 32, NT = 128, NM = C4wMax<LMAX>::n, NSL = C4wMax<LMAX>::nsl;
-  constexpr int n = S::n;
-  double* s_px = reinterpret_cast<double*>(smem_raw);
-  double* s_py = s_px + SS;
-  R* s_x = reinterpret_cast<R*>(s_py + SS);          // [source][2 n] complex: own slots then partner slots
-  R* s_scr = s_x + SS * 2 * NM * 2;                  // [warp][re/im][NM][TJ]
-  R* s_ang = s_scr + 4 * 2 * NM * TJ;                // [warp][2][TJ]: cos / sin of the pair's azimuth
-  int* s_sa = reinterpret_cast<int*>(s_ang + 4 * 2 * TJ);
-  int* s_sb = s_sa + 2 * NM;
-  int* s_ss = s_sb + 2 * NM;
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const bool live = lane < tile.tgt_count;
-  const int j = tile.tgt_start + (live ? lane : tile.tgt_count - 1);
-  const double xj = pos[3 * j], yj = pos[3 * j + 1];
-  const int per = (tile.src_count + gridDim.y - 1) / gridDim.y;
-  const int c0 = tile.src_start + blockIdx.y * per;
-  const int c1 = min(tile.src_start + tile.src_count, c0 + per);
-  for (int e = tid; e < 2 * n; e += NT) {
-    int a, b, sg;
-    S::entry(e, a, b, sg);
-    s_sa[e] = a; s_sb[e] = b; s_ss[e] = sg;
-  }
-  R* wr = s_scr + (size_t)warp * 2 * NM * TJ + lane;
-  R* wi = wr + NM * TJ;
-  R ar[NSL], ai[NSL], pr[NSL], pi[NSL];
-#pragma unroll
-  for (int q = 0; q < NSL; ++q) { ar[q] = R(0); ai[q] = R(0); pr[q] = R(0); pi[q] = R(0); }
-
-  for (int s0 = c0; s0 < c1; s0 += SS) {
-    const int ns = min(SS, c1 - s0);
-    __syncthreads();
-    for (int e = tid; e < ns; e += NT) { s_px[e] = pos[3 * (s0 + e)]; s_py[e] = pos[3 * (s0 + e) + 1]; }
-    for (int e = tid; e < ns * 2 * n; e += NT) {
-      const int src = e / (2 * n), kk = e - src * 2 * n;
-      const Cx<R>* xrow = x + (size_t)(s0 + src) * L;
-      const int ia = s_sa[kk], sg = s_ss[kk];
-      Cx<R> v = xrow[ia];
-      if (sg != 0) {
-        const Cx<R> o = xrow[s_sb[kk]];
-        v = sg > 0 ? cadd(v, o) : csub(v, o);
-      }
-      if (ia >= L / 2) v = cx<R>(-v.im, v.re);         // tilde basis: multiply p = 1 modes by i
-      s_x[2 * e] = v.re;
-      s_x[2 * e + 1] = v.im;
-    }
-    __syncthreads();
-#pragma unroll 1
-    for (int s = 0; s < ns; s += 4) {
-      const int sg = s + warp;
-      if (sg < ns) {
-        const double dx = xj - s_px[sg], dy = yj - s_py[sg];
-        const double r2 = dx * dx + dy * dy;
-        const double rinv = r2 > 0.0 ? rsqrt(r2) : 0.0;                            // self pair -> h_q = 0 -> t = 0
-        const double r = r2 * rinv;
-        const R cph = r2 > 0.0 ? (R)(dx * rinv) : R(1), sph = (R)(dy * rinv);
-        R* ang = s_ang + (size_t)warp * 2 * TJ + lane;
-        ang[0] = cph; ang[TJ] = sph;
-        S::template A<TJ>(&s_x[sg * 2 * n * 2], cph, sph, wr, wi);
-        R ck, sk;
-        phase_kr<R>(k_over_pi, r, ck, sk);
-        R hr[NQ], hi[NQ];
-        hankel_up<R, NQ>((R)(rinv * inv_k), ck, sk, hr, hi);
-        S::template B<TJ>(hr, hi, wr, wi);
-      }
-      __syncthreads();
-      const int nq = min(4, ns - s);
-#pragma unroll 1
-      for (int q = 0; q < nq; ++q) {
-        const R* ang = s_ang + (size_t)q * 2 * TJ + lane;
-        const R cph = ang[0], sph = ang[TJ];
-        const R* tr = s_scr + (size_t)q * 2 * NM * TJ + lane;
-        const R* ti = tr + NM * TJ;
-        switch (warp) {
-          case 0: C4wPart<R, LMAX, Z, 0>::template Cc<TJ>(cph, sph, tr, ti, ar, ai, pr, pi); break;
-          case 1: C4wPart<R, LMAX, Z, 1>::template Cc<TJ>(cph, sph, tr, ti, ar, ai, pr, pi); break;
-          case 2: C4wPart<R, LMAX, Z, 2>::template Cc<TJ>(cph, sph, tr, ti, ar, ai, pr, pi); break;
-          default: C4wPart<R, LMAX, Z, 3>::template Cc<TJ>(cph, sph, tr, ti, ar, ai, pr, pi); break;
-        }
-      }
-      __syncthreads();
-    }
-  }
-  if (live) {
-    Cx<R>* out = u_part + ((size_t)(blockIdx.y * 2 + (Z & 1)) * n_scat + j) * L;
-    switch (warp) {
-      case 0: C4wPart<R, LMAX, Z, 0>::unmix(ar, ai, pr, pi, out); break;
-      case 1: C4wPart<R, LMAX, Z, 1>::unmix(ar, ai, pr, pi, out); break;
-      case 2: C4wPart<R, LMAX, Z, 2>::unmix(ar, ai, pr, pi, out); break;
-      default: C4wPart<R, LMAX, Z, 3>::unmix(ar, ai, pr, pi, out); break;
-    }
-  }
-}
-
-#ifndef TM_C4W_MINBLOCKS
-#define TM_C4W_MINBLOCKS 2
-#endif
-template <typename R, int LMAX, int SS>
-__global__ void __launch_bounds__(128, TM_C4W_MINBLOCKS)
-k_allpairs_coplanar4_ws(const double* __restrict__ pos, const Cx<R>* __restrict__ x, Cx<R>* __restrict__ u_part,
-                        const TmTile* __restrict__ tiles, int n_scat, double k_over_pi, double inv_k,
-                        const int* __restrict__ n_active) {
-  if (n_active != nullptr && *n_active == 0) return;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  const TmTile tile = tiles[blockIdx.x];
-  switch (blockIdx.z) {
-    case 0: cop4_ws_sector<R, LMAX, 0, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, smem_raw); break;
-    case 1: cop4_ws_sector<R, LMAX, 1, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, smem_raw); break;
-    case 2: cop4_ws_sector<R, LMAX, 2, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, smem_raw); break;
-    default: cop4_ws_sector<R, LMAX, 3, SS>(pos, x, u_part, tile, n_scat, k_over_pi, inv_k, smem_raw); break;
-  }
-}
-#endif  // TM_SEC_COP4W

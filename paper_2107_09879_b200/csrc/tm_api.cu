@@ -280,8 +280,7 @@ cudaError_t launch_allpairs(tm_ctx* c, const Cx<R>* x, const int* n_active) {
   const TmLaunch a{c->d_pos, c->d_tiles, c->n_scat, c->k / M_PI, 1.0 / c->k, n_active, c->stream, dim3(c->n_tiles, c->n_chunk), c->lmax};
   tick(c, true);
   cudaError_t e;
-  if (c->kernel == TM_KERNEL_COPLANAR && tm_cop4_ws(c->lmax)) e = tm_launch_coplanar4_ws<R>(a, x, up);
-  else if (c->kernel == TM_KERNEL_COPLANAR && c->lmax > 3)
+  if (c->kernel == TM_KERNEL_COPLANAR && c->lmax > 3)
     e = c->lmax <= 5 ? tm_launch_coplanar4_lo<R>(a, x, up, c->shift) : tm_launch_coplanar4_hi<R>(a, x, up, c->shift);
   else if (c->kernel == TM_KERNEL_COPLANAR) e = tm_launch_coplanar<R>(a, x, up, c->cop_tj, c->cop_cl, c->shift);
   else if (c->kernel == TM_KERNEL_ROT3D) {
@@ -606,7 +605,7 @@ int configure_kernel(tm_ctx* ctx) {
   int tgt_per_tile;
   const bool gen = want == TM_KERNEL_COPLANAR || want == TM_KERNEL_SYM3D || want == TM_KERNEL_ROT3D;   // generated kernels: thread = target
   switch (gen ? 0 : ctx->lmax) {
-    case 0: tgt_per_tile = want == TM_KERNEL_ROT3D ? (tm_rot3d_ws(ctx->lmax) ? 32 : tm_rot3d_tj(ctx->lmax)) : (want == TM_KERNEL_SYM3D ? TM_SYM3D_TJ : (ctx->lmax > 3 ? (tm_cop4_ws(ctx->lmax) ? 32 : tm_cop4_tj(ctx->lmax)) : ctx->cop_tj)); break;
+    case 0: tgt_per_tile = want == TM_KERNEL_ROT3D ? (tm_rot3d_ws(ctx->lmax) ? 32 : tm_rot3d_tj(ctx->lmax)) : (want == TM_KERNEL_SYM3D ? TM_SYM3D_TJ : (ctx->lmax > 3 ? tm_cop4_tj(ctx->lmax) : ctx->cop_tj)); break;
     default: tgt_per_tile = tm_general_tj(ctx->lmax); break;
   }
   std::vector<TmTile> tiles;
@@ -621,9 +620,9 @@ int configure_kernel(tm_ctx* ctx) {
   // small problems fill the 148 SMs (2 resident 128-thread blocks each at 255 registers) and large ones end
   // without a long tail; bounded by 64 chunks, >= 32 sources per chunk and 2 GB of partial sums.
   const bool cop4 = want == TM_KERNEL_COPLANAR && ctx->lmax > 3;   // four-sector coplanar kernel (lmax 4..6)
-  const long long slots = 148LL * (cop4 ? (tm_cop4_ws(ctx->lmax) ? 2 : 256 / tm_cop4_tj(ctx->lmax)) : (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj :
+  const long long slots = 148LL * (cop4 ? 256 / tm_cop4_tj(ctx->lmax) : (want == TM_KERNEL_COPLANAR ? 256 / ctx->cop_tj :
                                    (want == TM_KERNEL_SYM3D ? 2 : (want == TM_KERNEL_ROT3D ? (tm_rot3d_ws(ctx->lmax) ? 2 : (ctx->lmax <= 6 ? 2 : 1)) : 4))));
-  const int cop4_z = !cop4 ? 0 : (tm_cop4_ws(ctx->lmax) ? 4 : 4 * tm_cop4_groups(ctx->lmax));
+  const int cop4_z = !cop4 ? 0 : 4 * tm_cop4_groups(ctx->lmax);
   const long long blocks1 = (long long)ctx->n_tiles * (cop4 ? cop4_z : (gen ? 2 : 1));
   const int part_mult = (want == TM_KERNEL_SYM3D || want == TM_KERNEL_ROT3D || cop4) ? 2 : 1;   // one partial buffer per (chunk, y'-sector)
   int max_win = 1;
@@ -1642,8 +1641,7 @@ extern "C" {
 int tm_pair_cost(const tm_ctx* ctx, double* fp_instructions, double* flop) {
   if (!ctx) return TM_E_INVALID;
   double inst = 0.0, fl = 0.0;
-  if (ctx->kernel == TM_KERNEL_COPLANAR && tm_cop4_ws(ctx->lmax)) tm_cost_coplanar4_ws(ctx->lmax, &inst, &fl);
-  else if (ctx->kernel == TM_KERNEL_COPLANAR) tm_cost_coplanar(ctx->lmax, &inst, &fl);
+  if (ctx->kernel == TM_KERNEL_COPLANAR) tm_cost_coplanar(ctx->lmax, &inst, &fl);
   else if (ctx->kernel == TM_KERNEL_ROT3D && tm_rot3d_ws(ctx->lmax)) tm_cost_rot3d_ws(ctx->lmax, &inst, &fl);
   else if (ctx->kernel == TM_KERNEL_ROT3D) tm_cost_rot3d(ctx->lmax, &inst, &fl);
   else if (ctx->kernel == TM_KERNEL_SYM3D) tm_cost_sym3d(ctx->lmax, &inst, &fl);

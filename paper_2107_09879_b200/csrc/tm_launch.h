@@ -49,13 +49,6 @@ template <typename R> cudaError_t tm_launch_rot3d_7(const TmLaunch& a, const Cx<
 inline bool tm_rot3d_ws(int lmax) { return TM_R3D_WS && lmax >= 4 && lmax <= 6; }
 template <typename R> cudaError_t tm_launch_rot3d_ws(const TmLaunch& a, const Cx<R>* x, Cx<R>* up);
 void tm_cost_rot3d_ws(int lmax, double* inst, double* flop);
-// warp-split four-sector coplanar kernel (lmax 4..6): 32 targets per tile
-#ifndef TM_COP4_WS
-#define TM_COP4_WS 0                 // build switch: 1 = use it for planar layouts at lmax 4..6 instead of k_allpairs_coplanar4
-#endif
-inline bool tm_cop4_ws(int lmax) { return TM_COP4_WS && lmax >= 4 && lmax <= 6; }
-template <typename R> cudaError_t tm_launch_coplanar4_ws(const TmLaunch& a, const Cx<R>* x, Cx<R>* up);
-void tm_cost_coplanar4_ws(int lmax, double* inst, double* flop);
 template <typename R> cudaError_t tm_launch_general(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, const TmConst* cst, TmTermsDev tb);   // lmax 1..7
 
 int tm_cop4_groups(int lmax);                                  // row groups per sector (generated constant)

@@ -194,34 +194,6 @@ void tm_cost_rot3d_ws(int lmax, double* inst, double* flop) {
 }
 #endif
 
-#ifdef TM_SEC_COP4W
-template <typename R> cudaError_t tm_launch_coplanar4_ws(const TmLaunch& a, const Cx<R>* x, Cx<R>* up) {
-  dim3 grid = a.grid;
-  grid.z = 4;                                         // mirror sector: slowest grid dimension
-#define TM_LAUNCH_C4W(LM)                                                                                       \
-  {                                                                                                             \
-    constexpr int SS_ = 8;                                                                                      \
-    const size_t sm = Cop4WsSmem<R, LM, SS_>::bytes;                                                            \
-    cudaFuncSetAttribute(k_allpairs_coplanar4_ws<R, LM, SS_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); \
-    k_allpairs_coplanar4_ws<R, LM, SS_><<<grid, 128, sm, a.stream>>>(a.pos, x, up, a.tiles, a.n_scat, a.k_over_pi, a.inv_k, a.n_active); \
-  }
-  switch (a.lmax) {
-    case 4: TM_LAUNCH_C4W(4) break;
-    case 5: TM_LAUNCH_C4W(5) break;
-    default: TM_LAUNCH_C4W(6) break;
-  }
-#undef TM_LAUNCH_C4W
-  return cudaGetLastError();
-}
-template cudaError_t tm_launch_coplanar4_ws<double>(const TmLaunch&, const Cx<double>*, Cx<double>*);
-template cudaError_t tm_launch_coplanar4_ws<float>(const TmLaunch&, const Cx<float>*, Cx<float>*);
-void tm_cost_coplanar4_ws(int lmax, double* inst, double* flop) {
-  const int I[7] = {0, 0, 0, 0, TM_C4W_FPINST_L4, TM_C4W_FPINST_L5, TM_C4W_FPINST_L6};
-  const int F[7] = {0, 0, 0, 0, TM_C4W_FLOP_L4, TM_C4W_FLOP_L5, TM_C4W_FLOP_L6};
-  *inst = I[lmax]; *flop = F[lmax];
-}
-#endif
-
 #ifdef TM_SEC_GEN
 template <typename R> cudaError_t tm_launch_general(const TmLaunch& a, const Cx<R>* x, Cx<R>* up, const TmConst* cst, TmTermsDev tb) {
   const dim3 grid = a.grid;
