@@ -292,6 +292,16 @@ int tm_nullfield_dtmatrix(int lmax, int lmax_internal, double k_b, tm_c64 eps_r,
  * Returns TM_OK or TM_E_CUDA. */
 int tm_release_cached_memory(void);
 
+/* Debug aid: guard bands around every INTERNAL device buffer (a stand-in for compute-sanitizer's memcheck where that tool cannot
+ * run).  enable = 1: every device block the library allocates FROM NOW ON (contexts created afterwards, their scratch, tables,
+ * Krylov state) carries a 4 KiB margin of sentinel bytes on each side; enable = 0: new blocks are plain again (blocks already
+ * guarded stay so until freed); enable < 0: query only.  Every call synchronises the device, compares the margins of all live
+ * guarded blocks and returns the number of damaged margins found so far, including those of blocks freed in the meantime
+ * (0 = no kernel wrote outside an internal buffer); *n_blocks (may be NULL) receives how many guarded blocks have been handed
+ * out.  Costs 8 KiB per block and nothing when off (the default).  Not thread-safe against concurrent compute calls on other host
+ * threads.  Returns a count >= 0 or TM_E_CUDA. */
+long long tm_debug_guards(int enable, long long *n_blocks);
+
 int tm_num_modes(int lmax);                    /* L = 2 lmax (lmax + 2) */
 const char *tm_last_error(const tm_ctx *ctx);  /* ctx may be NULL: last error of tm_create */
 void tm_destroy(tm_ctx *ctx);

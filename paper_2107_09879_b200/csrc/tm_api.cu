@@ -6,8 +6,10 @@
 #include <complex>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <type_traits>
+#include <unordered_map>
 #include <vector>
 
 #include "tm_launch.h"
@@ -29,6 +31,32 @@ std::string g_create_error;
 // created and destroyed once per step (an optimisation loop, the end-to-end bench leg) gets the same physical memory
 // back instead of paying the driver's map / unmap on every cudaMalloc / cudaFree (measured: 1-60 ms per call, at
 // random).  tm_release_cached_memory() returns the cached memory to the driver.
+// Debug aid (tm_debug_guards; compute-sanitizer is not available everywhere): with guards ON every block handed out below
+// carries a 4 KiB margin of 0xA5 bytes on each side; the margins are compared when the block is freed and whenever
+// tm_debug_guards is asked, so a kernel that writes outside ANY internal buffer (chunk partials, Krylov basis, tables,
+// quadrature scratch, ...) is caught.  Off (the default) the allocator is exactly what it was.
+constexpr size_t GUARD_BYTES = 4096;
+struct GuardRegistry {
+  std::mutex mu;
+  bool on = false;
+  std::unordered_map<void*, size_t> live;      // user pointer -> user bytes, guarded blocks only
+  long long violations = 0, blocks = 0;
+};
+GuardRegistry& guards() { static GuardRegistry g; return g; }
+
+// Number of margins of one block that no longer hold the sentinel (0, 1 or 2); the device is idle when this runs.
+int guard_damage(void* user, size_t bytes) {
+  static std::vector<unsigned char> h(2 * GUARD_BYTES);
+  char* u = static_cast<char*>(user);
+  if (cudaMemcpy(h.data(), u - GUARD_BYTES, GUARD_BYTES, cudaMemcpyDeviceToHost) != cudaSuccess ||
+      cudaMemcpy(h.data() + GUARD_BYTES, u + bytes, GUARD_BYTES, cudaMemcpyDeviceToHost) != cudaSuccess) { cudaGetLastError(); return 2; }
+  int bad = 0;
+  for (int side = 0; side < 2; ++side)
+    for (size_t i = 0; i < GUARD_BYTES; ++i)
+      if (h[side * GUARD_BYTES + i] != 0xA5) { ++bad; break; }
+  return bad;
+}
+
 template <typename T>
 cudaError_t tm_dev_alloc(T** p, size_t bytes) {
   *p = nullptr;
@@ -44,8 +72,19 @@ cudaError_t tm_dev_alloc(T** p, size_t bytes) {
     if ((e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep)) != cudaSuccess) return e;
     pool_set[dev] = true;
   }
+  GuardRegistry& g = guards();
+  std::lock_guard<std::mutex> lock(g.mu);
+  const size_t pad = g.on ? GUARD_BYTES : 0;
   void* q = nullptr;
-  if ((e = cudaMallocAsync(&q, bytes, (cudaStream_t)0)) != cudaSuccess) return e;
+  if ((e = cudaMallocAsync(&q, bytes + 2 * pad, (cudaStream_t)0)) != cudaSuccess) return e;
+  if (pad) {
+    char* c = static_cast<char*>(q);
+    if ((e = cudaMemsetAsync(c, 0xA5, pad, (cudaStream_t)0)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(c + pad + bytes, 0xA5, pad, (cudaStream_t)0)) != cudaSuccess) return e;
+    q = c + pad;
+    g.live[q] = bytes;
+    ++g.blocks;
+  }
   *p = static_cast<T*>(q);
   return cudaStreamSynchronize((cudaStream_t)0);      // usable from any stream on return
 }
@@ -54,6 +93,14 @@ cudaError_t tm_dev_alloc(T** p, size_t bytes) {
 inline cudaError_t tm_dev_free(void* p) {
   if (!p) return cudaSuccess;
   cudaError_t e = cudaDeviceSynchronize();
+  GuardRegistry& g = guards();
+  std::lock_guard<std::mutex> lock(g.mu);
+  const auto it = g.live.find(p);
+  if (it != g.live.end()) {                          // a guarded block: check its margins, free from its true start
+    g.violations += guard_damage(p, it->second);
+    g.live.erase(it);
+    p = static_cast<char*>(p) - GUARD_BYTES;
+  }
   const cudaError_t f = cudaFreeAsync(p, (cudaStream_t)0);
   return e != cudaSuccess ? e : f;
 }
@@ -1652,6 +1699,17 @@ int tm_pair_cost(const tm_ctx* ctx, double* fp_instructions, double* flop) {
   if (fp_instructions) *fp_instructions = inst;
   if (flop) *flop = fl;
   return TM_OK;
+}
+
+long long tm_debug_guards(int enable, long long* n_blocks) {
+  if (cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); return TM_E_CUDA; }
+  GuardRegistry& g = guards();
+  std::lock_guard<std::mutex> lock(g.mu);
+  if (enable >= 0) g.on = enable != 0;
+  long long bad = g.violations;
+  for (const auto& kv : g.live) bad += guard_damage(kv.first, kv.second);
+  if (n_blocks) *n_blocks = g.blocks;
+  return bad;
 }
 
 int tm_release_cached_memory(void) {

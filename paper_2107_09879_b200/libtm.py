@@ -25,7 +25,7 @@ EXPORTS = ["tm_create", "tm_set_tmatrices", "tm_set_incident", "tm_get_incident"
            "tm_kernel_time", "tm_pair_cost", "tm_measure_fma_peak", "tm_grad_tmatrix", "tm_grad_positions", "tm_mie_tmatrix_dR", "tm_mie_tmatrix",
            "tm_nullfield_tmatrix", "tm_nullfield_dtmatrix",
            "tm_fields_static_setup", "tm_fields_static", "tm_fields_static_error",
-           "tm_release_cached_memory", "tm_num_modes", "tm_last_error", "tm_destroy"]
+           "tm_release_cached_memory", "tm_debug_guards", "tm_num_modes", "tm_last_error", "tm_destroy"]
 
 
 class c64(ctypes.Structure):
@@ -108,6 +108,8 @@ def lib():
         L.tm_fields_static.argtypes = [ci, cd, ci, vp, vp, ci, vp, ci, vp, vp]
         L.tm_fields_static_error.argtypes = []
         L.tm_fields_static_error.restype = ctypes.c_char_p
+        L.tm_debug_guards.argtypes = [ci, ctypes.POINTER(ctypes.c_longlong)]
+        L.tm_debug_guards.restype = ctypes.c_longlong
         _lib = L
     return _lib
 
@@ -207,6 +209,16 @@ def fields_static(lmax, k_b, pos, s, pts, which=TM_FIELD_E_SCA, out=None, stream
     if rc != TM_OK:
         raise TmError(rc, lib().tm_fields_static_error().decode())
     return out
+
+
+def debug_guards(enable=-1):
+    """tm_debug_guards: switch the sentinel margins of the library's internal device buffers on (1) / off (0) or query (-1);
+    returns (damaged margins found so far, guarded blocks handed out)."""
+    nb = ctypes.c_longlong()
+    bad = lib().tm_debug_guards(int(enable), ctypes.byref(nb))
+    if bad < 0:
+        raise TmError(int(bad), "tm_debug_guards failed")
+    return int(bad), int(nb.value)
 
 
 def release_cached_memory():
