@@ -629,6 +629,55 @@ def run_nullfield(args):
     print(json.dumps(out), flush=True)
 
 
+def run_ttable(args):
+    """Recorded run (NEXT-4, not the contract line): T-matrices AND dT/dR of every scatterer of the paper's 120 um lens (112 x 112
+    cylinders) from a 64-node radius table at the paper's truncation (lmax 6, full 96 x 96 T), one tm_ttable_interp
+    call on device arrays.  Algorithmic bytes = the outputs written once (2 x n_out x L^2 x 16 B) + the table read once; the
+    peak is MEASURED_PEAKS.json's HBM copy bandwidth."""
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2107_09879_b200 import libtm
+    lmax = args.lmax or 6
+    L = W.n_modes(lmax)
+    n_tab, n_out = 64, (args.scale or 112) ** 2
+    rng = np.random.default_rng(0)
+    nodes = torch.linspace(0.05, 0.25, n_tab, dtype=torch.float64, device="cuda")
+    tab = torch.randn((n_tab, L, L), dtype=torch.complex128, device="cuda")
+    radii = torch.from_numpy(rng.uniform(0.05, 0.25, n_out)).cuda()
+    T = torch.empty((n_out, L, L), dtype=torch.complex128, device="cuda")
+    dT = torch.empty_like(T)
+    st = torch.cuda.current_stream().cuda_stream
+    for _ in range(3):
+        libtm.ttable_interp(nodes, tab, radii, out=T, dout=dT, stream=st)
+    ts = []
+    for _ in range(args.steps or 20):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        libtm.ttable_interp(nodes, tab, radii, out=T, dout=dT, stream=st)
+        e1.record(); torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    ms = float(np.median(ts))
+    alg = 2 * n_out * L * L * 16 + n_tab * L * L * 16 + n_out * 8
+    peak, src = 6540.5, "fallback"
+    try:
+        peak, src = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        pass
+    out = {"mode": "ttable", "lmax": lmax, "L": L, "n_tab": n_tab, "n_out": n_out, "call_ms_median": ms, "tmatrices_per_s": n_out / ms * 1e3,
+           "roofline": {"bound": "hbm", "achieved": alg / ms * 1e-6, "peak": peak, "unit": "GB/s", "frac": alg / ms * 1e-6 / peak,
+                        "peak_source": src, "algorithmic_bytes": alg,
+                        "note": "whole call incl. the per-site weight kernel, scratch allocation and the flag read-back"}}
+    if not args.no_cpu_baseline:
+        from oracle import ttable as ott
+        pick = rng.choice(n_out, 8, replace=False)
+        t0 = time.perf_counter()
+        T_ref, dT_ref = ott.interp_table(nodes.cpu().numpy(), tab.cpu().numpy(), radii.cpu().numpy()[pick])
+        out.update(oracle_seconds_per_site=(time.perf_counter() - t0) / len(pick),
+                   max_rel_error_vs_oracle=float(np.abs(T[torch.from_numpy(pick).cuda()].cpu().numpy() - T_ref).max() / np.abs(T_ref).max()),
+                   max_rel_error_derivative=float(np.abs(dT[torch.from_numpy(pick).cuda()].cpu().numpy() - dT_ref).max() / np.abs(dT_ref).max()))
+    print(json.dumps(out), flush=True)
+
+
 def run_paper_case(args):
     """Recorded run (not the contract line): the paper's own largest single-GPU case end to end on its own kind of meta-atom
     (workloads.paper_lens: 56 x 56 silicon cylinders, lmax 6; 1-1.5 h on a V100): null-field T-matrices of the
@@ -687,7 +736,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg5")
-    ap.add_argument("--mode", default=None, choices=["hotpath", "full", "matvec", "nyquist", "gradient", "nullfield", "paper_case", "multirhs"],
+    ap.add_argument("--mode", default=None, choices=["hotpath", "full", "matvec", "nyquist", "gradient", "nullfield", "paper_case", "multirhs", "ttable"],
                     help="hotpath (default for cfg5): every row of the path with both GMRES solves bounded to --cycle-iters iterations; "
                          "full (default otherwise): solves to tolerance; matvec: operator applications only; others: recorded runs")
     ap.add_argument("--cycle-iters", type=int, default=5, help="hotpath mode: Arnoldi iterations per (forward / adjoint) solve")
@@ -744,6 +793,9 @@ def main():
     if args.mode == "nullfield":
         if rank == 0:
             run_nullfield(args)
+    elif args.mode == "ttable":
+        if rank == 0:
+            run_ttable(args)
     elif args.mode == "paper_case":
         if rank == 0:
             run_paper_case(args)

@@ -285,6 +285,22 @@ int tm_nullfield_tmatrix(int lmax, int lmax_internal, double k_b, tm_c64 eps_r, 
 int tm_nullfield_dtmatrix(int lmax, int lmax_internal, double k_b, tm_c64 eps_r, int n_shapes, int n_nodes, const double *theta, const double *r,
                           const double *dr_dtheta, const double *weight, double h, tm_c64 *dT_out, void *cuda_stream);
 
+/* T-matrix look-up table ("we are setting up a lookup table for the transition matrices and interpolating between
+ * them, this derivative can be numerically approximated using the same lookup table"; Fig. 2c).
+ * Given the T-matrices of a scatterer family at n_tab >= 4 values p_tab[0] < p_tab[1] < ... of one geometry parameter (a radius;
+ * the nodes need not be equidistant) - T_tab [n_tab][n_entry], n_entry = L (diagonal T) or L*L (full T), e.g. from
+ * tm_mie_tmatrix / tm_nullfield_tmatrix - computes on the device, for n_out parameter values p[j],
+ *     T_out[j][e]  = sum_{a=0..3} w_a(p[j])  T_tab[i0 + a][e]          (cubic Lagrange polynomial through the four nodes
+ *     dT_out[j][e] = sum_{a=0..3} w_a'(p[j]) T_tab[i0 + a][e]           i0 .. i0+3 around the interval that holds p[j])
+ * with i0 = clamp(i - 1, 0, n_tab - 4) for p_tab[i] <= p[j] < p_tab[i+1] (last interval closed on the right): reading R20 of
+ * DESIGN.md; dT_out is the exact derivative of the interpolant, so gradients are consistent with the interpolated forward model.
+ * T_out [n_out][n_entry] is what tm_set_tmatrices takes with type_of[j] = j, dT_out what tm_grad_tmatrix takes; dT_out may be NULL.
+ * Every pointer may be host or device memory (device arrays are used in place, host arrays are staged); the call returns after
+ * the work on cuda_stream has finished.  Errors: TM_E_INVALID (n_tab < 4, nodes not finite / not strictly increasing, any p[j]
+ * outside [p_tab[0], p_tab[n_tab-1]] or NaN - nothing is extrapolated; the outputs are then unspecified), TM_E_NOMEM, TM_E_CUDA. */
+int tm_ttable_interp(int n_tab, const double *p_tab, long long n_entry, const tm_c64 *T_tab, int n_out, const double *p, tm_c64 *T_out,
+                     tm_c64 *dT_out, void *cuda_stream);
+
 /* Memory (the solver state is what limits the problem size on one GPU).  All device memory of the
  * library comes from the current device's stream-ordered pool (cudaMallocAsync) with the release threshold raised, so a
  * context created and destroyed once per optimisation step re-uses the same physical memory.  This call hands the cached,

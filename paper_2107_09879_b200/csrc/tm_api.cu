@@ -20,6 +20,7 @@
 #include "tm_incident.cuh"
 #include "tm_nullfield.cuh"
 #include "tm_special.cuh"
+#include "tm_ttable.cuh"
 #include "tm_vecops.cuh"
 #include "generated/tm_tables_gen.h"
 
@@ -1803,6 +1804,69 @@ int tm_nullfield_dtmatrix(int lmax, int lmax_internal, double k_b, tm_c64 eps_r,
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return TM_E_CUDA; }
   return nullfield_run(lmax, lmax_internal > 0 ? lmax_internal : lmax, k_b, eps_r, n_shapes, n_nodes, theta, r, dr_dtheta, weight, dT_out,
                        reinterpret_cast<cudaStream_t>(cuda_stream), h);
+}
+
+int tm_ttable_interp(int n_tab, const double* p_tab, long long n_entry, const tm_c64* T_tab, int n_out, const double* p, tm_c64* T_out,
+                     tm_c64* dT_out, void* cuda_stream) {
+  if (n_tab < 4 || !p_tab || n_entry < 1 || n_entry > 0x7fffffffLL || !T_tab || n_out < 1 || !p || !T_out) return TM_E_INVALID;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return TM_E_CUDA; }
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  {   // nodes: finite and strictly increasing
+    std::vector<double> h(n_tab);
+    if (cudaMemcpy(h.data(), p_tab, n_tab * sizeof(double), is_device_ptr(p_tab) ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost) != cudaSuccess) {
+      cudaGetLastError(); return TM_E_CUDA;
+    }
+    for (int i = 0; i < n_tab; ++i)
+      if (!std::isfinite(h[i]) || (i > 0 && !(h[i] > h[i - 1]))) return TM_E_INVALID;
+  }
+  const size_t tab_elems = (size_t)n_tab * n_entry, total = (size_t)n_out * n_entry;
+  // host arrays are staged on the device, device arrays are used where they are
+  double *s_ptab = nullptr, *s_p = nullptr, *d_w = nullptr;
+  double2 *s_tab = nullptr, *s_T = nullptr, *s_dT = nullptr;
+  int *d_i0 = nullptr;                                     // [n_out] stencil starts, then the out-of-table flag
+  cudaError_t e = cudaSuccess;
+  auto release = [&]() {
+    tm_dev_free(s_ptab); tm_dev_free(s_p); tm_dev_free(d_w); tm_dev_free(s_tab); tm_dev_free(s_T); tm_dev_free(s_dT); tm_dev_free(d_i0);
+  };
+  auto nomem = [&]() { cudaGetLastError(); release(); return TM_E_NOMEM; };
+  if (tm_dev_alloc(&d_w, (size_t)ttable::TT_NW * n_out * sizeof(double)) != cudaSuccess) return nomem();
+  if (tm_dev_alloc(&d_i0, ((size_t)n_out + 1) * sizeof(int)) != cudaSuccess) return nomem();
+  const double* d_ptab = p_tab; const double* d_p = p; const double2* d_tab = reinterpret_cast<const double2*>(T_tab);
+  double2* d_T = reinterpret_cast<double2*>(T_out); double2* d_dT = reinterpret_cast<double2*>(dT_out);
+  if (!is_device_ptr(p_tab)) { if (tm_dev_alloc(&s_ptab, n_tab * sizeof(double)) != cudaSuccess) return nomem(); d_ptab = s_ptab; }
+  if (!is_device_ptr(p)) { if (tm_dev_alloc(&s_p, n_out * sizeof(double)) != cudaSuccess) return nomem(); d_p = s_p; }
+  if (!is_device_ptr(T_tab)) { if (tm_dev_alloc(&s_tab, tab_elems * sizeof(double2)) != cudaSuccess) return nomem(); d_tab = s_tab; }
+  if (!is_device_ptr(T_out)) { if (tm_dev_alloc(&s_T, total * sizeof(double2)) != cudaSuccess) return nomem(); d_T = s_T; }
+  if (dT_out && !is_device_ptr(dT_out)) { if (tm_dev_alloc(&s_dT, total * sizeof(double2)) != cudaSuccess) return nomem(); d_dT = s_dT; }
+  if (s_ptab) e = cudaMemcpyAsync(s_ptab, p_tab, n_tab * sizeof(double), cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess && s_p) e = cudaMemcpyAsync(s_p, p, n_out * sizeof(double), cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess && s_tab) e = cudaMemcpyAsync(s_tab, T_tab, tab_elems * sizeof(double2), cudaMemcpyHostToDevice, st);
+  int* d_bad = d_i0 + n_out;
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_bad, 0, sizeof(int), st);
+  if (e == cudaSuccess) {
+    ttable::k_ttable_weights<<<(n_out + 127) / 128, 128, 0, st>>>(d_ptab, n_tab, d_p, n_out, d_i0, d_w, d_bad);
+    const unsigned ne = (unsigned)n_entry;
+    if (ne > 256) {
+      const unsigned grid = (unsigned)std::min<size_t>((size_t)n_out, (size_t)148 * 8);
+      if (d_dT) ttable::k_ttable_apply_wide<true><<<grid, 256, 0, st>>>(d_tab, ne, d_i0, d_w, n_out, d_T, d_dT);
+      else ttable::k_ttable_apply_wide<false><<<grid, 256, 0, st>>>(d_tab, ne, d_i0, d_w, n_out, d_T, nullptr);
+    } else {
+      const size_t per_block = 256 / ne;
+      const unsigned grid = (unsigned)std::min<size_t>(((size_t)n_out + per_block - 1) / per_block, (size_t)148 * 8 * 4);
+      if (d_dT) ttable::k_ttable_apply_narrow<true><<<grid, 256, 0, st>>>(d_tab, ne, d_i0, d_w, n_out, d_T, d_dT);
+      else ttable::k_ttable_apply_narrow<false><<<grid, 256, 0, st>>>(d_tab, ne, d_i0, d_w, n_out, d_T, nullptr);
+    }
+    e = cudaGetLastError();
+  }
+  int bad = 0;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && s_T) e = cudaMemcpyAsync(T_out, s_T, total * sizeof(double2), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && s_dT) e = cudaMemcpyAsync(dT_out, s_dT, total * sizeof(double2), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  release();
+  if (e != cudaSuccess) { cudaGetLastError(); return TM_E_CUDA; }
+  return bad ? TM_E_INVALID : TM_OK;
 }
 
 int tm_measure_fma_peak(int precision, double* tflops, void* cuda_stream) {

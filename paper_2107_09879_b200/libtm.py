@@ -23,7 +23,7 @@ TM_KERNEL_AUTO, TM_KERNEL_GENERAL, TM_KERNEL_COPLANAR, TM_KERNEL_SYM3D, TM_KERNE
 EXPORTS = ["tm_create", "tm_set_tmatrices", "tm_set_incident", "tm_get_incident", "tm_solve", "tm_solve_adjoint",
            "tm_matvec", "tm_solve_multi", "tm_fields", "tm_workspace_bytes", "tm_set_workspace", "tm_set_kernel", "tm_get_kernel",
            "tm_kernel_time", "tm_pair_cost", "tm_measure_fma_peak", "tm_grad_tmatrix", "tm_grad_positions", "tm_mie_tmatrix_dR", "tm_mie_tmatrix",
-           "tm_nullfield_tmatrix", "tm_nullfield_dtmatrix",
+           "tm_nullfield_tmatrix", "tm_nullfield_dtmatrix", "tm_ttable_interp",
            "tm_fields_static_setup", "tm_fields_static", "tm_fields_static_error",
            "tm_release_cached_memory", "tm_debug_guards", "tm_num_modes", "tm_last_error", "tm_destroy"]
 
@@ -108,6 +108,7 @@ def lib():
         L.tm_fields_static.argtypes = [ci, cd, ci, vp, vp, ci, vp, ci, vp, vp]
         L.tm_fields_static_error.argtypes = []
         L.tm_fields_static_error.restype = ctypes.c_char_p
+        L.tm_ttable_interp.argtypes = [ci, vp, ctypes.c_longlong, vp, ci, vp, vp, vp, vp]
         L.tm_debug_guards.argtypes = [ci, ctypes.POINTER(ctypes.c_longlong)]
         L.tm_debug_guards.restype = ctypes.c_longlong
         _lib = L
@@ -178,6 +179,37 @@ def nullfield_dtmatrix(lmax, k_b, eps_r, generatrix_fn, params, h, stream=None, 
     if rc != TM_OK:
         raise TmError(rc, "tm_nullfield_dtmatrix failed")
     return out
+
+
+def ttable_interp(p_tab, T_tab, p, deriv=True, out=None, dout=None, stream=None):
+    """tm_ttable_interp: T_tab (n_tab, ...) at the nodes p_tab -> (T (n_out, ...), dT/dp (n_out, ...) or None) at the values p.
+    numpy arrays or torch CUDA tensors (outputs are made where `p` lives)."""
+    on_dev = not isinstance(p, np.ndarray)
+    if isinstance(p_tab, np.ndarray):
+        p_tab = np.ascontiguousarray(p_tab, dtype=np.float64)
+    if isinstance(T_tab, np.ndarray):
+        T_tab = np.ascontiguousarray(T_tab, dtype=np.complex128)
+    if not on_dev:
+        p = np.ascontiguousarray(p, dtype=np.float64)
+    n_tab, n_out = int(T_tab.shape[0]), int(p.shape[0])
+    shape = (n_out,) + tuple(T_tab.shape[1:])
+    n_entry = 1
+    for d in T_tab.shape[1:]:
+        n_entry *= int(d)
+
+    def make():
+        if on_dev:
+            import torch
+            return torch.empty(shape, dtype=torch.complex128, device=p.device)
+        return np.empty(shape, dtype=np.complex128)
+    out = make() if out is None else out
+    if deriv and dout is None:
+        dout = make()
+    rc = lib().tm_ttable_interp(n_tab, _ptr(p_tab), n_entry, _ptr(T_tab), n_out, _ptr(p), _ptr(out), _ptr(dout) if deriv else None,
+                                ctypes.c_void_p(stream) if stream else None)
+    if rc != TM_OK:
+        raise TmError(rc, "tm_ttable_interp failed (TM_E_INVALID: a parameter outside the table, fewer than 4 nodes, nodes not increasing)")
+    return out, (dout if deriv else None)
 
 
 def measure_fma_peak(precision=TM_FP64, stream=None):
