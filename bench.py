@@ -678,6 +678,43 @@ def run_ttable(args):
     print(json.dumps(out), flush=True)
 
 
+def run_fields(args, w):
+    """Recorded run of row a8 (not the contract line): scattered E field of ALL scatterers of the workload on a --pts x --pts
+    detector grid (default 256 x 256 = the static entry point's maximum), device arrays, CUDA events around tm_fields (k_fields_sym +
+    k_fields_reduce) and, beside it, around tm_fields_static (same kernels, its own chunk count and scratch)."""
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2107_09879_b200 import libtm
+    n_side = args.pts
+    pts = torch.from_numpy(detector_points(w, n_side)).cuda()
+    N, L = w["pos"].shape[0], W.n_modes(w["lmax"])
+    rng = np.random.default_rng(0)
+    sol = torch.from_numpy(W.complex_normal((N, L), rng)).cuda()
+    pos = torch.from_numpy(w["pos"]).cuda()
+    ctx = libtm.Solver(w["pos"], w["lmax"], w["k"])
+    out = torch.empty((pts.shape[0], 3), dtype=torch.complex128, device="cuda")
+    out_s = torch.empty_like(out)
+    st = torch.cuda.current_stream().cuda_stream
+
+    def timed(fn):
+        for _ in range(2):
+            fn()
+        ts = []
+        for _ in range(args.steps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record(); torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return float(np.median(ts))
+    ms = timed(lambda: ctx.fields(pts, sol, libtm.TM_FIELD_E_SCA, out=out))
+    rec = {"mode": "fields", "workload": w["name"], "n_scat": N, "lmax": w["lmax"], "n_pts": int(pts.shape[0]), "tm_fields_ms": ms,
+           "point_source_pairs_per_s": N * pts.shape[0] / ms * 1e3, "mode_evaluations_per_s": N * pts.shape[0] * L / ms * 1e3}
+    if pts.shape[0] <= 65536 and not args.profile:
+        ms_s = timed(lambda: libtm.fields_static(w["lmax"], w["k"], pos, sol, pts, libtm.TM_FIELD_E_SCA, out=out_s, stream=st))
+        rec.update(tm_fields_static_ms=ms_s, max_rel_diff=float((out - out_s).abs().max() / out_s.abs().max()))
+    print(json.dumps(rec), flush=True)
+    ctx.close()
+
+
 def run_paper_case(args):
     """Recorded run (not the contract line): the paper's own largest single-GPU case end to end on its own kind of meta-atom
     (workloads.paper_lens: 56 x 56 silicon cylinders, lmax 6; 1-1.5 h on a V100): null-field T-matrices of the
@@ -736,7 +773,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg5")
-    ap.add_argument("--mode", default=None, choices=["hotpath", "full", "matvec", "nyquist", "gradient", "nullfield", "paper_case", "multirhs", "ttable"],
+    ap.add_argument("--mode", default=None, choices=["hotpath", "full", "matvec", "nyquist", "gradient", "nullfield", "paper_case", "multirhs", "ttable", "fields"],
                     help="hotpath (default for cfg5): every row of the path with both GMRES solves bounded to --cycle-iters iterations; "
                          "full (default otherwise): solves to tolerance; matvec: operator applications only; others: recorded runs")
     ap.add_argument("--cycle-iters", type=int, default=5, help="hotpath mode: Arnoldi iterations per (forward / adjoint) solve")
@@ -749,6 +786,7 @@ def main():
     ap.add_argument("--lmax", type=int, default=None, help="override the VSWF truncation of a Mie config (lmax 6 = the paper's, PAPER.md:271)")
     ap.add_argument("--lmax-internal", type=int, default=0,
                     help="paper_case / nullfield modes: internal truncation of the null-field method (0 = lmax, the paper's setting)")
+    ap.add_argument("--pts", type=int, default=256, help="--mode fields: detector grid side")
     ap.add_argument("--scale", type=int, default=None, help="lattice side override (parity-size runs)")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"],
                     help="mixed: GMRES with iterative refinement (fp32 Krylov cycles, fp64 iterate and true residual)")
@@ -807,6 +845,9 @@ def main():
     elif args.mode == "multirhs":
         if rank == 0:
             run_multirhs(args, w)
+    elif args.mode == "fields":
+        if rank == 0:
+            run_fields(args, w)
     elif args.impl == "reference":
         run_reference(args, w, rank, world)
     else:

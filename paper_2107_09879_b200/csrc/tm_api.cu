@@ -1400,8 +1400,19 @@ int tm_fields(tm_ctx* ctx, int n_pts, const double* pts, const tm_c64* s, int wh
   }
   if (n_pts < 1 || !pts || !s || !out) return fail(ctx, TM_E_INVALID, "bad arguments");
   if (which != TM_FIELD_E_SCA && which != TM_FIELD_H_SCA) return fail(ctx, TM_E_INVALID, "unknown field id");
-  const int nchunk = std::max(1, std::min(64, (int)(148LL * 8 * 128 / std::max(1, n_pts))));
-  const int nch = std::min(nchunk, std::max(1, ctx->n_scat / 32));
+  // source chunks: the grid (point blocks x chunks) should fill 148 SMs x 3 resident blocks in whole waves; among the chunk
+  // counts that leave >= 32 sources per chunk take the one whose last wave is fullest (ties: fewer chunks)
+  int nch = 1;
+  {
+    const long long pb = (n_pts + 127) / 128, slots = 148LL * 3;
+    const int max_ch = std::max(1, std::min(64, ctx->n_scat / 32));
+    double best = -1.0;
+    for (int c = 1; c <= max_ch; ++c) {
+      const double waves = (double)(pb * c) / (double)slots;
+      const double eff = waves / std::ceil(waves);
+      if (eff > best + 0.02) { best = eff; nch = c; }
+    }
+  }
   double* d_pts = nullptr; double2 *d_part = nullptr, *d_out = nullptr;
   const size_t nout = (size_t)n_pts * 3;
   cudaError_t e = scratch_get(ctx, 1, nout * sizeof(double), reinterpret_cast<void**>(&d_pts));
@@ -1412,7 +1423,7 @@ int tm_fields(tm_ctx* ctx, int n_pts, const double* pts, const tm_c64* s, int wh
   if (e == cudaSuccess) {
     dim3 grid((n_pts + 127) / 128, nch);
     const int swap = which == TM_FIELD_H_SCA ? 1 : 0;
-#define TM_FIELDS(LM) k_fields<LM><<<grid, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->n_scat, ctx->d_io, d_pts, n_pts, ctx->k, swap, d_part)
+#define TM_FIELDS(LM) k_fields_sym<LM><<<grid, 128, 0, ctx->stream>>>(ctx->d_pos, ctx->n_scat, ctx->d_io, d_pts, n_pts, ctx->k, 1.0 / ctx->k, swap, d_part)
     switch (ctx->lmax) {
       case 1: TM_FIELDS(1); break;
       case 2: TM_FIELDS(2); break;

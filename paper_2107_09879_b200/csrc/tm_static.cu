@@ -1,7 +1,7 @@
 // tm_fields_static: scattered-field evaluation (Eqs. I13/I24) through an entry point that ALLOCATES NOTHING -
 // for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).
 //
-// Same kernels as tm_fields (k_fields: thread per detector point x source chunk; k_fields_reduce: fixed-order sum of the
+// Same kernels as tm_fields (k_fields_sym: thread per detector point x source chunk; k_fields_reduce: fixed-order sum of the
 // chunk partials), but the per-chunk partial sums - the scratch tm_fields takes from the context's cached device buffers - live
 // in a file-scope static device array of a fixed, modest size.  Every GPU that loads libtm.so holds that array until the
 // process exits.  Consequences, all part of the contract (include/tm.h):
@@ -9,7 +9,7 @@
 //   * every call on a device shares the one array: calls that overlap on the GPU (two streams, two host threads, two
 //     captured graphs replayed concurrently) race on it - serialise them;
 //   * the array keeps the last call's contents.  Nothing has to start at zero here: every partial sum the reduction reads is
-//     written by k_fields of the SAME call first (all n_chunk x n_pts x 3 entries, also for an empty source chunk).
+//     written by k_fields_sym of the SAME call first (all n_chunk x n_pts x 3 entries, also for an empty source chunk).
 // In host code the array's name is a host-side stand-in, not a device address: the address the kernels get comes from
 // cudaGetSymbolAddress, taken once per device with that device current (static_scratch() below).
 #include "../../include/tm.h"
@@ -19,6 +19,7 @@
 #include <algorithm>
 #include <mutex>
 #include <string>
+#include <type_traits>
 
 #include "tm_common.cuh"
 #include "tm_special.cuh"
@@ -106,7 +107,7 @@ int tm_fields_static(int lmax, double k_b, int n_scat, const double* pos_dev, co
   const dim3 grid((n_pts + 127) / 128, nch);
   const int swap = which == TM_FIELD_H_SCA ? 1 : 0;
   const double2* s2 = reinterpret_cast<const double2*>(s_dev);
-#define TM_FIELDS_S(LM) k_fields<LM><<<grid, 128, 0, st>>>(pos_dev, n_scat, s2, pts_dev, n_pts, k_b, swap, scratch)
+#define TM_FIELDS_S(LM) k_fields_sym<LM><<<grid, 128, 0, st>>>(pos_dev, n_scat, s2, pts_dev, n_pts, k_b, 1.0 / k_b, swap, scratch)
   switch (lmax) {
     case 1: TM_FIELDS_S(1); break;
     case 2: TM_FIELDS_S(2); break;
