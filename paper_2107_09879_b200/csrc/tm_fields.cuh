@@ -21,8 +21,8 @@
 //    i.e. real trigonometric factors, half the complex products of the m loop;
 //  * the radial functions do not depend on m: the five m-sums of an l (radial, theta / phi of p = 1, theta / phi of p = 0) are
 //    formed first and multiplied by h_l, [x h_l]'/x, l(l+1) h_l / x once per l;
-//  * every loop over modes has a compile-time trip count and is unrolled (static_for below): U_l^m, the trigonometric and radial
-//    tables live in registers, the normalisation constants are immediates; divisions by loop constants are multiplications by
+//  * every loop over modes has a compile-time trip count and is unrolled (static_for below): the normalised N_lm U_l^m (recurrence
+//    with the constants folded), the trigonometric and radial tables live in registers, the constants are immediates; divisions by loop constants are multiplications by
 //    constexpr reciprocals, 1/r and 1/rho come from rsqrt;
 //  * 16 sources per round are staged in shared memory (positions + combined coefficients) and read back as broadcasts.
 // Staged coefficients of a source, L complex numbers: for l = 1..LMAX at offset 2 (l^2 - 1):
@@ -121,17 +121,17 @@ k_fields_sym(const double* __restrict__ pos, int n_scat, const double2* __restri
       hr[q + 2] = fma((2 * q + 1) * t, hr[q + 1], -hr[q]);
       hi[q + 2] = fma((2 * q + 1) * t, hi[q + 1], -hi[q]);
     });
-    double U[LMAX + 1][LMAX + 2];                    // U_l^m, m <= l; U_l^{l+1} = 0
+    double V[LMAX + 1][LMAX + 1];                    // normalised N_lm U_l^m, m <= l, by the recurrence of U_l^m with the constants folded
     static_for<0, LMAX + 1>([&](auto M) {
       constexpr int m = decltype(M)::value;
       constexpr double df = fsym::dfact(m);
-      U[m][m] = df;
-      U[m][m + 1] = 0.0;
-      if constexpr (m + 1 <= LMAX) U[m + 1][m] = ((2 * m + 1) * df) * ct;
+      V[m][m] = fsym::norm_lm(m, m) * df;
+      if constexpr (m + 1 <= LMAX) V[m + 1][m] = (fsym::norm_lm(m + 1, m) * (2 * m + 1) * df) * ct;
       static_for<m + 2, LMAX + 1>([&](auto Lq) {
         constexpr int l = decltype(Lq)::value;
-        constexpr double inv = 1.0 / (l - m);
-        U[l][m] = fma(((2 * l - 1) * inv) * ct, U[l - 1][m], -((l + m - 1) * inv) * U[l - 2][m]);
+        constexpr double a = (2 * l - 1) * fsym::norm_lm(l, m) / ((l - m) * fsym::norm_lm(l - 1, m));
+        constexpr double b = (l + m - 1) * fsym::norm_lm(l, m) / ((l - m) * fsym::norm_lm(l - 2, m));
+        V[l][m] = fma(a * ct, V[l - 1][m], -b * V[l - 2][m]);
       });
     });
     double sp_[LMAX + 2];                            // st^k
@@ -149,9 +149,14 @@ k_fields_sym(const double* __restrict__ pos, int n_scat, const double2* __restri
     static_for<1, LMAX + 1>([&](auto Lq) {
       constexpr int l = decltype(Lq)::value;
       const double2* sl = si + 2 * (l * l - 1);
+      // Pbar_{l,m} = s^m V_l^m;  m pibar = m s^{m-1} V_l^m;  taubar_{l,m} = x (m pibar) - kappa_{l,m} Pbar_{l,m+1},
+      // kappa_{l,m} = N_{l,m} / N_{l,m+1} = sqrt((l - m)(l + m + 1))  (Pbar_{l,l+1} = 0)
+      double Pb[l + 2];
+      static_for<0, l + 1>([&](auto M) { constexpr int m = decltype(M)::value; Pb[m] = m == 0 ? V[l][0] : sp_[m] * V[l][m]; });
+      Pb[l + 1] = 0.0;
       // m = 0: pibar term absent
-      constexpr double N0 = fsym::norm_lm(l, 0);
-      const double P0 = N0 * U[l][0], T0 = -(N0 * sp_[1]) * U[l][1];
+      constexpr double K0 = fsym::norm_lm(l, 0) / fsym::norm_lm(l, 1);
+      const double P0 = Pb[0], T0 = -K0 * Pb[1];
       const double2 a0 = sl[0], a1 = sl[1];
       double Fr_r = P0 * a1.x, Fr_i = P0 * a1.y;     // sum_m Pbar S1
       double Ft1_r = T0 * a1.x, Ft1_i = T0 * a1.y;   // sum_m taubar S1
@@ -159,23 +164,25 @@ k_fields_sym(const double* __restrict__ pos, int n_scat, const double2* __restri
       double Fp1_r = 0, Fp1_i = 0, Ft0_r = 0, Ft0_i = 0;   // sum_m m pibar D1, sum_m m pibar V0
       static_for<1, l + 1>([&](auto M) {
         constexpr int m = decltype(M)::value;
-        constexpr double N = fsym::norm_lm(l, m);
-        const double A = N * U[l][m];
-        const double P = sp_[m] * A;
-        const double MPI = (m * sp_[m - 1]) * A;
-        const double TAU = fma(ct, MPI, -(N * sp_[m + 1]) * U[l][m + 1]);
+        const double P = Pb[m];
+        const double MPI = (m * sp_[m - 1]) * V[l][m];
+        double TAU = ct * MPI;
+        if constexpr (m < l) {
+          constexpr double K = fsym::norm_lm(l, m) / fsym::norm_lm(l, m + 1);
+          TAU = fma(-K, Pb[m + 1], TAU);
+        }
         const double2 c0p = sl[2 + 4 * (m - 1)], c0m = sl[3 + 4 * (m - 1)];
         const double2 c1p = sl[4 + 4 * (m - 1)], c1m = sl[5 + 4 * (m - 1)];
         const double c = cm[m], s_ = sm[m];
-        const double U0r = fma(c0p.x, c, -c0m.y * s_), U0i = fma(c0p.y, c, c0m.x * s_);     // c0+ cos + i c0- sin
-        const double V0r = fma(c0m.x, c, -c0p.y * s_), V0i = fma(c0m.y, c, c0p.x * s_);     // c0- cos + i c0+ sin
+        // S1 = c1+ cos + i c1- sin feeds two sums; U0 = c0+ cos + i c0- sin, V0 = c0- cos + i c0+ sin, D1 = c1- cos + i c1+ sin feed one
+        // each: their real factors are applied to cos / sin first
         const double S1r = fma(c1p.x, c, -c1m.y * s_), S1i = fma(c1p.y, c, c1m.x * s_);
-        const double D1r = fma(c1m.x, c, -c1p.y * s_), D1i = fma(c1m.y, c, c1p.x * s_);
         Fr_r = fma(P, S1r, Fr_r);       Fr_i = fma(P, S1i, Fr_i);
         Ft1_r = fma(TAU, S1r, Ft1_r);   Ft1_i = fma(TAU, S1i, Ft1_i);
-        Fp1_r = fma(MPI, D1r, Fp1_r);   Fp1_i = fma(MPI, D1i, Fp1_i);
-        Ft0_r = fma(MPI, V0r, Ft0_r);   Ft0_i = fma(MPI, V0i, Ft0_i);
-        Fp0_r = fma(TAU, U0r, Fp0_r);   Fp0_i = fma(TAU, U0i, Fp0_i);
+        const double Tc = TAU * c, Ts = TAU * s_, Mc = MPI * c, Ms = MPI * s_;
+        Fp0_r = fma(Tc, c0p.x, fma(-Ts, c0m.y, Fp0_r));   Fp0_i = fma(Tc, c0p.y, fma(Ts, c0m.x, Fp0_i));
+        Ft0_r = fma(Mc, c0m.x, fma(-Ms, c0p.y, Ft0_r));   Ft0_i = fma(Mc, c0m.y, fma(Ms, c0p.x, Ft0_i));
+        Fp1_r = fma(Mc, c1m.x, fma(-Ms, c1p.y, Fp1_r));   Fp1_i = fma(Mc, c1m.y, fma(Ms, c1p.x, Fp1_i));
       });
       const double zr = hr[l + 1], zi = hi[l + 1];                               // h_l
       const double dr = fma(-(l * t), zr, hr[l]), di = fma(-(l * t), zi, hi[l]); // [x h_l]'/x
