@@ -178,6 +178,9 @@ struct tm_ctx {
   } cyc[2];
   bool graphs_ok = true;          // cleared when a capture fails (direct launches from then on)
   bool capturing = false;
+  // side branch of the captured cycle: the Givens update of step j runs beside the all-pairs product of step j + 1
+  cudaStream_t side = nullptr;
+  cudaEvent_t fork_ev = nullptr, join_ev = nullptr;
 
   // timing of the all-pairs kernel
   bool time_kernels = false;
@@ -418,18 +421,44 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
   bool all_ok = false;
   // cooperative single-launch Arnoldi step: only when every chunk's block can be resident at once
   bool coop = false;
+  int vcap = 0;                      // basis vectors whose chunk a block of k_arnoldi_fused keeps in shared memory
 #ifndef TM_NO_COOP                 // build switch (-DTM_NO_COOP): multi-kernel Arnoldi step everywhere, for A/B measurements
   if (ctx->max_chunks_per_win <= 512) {
-    int per_sm = 0, dev = 0, n_sm = 0, can = 0;
+    int per_sm = 0, dev = 0, n_sm = 0, can = 0, smem_sm = 0, smem_blk = 0;
     const void* fn = ctx->ept == 1 ? (const void*)k_arnoldi_fused<R, 1> : (const void*)k_arnoldi_fused<R, 4>;
     const size_t sm_max = (size_t)(2 * m + 2) * sizeof(double2) + (size_t)(m + 1) * sizeof(double);
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&can, cudaDevAttrCooperativeLaunch, dev);
-    if (ctx->ept == 1) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_arnoldi_fused<R, 1>, TM_VT, sm_max);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_arnoldi_fused<R, 4>, TM_VT, sm_max);
-    coop = can && (long long)per_sm * n_sm >= nc;
-    (void)fn;
+    cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+    cudaDeviceGetAttribute(&smem_blk, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    auto occ = [&](size_t dyn) {
+      per_sm = 0;
+      if (ctx->ept == 1) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_arnoldi_fused<R, 1>, TM_VT, dyn);
+      else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_arnoldi_fused<R, 4>, TM_VT, dyn);
+      return can && (long long)per_sm * n_sm >= nc;
+    };
+    coop = occ(sm_max);
+#ifndef TM_NO_VCACHE               // build switch (-DTM_NO_VCACHE): every pass over the basis reads global memory
+    if (coop) {                      // shared memory left per block when all nc blocks are co-resident -> cached vectors
+      cudaFuncAttributes fa;
+      cudaFuncGetAttributes(&fa, fn);
+      const int bps = (nc + n_sm - 1) / n_sm;
+      const long long per_blk = std::min<long long>(smem_blk, smem_sm / bps - 1024) - (long long)fa.sharedSizeBytes;
+      const long long vbytes = (long long)ctx->ept * TM_VT * (long long)sizeof(Cx<R>);
+      const long long room = per_blk - (long long)((sm_max + 15) & ~(size_t)15);
+      vcap = room > 0 ? (int)std::min<long long>(m + 1, room / vbytes) : 0;
+      if (vcap < 4) vcap = 0;
+      if (vcap > 0) {
+        const size_t dyn = ((sm_max + 15) & ~(size_t)15) + (size_t)vcap * vbytes;
+        if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn) != cudaSuccess || !occ(dyn)) {
+          cudaGetLastError();
+          vcap = 0;
+          coop = occ(sm_max);
+        }
+      }
+    }
+#endif
   }
 #endif
   const Cx<RX>* resid_vec = B;                        // first cycle: x0 = 0 so r = b
@@ -510,10 +539,27 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
         const int* wcp = ctx->d_win_chunk_ptr; TmGmresDev Sc = S;
         TmFuseT<R> ft{fuse_t ? (transpose == 1 ? 2 : 1) : 0, Vj, reinterpret_cast<const Cx<R>*>(ctx->d_upart), ctx->n_part, n,
                       Tptr<R>(ctx), ctx->d_type_of, ctx->d_const->perm_neg_m, ctx->L, ZV};
-        void* args[] = {&Vc, &nn, &jj, &Wc, &chk, &ncc, &prt, &npt, &wcp, &Sc, &nww, &tl, &ft};
+        int vc = std::min(vcap, j + 1), voff = (int)((std::max(sm_a, sm_g) + 15) & ~(size_t)15);
+        // Inside a captured cycle the Givens update (a long scalar recurrence run by ONE warp, ~5 us at the end of the step)
+        // leaves the critical path: it becomes a node of its own on a side branch that only the NEXT Arnoldi step (and the
+        // end of the cycle) waits for, so it runs beside the next all-pairs product.  That product may then read a stale
+        // `n_active`; a window that has just converged costs one more product whose result nobody uses.  Same arithmetic.
+        const bool side_givens = ctx->capturing && ctx->side != nullptr;
+        int dg = side_givens ? 0 : 1;
+        if (side_givens && j > j0) TM_CUDA(cudaStreamWaitEvent(st, ctx->join_ev, 0));
+        void* args[] = {&Vc, &nn, &jj, &Wc, &chk, &ncc, &prt, &npt, &wcp, &Sc, &nww, &tl, &ft, &vc, &voff, &dg};
         const void* fn = ctx->ept == 1 ? (const void*)k_arnoldi_fused<R, 1> : (const void*)k_arnoldi_fused<R, 4>;
-        TM_CUDA(cudaLaunchCooperativeKernel(fn, dim3(nc), dim3(TM_VT), args, std::max(sm_a, sm_g), st));
+        const size_t sm_v = (size_t)voff + (size_t)vc * ctx->ept * TM_VT * sizeof(Cx<R>);
+        TM_CUDA(cudaLaunchCooperativeKernel(fn, dim3(nc), dim3(TM_VT), args, sm_v, st));
         ctx->total_launches += 1;
+        if (side_givens) {
+          TM_CUDA(cudaEventRecord(ctx->fork_ev, st));
+          TM_CUDA(cudaStreamWaitEvent(ctx->side, ctx->fork_ev, 0));
+          k_gmres_givens<<<nw, 32, sm_g, ctx->side>>>(S, nw, j, o.tol, ctx->gm.normpart, ctx->d_win_chunk_ptr);
+          TM_CUDA(cudaEventRecord(ctx->join_ev, ctx->side));
+          if (j == j1 - 1) TM_CUDA(cudaStreamWaitEvent(st, ctx->join_ev, 0));
+          ctx->total_launches += 1;
+        }
       } else {
         TM_DOTS(S.h1);
         TM_AXPY(S.h1, nullptr);
@@ -542,6 +588,16 @@ int gmres_solve(tm_ctx* ctx, int transpose, const tm_solve_opts& o, tm_solve_inf
         if (G.exec) { cudaGraphExecDestroy(G.exec); G.exec = nullptr; }
         const long long l0 = ctx->total_launches, a0 = ctx->allpairs_launches;
         cudaGraph_t graph = nullptr;
+#ifndef TM_NO_SIDE_GIVENS           // build switch (-DTM_NO_SIDE_GIVENS): Givens update inside the Arnoldi kernel in captured cycles too
+        if (!ctx->side) {
+          if (cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking) != cudaSuccess ||
+              cudaEventCreateWithFlags(&ctx->fork_ev, cudaEventDisableTiming) != cudaSuccess ||
+              cudaEventCreateWithFlags(&ctx->join_ev, cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();
+            if (ctx->side) { cudaStreamDestroy(ctx->side); ctx->side = nullptr; }
+          }
+        }
+#endif
         if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
           ctx->capturing = true;
           const int rc_cap = enqueue(0, m);
@@ -783,6 +839,9 @@ void tm_destroy(tm_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
   for (auto& g : c->cyc) if (g.exec) cudaGraphExecDestroy(g.exec);
+  if (c->side) cudaStreamDestroy(c->side);
+  if (c->fork_ev) cudaEventDestroy(c->fork_ev);
+  if (c->join_ev) cudaEventDestroy(c->join_ev);
   if (c->grad_aux) tm_destroy(c->grad_aux);
   if (c->multi_aux) tm_destroy(c->multi_aux);
   tm_dev_free(c->d_grad_tab);
@@ -1890,3 +1949,12 @@ int tm_measure_fma_peak(int precision, double* tflops, void* cuda_stream) {
 }
 
 }  // extern "C"
+
+#ifdef TM_ARN_STAMPS
+extern "C" int tm_debug_arn_stamps(unsigned long long* out32) {
+  return cudaMemcpyFromSymbol(out32, g_arn_stamps, 32 * sizeof(unsigned long long)) == cudaSuccess ? 0 : -1;
+}
+extern "C" int tm_debug_fine_stamps(unsigned long long* out64) {
+  return cudaMemcpyFromSymbol(out64, g_fine, 64 * sizeof(unsigned long long)) == cudaSuccess ? 0 : -1;
+}
+#endif

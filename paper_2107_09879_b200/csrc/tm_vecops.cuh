@@ -9,7 +9,14 @@
 // A chunk holds EPT * TM_VT complex elements (EPT = elements per thread: 4 for large problems, 1 for small ones so
 // that a 30 720-element vector still spreads over 120 blocks; chosen once per context).
 
-struct TmChunk { int win; int start; int count; };   // element range [start, start+count) of window win
+struct TmChunk { int win; int start; int count; };
+#ifdef TM_ARN_STAMPS                // debug build: fine time stamps (clock64) of thread 0 of block 0 inside the vector phases
+__device__ unsigned long long g_fine[64];
+__device__ int g_fine_base;
+#define TM_FSTAMP(k) do { if (blockIdx.x == 0 && threadIdx.x == 0) g_fine[g_fine_base + (k)] = clock64(); } while (0)
+#else
+#define TM_FSTAMP(k) do { } while (0)
+#endif   // element range [start, start+count) of window win
 
 // ------------------------------------------------------------------------------------------------ conversions
 template <typename R>
@@ -92,25 +99,69 @@ k_tapply(int mode, int L, int n_scat, int n_chunk, const Cx<R>* __restrict__ x, 
 // grid = (n_chunks, G): block (c, g) handles the basis vectors i = g, g + G, ...; inside the block the chunk of w is
 // staged in shared memory and every WARP takes whole vectors (lanes stride over the chunk, one shuffle reduction per
 // vector instead of one per vector and warp).
-template <typename R, int EPT>
+// VC (k_arnoldi_fused only): 0 = basis vectors from global memory; 1 = from global memory, and the chunk of every vector
+// i < vcap is left in the block's shared-memory cache s_V[i][EPT * TM_VT]; 2 = vectors i < vcap from that cache.
+// With a short chunk (EPT = 1) a warp has TWO vectors in flight (16 independent loads per lane): the pass is bound
+// by the L2 latency, not by bandwidth.  Every sum keeps its order, so the results do not depend on VC or the pairing.
+template <typename R, int EPT, int VC = 0>
 __device__ __forceinline__ void dots_body(const Cx<R>* __restrict__ V, size_t stride, int nvec, const Cx<R>* __restrict__ w,
                                           const TmChunk ch, int cidx, int n_chunks, double2* __restrict__ part, int gy, int ngy,
-                                          Cx<R>* s_w) {
+                                          Cx<R>* s_w, Cx<R>* s_V = nullptr, int vcap = 0) {
+  constexpr int CH = EPT * TM_VT, NK = CH / 32;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  TM_FSTAMP(0);
 #pragma unroll
   for (int k = 0; k < EPT; ++k) {
     const int e = threadIdx.x + k * TM_VT;
     s_w[e] = e < ch.count ? w[(size_t)ch.start + e] : cx<R>(R(0), R(0));
   }
   __syncthreads();
-  for (int i = gy + warp * ngy; i < nvec; i += ngy * (TM_VT / 32)) {
-    const Cx<R>* v = V + (size_t)i * stride + ch.start;
+  TM_FSTAMP(1);
+  auto fetch = [&](int iv, int e) -> Cx<R> {
+    if (VC == 2 && iv < vcap) return s_V[(size_t)iv * CH + e];
+    const Cx<R> a = V[(size_t)iv * stride + ch.start + e];
+    if (VC == 1 && iv < vcap) s_V[(size_t)iv * CH + e] = a;
+    return a;
+  };
+  const int step = ngy * (TM_VT / 32);
+  int i = gy + warp * ngy;
+  if constexpr (NK <= 8) {
+    for (; i + step < nvec; i += 2 * step) {
+      Cx<R> a0[NK], a1[NK];
+#pragma unroll
+      for (int k = 0; k < NK; ++k) {
+        const int e = lane + 32 * k;
+        if (e < ch.count) { a0[k] = fetch(i, e); a1[k] = fetch(i + step, e); }
+      }
+      double sr = 0.0, si = 0.0, tr = 0.0, ti = 0.0;
+#pragma unroll
+      for (int k = 0; k < NK; ++k) {
+        const int e = lane + 32 * k;
+        if (e < ch.count) {
+          const Cx<R> b = s_w[e];
+          { const Cx<R> a = a0[k];
+            sr += (double)a.re * (double)b.re + (double)a.im * (double)b.im;
+            si += (double)a.re * (double)b.im - (double)a.im * (double)b.re; }
+          { const Cx<R> a = a1[k];
+            tr += (double)a.re * (double)b.re + (double)a.im * (double)b.im;
+            ti += (double)a.re * (double)b.im - (double)a.im * (double)b.re; }
+        }
+      }
+      sr = warp_sum(sr); si = warp_sum(si); tr = warp_sum(tr); ti = warp_sum(ti);
+      if (lane == 0) {
+        part[(size_t)i * n_chunks + cidx] = make_double2(sr, si);
+        part[(size_t)(i + step) * n_chunks + cidx] = make_double2(tr, ti);
+      }
+    }
+  }
+  TM_FSTAMP(2);
+  for (; i < nvec; i += step) {
     double sr = 0.0, si = 0.0;
 #pragma unroll
-    for (int k = 0; k < EPT * TM_VT / 32; ++k) {
+    for (int k = 0; k < NK; ++k) {
       const int e = lane + 32 * k;
       if (e < ch.count) {
-        const Cx<R> a = v[e], b = s_w[e];
+        const Cx<R> a = fetch(i, e), b = s_w[e];
         sr += (double)a.re * (double)b.re + (double)a.im * (double)b.im;
         si += (double)a.re * (double)b.im - (double)a.im * (double)b.re;
       }
@@ -118,6 +169,7 @@ __device__ __forceinline__ void dots_body(const Cx<R>* __restrict__ V, size_t st
     sr = warp_sum(sr); si = warp_sum(si);
     if (lane == 0) part[(size_t)i * n_chunks + cidx] = make_double2(sr, si);
   }
+  TM_FSTAMP(3);
 }
 
 template <typename R, int EPT>
@@ -157,11 +209,14 @@ __global__ void k_reduce_h(const double2* __restrict__ part, int n_chunks, const
 // Basis vectors must hold finite numbers (the workspace is zeroed at the start of a solve): a zero coefficient
 // multiplies whatever is there.
 // (R: precision of the basis vectors, RW: precision of the updated vector - they differ in mixed-precision solves)
-template <typename R, int EPT, typename RW = R>
+// (VC = 2: the chunks of the basis vectors i < vcap come from the shared-memory cache s_V, see dots_body)
+template <typename R, int EPT, typename RW = R, int VC = 0>
 __device__ __forceinline__ void axpy_body(const Cx<R>* __restrict__ V, size_t stride, int nvec, double2* __restrict__ coef, int ldc,
                                           double sign, Cx<RW>* __restrict__ w, const TmChunk ch, int cidx,
                                           double* __restrict__ normpart, const double2* __restrict__ part, int n_chunks,
-                                          const int* __restrict__ win_chunk_ptr, double2* s_c, double* s_n) {
+                                          const int* __restrict__ win_chunk_ptr, double2* s_c, double* s_n,
+                                          const Cx<R>* s_V = nullptr, int vcap = 0) {
+  TM_FSTAMP(0);
   if (part != nullptr) {
     const int c0 = win_chunk_ptr[ch.win], c1 = win_chunk_ptr[ch.win + 1];
     // 4 lanes per vector, each sums a contiguous quarter of the chunk list; lanes combined in fixed order
@@ -172,8 +227,14 @@ __device__ __forceinline__ void axpy_body(const Cx<R>* __restrict__ V, size_t st
         const int len = (c1 - c0 + 3) / 4;
         const int lo = c0 + q * len, hi = min(c1, lo + len);
         const double2* p = part + (size_t)i * n_chunks;
-#pragma unroll 4
-        for (int c = lo; c < hi; ++c) { sr += p[c].x; si += p[c].y; }
+        // 16 loads in flight, then the additions in list order (the pass is latency-bound: L2 round trips, not bytes)
+        for (int c = lo; c < hi; c += 16) {
+          double2 t[16];
+#pragma unroll
+          for (int u = 0; u < 16; ++u) if (c + u < hi) t[u] = p[c + u];
+#pragma unroll
+          for (int u = 0; u < 16; ++u) if (c + u < hi) { sr += t[u].x; si += t[u].y; }
+        }
       }
       sr += __shfl_xor_sync(0xffffffffu, sr, 1); si += __shfl_xor_sync(0xffffffffu, si, 1);
       sr += __shfl_xor_sync(0xffffffffu, sr, 2); si += __shfl_xor_sync(0xffffffffu, si, 2);
@@ -188,7 +249,9 @@ __device__ __forceinline__ void axpy_body(const Cx<R>* __restrict__ V, size_t st
       s_c[i] = make_double2(sign * c.x, sign * c.y);
     }
   }
+  TM_FSTAMP(1);
   __syncthreads();
+  TM_FSTAMP(2);
   double nrm = 0.0;
 #pragma unroll
   for (int k = 0; k < EPT; ++k) {
@@ -196,8 +259,19 @@ __device__ __forceinline__ void axpy_body(const Cx<R>* __restrict__ V, size_t st
     if (e < ch.count) {
       const size_t g = (size_t)ch.start + e;
       double ar = (double)w[g].re, ai = (double)w[g].im;
+      int i = 0;
+      if (VC == 2) {
+        const int nc_ = min(nvec, vcap);
 #pragma unroll 8
-      for (int i = 0; i < nvec; ++i) {
+        for (; i < nc_; ++i) {
+          const double2 c = s_c[i];
+          const Cx<R> v = s_V[(size_t)i * (EPT * TM_VT) + e];
+          ar += c.x * (double)v.re - c.y * (double)v.im;
+          ai += c.x * (double)v.im + c.y * (double)v.re;
+        }
+      }
+#pragma unroll (EPT == 1 ? 16 : 8)
+      for (; i < nvec; ++i) {
         const double2 c = s_c[i];
         const Cx<R> v = V[(size_t)i * stride + g];
         ar += c.x * (double)v.re - c.y * (double)v.im;
@@ -207,6 +281,7 @@ __device__ __forceinline__ void axpy_body(const Cx<R>* __restrict__ V, size_t st
       nrm += ar * ar + ai * ai;
     }
   }
+  TM_FSTAMP(3);
   if (normpart != nullptr) {
     nrm = warp_sum(nrm);
     if ((threadIdx.x & 31) == 0) s_n[threadIdx.x >> 5] = nrm;
