@@ -107,6 +107,9 @@ TM_COP_SPEC(1, 0) TM_COP_SPEC(1, 1) TM_COP_SPEC(2, 0) TM_COP_SPEC(2, 1) TM_COP_S
 // Thread t handles target tile.tgt_start + t.  Sources of the tile's window are split into n_chunk contiguous
 // chunks (blockIdx.y) so that small problems still fill 148 SMs; each chunk is streamed through shared memory
 // SS sources at a time (positions + this half's d-values in the tilde basis x~ = i^p x).
+#ifndef TM_COP_PIPE
+#define TM_COP_PIPE 1            // 1: the head of the pair set-up (rsqrt, phase of k r) is computed one source ahead
+#endif
 #ifndef TM_COP_MINBLOCKS
 #define TM_COP_MINBLOCKS 1       // resident blocks per SM the register allocation is asked to allow (experiments: 3)
 #endif
@@ -169,6 +172,39 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
       s_x[2 * e + 1] = v.im;
     }
     __syncthreads();
+#if TM_COP_PIPE
+    // Software pipeline over the sources of a stage: the serial head of a pair's set-up (rsqrt, then the phase of k r -
+    // two long dependent chains with no parallelism of their own) is computed ONE SOURCE AHEAD, so that it interleaves
+    // with the previous source's apply code instead of standing alone at the top of the loop body.
+    double n_dx, n_dy, n_rinv; R n_ck, n_sk;
+    auto head = [&](int s) {
+      n_dx = xj - s_px[s]; n_dy = yj - s_py[s];                // d = x_dest - x_source (reading R3)
+      const double r2 = n_dx * n_dx + n_dy * n_dy;
+      n_rinv = (r2 > 0.0 && !(shift.on && s0 + s == j)) ? rsqrt(r2) : 0.0;   // self pair -> h_q = 0 -> nothing
+      phase_kr<R>(k_over_pi, r2 * n_rinv, n_ck, n_sk);
+    };
+    head(0);
+#pragma unroll 1
+    for (int s = 0; s < ns; ++s) {
+      const double dx = n_dx, dy = n_dy, rinv = n_rinv;
+      const R ck = n_ck, sk = n_sk;
+      head(min(s + 1, ns - 1));
+      R cm[LMAX + 1], sm[LMAX + 1];
+      cm[0] = R(1); sm[0] = R(0);
+      cm[1] = (R)(dx * rinv); sm[1] = (R)(dy * rinv);
+      if (rinv == 0.0 && dx == 0.0 && dy == 0.0) cm[1] = R(1);
+#pragma unroll
+      for (int m = 2; m <= LMAX; ++m) {
+        cm[m] = cm[m - 1] * cm[1] - sm[m - 1] * sm[1];
+        sm[m] = sm[m - 1] * cm[1] + cm[m - 1] * sm[1];
+      }
+      R hr[NQ], hi[NQ];
+      hankel_up<R, NQ>((R)(rinv * inv_k), ck, sk, hr, hi);
+      const R* xs = &s_x[s * NH * 2];
+      if (half == 0) CopPair<R, LMAX, 0>::run(xs, cm, sm, hr, hi, acc);
+      else           CopPair<R, LMAX, 1>::run(xs, cm, sm, hr, hi, acc);
+    }
+#else
 #pragma unroll 1
     for (int s = 0; s < ns; ++s) {
       const double dx = xj - s_px[s], dy = yj - s_py[s];        // d = x_dest - x_source (reading R3)
@@ -192,6 +228,7 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
       if (half == 0) CopPair<R, LMAX, 0>::run(xs, cm, sm, hr, hi, acc);
       else           CopPair<R, LMAX, 1>::run(xs, cm, sm, hr, hi, acc);
     }
+#endif
   }
 
   // this chunk's partial sums of this half, back in the standard basis:
