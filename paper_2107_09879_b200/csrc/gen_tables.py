@@ -489,8 +489,11 @@ def coplanar_sectors_axial(lmax):
 COPLANAR_AXIAL = True      # False: direct pair-frame operator (sum over (row, col, q) terms), the round's first version
 
 
-def emit_axial_core(f, fac, sync_tag=None):
+def emit_axial_core(f, fac, sync_tag=None, hooks=False):
     """Straight-line code  u' = Gout (sum_q h_q Z''_q) G x'  for one half; x' in xr{k}/xi{k}, result in ur{k}/ui{k}.
+    hooks: emit `hk.template at<K>();` after the frame change (K = 0) and after every row of the axial translation (K = 1 ..):
+    places where the calling kernel may put independent work of its own (k_allpairs_coplanar: the set-up of the NEXT pair) into
+    the middle of this straight-line code; a no-op functor leaves the code as it was.
     sync_tag: emit TM_PHASE_SYNC(tag, k) after the frame change (k = 0) and after every |m''| block of the axial translation
     (k = 1, 2, ...): block-wide barriers that keep the warps of a block inside one phase of the straight-line code, so that
     the phase - not the whole loop body - has to fit the 32 KB instruction cache (lmax >= 5; a no-op elsewhere).
@@ -520,6 +523,8 @@ def emit_axial_core(f, fac, sync_tag=None):
     # axial translation, one |m''| block after the other; identical radial sums are formed once
     if sync_tag is not None:
         f.write(f"  TM_PHASE_SYNC({sync_tag}, 0);\n")
+    if hooks:
+        f.write("  hk.template at<0>();\n")
     f.write("  // axial translation along z'': diagonal in m''\n")
     known = {}
     by_row = {}
@@ -567,6 +572,8 @@ def emit_axial_core(f, fac, sync_tag=None):
                 inst += 4
                 flop += 8
         assert not first, "every F'' slot receives something"
+        if hooks:
+            f.write(f"  hk.template at<{i + 1}>();\n")
     # u' = Gout u''
     if sync_tag is not None:
         f.write(f"  TM_PHASE_SYNC({sync_tag}, {n_sync});\n")
@@ -599,7 +606,10 @@ def emit_coplanar(lmaxes, path):
         f.write("// the pair's y'-mirror symmetry (DESIGN.md, kernel K2c).  Basis of a half (\"slots\"): for every (l, |m|, p):\n")
         f.write("// d^0 = x~_{l,0,p};  d^+- = x~_{l,m,p} +- x~_{l,-m,p}  (x~ = i^p x), staged by the kernel with the tables below.\n")
         f.write("// xs: interleaved (re,im) d-values of this half; cm/sm: cos/sin(m phi); hr/hi: Re/Im h_q^(1)(kr);\n")
-        f.write("// ar/ai: accumulators A^0, A^+- = u~_{l,m,p} +- u~_{l,-m,p} of this half (unmixed once at the end).\n#pragma once\n\n")
+        f.write("// ar/ai: accumulators A^0, A^+- = u~_{l,m,p} +- u~_{l,-m,p} of this half (unmixed once at the end).\n")
+        f.write("// tm_cop_pair_*_hk: the same code with hook points hk.at<K>() (after the frame change: K = 0; after row K - 1 of the axial\n")
+        f.write("// translation: K = 1 ..) where the caller may place independent work; TmCopNoHook leaves the code as it is.\n#pragma once\n\n")
+        f.write("struct TmCopNoHook { template <int K> __device__ __forceinline__ void at() const {} };\n\n")
         for lmax in lmaxes:
             md = modes(lmax)
             idx = {t: i for i, t in enumerate(md)}
@@ -612,8 +622,8 @@ def emit_coplanar(lmaxes, path):
                 nq = 2 * lmax + 1
                 nterm = nrowq = 0
                 f.write(f"// lmax={lmax} half={h}: slots (l,|m|,p,kind) {[(l, am, p, k) for (l, am, p, k) in slots]}\n")
-                f.write("template <typename R>\n__device__ __forceinline__ void "
-                        f"tm_cop_pair_L{lmax}_H{h}(const R* __restrict__ xs, const R* cm, const R* sm, const R* hr, const R* hi, R* ar, R* ai) {{\n")
+                f.write("template <typename R, typename HK>\n__device__ __forceinline__ void "
+                        f"tm_cop_pair_L{lmax}_H{h}_hk(const R* __restrict__ xs, const R* cm, const R* sm, const R* hr, const R* hi, R* ar, R* ai, const HK& hk) {{\n")
                 # input phase rotation in the +- basis
                 k = 0
                 n_pairs = n_zero = 0
@@ -634,7 +644,7 @@ def emit_coplanar(lmaxes, path):
 
                 core = None
                 if COPLANAR_AXIAL:
-                    core = emit_axial_core(f, axial[h])
+                    core = emit_axial_core(f, axial[h], hooks=True)
 
                 def row_code(r):
                     nonlocal nterm, nrowq
@@ -678,6 +688,9 @@ def emit_coplanar(lmaxes, path):
                         k += 2
                     f.write("  }\n")
                 f.write("}\n")
+                f.write("template <typename R>\n__device__ __forceinline__ void "
+                        f"tm_cop_pair_L{lmax}_H{h}(const R* __restrict__ xs, const R* cm, const R* sm, const R* hr, const R* hi, R* ar, R* ai) {{\n"
+                        f"  tm_cop_pair_L{lmax}_H{h}_hk<R, TmCopNoHook>(xs, cm, sm, hr, hi, ar, ai, TmCopNoHook());\n}}\n")
                 # executed FP work per pair-half (generated code only; geometry/Hankel not counted):
                 #   first term of a (row,q): 2 MUL, other terms 2 FMA; per (row,q): 4 FMA (first q of a row: 2 MUL + 2 FMA);
                 #   input rotation per +- pair: 4 MUL + 4 FMA; output per pair: 8 FMA; m = 0 rows: 2 ADD

@@ -76,6 +76,11 @@ template <typename R, int LMAX, int H> struct CopPair;
                                                const double* hr, const double* hi, CopAcc<double, NH>& A) { \
       tm_cop_pair_L##LM##_H##HH<double>(xs, cm, sm, hr, hi, A.ar, A.ai);                                 \
     }                                                                                                    \
+    template <typename HK>                                                                               \
+    static __device__ __forceinline__ void run_hk(const double* xs, const double* cm, const double* sm,  \
+                                                  const double* hr, const double* hi, CopAcc<double, NH>& A, const HK& hk) { \
+      tm_cop_pair_L##LM##_H##HH##_hk<double, HK>(xs, cm, sm, hr, hi, A.ar, A.ai, hk);                    \
+    }                                                                                                    \
     static __device__ __forceinline__ void unmix(const CopAcc<double, NH>& A, Cx<double>* out) {         \
       tm_cop_unmix_L##LM##_H##HH<double, Cx<double>>(A.ar, A.ai, out);                                   \
     }                                                                                                    \
@@ -87,6 +92,12 @@ template <typename R, int LMAX, int H> struct CopPair;
     static constexpr int NH = TM_COP_NH_L##LM;                                                           \
     static __device__ __forceinline__ void run(const float* xs, const float* cm, const float* sm,        \
                                                const float* hr, const float* hi, CopAcc<float, NH>& A) { \
+      tm_cop_pair_f2_L##LM##_H##HH(reinterpret_cast<const float2*>(xs), cm, sm, hr, hi, A.a);            \
+    }                                                                                                    \
+    template <typename HK>                                                                               \
+    static __device__ __forceinline__ void run_hk(const float* xs, const float* cm, const float* sm,     \
+                                                  const float* hr, const float* hi, CopAcc<float, NH>& A, const HK& hk) { \
+      hk.template at<0>(); hk.template at<HK::B>();                /* packed-fp32 code has no hook points */ \
       tm_cop_pair_f2_L##LM##_H##HH(reinterpret_cast<const float2*>(xs), cm, sm, hr, hi, A.a);            \
     }                                                                                                    \
     static __device__ __forceinline__ void unmix(const CopAcc<float, NH>& A, Cx<float>* out) {           \
@@ -110,6 +121,26 @@ TM_COP_SPEC(1, 0) TM_COP_SPEC(1, 1) TM_COP_SPEC(2, 0) TM_COP_SPEC(2, 1) TM_COP_S
 #ifndef TM_COP_PIPE
 #define TM_COP_PIPE 1            // 1: the head of the pair set-up (rsqrt, phase of k r) is computed one source ahead
 #endif
+#ifndef TM_COP_HOOK_NUM
+#define TM_COP_HOOK_NUM 1        // the phase of the next pair is computed at hook point NH * NUM / DEN + 1 (row of the axial translation)
+#define TM_COP_HOOK_DEN 2
+#endif
+// Set-up head of the NEXT pair, run from the hook points of the generated apply code (mutable: the hooks take it by const reference).
+template <typename R, int B_> struct CopHead {
+  static constexpr int B = B_;
+  const double* px; const double* py; double xj, yj, k_over_pi; int self;   // self: stage index of the pair to annihilate (shifted targets), or -1
+  mutable int sn;                                                             // stage index of the next source
+  mutable double dx, dy, r2, rinv; mutable R ck, sk;
+  template <int K> __device__ __forceinline__ void at() const {
+    if constexpr (K == 0) {
+      dx = xj - px[sn]; dy = yj - py[sn];                      // d = x_dest - x_source (reading R3)
+      r2 = dx * dx + dy * dy;
+      rinv = (r2 > 0.0 && sn != self) ? rsqrt(r2) : 0.0;       // self pair -> h_q = 0 -> nothing
+    } else if constexpr (K == B) {
+      phase_kr<R>(k_over_pi, r2 * rinv, ck, sk);
+    }
+  }
+};
 #ifndef TM_COP_MINBLOCKS
 #define TM_COP_MINBLOCKS 1       // resident blocks per SM the register allocation is asked to allow (experiments: 3)
 #endif
@@ -176,19 +207,16 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
     // Software pipeline over the sources of a stage: the serial head of a pair's set-up (rsqrt, then the phase of k r -
     // two long dependent chains with no parallelism of their own) is computed ONE SOURCE AHEAD, so that it interleaves
     // with the previous source's apply code instead of standing alone at the top of the loop body.
-    double n_dx, n_dy, n_rinv; R n_ck, n_sk;
-    auto head = [&](int s) {
-      n_dx = xj - s_px[s]; n_dy = yj - s_py[s];                // d = x_dest - x_source (reading R3)
-      const double r2 = n_dx * n_dx + n_dy * n_dy;
-      n_rinv = (r2 > 0.0 && !(shift.on && s0 + s == j)) ? rsqrt(r2) : 0.0;   // self pair -> h_q = 0 -> nothing
-      phase_kr<R>(k_over_pi, r2 * n_rinv, n_ck, n_sk);
-    };
-    head(0);
+    // With the hook points of the generated code (tm_cop_pair_*_hk) the two chains sit INSIDE the previous source's apply
+    // code: the rsqrt after its frame change (hook 0), the phase after row TM_COP_HOOK_B - 1 of its axial translation.
+    using Head = CopHead<R, NH * TM_COP_HOOK_NUM / TM_COP_HOOK_DEN + 1>;
+    Head hd{s_px, s_py, xj, yj, k_over_pi, shift.on ? j - s0 : -1, 0, 0.0, 0.0, 0.0, 0.0, R(0), R(0)};
+    hd.template at<0>(); hd.template at<Head::B>();
 #pragma unroll 1
     for (int s = 0; s < ns; ++s) {
-      const double dx = n_dx, dy = n_dy, rinv = n_rinv;
-      const R ck = n_ck, sk = n_sk;
-      head(min(s + 1, ns - 1));
+      const double dx = hd.dx, dy = hd.dy, rinv = hd.rinv;
+      const R ck = hd.ck, sk = hd.sk;
+      hd.sn = min(s + 1, ns - 1);
       R cm[LMAX + 1], sm[LMAX + 1];
       cm[0] = R(1); sm[0] = R(0);
       cm[1] = (R)(dx * rinv); sm[1] = (R)(dy * rinv);
@@ -201,8 +229,8 @@ k_allpairs_coplanar(const double* __restrict__ pos, const Cx<R>* __restrict__ x,
       R hr[NQ], hi[NQ];
       hankel_up<R, NQ>((R)(rinv * inv_k), ck, sk, hr, hi);
       const R* xs = &s_x[s * NH * 2];
-      if (half == 0) CopPair<R, LMAX, 0>::run(xs, cm, sm, hr, hi, acc);
-      else           CopPair<R, LMAX, 1>::run(xs, cm, sm, hr, hi, acc);
+      if (half == 0) CopPair<R, LMAX, 0>::run_hk(xs, cm, sm, hr, hi, acc, hd);
+      else           CopPair<R, LMAX, 1>::run_hk(xs, cm, sm, hr, hi, acc, hd);
     }
 #else
 #pragma unroll 1
